@@ -1,0 +1,215 @@
+"""ctypes wrapper around oracle/smcx_oracle.cpp -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference leg may
+import this package.  It imports nothing from paper_2509_20949_b200.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+import threading
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "smcx_oracle.cpp")
+_LIB = os.path.join(_HERE, "libsmcx_oracle.so")
+_lock = threading.Lock()
+_lib = None
+
+BCC, FCC = 0, 1
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 the oracle into oracle/libsmcx_oracle.so (rebuilt when the source is newer)."""
+    with _lock:
+        stale = (not os.path.exists(_LIB)) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC)
+        if force or stale:
+            tmp = _LIB + f".tmp{os.getpid()}"
+            subprocess.check_call(
+                ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC])
+            os.replace(tmp, _LIB)
+    return _LIB
+
+
+def _load():
+    global _lib
+    if _lib is not None:
+        return _lib
+    lib = C.CDLL(build())
+    u32p, i32p, i64p = C.POINTER(C.c_uint32), C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+    u8p, f64p = C.POINTER(C.c_uint8), C.POINTER(C.c_double)
+    sig = {
+        "oracle_philox4x32_10": (None, [u32p, u32p, u32p]),
+        "oracle_shell": (C.c_int, [C.c_int, C.c_int, i32p, C.c_int]),
+        "oracle_create": (C.c_void_p, [C.c_int, i32p, C.c_int, C.c_int, i32p, C.c_int, u32p, C.c_int,
+                                       C.c_uint64]),
+        "oracle_destroy": (None, [C.c_void_p]),
+        "oracle_n_sites": (C.c_int64, [C.c_void_p]),
+        "oracle_init_species": (None, [C.c_void_p]),
+        "oracle_init_permutation": (C.c_uint64, [C.c_void_p, C.c_uint64]),
+        "oracle_set_species": (C.c_int, [C.c_void_p, u8p]),
+        "oracle_get_species": (None, [C.c_void_p, u8p]),
+        "oracle_set_temperature": (None, [C.c_void_p, u32p, C.c_int]),
+        "oracle_energy": (C.c_int64, [C.c_void_p]),
+        "oracle_running_energy": (C.c_int64, [C.c_void_p]),
+        "oracle_neighbour": (C.c_int64, [C.c_void_p, C.c_int64, C.c_int, C.c_int]),
+        "oracle_delta_e": (C.c_int64, [C.c_void_p, C.c_int64, C.c_int]),
+        "oracle_lc_valid": (C.c_int, [C.c_void_p]),
+        "oracle_sweep_lc": (C.c_int, [C.c_void_p, C.c_int64, C.c_int, C.c_uint32]),
+        "oracle_sweep_seq": (None, [C.c_void_p, C.c_int64]),
+        "oracle_shift": (None, [C.c_void_p, C.c_uint32, i32p]),
+        "oracle_stats": (None, [C.c_void_p, i64p, i64p, i64p]),
+        "oracle_trace": (C.c_int64, [C.c_void_p, C.c_int64, C.c_int64, i64p]),
+        "oracle_count_visits": (None, [C.c_void_p, C.c_int]),
+        "oracle_get_visits": (None, [C.c_void_p, u32p]),
+        "oracle_pair_counts": (None, [C.c_void_p, i64p]),
+        "oracle_sro": (None, [C.c_void_p, f64p, i64p]),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype = res
+        fn.argtypes = args
+    _lib = lib
+    return lib
+
+
+def _ptr(a: np.ndarray, ctype):
+    return a.ctypes.data_as(C.POINTER(ctype))
+
+
+def philox4x32_10(ctr, key):
+    lib = _load()
+    c = np.asarray(ctr, dtype=np.uint32).copy()
+    k = np.asarray(key, dtype=np.uint32).copy()
+    out = np.zeros(4, dtype=np.uint32)
+    lib.oracle_philox4x32_10(_ptr(c, C.c_uint32), _ptr(k, C.c_uint32), _ptr(out, C.c_uint32))
+    return tuple(int(v) for v in out)
+
+
+def shell(lattice: int, s: int) -> np.ndarray:
+    """Offsets (dx,dy,dz) of neighbour shell s in half-lattice units, in the oracle's order."""
+    lib = _load()
+    buf = np.zeros((512, 3), dtype=np.int32)
+    n = lib.oracle_shell(lattice, s, _ptr(buf, C.c_int32), 512)
+    return buf[:n].copy()
+
+
+class Oracle:
+    """One lattice + schedule state.  Method names follow include/smcx.h where they overlap."""
+
+    def __init__(self, lattice, dims, n_species, n_shells, epi, link_cell, accept, seed,
+                 init: bool = True):
+        lib = _load()
+        self._lib = lib
+        self.lattice, self.dims = int(lattice), tuple(int(d) for d in dims)
+        self.n_species, self.n_shells = int(n_species), int(n_shells)
+        epi = np.ascontiguousarray(epi, dtype=np.int32)
+        assert epi.shape == (n_shells, n_species, n_species)
+        accept = np.ascontiguousarray(accept, dtype=np.uint32)
+        d = np.asarray(self.dims, dtype=np.int32)
+        self._h = lib.oracle_create(self.lattice, _ptr(d, C.c_int32), self.n_species, self.n_shells,
+                                    _ptr(epi, C.c_int32), int(link_cell), _ptr(accept, C.c_uint32),
+                                    int(accept.size), C.c_uint64(int(seed)))
+        if not self._h:
+            raise ValueError("oracle_create rejected the parameters")
+        self.n_sites = int(lib.oracle_n_sites(self._h))
+        if init:
+            lib.oracle_init_species(self._h)
+
+    @classmethod
+    def from_config(cls, cfg, init: bool = True, **over):
+        kw = dict(lattice=cfg.lattice, dims=cfg.dims, n_species=cfg.n_species, n_shells=cfg.n_shells,
+                  epi=cfg.epi(), link_cell=cfg.link_cell, accept=cfg.accept_table(0), seed=cfg.seed)
+        kw.update(over)
+        return cls(init=init, **kw)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.oracle_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def init_species(self):
+        self._lib.oracle_init_species(self._h)
+
+    def init_permutation(self, i: int) -> int:
+        return int(self._lib.oracle_init_permutation(self._h, C.c_uint64(i)))
+
+    def set_species(self, s):
+        s = np.ascontiguousarray(s, dtype=np.uint8)
+        assert s.size == self.n_sites
+        if self._lib.oracle_set_species(self._h, _ptr(s, C.c_uint8)) != 0:
+            raise ValueError("species value out of range")
+
+    def species(self) -> np.ndarray:
+        out = np.empty(self.n_sites, dtype=np.uint8)
+        self._lib.oracle_get_species(self._h, _ptr(out, C.c_uint8))
+        return out
+
+    def set_temperature(self, accept):
+        accept = np.ascontiguousarray(accept, dtype=np.uint32)
+        self._lib.oracle_set_temperature(self._h, _ptr(accept, C.c_uint32), int(accept.size))
+
+    def energy(self) -> int:
+        """H recomputed from scratch (S1)."""
+        return int(self._lib.oracle_energy(self._h))
+
+    def running_energy(self) -> int:
+        return int(self._lib.oracle_running_energy(self._h))
+
+    def neighbour(self, i: int, s: int, k: int) -> int:
+        return int(self._lib.oracle_neighbour(self._h, i, s, k))
+
+    def delta_e(self, i: int, direction: int) -> int:
+        return int(self._lib.oracle_delta_e(self._h, i, direction))
+
+    def lc_valid(self) -> bool:
+        return bool(self._lib.oracle_lc_valid(self._h))
+
+    def sweep(self, n: int = 1, order_mode: int = 0, order_seed: int = 0):
+        if self._lib.oracle_sweep_lc(self._h, int(n), int(order_mode), int(order_seed)) != 0:
+            raise ValueError("lattice dimensions not divisible by 2*link_cell")
+
+    def sweep_sequential(self, n: int = 1):
+        self._lib.oracle_sweep_seq(self._h, int(n))
+
+    def shift(self, t: int):
+        o = np.zeros(3, dtype=np.int32)
+        self._lib.oracle_shift(self._h, int(t), _ptr(o, C.c_int32))
+        return tuple(int(v) for v in o)
+
+    def stats(self):
+        a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
+        self._lib.oracle_stats(self._h, C.byref(a), C.byref(b), C.byref(c))
+        return a.value, b.value, c.value
+
+    def energy_trace(self, first: int = 0, count: int | None = None) -> np.ndarray:
+        if count is None:
+            count = self.stats()[0] - first
+        out = np.zeros(count, dtype=np.int64)
+        if self._lib.oracle_trace(self._h, first, count, _ptr(out, C.c_int64)) != count:
+            raise IndexError("trace range")
+        return out
+
+    def count_visits(self, on: bool = True):
+        self._lib.oracle_count_visits(self._h, 1 if on else 0)
+
+    def visits(self) -> np.ndarray:
+        out = np.zeros(self.n_sites, dtype=np.uint32)
+        self._lib.oracle_get_visits(self._h, _ptr(out, C.c_uint32))
+        return out
+
+    def pair_counts(self) -> np.ndarray:
+        out = np.zeros((self.n_shells, self.n_species, self.n_species), dtype=np.int64)
+        self._lib.oracle_pair_counts(self._h, _ptr(out, C.c_int64))
+        return out
+
+    def sro(self):
+        """(alpha, pair_counts), both [n_shells][p'][p]; Eq. 8."""
+        a = np.zeros((self.n_shells, self.n_species, self.n_species), dtype=np.float64)
+        c = np.zeros((self.n_shells, self.n_species, self.n_species), dtype=np.int64)
+        self._lib.oracle_sro(self._h, _ptr(a, C.c_double), _ptr(c, C.c_int64))
+        return a, c

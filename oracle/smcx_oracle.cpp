@@ -1,0 +1,587 @@
+// SMC-X oracle -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// A plain, slow, single-threaded CPU implementation of the hot path of SMC-X
+// (arxiv 2509.20949): Metropolis atom-swap sweeps over a BCC/FCC alloy with an
+// effective-pair-interaction (EPI) Hamiltonian, scheduled by dynamic link cells (LC).
+// It exists only so that tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+// --impl reference leg can check and time the CUDA path against it.  Nothing under
+// paper_2509_20949_b200/ may include, link or call this file, and this file shares no
+// code with the CUDA path (its own Philox, geometry, energy, schedule, SRO).
+//
+// The method is a stochastic iteration, so the oracle follows the algorithm step by step.
+// What the paper fixes:
+//   Eq. 1-3  PAPER.md:51-63   canonical ensemble, Metropolis acceptance
+//   sweep    PAPER.md:65      exactly one trial move per lattice site
+//   move     PAPER.md:23      swap of two neighbouring lattice sites
+//   LC/LIZ   PAPER.md:71-81   dynamic link cells, every site visited once per step, O(1) trial
+//   EPI      PAPER.md:118     pairwise interactions only
+//   SRO      PAPER.md:159-163 Warren-Cowley parameter, Eq. 8
+//   indexing PAPER.md:165     lattice written nx*ny*nz*basis
+// What the paper leaves open (it defers the algorithm to its Ref. 22) is fixed by the
+// readings S0-S8 of SURVEY.md 8(c), restated in DESIGN.md "Readings"; each function below
+// names the step it follows.
+//
+// Pins (tests/test_oracle_*.py, -m "not gpu"): Philox known answers; shell coordination
+// numbers; closed-form energies (single species, B2); dE against full recomputation;
+// conservation; energy bookkeeping; order independence of same-colour cells and its failure
+// for w=1; exact Boltzmann histogram on 16 sites; B2 SRO values and sum rules.
+// Parity unpinned: the authors' own trajectories and Fig. 6 curves (their EPI values and
+// code are not available).
+#include <algorithm>
+#include <array>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <random>
+#include <vector>
+
+namespace {
+
+enum { LAT_BCC = 0, LAT_FCC = 1 };
+enum { TAG_SHIFT = 1, TAG_TRIAL = 2, TAG_INIT = 3, TAG_SEQ = 5 };
+
+// ---------------------------------------------------------------------------------------
+// Philox4x32-10, Salmon, Moraes, Dror, Shaw, SC'11 (reading Q5 / S4).
+// ---------------------------------------------------------------------------------------
+void philox4x32_10(const uint32_t ctr[4], const uint32_t key[2], uint32_t out[4]) {
+  uint32_t c0 = ctr[0], c1 = ctr[1], c2 = ctr[2], c3 = ctr[3];
+  uint32_t k0 = key[0], k1 = key[1];
+  for (int round = 0; round < 10; ++round) {
+    const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+    const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+    const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+    const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+    const uint32_t n0 = hi1 ^ c1 ^ k0;
+    const uint32_t n1 = lo1;
+    const uint32_t n2 = hi0 ^ c3 ^ k1;
+    const uint32_t n3 = lo0;
+    c0 = n0; c1 = n1; c2 = n2; c3 = n3;
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+inline uint32_t mulhi32(uint32_t a, uint32_t b) { return (uint32_t)(((uint64_t)a * b) >> 32); }
+
+struct Vec3 { int x, y, z; };
+
+struct Oracle {
+  int lattice = 0;
+  int L[3] = {0, 0, 0};      // conventional cells
+  int P[3] = {0, 0, 0};      // period in half-lattice units = 2 L
+  int B = 0;                 // sites per conventional cell
+  int n_species = 0;
+  int n_shells = 0;
+  int w = 0;                 // link-cell edge in conventional cells
+  uint64_t seed = 0;
+  int64_t N = 0;
+  std::vector<int32_t> epi;             // [s][a][b]
+  std::vector<uint32_t> accept;         // threshold table T[d]
+  std::vector<std::vector<Vec3>> shell; // offsets per shell, half-lattice units
+  std::vector<uint8_t> sigma;           // species per site
+  std::vector<uint32_t> visits;         // per-site primary-visit counter (optional)
+  bool count_visits = false;
+  int64_t sweeps_done = 0;
+  int64_t trials = 0;
+  int64_t accepted = 0;
+  int64_t E_run = 0;
+  bool E_valid = false;
+  std::vector<int64_t> trace;           // E_run after each sweep
+};
+
+// S0: basis positions in half-lattice units.
+const int kBasisBCC[2][3] = {{0, 0, 0}, {1, 1, 1}};
+const int kBasisFCC[4][3] = {{0, 0, 0}, {0, 1, 1}, {1, 0, 1}, {1, 1, 0}};
+
+inline const int* basis_of(const Oracle& o, int b) {
+  return o.lattice == LAT_BCC ? kBasisBCC[b] : kBasisFCC[b];
+}
+
+// S0: is the integer vector d (half-lattice units) a lattice translation?
+bool is_lattice_vector(int lattice, int dx, int dy, int dz) {
+  if (lattice == LAT_BCC) {
+    const int px = dx & 1, py = dy & 1, pz = dz & 1;
+    return px == py && py == pz;
+  }
+  return ((dx + dy + dz) & 1) == 0;
+}
+
+// S0: shell s = all lattice vectors with the s-th smallest non-zero |d|^2,
+// listed in ascending (dz, dy, dx) order.
+std::vector<std::vector<Vec3>> make_shells(int lattice, int n_shells) {
+  const int R = 8;
+  std::vector<int> d2s;
+  for (int dz = -R; dz <= R; ++dz)
+    for (int dy = -R; dy <= R; ++dy)
+      for (int dx = -R; dx <= R; ++dx) {
+        if (!(dx | dy | dz)) continue;
+        if (!is_lattice_vector(lattice, dx, dy, dz)) continue;
+        d2s.push_back(dx * dx + dy * dy + dz * dz);
+      }
+  std::sort(d2s.begin(), d2s.end());
+  d2s.erase(std::unique(d2s.begin(), d2s.end()), d2s.end());
+  std::vector<std::vector<Vec3>> out;
+  for (int s = 0; s < n_shells; ++s) {
+    const int want = d2s[s];
+    std::vector<Vec3> v;
+    for (int dz = -R; dz <= R; ++dz)
+      for (int dy = -R; dy <= R; ++dy)
+        for (int dx = -R; dx <= R; ++dx) {
+          if (!is_lattice_vector(lattice, dx, dy, dz)) continue;
+          if (dx * dx + dy * dy + dz * dz == want) v.push_back({dx, dy, dz});
+        }
+    out.push_back(v);
+  }
+  return out;
+}
+
+// S0: site id -> position (half-lattice units), and back.
+inline void site_to_pos(const Oracle& o, int64_t i, int p[3]) {
+  const int b = (int)(i % o.B);
+  int64_t c = i / o.B;
+  const int x = (int)(c % o.L[0]); c /= o.L[0];
+  const int y = (int)(c % o.L[1]); c /= o.L[1];
+  const int z = (int)c;
+  const int* beta = basis_of(o, b);
+  p[0] = 2 * x + beta[0];
+  p[1] = 2 * y + beta[1];
+  p[2] = 2 * z + beta[2];
+}
+
+// v is a site coordinate plus one shell offset, so it lies within one period of [0, period)
+// whenever period >= 8; tiny lattices (the 16-site exact test) need the general form.
+inline int wrap(int v, int period) {
+  if (v >= 0 && v < period) return v;
+  v %= period;
+  return v < 0 ? v + period : v;
+}
+
+inline int64_t pos_to_site(const Oracle& o, int px, int py, int pz) {
+  px = wrap(px, o.P[0]); py = wrap(py, o.P[1]); pz = wrap(pz, o.P[2]);
+  int b;
+  if (o.lattice == LAT_BCC) {
+    b = px & 1;
+  } else {
+    const int par = (px & 1) | ((py & 1) << 1) | ((pz & 1) << 2);
+    // (0,0,0)->0  (0,1,1)->1  (1,0,1)->2  (1,1,0)->3
+    b = par == 0 ? 0 : par == 6 ? 1 : par == 5 ? 2 : 3;
+  }
+  const int x = px >> 1, y = py >> 1, z = pz >> 1;
+  return (((int64_t)z * o.L[1] + y) * o.L[0] + x) * o.B + b;
+}
+
+inline int64_t neighbour(const Oracle& o, int64_t i, const Vec3& d) {
+  int p[3];
+  site_to_pos(o, i, p);
+  return pos_to_site(o, p[0] + d.x, p[1] + d.y, p[2] + d.z);
+}
+
+inline int32_t V(const Oracle& o, int s, int a, int b) {
+  return o.epi[((size_t)s * o.n_species + a) * o.n_species + b];
+}
+
+// S1: H = sum over shells, sites and the "positive half" O_s^+ of each shell of
+// V_s(sigma_i, sigma_{i+d}); every unordered bond once; int64.
+bool in_positive_half(const Vec3& d) {
+  if (d.z != 0) return d.z > 0;
+  if (d.y != 0) return d.y > 0;
+  return d.x > 0;
+}
+
+int64_t total_energy(const Oracle& o) {
+  int64_t H = 0;
+  for (int s = 0; s < o.n_shells; ++s)
+    for (const Vec3& d : o.shell[s]) {
+      if (!in_positive_half(d)) continue;
+      for (int64_t i = 0; i < o.N; ++i) H += V(o, s, o.sigma[i], o.sigma[neighbour(o, i, d)]);
+    }
+  return H;
+}
+
+// S1: the sites bonded to i and to j (one entry per shell offset, shells in order), with
+// the i-j bond(s) kept on i's side only: an entry of nbr_j that is i itself is marked -1.
+struct Bonds {
+  std::vector<int64_t> nbr_i, nbr_j;
+};
+
+void collect_bonds(const Oracle& o, int64_t i, int64_t j, Bonds& bonds) {
+  int pi[3], pj[3];
+  site_to_pos(o, i, pi);
+  site_to_pos(o, j, pj);
+  bonds.nbr_i.clear();
+  bonds.nbr_j.clear();
+  for (int s = 0; s < o.n_shells; ++s)
+    for (const Vec3& d : o.shell[s]) {
+      bonds.nbr_i.push_back(pos_to_site(o, pi[0] + d.x, pi[1] + d.y, pi[2] + d.z));
+      const int64_t n = pos_to_site(o, pj[0] + d.x, pj[1] + d.y, pj[2] + d.z);
+      bonds.nbr_j.push_back(n == i ? -1 : n);  // that bond is counted from i's side
+    }
+}
+
+// S1: energy of all bonds touching i or j (the i-j bond(s) counted once), as it stands.
+int64_t local_energy(const Oracle& o, int64_t i, int64_t j, const Bonds& bonds) {
+  int64_t e = 0;
+  size_t k = 0;
+  for (int s = 0; s < o.n_shells; ++s)
+    for (size_t m = 0; m < o.shell[s].size(); ++m, ++k) {
+      e += V(o, s, o.sigma[i], o.sigma[bonds.nbr_i[k]]);
+      if (bonds.nbr_j[k] >= 0) e += V(o, s, o.sigma[j], o.sigma[bonds.nbr_j[k]]);
+    }
+  return e;
+}
+
+// S1: dE of swapping sigma_i and sigma_j = H(sigma') - H(sigma), the plain way:
+// local energy after the swap minus before.  The state is left unchanged.
+int64_t swap_delta(Oracle& o, int64_t i, int64_t j) {
+  static thread_local Bonds bonds;
+  collect_bonds(o, i, j, bonds);
+  const int64_t before = local_energy(o, i, j, bonds);
+  std::swap(o.sigma[i], o.sigma[j]);
+  const int64_t after = local_energy(o, i, j, bonds);
+  std::swap(o.sigma[i], o.sigma[j]);
+  return after - before;
+}
+
+// S4: one trial with primary site i, direction word w_dir and acceptance word u.
+void trial(Oracle& o, int64_t i, uint32_t w_dir, uint32_t u) {
+  const std::vector<Vec3>& nn = o.shell[0];
+  const uint32_t dir = mulhi32(w_dir, (uint32_t)nn.size());
+  const int64_t j = neighbour(o, i, nn[dir]);
+  o.trials++;
+  if (o.count_visits) o.visits[i]++;
+  const uint8_t a = o.sigma[i], b = o.sigma[j];
+  if (a == b) return;  // Q8: same species, nothing changes
+  const int64_t dE = swap_delta(o, i, j);
+  // Eq. 3 in integer form (S5): P=1 for dE<=0, else u < T[dE].
+  const bool ok = dE <= 0 || (dE < (int64_t)o.accept.size() && u < o.accept[(size_t)dE]);
+  if (ok) {
+    std::swap(o.sigma[i], o.sigma[j]);
+    o.E_run += dE;
+    o.accepted++;
+  }
+}
+
+void ensure_energy(Oracle& o) {
+  if (!o.E_valid) {
+    o.E_run = total_energy(o);
+    o.E_valid = true;
+  }
+}
+
+// S3 + S4: one link-cell sweep.  order_mode: 0 = cells in ascending id, 1 = descending,
+// 2 = shuffled with std::mt19937(order_seed) (test-only; results must not depend on it).
+void sweep_lc(Oracle& o, int order_mode, uint32_t order_seed) {
+  ensure_energy(o);
+  const uint32_t key[2] = {(uint32_t)(o.seed & 0xffffffffu), (uint32_t)(o.seed >> 32)};
+  const uint32_t t = (uint32_t)o.sweeps_done;
+  const int w = o.w;
+  // S3.1: link-cell grid origin for this sweep.
+  const uint32_t cs[4] = {0u, 0u, t, (uint32_t)TAG_SHIFT};
+  uint32_t r[4];
+  philox4x32_10(cs, key, r);
+  const int ox = (int)mulhi32(r[0], (uint32_t)w);
+  const int oy = (int)mulhi32(r[1], (uint32_t)w);
+  const int oz = (int)mulhi32(r[2], (uint32_t)w);
+  const int ncx = o.L[0] / w, ncy = o.L[1] / w, ncz = o.L[2] / w;
+  const int S = w * w * w * o.B;
+  std::vector<uint32_t> cells;
+  for (int colour = 0; colour < 8; ++colour) {
+    // S2: cells of this colour.
+    cells.clear();
+    for (int cz = 0; cz < ncz; ++cz)
+      for (int cy = 0; cy < ncy; ++cy)
+        for (int cx = 0; cx < ncx; ++cx)
+          if (((cx & 1) | ((cy & 1) << 1) | ((cz & 1) << 2)) == colour)
+            cells.push_back((uint32_t)((cz * ncy + cy) * ncx + cx));
+    if (order_mode == 1) std::reverse(cells.begin(), cells.end());
+    if (order_mode == 2) {
+      std::mt19937 g(order_seed + (uint32_t)colour + 8u * t);
+      std::shuffle(cells.begin(), cells.end(), g);
+    }
+    for (uint32_t cell_id : cells) {
+      const int cx = (int)(cell_id % (uint32_t)ncx);
+      const int cy = (int)((cell_id / (uint32_t)ncx) % (uint32_t)ncy);
+      const int cz = (int)(cell_id / (uint32_t)(ncx * ncy));
+      for (int k = 0; k < S; ++k) {
+        // S3.2: slot k -> local site ((lz*w + ly)*w + lx)*B + b.
+        const int b = k % o.B;
+        int rest = k / o.B;
+        const int lx = rest % w; rest /= w;
+        const int ly = rest % w; rest /= w;
+        const int lz = rest;
+        const int x = (ox + cx * w + lx) % o.L[0];
+        const int y = (oy + cy * w + ly) % o.L[1];
+        const int z = (oz + cz * w + lz) % o.L[2];
+        const int64_t i = (((int64_t)z * o.L[1] + y) * o.L[0] + x) * o.B + b;
+        // S4: one Philox call serves two consecutive slots.
+        const uint32_t q = (uint32_t)(k >> 1);
+        const uint32_t ct[4] = {cell_id, q, t, (uint32_t)TAG_TRIAL | ((uint32_t)colour << 8)};
+        philox4x32_10(ct, key, r);
+        if (k & 1) trial(o, i, r[2], r[3]);
+        else       trial(o, i, r[0], r[1]);
+      }
+    }
+  }
+  // S3.3
+  o.trace.push_back(o.E_run);
+  o.sweeps_done++;
+}
+
+// S8: plain single-site-sequential Metropolis (no link cells); used for the exact
+// Boltzmann test and as the ensemble reference for the LC schedule.
+void sweep_seq(Oracle& o) {
+  ensure_energy(o);
+  const uint32_t key[2] = {(uint32_t)(o.seed & 0xffffffffu), (uint32_t)(o.seed >> 32)};
+  const uint32_t t = (uint32_t)o.sweeps_done;
+  uint32_t r[4];
+  for (int64_t i = 0; i < o.N; ++i) {
+    const uint32_t ct[4] = {(uint32_t)((uint64_t)i & 0xffffffffu), (uint32_t)((uint64_t)i >> 32), t,
+                            (uint32_t)TAG_SEQ};
+    philox4x32_10(ct, key, r);
+    trial(o, i, r[0], r[1]);
+  }
+  o.trace.push_back(o.E_run);
+  o.sweeps_done++;
+}
+
+// S6: seeded bijection of [0,N): 4-round balanced Feistel network over 2h bits with
+// cycle walking; sigma_i = pi(i) mod n_species, so the species counts are exactly
+// floor(N/n) + (p < N mod n).
+uint64_t feistel_permute(const Oracle& o, uint64_t v, int h) {
+  const uint32_t key[2] = {(uint32_t)(o.seed & 0xffffffffu), (uint32_t)(o.seed >> 32)};
+  const uint64_t mask = (1ull << h) - 1ull;
+  do {
+    uint64_t left = v >> h, right = v & mask;
+    for (uint32_t round = 0; round < 4; ++round) {
+      const uint32_t ct[4] = {(uint32_t)right, round, 0u, (uint32_t)TAG_INIT};
+      uint32_t r[4];
+      philox4x32_10(ct, key, r);
+      const uint64_t f = (uint64_t)r[0] & mask;
+      const uint64_t new_right = left ^ f;
+      left = right;
+      right = new_right;
+    }
+    v = (left << h) | right;
+  } while (v >= (uint64_t)o.N);
+  return v;
+}
+
+void init_species(Oracle& o) {
+  int h = 1;
+  while ((1ull << (2 * h)) < (uint64_t)o.N) ++h;
+  for (int64_t i = 0; i < o.N; ++i)
+    o.sigma[i] = (uint8_t)(feistel_permute(o, (uint64_t)i, h) % (uint64_t)o.n_species);
+  o.E_valid = false;
+}
+
+// S7: ordered pair counts N_s(p',p) = sum_i [sigma_i=p'] sum_{d in O_s} [sigma_{i+d}=p].
+void pair_counts(const Oracle& o, int64_t* counts) {
+  const int n = o.n_species;
+  std::fill(counts, counts + (size_t)o.n_shells * n * n, (int64_t)0);
+  for (int s = 0; s < o.n_shells; ++s)
+    for (const Vec3& d : o.shell[s])
+      for (int64_t i = 0; i < o.N; ++i) {
+        const int pc = o.sigma[i];
+        const int pn = o.sigma[neighbour(o, i, d)];
+        counts[((size_t)s * n + pc) * n + pn]++;
+      }
+}
+
+// Eq. 8: alpha_s^{pp'} = 1 - P_s(p | p') / c_p with
+// P_s(p|p') = N_s(p',p) / (Z_s n_{p'}) and c_p = n_p / N.  Stored at [s][p'][p].
+void sro(const Oracle& o, const int64_t* counts, double* alpha) {
+  const int n = o.n_species;
+  std::vector<int64_t> n_of(n, 0);
+  for (int64_t i = 0; i < o.N; ++i) n_of[o.sigma[i]]++;
+  for (int s = 0; s < o.n_shells; ++s) {
+    const double Z = (double)o.shell[s].size();
+    for (int pc = 0; pc < n; ++pc)
+      for (int pn = 0; pn < n; ++pn) {
+        const size_t idx = ((size_t)s * n + pc) * n + pn;
+        if (n_of[pc] == 0 || n_of[pn] == 0) {
+          alpha[idx] = std::numeric_limits<double>::quiet_NaN();
+          continue;
+        }
+        const double P = (double)counts[idx] / (Z * (double)n_of[pc]);
+        const double c = (double)n_of[pn] / (double)o.N;
+        alpha[idx] = 1.0 - P / c;
+      }
+  }
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------
+// C entry points for the ctypes wrapper in oracle/__init__.py.
+// ---------------------------------------------------------------------------------------
+extern "C" {
+
+void oracle_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
+  philox4x32_10(ctr, key, out);
+}
+
+// Writes up to max_out offsets (dx,dy,dz triples) of shell s; returns the shell size.
+int oracle_shell(int lattice, int s, int* out_xyz, int max_out) {
+  std::vector<std::vector<Vec3>> sh = make_shells(lattice, s + 1);
+  const std::vector<Vec3>& v = sh[s];
+  for (int k = 0; k < (int)v.size() && k < max_out; ++k) {
+    out_xyz[3 * k + 0] = v[k].x;
+    out_xyz[3 * k + 1] = v[k].y;
+    out_xyz[3 * k + 2] = v[k].z;
+  }
+  return (int)v.size();
+}
+
+void* oracle_create(int lattice, const int* dims, int n_species, int n_shells, const int32_t* epi,
+                    int link_cell, const uint32_t* accept, int accept_len, uint64_t seed) {
+  if (lattice != LAT_BCC && lattice != LAT_FCC) return nullptr;
+  if (n_species < 1 || n_species > 255 || n_shells < 1 || n_shells > 8) return nullptr;
+  for (int a = 0; a < 3; ++a)
+    if (dims[a] < 2) return nullptr;  // L=1 would make a 2nd-shell offset a self-bond
+  Oracle* o = new Oracle();
+  o->lattice = lattice;
+  o->B = lattice == LAT_BCC ? 2 : 4;
+  for (int a = 0; a < 3; ++a) { o->L[a] = dims[a]; o->P[a] = 2 * dims[a]; }
+  o->N = (int64_t)dims[0] * dims[1] * dims[2] * o->B;
+  o->n_species = n_species;
+  o->n_shells = n_shells;
+  o->epi.assign(epi, epi + (size_t)n_shells * n_species * n_species);
+  o->w = link_cell;
+  o->accept.assign(accept, accept + accept_len);
+  o->seed = seed;
+  o->shell = make_shells(lattice, n_shells);
+  o->sigma.assign((size_t)o->N, 0);
+  return o;
+}
+
+void oracle_destroy(void* h) { delete (Oracle*)h; }
+
+int64_t oracle_n_sites(void* h) { return ((Oracle*)h)->N; }
+
+void oracle_init_species(void* h) { init_species(*(Oracle*)h); }
+
+// pi(i) itself, for the bijection pin.
+uint64_t oracle_init_permutation(void* h, uint64_t i) {
+  Oracle& o = *(Oracle*)h;
+  int hh = 1;
+  while ((1ull << (2 * hh)) < (uint64_t)o.N) ++hh;
+  return feistel_permute(o, i, hh);
+}
+
+int oracle_set_species(void* h, const uint8_t* src) {
+  Oracle& o = *(Oracle*)h;
+  for (int64_t i = 0; i < o.N; ++i)
+    if (src[i] >= o.n_species) return -1;
+  std::memcpy(o.sigma.data(), src, (size_t)o.N);
+  o.E_valid = false;
+  return 0;
+}
+
+void oracle_get_species(void* h, uint8_t* dst) {
+  Oracle& o = *(Oracle*)h;
+  std::memcpy(dst, o.sigma.data(), (size_t)o.N);
+}
+
+void oracle_set_temperature(void* h, const uint32_t* accept, int accept_len) {
+  ((Oracle*)h)->accept.assign(accept, accept + accept_len);
+}
+
+int64_t oracle_energy(void* h) { return total_energy(*(Oracle*)h); }
+
+int64_t oracle_running_energy(void* h) {
+  Oracle& o = *(Oracle*)h;
+  ensure_energy(o);
+  return o.E_run;
+}
+
+int64_t oracle_neighbour(void* h, int64_t i, int s, int k) {
+  Oracle& o = *(Oracle*)h;
+  return neighbour(o, i, o.shell[s][k]);
+}
+
+// dE of swapping site i with its shell-0 neighbour number dir (state unchanged).
+int64_t oracle_delta_e(void* h, int64_t i, int dir) {
+  Oracle& o = *(Oracle*)h;
+  const int64_t j = neighbour(o, i, o.shell[0][dir]);
+  return swap_delta(o, i, j);
+}
+
+int oracle_lc_valid(void* h) {
+  // S2: 2w >= 2 r0 + R (per-axis reaches in half-lattice units; w in conventional cells
+  // = 2 half-units), and every dimension divisible by 2w.
+  Oracle& o = *(Oracle*)h;
+  if (o.w < 1) return 0;
+  for (int a = 0; a < 3; ++a)
+    if (o.L[a] % (2 * o.w)) return 0;
+  int r0 = 0, R = 0;
+  for (int s = 0; s < o.n_shells; ++s)
+    for (const Vec3& d : o.shell[s]) {
+      const int m = std::max(std::abs(d.x), std::max(std::abs(d.y), std::abs(d.z)));
+      if (s == 0) r0 = std::max(r0, m);
+      R = std::max(R, m);
+    }
+  return 2 * o.w >= 2 * r0 + R ? 1 : 0;
+}
+
+// n link-cell sweeps.  The caller is responsible for oracle_lc_valid(); an invalid w is
+// allowed on purpose so that a test can show the order dependence it causes.
+int oracle_sweep_lc(void* h, int64_t n, int order_mode, uint32_t order_seed) {
+  Oracle& o = *(Oracle*)h;
+  if (o.w < 1) return -1;
+  for (int a = 0; a < 3; ++a)
+    if (o.L[a] % (2 * o.w)) return -1;
+  for (int64_t s = 0; s < n; ++s) sweep_lc(o, order_mode, order_seed);
+  return 0;
+}
+
+void oracle_sweep_seq(void* h, int64_t n) {
+  Oracle& o = *(Oracle*)h;
+  for (int64_t s = 0; s < n; ++s) sweep_seq(o);
+}
+
+// The link-cell origin S3.1 draws for sweep t.
+void oracle_shift(void* h, uint32_t t, int* oxyz) {
+  Oracle& o = *(Oracle*)h;
+  const uint32_t key[2] = {(uint32_t)(o.seed & 0xffffffffu), (uint32_t)(o.seed >> 32)};
+  const uint32_t cs[4] = {0u, 0u, t, (uint32_t)TAG_SHIFT};
+  uint32_t r[4];
+  philox4x32_10(cs, key, r);
+  for (int a = 0; a < 3; ++a) oxyz[a] = (int)mulhi32(r[a], (uint32_t)o.w);
+}
+
+void oracle_stats(void* h, int64_t* sweeps, int64_t* trials, int64_t* accepted) {
+  Oracle& o = *(Oracle*)h;
+  *sweeps = o.sweeps_done; *trials = o.trials; *accepted = o.accepted;
+}
+
+int64_t oracle_trace(void* h, int64_t first, int64_t count, int64_t* dst) {
+  Oracle& o = *(Oracle*)h;
+  if (first < 0 || first + count > (int64_t)o.trace.size()) return -1;
+  for (int64_t k = 0; k < count; ++k) dst[k] = o.trace[(size_t)(first + k)];
+  return count;
+}
+
+void oracle_count_visits(void* h, int on) {
+  Oracle& o = *(Oracle*)h;
+  o.count_visits = on != 0;
+  o.visits.assign(on ? (size_t)o.N : 0, 0u);
+}
+
+void oracle_get_visits(void* h, uint32_t* dst) {
+  Oracle& o = *(Oracle*)h;
+  std::memcpy(dst, o.visits.data(), o.visits.size() * sizeof(uint32_t));
+}
+
+void oracle_pair_counts(void* h, int64_t* counts) { pair_counts(*(Oracle*)h, counts); }
+
+void oracle_sro(void* h, double* alpha, int64_t* counts_or_null) {
+  Oracle& o = *(Oracle*)h;
+  std::vector<int64_t> c((size_t)o.n_shells * o.n_species * o.n_species);
+  pair_counts(o, c.data());
+  sro(o, c.data(), alpha);
+  if (counts_or_null) std::memcpy(counts_or_null, c.data(), c.size() * sizeof(int64_t));
+}
+
+}  // extern "C"

@@ -1,0 +1,68 @@
+"""EPI tables and acceptance-threshold tables (input data, see package docstring)."""
+from __future__ import annotations
+
+import math
+
+import numpy as np
+
+TAG_EPI = 4  # low byte of ctr[3]; SURVEY.md 8(c) S4 tag list
+
+_M0 = 0xD2511F53
+_M1 = 0xCD9E8D57
+_W0 = 0x9E3779B9
+_W1 = 0xBB67AE85
+_MASK = 0xFFFFFFFF
+
+
+def philox4x32_10(ctr, key):
+    """Philox4x32-10 (Salmon et al., SC'11), pure-Python integers.
+
+    Only used to draw the handful of EPI entries; the oracle and the CUDA path each carry
+    their own implementation.  ``ctr`` is 4 and ``key`` 2 unsigned 32-bit integers.
+    """
+    c0, c1, c2, c3 = (int(c) & _MASK for c in ctr)
+    k0, k1 = (int(k) & _MASK for k in key)
+    for _ in range(10):
+        p0 = _M0 * c0
+        p1 = _M1 * c2
+        hi0, lo0 = p0 >> 32, p0 & _MASK
+        hi1, lo1 = p1 >> 32, p1 & _MASK
+        c0, c1, c2, c3 = hi1 ^ c1 ^ k0, lo1, hi0 ^ c3 ^ k1, lo0
+        k0 = (k0 + _W0) & _MASK
+        k1 = (k1 + _W1) & _MASK
+    return c0, c1, c2, c3
+
+
+def make_epi(n_shells: int, n_species: int, amplitude: int, seed: int) -> np.ndarray:
+    """Symmetric int32 EPI tables, shape [n_shells][n_species][n_species], 0.1 meV units."""
+    key = (seed & _MASK, (seed >> 32) & _MASK)
+    v = np.zeros((n_shells, n_species, n_species), dtype=np.int32)
+    span = 2 * amplitude + 1
+    for s in range(n_shells):
+        for a in range(n_species):
+            for b in range(a, n_species):
+                r0 = philox4x32_10((a, b, s, TAG_EPI), key)[0]
+                val = -amplitude + ((r0 * span) >> 32)
+                v[s, a, b] = val
+                v[s, b, a] = val
+    return v
+
+
+def accept_table_len(kT_units: int) -> int:
+    return int(math.floor(32.0 * math.log(2.0) * kT_units)) + 2
+
+
+def make_accept_table(kT_units: int) -> np.ndarray:
+    """uint32 thresholds: a trial with dE = d > 0 is accepted iff u < T[d] (u a 32-bit draw)."""
+    n = accept_table_len(kT_units)
+    d = np.arange(n, dtype=np.float64)
+    x = np.exp(-d / float(kT_units)) * 4294967296.0
+    t = np.where(x >= 4294967295.0, 4294967295.0, np.floor(x))
+    return t.astype(np.uint32)
+
+
+def anneal_kT_units(t: int, n_sweeps: int = 2000, kT_hi: int = 1720, kT_lo: int = 430) -> int:
+    """Linear anneal of config 2: kT(t) = kT_hi - floor((kT_hi-kT_lo) * t / (n_sweeps-1))."""
+    if n_sweeps <= 1:
+        return kT_hi
+    return kT_hi - ((kT_hi - kT_lo) * t) // (n_sweeps - 1)
