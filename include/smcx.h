@@ -1,0 +1,156 @@
+/* smcx.h -- C ABI of the B200-native SMC-X hot path (arxiv 2509.20949).
+ *
+ * What the library computes: parallel Metropolis atom-swap sweeps over a multicomponent
+ * BCC/FCC lattice alloy with an effective-pair-interaction (EPI) Hamiltonian, scheduled by
+ * dynamic link cells (LC):
+ *   - canonical ensemble and Metropolis acceptance, Eq. 1-3;
+ *   - one Monte Carlo step (sweep) = exactly one trial move per lattice site;
+ *   - a trial move swaps two neighbouring lattice sites;
+ *   - link cells are re-built every step so that every site is visited exactly once and
+ *     distant cells update concurrently; each trial costs O(1) through the local interaction
+ *     zone (LIZ / LIZ+), section "Distributed SMC-X" (Eq. 4);
+ *   - the EPI model is pairwise (section "Results and discussion");
+ *   - the Warren-Cowley short-range-order parameter, Eq. 8.
+ * The paper defers the concrete schedule to its Ref. 22; the schedule implemented here (per-sweep
+ * random LC origin, 2x2x2 colouring, raster order inside a cell, Philox4x32-10 keyed by
+ * (seed, sweep, colour, cell), integer energies and table-driven integer acceptance) is the
+ * reading S0-S8 listed in DESIGN.md.  Given that schedule the species array and the energy trace
+ * after n sweeps are unique, and the library reproduces them bit for bit.
+ *
+ * Conventions
+ *   - Every call returns SMCX_OK (0) or a negative SMCX_E_* code.  Nothing throws or aborts
+ *     across this boundary.  Out-parameters are written only on success.
+ *   - "host" pointers are ordinary CPU memory, "device" pointers are CUDA device memory on the
+ *     handle's device.  The caller owns every pointer it passes; host tables are copied during
+ *     the call.  Device buffers passed at creation must outlive the handle.
+ *   - All GPU work is enqueued on the stream given at creation.  Calls that return results to
+ *     the host synchronise that stream; smcx_sweep and smcx_set_temperature do not.
+ *   - A handle is not thread-safe.  One handle drives one GPU; there is no CPU fallback:
+ *     without a CUDA device smcx_create fails with SMCX_E_CUDA.
+ *
+ * Geometry (reading S0).  Lengths in units of a/2.  BCC: 2 sites per conventional cell at
+ * (0,0,0),(1,1,1); FCC: 4 sites at (0,0,0),(0,1,1),(1,0,1),(1,1,0).  Site id
+ * i = ((z*Ly + y)*Lx + x)*B + b (PAPER.md:165 writes lattices as nx*ny*nz*basis), periodic in
+ * all three directions.  Shell s is the set of lattice vectors with the s-th smallest
+ * non-zero length, in ascending (dz, dy, dx) order.
+ */
+#ifndef SMCX_H_
+#define SMCX_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct smcx smcx_t; /* opaque; one per (GPU, stream) */
+
+enum { SMCX_BCC = 0, SMCX_FCC = 1 };
+
+/* Device storage of the species array. U8: one byte per site in site-id order.
+ * 2BIT: 16 sites per 32-bit word in site-id order (n_species <= 4).  Results never depend on it. */
+enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
+
+/* Which sweep kernel runs.  WARP_PER_CELL: any lattice/shell list, U8 storage.
+ * THREAD_PER_CELL: BCC, first two shells, link_cell = 4, n_species <= 4, 2BIT storage.
+ * AUTO picks THREAD_PER_CELL when the parameters allow it.  Results never depend on it. */
+enum { SMCX_KERNEL_AUTO = 0, SMCX_KERNEL_WARP_PER_CELL = 1, SMCX_KERNEL_THREAD_PER_CELL = 2 };
+
+enum {
+  SMCX_OK = 0,
+  SMCX_E_NULL_ARG = -1,
+  SMCX_E_BAD_LATTICE = -2,
+  SMCX_E_BAD_DIMS = -3,            /* non-positive, not divisible by 2*link_cell, smaller than a
+                                      cell plus its halo, or too many sites/cells */
+  SMCX_E_BAD_SPECIES = -4,         /* n_species outside 2..16 */
+  SMCX_E_BAD_SHELLS = -5,          /* n_shells outside 1..5 */
+  SMCX_E_EPI_NOT_SYMMETRIC = -6,
+  SMCX_E_LINK_CELL_TOO_SMALL = -7, /* violates 2w >= 2 r0 + R (reading S2) */
+  SMCX_E_BAD_TABLE = -8,           /* acceptance table missing, empty or too long */
+  SMCX_E_BAD_STATE = -9,           /* uploaded species value >= n_species */
+  SMCX_E_NO_MEMORY = -10,          /* host or device allocation failed / workspace too small */
+  SMCX_E_CUDA = -11,               /* CUDA error; text via smcx_last_error */
+  SMCX_E_UNSUPPORTED = -12,        /* storage/kernel choice not valid for these parameters */
+  SMCX_E_RANGE = -13               /* trace range not retained, sweep counter overflow */
+};
+
+typedef struct {
+  int32_t lattice;          /* SMCX_BCC | SMCX_FCC */
+  int32_t dims[3];          /* Lx, Ly, Lz conventional cells; each divisible by 2*link_cell */
+  int32_t n_species;        /* 2..16; species values are 0..n_species-1 */
+  int32_t n_shells;         /* the first n_shells neighbour shells, 1..5 */
+  const int32_t *epi;       /* host, [n_shells][n_species][n_species], symmetric, 0.1 meV units */
+  int32_t link_cell;        /* w, conventional cells per link-cell edge; 0 means 4 */
+  int32_t kT_units;         /* kT in 0.1 meV; recorded for reports only (see accept) */
+  const uint32_t *accept;   /* host, thresholds T[0..accept_len): a trial with dE = d > 0 is
+                               accepted iff d < accept_len and u < T[d], u a 32-bit Philox word
+                               (Eq. 3 in integer form); the library never evaluates exp() */
+  int32_t accept_len;       /* 1 .. 2^22 */
+  uint64_t seed;            /* Philox key */
+  int32_t storage;          /* SMCX_STORAGE_* */
+  int32_t kernel;           /* SMCX_KERNEL_* */
+  int32_t device;           /* CUDA device ordinal */
+  int32_t trace_capacity;   /* sweeps of energy trace retained (ring buffer); 0 means 65536 */
+  void *stream;             /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy default */
+  void *d_workspace;        /* device, caller-owned, >= smcx_workspace_bytes(); NULL = library allocates */
+  size_t workspace_bytes;   /* size of d_workspace */
+} smcx_params_t;
+
+/* Bytes of device workspace a handle with these parameters needs (species array in its storage
+ * format, tables, trace, counters).  Validates the parameters like smcx_create. */
+int smcx_workspace_bytes(const smcx_params_t *p, size_t *bytes);
+
+/* Validates, copies the tables, builds the shell-offset tables, and fills the lattice with the
+ * seeded equiatomic initial state (reading S6: sigma_i = pi(i) mod n_species, pi a 4-round Feistel
+ * permutation of [0,N) keyed by seed).  The sweep counter starts at 0. */
+int smcx_create(smcx_t **out, const smcx_params_t *p);
+void smcx_destroy(smcx_t *h);
+
+/* Replace the lattice state.  host_src / d_src: N bytes, one species per site in site-id order.
+ * Returns SMCX_E_BAD_STATE (state unchanged on the host path) if a value is >= n_species.
+ * The running energy is recomputed; the sweep counter and trace are kept. */
+int smcx_set_species(smcx_t *h, const uint8_t *host_src);
+int smcx_set_species_device(smcx_t *h, const void *d_src);
+
+/* New acceptance table (a new temperature) for the following sweeps.  Asynchronous with respect
+ * to the host: the table is copied into library-owned pinned memory before the call returns. */
+int smcx_set_temperature(smcx_t *h, int32_t kT_units, const uint32_t *accept, int32_t accept_len);
+
+/* Enqueue n sweeps (reading S3).  Asynchronous.  The sweep counter is global to the handle:
+ * sweep(a); sweep(b) is identical to sweep(a+b). */
+int smcx_sweep(smcx_t *h, int64_t n);
+
+/* Total energy H (reading S1: every unordered bond once, int64) recomputed from the lattice by the
+ * pair-count reduction kernel.  Synchronises. */
+int smcx_energy(smcx_t *h, int64_t *E);
+/* Running energy E_0 + sum of accepted dE as kept by the sweep kernels.  Synchronises. */
+int smcx_running_energy(smcx_t *h, int64_t *E);
+/* dst[k] = running energy after sweep first_sweep + k, k < count.  Synchronises. */
+int smcx_energy_trace(smcx_t *h, int64_t first_sweep, int64_t count, int64_t *dst);
+
+/* Species, N bytes, one per site in site-id order whatever the device storage.  Synchronises. */
+int smcx_species(smcx_t *h, uint8_t *host_dst);
+int smcx_species_device(smcx_t *h, void *d_dst); /* asynchronous, on the handle's stream */
+
+/* Warren-Cowley parameters, Eq. 8: alpha[(s*n + p')*n + p] = 1 - N_s(p',p) N / (Z_s n_p' n_p) in
+ * fp64 from the exact ordered pair counts N_s(p',p) = #{(i,d): d in shell s, sigma_i = p',
+ * sigma_{i+d} = p} (int64).  NaN where a species is absent.  pair_counts may be NULL.  Synchronises. */
+int smcx_sro(smcx_t *h, double *alpha, int64_t *pair_counts);
+
+int smcx_stats(smcx_t *h, int64_t *sweeps_done, int64_t *trials, int64_t *accepted);
+int smcx_synchronize(smcx_t *h);
+
+/* Introspection for tests and benchmarks. */
+int smcx_shell_offsets(smcx_t *h, int32_t shell, int32_t *xyz, int32_t max_offsets, int32_t *n_offsets);
+int smcx_get_config(smcx_t *h, int32_t *storage, int32_t *kernel, int64_t *n_sites, int64_t *n_cells);
+int64_t smcx_kernel_launches(smcx_t *h); /* kernels launched by this handle so far */
+
+const char *smcx_last_error(smcx_t *h); /* text of the last CUDA error seen by this handle */
+const char *smcx_strerror(int code);
+const char *smcx_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SMCX_H_ */

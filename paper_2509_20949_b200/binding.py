@@ -1,0 +1,266 @@
+"""ctypes binding for include/smcx.h -- same names, argument marshalling only."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import re
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libsmcx.so")
+_HEADER = os.path.join(os.path.dirname(_HERE), "include", "smcx.h")
+_lib = None
+
+BCC, FCC = 0, 1
+STORAGE_AUTO, STORAGE_2BIT, STORAGE_U8 = 0, 2, 8
+KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL = 0, 1, 2
+
+
+class SmcxError(RuntimeError):
+    def __init__(self, code: int, what: str, detail: str = ""):
+        self.code = code
+        super().__init__(f"{what}: [{code}] {_strerror(code)}" + (f" ({detail})" if detail else ""))
+
+
+class _Params(C.Structure):
+    _fields_ = [
+        ("lattice", C.c_int32), ("dims", C.c_int32 * 3), ("n_species", C.c_int32), ("n_shells", C.c_int32),
+        ("epi", C.POINTER(C.c_int32)), ("link_cell", C.c_int32), ("kT_units", C.c_int32),
+        ("accept", C.POINTER(C.c_uint32)), ("accept_len", C.c_int32), ("seed", C.c_uint64),
+        ("storage", C.c_int32), ("kernel", C.c_int32), ("device", C.c_int32), ("trace_capacity", C.c_int32),
+        ("stream", C.c_void_p), ("d_workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+    ]
+
+
+def library_path() -> str:
+    return _LIB_PATH
+
+
+def exported_symbols() -> list:
+    """Function names declared in include/smcx.h."""
+    text = open(_HEADER).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(smcx_[a-z_0-9]+)\s*\(", text)))
+
+
+def load_library(build_if_missing: bool = True):
+    """dlopen libsmcx.so (built in-tree by paper_2509_20949_b200/build.py).  Raises if absent."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_missing:
+        from . import build as _build
+        try:
+            _build.build()
+        except Exception as exc:  # nvcc missing or compile error
+            if not os.path.exists(_LIB_PATH):
+                raise RuntimeError(f"libsmcx.so is not built and could not be built: {exc}") from exc
+    if not os.path.exists(_LIB_PATH):
+        raise RuntimeError("libsmcx.so not found; run `python -m paper_2509_20949_b200.build`")
+    lib = C.CDLL(_LIB_PATH)
+    vp, i64p, i32p = C.c_void_p, C.POINTER(C.c_int64), C.POINTER(C.c_int32)
+    sig = {
+        "smcx_workspace_bytes": (C.c_int, [C.POINTER(_Params), C.POINTER(C.c_size_t)]),
+        "smcx_create": (C.c_int, [C.POINTER(vp), C.POINTER(_Params)]),
+        "smcx_destroy": (None, [vp]),
+        "smcx_set_species": (C.c_int, [vp, C.POINTER(C.c_uint8)]),
+        "smcx_set_species_device": (C.c_int, [vp, vp]),
+        "smcx_set_temperature": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_uint32), C.c_int32]),
+        "smcx_sweep": (C.c_int, [vp, C.c_int64]),
+        "smcx_energy": (C.c_int, [vp, i64p]),
+        "smcx_running_energy": (C.c_int, [vp, i64p]),
+        "smcx_energy_trace": (C.c_int, [vp, C.c_int64, C.c_int64, i64p]),
+        "smcx_species": (C.c_int, [vp, C.POINTER(C.c_uint8)]),
+        "smcx_species_device": (C.c_int, [vp, vp]),
+        "smcx_sro": (C.c_int, [vp, C.POINTER(C.c_double), i64p]),
+        "smcx_stats": (C.c_int, [vp, i64p, i64p, i64p]),
+        "smcx_synchronize": (C.c_int, [vp]),
+        "smcx_shell_offsets": (C.c_int, [vp, C.c_int32, i32p, C.c_int32, i32p]),
+        "smcx_get_config": (C.c_int, [vp, i32p, i32p, i64p, i64p]),
+        "smcx_kernel_launches": (C.c_int64, [vp]),
+        "smcx_last_error": (C.c_char_p, [vp]),
+        "smcx_strerror": (C.c_char_p, [C.c_int]),
+        "smcx_version": (C.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    _lib = lib
+    return lib
+
+
+def _strerror(code: int) -> str:
+    try:
+        return load_library(False).smcx_strerror(code).decode()
+    except Exception:
+        return "?"
+
+
+def _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage, kernel,
+                 device, trace_capacity):
+    epi = np.ascontiguousarray(epi, dtype=np.int32)
+    accept = np.ascontiguousarray(accept, dtype=np.uint32)
+    p = _Params()
+    p.lattice = int(lattice)
+    p.dims = (C.c_int32 * 3)(*[int(d) for d in dims])
+    p.n_species, p.n_shells = int(n_species), int(n_shells)
+    p.epi = epi.ctypes.data_as(C.POINTER(C.c_int32))
+    p.link_cell, p.kT_units = int(link_cell), int(kT_units)
+    p.accept = accept.ctypes.data_as(C.POINTER(C.c_uint32))
+    p.accept_len = int(accept.size)
+    p.seed = int(seed)
+    p.storage, p.kernel, p.device, p.trace_capacity = int(storage), int(kernel), int(device), int(trace_capacity)
+    return p, (epi, accept)
+
+
+class Lattice:
+    """One smcx_t handle.  Methods mirror the C entry points of include/smcx.h."""
+
+    def __init__(self, lattice, dims, n_species, n_shells, epi, accept, seed, link_cell=4, kT_units=0,
+                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0):
+        import torch  # device memory + stream only
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2509_20949_b200 needs a CUDA device; there is no CPU fallback")
+        self._lib = lib = load_library()
+        self._h = None
+        p, keep = _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage,
+                               kernel, device, trace_capacity)
+        need = C.c_size_t(0)
+        rc = lib.smcx_workspace_bytes(C.byref(p), C.byref(need))
+        if rc != 0:
+            raise SmcxError(rc, "smcx_workspace_bytes")
+        self.device = torch.device("cuda", int(device))
+        with torch.cuda.device(self.device):
+            self._workspace = torch.empty(int(need.value), dtype=torch.uint8, device=self.device)
+            self._stream = torch.cuda.current_stream(self.device)
+        p.stream = C.c_void_p(self._stream.cuda_stream)
+        p.d_workspace = C.c_void_p(self._workspace.data_ptr())
+        p.workspace_bytes = int(need.value)
+        h = C.c_void_p()
+        rc = lib.smcx_create(C.byref(h), C.byref(p))
+        if rc != 0:
+            raise SmcxError(rc, "smcx_create")
+        self._h = h
+        del keep
+        self.lattice, self.dims = int(lattice), tuple(int(d) for d in dims)
+        self.n_species, self.n_shells = int(n_species), int(n_shells)
+        st, kn, ns, nc = C.c_int32(), C.c_int32(), C.c_int64(), C.c_int64()
+        self._check(lib.smcx_get_config(h, C.byref(st), C.byref(kn), C.byref(ns), C.byref(nc)), "smcx_get_config")
+        self.storage, self.kernel, self.n_sites, self.n_cells = st.value, kn.value, ns.value, nc.value
+
+    @classmethod
+    def from_config(cls, cfg, **over):
+        kw = dict(lattice=cfg.lattice, dims=cfg.dims, n_species=cfg.n_species, n_shells=cfg.n_shells, epi=cfg.epi(),
+                  accept=cfg.accept_table(0), seed=cfg.seed, link_cell=cfg.link_cell, kT_units=cfg.kT_at(0))
+        kw.update(over)
+        return cls(**kw)
+
+    # -- plumbing ---------------------------------------------------------------------------
+    def _check(self, rc, what):
+        if rc != 0:
+            detail = self._lib.smcx_last_error(self._h).decode() if self._h else ""
+            raise SmcxError(rc, what, detail)
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._lib.smcx_destroy(self._h)
+            self._h = None
+            self._workspace = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- smcx.h -----------------------------------------------------------------------------
+    def set_species(self, species):
+        s = np.ascontiguousarray(species, dtype=np.uint8)
+        if s.size != self.n_sites:
+            raise ValueError("species must have n_sites entries")
+        self._check(self._lib.smcx_set_species(self._h, s.ctypes.data_as(C.POINTER(C.c_uint8))), "smcx_set_species")
+
+    def set_species_device(self, tensor):
+        assert tensor.is_cuda and tensor.dtype.itemsize == 1 and tensor.numel() == self.n_sites and tensor.is_contiguous()
+        self._check(self._lib.smcx_set_species_device(self._h, C.c_void_p(tensor.data_ptr())), "smcx_set_species_device")
+
+    def set_temperature(self, kT_units, accept):
+        a = np.ascontiguousarray(accept, dtype=np.uint32)
+        self._check(self._lib.smcx_set_temperature(self._h, int(kT_units), a.ctypes.data_as(C.POINTER(C.c_uint32)),
+                                                   int(a.size)), "smcx_set_temperature")
+
+    def sweep(self, n=1):
+        self._check(self._lib.smcx_sweep(self._h, int(n)), "smcx_sweep")
+
+    def energy(self) -> int:
+        e = C.c_int64()
+        self._check(self._lib.smcx_energy(self._h, C.byref(e)), "smcx_energy")
+        return e.value
+
+    def running_energy(self) -> int:
+        e = C.c_int64()
+        self._check(self._lib.smcx_running_energy(self._h, C.byref(e)), "smcx_running_energy")
+        return e.value
+
+    def energy_trace(self, first=0, count=None) -> np.ndarray:
+        if count is None:
+            count = self.stats()[0] - first
+        out = np.zeros(int(count), dtype=np.int64)
+        self._check(self._lib.smcx_energy_trace(self._h, int(first), int(count), out.ctypes.data_as(C.POINTER(C.c_int64))),
+                    "smcx_energy_trace")
+        return out
+
+    def species(self, out=None) -> np.ndarray:
+        if out is None:
+            out = np.empty(self.n_sites, dtype=np.uint8)
+        assert out.dtype == np.uint8 and out.size == self.n_sites and out.flags.c_contiguous
+        self._check(self._lib.smcx_species(self._h, out.ctypes.data_as(C.POINTER(C.c_uint8))), "smcx_species")
+        return out
+
+    def species_device(self, out=None):
+        import torch
+        if out is None:
+            out = torch.empty(self.n_sites, dtype=torch.uint8, device=self.device)
+        self._check(self._lib.smcx_species_device(self._h, C.c_void_p(out.data_ptr())), "smcx_species_device")
+        return out
+
+    def sro(self):
+        shape = (self.n_shells, self.n_species, self.n_species)
+        alpha = np.zeros(shape, dtype=np.float64)
+        counts = np.zeros(shape, dtype=np.int64)
+        self._check(self._lib.smcx_sro(self._h, alpha.ctypes.data_as(C.POINTER(C.c_double)),
+                                       counts.ctypes.data_as(C.POINTER(C.c_int64))), "smcx_sro")
+        return alpha, counts
+
+    def stats(self):
+        a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
+        self._check(self._lib.smcx_stats(self._h, C.byref(a), C.byref(b), C.byref(c)), "smcx_stats")
+        return a.value, b.value, c.value
+
+    def synchronize(self):
+        self._check(self._lib.smcx_synchronize(self._h), "smcx_synchronize")
+
+    def shell_offsets(self, shell) -> np.ndarray:
+        buf = np.zeros((64, 3), dtype=np.int32)
+        n = C.c_int32()
+        self._check(self._lib.smcx_shell_offsets(self._h, int(shell), buf.ctypes.data_as(C.POINTER(C.c_int32)), 64,
+                                                 C.byref(n)), "smcx_shell_offsets")
+        return buf[: n.value].copy()
+
+    @property
+    def kernel_launches(self) -> int:
+        return int(self._lib.smcx_kernel_launches(self._h))
+
+
+def workspace_bytes(**kw) -> int:
+    lib = load_library()
+    defaults = dict(link_cell=4, kT_units=0, storage=0, kernel=0, device=0, trace_capacity=0)
+    defaults.update(kw)
+    p, _keep = _make_params(**defaults)
+    need = C.c_size_t(0)
+    rc = lib.smcx_workspace_bytes(C.byref(p), C.byref(need))
+    if rc != 0:
+        raise SmcxError(rc, "smcx_workspace_bytes")
+    return int(need.value)

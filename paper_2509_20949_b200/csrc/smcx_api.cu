@@ -1,0 +1,681 @@
+// C ABI of the SMC-X CUDA path (include/smcx.h): validation, host-side geometry tables,
+// workspace layout, launch orchestration.  No CPU fallback: every step of the hot path runs in
+// the kernels of this directory.
+#include "../../include/smcx.h"
+
+#include <algorithm>
+#include <cmath>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <limits>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "lattice_kernels.cuh"
+#include "smcx_common.cuh"
+#include "sweep_thread.cuh"
+#include "sweep_warp.cuh"
+
+using namespace smcxk;
+
+namespace {
+
+constexpr int kAcceptCapacity = 1 << 20;  // entries reserved on the device for the threshold table
+constexpr int kStagingSlots = 4;
+constexpr long long kChunkSites = 1ll << 26;  // bounce-buffer size for packed <-> uint8 transfers
+
+struct ShellVec { int x, y, z, d2; };
+
+// S0: lattice translations of BCC (all components of equal parity) and FCC (even component sum)
+// in units of a/2, grouped by squared length; within a shell ascending (dz, dy, dx).
+std::vector<std::vector<ShellVec>> build_shells(int lattice, int n_shells) {
+  std::vector<ShellVec> all;
+  const int R = 6;
+  for (int z = -R; z <= R; ++z)
+    for (int y = -R; y <= R; ++y)
+      for (int x = -R; x <= R; ++x) {
+        if (x == 0 && y == 0 && z == 0) continue;
+        const bool ok = lattice == SMCX_BCC ? (((x ^ y) & 1) == 0 && ((y ^ z) & 1) == 0) : (((x + y + z) & 1) == 0);
+        if (ok) all.push_back({x, y, z, x * x + y * y + z * z});
+      }
+  std::stable_sort(all.begin(), all.end(), [](const ShellVec& a, const ShellVec& b) {
+    if (a.d2 != b.d2) return a.d2 < b.d2;
+    if (a.z != b.z) return a.z < b.z;
+    if (a.y != b.y) return a.y < b.y;
+    return a.x < b.x;
+  });
+  std::vector<std::vector<ShellVec>> shells;
+  for (size_t k = 0; k < all.size() && (int)shells.size() <= n_shells; ++k) {
+    if (k == 0 || all[k].d2 != all[k - 1].d2) {
+      if ((int)shells.size() == n_shells) break;
+      shells.emplace_back();
+    }
+    shells.back().push_back(all[k]);
+  }
+  return shells;
+}
+
+void basis_pos(int lattice, int b, int p[3]) {
+  if (lattice == SMCX_BCC) { p[0] = p[1] = p[2] = b; return; }
+  static const int f[4][3] = {{0, 0, 0}, {0, 1, 1}, {1, 0, 1}, {1, 1, 0}};
+  p[0] = f[b][0]; p[1] = f[b][1]; p[2] = f[b][2];
+}
+
+int basis_from_parity(int lattice, int px, int py, int pz) {
+  if (lattice == SMCX_BCC) return px & 1;
+  const int par = (px & 1) | ((py & 1) << 1) | ((pz & 1) << 2);
+  return par == 0 ? 0 : par == 6 ? 1 : par == 5 ? 2 : 3;
+}
+
+inline int floor_div2(int v) { return v >= 0 ? v / 2 : -((-v + 1) / 2); }
+
+struct Layout {
+  size_t species, epi, accept, trace, state, counts, total;
+};
+
+struct Plan {
+  Geom G;
+  long long n_sites;
+  long long n_cells;
+  int storage;
+  int kernel;
+  Layout lay;
+};
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+int make_plan(const smcx_params_t* p, Plan* plan) {
+  if (!p || !plan) return SMCX_E_NULL_ARG;
+  if (p->lattice != SMCX_BCC && p->lattice != SMCX_FCC) return SMCX_E_BAD_LATTICE;
+  if (p->n_species < 2 || p->n_species > kMaxSpecies) return SMCX_E_BAD_SPECIES;
+  if (p->n_shells < 1 || p->n_shells > kMaxShells) return SMCX_E_BAD_SHELLS;
+  if (!p->epi) return SMCX_E_NULL_ARG;
+  if (!p->accept || p->accept_len < 1 || p->accept_len > kAcceptCapacity) return SMCX_E_BAD_TABLE;
+  const int n = p->n_species;
+  for (int s = 0; s < p->n_shells; ++s)
+    for (int a = 0; a < n; ++a)
+      for (int b = 0; b < a; ++b)
+        if (p->epi[(s * n + a) * n + b] != p->epi[(s * n + b) * n + a]) return SMCX_E_EPI_NOT_SYMMETRIC;
+  const int w = p->link_cell == 0 ? 4 : p->link_cell;
+  if (w < 1 || w > 16) return SMCX_E_LINK_CELL_TOO_SMALL;
+
+  Geom& G = plan->G;
+  std::memset(&G, 0, sizeof(G));
+  G.lattice = p->lattice;
+  G.B = p->lattice == SMCX_BCC ? 2 : 4;
+  G.n_species = n;
+  G.n_shells = p->n_shells;
+  G.w = w;
+  const auto shells = build_shells(p->lattice, p->n_shells);
+  int m = 0, R = 0, r0 = 0, nh = 0;
+  for (int s = 0; s < p->n_shells; ++s)
+    for (const ShellVec& v : shells[s]) {
+      if (m >= kMaxNeighbours) return SMCX_E_BAD_SHELLS;
+      G.off[m][0] = (signed char)v.x; G.off[m][1] = (signed char)v.y; G.off[m][2] = (signed char)v.z;
+      G.shell_of[m] = (unsigned char)s;
+      const int reach = std::max(std::abs(v.x), std::max(std::abs(v.y), std::abs(v.z)));
+      R = std::max(R, reach);
+      if (s == 0) r0 = std::max(r0, reach);
+      const int first = v.z != 0 ? v.z : (v.y != 0 ? v.y : v.x);
+      if (first > 0) G.half_idx[nh++] = (unsigned char)m;
+      ++m;
+    }
+  G.ZT = m;
+  G.ZH = nh;
+  G.Z0 = (int)shells[0].size();
+  G.r0 = r0;
+  // S2: same-colour cells must not interact during a pass: 2w >= 2 r0 + R (w in conventional cells).
+  if (2 * w < 2 * r0 + R) return SMCX_E_LINK_CELL_TOO_SMALL;
+  G.H = (r0 + R + 1) / 2;
+  G.TW = w + 2 * G.H;
+  long long n_sites = G.B;
+  for (int a = 0; a < 3; ++a) {
+    const int L = p->dims[a];
+    if (L <= 0 || L % (2 * w) != 0 || L < G.TW) return SMCX_E_BAD_DIMS;
+    n_sites *= L;
+    if (n_sites > (1ll << 40)) return SMCX_E_BAD_DIMS;
+  }
+  G.Lx = p->dims[0]; G.Ly = p->dims[1]; G.Lz = p->dims[2];
+  G.ncx = G.Lx / w; G.ncy = G.Ly / w; G.ncz = G.Lz / w;
+  const long long n_cells = (long long)G.ncx * G.ncy * G.ncz;
+  if (n_cells > 0xffffffffll) return SMCX_E_BAD_DIMS;  // cell id is a 32-bit Philox counter word
+  G.cells_per_colour = (unsigned)(n_cells / 8);
+  G.S = w * w * w * G.B;
+  G.key0 = (uint32_t)(p->seed & 0xffffffffull);
+  G.key1 = (uint32_t)(p->seed >> 32);
+  G.accept_len = p->accept_len;
+  G.trace_capacity = p->trace_capacity > 0 ? p->trace_capacity : 65536;
+  // tile-linear deltas
+  for (int b = 0; b < G.B; ++b) {
+    int bp[3];
+    basis_pos(p->lattice, b, bp);
+    for (int k = 0; k < G.ZT; ++k) {
+      const int qx = bp[0] + G.off[k][0], qy = bp[1] + G.off[k][1], qz = bp[2] + G.off[k][2];
+      const int nb = basis_from_parity(p->lattice, qx, qy, qz);
+      const int dcx = floor_div2(qx), dcy = floor_div2(qy), dcz = floor_div2(qz);
+      const int d = ((dcz * G.TW + dcy) * G.TW + dcx) * G.B + (nb - b);
+      if (d < -32768 || d > 32767) return SMCX_E_LINK_CELL_TOO_SMALL;
+      G.delta[b][k] = (short)d;
+    }
+  }
+  plan->n_sites = n_sites;
+  plan->n_cells = n_cells;
+
+  // kernel / storage choice
+  const bool fast_ok = thread_kernel_supported(G);
+  int kernel = p->kernel, storage = p->storage;
+  if (kernel == SMCX_KERNEL_AUTO) {
+    if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_WARP_PER_CELL;
+    else kernel = fast_ok ? SMCX_KERNEL_THREAD_PER_CELL : SMCX_KERNEL_WARP_PER_CELL;
+  }
+  if (kernel == SMCX_KERNEL_THREAD_PER_CELL) {
+    if (!fast_ok) return SMCX_E_UNSUPPORTED;
+    if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_2BIT;
+    if (storage != SMCX_STORAGE_2BIT) return SMCX_E_UNSUPPORTED;
+  } else if (kernel == SMCX_KERNEL_WARP_PER_CELL) {
+    if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_U8;
+    if (storage != SMCX_STORAGE_U8) return SMCX_E_UNSUPPORTED;
+  } else {
+    return SMCX_E_UNSUPPORTED;
+  }
+  plan->kernel = kernel;
+  plan->storage = storage;
+
+  Layout& L = plan->lay;
+  size_t off = 0;
+  L.species = off;
+  off += align_up(storage == SMCX_STORAGE_U8 ? (size_t)n_sites : (size_t)((n_sites + 15) / 16) * 4, 256);
+  L.epi = off;     off += align_up((size_t)p->n_shells * n * n * sizeof(int32_t), 256);
+  L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
+  L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
+  L.state = off;   off += align_up(sizeof(DevState), 256);
+  L.counts = off;  off += align_up((size_t)kMaxShells * kMaxSpecies * kMaxSpecies * sizeof(unsigned long long), 256);
+  L.total = off;
+  return SMCX_OK;
+}
+
+}  // namespace
+
+struct smcx {
+  Plan plan;
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  char* ws = nullptr;
+  bool owns_ws = false;
+  std::vector<int32_t> epi;
+  int kT_units = 0;
+  uint32_t* staging[kStagingSlots] = {nullptr, nullptr, nullptr, nullptr};
+  cudaEvent_t staging_ev[kStagingSlots] = {nullptr, nullptr, nullptr, nullptr};
+  size_t staging_cap = 0;
+  int staging_next = 0;
+  uint8_t* bounce = nullptr;  // device, kChunkSites bytes, lazily allocated
+  long long sweeps_enqueued = 0;
+  long long launches = 0;
+  int sm_count = 148;
+  std::string err;
+
+  uint8_t* d_species() const { return reinterpret_cast<uint8_t*>(ws + plan.lay.species); }
+  int32_t* d_epi() const { return reinterpret_cast<int32_t*>(ws + plan.lay.epi); }
+  uint32_t* d_accept() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.accept); }
+  long long* d_trace() const { return reinterpret_cast<long long*>(ws + plan.lay.trace); }
+  DevState* d_state() const { return reinterpret_cast<DevState*>(ws + plan.lay.state); }
+  unsigned long long* d_counts() const { return reinterpret_cast<unsigned long long*>(ws + plan.lay.counts); }
+};
+
+namespace {
+
+#define SMCX_CUDA(h, call)                                                        \
+  do {                                                                            \
+    cudaError_t e_ = (call);                                                      \
+    if (e_ != cudaSuccess) {                                                      \
+      (h)->err = std::string(#call) + ": " + cudaGetErrorString(e_);              \
+      return SMCX_E_CUDA;                                                         \
+    }                                                                             \
+  } while (0)
+
+int grid_for(const smcx* h, long long work_items, int block) {
+  const long long want = (work_items + block - 1) / block;
+  const long long cap = (long long)h->sm_count * 16;
+  return (int)std::max(1ll, std::min(want, cap));
+}
+
+int launch_init(smcx* h) {
+  const Plan& P = h->plan;
+  int hh = 1;
+  while ((1ull << (2 * hh)) < (unsigned long long)P.n_sites) ++hh;
+  const int grid = grid_for(h, (P.n_sites + 15) / 16, 256);
+  if (P.storage == SMCX_STORAGE_U8)
+    init_species_kernel<StoreU8><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh, P.G.key0, P.G.key1);
+  else
+    init_species_kernel<Store2><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh, P.G.key0, P.G.key1);
+  h->launches++;
+  SMCX_CUDA(h, cudaGetLastError());
+  return SMCX_OK;
+}
+
+// Runs the pair-count reduction and leaves M[s][x][y] (positive-half counts) in host_M.
+int run_pair_counts(smcx* h, std::vector<unsigned long long>& host_M) {
+  const Plan& P = h->plan;
+  const Geom& G = P.G;
+  const int n_hist = G.n_shells * G.n_species * G.n_species;
+  zero_u64_kernel<<<1, 256, 0, h->stream>>>(h->d_counts(), n_hist);
+  h->launches++;
+  const long long n_conv = (long long)G.Lx * G.Ly * G.Lz;
+  const int grid = grid_for(h, n_conv, 256);
+  const size_t sm = (size_t)n_hist * sizeof(unsigned);
+  if (P.storage == SMCX_STORAGE_U8) {
+    if (G.B == 2) pair_count_kernel<StoreU8, 2><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
+    else          pair_count_kernel<StoreU8, 4><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
+  } else {
+    if (G.B == 2) pair_count_kernel<Store2, 2><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
+    else          pair_count_kernel<Store2, 4><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
+  }
+  h->launches++;
+  SMCX_CUDA(h, cudaGetLastError());
+  host_M.assign((size_t)n_hist, 0ull);
+  SMCX_CUDA(h, cudaMemcpyAsync(host_M.data(), h->d_counts(), (size_t)n_hist * sizeof(unsigned long long),
+                               cudaMemcpyDeviceToHost, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  return SMCX_OK;
+}
+
+long long energy_from_counts(const smcx* h, const std::vector<unsigned long long>& M) {
+  const Geom& G = h->plan.G;
+  const int n = G.n_species;
+  long long E = 0;
+  for (int s = 0; s < G.n_shells; ++s)
+    for (int a = 0; a < n; ++a)
+      for (int b = 0; b < n; ++b)
+        E += (long long)h->epi[(size_t)(s * n + a) * n + b] * (long long)M[(size_t)(s * n + a) * n + b];
+  return E;
+}
+
+// Recompute H from the lattice and store it as the running energy.
+int reset_running_energy(smcx* h) {
+  std::vector<unsigned long long> M;
+  const int rc = run_pair_counts(h, M);
+  if (rc != SMCX_OK) return rc;
+  const long long E = energy_from_counts(h, M);
+  SMCX_CUDA(h, cudaMemcpyAsync(&h->d_state()->e_run, &E, sizeof(E), cudaMemcpyHostToDevice, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  return SMCX_OK;
+}
+
+int upload_table(smcx* h, const uint32_t* accept, int len) {
+  if (!accept || len < 1 || len > kAcceptCapacity) return SMCX_E_BAD_TABLE;
+  const int slot = h->staging_next;
+  h->staging_next = (slot + 1) % kStagingSlots;
+  SMCX_CUDA(h, cudaEventSynchronize(h->staging_ev[slot]));
+  std::memcpy(h->staging[slot], accept, (size_t)len * sizeof(uint32_t));
+  SMCX_CUDA(h, cudaMemcpyAsync(h->d_accept(), h->staging[slot], (size_t)len * sizeof(uint32_t),
+                               cudaMemcpyHostToDevice, h->stream));
+  SMCX_CUDA(h, cudaEventRecord(h->staging_ev[slot], h->stream));
+  h->plan.G.accept_len = len;
+  return SMCX_OK;
+}
+
+int ensure_bounce(smcx* h) {
+  if (!h->bounce) SMCX_CUDA(h, cudaMalloc(&h->bounce, (size_t)kChunkSites));
+  return SMCX_OK;
+}
+
+int launch_colour_pass(smcx* h, int colour) {
+  const Plan& P = h->plan;
+  const Geom& G = P.G;
+  if (P.kernel == SMCX_KERNEL_THREAD_PER_CELL) {
+    const int rc = launch_thread_per_cell(G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_epi(), h->d_accept(),
+                                          h->d_state(), colour, h->stream);
+    h->launches++;
+    if (rc != 0) { h->err = "thread-per-cell launch failed"; return SMCX_E_CUDA; }
+    return SMCX_OK;
+  }
+  const int n2 = G.n_species * G.n_species;
+  const int tables = (G.n_shells * n2 * 4 + G.B * G.ZT * 2 + G.ZT + 15) & ~15;
+  const int tile = (G.TW * G.TW * G.TW * G.B + 15) & ~15;
+  const size_t sm = (size_t)tables + (size_t)kWarpsPerBlock * tile;
+  const unsigned grid = (G.cells_per_colour + kWarpsPerBlock - 1) / kWarpsPerBlock;
+  if (G.B == 2)
+    sweep_warp_per_cell<2><<<grid, kWarpsPerBlock * 32, sm, h->stream>>>(G, h->d_species(), h->d_epi(), h->d_accept(), h->d_state(), colour);
+  else
+    sweep_warp_per_cell<4><<<grid, kWarpsPerBlock * 32, sm, h->stream>>>(G, h->d_species(), h->d_epi(), h->d_accept(), h->d_state(), colour);
+  h->launches++;
+  return SMCX_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* smcx_version(void) { return "smcx-b200 0.1 (sm_100a)"; }
+
+const char* smcx_strerror(int code) {
+  switch (code) {
+    case SMCX_OK: return "ok";
+    case SMCX_E_NULL_ARG: return "null argument";
+    case SMCX_E_BAD_LATTICE: return "lattice must be SMCX_BCC or SMCX_FCC";
+    case SMCX_E_BAD_DIMS: return "dims must be positive, divisible by 2*link_cell, at least link_cell+2*halo, and small enough";
+    case SMCX_E_BAD_SPECIES: return "n_species must be in 2..16";
+    case SMCX_E_BAD_SHELLS: return "n_shells must be in 1..5";
+    case SMCX_E_EPI_NOT_SYMMETRIC: return "EPI table is not symmetric";
+    case SMCX_E_LINK_CELL_TOO_SMALL: return "link cell violates 2w >= 2 r0 + R (or is out of range)";
+    case SMCX_E_BAD_TABLE: return "acceptance table missing, empty or too long";
+    case SMCX_E_BAD_STATE: return "species value >= n_species";
+    case SMCX_E_NO_MEMORY: return "out of memory or workspace too small";
+    case SMCX_E_CUDA: return "CUDA error (see smcx_last_error)";
+    case SMCX_E_UNSUPPORTED: return "storage/kernel choice not valid for these parameters";
+    case SMCX_E_RANGE: return "range not available";
+    default: return "unknown error";
+  }
+}
+
+const char* smcx_last_error(smcx_t* h) { return h ? h->err.c_str() : "null handle"; }
+
+int smcx_workspace_bytes(const smcx_params_t* p, size_t* bytes) {
+  if (!p || !bytes) return SMCX_E_NULL_ARG;
+  Plan plan;
+  const int rc = make_plan(p, &plan);
+  if (rc != SMCX_OK) return rc;
+  *bytes = plan.lay.total;
+  return SMCX_OK;
+}
+
+int smcx_create(smcx_t** out, const smcx_params_t* p) {
+  if (!out || !p) return SMCX_E_NULL_ARG;
+  smcx* h = new (std::nothrow) smcx();
+  if (!h) return SMCX_E_NO_MEMORY;
+  int rc = make_plan(p, &h->plan);
+  if (rc != SMCX_OK) { delete h; return rc; }
+  h->device = p->device;
+  h->stream = reinterpret_cast<cudaStream_t>(p->stream);
+  h->kT_units = p->kT_units;
+  const int n = p->n_species;
+  h->epi.assign(p->epi, p->epi + (size_t)p->n_shells * n * n);
+
+  auto fail = [&](int code) { smcx_destroy(h); return code; };
+  int n_dev = 0;
+  if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev <= 0 || p->device < 0 || p->device >= n_dev) {
+    cudaGetLastError();
+    return fail(SMCX_E_CUDA);
+  }
+  if (cudaSetDevice(p->device) != cudaSuccess) return fail(SMCX_E_CUDA);
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) return fail(SMCX_E_CUDA);
+  h->sm_count = prop.multiProcessorCount;
+
+  if (p->d_workspace) {
+    if (p->workspace_bytes < h->plan.lay.total) return fail(SMCX_E_NO_MEMORY);
+    h->ws = reinterpret_cast<char*>(p->d_workspace);
+  } else {
+    void* ws = nullptr;
+    if (cudaMalloc(&ws, h->plan.lay.total) != cudaSuccess) { cudaGetLastError(); return fail(SMCX_E_NO_MEMORY); }
+    h->ws = reinterpret_cast<char*>(ws);
+    h->owns_ws = true;
+  }
+  h->staging_cap = (size_t)kAcceptCapacity * sizeof(uint32_t);
+  for (int s = 0; s < kStagingSlots; ++s) {
+    if (cudaMallocHost(reinterpret_cast<void**>(&h->staging[s]), h->staging_cap) != cudaSuccess) return fail(SMCX_E_NO_MEMORY);
+    if (cudaEventCreateWithFlags(&h->staging_ev[s], cudaEventDisableTiming) != cudaSuccess) return fail(SMCX_E_CUDA);
+  }
+  if (configure_thread_per_cell() != 0) return fail(SMCX_E_CUDA);
+  {
+    const Geom& G = h->plan.G;
+    const int n2 = G.n_species * G.n_species;
+    const size_t sm = (size_t)((G.n_shells * n2 * 4 + G.B * G.ZT * 2 + G.ZT + 15) & ~15) +
+                      (size_t)kWarpsPerBlock * ((G.TW * G.TW * G.TW * G.B + 15) & ~15);
+    if (h->plan.kernel == SMCX_KERNEL_WARP_PER_CELL) {
+      if (sm > 227 * 1024) return fail(SMCX_E_LINK_CELL_TOO_SMALL);
+      cudaError_t e = G.B == 2
+          ? cudaFuncSetAttribute(sweep_warp_per_cell<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm)
+          : cudaFuncSetAttribute(sweep_warp_per_cell<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sm);
+      if (e != cudaSuccess) { h->err = cudaGetErrorString(e); return fail(SMCX_E_CUDA); }
+    }
+  }
+
+  rc = [&]() -> int {
+    DevState zero{};
+    SMCX_CUDA(h, cudaMemcpyAsync(h->d_state(), &zero, sizeof(zero), cudaMemcpyHostToDevice, h->stream));
+    SMCX_CUDA(h, cudaMemcpyAsync(h->d_epi(), h->epi.data(), h->epi.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+    SMCX_CUDA(h, cudaMemsetAsync(h->d_trace(), 0, (size_t)h->plan.G.trace_capacity * sizeof(long long), h->stream));
+    SMCX_CUDA(h, cudaStreamSynchronize(h->stream));  // &zero and epi must stay valid until copied
+    int r = upload_table(h, p->accept, p->accept_len);
+    if (r != SMCX_OK) return r;
+    r = launch_init(h);
+    if (r != SMCX_OK) return r;
+    return reset_running_energy(h);
+  }();
+  if (rc != SMCX_OK) return fail(rc);
+  *out = h;
+  return SMCX_OK;
+}
+
+void smcx_destroy(smcx_t* h) {
+  if (!h) return;
+  if (h->stream || h->ws) cudaStreamSynchronize(h->stream);
+  for (int s = 0; s < kStagingSlots; ++s) {
+    if (h->staging[s]) cudaFreeHost(h->staging[s]);
+    if (h->staging_ev[s]) cudaEventDestroy(h->staging_ev[s]);
+  }
+  if (h->bounce) cudaFree(h->bounce);
+  if (h->owns_ws && h->ws) cudaFree(h->ws);
+  cudaGetLastError();
+  delete h;
+}
+
+int smcx_set_species_device(smcx_t* h, const void* d_src) {
+  if (!h || !d_src) return SMCX_E_NULL_ARG;
+  const Plan& P = h->plan;
+  const uint8_t* src = reinterpret_cast<const uint8_t*>(d_src);
+  unsigned long long zero = 0;
+  SMCX_CUDA(h, cudaMemcpyAsync(&h->d_state()->bad_state, &zero, sizeof(zero), cudaMemcpyHostToDevice, h->stream));
+  validate_u8_kernel<<<grid_for(h, P.n_sites, 256), 256, 0, h->stream>>>(src, P.n_sites, P.G.n_species, h->d_state());
+  h->launches++;
+  unsigned long long bad = 0;
+  SMCX_CUDA(h, cudaMemcpyAsync(&bad, &h->d_state()->bad_state, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  if (bad) return SMCX_E_BAD_STATE;
+  if (P.storage == SMCX_STORAGE_U8) {
+    SMCX_CUDA(h, cudaMemcpyAsync(h->d_species(), src, (size_t)P.n_sites, cudaMemcpyDeviceToDevice, h->stream));
+  } else {
+    pack2_kernel<<<grid_for(h, (P.n_sites + 15) / 16, 256), 256, 0, h->stream>>>(src, reinterpret_cast<uint32_t*>(h->d_species()), 0, P.n_sites);
+    h->launches++;
+    SMCX_CUDA(h, cudaGetLastError());
+  }
+  return reset_running_energy(h);
+}
+
+int smcx_set_species(smcx_t* h, const uint8_t* host_src) {
+  if (!h || !host_src) return SMCX_E_NULL_ARG;
+  const Plan& P = h->plan;
+  for (long long i = 0; i < P.n_sites; ++i)
+    if (host_src[i] >= P.G.n_species) return SMCX_E_BAD_STATE;
+  if (P.storage == SMCX_STORAGE_U8) {
+    SMCX_CUDA(h, cudaMemcpyAsync(h->d_species(), host_src, (size_t)P.n_sites, cudaMemcpyHostToDevice, h->stream));
+  } else {
+    int rc = ensure_bounce(h);
+    if (rc != SMCX_OK) return rc;
+    for (long long first = 0; first < P.n_sites; first += kChunkSites) {
+      const long long cnt = std::min(kChunkSites, P.n_sites - first);
+      SMCX_CUDA(h, cudaMemcpyAsync(h->bounce, host_src + first, (size_t)cnt, cudaMemcpyHostToDevice, h->stream));
+      pack2_kernel<<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(h->bounce, reinterpret_cast<uint32_t*>(h->d_species()), first, cnt);
+      h->launches++;
+      SMCX_CUDA(h, cudaGetLastError());
+    }
+  }
+  return reset_running_energy(h);
+}
+
+int smcx_set_temperature(smcx_t* h, int32_t kT_units, const uint32_t* accept, int32_t accept_len) {
+  if (!h) return SMCX_E_NULL_ARG;
+  const int rc = upload_table(h, accept, accept_len);
+  if (rc == SMCX_OK) h->kT_units = kT_units;
+  return rc;
+}
+
+int smcx_sweep(smcx_t* h, int64_t n) {
+  if (!h) return SMCX_E_NULL_ARG;
+  if (n < 0 || h->sweeps_enqueued + n > 0xffffffffll) return SMCX_E_RANGE;  // t is a 32-bit counter word
+  for (int64_t s = 0; s < n; ++s) {
+    for (int colour = 0; colour < 8; ++colour) {
+      const int rc = launch_colour_pass(h, colour);
+      if (rc != SMCX_OK) return rc;
+    }
+    sweep_epilogue<<<1, 1, 0, h->stream>>>(h->d_state(), h->d_trace(), h->plan.G.trace_capacity);
+    h->launches++;
+    h->sweeps_enqueued++;
+  }
+  SMCX_CUDA(h, cudaGetLastError());
+  return SMCX_OK;
+}
+
+int smcx_synchronize(smcx_t* h) {
+  if (!h) return SMCX_E_NULL_ARG;
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  return SMCX_OK;
+}
+
+int smcx_energy(smcx_t* h, int64_t* E) {
+  if (!h || !E) return SMCX_E_NULL_ARG;
+  std::vector<unsigned long long> M;
+  const int rc = run_pair_counts(h, M);
+  if (rc != SMCX_OK) return rc;
+  *E = energy_from_counts(h, M);
+  return SMCX_OK;
+}
+
+int smcx_running_energy(smcx_t* h, int64_t* E) {
+  if (!h || !E) return SMCX_E_NULL_ARG;
+  long long e = 0;
+  SMCX_CUDA(h, cudaMemcpyAsync(&e, &h->d_state()->e_run, sizeof(e), cudaMemcpyDeviceToHost, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  *E = e;
+  return SMCX_OK;
+}
+
+int smcx_energy_trace(smcx_t* h, int64_t first_sweep, int64_t count, int64_t* dst) {
+  if (!h || (!dst && count > 0)) return SMCX_E_NULL_ARG;
+  const long long cap = h->plan.G.trace_capacity;
+  if (first_sweep < 0 || count < 0 || first_sweep + count > h->sweeps_enqueued ||
+      h->sweeps_enqueued - first_sweep > cap)
+    return SMCX_E_RANGE;
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  int64_t done = 0;
+  while (done < count) {
+    const long long pos = (first_sweep + done) % cap;
+    const long long run = std::min<long long>(count - done, cap - pos);
+    SMCX_CUDA(h, cudaMemcpy(dst + done, h->d_trace() + pos, (size_t)run * sizeof(long long), cudaMemcpyDeviceToHost));
+    done += run;
+  }
+  return SMCX_OK;
+}
+
+int smcx_species_device(smcx_t* h, void* d_dst) {
+  if (!h || !d_dst) return SMCX_E_NULL_ARG;
+  const Plan& P = h->plan;
+  if (P.storage == SMCX_STORAGE_U8) {
+    SMCX_CUDA(h, cudaMemcpyAsync(d_dst, h->d_species(), (size_t)P.n_sites, cudaMemcpyDeviceToDevice, h->stream));
+  } else {
+    unpack2_kernel<<<grid_for(h, (P.n_sites + 15) / 16, 256), 256, 0, h->stream>>>(
+        reinterpret_cast<const uint32_t*>(h->d_species()), reinterpret_cast<uint8_t*>(d_dst), 0, P.n_sites);
+    h->launches++;
+    SMCX_CUDA(h, cudaGetLastError());
+  }
+  return SMCX_OK;
+}
+
+int smcx_species(smcx_t* h, uint8_t* host_dst) {
+  if (!h || !host_dst) return SMCX_E_NULL_ARG;
+  const Plan& P = h->plan;
+  if (P.storage == SMCX_STORAGE_U8) {
+    SMCX_CUDA(h, cudaMemcpyAsync(host_dst, h->d_species(), (size_t)P.n_sites, cudaMemcpyDeviceToHost, h->stream));
+    SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+    return SMCX_OK;
+  }
+  int rc = ensure_bounce(h);
+  if (rc != SMCX_OK) return rc;
+  for (long long first = 0; first < P.n_sites; first += kChunkSites) {
+    const long long cnt = std::min(kChunkSites, P.n_sites - first);
+    unpack2_kernel<<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(
+        reinterpret_cast<const uint32_t*>(h->d_species()), h->bounce, first, cnt);
+    h->launches++;
+    SMCX_CUDA(h, cudaGetLastError());
+    SMCX_CUDA(h, cudaMemcpyAsync(host_dst + first, h->bounce, (size_t)cnt, cudaMemcpyDeviceToHost, h->stream));
+    SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  }
+  return SMCX_OK;
+}
+
+int smcx_sro(smcx_t* h, double* alpha, int64_t* pair_counts) {
+  if (!h || !alpha) return SMCX_E_NULL_ARG;
+  std::vector<unsigned long long> M;
+  const int rc = run_pair_counts(h, M);
+  if (rc != SMCX_OK) return rc;
+  const Geom& G = h->plan.G;
+  const int n = G.n_species;
+  std::vector<int> Z(G.n_shells, 0);
+  for (int m = 0; m < G.ZT; ++m) Z[G.shell_of[m]]++;
+  // ordered counts N_s(p',p) = M_s(p',p) + M_s(p,p'); species counts from the row sums of shell 0
+  std::vector<long long> Ns((size_t)G.n_shells * n * n);
+  for (int s = 0; s < G.n_shells; ++s)
+    for (int a = 0; a < n; ++a)
+      for (int b = 0; b < n; ++b)
+        Ns[(size_t)(s * n + a) * n + b] = (long long)(M[(size_t)(s * n + a) * n + b] + M[(size_t)(s * n + b) * n + a]);
+  std::vector<long long> n_of(n, 0);
+  for (int a = 0; a < n; ++a) {
+    long long row = 0;
+    for (int b = 0; b < n; ++b) row += Ns[(size_t)a * n + b];
+    n_of[a] = row / Z[0];
+  }
+  const double N = (double)h->plan.n_sites;
+  for (int s = 0; s < G.n_shells; ++s)
+    for (int a = 0; a < n; ++a)
+      for (int b = 0; b < n; ++b) {
+        const size_t idx = (size_t)(s * n + a) * n + b;
+        if (n_of[a] == 0 || n_of[b] == 0) { alpha[idx] = std::numeric_limits<double>::quiet_NaN(); continue; }
+        // Eq. 8: alpha = 1 - P(p|p')/c_p, P = N_s(p',p)/(Z_s n_p'), c_p = n_p/N
+        const double P = (double)Ns[idx] / ((double)Z[s] * (double)n_of[a]);
+        const double c = (double)n_of[b] / N;
+        alpha[idx] = 1.0 - P / c;
+      }
+  if (pair_counts) std::memcpy(pair_counts, Ns.data(), Ns.size() * sizeof(long long));
+  return SMCX_OK;
+}
+
+int smcx_stats(smcx_t* h, int64_t* sweeps_done, int64_t* trials, int64_t* accepted) {
+  if (!h) return SMCX_E_NULL_ARG;
+  DevState st;
+  SMCX_CUDA(h, cudaMemcpyAsync(&st, h->d_state(), sizeof(st), cudaMemcpyDeviceToHost, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  if (sweeps_done) *sweeps_done = (int64_t)st.sweep;
+  if (trials) *trials = (int64_t)st.sweep * h->plan.n_sites;
+  if (accepted) *accepted = (int64_t)st.accepted;
+  return SMCX_OK;
+}
+
+int smcx_shell_offsets(smcx_t* h, int32_t shell, int32_t* xyz, int32_t max_offsets, int32_t* n_offsets) {
+  if (!h || !n_offsets) return SMCX_E_NULL_ARG;
+  const Geom& G = h->plan.G;
+  if (shell < 0 || shell >= G.n_shells) return SMCX_E_BAD_SHELLS;
+  int k = 0;
+  for (int m = 0; m < G.ZT; ++m)
+    if (G.shell_of[m] == shell) {
+      if (xyz && k < max_offsets) { xyz[3 * k] = G.off[m][0]; xyz[3 * k + 1] = G.off[m][1]; xyz[3 * k + 2] = G.off[m][2]; }
+      ++k;
+    }
+  *n_offsets = k;
+  return SMCX_OK;
+}
+
+int smcx_get_config(smcx_t* h, int32_t* storage, int32_t* kernel, int64_t* n_sites, int64_t* n_cells) {
+  if (!h) return SMCX_E_NULL_ARG;
+  if (storage) *storage = h->plan.storage;
+  if (kernel) *kernel = h->plan.kernel;
+  if (n_sites) *n_sites = h->plan.n_sites;
+  if (n_cells) *n_cells = h->plan.n_cells;
+  return SMCX_OK;
+}
+
+int64_t smcx_kernel_launches(smcx_t* h) { return h ? h->launches : 0; }
+
+}  // extern "C"

@@ -1,0 +1,90 @@
+// Shared device-side definitions of the SMC-X CUDA path (sm_100a).
+// Independent of oracle/: its own Philox, geometry tables and schedule arithmetic.
+#pragma once
+#include <cstdint>
+#include <cuda_runtime.h>
+
+namespace smcxk {
+
+// Counter tags (low byte of ctr[3]), S4.
+enum : uint32_t { TAG_SHIFT = 1u, TAG_TRIAL = 2u, TAG_INIT = 3u };
+
+constexpr int kMaxShells = 5;
+constexpr int kMaxNeighbours = 80;  // FCC, 5 shells: 12+6+24+12+24 = 78
+constexpr int kMaxSpecies = 16;
+
+// Philox4x32-10 (Salmon et al., SC'11).  Round keys are recomputed from the key each call; the
+// additions fold into immediates when the key is a kernel parameter.
+__host__ __device__ __forceinline__ void philox_round(uint32_t& c0, uint32_t& c1, uint32_t& c2,
+                                                      uint32_t& c3, uint32_t k0, uint32_t k1) {
+#ifdef __CUDA_ARCH__
+  const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
+  const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
+#else
+  const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+  const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
+  const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
+#endif
+  const uint32_t n0 = hi1 ^ c1 ^ k0;
+  const uint32_t n2 = hi0 ^ c3 ^ k1;
+  c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
+}
+
+struct Philox4 { uint32_t x, y, z, w; };
+
+__host__ __device__ __forceinline__ Philox4 philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2,
+                                                          uint32_t c3, uint32_t k0, uint32_t k1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) {
+    philox_round(c0, c1, c2, c3, k0, k1);
+    k0 += 0x9E3779B9u;
+    k1 += 0xBB67AE85u;
+  }
+  return Philox4{c0, c1, c2, c3};
+}
+
+__host__ __device__ __forceinline__ uint32_t mulhi_u32(uint32_t a, uint32_t b) {
+#ifdef __CUDA_ARCH__
+  return __umulhi(a, b);
+#else
+  return (uint32_t)(((uint64_t)a * b) >> 32);
+#endif
+}
+
+// Device-resident bookkeeping, one per handle.
+struct DevState {
+  unsigned long long sweep;      // sweeps completed
+  long long e_run;               // running energy E_0 + sum of accepted dE
+  unsigned long long accepted;   // accepted swaps
+  unsigned long long bad_state;  // set by validation kernels
+};
+
+// Lattice + link-cell geometry and the shell-offset tables.  Passed to kernels by value, i.e. it
+// lives in the constant bank (the "shell-offset table in constant memory").
+struct Geom {
+  int Lx, Ly, Lz;      // conventional cells
+  int B;               // sites per conventional cell (2 BCC, 4 FCC)
+  int lattice;
+  int n_species, n_shells;
+  int w;               // link-cell edge (conventional cells)
+  int H;               // halo (conventional cells) = ceil((r0 + R)/2)
+  int TW;              // tile edge = w + 2H
+  int r0;              // per-axis reach of shell 0 (half-lattice units)
+  int ncx, ncy, ncz;   // link cells per axis
+  unsigned cells_per_colour;
+  int S;               // trials per cell = w^3 B
+  int Z0;              // coordination number of shell 0
+  int ZT;              // neighbours over all shells
+  int ZH;              // positive-half offsets over all shells (ZT/2)
+  uint32_t key0, key1; // Philox key = seed
+  int accept_len;
+  int trace_capacity;
+  // all shells concatenated, shell by shell, each in ascending (dz,dy,dx) order
+  signed char off[kMaxNeighbours][3];   // half-lattice units
+  unsigned char shell_of[kMaxNeighbours];
+  unsigned char half_idx[kMaxNeighbours / 2];  // indices (into off) of the positive half
+  // tile-linear index delta of neighbour m for a site with basis index b, and its basis index
+  short delta[4][kMaxNeighbours];
+};
+
+}  // namespace smcxk

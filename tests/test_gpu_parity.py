@@ -1,0 +1,256 @@
+"""GPU-vs-oracle parity through the C ABI (pytest -m gpu): species arrays, energy traces and pair
+counts bit-exact, fp64 SRO within 1e-9 relative (BASELINE.json north_star)."""
+import os
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_2509_20949_b200 as smcx
+from smcx_inputs import get_config, make_accept_table, make_epi, scaled_config
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_THREAD_PER_CELL]
+
+
+def _supported(cfg, kernel):
+    if kernel == smcx.KERNEL_WARP_PER_CELL:
+        return True
+    return cfg.lattice == 0 and cfg.n_shells == 2 and cfg.link_cell == 4 and cfg.n_species <= 4
+
+
+def _pair(cfg, kernel=smcx.KERNEL_AUTO, **over):
+    g = smcx.Lattice.from_config(cfg, kernel=kernel, **over)
+    o = oracle.Oracle.from_config(cfg, **{k: v for k, v in over.items() if k in ("seed", "link_cell")})
+    return g, o
+
+
+def _assert_same_state(g, o):
+    gs, os_ = g.species(), o.species()
+    assert gs.dtype == np.uint8 and gs.shape == os_.shape
+    bad = np.flatnonzero(gs != os_)
+    assert bad.size == 0, f"{bad.size} sites differ, first at {bad[:5]}"
+
+
+def _assert_sro(g, o):
+    ga, gc = g.sro()
+    oa, oc = o.sro()
+    assert (gc == oc).all()
+    assert np.allclose(ga, oa, rtol=1e-9, atol=1e-9, equal_nan=True)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+def test_config1_full_run_species_after_every_sweep(kernel):
+    cfg = get_config(1)
+    g, o = _pair(cfg, kernel)
+    _assert_same_state(g, o)                       # S6 initial state
+    assert g.energy() == o.energy() == g.running_energy()
+    for t in range(cfg.n_sweeps):
+        g.sweep(1)
+        o.sweep(1)
+        _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.stats() == o.stats()
+    assert g.energy() == o.energy() == o.running_energy() == g.running_energy()
+    _assert_sro(g, o)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+def test_config2_anneal_prefix(kernel):
+    """Config 2 with its per-sweep temperature table; SRO sampled every 10 sweeps here
+    (every 100 over the full 2,000 in the slow test)."""
+    cfg = get_config(2)
+    n = 30
+    g, o = _pair(cfg, kernel)
+    _assert_sro(g, o)
+    for t in range(n):
+        table = cfg.accept_table(t)
+        g.set_temperature(cfg.kT_at(t), table)
+        o.set_temperature(table)
+        g.sweep(1)
+        o.sweep(1)
+        if (t + 1) % 10 == 0:
+            _assert_same_state(g, o)
+            _assert_sro(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.stats() == o.stats()
+
+
+@pytest.mark.slow
+def test_config2_anneal_full_length():
+    cfg = get_config(2)
+    g, o = _pair(cfg)
+    for t in range(cfg.n_sweeps):
+        table = cfg.accept_table(t)
+        g.set_temperature(cfg.kT_at(t), table)
+        o.set_temperature(table)
+        g.sweep(1)
+        o.sweep(1)
+        if (t + 1) % cfg.sro_every == 0:
+            _assert_same_state(g, o)
+            _assert_sro(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+
+
+def test_config3_fcc_five_species_prefix():
+    cfg = get_config(3)
+    g, o = _pair(cfg)
+    _assert_same_state(g, o)
+    g.sweep(2)
+    o.sweep(2)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.energy() == o.energy()
+    _assert_sro(g, o)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+def test_config4_shape_ragged_grid(kernel):
+    """Config 4's species/EPI/kT on a non-cubic lattice whose cells per colour (13*11*9) fill
+    neither a warp nor a block evenly."""
+    cfg = scaled_config(4, (104, 88, 72))
+    g, o = _pair(cfg, kernel)
+    g.sweep(3)
+    o.sweep(3)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.stats() == o.stats()
+    _assert_sro(g, o)
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+def test_config4_full_size_invariants(kernel):
+    """BCC 800^3 in the launch configuration bench.py times: conservation (P5), energy bookkeeping
+    (P6: H recomputed by the reduction kernel == E0 + sum of accepted dE) and the species counts."""
+    cfg = get_config(4)
+    g = smcx.Lattice.from_config(cfg, kernel=kernel)
+    _, c0 = g.sro()
+    n_p = c0[0].sum(axis=1) // 8
+    assert (n_p == cfg.n_sites // 4).all()
+    e0 = g.energy()
+    assert e0 == g.running_energy()
+    g.sweep(2)
+    _, c1 = g.sro()
+    assert (c1[0].sum(axis=1) // 8 == n_p).all()
+    assert (c1 == c1.transpose(0, 2, 1)).all()
+    assert g.energy() == g.running_energy() == g.energy_trace()[-1]
+    sweeps, trials, accepted = g.stats()
+    assert sweeps == 2 and trials == 2 * cfg.n_sites and 0 < accepted < trials
+    # P13: H = 1/2 sum V N
+    assert int((cfg.epi().astype(np.int64) * c1).sum()) == 2 * g.energy()
+
+
+@pytest.mark.slow
+@pytest.mark.parametrize("k,n", [(4, 1), (3, 20)])
+def test_full_size_oracle_prefix(k, n):
+    cfg = get_config(k)
+    g, o = _pair(cfg)
+    g.sweep(n)
+    o.sweep(n)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+def test_resume_and_determinism(kernel):
+    cfg = scaled_config(1, (24, 16, 32))
+    a = smcx.Lattice.from_config(cfg, kernel=kernel)
+    b = smcx.Lattice.from_config(cfg, kernel=kernel)
+    a.sweep(7)
+    b.sweep(3)
+    b.sweep(4)
+    assert (a.species() == b.species()).all() and (a.energy_trace() == b.energy_trace()).all()
+    c = smcx.Lattice.from_config(cfg, kernel=kernel, seed=cfg.seed + 1)
+    c.sweep(7)
+    assert (a.species() != c.species()).any()
+
+
+def test_thread_and_warp_kernels_agree():
+    """P14: uint8/warp-per-cell and 2-bit/thread-per-cell agree bit for bit."""
+    cfg = scaled_config(2, (40, 48, 56), n_sweeps=5)
+    a = smcx.Lattice.from_config(cfg, kernel=smcx.KERNEL_WARP_PER_CELL)
+    b = smcx.Lattice.from_config(cfg, kernel=smcx.KERNEL_THREAD_PER_CELL)
+    assert (a.storage, b.storage) == (smcx.STORAGE_U8, smcx.STORAGE_2BIT)
+    a.sweep(5)
+    b.sweep(5)
+    assert (a.species() == b.species()).all()
+    assert (a.energy_trace() == b.energy_trace()).all()
+    assert (a.sro()[1] == b.sro()[1]).all()
+
+
+@pytest.mark.parametrize("lat,dims,n_sp,n_shells,w", [
+    (0, (8, 8, 8), 2, 1, 4),       # one cell per colour, NN only
+    (0, (8, 16, 8), 3, 2, 2),      # smallest link cell the bound allows
+    (0, (16, 24, 16), 4, 4, 4),    # four shells (reach 3)
+    (0, (12, 12, 24), 4, 3, 3),    # odd link cell
+    (1, (8, 8, 8), 2, 1, 2),       # FCC nearest neighbours
+    (1, (16, 8, 8), 5, 3, 4),      # FCC three shells
+    (1, (16, 16, 16), 16, 2, 4),   # maximum species count
+])
+def test_edge_geometries(lat, dims, n_sp, n_shells, w):
+    amplitude, kT, seed = 350, 500, 4711
+    epi = make_epi(n_shells, n_sp, amplitude, seed)
+    table = make_accept_table(kT)
+    g = smcx.Lattice(lat, dims, n_sp, n_shells, epi, table, seed, link_cell=w, kT_units=kT)
+    o = oracle.Oracle(lat, dims, n_sp, n_shells, epi, w, table, seed)
+    assert o.lc_valid()
+    for s in range(n_shells):
+        assert (g.shell_offsets(s) == oracle.shell(lat, s)).all()
+    _assert_same_state(g, o)
+    g.sweep(4)
+    o.sweep(4)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    _assert_sro(g, o)
+
+
+def test_set_species_roundtrip_and_validation():
+    cfg = scaled_config(1, (16, 16, 16))
+    g, o = _pair(cfg)
+    rng = np.random.default_rng(3)
+    s = rng.integers(0, cfg.n_species, cfg.n_sites).astype(np.uint8)
+    g.set_species(s)
+    o.set_species(s)
+    assert (g.species() == s).all()
+    assert g.energy() == o.energy() == g.running_energy()
+    g.sweep(2)
+    o.sweep(2)
+    _assert_same_state(g, o)
+    s[5] = cfg.n_species
+    with pytest.raises(smcx.SmcxError) as ei:
+        g.set_species(s)
+    assert ei.value.code == -9
+    import torch
+    t = torch.from_numpy(o.species()).cuda()
+    g.set_species_device(t)
+    assert (g.species_device().cpu().numpy() == o.species()).all()
+    t[7] = 200
+    with pytest.raises(smcx.SmcxError):
+        g.set_species_device(t)
+
+
+def test_b2_state_sro_and_energy_closed_forms():
+    """Closed forms straight through the GPU reduction kernel: B2 energy and alpha = -1/+1."""
+    epi = make_epi(2, 2, 300, 5)
+    g = smcx.Lattice(0, (16, 16, 16), 2, 2, epi, make_accept_table(600), 1)
+    N = g.n_sites
+    s = np.zeros(N, np.uint8)
+    s[1::2] = 1
+    g.set_species(s)
+    assert g.energy() == 4 * N * int(epi[0, 0, 1]) + (3 * N // 2) * int(epi[1, 0, 0] + epi[1, 1, 1])
+    alpha, _ = g.sro()
+    assert np.allclose(alpha[0], [[1, -1], [-1, 1]]) and np.allclose(alpha[1], [[-1, 1], [1, -1]])
+
+
+def test_energy_trace_ring_and_ranges():
+    cfg = scaled_config(1, (16, 16, 16))
+    g = smcx.Lattice.from_config(cfg, trace_capacity=4)
+    o = oracle.Oracle.from_config(cfg)
+    g.sweep(6)
+    o.sweep(6)
+    assert (g.energy_trace(2, 4) == o.energy_trace(2, 4)).all()
+    with pytest.raises(smcx.SmcxError):
+        g.energy_trace(0, 6)       # sweeps 0-1 are no longer retained
+    with pytest.raises(smcx.SmcxError):
+        g.energy_trace(5, 3)       # beyond the sweeps done

@@ -1,0 +1,95 @@
+"""Host-side checks of the C-ABI library that need no GPU: it loads, exports every symbol that
+include/smcx.h declares, and validates parameters with the documented error codes."""
+import ctypes as C
+
+import numpy as np
+import pytest
+
+import paper_2509_20949_b200 as smcx
+from paper_2509_20949_b200.binding import SmcxError, workspace_bytes
+from smcx_inputs import get_config, make_accept_table, make_epi
+
+E = dict(NULL_ARG=-1, BAD_LATTICE=-2, BAD_DIMS=-3, BAD_SPECIES=-4, BAD_SHELLS=-5, EPI_NOT_SYMMETRIC=-6,
+         LINK_CELL_TOO_SMALL=-7, BAD_TABLE=-8, UNSUPPORTED=-12)
+
+
+def test_library_loads_and_exports_every_declared_symbol():
+    lib = smcx.load_library()
+    names = smcx.exported_symbols()
+    assert len(names) >= 20 and "smcx_create" in names and "smcx_sweep" in names and "smcx_sro" in names
+    for name in names:
+        assert hasattr(lib, name), name
+    assert b"sm_100a" in lib.smcx_version()
+    assert lib.smcx_strerror(0) == b"ok" and lib.smcx_strerror(-3) != lib.smcx_strerror(-4)
+
+
+def _kw(**over):
+    kw = dict(lattice=0, dims=(16, 16, 16), n_species=4, n_shells=2, epi=make_epi(2, 4, 300, 1),
+              accept=make_accept_table(600), seed=1, link_cell=4)
+    kw.update(over)
+    return kw
+
+
+def _code(**over):
+    with pytest.raises(SmcxError) as ei:
+        workspace_bytes(**_kw(**over))
+    return ei.value.code
+
+
+def test_workspace_size_covers_the_species_array():
+    for k in (1, 2, 3, 4, 5):
+        c = get_config(k)
+        for storage, per_site in ((smcx.STORAGE_U8, 1.0), (smcx.STORAGE_2BIT, 0.25)):
+            if storage == smcx.STORAGE_2BIT:
+                continue  # thread-per-cell path is validated separately
+            need = workspace_bytes(lattice=c.lattice, dims=c.dims, n_species=c.n_species, n_shells=c.n_shells,
+                                   epi=c.epi(), accept=c.accept_table(), seed=c.seed, storage=storage)
+            assert c.n_sites * per_site <= need <= c.n_sites * per_site + (16 << 20)
+
+
+def test_parameter_validation_codes():
+    assert _code(lattice=2) == E["BAD_LATTICE"]
+    assert _code(dims=(16, 16, 12)) == E["BAD_DIMS"]          # not divisible by 2w
+    assert _code(dims=(0, 16, 16)) == E["BAD_DIMS"]
+    assert _code(dims=(4, 4, 4), link_cell=2) == E["BAD_DIMS"]  # smaller than a cell plus its halo
+    assert _code(n_species=1, epi=np.zeros((2, 1, 1), np.int32)) == E["BAD_SPECIES"]
+    assert _code(n_species=17, epi=np.zeros((2, 17, 17), np.int32)) == E["BAD_SPECIES"]
+    assert _code(n_shells=0) == E["BAD_SHELLS"]
+    assert _code(n_shells=6, epi=make_epi(6, 4, 300, 1)) == E["BAD_SHELLS"]
+    bad = make_epi(2, 4, 300, 1)
+    bad[1, 0, 3] += 1
+    assert _code(epi=bad) == E["EPI_NOT_SYMMETRIC"]
+    assert _code(link_cell=1, dims=(16, 16, 16)) == E["LINK_CELL_TOO_SMALL"]   # 2w >= 2 r0 + R
+    assert _code(n_shells=4, epi=make_epi(4, 4, 300, 1), link_cell=2, dims=(16, 16, 16)) == E["LINK_CELL_TOO_SMALL"]
+    assert _code(accept=np.zeros(0, np.uint32)) == E["BAD_TABLE"]
+    assert _code(storage=smcx.STORAGE_2BIT, kernel=smcx.KERNEL_WARP_PER_CELL) == E["UNSUPPORTED"]
+    assert _code(lattice=1, n_shells=3, epi=make_epi(3, 4, 300, 1), kernel=smcx.KERNEL_THREAD_PER_CELL) == E["UNSUPPORTED"]
+    # valid combinations pass
+    assert workspace_bytes(**_kw()) > 0
+    assert workspace_bytes(**_kw(n_shells=4, epi=make_epi(4, 4, 300, 1), link_cell=4, dims=(24, 16, 16))) > 0
+    assert workspace_bytes(**_kw(lattice=1, n_shells=3, n_species=5, epi=make_epi(3, 5, 400, 1), link_cell=2,
+                                 dims=(8, 8, 12))) > 0
+
+
+def test_null_arguments_are_rejected_not_dereferenced():
+    lib = smcx.load_library()
+    assert lib.smcx_workspace_bytes(None, None) == E["NULL_ARG"]
+    assert lib.smcx_create(None, None) == E["NULL_ARG"]
+    assert lib.smcx_sweep(None, 1) == E["NULL_ARG"]
+    assert lib.smcx_energy(None, None) == E["NULL_ARG"]
+    lib.smcx_destroy(None)
+
+
+def test_no_cpu_fallback_without_a_device():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a CUDA device is present")
+    with pytest.raises(RuntimeError):
+        smcx.Lattice(**_kw())
+    # and straight through the C ABI: smcx_create must fail with SMCX_E_CUDA
+    from paper_2509_20949_b200.binding import _make_params
+    lib = smcx.load_library()
+    p, keep = _make_params(kT_units=600, storage=0, kernel=0, device=0, trace_capacity=0, **_kw())
+    h = C.c_void_p()
+    assert lib.smcx_create(C.byref(h), C.byref(p)) == -11
+    assert not h.value
