@@ -72,7 +72,7 @@ int basis_from_parity(int lattice, int px, int py, int pz) {
 inline int floor_div2(int v) { return v >= 0 ? v / 2 : -((-v + 1) / 2); }
 
 struct Layout {
-  size_t species, epi, accept, trace, state, counts, total;
+  size_t species, epi, coef, accept, trace, state, counts, total;
 };
 
 struct Plan {
@@ -188,6 +188,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   L.species = off;
   off += align_up(storage == SMCX_STORAGE_U8 ? (size_t)n_sites : (size_t)((n_sites + 15) / 16) * 4, 256);
   L.epi = off;     off += align_up((size_t)p->n_shells * n * n * sizeof(int32_t), 256);
+  L.coef = off;    off += align_up((size_t)16 * kCoefInts * sizeof(int32_t), 256);
   L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
   L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
   L.state = off;   off += align_up(sizeof(DevState), 256);
@@ -218,6 +219,7 @@ struct smcx {
 
   uint8_t* d_species() const { return reinterpret_cast<uint8_t*>(ws + plan.lay.species); }
   int32_t* d_epi() const { return reinterpret_cast<int32_t*>(ws + plan.lay.epi); }
+  int32_t* d_coef() const { return reinterpret_cast<int32_t*>(ws + plan.lay.coef); }
   uint32_t* d_accept() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.accept); }
   long long* d_trace() const { return reinterpret_cast<long long*>(ws + plan.lay.trace); }
   DevState* d_state() const { return reinterpret_cast<DevState*>(ws + plan.lay.state); }
@@ -325,7 +327,7 @@ int launch_colour_pass(smcx* h, int colour) {
   const Plan& P = h->plan;
   const Geom& G = P.G;
   if (P.kernel == SMCX_KERNEL_THREAD_PER_CELL) {
-    const int rc = launch_thread_per_cell(G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_epi(), h->d_accept(),
+    const int rc = launch_thread_per_cell(G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_coef(), h->d_accept(),
                                           h->d_state(), colour, h->stream);
     h->launches++;
     if (rc != 0) { h->err = "thread-per-cell launch failed"; return SMCX_E_CUDA; }
@@ -437,6 +439,9 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     DevState zero{};
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_state(), &zero, sizeof(zero), cudaMemcpyHostToDevice, h->stream));
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_epi(), h->epi.data(), h->epi.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+    int32_t coef[16 * kCoefInts] = {0};
+    if (h->plan.kernel == SMCX_KERNEL_THREAD_PER_CELL) build_thread_coefficients(h->epi.data(), h->plan.G.n_species, coef);
+    SMCX_CUDA(h, cudaMemcpyAsync(h->d_coef(), coef, sizeof(coef), cudaMemcpyHostToDevice, h->stream));
     SMCX_CUDA(h, cudaMemsetAsync(h->d_trace(), 0, (size_t)h->plan.G.trace_capacity * sizeof(long long), h->stream));
     SMCX_CUDA(h, cudaStreamSynchronize(h->stream));  // &zero and epi must stay valid until copied
     int r = upload_table(h, p->accept, p->accept_len);

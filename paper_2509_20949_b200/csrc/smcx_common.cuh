@@ -17,14 +17,9 @@ constexpr int kMaxSpecies = 16;
 // additions fold into immediates when the key is a kernel parameter.
 __host__ __device__ __forceinline__ void philox_round(uint32_t& c0, uint32_t& c1, uint32_t& c2,
                                                       uint32_t& c3, uint32_t k0, uint32_t k1) {
-#ifdef __CUDA_ARCH__
-  const uint32_t hi0 = __umulhi(0xD2511F53u, c0), lo0 = 0xD2511F53u * c0;
-  const uint32_t hi1 = __umulhi(0xCD9E8D57u, c2), lo1 = 0xCD9E8D57u * c2;
-#else
-  const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;
+  const uint64_t p0 = (uint64_t)0xD2511F53u * c0, p1 = (uint64_t)0xCD9E8D57u * c2;  // IMAD.WIDE.U32
   const uint32_t hi0 = (uint32_t)(p0 >> 32), lo0 = (uint32_t)p0;
   const uint32_t hi1 = (uint32_t)(p1 >> 32), lo1 = (uint32_t)p1;
-#endif
   const uint32_t n0 = hi1 ^ c1 ^ k0;
   const uint32_t n2 = hi0 ^ c3 ^ k1;
   c0 = n0; c1 = lo1; c2 = n2; c3 = lo0;
