@@ -1,0 +1,371 @@
+#!/usr/bin/env python
+"""bench.py -- trial swaps/s of the SMC-X hot path on B200 (BASELINE.json metric).
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl reference]
+
+A "step" is one Monte Carlo sweep of the whole hot path (LC origin, 8 colour
+passes with tile staging / proposal / dE / accept / write-back, energy trace), plus a9 (pair-count
+reduction -> energy + Warren-Cowley SRO) once every `sro_every` sweeps as the config prescribes and
+at least once inside the timed region.  N = 1 times BASELINE.json configs[3] (BCC 800^3, 1.024e9
+sites, the configuration the metric is quoted on).  N > 1 runs N independent replicas, one per GPU
+(the path is single-GPU by north_star: "replicas only", weak scaling, no data-path collective).
+
+`--impl reference` times the CPU oracle (oracle/, test infrastructure) on the host cores for the
+same metric; under torchrun only rank 0 works.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from dataclasses import replace  # noqa: E402
+
+from smcx_inputs import get_config  # noqa: E402
+
+ALGO_BYTES_PER_TRIAL = (686 + 250) / 128.0   # LIZ+ box read + modified box written per 128 trials
+FALLBACK_HBM_GBS = 6650.0                    # B200_PROFILING.md fallback
+
+
+def metric_name() -> str:
+    try:
+        return json.load(open(os.path.join(ROOT, "BASELINE.json")))["metric"]
+    except Exception:
+        return "trial swaps/sec on 1 B200 (1e9-site BCC, 4 species) and % of HBM roofline"
+
+
+def measured_peak():
+    try:
+        return float(json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]), "measured"
+    except Exception:
+        return FALLBACK_HBM_GBS, "fallback"
+
+
+def workload_string(cfg) -> str:
+    lat = "BCC" if cfg.lattice == 0 else "FCC"
+    return (f"{lat} {cfg.dims[0]}x{cfg.dims[1]}x{cfg.dims[2]} conventional cells ({cfg.n_sites} sites), "
+            f"{cfg.n_species} species equiatomic, {cfg.n_shells}-shell int32 EPI in [-{cfg.amplitude},{cfg.amplitude}], "
+            f"kT={cfg.kT_units / 10:g} meV, link cell {cfg.link_cell}, seed {cfg.seed}")
+
+
+# --------------------------------------------------------------------------------------------
+# clocks during the timed region (B200_PROFILING.md recipe)
+# --------------------------------------------------------------------------------------------
+class ClockSampler:
+    QUERY = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+             "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.proc = None
+        self.lines = []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.gpu}", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
+                 "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._pump, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _pump(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.lines:
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); smax.append(float(f[2])); power.append(float(f[3]))
+            except ValueError:
+                continue
+            for name, val in zip(names, f[5:9]):
+                if val.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None, "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# --------------------------------------------------------------------------------------------
+# CPU oracle timing (cpu_baseline and --impl reference)
+# --------------------------------------------------------------------------------------------
+def oracle_sample_config(cfg, max_sites: float = 8.3e6):
+    """A bounded sample of the workload: same lattice type, species, EPI, kT, link cell, smaller box."""
+    per_cell = 2 if cfg.lattice == 0 else 4
+    edge = 16
+    for e in (32, 48, 64, 96, 128, 160):
+        if e ** 3 * per_cell <= max_sites:
+            edge = e
+    dims = tuple(min(d, edge) for d in cfg.dims)
+    return replace(cfg, name=f"{cfg.name}@sample{edge}", dims=dims)
+
+
+class OracleTimer:
+    """The oracle as it stands (never tuned), one thread, on a bounded sample of the workload."""
+
+    def __init__(self, cfg, max_sites: float = 8.3e6):
+        import oracle
+        self.sample = oracle_sample_config(cfg, max_sites)
+        self.o = oracle.Oracle.from_config(self.sample)
+        self.o.running_energy()
+        self.t = 0
+
+    def sweeps(self, n: int):
+        t0 = time.perf_counter()
+        for _ in range(n):
+            if self.sample.anneal:
+                self.o.set_temperature(self.sample.accept_table(self.t % self.sample.n_sweeps))
+            self.o.sweep(1)
+            self.t += 1
+        return time.perf_counter() - t0
+
+    def describe(self, n: int) -> str:
+        d = self.sample.dims
+        return (f"oracle (single thread, g++ -O2) on {d[0]}x{d[1]}x{d[2]} cells ({self.sample.n_sites} sites) "
+                f"x {n} sweeps of the same workload (species, EPI, kT, link cell)")
+
+
+def run_reference(args, cfg, rank):
+    if rank != 0:
+        return
+    # size the per-step sample so that steps + warmup sweeps take about two minutes at ~2.5e6 trials/s
+    budget_sites = 2.5e6 * 120.0 / max(1, args.steps + args.warmup)
+    timer = OracleTimer(cfg, max_sites=min(8.3e6, max(7e4, budget_sites)))
+    timer.sweeps(args.warmup)
+    dt = timer.sweeps(args.steps)
+    value = timer.sample.n_sites * args.steps / dt
+    desc = timer.describe(args.steps)
+    out = {
+        "impl": "reference", "metric": metric_name(), "value": value, "unit": "trial swaps/s", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / max(1, args.steps),
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+        "config": {"workload": workload_string(cfg), "note": "each step = 1 oracle sweep on the bounded sample"},
+        "cpu_baseline": {"value": value, "unit": "trial swaps/s", "cores": 1, "kind": "oracle", "sample": desc,
+                         "host_cores_available": os.cpu_count()},
+        "e2e": {"value": value, "unit": "trial swaps/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(out))
+
+
+# --------------------------------------------------------------------------------------------
+# aggregation across ranks (testable with gloo on CPU)
+# --------------------------------------------------------------------------------------------
+def aggregate_over_ranks(local_ms: float, local_units: float, dist=None, device=None):
+    """Whole-job throughput: units summed over ranks / max time over ranks.  Returns (value, max_ms)."""
+    if dist is None or not dist.is_initialized() or dist.get_world_size() == 1:
+        return local_units / (local_ms * 1e-3), local_ms
+    import torch
+    t = torch.tensor([local_ms], dtype=torch.float64, device=device)
+    u = torch.tensor([local_units], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    dist.all_reduce(u, op=dist.ReduceOp.SUM)
+    return float(u.item()) / (float(t.item()) * 1e-3), float(t.item())
+
+
+def replica_seed(base_seed: int, rank: int) -> int:
+    """Independent replicas: rank r simulates the same workload with seed base + 7919 r."""
+    return base_seed + 7919 * rank
+
+
+# --------------------------------------------------------------------------------------------
+# the CUDA arm
+# --------------------------------------------------------------------------------------------
+def run_cuda(args, cfg, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    import paper_2509_20949_b200 as smcx
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the CUDA path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1 and not dist.is_initialized():
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    sro_every = cfg.sro_every if cfg.sro_every > 0 else 1000
+    lat = smcx.Lattice.from_config(cfg, seed=replica_seed(cfg.seed, rank), device=local_rank,
+                                   kernel=args.kernel, storage=args.storage)
+    tables = None
+    if cfg.anneal:
+        tables = [(cfg.kT_at(t), cfg.accept_table(t)) for t in range(min(cfg.n_sweeps, args.steps + args.warmup))]
+
+    def one_step(t):
+        if tables is not None:
+            kT, tab = tables[t % len(tables)]
+            lat.set_temperature(kT, tab)
+        lat.sweep(1)
+
+    for t in range(args.warmup):
+        one_step(t)
+    lat.sro()
+    barrier()
+
+    # ---- device-resident timing -----------------------------------------------------------
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+    launches0 = lat.kernel_launches
+    barrier()
+    ev[0].record()
+    sweep_ms = 0.0
+    sro_ms = 0.0
+    done = 0
+    n_sro = 0
+    while done < args.steps:
+        chunk = min(sro_every - (done % sro_every), args.steps - done)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for t in range(chunk):
+            one_step(args.warmup + done + t)
+        b.record()
+        done += chunk
+        c0 = torch.cuda.Event(enable_timing=True); c1 = torch.cuda.Event(enable_timing=True)
+        c0.record()
+        if done % sro_every == 0 or done == args.steps:
+            alpha, counts = lat.sro()      # a9: synchronises
+            n_sro += 1
+        c1.record()
+        torch.cuda.synchronize()
+        sweep_ms += a.elapsed_time(b)
+        sro_ms += c0.elapsed_time(c1)
+    ev[1].record()
+    barrier()
+    total_ms = ev[0].elapsed_time(ev[1])
+    launches = lat.kernel_launches - launches0
+    clocks = sampler.stop()
+
+    trials = float(cfg.n_sites) * args.steps
+    value, max_ms = aggregate_over_ranks(total_ms, trials, dist if world > 1 else None, dev)
+
+    # ---- end to end through the C ABI with host buffers -------------------------------------
+    # one job = upload the lattice from pinned host memory, K x (upload that sweep's threshold
+    # table, sweep, read the sweep's energy back), download the lattice, SRO.
+    host_species = torch.empty(cfg.n_sites, dtype=torch.uint8).pin_memory().numpy()
+    lat.species(out=host_species)
+    e2e_steps = min(args.steps, 20)
+    table = cfg.accept_table(0)
+    barrier()
+    t0 = time.perf_counter()
+    lat.set_species(host_species)
+    first = lat.stats()[0]
+    for t in range(e2e_steps):
+        if tables is not None:
+            kT, table = tables[t % len(tables)]
+        lat.set_temperature(cfg.kT_at(0) if tables is None else kT, table)
+        lat.sweep(1)
+        lat.energy_trace(first + t, 1)
+    lat.species(out=host_species)
+    lat.sro()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_value, _ = aggregate_over_ranks(e2e_s * 1e3, float(cfg.n_sites) * e2e_steps, dist if world > 1 else None, dev)
+    h2d = (cfg.n_sites + e2e_steps * table.nbytes) / e2e_steps
+    d2h = (cfg.n_sites + e2e_steps * 8 + 2 * counts.nbytes) / e2e_steps
+
+    if rank == 0:
+        peak, peak_kind = measured_peak()
+        # dominant kernel: one colour pass = n_sites/8 trials per launch, 8 launches per sweep
+        launch_ms = sweep_ms / (8.0 * args.steps)
+        achieved = ALGO_BYTES_PER_TRIAL * (cfg.n_sites / 8.0) / (launch_ms * 1e-3) / 1e9
+        traffic = None
+        tp = os.path.join(ROOT, "profiles", "dram_traffic_per_launch.json")
+        if os.path.exists(tp):
+            try:
+                rec = json.load(open(tp))
+                if rec.get("workload_sites") == cfg.n_sites and rec.get("kernel") == lat.kernel:
+                    traffic = rec["dram_bytes_per_launch"]
+            except Exception:
+                pass
+        out = {
+            "metric": metric_name(), "value": value, "unit": "trial swaps/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {
+                "workload": workload_string(cfg), "config_id": args.config,
+                "step": f"1 sweep = 8 colour-pass launches + trace; pair-count/SRO reduction every {sro_every} sweeps "
+                        f"and once at the end ({n_sro} inside the timed region)",
+                "kernel": {1: "warp_per_cell/u8", 2: "thread_per_cell/2bit"}[lat.kernel],
+                "l2": "lattice (%.0f MB in device storage) larger than the 126 MB L2; no flush" %
+                      (cfg.n_sites * (0.25 if lat.storage == 2 else 1.0) / 1e6),
+                "parallelism": "replicas only" if world > 1 else "single GPU",
+            },
+            "pct_of_hbm_roofline": 100.0 * (value / world) * ALGO_BYTES_PER_TRIAL / (peak * 1e9),
+            "sweep_ms": sweep_ms / args.steps, "sro_ms_each": sro_ms / max(1, n_sro),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": traffic, "peak_kind": peak_kind,
+                         "kernel": "sweep_thread_per_cell" if lat.kernel == 2 else "sweep_warp_per_cell",
+                         "algorithmic_bytes_per_trial": ALGO_BYTES_PER_TRIAL, "launch_ms": launch_ms},
+            "e2e": {"value": e2e_value, "unit": "trial swaps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps,
+                    "what": "smcx_set_species(host) + steps x (smcx_set_temperature(host table) + smcx_sweep(1) + "
+                            "smcx_energy_trace read) + smcx_species(host) + smcx_sro, wall clock"},
+            "gpu_launches": int(launches), "clocks": clocks,
+        }
+        if not args.no_cpu_baseline and world == 1:
+            timer = OracleTimer(cfg)
+            n_or = 3
+            dt = timer.sweeps(n_or)
+            v, desc = timer.sample.n_sites * n_or / dt, timer.describe(n_or)
+            out["cpu_baseline"] = {"value": v, "unit": "trial swaps/s", "cores": 1, "kind": "oracle", "sample": desc,
+                                   "host_cores_available": os.cpu_count()}
+        print(json.dumps(out))
+    lat.close()
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=100)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
+    ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default: 4, the graded one)")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 warp-per-cell, 2 thread-per-cell")
+    ap.add_argument("--storage", type=int, default=0, help="0 auto, 2 packed 2-bit, 8 uint8")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = get_config(args.config)
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+        return
+    run_cuda(args, cfg, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()
