@@ -72,7 +72,7 @@ int basis_from_parity(int lattice, int px, int py, int pz) {
 inline int floor_div2(int v) { return v >= 0 ? v / 2 : -((-v + 1) / 2); }
 
 struct Layout {
-  size_t species, epi, coef, accept, trace, state, counts, total;
+  size_t species, epi, coef, accept, filter, trace, state, counts, total;
 };
 
 struct Plan {
@@ -147,6 +147,8 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   G.key1 = (uint32_t)(p->seed >> 32);
   G.accept_len = p->accept_len;
   G.trace_capacity = p->trace_capacity > 0 ? p->trace_capacity : 65536;
+  G.filter_E = -1;
+  set_thread_masks(G);
   // tile-linear deltas
   for (int b = 0; b < G.B; ++b) {
     int bp[3];
@@ -190,6 +192,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   L.epi = off;     off += align_up((size_t)p->n_shells * n * n * sizeof(int32_t), 256);
   L.coef = off;    off += align_up((size_t)16 * kCoefInts * sizeof(int32_t), 256);
   L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
+  L.filter = off;  off += align_up((size_t)kFilterWords * sizeof(uint32_t), 256);
   L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
   L.state = off;   off += align_up(sizeof(DevState), 256);
   L.counts = off;  off += align_up((size_t)kMaxShells * kMaxSpecies * kMaxSpecies * sizeof(unsigned long long), 256);
@@ -221,6 +224,7 @@ struct smcx {
   int32_t* d_epi() const { return reinterpret_cast<int32_t*>(ws + plan.lay.epi); }
   int32_t* d_coef() const { return reinterpret_cast<int32_t*>(ws + plan.lay.coef); }
   uint32_t* d_accept() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.accept); }
+  uint32_t* d_filter() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.filter); }
   long long* d_trace() const { return reinterpret_cast<long long*>(ws + plan.lay.trace); }
   DevState* d_state() const { return reinterpret_cast<DevState*>(ws + plan.lay.state); }
   unsigned long long* d_counts() const { return reinterpret_cast<unsigned long long*>(ws + plan.lay.counts); }
@@ -313,6 +317,19 @@ int upload_table(smcx* h, const uint32_t* accept, int len) {
   std::memcpy(h->staging[slot], accept, (size_t)len * sizeof(uint32_t));
   SMCX_CUDA(h, cudaMemcpyAsync(h->d_accept(), h->staging[slot], (size_t)len * sizeof(uint32_t),
                                cudaMemcpyHostToDevice, h->stream));
+  h->plan.G.filter_E = -1;
+  h->plan.G.filter_nq = 0;
+  if (h->plan.kernel == SMCX_KERNEL_THREAD_PER_CELL) {
+    uint32_t* filt = h->staging[slot] + kAcceptCapacity;
+    int nq = 0;
+    const int E = build_accept_filter(accept, len, filt, &nq);
+    if (E >= 0) {
+      SMCX_CUDA(h, cudaMemcpyAsync(h->d_filter(), filt, (size_t)kFilterWords * sizeof(uint32_t),
+                                   cudaMemcpyHostToDevice, h->stream));
+      h->plan.G.filter_E = E;
+      h->plan.G.filter_nq = nq;
+    }
+  }
   SMCX_CUDA(h, cudaEventRecord(h->staging_ev[slot], h->stream));
   h->plan.G.accept_len = len;
   return SMCX_OK;
@@ -328,7 +345,7 @@ int launch_colour_pass(smcx* h, int colour) {
   const Geom& G = P.G;
   if (P.kernel == SMCX_KERNEL_THREAD_PER_CELL) {
     const int rc = launch_thread_per_cell(G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_coef(), h->d_accept(),
-                                          h->d_state(), colour, h->stream);
+                                          h->d_filter(), h->d_state(), colour, h->stream);
     h->launches++;
     if (rc != 0) { h->err = "thread-per-cell launch failed"; return SMCX_E_CUDA; }
     return SMCX_OK;
@@ -415,7 +432,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     h->ws = reinterpret_cast<char*>(ws);
     h->owns_ws = true;
   }
-  h->staging_cap = (size_t)kAcceptCapacity * sizeof(uint32_t);
+  h->staging_cap = ((size_t)kAcceptCapacity + kFilterWords) * sizeof(uint32_t);
   for (int s = 0; s < kStagingSlots; ++s) {
     if (cudaMallocHost(reinterpret_cast<void**>(&h->staging[s]), h->staging_cap) != cudaSuccess) return fail(SMCX_E_NO_MEMORY);
     if (cudaEventCreateWithFlags(&h->staging_ev[s], cudaEventDisableTiming) != cudaSuccess) return fail(SMCX_E_CUDA);

@@ -74,6 +74,12 @@ struct Geom {
   uint32_t key0, key1; // Philox key = seed
   int accept_len;
   int trace_capacity;
+  // Two-level acceptance filter of the thread-per-cell kernel (see sweep_thread.cuh): disabled when
+  // filter_E < 0, else T[d] - mulhi(Tq[d>>6], Tr[d&63]) lies in [0, filter_E] for every d.
+  int filter_E;
+  int filter_nq;
+  // bit masks handed over as parameters so that ptxas keeps them in registers (one LOP3 per term)
+  uint32_t kH, kM1, kF1, kH2, kM2, kF2;
   // all shells concatenated, shell by shell, each in ascending (dz,dy,dx) order
   signed char off[kMaxNeighbours][3];   // half-lattice units
   unsigned char shell_of[kMaxNeighbours];

@@ -16,15 +16,22 @@
 //    the bit counts around i and around j and corr = 2 V_0(a,b) - V_0(a,a) - V_0(b,b) undoing
 //    the i-j bond that both sums include.  Integer arithmetic throughout: results are bit-identical
 //    to the plain before/after energy difference.
+//  * the integer pipe (LOP3/SHF) is the binding unit (ncu: profiles/), so the code is arranged to
+//    keep its instruction count down: fused three-input logic with masks held in registers,
+//    merges by multiply-add on the FMA pipe, coefficient tables replicated per lane slot so that
+//    the 128-bit loads are conflict-free, and a two-level acceptance filter in shared memory.
 #pragma once
 #include "smcx_common.cuh"
 #include "sweep_warp.cuh"
 
 namespace smcxk {
 
-constexpr int kThreadNT = 128;          // threads (= cells) per block
+constexpr int kThreadNT = 256;          // threads (= cells) per block
 constexpr int kThreadTileWords = 64;    // 8 x 8 rows of one word
-constexpr int kCoefInts = 8;            // per (a,b): cl0 ch0 cb0 cl1 ch1 cb1 corr' pad
+constexpr int kCoefInts = 8;            // per (a,b): cl0 ch0 cb0 cl1 | ch1 cb1 corr' pad
+constexpr int kFilterTr = 64;           // Tr[r] = T[r], r < 64
+constexpr int kFilterMaxTq = 1024;      // Tq[q] = T[64 q]; tables up to 65,536 entries (power of two: indices are masked)
+constexpr int kFilterWords = kFilterTr + kFilterMaxTq;
 
 inline bool thread_kernel_supported(const Geom& G) {
   return G.lattice == 0 && G.n_shells == 2 && G.w == 4 && G.n_species <= 4 && G.H == 2 && G.TW == 8;
@@ -53,88 +60,144 @@ inline void build_thread_coefficients(const int32_t* epi, int n_species, int32_t
     }
 }
 
-__device__ __forceinline__ uint32_t rotr32(uint32_t v, int n) { return __funnelshift_r(v, v, n); }
+// Host: two-level filter tables for a threshold table T.  Returns E >= 0 such that
+// 0 <= T[d] - mulhi(Tq[d>>6], Tr[d&63]) <= E for all d < len, or -1 if no such small bound holds
+// (then the kernel reads T[d] directly).  For T[d] = floor(2^32 exp(-d/kT)) the product of the
+// two floors never exceeds T[d] and falls short by a few units at most.
+inline int build_accept_filter(const uint32_t* T, int len, uint32_t* filt /*kFilterWords*/, int* nq_out) {
+  const int nq = (len + 63) / 64;
+  *nq_out = nq;
+  if (nq > kFilterMaxTq) return -1;
+  for (int r = 0; r < kFilterTr; ++r) filt[r] = r < len ? T[r] : 0u;
+  for (int q = 0; q < kFilterMaxTq; ++q) filt[kFilterTr + q] = q < nq ? T[64 * q] : 0u;
+  uint32_t E = 0;
+  for (int d = 0; d < len; ++d) {
+    const uint32_t ta = (uint32_t)(((uint64_t)filt[kFilterTr + (d >> 6)] * filt[d & 63]) >> 32);
+    if (ta > T[d]) return -1;
+    E = T[d] - ta > E ? T[d] - ta : E;
+  }
+  return E <= 1024u ? (int)E : -1;
+}
 
-// Gather the shell-0 (8 fields, bits 0..15) and shell-1 (6 fields at bits 0,2,4,6,8,12) neighbour
-// species of site (X,Y,Z,b) of this thread's tile; also returns the site's own row word.
+inline void set_thread_masks(Geom& G) {
+  // count words (see trial_thread): shell 0 = [n01_i n23_i | n01_j n23_j], one byte each;
+  // shell 1 = [v_i | v_j | own-row fields of i at bits 16,24 and of j at bits 18,26]
+  G.kH = 0xFFFF0000u; G.kM1 = 0x55555555u; G.kF1 = 0x55550000u;
+  G.kH2 = 0x0C0CFF00u; G.kM2 = 0x05055555u; G.kF2 = 0x04045500u;
+}
+
+__device__ __forceinline__ uint32_t lop3_maj(uint32_t a, uint32_t b, uint32_t c) {
+  uint32_t d;
+  asm("lop3.b32 %0, %1, %2, %3, 0xE8;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+}
+
+// Neighbour species of the site of sublattice b whose own 2-bit field sits at bit s0 of the row
+// word at p (p1 = 1 << (s0 - 4)).  Fields are masked in place, merged by multiply-add (FMA pipe)
+// and shifted down once:
+//   n01, n23: shell 0, 4 fields each (the 2x2x2 block of the other sublattice, rows pairwise)
+//   v:        shell 1, the fields at X of the four adjacent rows
+//   t_own:    own row >> (s0 - 4): shell-1 fields of X-1 / X+1 at bits 0 / 8, own species at bit 4
 template <int b>
-__device__ __forceinline__ void gather_site(const uint32_t* tile, int X, int row, uint32_t& V1, uint32_t& V2,
-                                            uint32_t& own) {
+__device__ __forceinline__ void gather_site(const uint32_t* p, int s0, uint32_t p1, uint32_t& n01, uint32_t& n23,
+                                            uint32_t& v, uint32_t& own, uint32_t& t_own) {
   constexpr int NT = kThreadNT;
-  const uint32_t* p = tile + row * NT;
   own = p[0];
   const uint32_t yM = p[-NT], yP = p[NT], zM = p[-8 * NT], zP = p[8 * NT];
   const uint32_t dg = b ? p[9 * NT] : p[-9 * NT];
-  // shell 0: the 2x2x2 block of the other sublattice; fields at bit s1 and s1+4 of four rows
-  const int s1 = 4 * X + 2 * b - 2;
   const uint32_t A = b ? own : dg, Bq = b ? yP : zM, Cq = b ? zP : yM, Dq = b ? dg : own;
-  const uint32_t b01 = ((A >> s1) & 0x33u) | ((Bq >> (s1 - 2)) & 0xCCu);
-  const uint32_t b23 = ((Cq >> s1) & 0x33u) | ((Dq >> (s1 - 2)) & 0xCCu);
-  V1 = b01 | (b23 << 8);
-  // shell 1: same sublattice at X-1, X+1 of the own row and at X of the four adjacent rows
-  const int s0 = 4 * X + 2 * b;
-  uint32_t acc = (own >> (s0 - 4)) & 0x303u;
-  acc |= rotr32(yM, (s0 - 2) & 31) & 0xCu;
-  acc |= rotr32(yP, (s0 - 4) & 31) & 0x30u;
-  acc |= rotr32(zM, (s0 - 6) & 31) & 0xC0u;
-  acc |= rotr32(zP, (s0 - 12) & 31) & 0x3000u;
-  V2 = acc;
+  const uint32_t mA = p1 * 204u;     // 0x33 << (s0 - 2)
+  const uint32_t m0 = p1 * 48u;      // 0x3 << s0
+  n01 = ((A & mA) + (Bq & mA) * 4u) >> (s0 - 2);
+  n23 = ((Cq & mA) + (Dq & mA) * 4u) >> (s0 - 2);
+  v = ((yM & m0) + (yP & m0) * 4u + (zM & m0) * 16u + (zP & m0) * 64u) >> s0;
+  t_own = own >> (s0 - 4);
 }
 
-// U holds the fields around i in its low half and around j in its high half.  Returns the three
-// merged counts; each equals (count around i) - (count around j) + (number of fields).
-__device__ __forceinline__ void count3(uint32_t U, uint32_t M, uint32_t F, int& plo, int& phi, int& pbt) {
+// U holds 2-bit fields; those selected by H belong to j, the others to i; M marks the low bit of
+// every field, F = M & H.  Returns for lo bits, hi bits and lo&hi the merged population counts
+// (count over i's fields) - (count over j's fields) + (number of j fields).
+__device__ __forceinline__ void count3(uint32_t U, uint32_t H, uint32_t M, uint32_t F, int& plo, int& phi, int& pbt) {
   const uint32_t Us = U >> 1;
-  plo = __popc((U & M) ^ F);
-  phi = __popc((Us & M) ^ F);
-  pbt = __popc((U & Us & M) ^ F);
+  const uint32_t tl = (U ^ H) & M;           // lo bits; complemented in j's fields
+  const uint32_t th = (Us ^ H) & M;          // hi bits; complemented in j's fields
+  const uint32_t tb = lop3_maj(tl, th, F);   // lo & hi for i, ~(lo & hi) for j
+  plo = __popc(tl);
+  phi = __popc(th);
+  pbt = __popc(tb);
 }
 
-template <int bi>
-__device__ __forceinline__ void trial_thread(uint32_t* tile, const int4* s_coef, const uint32_t* __restrict__ accept,
-                                             int accept_len, int X, int Y, int Z, uint32_t w_dir, uint32_t u,
-                                             int& esum, unsigned& nacc) {
+template <int bi, int X, bool kFilter>
+__device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const char* coef_base,
+                                             const uint32_t* s_filt, const uint32_t* __restrict__ accept,
+                                             uint32_t w_dir, uint32_t u, int& esum, unsigned& nacc) {
   constexpr int NT = kThreadNT;
   constexpr int bj = 1 - bi;
-  const int dir = (int)(w_dir >> 29);                 // mulhi(w_dir, 8)
-  const int Xj = X - 1 + bi + (dir & 1);
-  const int Yj = Y - 1 + bi + ((dir >> 1) & 1);
-  const int Zj = Z - 1 + bi + (dir >> 2);
-  const int row_i = Z * 8 + Y, row_j = Zj * 8 + Yj;
-  uint32_t V1i, V2i, own_i, V1j, V2j, own_j;
-  gather_site<bi>(tile, X, row_i, V1i, V2i, own_i);
-  gather_site<bj>(tile, Xj, row_j, V1j, V2j, own_j);
-  const int sh_i = 4 * X + 2 * bi, sh_j = 4 * Xj + 2 * bj;
-  const uint32_t a = (own_i >> sh_i) & 3u, b = (own_j >> sh_j) & 3u;
-  const int4 c0 = s_coef[(a * 4 + b) * 2], c1 = s_coef[(a * 4 + b) * 2 + 1];
+  constexpr int s0_i = 4 * X + 2 * bi;
+  // direction: top three bits of the draw (= mulhi(w_dir, 8)); dx = bit 0, dy = bit 1, dz = bit 2
+  const int t1 = (int)(w_dir >> 30);                      // dy + 2 dz
+  const int dz = (int)(w_dir >> 31);
+  const int dir = (int)(w_dir >> 29);
+  const int rd = t1 + 6 * dz - 9 * (1 - bi);              // row_j - row_i = (dy-1+bi) + 8 (dz-1+bi)
+  const int s0_j = (4 * X + 4 * bi + 2 * bj - 4) + 4 * dir - 8 * t1;   // 4 (X-1+bi+dx) + 2 bj
+  const uint32_t p1_j = 1u << (s0_j - 4);
+  uint32_t* p_j = p_i + rd * NT;
+  uint32_t n01i, n23i, vi, own_i, t_i, n01j, n23j, vj, own_j, t_j;
+  gather_site<bi>(p_i, s0_i, 1u << (s0_i - 4), n01i, n23i, vi, own_i, t_i);
+  gather_site<bj>(p_j, s0_j, p1_j, n01j, n23j, vj, own_j, t_j);
+  const uint32_t a4 = t_i & 0x30u, b4 = t_j & 0x30u;      // species of i and j, times 16
+  const int4 c0 = *reinterpret_cast<const int4*>(coef_base + a4 * 32u + b4 * 8u);            // [(a*4+b)*8 + slot]
+  const int4 c1 = *reinterpret_cast<const int4*>(coef_base + 2048 + a4 * 32u + b4 * 8u);
+  const uint32_t U1 = n01i + n23i * 256u + n01j * 65536u + n23j * 16777216u;
+  const uint32_t U2 = vi + vj * 256u + (t_i & 0x303u) * 65536u + (t_j & 0x303u) * 262144u;
   int p1l, p1h, p1b, p2l, p2h, p2b;
-  count3(__byte_perm(V1i, V1j, 0x5410), 0x55555555u, 0x55550000u, p1l, p1h, p1b);
-  count3(__byte_perm(V2i, V2j, 0x5410), 0x11551155u, 0x11550000u, p2l, p2h, p2b);
+  count3(U1, G.kH, G.kM1, G.kF1, p1l, p1h, p1b);
+  count3(U2, G.kH2, G.kM2, G.kF2, p2l, p2h, p2b);
   const int dE = c1.z + c0.x * p1l + c0.y * p1h + c0.z * p1b + c0.w * p2l + c1.x * p2h + c1.y * p2b;
-  bool ok = dE <= 0;
-  if (!ok && dE < accept_len) ok = u < __ldg(accept + dE);
-  ok = ok && (a != b);
-  if (ok) {
-    const uint32_t x = a ^ b;
-    const uint32_t new_i = own_i ^ (x << sh_i);
-    const uint32_t new_j = (row_j == row_i ? new_i : own_j) ^ (x << sh_j);
-    tile[row_i * NT] = new_i;
-    tile[row_j * NT] = new_j;
+  bool ok;
+  if (kFilter) {
+    // two-level threshold: ta <= T[dE] <= ta + E; tables are zero beyond the last entry and the
+    // indices are masked, so every lane can evaluate it whatever its dE
+    const uint32_t ta = __umulhi(s_filt[kFilterTr + (((uint32_t)dE >> 6) & (kFilterMaxTq - 1))], s_filt[dE & 63]);
+    const bool in_table = dE < G.accept_len;
+    ok = dE <= 0 || (in_table && u < ta);
+    if (!ok && in_table && u - ta <= (uint32_t)G.filter_E) ok = u < __ldg(accept + dE);   // rare exact look-up
+  } else {
+    ok = dE <= 0;
+    if (!ok && dE < G.accept_len) ok = u < __ldg(accept + dE);
+  }
+  if (ok && a4 != b4) {
+    const uint32_t x4 = a4 ^ b4;
+    const uint32_t new_i = own_i ^ (x4 << (s0_i - 4));
+    const uint32_t new_j = (rd == 0 ? new_i : own_j) ^ (x4 * p1_j);
+    p_i[0] = new_i;
+    p_j[0] = new_j;
     esum += dE;
     ++nacc;
   }
 }
 
-__global__ void __launch_bounds__(kThreadNT, 6)
+template <bool kFilter>
+__global__ void __launch_bounds__(kThreadNT, 3)
 sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* __restrict__ coef,
-                      const uint32_t* __restrict__ accept, DevState* __restrict__ st, int colour) {
+                      const uint32_t* __restrict__ accept, const uint32_t* __restrict__ filt,
+                      DevState* __restrict__ st, int colour) {
   constexpr int NT = kThreadNT;
   extern __shared__ __align__(16) uint32_t smem_w[];
   uint32_t* tile = smem_w + threadIdx.x;                        // row r at tile[r * NT]
-  int4* s_coef = reinterpret_cast<int4*>(smem_w + kThreadTileWords * NT);
+  int4* s_coef0 = reinterpret_cast<int4*>(smem_w + kThreadTileWords * NT);   // [16][8 slots]
+  int4* s_coef1 = s_coef0 + 16 * 8;
+  uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_coef1 + 16 * 8);
   __shared__ int s_dE[NT / 32];
   __shared__ unsigned s_acc[NT / 32];
-  if (threadIdx.x < 32) s_coef[threadIdx.x] = coef[threadIdx.x];
+  // coefficient rows replicated over the 8 lane slots of a quarter warp: conflict-free LDS.128
+  if (threadIdx.x < 128) {
+    const int ent = threadIdx.x >> 3;
+    s_coef0[threadIdx.x] = coef[ent * 2];
+    s_coef1[threadIdx.x] = coef[ent * 2 + 1];
+  }
+  if (kFilter)
+    for (int k = threadIdx.x; k < kFilterWords; k += NT) s_filt[k] = filt[k];
 
   const uint32_t t = (uint32_t)st->sweep;
   int ox, oy, oz;
@@ -171,15 +234,20 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
     // a4-a6: the 128 trials of this cell, raster order, one Philox call per two slots
     const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
     const uint32_t ctr3 = TAG_TRIAL | ((uint32_t)colour << 8);
-    const int accept_len = G.accept_len;
-    for (int lz = 0; lz < 4; ++lz)
-      for (int ly = 0; ly < 4; ++ly)
+    const char* coef_base = reinterpret_cast<const char*>(s_coef0) + (threadIdx.x & 7) * 16;
 #pragma unroll 1
-        for (int lx = 0; lx < 4; ++lx) {
-          const Philox4 r = philox4x32_10(cell_id, (uint32_t)((lz * 4 + ly) * 4 + lx), t, ctr3, G.key0, G.key1);
-          trial_thread<0>(tile, s_coef, accept, accept_len, lx + 2, ly + 2, lz + 2, r.x, r.y, esum, nacc);
-          trial_thread<1>(tile, s_coef, accept, accept_len, lx + 2, ly + 2, lz + 2, r.z, r.w, esum, nacc);
-        }
+    for (int lzy = 0; lzy < 16; ++lzy) {
+      uint32_t* p_row = tile + (((lzy >> 2) + 2) * 8 + (lzy & 3) + 2) * NT;
+      const uint32_t q0 = (uint32_t)lzy * 4u;
+#define SMCX_TRIAL_PAIR(LX)                                                                                   \
+      {                                                                                                       \
+        const Philox4 r = philox4x32_10(cell_id, q0 + LX, t, ctr3, G.key0, G.key1);                           \
+        trial_thread<0, LX + 2, kFilter>(G, p_row, coef_base, s_filt, accept, r.x, r.y, esum, nacc);          \
+        trial_thread<1, LX + 2, kFilter>(G, p_row, coef_base, s_filt, accept, r.z, r.w, esum, nacc);          \
+      }
+      SMCX_TRIAL_PAIR(0) SMCX_TRIAL_PAIR(1) SMCX_TRIAL_PAIR(2) SMCX_TRIAL_PAIR(3)
+#undef SMCX_TRIAL_PAIR
+    }
     // a7: write back tile rows 1..6 x 1..6; only the bytes that lie wholly inside this tile and
     // can hold a modified site (conventional cells 1..6 of the row)
     const int rb = G.Lx >> 1;                                   // bytes per lattice row
@@ -216,18 +284,27 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
   }
 }
 
-inline size_t thread_kernel_smem() { return (size_t)kThreadTileWords * kThreadNT * 4 + 16 * kCoefInts * 4; }
+inline size_t thread_kernel_smem() {
+  return (size_t)kThreadTileWords * kThreadNT * 4 + 2 * 16 * 8 * sizeof(int4) + kFilterWords * 4;
+}
 
 inline int configure_thread_per_cell() {
-  return cudaFuncSetAttribute(sweep_thread_per_cell, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                              (int)thread_kernel_smem()) == cudaSuccess ? 0 : -1;
+  if (cudaFuncSetAttribute(sweep_thread_per_cell<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)thread_kernel_smem()) != cudaSuccess) return -1;
+  if (cudaFuncSetAttribute(sweep_thread_per_cell<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           (int)thread_kernel_smem()) != cudaSuccess) return -1;
+  return 0;
 }
 
 inline int launch_thread_per_cell(const Geom& G, uint32_t* lattice, const int32_t* d_coef, const uint32_t* accept,
-                                  DevState* st, int colour, cudaStream_t stream) {
+                                  const uint32_t* d_filter, DevState* st, int colour, cudaStream_t stream) {
   const unsigned grid = (G.cells_per_colour + kThreadNT - 1) / kThreadNT;
-  sweep_thread_per_cell<<<grid, kThreadNT, thread_kernel_smem(), stream>>>(
-      G, lattice, reinterpret_cast<const int4*>(d_coef), accept, st, colour);
+  if (G.filter_E >= 0)
+    sweep_thread_per_cell<true><<<grid, kThreadNT, thread_kernel_smem(), stream>>>(
+        G, lattice, reinterpret_cast<const int4*>(d_coef), accept, d_filter, st, colour);
+  else
+    sweep_thread_per_cell<false><<<grid, kThreadNT, thread_kernel_smem(), stream>>>(
+        G, lattice, reinterpret_cast<const int4*>(d_coef), accept, d_filter, st, colour);
   return 0;
 }
 
