@@ -8,7 +8,7 @@ import re
 import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-_LIB_PATH = os.path.join(_HERE, "libsmcx.so")
+_LIB_PATH = os.environ.get("SMCX_LIBRARY") or os.path.join(_HERE, "libsmcx.so")  # override: a differently built libsmcx
 _HEADER = os.path.join(os.path.dirname(_HERE), "include", "smcx.h")
 _lib = None
 
@@ -49,7 +49,7 @@ def load_library(build_if_missing: bool = True):
     global _lib
     if _lib is not None:
         return _lib
-    if build_if_missing:
+    if build_if_missing and not os.environ.get("SMCX_LIBRARY"):
         from . import build as _build
         try:
             _build.build()

@@ -148,7 +148,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   G.accept_len = p->accept_len;
   G.trace_capacity = p->trace_capacity > 0 ? p->trace_capacity : 65536;
   G.filter_E = -1;
-  set_thread_masks(G);
+  set_thread_masks(G);  // needs key0/key1
   // tile-linear deltas
   for (int b = 0; b < G.B; ++b) {
     int bp[3];

@@ -38,6 +38,14 @@ __host__ __device__ __forceinline__ Philox4 philox4x32_10(uint32_t c0, uint32_t 
   return Philox4{c0, c1, c2, c3};
 }
 
+// Same generator with the ten round keys precomputed (Geom::rk0 / rk1).
+__device__ __forceinline__ Philox4 philox4x32_10_rk(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                    const uint32_t* rk0, const uint32_t* rk1) {
+#pragma unroll
+  for (int r = 0; r < 10; ++r) philox_round(c0, c1, c2, c3, rk0[r], rk1[r]);
+  return Philox4{c0, c1, c2, c3};
+}
+
 __host__ __device__ __forceinline__ uint32_t mulhi_u32(uint32_t a, uint32_t b) {
 #ifdef __CUDA_ARCH__
   return __umulhi(a, b);
@@ -80,6 +88,10 @@ struct Geom {
   int filter_nq;
   // bit masks handed over as parameters so that ptxas keeps them in registers (one LOP3 per term)
   uint32_t kH, kM1, kF1, kH2, kM2, kF2;
+  // Philox round keys key + r * (W0, W1), r = 0..9, and multipliers 2^1, 2^2, 2^3, 2^31: operands
+  // taken straight from the constant bank (no per-call key schedule, right shifts as IMAD.HI)
+  uint32_t rk0[10], rk1[10];
+  uint32_t mul2, mul4, mul8, mul_half;
   // all shells concatenated, shell by shell, each in ascending (dz,dy,dx) order
   signed char off[kMaxNeighbours][3];   // half-lattice units
   unsigned char shell_of[kMaxNeighbours];

@@ -26,7 +26,19 @@
 
 namespace smcxk {
 
-constexpr int kThreadNT = 256;          // threads (= cells) per block
+#ifndef SMCX_NT
+#define SMCX_NT 256
+#endif
+#ifndef SMCX_BLOCKS_PER_SM
+#define SMCX_BLOCKS_PER_SM 3
+#endif
+#ifndef SMCX_OPT_RK
+#define SMCX_OPT_RK 1   // Philox round keys from the constant bank
+#endif
+#ifndef SMCX_OPT_HI
+#define SMCX_OPT_HI 0   // (measured slower: IMAD.HI issues at half the IMAD rate)  direction bits and U >> 1 via IMAD.HI (FMA pipe) instead of SHF (ALU pipe)
+#endif
+constexpr int kThreadNT = SMCX_NT;      // threads (= cells) per block
 constexpr int kThreadTileWords = 64;    // 8 x 8 rows of one word
 constexpr int kCoefInts = 8;            // per (a,b): cl0 ch0 cb0 cl1 | ch1 cb1 corr' pad
 constexpr int kFilterTr = 64;           // Tr[r] = T[r], r < 64
@@ -84,6 +96,11 @@ inline void set_thread_masks(Geom& G) {
   // shell 1 = [v_i | v_j | own-row fields of i at bits 16,24 and of j at bits 18,26]
   G.kH = 0xFFFF0000u; G.kM1 = 0x55555555u; G.kF1 = 0x55550000u;
   G.kH2 = 0x0C0CFF00u; G.kM2 = 0x05055555u; G.kF2 = 0x04045500u;
+  for (int r = 0; r < 10; ++r) {
+    G.rk0[r] = G.key0 + (uint32_t)r * 0x9E3779B9u;
+    G.rk1[r] = G.key1 + (uint32_t)r * 0xBB67AE85u;
+  }
+  G.mul2 = 2u; G.mul4 = 4u; G.mul8 = 8u; G.mul_half = 0x80000000u;
 }
 
 __device__ __forceinline__ uint32_t lop3_maj(uint32_t a, uint32_t b, uint32_t c) {
@@ -117,8 +134,13 @@ __device__ __forceinline__ void gather_site(const uint32_t* p, int s0, uint32_t 
 // U holds 2-bit fields; those selected by H belong to j, the others to i; M marks the low bit of
 // every field, F = M & H.  Returns for lo bits, hi bits and lo&hi the merged population counts
 // (count over i's fields) - (count over j's fields) + (number of j fields).
-__device__ __forceinline__ void count3(uint32_t U, uint32_t H, uint32_t M, uint32_t F, int& plo, int& phi, int& pbt) {
-  const uint32_t Us = U >> 1;
+__device__ __forceinline__ void count3(uint32_t U, uint32_t half, uint32_t H, uint32_t M, uint32_t F, int& plo,
+                                       int& phi, int& pbt) {
+#if SMCX_OPT_HI
+  const uint32_t Us = __umulhi(U, half);     // U >> 1 on the FMA pipe (half = 2^31)
+#else
+  const uint32_t Us = U >> 1; (void)half;
+#endif
   const uint32_t tl = (U ^ H) & M;           // lo bits; complemented in j's fields
   const uint32_t th = (Us ^ H) & M;          // hi bits; complemented in j's fields
   const uint32_t tb = lop3_maj(tl, th, F);   // lo & hi for i, ~(lo & hi) for j
@@ -135,9 +157,15 @@ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const
   constexpr int bj = 1 - bi;
   constexpr int s0_i = 4 * X + 2 * bi;
   // direction: top three bits of the draw (= mulhi(w_dir, 8)); dx = bit 0, dy = bit 1, dz = bit 2
+#if SMCX_OPT_HI
+  const int t1 = (int)__umulhi(w_dir, G.mul4);            // w_dir >> 30 = dy + 2 dz   (IMAD.HI: FMA pipe)
+  const int dz = (int)__umulhi(w_dir, G.mul2);            // w_dir >> 31
+  const int dir = (int)__umulhi(w_dir, G.mul8);           // w_dir >> 29
+#else
   const int t1 = (int)(w_dir >> 30);                      // dy + 2 dz
   const int dz = (int)(w_dir >> 31);
   const int dir = (int)(w_dir >> 29);
+#endif
   const int rd = t1 + 6 * dz - 9 * (1 - bi);              // row_j - row_i = (dy-1+bi) + 8 (dz-1+bi)
   const int s0_j = (4 * X + 4 * bi + 2 * bj - 4) + 4 * dir - 8 * t1;   // 4 (X-1+bi+dx) + 2 bj
   const uint32_t p1_j = 1u << (s0_j - 4);
@@ -151,8 +179,8 @@ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const
   const uint32_t U1 = n01i + n23i * 256u + n01j * 65536u + n23j * 16777216u;
   const uint32_t U2 = vi + vj * 256u + (t_i & 0x303u) * 65536u + (t_j & 0x303u) * 262144u;
   int p1l, p1h, p1b, p2l, p2h, p2b;
-  count3(U1, G.kH, G.kM1, G.kF1, p1l, p1h, p1b);
-  count3(U2, G.kH2, G.kM2, G.kF2, p2l, p2h, p2b);
+  count3(U1, G.mul_half, G.kH, G.kM1, G.kF1, p1l, p1h, p1b);
+  count3(U2, G.mul_half, G.kH2, G.kM2, G.kF2, p2l, p2h, p2b);
   const int dE = c1.z + c0.x * p1l + c0.y * p1h + c0.z * p1b + c0.w * p2l + c1.x * p2h + c1.y * p2b;
   bool ok;
   if (kFilter) {
@@ -178,7 +206,7 @@ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const
 }
 
 template <bool kFilter>
-__global__ void __launch_bounds__(kThreadNT, 3)
+__global__ void __launch_bounds__(kThreadNT, SMCX_BLOCKS_PER_SM)
 sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* __restrict__ coef,
                       const uint32_t* __restrict__ accept, const uint32_t* __restrict__ filt,
                       DevState* __restrict__ st, int colour) {
@@ -191,10 +219,10 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
   __shared__ int s_dE[NT / 32];
   __shared__ unsigned s_acc[NT / 32];
   // coefficient rows replicated over the 8 lane slots of a quarter warp: conflict-free LDS.128
-  if (threadIdx.x < 128) {
-    const int ent = threadIdx.x >> 3;
-    s_coef0[threadIdx.x] = coef[ent * 2];
-    s_coef1[threadIdx.x] = coef[ent * 2 + 1];
+  for (int k = threadIdx.x; k < 128; k += NT) {
+    const int ent = k >> 3;
+    s_coef0[k] = coef[ent * 2];
+    s_coef1[k] = coef[ent * 2 + 1];
   }
   if (kFilter)
     for (int k = threadIdx.x; k < kFilterWords; k += NT) s_filt[k] = filt[k];
@@ -217,6 +245,8 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
     const int wlo = x0 >> 3, sh = 4 * (x0 & 7);
     const int whi = wlo + 1 == rw ? 0 : wlo + 1;
     // a3: stage the tile (funnel-shift two aligned words per row into one tile word)
+    const uint32_t* lat_lo = lattice + wlo;
+    const uint32_t* lat_hi = lattice + whi;
 #pragma unroll 2
     for (int rz = 0; rz < 8; ++rz) {
       int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
@@ -224,9 +254,9 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
 #pragma unroll
       for (int ry = 0; ry < 8; ++ry) {
         int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
-        const uint32_t* rowp = lattice + ((long long)gz * G.Ly + gy) * rw;
-        lo[ry] = rowp[wlo];
-        hi[ry] = sh ? rowp[whi] : 0u;
+        const size_t roff = (size_t)((uint32_t)(gz * G.Ly + gy)) * (uint32_t)rw;   // row index fits 32 bits
+        lo[ry] = lat_lo[roff];
+        hi[ry] = sh ? lat_hi[roff] : 0u;
       }
 #pragma unroll
       for (int ry = 0; ry < 8; ++ry) tile[(rz * 8 + ry) * NT] = __funnelshift_r(lo[ry], hi[ry], sh);
@@ -241,28 +271,51 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
       const uint32_t q0 = (uint32_t)lzy * 4u;
 #define SMCX_TRIAL_PAIR(LX)                                                                                   \
       {                                                                                                       \
-        const Philox4 r = philox4x32_10(cell_id, q0 + LX, t, ctr3, G.key0, G.key1);                           \
+        const Philox4 r = SMCX_OPT_RK ? philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1)             \
+                                      : philox4x32_10(cell_id, q0 + LX, t, ctr3, G.key0, G.key1);             \
         trial_thread<0, LX + 2, kFilter>(G, p_row, coef_base, s_filt, accept, r.x, r.y, esum, nacc);          \
         trial_thread<1, LX + 2, kFilter>(G, p_row, coef_base, s_filt, accept, r.z, r.w, esum, nacc);          \
       }
       SMCX_TRIAL_PAIR(0) SMCX_TRIAL_PAIR(1) SMCX_TRIAL_PAIR(2) SMCX_TRIAL_PAIR(3)
 #undef SMCX_TRIAL_PAIR
     }
-    // a7: write back tile rows 1..6 x 1..6; only the bytes that lie wholly inside this tile and
-    // can hold a modified site (conventional cells 1..6 of the row)
-    const int rb = G.Lx >> 1;                                   // bytes per lattice row
-    const bool odd = x0 & 1;
-    const int nbytes = odd ? 3 : 4;
-    const int byte0 = (x0 + (odd ? 1 : 0)) >> 1;
-    for (int rz = 1; rz < 7; ++rz) {
-      int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
-      for (int ry = 1; ry < 7; ++ry) {
-        int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
-        unsigned char* rowb = reinterpret_cast<unsigned char*>(lattice) + ((long long)gz * G.Ly + gy) * rb;
-        const uint32_t wv = tile[(rz * 8 + ry) * NT] >> (odd ? 4 : 0);
-        for (int k = 0; k < nbytes; ++k) {
-          int bx = byte0 + k; if (bx >= rb) bx -= rb;
-          rowb[bx] = (unsigned char)((wv >> (8 * k)) & 0xffu);
+    // a7: write back tile rows 1..6 x 1..6; only the bytes that lie wholly inside this tile and can
+    // hold a modified site (conventional cells 1..6 of the row: 4 bytes if x0 is even, else 3), cut
+    // into at most three naturally aligned stores.  The cut depends on x0 mod 8 only, which is the
+    // same for every cell of a pass, so the branches below are uniform.
+    {
+      const int rb = G.Lx >> 1;                                 // bytes per lattice row (multiple of 4)
+      const bool odd = x0 & 1;
+      int pos = (x0 + (odd ? 1 : 0)) >> 1;                      // first byte, before wrapping
+      int rem = odd ? 3 : 4, done = 0, nseg = 0;
+      int seg_sz[3] = {0, 0, 0}, seg_sh[3] = {0, 0, 0};
+      unsigned char* seg_p[3] = {nullptr, nullptr, nullptr};
+#pragma unroll
+      for (int k = 0; k < 3; ++k) {
+        if (rem > 0) {
+          const int sz = ((pos & 3) == 0 && rem >= 4) ? 4 : (((pos & 1) == 0 && rem >= 2) ? 2 : 1);
+          seg_sz[k] = sz;
+          seg_sh[k] = 8 * done + (odd ? 4 : 0);
+          seg_p[k] = reinterpret_cast<unsigned char*>(lattice) + (pos >= rb ? pos - rb : pos);
+          pos += sz; rem -= sz; done += sz; nseg = k + 1;
+        }
+      }
+      for (int rz = 1; rz < 7; ++rz) {
+        int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
+#pragma unroll
+        for (int ry = 1; ry < 7; ++ry) {
+          int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
+          const size_t roff = (size_t)((uint32_t)(gz * G.Ly + gy)) * (uint32_t)rb;
+          const uint32_t wv = tile[(rz * 8 + ry) * NT];
+#pragma unroll
+          for (int k = 0; k < 3; ++k) {
+            if (k < nseg) {
+              const uint32_t val = wv >> seg_sh[k];
+              if (seg_sz[k] == 4) *reinterpret_cast<uint32_t*>(seg_p[k] + roff) = val;
+              else if (seg_sz[k] == 2) *reinterpret_cast<uint16_t*>(seg_p[k] + roff) = (uint16_t)val;
+              else seg_p[k][roff] = (unsigned char)val;
+            }
+          }
         }
       }
     }
