@@ -297,15 +297,13 @@ def run_cuda(args, cfg, rank, world, local_rank):
         # dominant kernel: one colour pass = n_sites/8 trials per launch, 8 launches per sweep
         launch_ms = sweep_ms / (8.0 * args.steps)
         achieved = ALGO_BYTES_PER_TRIAL * (cfg.n_sites / 8.0) / (launch_ms * 1e-3) / 1e9
-        traffic = None
-        tp = os.path.join(ROOT, "profiles", "dram_traffic_per_launch.json")
+        traffic = None   # measured dram bytes per launch from the committed ncu capture, if it matches this run
+        tp = os.path.join(ROOT, "profiles", "dram_traffic.csv")
         if os.path.exists(tp):
-            try:
-                rec = json.load(open(tp))
-                if rec.get("workload_sites") == cfg.n_sites and rec.get("kernel") == lat.kernel:
-                    traffic = rec["dram_bytes_per_launch"]
-            except Exception:
-                pass
+            for line in open(tp):
+                f = line.strip().split(",")
+                if len(f) == 3 and f[0].isdigit() and int(f[0]) == lat.kernel and int(f[1]) == cfg.n_sites:
+                    traffic = float(f[2])
         out = {
             "metric": metric_name(), "value": value, "unit": "trial swaps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",

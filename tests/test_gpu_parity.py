@@ -22,7 +22,7 @@ def _supported(cfg, kernel):
 
 def _pair(cfg, kernel=smcx.KERNEL_AUTO, **over):
     g = smcx.Lattice.from_config(cfg, kernel=kernel, **over)
-    o = oracle.Oracle.from_config(cfg, **{k: v for k, v in over.items() if k in ("seed", "link_cell")})
+    o = oracle.Oracle.from_config(cfg, **{k: v for k, v in over.items() if k in ("seed", "link_cell", "epi", "accept")})
     return g, o
 
 
@@ -254,3 +254,52 @@ def test_energy_trace_ring_and_ranges():
         g.energy_trace(0, 6)       # sweeps 0-1 are no longer retained
     with pytest.raises(smcx.SmcxError):
         g.energy_trace(5, 3)       # beyond the sweeps done
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+@pytest.mark.parametrize("kind", ["staircase", "short", "non_monotone", "long_kT"])
+def test_arbitrary_threshold_tables(kernel, kind):
+    """The threshold table is input data: the library must take the same decisions as `u < T[dE]` for
+    any table, including ones that are not of the exp(-d/kT) form (the thread kernel's two-level
+    filter must then be refused by the host-side check and the exact look-up used)."""
+    cfg = scaled_config(1, (16, 24, 16))
+    rng = np.random.default_rng(11)
+    if kind == "staircase":
+        table = np.repeat(np.sort(rng.integers(0, 2 ** 32, 40, dtype=np.uint64))[::-1], 100).astype(np.uint32)
+    elif kind == "short":
+        table = make_accept_table(600)[:37].copy()          # truncated: dE >= 37 is always rejected
+    elif kind == "non_monotone":
+        table = rng.integers(0, 2 ** 32, 5000, dtype=np.uint64).astype(np.uint32)
+    else:
+        table = make_accept_table(2900)                     # 64,325 entries: longer than the filter covers
+    g = smcx.Lattice.from_config(cfg, kernel=kernel, accept=table)
+    o = oracle.Oracle.from_config(cfg, accept=table)
+    g.sweep(4)
+    o.sweep(4)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.stats() == o.stats()
+    # and back to a regular table on the same handles
+    table2 = make_accept_table(430)
+    g.set_temperature(430, table2)
+    o.set_temperature(table2)
+    g.sweep(3)
+    o.sweep(3)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+
+
+def test_large_epi_values_thread_kernel():
+    """int32 EPI far beyond the configs' range (|V| up to 6e4, dE up to ~1e6) with the longest table the
+    library reserves room for (2^20 entries): coefficients and dE stay exact."""
+    cfg = scaled_config(1, (16, 16, 16))
+    epi = make_epi(2, 4, 60_000, 77)
+    table = make_accept_table(45_000)
+    assert 900_000 < table.size <= 1 << 20
+    for kernel in KERNELS:
+        g = smcx.Lattice.from_config(cfg, kernel=kernel, epi=epi, accept=table)
+        o = oracle.Oracle.from_config(cfg, epi=epi, accept=table)
+        g.sweep(3)
+        o.sweep(3)
+        _assert_same_state(g, o)
+        assert (g.energy_trace() == o.energy_trace()).all()
