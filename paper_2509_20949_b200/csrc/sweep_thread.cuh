@@ -182,22 +182,25 @@ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const
   count3(U1, G.mul_half, G.kH, G.kM1, G.kF1, p1l, p1h, p1b);
   count3(U2, G.mul_half, G.kH2, G.kM2, G.kF2, p2l, p2h, p2b);
   const int dE = c1.z + c0.x * p1l + c0.y * p1h + c0.z * p1b + c0.w * p2l + c1.x * p2h + c1.y * p2b;
+  // Eq. 3 in integer form.  in_tab: 0 < dE < len (one unsigned compare).
+  const bool in_tab = (uint32_t)(dE - 1) < (uint32_t)(G.accept_len - 1);
   bool ok;
   if (kFilter) {
     // two-level threshold: ta <= T[dE] <= ta + E; tables are zero beyond the last entry and the
     // indices are masked, so every lane can evaluate it whatever its dE
     const uint32_t ta = __umulhi(s_filt[kFilterTr + (((uint32_t)dE >> 6) & (kFilterMaxTq - 1))], s_filt[dE & 63]);
-    const bool in_table = dE < G.accept_len;
-    ok = dE <= 0 || (in_table && u < ta);
-    if (!ok && in_table && u - ta <= (uint32_t)G.filter_E) ok = u < __ldg(accept + dE);   // rare exact look-up
+    ok = dE <= 0 || (in_tab && u < ta);
+    if (in_tab && u - ta <= (uint32_t)G.filter_E) ok = u < __ldg(accept + dE);   // u in [ta, ta+E]: rare exact look-up
   } else {
     ok = dE <= 0;
-    if (!ok && dE < G.accept_len) ok = u < __ldg(accept + dE);
+    if (in_tab) ok = u < __ldg(accept + dE);
   }
-  if (ok && a4 != b4) {
-    const uint32_t x4 = a4 ^ b4;
-    const uint32_t new_i = own_i ^ (x4 << (s0_i - 4));
-    const uint32_t new_j = (rd == 0 ? new_i : own_j) ^ (x4 * p1_j);
+  // swap by arithmetic on the FMA pipe: the field of i holds a and becomes b, that of j holds b
+  // and becomes a, so the row words change by +-(b - a) << position
+  const int d4 = (int)b4 - (int)a4;
+  if (ok && d4 != 0) {
+    const uint32_t new_i = own_i + (uint32_t)d4 * (1u << (s0_i - 4));
+    const uint32_t new_j = (rd == 0 ? new_i : own_j) - (uint32_t)d4 * p1_j;
     p_i[0] = new_i;
     p_j[0] = new_j;
     esum += dE;
