@@ -245,8 +245,11 @@ def run_cuda(args, cfg, rank, world, local_rank):
         chunk = min(sro_every - (done % sro_every), args.steps - done)
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record()
-        for t in range(chunk):
-            one_step(args.warmup + done + t)
+        if tables is None:
+            lat.sweep(chunk)          # fixed temperature: one call, replayed from the captured sweep graph
+        else:
+            for t in range(chunk):
+                one_step(args.warmup + done + t)
         b.record()
         done += chunk
         c0 = torch.cuda.Event(enable_timing=True); c1 = torch.cuda.Event(enable_timing=True)

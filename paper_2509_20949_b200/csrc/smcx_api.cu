@@ -217,6 +217,12 @@ struct smcx {
   uint8_t* bounce = nullptr;  // device, kChunkSites bytes, lazily allocated
   long long sweeps_enqueued = 0;
   long long launches = 0;
+  // one sweep (8 colour passes + epilogue) captured as a CUDA graph; re-captured when the kernel
+  // parameters change (new threshold table)
+  cudaStream_t capture_stream = nullptr;
+  cudaGraphExec_t sweep_graph = nullptr;
+  long long params_epoch = 0, graph_epoch = -1;
+  bool graphs_ok = true;
   int sm_count = 148;
   std::string err;
 
@@ -332,6 +338,7 @@ int upload_table(smcx* h, const uint32_t* accept, int len) {
   }
   SMCX_CUDA(h, cudaEventRecord(h->staging_ev[slot], h->stream));
   h->plan.G.accept_len = len;
+  h->params_epoch++;
   return SMCX_OK;
 }
 
@@ -359,6 +366,17 @@ int launch_colour_pass(smcx* h, int colour) {
     sweep_warp_per_cell<2><<<grid, kWarpsPerBlock * 32, sm, h->stream>>>(G, h->d_species(), h->d_epi(), h->d_accept(), h->d_state(), colour);
   else
     sweep_warp_per_cell<4><<<grid, kWarpsPerBlock * 32, sm, h->stream>>>(G, h->d_species(), h->d_epi(), h->d_accept(), h->d_state(), colour);
+  h->launches++;
+  return SMCX_OK;
+}
+
+// One sweep on h->stream: 8 colour passes and the trace/counter epilogue.
+int enqueue_sweep(smcx* h) {
+  for (int colour = 0; colour < 8; ++colour) {
+    const int rc = launch_colour_pass(h, colour);
+    if (rc != SMCX_OK) return rc;
+  }
+  sweep_epilogue<<<1, 1, 0, h->stream>>>(h->d_state(), h->d_trace(), h->plan.G.trace_capacity);
   h->launches++;
   return SMCX_OK;
 }
@@ -438,6 +456,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     if (cudaEventCreateWithFlags(&h->staging_ev[s], cudaEventDisableTiming) != cudaSuccess) return fail(SMCX_E_CUDA);
   }
   if (configure_thread_per_cell() != 0) return fail(SMCX_E_CUDA);
+  if (cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); h->capture_stream = nullptr; }
   {
     const Geom& G = h->plan.G;
     const int n2 = G.n_species * G.n_species;
@@ -479,6 +498,8 @@ void smcx_destroy(smcx_t* h) {
     if (h->staging[s]) cudaFreeHost(h->staging[s]);
     if (h->staging_ev[s]) cudaEventDestroy(h->staging_ev[s]);
   }
+  if (h->sweep_graph) cudaGraphExecDestroy(h->sweep_graph);
+  if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
   if (h->bounce) cudaFree(h->bounce);
   if (h->owns_ws && h->ws) cudaFree(h->ws);
   cudaGetLastError();
@@ -538,13 +559,39 @@ int smcx_set_temperature(smcx_t* h, int32_t kT_units, const uint32_t* accept, in
 int smcx_sweep(smcx_t* h, int64_t n) {
   if (!h) return SMCX_E_NULL_ARG;
   if (n < 0 || h->sweeps_enqueued + n > 0xffffffffll) return SMCX_E_RANGE;  // t is a 32-bit counter word
-  for (int64_t s = 0; s < n; ++s) {
-    for (int colour = 0; colour < 8; ++colour) {
-      const int rc = launch_colour_pass(h, colour);
-      if (rc != SMCX_OK) return rc;
+  // Runs of sweeps at fixed parameters are replayed from a captured graph of one sweep (the kernels
+  // read the sweep counter from device memory, so the same graph serves every sweep).
+  if (n >= 3 && h->graphs_ok && h->capture_stream) {
+    if (h->graph_epoch != h->params_epoch) {
+      if (h->sweep_graph) { cudaGraphExecDestroy(h->sweep_graph); h->sweep_graph = nullptr; }
+      cudaGraph_t graph = nullptr;
+      cudaStream_t user = h->stream;
+      bool ok = cudaStreamBeginCapture(h->capture_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess;
+      if (ok) {
+        const long long launches_before = h->launches;
+        h->stream = h->capture_stream;
+        ok = enqueue_sweep(h) == SMCX_OK;
+        h->stream = user;
+        h->launches = launches_before;
+        ok = (cudaStreamEndCapture(h->capture_stream, &graph) == cudaSuccess) && ok && graph;
+      }
+      if (ok) ok = cudaGraphInstantiate(&h->sweep_graph, graph, 0) == cudaSuccess;
+      if (graph) cudaGraphDestroy(graph);
+      if (!ok) { cudaGetLastError(); h->graphs_ok = false; h->sweep_graph = nullptr; }
+      else h->graph_epoch = h->params_epoch;
     }
-    sweep_epilogue<<<1, 1, 0, h->stream>>>(h->d_state(), h->d_trace(), h->plan.G.trace_capacity);
-    h->launches++;
+    if (h->sweep_graph) {
+      for (int64_t s = 0; s < n; ++s) {
+        SMCX_CUDA(h, cudaGraphLaunch(h->sweep_graph, h->stream));
+        h->launches += 9;
+        h->sweeps_enqueued++;
+      }
+      return SMCX_OK;
+    }
+  }
+  for (int64_t s = 0; s < n; ++s) {
+    const int rc = enqueue_sweep(h);
+    if (rc != SMCX_OK) return rc;
     h->sweeps_enqueued++;
   }
   SMCX_CUDA(h, cudaGetLastError());

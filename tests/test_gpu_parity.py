@@ -142,6 +142,34 @@ def test_config4_full_size_invariants(kernel):
 
 
 @pytest.mark.slow
+def test_config5_shape_at_400_cubed():
+    """Config 5's parameters on 400^3 cells (1.28e8 sites): the oracle cannot reach 1.6e10 sites in
+    reasonable time, so parity is checked on the same build at this size and invariants at full
+    size (test_config5_full_size_invariants)."""
+    cfg = scaled_config(5, (400, 400, 400))
+    g, o = _pair(cfg)
+    g.sweep(1)
+    o.sweep(1)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+
+
+@pytest.mark.slow
+def test_config5_full_size_invariants():
+    cfg = get_config(5)
+    g = smcx.Lattice.from_config(cfg)
+    _, c0 = g.sro()
+    n_p = c0[0].sum(axis=1) // 8
+    assert (n_p == cfg.n_sites // 4).all()
+    assert g.energy() == g.running_energy()
+    g.sweep(3)
+    _, c1 = g.sro()
+    assert (c1[0].sum(axis=1) // 8 == n_p).all()
+    assert g.energy() == g.running_energy() == g.energy_trace()[-1]
+    assert int((cfg.epi().astype(np.int64) * c1).sum()) == 2 * g.energy()
+
+
+@pytest.mark.slow
 @pytest.mark.parametrize("k,n", [(4, 1), (3, 20)])
 def test_full_size_oracle_prefix(k, n):
     cfg = get_config(k)
