@@ -166,7 +166,11 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   plan->n_cells = n_cells;
 
   // kernel / storage choice
-  const bool fast_ok = thread_kernel_supported(G);
+  bool fast_ok = thread_kernel_supported(G);
+  if (fast_ok) {  // the packed kernel computes dE in int32 from a coefficient table: magnitudes must fit
+    int32_t coef[16 * kCoefInts];
+    fast_ok = build_thread_coefficients(p->epi, n, coef);
+  }
   int kernel = p->kernel, storage = p->storage;
   if (kernel == SMCX_KERNEL_AUTO) {
     if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_WARP_PER_CELL;

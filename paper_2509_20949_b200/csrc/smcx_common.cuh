@@ -86,12 +86,9 @@ struct Geom {
   // filter_E < 0, else T[d] - mulhi(Tq[d>>6], Tr[d&63]) lies in [0, filter_E] for every d.
   int filter_E;
   int filter_nq;
-  // bit masks handed over as parameters so that ptxas keeps them in registers (one LOP3 per term)
-  uint32_t kH, kM1, kF1, kH2, kM2, kF2;
-  // Philox round keys key + r * (W0, W1), r = 0..9, and multipliers 2^1, 2^2, 2^3, 2^31: operands
-  // taken straight from the constant bank (no per-call key schedule, right shifts as IMAD.HI)
+  // Philox round keys key + r * (W0, W1), r = 0..9: operands taken straight from the constant
+  // bank (no per-call key schedule)
   uint32_t rk0[10], rk1[10];
-  uint32_t mul2, mul4, mul8, mul_half;
   // all shells concatenated, shell by shell, each in ascending (dz,dy,dx) order
   signed char off[kMaxNeighbours][3];   // half-lattice units
   unsigned char shell_of[kMaxNeighbours];

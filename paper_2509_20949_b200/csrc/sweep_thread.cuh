@@ -3,24 +3,29 @@
 //
 // Layout facts this kernel rests on:
 //  * a row of 8 conventional cells (both sublattices) is exactly one 32-bit word: conventional
-//    cell X sits in bits [4X, 4X+4), its corner site in the low two, its body site in the high two;
+//    cell X is nibble X, its corner site the low two bits, its body site the high two;
 //  * with w = 4 the LIZ+ tile is 8^3 conventional cells = 64 such words, and the tiles of the
 //    cells of one colour tile the whole lattice exactly once, so a pass streams the lattice
 //    through shared memory once and no two threads ever touch the same tile;
 //  * the tile of thread t is kept at smem[row * NT + t]: every access of a warp hits 32 distinct
 //    banks whatever row each lane addresses (lanes differ in the direction they drew);
-//  * the 8 + 6 neighbour species of a site are gathered into two 16-bit words of 2-bit fields and
-//    reduced with population counts: with species x = lo + 2 hi,
+//  * the neighbours of a site sit in at most two adjacent nibbles of four (shell 0) or five
+//    (shell 1) rows.  They are gathered with byte permutes (PRMT) of 16-bit windows and one
+//    bit-select per four rows; because the neighbours of i and of j lie on opposite sublattices,
+//    the gathered words of i and (complemented) j interleave into one dense word per shell with a
+//    single three-input logic operation.  Population counts then give, with species x = lo + 2 hi,
 //      D_s(x) = V_s(b,x) - V_s(a,x) = D_s(0) + lo cl_s + hi ch_s + lo hi cb_s,
-//    so dE = sum_s [cl_s dlo_s + ch_s dhi_s + cb_s dboth_s] + corr(a,b) with d* the differences of
-//    the bit counts around i and around j and corr = 2 V_0(a,b) - V_0(a,a) - V_0(b,b) undoing
-//    the i-j bond that both sums include.  Integer arithmetic throughout: results are bit-identical
-//    to the plain before/after energy difference.
-//  * the integer pipe (LOP3/SHF) is the binding unit (ncu: profiles/), so the code is arranged to
-//    keep its instruction count down: fused three-input logic with masks held in registers,
-//    merges by multiply-add on the FMA pipe, coefficient tables replicated per lane slot so that
-//    the 128-bit loads are conflict-free, and a two-level acceptance filter in shared memory.
+//    dE = sum_s [cl_s dlo_s + ch_s dhi_s + cb_s dboth_s] + corr(a,b), d* the differences of the
+//    bit counts around i and around j, corr = 2 V_0(a,b) - V_0(a,a) - V_0(b,b) undoing the i-j
+//    bond that both sums include.  Integer arithmetic throughout: results are bit-identical to
+//    the plain before/after energy difference;
+//  * the site i of a trial is known at compile time (the 128 slots are unrolled per x-row), only
+//    the direction is per lane: its y/z bits select rows (shared-memory addresses), its x bit
+//    selects between two sets of masks (one multiply-add per mask on the FMA pipe).
+//  * the integer pipe (LOP3/SHF/PRMT/ISETP) is the binding unit (ncu: profiles/), so everything
+//    is arranged to keep its instruction count down.
 #pragma once
+#include <cstdlib>
 #include "smcx_common.cuh"
 #include "sweep_warp.cuh"
 
@@ -32,182 +37,240 @@ namespace smcxk {
 #ifndef SMCX_BLOCKS_PER_SM
 #define SMCX_BLOCKS_PER_SM 3
 #endif
-#ifndef SMCX_OPT_RK
-#define SMCX_OPT_RK 1   // Philox round keys from the constant bank
-#endif
-#ifndef SMCX_OPT_HI
-#define SMCX_OPT_HI 0   // (measured slower: IMAD.HI issues at half the IMAD rate)  direction bits and U >> 1 via IMAD.HI (FMA pipe) instead of SHF (ALU pipe)
-#endif
 constexpr int kThreadNT = SMCX_NT;      // threads (= cells) per block
 constexpr int kThreadTileWords = 64;    // 8 x 8 rows of one word
-constexpr int kCoefInts = 8;            // per (a,b): cl0 ch0 cb0 cl1 | ch1 cb1 corr' pad
+constexpr int kCoefInts = 8;            // per (a,b): cl0 ch0' cb0 cl1 | ch1' cb1 corr' pad
 constexpr int kFilterTr = 64;           // Tr[r] = T[r], r < 64
-constexpr int kFilterMaxTq = 1024;      // Tq[q] = T[64 q]; tables up to 65,536 entries (power of two: indices are masked)
+constexpr int kFilterMaxTq = 1024;      // Tq[q] = T[64 q]
 constexpr int kFilterWords = kFilterTr + kFilterMaxTq;
+constexpr int kFilterDmax = 64 * kFilterMaxTq - 1;   // dE is clamped to [0, kFilterDmax] before the look-up
+constexpr int32_t kSameSpecies = 1 << 29;            // "dE" of a trial between equal species: never accepted
+constexpr long long kCoefBudget = 1ll << 28;         // bound on |dE| the coefficient table may produce
 
 inline bool thread_kernel_supported(const Geom& G) {
   return G.lattice == 0 && G.n_shells == 2 && G.w == 4 && G.n_species <= 4 && G.H == 2 && G.TW == 8;
 }
 
-// Host: coefficient table from the EPI tables, [a*4+b][8] int32.
-inline void build_thread_coefficients(const int32_t* epi, int n_species, int32_t* coef /*16*8*/) {
-  auto V = [&](int s, int a, int b) -> int32_t {
-    return (a < n_species && b < n_species) ? epi[(s * n_species + a) * n_species + b] : 0;
+// Host: coefficient table from the EPI tables, [a*4+b][8] int32.  With PT / PH / PB the population
+// counts of trial_thread (all fields, high bits, both bits; j's fields complemented, Z_s of them):
+//   dE = corr' + sum_s cl_s PT_s + (ch_s - cl_s) PH_s + cb_s PB_s,
+//   corr' = corr - sum_s Z_s (cl_s + ch_s + cb_s).
+// Entries with a == b hold kSameSpecies in corr' and zeros elsewhere.  Returns false if the
+// magnitudes could overflow the int32 arithmetic of the kernel.
+inline bool build_thread_coefficients(const int32_t* epi, int n_species, int32_t* coef /*16*8*/) {
+  auto V = [&](int s, int a, int b) -> long long {
+    return (a < n_species && b < n_species) ? (long long)epi[(s * n_species + a) * n_species + b] : 0ll;
   };
   const int Z[2] = {8, 6};
+  bool fits = true;
   for (int a = 0; a < 4; ++a)
     for (int b = 0; b < 4; ++b) {
       int32_t* c = coef + (a * 4 + b) * kCoefInts;
-      int32_t corr = 2 * V(0, a, b) - V(0, a, a) - V(0, b, b);
+      for (int k = 0; k < kCoefInts; ++k) c[k] = 0;
+      if (a == b) { c[6] = kSameSpecies; continue; }
+      long long corr = 2 * V(0, a, b) - V(0, a, a) - V(0, b, b);
+      long long budget = 0;
       for (int s = 0; s < 2; ++s) {
-        int32_t D[4];
+        long long D[4];
         for (int x = 0; x < 4; ++x) D[x] = V(s, b, x) - V(s, a, x);
-        const int32_t cl = D[1] - D[0], ch = D[2] - D[0], cb = D[3] - D[1] - D[2] + D[0];
-        c[3 * s + 0] = cl; c[3 * s + 1] = ch; c[3 * s + 2] = cb;
-        // the merged population counts carry an offset of Z_s per term (see count3)
+        const long long cl = D[1] - D[0], ch = D[2] - D[0], cb = D[3] - D[1] - D[2] + D[0];
+        c[3 * s + 0] = (int32_t)cl; c[3 * s + 1] = (int32_t)(ch - cl); c[3 * s + 2] = (int32_t)cb;
         corr -= Z[s] * (cl + ch + cb);
+        budget += 32 * (std::llabs(cl) + std::llabs(ch - cl) + std::llabs(cb));
       }
-      c[6] = corr;
-      c[7] = 0;
+      c[6] = (int32_t)corr;
+      if (budget + std::llabs(corr) >= kCoefBudget) fits = false;
     }
+  return fits;
 }
 
-// Host: two-level filter tables for a threshold table T.  Returns E >= 0 such that
-// 0 <= T[d] - mulhi(Tq[d>>6], Tr[d&63]) <= E for all d < len, or -1 if no such small bound holds
-// (then the kernel reads T[d] directly).  For T[d] = floor(2^32 exp(-d/kT)) the product of the
-// two floors never exceeds T[d] and falls short by a few units at most.
+// Host: two-level filter tables for a threshold table T (T[d] = 0 understood for d >= len).
+// Returns E >= 0 such that 0 <= T[d] - mulhi(Tq[d>>6], Tr[d&63]) <= E for all d <= kFilterDmax, or
+// -1 if no such small bound holds (then the kernel reads T[d] directly).  For
+// T[d] = floor(2^32 exp(-d/kT)) the product of the two floors never exceeds T[d] and falls short
+// by a few units at most.  The last Tq slot is kept zero: clamped dE values land there.
 inline int build_accept_filter(const uint32_t* T, int len, uint32_t* filt /*kFilterWords*/, int* nq_out) {
   const int nq = (len + 63) / 64;
   *nq_out = nq;
-  if (nq > kFilterMaxTq) return -1;
+  if (nq > kFilterMaxTq - 1) return -1;
   for (int r = 0; r < kFilterTr; ++r) filt[r] = r < len ? T[r] : 0u;
   for (int q = 0; q < kFilterMaxTq; ++q) filt[kFilterTr + q] = q < nq ? T[64 * q] : 0u;
   uint32_t E = 0;
-  for (int d = 0; d < len; ++d) {
+  for (int d = 0; d < 64 * nq; ++d) {
     const uint32_t ta = (uint32_t)(((uint64_t)filt[kFilterTr + (d >> 6)] * filt[d & 63]) >> 32);
-    if (ta > T[d]) return -1;
-    E = T[d] - ta > E ? T[d] - ta : E;
+    const uint32_t td = d < len ? T[d] : 0u;
+    if (ta > td) return -1;
+    E = td - ta > E ? td - ta : E;
   }
   return E <= 1024u ? (int)E : -1;
 }
 
 inline void set_thread_masks(Geom& G) {
-  // count words (see trial_thread): shell 0 = [n01_i n23_i | n01_j n23_j], one byte each;
-  // shell 1 = [v_i | v_j | own-row fields of i at bits 16,24 and of j at bits 18,26]
-  G.kH = 0xFFFF0000u; G.kM1 = 0x55555555u; G.kF1 = 0x55550000u;
-  G.kH2 = 0x0C0CFF00u; G.kM2 = 0x05055555u; G.kF2 = 0x04045500u;
   for (int r = 0; r < 10; ++r) {
     G.rk0[r] = G.key0 + (uint32_t)r * 0x9E3779B9u;
     G.rk1[r] = G.key1 + (uint32_t)r * 0xBB67AE85u;
   }
-  G.mul2 = 2u; G.mul4 = 4u; G.mul8 = 8u; G.mul_half = 0x80000000u;
 }
 
-__device__ __forceinline__ uint32_t lop3_maj(uint32_t a, uint32_t b, uint32_t c) {
-  uint32_t d;
-  asm("lop3.b32 %0, %1, %2, %3, 0xE8;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+// ---- bit helpers (host versions exist so that the trial arithmetic can be unit-tested on the CPU) ----
+__host__ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
+#ifdef __CUDA_ARCH__
+  return __byte_perm(a, b, sel);
+#else
+  const uint64_t ab = ((uint64_t)b << 32) | a;
+  uint32_t d = 0;
+  for (int k = 0; k < 4; ++k) d |= (uint32_t)((ab >> (8 * ((sel >> (4 * k)) & 7u))) & 0xffu) << (8 * k);
   return d;
-}
-
-// Neighbour species of the site of sublattice b whose own 2-bit field sits at bit s0 of the row
-// word at p (p1 = 1 << (s0 - 4)).  Fields are masked in place, merged by multiply-add (FMA pipe)
-// and shifted down once:
-//   n01, n23: shell 0, 4 fields each (the 2x2x2 block of the other sublattice, rows pairwise)
-//   v:        shell 1, the fields at X of the four adjacent rows
-//   t_own:    own row >> (s0 - 4): shell-1 fields of X-1 / X+1 at bits 0 / 8, own species at bit 4
-template <int b>
-__device__ __forceinline__ void gather_site(const uint32_t* p, int s0, uint32_t p1, uint32_t& n01, uint32_t& n23,
-                                            uint32_t& v, uint32_t& own, uint32_t& t_own) {
-  constexpr int NT = kThreadNT;
-  own = p[0];
-  const uint32_t yM = p[-NT], yP = p[NT], zM = p[-8 * NT], zP = p[8 * NT];
-  const uint32_t dg = b ? p[9 * NT] : p[-9 * NT];
-  const uint32_t A = b ? own : dg, Bq = b ? yP : zM, Cq = b ? zP : yM, Dq = b ? dg : own;
-  const uint32_t mA = p1 * 204u;     // 0x33 << (s0 - 2)
-  const uint32_t m0 = p1 * 48u;      // 0x3 << s0
-  n01 = ((A & mA) + (Bq & mA) * 4u) >> (s0 - 2);
-  n23 = ((Cq & mA) + (Dq & mA) * 4u) >> (s0 - 2);
-  v = ((yM & m0) + (yP & m0) * 4u + (zM & m0) * 16u + (zP & m0) * 64u) >> s0;
-  t_own = own >> (s0 - 4);
-}
-
-// U holds 2-bit fields; those selected by H belong to j, the others to i; M marks the low bit of
-// every field, F = M & H.  Returns for lo bits, hi bits and lo&hi the merged population counts
-// (count over i's fields) - (count over j's fields) + (number of j fields).
-__device__ __forceinline__ void count3(uint32_t U, uint32_t half, uint32_t H, uint32_t M, uint32_t F, int& plo,
-                                       int& phi, int& pbt) {
-#if SMCX_OPT_HI
-  const uint32_t Us = __umulhi(U, half);     // U >> 1 on the FMA pipe (half = 2^31)
-#else
-  const uint32_t Us = U >> 1; (void)half;
 #endif
-  const uint32_t tl = (U ^ H) & M;           // lo bits; complemented in j's fields
-  const uint32_t th = (Us ^ H) & M;          // hi bits; complemented in j's fields
-  const uint32_t tb = lop3_maj(tl, th, F);   // lo & hi for i, ~(lo & hi) for j
-  plo = __popc(tl);
-  phi = __popc(th);
-  pbt = __popc(tb);
+}
+// d = f(a, b, c) with the truth table LUT (bit (4 a + 2 b + c) of LUT), one LOP3
+template <int LUT>
+__host__ __device__ __forceinline__ uint32_t lop3(uint32_t a, uint32_t b, uint32_t c) {
+#ifdef __CUDA_ARCH__
+  uint32_t d;
+  asm("lop3.b32 %0, %1, %2, %3, %4;" : "=r"(d) : "r"(a), "r"(b), "r"(c), "n"(LUT));
+  return d;
+#else
+  uint32_t d = 0;
+  for (int k = 0; k < 8; ++k)
+    if ((LUT >> k) & 1) d |= ((k & 4) ? a : ~a) & ((k & 2) ? b : ~b) & ((k & 1) ? c : ~c);
+  return d;
+#endif
+}
+constexpr int kLutSel = 0xE4;      // c ? a : b
+constexpr int kLutSelNotB = 0xB1;  // c ? a : ~b
+constexpr int kLutMaj = 0xE8;      // majority
+constexpr int kLutAndOr = 0xE0;    // a & (b | c)
+__host__ __device__ __forceinline__ int popc32(uint32_t v) {
+#ifdef __CUDA_ARCH__
+  return __popc(v);
+#else
+  return __builtin_popcount(v);
+#endif
+}
+__host__ __device__ __forceinline__ uint32_t ldg_u32(const uint32_t* p) {
+#ifdef __CUDA_ARCH__
+  return __ldg(p);
+#else
+  return *p;
+#endif
 }
 
-template <int bi, int X, bool kFilter>
-__device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const char* coef_base,
-                                             const uint32_t* s_filt, const uint32_t* __restrict__ accept,
-                                             uint32_t w_dir, uint32_t u, int& esum, unsigned& nacc) {
-  constexpr int NT = kThreadNT;
-  constexpr int bj = 1 - bi;
-  constexpr int s0_i = 4 * X + 2 * bi;
+// ---- compile-time description of a trial slot: site i = sublattice bi of tile nibble X ----------
+__host__ __device__ constexpr uint32_t nib_mask(int n) { return 0xFu << (4 * n); }
+__host__ __device__ constexpr uint32_t sel_win_a(int k) { return (uint32_t)(k | ((k + 1) << 4) | ((4 + k) << 8) | ((5 + k) << 12)); }
+__host__ __device__ constexpr uint32_t sel_win_b(int k) { return (uint32_t)((5 + k) | (k << 4) | ((k + 1) << 8) | ((4 + k) << 12)); }
+__host__ __device__ constexpr uint32_t sel_byte(int k) { return (uint32_t)(k | ((4 + k) << 4) | (k << 8) | ((4 + k) << 12)); }
+
+template <int bi, int X>
+struct SlotConst {
+  static constexpr int bj = 1 - bi;
+  static constexpr uint32_t Ci = bi ? 0xCCCCCCCCu : 0x33333333u;   // bits of the fields of sublattice bi
+  static constexpr uint32_t Cj = ~Ci;
+  static constexpr uint32_t kHi = 0xAAAAAAAAu;                     // high bit of every field
+  // shell 0 of i: nibbles n0i, n0i + 1 of four rows (fields of sublattice bj)
+  static constexpr int n0i = X - 1 + bi;
+  static constexpr int ki = (n0i & 1) ? (n0i - 1) / 2 : n0i / 2;   // first byte of the 16-bit window
+  static constexpr uint32_t mi = (n0i & 1) ? 0x0FF00FF0u : 0x00FF00FFu;
+  // shell 0 of j: nibbles X - 1 + dx, X + dx (fields of sublattice bi); window holds X-1, X, X+1
+  static constexpr int kj = (X & 1) ? (X - 1) / 2 : (X - 2) / 2;
+  static constexpr uint32_t mj0 = (X & 1) ? 0x00FF00FFu : 0x0FF00FF0u;
+  static constexpr uint32_t mj1 = mj0 << 4;
+  // shell 1 of i: nibble X of the four adjacent rows, nibbles X - 1 and X + 1 of the own row
+  static constexpr uint32_t s2i = sel_byte(X >> 1);
+  static constexpr uint32_t moi = nib_mask(X - 1) | nib_mask(X + 1);
+  static constexpr uint32_t Mi = ((0x0F0F0F0Fu << (4 * (X & 1))) | moi) & Ci;
+  // shell 1 of j: the same around nibble Xj = X0 + dx
+  static constexpr int X0 = X - 1 + bi;
+  static constexpr uint32_t s2j_f(int dx) { return sel_byte((X0 + dx) >> 1); }
+  static constexpr uint32_t moj_f(int dx) { return nib_mask(X0 + dx - 1) | nib_mask(X0 + dx + 1); }
+  static constexpr uint32_t Mj_f(int dx) { return ((0x0F0F0F0Fu << (4 * ((X0 + dx) & 1))) | moj_f(dx)) & Cj; }
+  static constexpr uint32_t s2j0 = s2j_f(0), s2j1 = s2j_f(1);
+  static constexpr uint32_t moj0 = moj_f(0), moj1 = moj_f(1);
+  static constexpr uint32_t Mj0 = Mj_f(0), Mj1 = Mj_f(1);
+  static constexpr uint32_t swa_i = sel_win_a(ki), swb_i = sel_win_b(ki), swa_j = sel_win_a(kj), swb_j = sel_win_b(kj);
+  // own fields, normalised to bits 4..5
+  static constexpr int shi = 4 * X + 2 * bi - 4;
+  static constexpr int shj0 = 4 * X0 + 2 * bj - 4;                 // + 4 dx
+};
+
+// c0 + dx * (c1 - c0): a per-lane choice between two compile-time constants as one IMAD
+__host__ __device__ __forceinline__ uint32_t pick(uint32_t dx, uint32_t c0, uint32_t c1) {
+  return c0 + dx * (c1 - c0);
+}
+
+// One trial (a4-a6).  p_i points at the tile row of site i (row stride STRIDE words).
+template <int bi, int X, bool kFilter, int STRIDE>
+__host__ __device__ __forceinline__ void trial_thread(uint32_t* p_i, const char* coef_base, const uint32_t* s_filt,
+                                                      const uint32_t* __restrict__ accept, int accept_len,
+                                                      int filter_E, uint32_t w_dir, uint32_t u, int& esum,
+                                                      unsigned& nacc) {
+  using K = SlotConst<bi, X>;
+  constexpr int NT = STRIDE;
   // direction: top three bits of the draw (= mulhi(w_dir, 8)); dx = bit 0, dy = bit 1, dz = bit 2
-#if SMCX_OPT_HI
-  const int t1 = (int)__umulhi(w_dir, G.mul4);            // w_dir >> 30 = dy + 2 dz   (IMAD.HI: FMA pipe)
-  const int dz = (int)__umulhi(w_dir, G.mul2);            // w_dir >> 31
-  const int dir = (int)__umulhi(w_dir, G.mul8);           // w_dir >> 29
-#else
+  const uint32_t dx = (w_dir >> 29) & 1u;
   const int t1 = (int)(w_dir >> 30);                      // dy + 2 dz
   const int dz = (int)(w_dir >> 31);
-  const int dir = (int)(w_dir >> 29);
-#endif
   const int rd = t1 + 6 * dz - 9 * (1 - bi);              // row_j - row_i = (dy-1+bi) + 8 (dz-1+bi)
-  const int s0_j = (4 * X + 4 * bi + 2 * bj - 4) + 4 * dir - 8 * t1;   // 4 (X-1+bi+dx) + 2 bj
-  const uint32_t p1_j = 1u << (s0_j - 4);
   uint32_t* p_j = p_i + rd * NT;
-  uint32_t n01i, n23i, vi, own_i, t_i, n01j, n23j, vj, own_j, t_j;
-  gather_site<bi>(p_i, s0_i, 1u << (s0_i - 4), n01i, n23i, vi, own_i, t_i);
-  gather_site<bj>(p_j, s0_j, p1_j, n01j, n23j, vj, own_j, t_j);
-  const uint32_t a4 = t_i & 0x30u, b4 = t_j & 0x30u;      // species of i and j, times 16
+  // rows around i and j
+  const uint32_t own_i = p_i[0], yMi = p_i[-NT], yPi = p_i[NT], zMi = p_i[-8 * NT], zPi = p_i[8 * NT];
+  const uint32_t dgi = bi ? p_i[9 * NT] : p_i[-9 * NT];
+  const uint32_t own_j = p_j[0], yMj = p_j[-NT], yPj = p_j[NT], zMj = p_j[-8 * NT], zPj = p_j[8 * NT];
+  const uint32_t dgj = bi ? p_j[-9 * NT] : p_j[9 * NT];
+  const uint32_t mul = dx * 15u + 1u;                      // 16^dx: masks that move by one nibble with dx
+  // shell 0: i's rows are own, y-+1, z-+1, diagonal on the side of the other sublattice; j's mirror them
+  const uint32_t Wi = lop3<kLutSel>(prmt(own_i, bi ? yPi : yMi, K::swa_i), prmt(bi ? zPi : zMi, dgi, K::swb_i), K::mi);
+  const uint32_t Wj = lop3<kLutSel>(prmt(own_j, bi ? yMj : yPj, K::swa_j), prmt(bi ? zMj : zPj, dgj, K::swb_j),
+                                    K::mj0 * mul);
+  const uint32_t U1 = lop3<kLutSelNotB>(Wi, Wj, K::Cj);     // i's fields as they are, j's complemented
+  // shell 1
+  const uint32_t n3i = prmt(prmt(yMi, yPi, K::s2i), prmt(zMi, zPi, K::s2i), 0x7610u);
+  const uint32_t W2i = lop3<kLutSel>(own_i, n3i, K::moi);
+  const uint32_t s2j = (K::s2j0 == K::s2j1) ? K::s2j0 : K::s2j0 + dx * (K::s2j1 - K::s2j0);
+  const uint32_t n3j = prmt(prmt(yMj, yPj, s2j), prmt(zMj, zPj, s2j), 0x7610u);
+  const uint32_t W2j = lop3<kLutSel>(own_j, n3j, K::moj0 * mul);
+  const uint32_t MjD = (K::Mj1 == (K::Mj0 << 4)) ? K::Mj0 * mul : pick(dx, K::Mj0, K::Mj1);
+  const uint32_t U2 = lop3<kLutAndOr>(lop3<kLutSelNotB>(W2i, W2j, K::Ci), MjD, K::Mi);
+  // population counts: all field bits, high bits, "both bits" (AND for i, OR of complements for j)
+  const uint32_t h1 = U1 & K::kHi, h2 = U2 & K::kHi;
+  const uint32_t b1 = lop3<kLutMaj>(U1 << 1, h1, K::Ci & K::kHi);
+  const uint32_t b2 = lop3<kLutMaj>(U2 << 1, h2, K::Cj & K::kHi);
+  const int pt1 = popc32(U1), ph1 = popc32(h1), pb1 = popc32(b1);
+  const int pt2 = popc32(U2), ph2 = popc32(h2), pb2 = popc32(b2);
+  // species of i and j (times 16) and the coefficient row of the ordered pair
+  const uint32_t a4 = (own_i >> K::shi) & 0x30u;
+  const uint32_t shj = (uint32_t)K::shj0 + 4u * dx;
+  const uint32_t b4 = (own_j >> shj) & 0x30u;
   const int4 c0 = *reinterpret_cast<const int4*>(coef_base + a4 * 32u + b4 * 8u);            // [(a*4+b)*8 + slot]
   const int4 c1 = *reinterpret_cast<const int4*>(coef_base + 2048 + a4 * 32u + b4 * 8u);
-  const uint32_t U1 = n01i + n23i * 256u + n01j * 65536u + n23j * 16777216u;
-  const uint32_t U2 = vi + vj * 256u + (t_i & 0x303u) * 65536u + (t_j & 0x303u) * 262144u;
-  int p1l, p1h, p1b, p2l, p2h, p2b;
-  count3(U1, G.mul_half, G.kH, G.kM1, G.kF1, p1l, p1h, p1b);
-  count3(U2, G.mul_half, G.kH2, G.kM2, G.kF2, p2l, p2h, p2b);
-  const int dE = c1.z + c0.x * p1l + c0.y * p1h + c0.z * p1b + c0.w * p2l + c1.x * p2h + c1.y * p2b;
-  // Eq. 3 in integer form.  in_tab: 0 < dE < len (one unsigned compare).
-  const bool in_tab = (uint32_t)(dE - 1) < (uint32_t)(G.accept_len - 1);
+  const int dE = c1.z + c0.x * pt1 + c0.y * ph1 + c0.z * pb1 + c0.w * pt2 + c1.x * ph2 + c1.y * pb2;
+  // Eq. 3 in integer form
   bool ok;
   if (kFilter) {
-    // two-level threshold: ta <= T[dE] <= ta + E; tables are zero beyond the last entry and the
-    // indices are masked, so every lane can evaluate it whatever its dE
-    const uint32_t ta = __umulhi(s_filt[kFilterTr + (((uint32_t)dE >> 6) & (kFilterMaxTq - 1))], s_filt[dE & 63]);
-    ok = dE <= 0 || (in_tab && u < ta);
-    if (in_tab && u - ta <= (uint32_t)G.filter_E) ok = u < __ldg(accept + dE);   // u in [ta, ta+E]: rare exact look-up
+    // two-level threshold: ta <= T[dE] <= ta + E for the clamped dE (tables are zero beyond the last
+    // entry; dE <= 0 maps to entry 0, equal species to the zero entry at the top)
+    const uint32_t dc = (uint32_t)min(max(dE, 0), kFilterDmax);
+    const uint32_t ta = mulhi_u32(s_filt[kFilterTr + (dc >> 6)], s_filt[dc & 63u]);
+    ok = u < ta;
+    if (u - ta <= (uint32_t)filter_E)                      // u in [ta, ta+E]: rare exact decision
+      ok = dE <= 0 || (dE < accept_len && u < ldg_u32(accept + dE));
   } else {
     ok = dE <= 0;
-    if (in_tab) ok = u < __ldg(accept + dE);
+    if (dE > 0 && dE < accept_len) ok = u < ldg_u32(accept + dE);
   }
-  // swap by arithmetic on the FMA pipe: the field of i holds a and becomes b, that of j holds b
-  // and becomes a, so the row words change by +-(b - a) << position
-  const int d4 = (int)b4 - (int)a4;
-  if (ok && d4 != 0) {
-    const uint32_t new_i = own_i + (uint32_t)d4 * (1u << (s0_i - 4));
-    const uint32_t new_j = (rd == 0 ? new_i : own_j) - (uint32_t)d4 * p1_j;
-    p_i[0] = new_i;
-    p_j[0] = new_j;
-    esum += dE;
-    ++nacc;
-  }
+  // swap by arithmetic: the field of i holds a and becomes b, that of j holds b and becomes a; a
+  // rejected trial stores the rows back unchanged (no branch)
+  const uint32_t d4 = ok ? b4 - a4 : 0u;
+  const uint32_t new_i = own_i + d4 * (1u << K::shi);
+  const uint32_t new_j = (rd == 0 ? new_i : own_j) - d4 * ((1u << K::shj0) * mul);
+  p_i[0] = new_i;
+  p_j[0] = new_j;
+  esum += ok ? dE : 0;
+  nacc += ok ? 1u : 0u;
 }
 
+#ifdef __CUDACC__
 template <bool kFilter>
 __global__ void __launch_bounds__(kThreadNT, SMCX_BLOCKS_PER_SM)
 sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* __restrict__ coef,
@@ -268,16 +331,16 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
     const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
     const uint32_t ctr3 = TAG_TRIAL | ((uint32_t)colour << 8);
     const char* coef_base = reinterpret_cast<const char*>(s_coef0) + (threadIdx.x & 7) * 16;
+    const int accept_len = G.accept_len, filter_E = G.filter_E;
 #pragma unroll 1
     for (int lzy = 0; lzy < 16; ++lzy) {
       uint32_t* p_row = tile + (((lzy >> 2) + 2) * 8 + (lzy & 3) + 2) * NT;
       const uint32_t q0 = (uint32_t)lzy * 4u;
-#define SMCX_TRIAL_PAIR(LX)                                                                                   \
-      {                                                                                                       \
-        const Philox4 r = SMCX_OPT_RK ? philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1)             \
-                                      : philox4x32_10(cell_id, q0 + LX, t, ctr3, G.key0, G.key1);             \
-        trial_thread<0, LX + 2, kFilter>(G, p_row, coef_base, s_filt, accept, r.x, r.y, esum, nacc);          \
-        trial_thread<1, LX + 2, kFilter>(G, p_row, coef_base, s_filt, accept, r.z, r.w, esum, nacc);          \
+#define SMCX_TRIAL_PAIR(LX)                                                                                          \
+      {                                                                                                              \
+        const Philox4 r = philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1);                                 \
+        trial_thread<0, LX + 2, kFilter, NT>(p_row, coef_base, s_filt, accept, accept_len, filter_E, r.x, r.y, esum, nacc); \
+        trial_thread<1, LX + 2, kFilter, NT>(p_row, coef_base, s_filt, accept, accept_len, filter_E, r.z, r.w, esum, nacc); \
       }
       SMCX_TRIAL_PAIR(0) SMCX_TRIAL_PAIR(1) SMCX_TRIAL_PAIR(2) SMCX_TRIAL_PAIR(3)
 #undef SMCX_TRIAL_PAIR
@@ -363,5 +426,6 @@ inline int launch_thread_per_cell(const Geom& G, uint32_t* lattice, const int32_
         G, lattice, reinterpret_cast<const int4*>(d_coef), accept, d_filter, st, colour);
   return 0;
 }
+#endif  // __CUDACC__
 
 }  // namespace smcxk
