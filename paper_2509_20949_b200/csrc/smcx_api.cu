@@ -81,6 +81,7 @@ struct Plan {
   long long n_cells;
   int storage;
   int kernel;
+  int coef_class;   // build_thread_coefficients: 2 = the filter variant of the thread kernel applies
   Layout lay;
 };
 
@@ -167,9 +168,11 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
 
   // kernel / storage choice
   bool fast_ok = thread_kernel_supported(G);
+  plan->coef_class = 0;
   if (fast_ok) {  // the packed kernel computes dE in int32 from a coefficient table: magnitudes must fit
     int32_t coef[16 * kCoefInts];
-    fast_ok = build_thread_coefficients(p->epi, n, coef);
+    plan->coef_class = build_thread_coefficients(p->epi, n, coef);
+    fast_ok = plan->coef_class > 0;
   }
   int kernel = p->kernel, storage = p->storage;
   if (kernel == SMCX_KERNEL_AUTO) {
@@ -332,7 +335,7 @@ int upload_table(smcx* h, const uint32_t* accept, int len) {
   if (h->plan.kernel == SMCX_KERNEL_THREAD_PER_CELL) {
     uint32_t* filt = h->staging[slot] + kAcceptCapacity;
     int nq = 0;
-    const int E = build_accept_filter(accept, len, filt, &nq);
+    const int E = h->plan.coef_class == 2 ? build_accept_filter(accept, len, filt, &nq) : -1;
     if (E >= 0) {
       SMCX_CUDA(h, cudaMemcpyAsync(h->d_filter(), filt, (size_t)kFilterWords * sizeof(uint32_t),
                                    cudaMemcpyHostToDevice, h->stream));

@@ -89,6 +89,10 @@ struct Geom {
   // Philox round keys key + r * (W0, W1), r = 0..9: operands taken straight from the constant
   // bank (no per-call key schedule)
   uint32_t rk0[10], rk1[10];
+  // constants the thread-per-cell kernel wants as constant-bank operands rather than immediates
+  // (an IMAD takes one immediate; "dx * c0 + c1" with both constant needs the other from here):
+  // kc[0] = 1, kc[1] = 0x1111, kc[2 + slot] and kc[10 + slot] per-slot constants (sweep_thread.cuh)
+  uint32_t kc[18];
   // all shells concatenated, shell by shell, each in ascending (dz,dy,dx) order
   signed char off[kMaxNeighbours][3];   // half-lattice units
   unsigned char shell_of[kMaxNeighbours];

@@ -25,6 +25,7 @@
 //  * the integer pipe (LOP3/SHF/PRMT/ISETP) is the binding unit (ncu: profiles/), so everything
 //    is arranged to keep its instruction count down.
 #pragma once
+#include <algorithm>
 #include <cstdlib>
 #include "smcx_common.cuh"
 #include "sweep_warp.cuh"
@@ -43,45 +44,52 @@ constexpr int kCoefInts = 8;            // per (a,b): cl0 ch0' cb0 cl1 | ch1' cb
 constexpr int kFilterTr = 64;           // Tr[r] = T[r], r < 64
 constexpr int kFilterMaxTq = 1024;      // Tq[q] = T[64 q]
 constexpr int kFilterWords = kFilterTr + kFilterMaxTq;
-constexpr int kFilterDmax = 64 * kFilterMaxTq - 1;   // dE is clamped to [0, kFilterDmax] before the look-up
-constexpr int32_t kSameSpecies = 1 << 29;            // "dE" of a trial between equal species: never accepted
-constexpr long long kCoefBudget = 1ll << 28;         // bound on |dE| the coefficient table may produce
+constexpr int kFilterDmax = 64 * kFilterMaxTq - 1;   // largest dE the filter tables cover (zero entries at the top)
+constexpr int32_t kSameSpecies = kFilterDmax - 31;   // "dE" of a trial between equal species: never accepted
+constexpr int kDEScale = 4;                          // the kernel computes 4 dE (= byte offset into Tr)
 
 inline bool thread_kernel_supported(const Geom& G) {
-  return G.lattice == 0 && G.n_shells == 2 && G.w == 4 && G.n_species <= 4 && G.H == 2 && G.TW == 8;
+  // the last condition keeps word indices of the packed lattice (16 sites per word) in 32 bits
+  return G.lattice == 0 && G.n_shells == 2 && G.w == 4 && G.n_species <= 4 && G.H == 2 && G.TW == 8 &&
+         (long long)G.Lx * G.Ly * G.Lz / 8 < (1ll << 32);
 }
 
 // Host: coefficient table from the EPI tables, [a*4+b][8] int32.  With PT / PH / PB the population
 // counts of trial_thread (all fields, high bits, both bits; j's fields complemented, Z_s of them):
 //   dE = corr' + sum_s cl_s PT_s + (ch_s - cl_s) PH_s + cb_s PB_s,
 //   corr' = corr - sum_s Z_s (cl_s + ch_s + cb_s).
-// Entries with a == b hold kSameSpecies in corr' and zeros elsewhere.  Returns false if the
-// magnitudes could overflow the int32 arithmetic of the kernel.
-inline bool build_thread_coefficients(const int32_t* epi, int n_species, int32_t* coef /*16*8*/) {
+// The table holds kDEScale times these values.  Entries with a == b hold kSameSpecies in corr' and
+// zeros elsewhere.  Returns, from the bound |dE| <= 2 sum_s Z_s max_x |D_s(x)| + |corr|:
+//   0  kDEScale dE could overflow int32: the kernel cannot be used;
+//   1  exact, but dE can reach kSameSpecies: only the variant without the filter tables applies;
+//   2  every dE of a trial between different species is below kSameSpecies: the filter variant applies.
+inline int build_thread_coefficients(const int32_t* epi, int n_species, int32_t* coef /*16*8*/) {
   auto V = [&](int s, int a, int b) -> long long {
     return (a < n_species && b < n_species) ? (long long)epi[(s * n_species + a) * n_species + b] : 0ll;
   };
   const int Z[2] = {8, 6};
-  bool fits = true;
+  int cls = 2;
   for (int a = 0; a < 4; ++a)
     for (int b = 0; b < 4; ++b) {
       int32_t* c = coef + (a * 4 + b) * kCoefInts;
       for (int k = 0; k < kCoefInts; ++k) c[k] = 0;
-      if (a == b) { c[6] = kSameSpecies; continue; }
+      if (a == b) { c[6] = kDEScale * kSameSpecies; continue; }
       long long corr = 2 * V(0, a, b) - V(0, a, a) - V(0, b, b);
-      long long budget = 0;
+      long long bound = std::llabs(corr);
       for (int s = 0; s < 2; ++s) {
-        long long D[4];
-        for (int x = 0; x < 4; ++x) D[x] = V(s, b, x) - V(s, a, x);
+        long long D[4], maxD = 0;
+        for (int x = 0; x < 4; ++x) { D[x] = V(s, b, x) - V(s, a, x); maxD = std::max(maxD, std::llabs(D[x])); }
         const long long cl = D[1] - D[0], ch = D[2] - D[0], cb = D[3] - D[1] - D[2] + D[0];
-        c[3 * s + 0] = (int32_t)cl; c[3 * s + 1] = (int32_t)(ch - cl); c[3 * s + 2] = (int32_t)cb;
+        c[3 * s + 0] = (int32_t)(kDEScale * cl); c[3 * s + 1] = (int32_t)(kDEScale * (ch - cl));
+        c[3 * s + 2] = (int32_t)(kDEScale * cb);
         corr -= Z[s] * (cl + ch + cb);
-        budget += 32 * (std::llabs(cl) + std::llabs(ch - cl) + std::llabs(cb));
+        bound += 2 * Z[s] * maxD;
       }
-      c[6] = (int32_t)corr;
-      if (budget + std::llabs(corr) >= kCoefBudget) fits = false;
+      c[6] = (int32_t)(kDEScale * corr);
+      if (bound >= kSameSpecies) cls = std::min(cls, 1);
+      if (bound >= (1ll << 28)) cls = 0;
     }
-  return fits;
+  return cls;
 }
 
 // Host: two-level filter tables for a threshold table T (T[d] = 0 understood for d >= len).
@@ -105,17 +113,14 @@ inline int build_accept_filter(const uint32_t* T, int len, uint32_t* filt /*kFil
   return E <= 1024u ? (int)E : -1;
 }
 
-inline void set_thread_masks(Geom& G) {
-  for (int r = 0; r < 10; ++r) {
-    G.rk0[r] = G.key0 + (uint32_t)r * 0x9E3779B9u;
-    G.rk1[r] = G.key1 + (uint32_t)r * 0xBB67AE85u;
-  }
-}
+inline void set_thread_masks(Geom& G);   // below, after SlotConst
 
 // ---- bit helpers (host versions exist so that the trial arithmetic can be unit-tested on the CPU) ----
 __host__ __device__ __forceinline__ uint32_t prmt(uint32_t a, uint32_t b, uint32_t sel) {
 #ifdef __CUDA_ARCH__
-  return __byte_perm(a, b, sel);
+  uint32_t d;
+  asm("prmt.b32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(sel));   // no selector masking (__byte_perm adds one)
+  return d;
 #else
   const uint64_t ab = ((uint64_t)b << 32) | a;
   uint32_t d = 0;
@@ -153,6 +158,44 @@ __host__ __device__ __forceinline__ uint32_t ldg_u32(const uint32_t* p) {
   return __ldg(p);
 #else
   return *p;
+#endif
+}
+
+// a * b + c as one IMAD (FMA pipe); written in PTX so that it is not rewritten into shifts and masks
+__host__ __device__ __forceinline__ uint32_t mad_u32(uint32_t a, uint32_t b, uint32_t c) {
+#ifdef __CUDA_ARCH__
+  uint32_t d;
+  asm("mad.lo.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+#else
+  return a * b + c;
+#endif
+}
+// Shared-memory tables are addressed on the device by 32-bit shared addresses formed with mad_u32.
+#ifdef __CUDA_ARCH__
+typedef uint32_t smem_ptr_t;
+__device__ __forceinline__ smem_ptr_t smem_ptr(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ uint32_t lds_u32(smem_ptr_t base, uint32_t byte_off) {
+  uint32_t v;
+  asm("ld.shared.u32 %0, [%1];" : "=r"(v) : "r"(base + byte_off));
+  return v;
+}
+__device__ __forceinline__ int4 lds_int4(smem_ptr_t addr, int imm) {
+  int4 v;
+  asm("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr + imm));
+  return v;
+}
+#else
+typedef const char* smem_ptr_t;
+inline smem_ptr_t smem_ptr(const void* p) { return reinterpret_cast<const char*>(p); }
+inline uint32_t lds_u32(smem_ptr_t base, uint32_t byte_off) { return *reinterpret_cast<const uint32_t*>(base + byte_off); }
+inline int4 lds_int4(smem_ptr_t addr, int imm) { return *reinterpret_cast<const int4*>(addr + imm); }
+#endif
+__host__ __device__ __forceinline__ smem_ptr_t smem_index(smem_ptr_t base, uint32_t idx, uint32_t scale) {
+#ifdef __CUDA_ARCH__
+  return mad_u32(idx, scale, base);
+#else
+  return base + idx * scale;
 #endif
 }
 
@@ -199,26 +242,61 @@ __host__ __device__ __forceinline__ uint32_t pick(uint32_t dx, uint32_t c0, uint
   return c0 + dx * (c1 - c0);
 }
 
-// One trial (a4-a6).  p_i points at the tile row of site i (row stride STRIDE words).
+// Loop-invariant operands of a trial, kept in registers.
+struct TrialEnv {
+  smem_ptr_t coef;           // coefficient rows of this lane's slot
+  smem_ptr_t filt;           // Tr[64] then Tq[1024]
+  const uint32_t* accept;    // global threshold table (rare exact look-up)
+  int accept_len, filter_E;
+};
+
+// Geom::kc: constants used as the constant-bank operand of an IMAD whose other constant is an
+// immediate.  Slot = bi * 4 + X - 2.
+constexpr int kKcOne = 0, kKc1111 = 1, kKcMjDelta = 2, kKcShj0 = 10;
+
+template <int bi, int X>
+inline void set_slot_constants(Geom& G) {
+  using K = SlotConst<bi, X>;
+  G.kc[kKcMjDelta + bi * 4 + X - 2] = K::Mj1 - K::Mj0;
+  G.kc[kKcShj0 + bi * 4 + X - 2] = (uint32_t)K::shj0;
+}
+
+inline void set_thread_masks(Geom& G) {
+  for (int r = 0; r < 10; ++r) {
+    G.rk0[r] = G.key0 + (uint32_t)r * 0x9E3779B9u;
+    G.rk1[r] = G.key1 + (uint32_t)r * 0xBB67AE85u;
+  }
+  G.kc[kKcOne] = 1u;
+  G.kc[kKc1111] = 0x1111u;
+  set_slot_constants<0, 2>(G); set_slot_constants<0, 3>(G); set_slot_constants<0, 4>(G); set_slot_constants<0, 5>(G);
+  set_slot_constants<1, 2>(G); set_slot_constants<1, 3>(G); set_slot_constants<1, 4>(G); set_slot_constants<1, 5>(G);
+}
+
+// One trial (a4-a6).  p_i points at the tile row of site i (row stride STRIDE words).  ra / rb carry
+// two rows from one trial of an x-row to the next: a trial with bi == 0 takes rows y-1 and z-1 and
+// leaves y+1 and z+1 (which it cannot have modified), a trial with bi == 1 the other way round.
 template <int bi, int X, bool kFilter, int STRIDE>
-__host__ __device__ __forceinline__ void trial_thread(uint32_t* p_i, const char* coef_base, const uint32_t* s_filt,
-                                                      const uint32_t* __restrict__ accept, int accept_len,
-                                                      int filter_E, uint32_t w_dir, uint32_t u, int& esum,
+__host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const TrialEnv& env, uint32_t w_dir,
+                                                      uint32_t u, uint32_t& ra, uint32_t& rb, int& esum4,
                                                       unsigned& nacc) {
   using K = SlotConst<bi, X>;
   constexpr int NT = STRIDE;
-  // direction: top three bits of the draw (= mulhi(w_dir, 8)); dx = bit 0, dy = bit 1, dz = bit 2
+  constexpr int slot = bi * 4 + X - 2;
+  // direction: top three bits of the draw (= mulhi(w_dir, 8)); dx = bit 0, dy = bit 1, dz = bit 2.
+  // row_j - row_i = (dy - 1 + bi) + 8 (dz - 1 + bi): byte (dy + 2 dz) of 0x09080100, less 9 if bi == 0
   const uint32_t dx = (w_dir >> 29) & 1u;
-  const int t1 = (int)(w_dir >> 30);                      // dy + 2 dz
-  const int dz = (int)(w_dir >> 31);
-  const int rd = t1 + 6 * dz - 9 * (1 - bi);              // row_j - row_i = (dy-1+bi) + 8 (dz-1+bi)
-  uint32_t* p_j = p_i + rd * NT;
+  const uint32_t rdp = prmt(0x09080100u, 0u, w_dir >> 30);
+  uint32_t* p_j = p_i - 9 * (1 - bi) * NT + rdp * NT;
   // rows around i and j
-  const uint32_t own_i = p_i[0], yMi = p_i[-NT], yPi = p_i[NT], zMi = p_i[-8 * NT], zPi = p_i[8 * NT];
+  const uint32_t own_i = p_i[0];
+  const uint32_t yMi = bi ? p_i[-NT] : ra, zMi = bi ? p_i[-8 * NT] : rb;
+  const uint32_t yPi = bi ? ra : p_i[NT], zPi = bi ? rb : p_i[8 * NT];
   const uint32_t dgi = bi ? p_i[9 * NT] : p_i[-9 * NT];
   const uint32_t own_j = p_j[0], yMj = p_j[-NT], yPj = p_j[NT], zMj = p_j[-8 * NT], zPj = p_j[8 * NT];
   const uint32_t dgj = bi ? p_j[-9 * NT] : p_j[9 * NT];
-  const uint32_t mul = dx * 15u + 1u;                      // 16^dx: masks that move by one nibble with dx
+  ra = bi ? yMi : yPi;
+  rb = bi ? zMi : zPi;
+  const uint32_t mul = mad_u32(dx, 15u, G.kc[kKcOne]);     // 16^dx: masks that move by one nibble with dx
   // shell 0: i's rows are own, y-+1, z-+1, diagonal on the side of the other sublattice; j's mirror them
   const uint32_t Wi = lop3<kLutSel>(prmt(own_i, bi ? yPi : yMi, K::swa_i), prmt(bi ? zPi : zMi, dgi, K::swb_i), K::mi);
   const uint32_t Wj = lop3<kLutSel>(prmt(own_j, bi ? yMj : yPj, K::swa_j), prmt(bi ? zMj : zPj, dgj, K::swb_j),
@@ -227,10 +305,10 @@ __host__ __device__ __forceinline__ void trial_thread(uint32_t* p_i, const char*
   // shell 1
   const uint32_t n3i = prmt(prmt(yMi, yPi, K::s2i), prmt(zMi, zPi, K::s2i), 0x7610u);
   const uint32_t W2i = lop3<kLutSel>(own_i, n3i, K::moi);
-  const uint32_t s2j = (K::s2j0 == K::s2j1) ? K::s2j0 : K::s2j0 + dx * (K::s2j1 - K::s2j0);
+  const uint32_t s2j = (K::s2j0 == K::s2j1) ? K::s2j0 : mad_u32(dx, G.kc[kKc1111], K::s2j0);
   const uint32_t n3j = prmt(prmt(yMj, yPj, s2j), prmt(zMj, zPj, s2j), 0x7610u);
   const uint32_t W2j = lop3<kLutSel>(own_j, n3j, K::moj0 * mul);
-  const uint32_t MjD = (K::Mj1 == (K::Mj0 << 4)) ? K::Mj0 * mul : pick(dx, K::Mj0, K::Mj1);
+  const uint32_t MjD = (K::Mj1 == (K::Mj0 << 4)) ? K::Mj0 * mul : mad_u32(dx, G.kc[kKcMjDelta + slot], K::Mj0);
   const uint32_t U2 = lop3<kLutAndOr>(lop3<kLutSelNotB>(W2i, W2j, K::Ci), MjD, K::Mi);
   // population counts: all field bits, high bits, "both bits" (AND for i, OR of complements for j)
   const uint32_t h1 = U1 & K::kHi, h2 = U2 & K::kHi;
@@ -238,37 +316,86 @@ __host__ __device__ __forceinline__ void trial_thread(uint32_t* p_i, const char*
   const uint32_t b2 = lop3<kLutMaj>(U2 << 1, h2, K::Cj & K::kHi);
   const int pt1 = popc32(U1), ph1 = popc32(h1), pb1 = popc32(b1);
   const int pt2 = popc32(U2), ph2 = popc32(h2), pb2 = popc32(b2);
-  // species of i and j (times 16) and the coefficient row of the ordered pair
+  // species of i and j (times 16) and the coefficient row of the ordered pair: [(a*4+b)*8 + slot] int4
   const uint32_t a4 = (own_i >> K::shi) & 0x30u;
-  const uint32_t shj = (uint32_t)K::shj0 + 4u * dx;
-  const uint32_t b4 = (own_j >> shj) & 0x30u;
-  const int4 c0 = *reinterpret_cast<const int4*>(coef_base + a4 * 32u + b4 * 8u);            // [(a*4+b)*8 + slot]
-  const int4 c1 = *reinterpret_cast<const int4*>(coef_base + 2048 + a4 * 32u + b4 * 8u);
-  const int dE = c1.z + c0.x * pt1 + c0.y * ph1 + c0.z * pb1 + c0.w * pt2 + c1.x * ph2 + c1.y * pb2;
+  const uint32_t b4 = (own_j >> mad_u32(dx, 4u, G.kc[kKcShj0 + slot])) & 0x30u;
+  const smem_ptr_t crow = smem_index(smem_index(env.coef, a4, 32u), b4, 8u);
+  const int4 c0 = lds_int4(crow, 0), c1 = lds_int4(crow, 2048);
+  const int dE4 = c1.z + c0.x * pt1 + c0.y * ph1 + c0.z * pb1 + c0.w * pt2 + c1.x * ph2 + c1.y * pb2;   // 4 dE
   // Eq. 3 in integer form
   bool ok;
   if (kFilter) {
-    // two-level threshold: ta <= T[dE] <= ta + E for the clamped dE (tables are zero beyond the last
-    // entry; dE <= 0 maps to entry 0, equal species to the zero entry at the top)
-    const uint32_t dc = (uint32_t)min(max(dE, 0), kFilterDmax);
-    const uint32_t ta = mulhi_u32(s_filt[kFilterTr + (dc >> 6)], s_filt[dc & 63u]);
+    // two-level threshold: ta <= T[dE] <= ta + E; dE <= 0 maps to entry 0, a trial between equal
+    // species (dE = kSameSpecies by construction) to the zero entries at the top of Tq
+    const uint32_t dc4 = (uint32_t)max(dE4, 0);
+    const uint32_t ta = mulhi_u32(lds_u32(env.filt, 4 * kFilterTr + ((dc4 >> 6) & 0xFFCu)), lds_u32(env.filt, dc4 & 0xFCu));
     ok = u < ta;
-    if (u - ta <= (uint32_t)filter_E)                      // u in [ta, ta+E]: rare exact decision
-      ok = dE <= 0 || (dE < accept_len && u < ldg_u32(accept + dE));
+    if (u - ta <= (uint32_t)env.filter_E) {                // u in [ta, ta+E]: rare exact decision
+      const int dE = dE4 >> 2;
+      ok = dE <= 0 || (dE < env.accept_len && u < ldg_u32(env.accept + dE));
+    }
   } else {
+    const int dE = dE4 >> 2;
     ok = dE <= 0;
-    if (dE > 0 && dE < accept_len) ok = u < ldg_u32(accept + dE);
+    if (dE > 0 && dE < env.accept_len) ok = u < ldg_u32(env.accept + dE);
+    ok = ok && a4 != b4;
   }
   // swap by arithmetic: the field of i holds a and becomes b, that of j holds b and becomes a; a
   // rejected trial stores the rows back unchanged (no branch)
-  const uint32_t d4 = ok ? b4 - a4 : 0u;
-  const uint32_t new_i = own_i + d4 * (1u << K::shi);
-  const uint32_t new_j = (rd == 0 ? new_i : own_j) - d4 * ((1u << K::shj0) * mul);
+  const uint32_t oki = ok ? 1u : 0u;
+  const uint32_t od = mad_u32(oki, b4 - a4, 0u);
+  const uint32_t new_i = mad_u32(od, 1u << K::shi, own_i);
+  const uint32_t new_j = mad_u32(od, (0u - (1u << K::shj0)) * mul, rdp == 9u * (1 - bi) ? new_i : own_j);
   p_i[0] = new_i;
   p_j[0] = new_j;
-  esum += ok ? dE : 0;
-  nacc += ok ? 1u : 0u;
+  esum4 = (int)mad_u32(oki, (uint32_t)dE4, (uint32_t)esum4);
+  nacc += oki;
 }
+
+#ifdef __CUDACC__
+// Write-back of one tile word whose first nibble sits at nibble C of the aligned word pair (hi:lo).
+// Bytes [P0, P1) of the pair lie wholly inside the tile word; they are cut into naturally aligned
+// 4 / 2 / 1-byte stores at compile time.
+template <int C, int P>
+__device__ __forceinline__ void store_tile_bytes(unsigned char* lo, unsigned char* hi, uint32_t wv) {
+  constexpr int P1 = (4 * C + 32) / 8;
+  if constexpr (P < P1) {
+    constexpr int off = P & 3;
+    constexpr int room = (P1 - P) < (4 - off) ? (P1 - P) : (4 - off);
+    constexpr int size = (off == 0 && room >= 4) ? 4 : ((off % 2 == 0 && room >= 2) ? 2 : 1);
+    unsigned char* dst = (P < 4 ? lo : hi) + off;
+    const uint32_t val = wv >> (8 * P - 4 * C);
+    if constexpr (size == 4) *reinterpret_cast<uint32_t*>(dst) = val;
+    else if constexpr (size == 2) *reinterpret_cast<uint16_t*>(dst) = (uint16_t)val;
+    else *dst = (unsigned char)val;
+    store_tile_bytes<C, P + size>(lo, hi, wv);
+  }
+}
+
+template <int C>
+__device__ __forceinline__ void write_back_tile(const Geom& G, const uint32_t* tile, uint32_t* lattice, int wlo,
+                                                uint32_t dwh, int t0y, int t0z, int rw, uint32_t zstride) {
+  constexpr int NT = kThreadNT;
+  uint32_t offy[6];
+#pragma unroll
+  for (int ry = 1; ry < 7; ++ry) {
+    int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
+    offy[ry - 1] = (uint32_t)gy * (uint32_t)rw + (uint32_t)wlo;
+  }
+#pragma unroll 1
+  for (int rz = 1; rz < 7; ++rz) {
+    int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
+    const uint32_t zoff = (uint32_t)gz * zstride;
+#pragma unroll
+    for (int ry = 1; ry < 7; ++ry) {
+      const uint32_t idx = zoff + offy[ry - 1];
+      store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(lattice + idx),
+                                           reinterpret_cast<unsigned char*>(lattice + (uint32_t)(idx + dwh)),
+                                           tile[(rz * 8 + ry) * NT]);
+    }
+  }
+}
+#endif
 
 #ifdef __CUDACC__
 template <bool kFilter>
@@ -310,83 +437,73 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
     const int rw = G.Lx >> 3;                                   // words per lattice row
     const int wlo = x0 >> 3, sh = 4 * (x0 & 7);
     const int whi = wlo + 1 == rw ? 0 : wlo + 1;
-    // a3: stage the tile (funnel-shift two aligned words per row into one tile word)
-    const uint32_t* lat_lo = lattice + wlo;
-    const uint32_t* lat_hi = lattice + whi;
-#pragma unroll 2
-    for (int rz = 0; rz < 8; ++rz) {
-      int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
-      uint32_t lo[8], hi[8];
+    // a3: stage the tile (funnel-shift two aligned words per row into one tile word).  Row (gz, gy)
+    // starts at word (gz Ly + gy) rw of the lattice (a 32-bit index: thread_kernel_supported).
+    const uint32_t zstride = (uint32_t)G.Ly * (uint32_t)rw;
+    const uint32_t dwh = (uint32_t)(whi - wlo);                 // index step from the low to the high word of a row
+    {
+      uint32_t offy[8];
 #pragma unroll
       for (int ry = 0; ry < 8; ++ry) {
         int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
-        const size_t roff = (size_t)((uint32_t)(gz * G.Ly + gy)) * (uint32_t)rw;   // row index fits 32 bits
-        lo[ry] = lat_lo[roff];
-        hi[ry] = sh ? lat_hi[roff] : 0u;
+        offy[ry] = (uint32_t)gy * (uint32_t)rw + (uint32_t)wlo;
       }
+#pragma unroll 2
+      for (int rz = 0; rz < 8; ++rz) {
+        int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
+        const uint32_t zoff = (uint32_t)gz * zstride;
+        uint32_t lo[8], hi[8];
 #pragma unroll
-      for (int ry = 0; ry < 8; ++ry) tile[(rz * 8 + ry) * NT] = __funnelshift_r(lo[ry], hi[ry], sh);
+        for (int ry = 0; ry < 8; ++ry) {
+          const uint32_t idx = zoff + offy[ry];
+          lo[ry] = lattice[idx];
+          hi[ry] = lattice[idx + dwh];
+        }
+#pragma unroll
+        for (int ry = 0; ry < 8; ++ry) tile[(rz * 8 + ry) * NT] = __funnelshift_r(lo[ry], hi[ry], sh);
+      }
     }
     // a4-a6: the 128 trials of this cell, raster order, one Philox call per two slots
     const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
     const uint32_t ctr3 = TAG_TRIAL | ((uint32_t)colour << 8);
-    const char* coef_base = reinterpret_cast<const char*>(s_coef0) + (threadIdx.x & 7) * 16;
-    const int accept_len = G.accept_len, filter_E = G.filter_E;
+    TrialEnv env;
+    env.coef = smem_ptr(s_coef0) + (threadIdx.x & 7) * 16;
+    env.filt = smem_ptr(s_filt);
+    env.accept = accept;
+    env.accept_len = G.accept_len;
+    env.filter_E = G.filter_E;
 #pragma unroll 1
     for (int lzy = 0; lzy < 16; ++lzy) {
       uint32_t* p_row = tile + (((lzy >> 2) + 2) * 8 + (lzy & 3) + 2) * NT;
       const uint32_t q0 = (uint32_t)lzy * 4u;
+      uint32_t ra = p_row[-NT], rb = p_row[-8 * NT];
 #define SMCX_TRIAL_PAIR(LX)                                                                                          \
       {                                                                                                              \
         const Philox4 r = philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1);                                 \
-        trial_thread<0, LX + 2, kFilter, NT>(p_row, coef_base, s_filt, accept, accept_len, filter_E, r.x, r.y, esum, nacc); \
-        trial_thread<1, LX + 2, kFilter, NT>(p_row, coef_base, s_filt, accept, accept_len, filter_E, r.z, r.w, esum, nacc); \
+        trial_thread<0, LX + 2, kFilter, NT>(G, p_row, env, r.x, r.y, ra, rb, esum, nacc);                                                \
+        trial_thread<1, LX + 2, kFilter, NT>(G, p_row, env, r.z, r.w, ra, rb, esum, nacc);                                                \
       }
       SMCX_TRIAL_PAIR(0) SMCX_TRIAL_PAIR(1) SMCX_TRIAL_PAIR(2) SMCX_TRIAL_PAIR(3)
 #undef SMCX_TRIAL_PAIR
     }
-    // a7: write back tile rows 1..6 x 1..6; only the bytes that lie wholly inside this tile and can
-    // hold a modified site (conventional cells 1..6 of the row: 4 bytes if x0 is even, else 3), cut
-    // into at most three naturally aligned stores.  The cut depends on x0 mod 8 only, which is the
-    // same for every cell of a pass, so the branches below are uniform.
+    // a7: write back tile rows 1..6 x 1..6: the bytes that lie wholly inside this tile (no other
+    // cell of the pass touches them) and can hold a modified site.  The byte pattern depends on
+    // x0 mod 8 only, which is the same for every cell of a pass: one uniform switch.
     {
-      const int rb = G.Lx >> 1;                                 // bytes per lattice row (multiple of 4)
-      const bool odd = x0 & 1;
-      int pos = (x0 + (odd ? 1 : 0)) >> 1;                      // first byte, before wrapping
-      int rem = odd ? 3 : 4, done = 0, nseg = 0;
-      int seg_sz[3] = {0, 0, 0}, seg_sh[3] = {0, 0, 0};
-      unsigned char* seg_p[3] = {nullptr, nullptr, nullptr};
-#pragma unroll
-      for (int k = 0; k < 3; ++k) {
-        if (rem > 0) {
-          const int sz = ((pos & 3) == 0 && rem >= 4) ? 4 : (((pos & 1) == 0 && rem >= 2) ? 2 : 1);
-          seg_sz[k] = sz;
-          seg_sh[k] = 8 * done + (odd ? 4 : 0);
-          seg_p[k] = reinterpret_cast<unsigned char*>(lattice) + (pos >= rb ? pos - rb : pos);
-          pos += sz; rem -= sz; done += sz; nseg = k + 1;
-        }
-      }
-      for (int rz = 1; rz < 7; ++rz) {
-        int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
-#pragma unroll
-        for (int ry = 1; ry < 7; ++ry) {
-          int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
-          const size_t roff = (size_t)((uint32_t)(gz * G.Ly + gy)) * (uint32_t)rb;
-          const uint32_t wv = tile[(rz * 8 + ry) * NT];
-#pragma unroll
-          for (int k = 0; k < 3; ++k) {
-            if (k < nseg) {
-              const uint32_t val = wv >> seg_sh[k];
-              if (seg_sz[k] == 4) *reinterpret_cast<uint32_t*>(seg_p[k] + roff) = val;
-              else if (seg_sz[k] == 2) *reinterpret_cast<uint16_t*>(seg_p[k] + roff) = (uint16_t)val;
-              else seg_p[k][roff] = (unsigned char)val;
-            }
-          }
-        }
+      switch (x0 & 7) {
+        case 0: write_back_tile<0>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 1: write_back_tile<1>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 2: write_back_tile<2>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 3: write_back_tile<3>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 4: write_back_tile<4>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 5: write_back_tile<5>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 6: write_back_tile<6>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        default: write_back_tile<7>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
       }
     }
   }
-  // a8: block reduction, one atomic pair per block
+  // a8: block reduction, one atomic pair per block (the trials accumulated kDEScale dE)
+  esum /= kDEScale;
   for (int o = 16; o > 0; o >>= 1) {
     esum += __shfl_down_sync(0xffffffffu, esum, o);
     nacc += __shfl_down_sync(0xffffffffu, nacc, o);
