@@ -33,10 +33,16 @@
 namespace smcxk {
 
 #ifndef SMCX_NT
-#define SMCX_NT 256
+#define SMCX_NT 128
 #endif
 #ifndef SMCX_BLOCKS_PER_SM
-#define SMCX_BLOCKS_PER_SM 3
+#define SMCX_BLOCKS_PER_SM 5
+#endif
+#ifndef SMCX_OPT_DXMAD
+#define SMCX_OPT_DXMAD 1     // x bit of the direction by multiply-add instead of a mask
+#endif
+#ifndef SMCX_OPT_ATOMSWAP
+#define SMCX_OPT_ATOMSWAP 1  // swap by two shared-memory atomic adds instead of two stores
 #endif
 constexpr int kThreadNT = SMCX_NT;      // threads (= cells) per block
 constexpr int kThreadTileWords = 64;    // 8 x 8 rows of one word
@@ -284,8 +290,14 @@ __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p
   constexpr int slot = bi * 4 + X - 2;
   // direction: top three bits of the draw (= mulhi(w_dir, 8)); dx = bit 0, dy = bit 1, dz = bit 2.
   // row_j - row_i = (dy - 1 + bi) + 8 (dz - 1 + bi): byte (dy + 2 dz) of 0x09080100, less 9 if bi == 0
+#if SMCX_OPT_DXMAD
+  const uint32_t t1 = w_dir >> 30;
+  const uint32_t dx = mad_u32(t1, 0xFFFFFFFEu, w_dir >> 29);   // dir - 2 (dir >> 1), on the FMA pipe
+  const uint32_t rdp = prmt(0x09080100u, 0u, t1);
+#else
   const uint32_t dx = (w_dir >> 29) & 1u;
   const uint32_t rdp = prmt(0x09080100u, 0u, w_dir >> 30);
+#endif
   uint32_t* p_j = p_i - 9 * (1 - bi) * NT + rdp * NT;
   // rows around i and j
   const uint32_t own_i = p_i[0];
@@ -344,10 +356,15 @@ __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p
   // rejected trial stores the rows back unchanged (no branch)
   const uint32_t oki = ok ? 1u : 0u;
   const uint32_t od = mad_u32(oki, b4 - a4, 0u);
+#if SMCX_OPT_ATOMSWAP && defined(__CUDA_ARCH__)
+  atomicAdd(p_i, od * (1u << K::shi));                       // shared-memory adds: i and j may share a row
+  atomicAdd(p_j, od * ((0u - (1u << K::shj0)) * mul));
+#else
   const uint32_t new_i = mad_u32(od, 1u << K::shi, own_i);
   const uint32_t new_j = mad_u32(od, (0u - (1u << K::shj0)) * mul, rdp == 9u * (1 - bi) ? new_i : own_j);
   p_i[0] = new_i;
   p_j[0] = new_j;
+#endif
   esum4 = (int)mad_u32(oki, (uint32_t)dE4, (uint32_t)esum4);
   nacc += oki;
 }
