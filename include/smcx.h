@@ -53,9 +53,15 @@ enum { SMCX_BCC = 0, SMCX_FCC = 1 };
 enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
 
 /* Which sweep kernel runs.  WARP_PER_CELL: any lattice/shell list, U8 storage.
- * THREAD_PER_CELL: BCC, first two shells, link_cell = 4, n_species <= 4, 2BIT storage.
- * AUTO picks THREAD_PER_CELL when the parameters allow it.  Results never depend on it. */
-enum { SMCX_KERNEL_AUTO = 0, SMCX_KERNEL_WARP_PER_CELL = 1, SMCX_KERNEL_THREAD_PER_CELL = 2 };
+ * THREAD_PER_CELL: BCC, first two shells, link_cell = 4, n_species <= 4, 2BIT storage; one block per
+ * 128 cells, two-level acceptance filter in shared memory.
+ * THREAD_PERSISTENT: same restrictions; one block per SM whose warps walk over the cells of the
+ * colour, the whole threshold table in shared memory.  While the current table is too long for that
+ * (more than about 16,000 entries next to 20 warps, 32,000 next to 16) passes run the THREAD_PER_CELL
+ * kernel instead.
+ * AUTO picks THREAD_PERSISTENT when the parameters allow it.  Results never depend on it. */
+enum { SMCX_KERNEL_AUTO = 0, SMCX_KERNEL_WARP_PER_CELL = 1, SMCX_KERNEL_THREAD_PER_CELL = 2,
+       SMCX_KERNEL_THREAD_PERSISTENT = 3 };
 
 enum {
   SMCX_OK = 0,

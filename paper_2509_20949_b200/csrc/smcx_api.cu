@@ -71,6 +71,8 @@ int basis_from_parity(int lattice, int px, int py, int pz) {
 
 inline int floor_div2(int v) { return v >= 0 ? v / 2 : -((-v + 1) / 2); }
 
+inline bool is_thread_kernel(int k) { return k == SMCX_KERNEL_THREAD_PER_CELL || k == SMCX_KERNEL_THREAD_PERSISTENT; }
+
 struct Layout {
   size_t species, epi, coef, accept, filter, trace, state, counts, total;
 };
@@ -177,9 +179,9 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   int kernel = p->kernel, storage = p->storage;
   if (kernel == SMCX_KERNEL_AUTO) {
     if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_WARP_PER_CELL;
-    else kernel = fast_ok ? SMCX_KERNEL_THREAD_PER_CELL : SMCX_KERNEL_WARP_PER_CELL;
+    else kernel = fast_ok ? SMCX_KERNEL_THREAD_PERSISTENT : SMCX_KERNEL_WARP_PER_CELL;
   }
-  if (kernel == SMCX_KERNEL_THREAD_PER_CELL) {
+  if (kernel == SMCX_KERNEL_THREAD_PER_CELL || kernel == SMCX_KERNEL_THREAD_PERSISTENT) {
     if (!fast_ok) return SMCX_E_UNSUPPORTED;
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_2BIT;
     if (storage != SMCX_STORAGE_2BIT) return SMCX_E_UNSUPPORTED;
@@ -332,7 +334,7 @@ int upload_table(smcx* h, const uint32_t* accept, int len) {
                                cudaMemcpyHostToDevice, h->stream));
   h->plan.G.filter_E = -1;
   h->plan.G.filter_nq = 0;
-  if (h->plan.kernel == SMCX_KERNEL_THREAD_PER_CELL) {
+  if (is_thread_kernel(h->plan.kernel)) {
     uint32_t* filt = h->staging[slot] + kAcceptCapacity;
     int nq = 0;
     const int E = h->plan.coef_class == 2 ? build_accept_filter(accept, len, filt, &nq) : -1;
@@ -357,7 +359,17 @@ int ensure_bounce(smcx* h) {
 int launch_colour_pass(smcx* h, int colour) {
   const Plan& P = h->plan;
   const Geom& G = P.G;
-  if (P.kernel == SMCX_KERNEL_THREAD_PER_CELL) {
+  if (P.kernel == SMCX_KERNEL_THREAD_PERSISTENT) {
+    const int warps = persist_warps_for(G.accept_len);
+    if (warps > 0) {
+      const int rc = launch_thread_persistent(G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_coef(), h->d_accept(),
+                                              h->d_state(), colour, warps, h->sm_count, h->stream);
+      h->launches++;
+      if (rc != 0) { h->err = "persistent thread-per-cell launch failed"; return SMCX_E_CUDA; }
+      return SMCX_OK;
+    }
+  }
+  if (is_thread_kernel(P.kernel)) {
     const int rc = launch_thread_per_cell(G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_coef(), h->d_accept(),
                                           h->d_filter(), h->d_state(), colour, h->stream);
     h->launches++;
@@ -483,7 +495,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_state(), &zero, sizeof(zero), cudaMemcpyHostToDevice, h->stream));
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_epi(), h->epi.data(), h->epi.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
     int32_t coef[16 * kCoefInts] = {0};
-    if (h->plan.kernel == SMCX_KERNEL_THREAD_PER_CELL) build_thread_coefficients(h->epi.data(), h->plan.G.n_species, coef);
+    if (is_thread_kernel(h->plan.kernel)) build_thread_coefficients(h->epi.data(), h->plan.G.n_species, coef);
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_coef(), coef, sizeof(coef), cudaMemcpyHostToDevice, h->stream));
     SMCX_CUDA(h, cudaMemsetAsync(h->d_trace(), 0, (size_t)h->plan.G.trace_capacity * sizeof(long long), h->stream));
     SMCX_CUDA(h, cudaStreamSynchronize(h->stream));  // &zero and epi must stay valid until copied

@@ -44,6 +44,13 @@ namespace smcxk {
 #ifndef SMCX_OPT_ATOMSWAP
 #define SMCX_OPT_ATOMSWAP 1  // swap by two shared-memory atomic adds instead of two stores
 #endif
+#ifndef SMCX_OPT_XORSWAP
+#define SMCX_OPT_XORSWAP 1   // swap by two predicated shared-memory atomic XORs of (a ^ b)
+#endif
+// Acceptance variants of trial_thread (template parameter MODE)
+constexpr int kAcceptGlobal = 0;   // explicit a != b test, T[dE] from global memory
+constexpr int kAcceptFilter = 1;   // two-level filter tables in shared memory, rare exact look-up
+constexpr int kAcceptDirect = 2;   // the whole table T (plus one zero entry) in shared memory
 constexpr int kThreadNT = SMCX_NT;      // threads (= cells) per block
 constexpr int kThreadTileWords = 64;    // 8 x 8 rows of one word
 constexpr int kCoefInts = 8;            // per (a,b): cl0 ch0' cb0 cl1 | ch1' cb1 corr' pad
@@ -254,6 +261,7 @@ struct TrialEnv {
   smem_ptr_t filt;           // Tr[64] then Tq[1024]
   const uint32_t* accept;    // global threshold table (rare exact look-up)
   int accept_len, filter_E;
+  uint32_t tmax4;            // kAcceptDirect: byte offset of the zero entry that ends the table in shared memory
 };
 
 // Geom::kc: constants used as the constant-bank operand of an IMAD whose other constant is an
@@ -281,7 +289,7 @@ inline void set_thread_masks(Geom& G) {
 // One trial (a4-a6).  p_i points at the tile row of site i (row stride STRIDE words).  ra / rb carry
 // two rows from one trial of an x-row to the next: a trial with bi == 0 takes rows y-1 and z-1 and
 // leaves y+1 and z+1 (which it cannot have modified), a trial with bi == 1 the other way round.
-template <int bi, int X, bool kFilter, int STRIDE>
+template <int bi, int X, int MODE, int STRIDE>
 __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const TrialEnv& env, uint32_t w_dir,
                                                       uint32_t u, uint32_t& ra, uint32_t& rb, int& esum4,
                                                       unsigned& nacc) {
@@ -336,7 +344,33 @@ __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p
   const int dE4 = c1.z + c0.x * pt1 + c0.y * ph1 + c0.z * pb1 + c0.w * pt2 + c1.x * ph2 + c1.y * pb2;   // 4 dE
   // Eq. 3 in integer form
   bool ok;
-  if (kFilter) {
+  if (MODE == kAcceptDirect) {
+    // the whole table sits in shared memory, followed by one zero entry at byte offset tmax4: dE <= 0
+    // (huge as unsigned), dE >= len and a trial between equal species (dE = kSameSpecies by
+    // construction) all clamp to that entry and are decided by the sign test alone
+    const uint32_t i4 = min((uint32_t)dE4, env.tmax4);
+    const uint32_t thr = lds_u32(env.filt, i4);
+#if defined(__CUDA_ARCH__) && SMCX_OPT_XORSWAP
+    // decision without a branch or a 0/1 value: reject = dE > 0 and u >= T.  A rejected trial XORs
+    // zeros (ptxas would wrap a predicated shared-memory atomic in a branch of its own).
+    uint32_t xm;
+    asm("{\n\t"
+        ".reg .pred q, r;\n\t"
+        "setp.gt.s32 q, %3, 0;\n\t"
+        "setp.ge.and.u32 r, %4, %5, q;\n\t"
+        "selp.b32 %2, 0, %6, r;\n\t"
+        "@!r add.s32 %0, %0, %3;\n\t"
+        "@!r add.u32 %1, %1, 1;\n\t"
+        "}"
+        : "+r"(esum4), "+r"(nacc), "=r"(xm)
+        : "r"(dE4), "r"(u), "r"(thr), "r"(a4 ^ b4));
+    atomicXor(p_i, xm << K::shi);
+    atomicXor(p_j, xm * ((1u << K::shj0) * mul));
+    return;
+#else
+    ok = (dE4 <= 0) | (u < thr);
+#endif
+  } else if (MODE == kAcceptFilter) {
     // two-level threshold: ta <= T[dE] <= ta + E; dE <= 0 maps to entry 0, a trial between equal
     // species (dE = kSameSpecies by construction) to the zero entries at the top of Tq
     const uint32_t dc4 = (uint32_t)max(dE4, 0);
@@ -351,6 +385,17 @@ __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p
     ok = dE <= 0;
     if (dE > 0 && dE < env.accept_len) ok = u < ldg_u32(env.accept + dE);
     ok = ok && a4 != b4;
+  }
+  if (MODE == kAcceptDirect) {
+    // host build of the XOR swap (the device build returned above): both fields change by a ^ b
+    if (ok) {
+      const uint32_t x4 = a4 ^ b4;
+      p_i[0] ^= x4 << K::shi;
+      p_j[0] ^= x4 * ((1u << K::shj0) * mul);
+      esum4 += dE4;
+      nacc += 1u;
+    }
+    return;
   }
   // swap by arithmetic: the field of i holds a and becomes b, that of j holds b and becomes a; a
   // rejected trial stores the rows back unchanged (no branch)
@@ -389,10 +434,9 @@ __device__ __forceinline__ void store_tile_bytes(unsigned char* lo, unsigned cha
   }
 }
 
-template <int C>
+template <int C, int NT>
 __device__ __forceinline__ void write_back_tile(const Geom& G, const uint32_t* tile, uint32_t* lattice, int wlo,
                                                 uint32_t dwh, int t0y, int t0z, int rw, uint32_t zstride) {
-  constexpr int NT = kThreadNT;
   uint32_t offy[6];
 #pragma unroll
   for (int ry = 1; ry < 7; ++ry) {
@@ -415,7 +459,7 @@ __device__ __forceinline__ void write_back_tile(const Geom& G, const uint32_t* t
 #endif
 
 #ifdef __CUDACC__
-template <bool kFilter>
+template <int kFilter>
 __global__ void __launch_bounds__(kThreadNT, SMCX_BLOCKS_PER_SM)
 sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* __restrict__ coef,
                       const uint32_t* __restrict__ accept, const uint32_t* __restrict__ filt,
@@ -508,14 +552,14 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
     // x0 mod 8 only, which is the same for every cell of a pass: one uniform switch.
     {
       switch (x0 & 7) {
-        case 0: write_back_tile<0>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
-        case 1: write_back_tile<1>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
-        case 2: write_back_tile<2>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
-        case 3: write_back_tile<3>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
-        case 4: write_back_tile<4>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
-        case 5: write_back_tile<5>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
-        case 6: write_back_tile<6>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
-        default: write_back_tile<7>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 0: write_back_tile<0, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 1: write_back_tile<1, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 2: write_back_tile<2, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 3: write_back_tile<3, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 4: write_back_tile<4, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 5: write_back_tile<5, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 6: write_back_tile<6, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        default: write_back_tile<7, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
       }
     }
   }
@@ -537,11 +581,165 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
   }
 }
 
+
+// ---- persistent variant ---------------------------------------------------------------------------
+// One block of kPersistWarps warps per SM for the whole colour pass.  Every warp owns an 8 KB tile
+// area (32 cells, row r of lane l at word r * 32 + l) and walks over batches of 32 consecutive cells
+// of the colour on its own: no block barrier after the table load, so the warps of an SM drift apart
+// and the staging / write-back of one overlaps the trial arithmetic of the others.  The shared memory
+// left over holds the whole threshold table T (kAcceptDirect), which turns the acceptance test into
+// one clamp, one load and two compares.
+constexpr int kPersistMaxWarps = 20;
+constexpr int kPersistMinWarps = 16;
+constexpr int kPersistTileBytes = kThreadTileWords * 32 * 4;             // per warp
+constexpr int kPersistSmemMax = 232448 - 1024;                           // 227 KB less the static part / reserve
+
+// warps per block for a table of len entries, or 0 if the table does not fit next to 16 warps
+inline int persist_warps_for(int accept_len) {
+  for (int w = kPersistMaxWarps; w >= kPersistMinWarps; --w)
+    if ((size_t)w * kPersistTileBytes + 2 * 16 * 8 * sizeof(int4) + ((size_t)accept_len + 1) * 4 <= (size_t)kPersistSmemMax)
+      return w;
+  return 0;
+}
+inline size_t persist_smem(int warps, int accept_len) {
+  return (size_t)warps * kPersistTileBytes + 2 * 16 * 8 * sizeof(int4) + (((size_t)accept_len + 1) * 4 + 15) / 16 * 16;
+}
+
+__global__ void __launch_bounds__(kPersistMaxWarps * 32, 1)
+sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4* __restrict__ coef,
+                        const uint32_t* __restrict__ accept, DevState* __restrict__ st, int colour) {
+  constexpr int NT = 32;                                        // row stride of a warp's tile area (words)
+  extern __shared__ __align__(16) uint32_t smem_w[];
+  const int n_warps = blockDim.x >> 5, warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  uint32_t* tile = smem_w + warp * (kThreadTileWords * NT) + lane;
+  int4* s_coef0 = reinterpret_cast<int4*>(smem_w + n_warps * (kThreadTileWords * NT));   // [16][8 slots]
+  int4* s_coef1 = s_coef0 + 16 * 8;
+  uint32_t* s_T = reinterpret_cast<uint32_t*>(s_coef1 + 16 * 8);
+  __shared__ unsigned s_acc[kPersistMaxWarps];
+  for (int k = threadIdx.x; k < 128; k += blockDim.x) {
+    const int ent = k >> 3;
+    s_coef0[k] = coef[ent * 2];
+    s_coef1[k] = coef[ent * 2 + 1];
+  }
+  for (int k = threadIdx.x; k <= G.accept_len; k += blockDim.x) s_T[k] = k < G.accept_len ? accept[k] : 0u;
+
+  const uint32_t t = (uint32_t)st->sweep;
+  int ox, oy, oz;
+  sweep_origin(G, t, ox, oy, oz);
+  int esum = 0;                                                 // kDEScale * sum of accepted dE of this thread
+  unsigned nacc = 0;
+  long long esum_total = 0;
+  const int rw = G.Lx >> 3;                                     // words per lattice row
+  const uint32_t zstride = (uint32_t)G.Ly * (uint32_t)rw;
+  const uint32_t ctr3 = TAG_TRIAL | ((uint32_t)colour << 8);
+  TrialEnv env;
+  env.coef = smem_ptr(s_coef0) + (lane & 7) * 16;
+  env.filt = smem_ptr(s_T);
+  env.accept = accept;
+  env.accept_len = G.accept_len;
+  env.filter_E = 0;
+  env.tmax4 = 4u * (uint32_t)G.accept_len;
+  const uint32_t n_batches = (G.cells_per_colour + 31u) >> 5;
+  __syncthreads();
+  // warp-major numbering: the batches left over after the last full round go to the low warps of
+  // every block, not to all warps of the low blocks
+  for (uint32_t batch = (uint32_t)warp * gridDim.x + blockIdx.x; batch < n_batches; batch += (uint32_t)n_warps * gridDim.x) {
+    const uint32_t m = batch * 32u + (uint32_t)lane;
+    if (m < G.cells_per_colour) {
+      int cx, cy, cz;
+      colour_cell(G, m, colour, cx, cy, cz);
+      const int x0 = (ox + cx * 4 - 2 + G.Lx) % G.Lx;
+      const int t0y = (oy + cy * 4 - 2 + G.Ly) % G.Ly;
+      const int t0z = (oz + cz * 4 - 2 + G.Lz) % G.Lz;
+      const int wlo = x0 >> 3, sh = 4 * (x0 & 7);
+      const int whi = wlo + 1 == rw ? 0 : wlo + 1;
+      const uint32_t dwh = (uint32_t)(whi - wlo);
+      {
+        uint32_t offy[8];
+#pragma unroll
+        for (int ry = 0; ry < 8; ++ry) {
+          int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
+          offy[ry] = (uint32_t)gy * (uint32_t)rw + (uint32_t)wlo;
+        }
+#pragma unroll 2
+        for (int rz = 0; rz < 8; ++rz) {
+          int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
+          const uint32_t zoff = (uint32_t)gz * zstride;
+          uint32_t lo[8], hi[8];
+#pragma unroll
+          for (int ry = 0; ry < 8; ++ry) {
+            const uint32_t idx = zoff + offy[ry];
+            lo[ry] = lattice[idx];
+            hi[ry] = lattice[idx + dwh];
+          }
+#pragma unroll
+          for (int ry = 0; ry < 8; ++ry) tile[(rz * 8 + ry) * NT] = __funnelshift_r(lo[ry], hi[ry], sh);
+        }
+      }
+      const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
+#pragma unroll 1
+      for (int lzy = 0; lzy < 16; ++lzy) {
+        uint32_t* p_row = tile + (((lzy >> 2) + 2) * 8 + (lzy & 3) + 2) * NT;
+        const uint32_t q0 = (uint32_t)lzy * 4u;
+        uint32_t ra = p_row[-NT], rb = p_row[-8 * NT];
+#define SMCX_TRIAL_PAIR(LX)                                                                                          \
+        {                                                                                                            \
+          const Philox4 r = philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1);                               \
+          trial_thread<0, LX + 2, kAcceptDirect, NT>(G, p_row, env, r.x, r.y, ra, rb, esum, nacc);                   \
+          trial_thread<1, LX + 2, kAcceptDirect, NT>(G, p_row, env, r.z, r.w, ra, rb, esum, nacc);                   \
+        }
+        SMCX_TRIAL_PAIR(0) SMCX_TRIAL_PAIR(1) SMCX_TRIAL_PAIR(2) SMCX_TRIAL_PAIR(3)
+#undef SMCX_TRIAL_PAIR
+      }
+      switch (x0 & 7) {
+        case 0: write_back_tile<0, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 1: write_back_tile<1, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 2: write_back_tile<2, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 3: write_back_tile<3, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 4: write_back_tile<4, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 5: write_back_tile<5, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        case 6: write_back_tile<6, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+        default: write_back_tile<7, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
+      }
+      esum_total += esum / kDEScale;                            // per cell: 128 trials cannot overflow int32
+      esum = 0;
+    }
+  }
+  // a8: one atomic pair per block
+  for (int o = 16; o > 0; o >>= 1) {
+    esum_total += __shfl_down_sync(0xffffffffu, esum_total, o);
+    nacc += __shfl_down_sync(0xffffffffu, nacc, o);
+  }
+  __shared__ long long s_e64[kPersistMaxWarps];
+  if (lane == 0) { s_e64[warp] = esum_total; s_acc[warp] = nacc; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    long long e = 0; unsigned a = 0;
+    for (int i = 0; i < n_warps; ++i) { e += s_e64[i]; a += s_acc[i]; }
+    if (a) {
+      atomicAdd(reinterpret_cast<unsigned long long*>(&st->e_run), (unsigned long long)e);
+      atomicAdd(&st->accepted, (unsigned long long)a);
+    }
+  }
+}
+
 inline size_t thread_kernel_smem() {
   return (size_t)kThreadTileWords * kThreadNT * 4 + 2 * 16 * 8 * sizeof(int4) + kFilterWords * 4;
 }
 
+inline int launch_thread_persistent(const Geom& G, uint32_t* lattice, const int32_t* d_coef, const uint32_t* accept,
+                                    DevState* st, int colour, int warps, int sm_count, cudaStream_t stream) {
+  const unsigned n_batches = (G.cells_per_colour + 31u) / 32u;
+  const unsigned want = (n_batches + warps - 1) / warps;
+  const unsigned grid = want < (unsigned)sm_count ? want : (unsigned)sm_count;
+  sweep_thread_persistent<<<grid, warps * 32, persist_smem(warps, G.accept_len), stream>>>(
+      G, lattice, reinterpret_cast<const int4*>(d_coef), accept, st, colour);
+  return 0;
+}
+
 inline int configure_thread_per_cell() {
+  if (cudaFuncSetAttribute(sweep_thread_persistent, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           kPersistSmemMax) != cudaSuccess) return -1;
   if (cudaFuncSetAttribute(sweep_thread_per_cell<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)thread_kernel_smem()) != cudaSuccess) return -1;
   if (cudaFuncSetAttribute(sweep_thread_per_cell<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,

@@ -35,10 +35,12 @@ static long long local_energy(const uint32_t* tile, int px, int py, int pz, int 
   return e;
 }
 
-template <bool F>
+// F: kAcceptGlobal / kAcceptFilter (filt = two-level tables) / kAcceptDirect (filt = T followed by one zero entry)
+template <int F>
 static void run_trial(int bi, int X, uint32_t* p, const char* cb, const uint32_t* filt, const uint32_t* T, int len, int E,
                       uint32_t w, uint32_t u, int& es, unsigned& na) {
   TrialEnv env; env.coef = smem_ptr(cb); env.filt = smem_ptr(filt); env.accept = T; env.accept_len = len; env.filter_E = E;
+  env.tmax4 = 4u * (uint32_t)len;
   static Geom G; static bool init = false; if (!init) { G.key0 = 1; G.key1 = 2; set_thread_masks(G); init = true; }
   uint32_t ra = bi ? p[1] : p[-1], rb = bi ? p[8] : p[-8];
   const uint32_t era = bi ? p[-1] : p[1], erb = bi ? p[-8] : p[8];
@@ -53,6 +55,7 @@ int main() {
   const int len = (int)std::floor(32.0 * std::log(2.0) * kT) + 2;
   std::vector<uint32_t> T(len);
   for (int d = 0; d < len; ++d) { double x = std::exp(-(double)d / kT) * 4294967296.0; T[d] = x >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)std::floor(x); }
+  std::vector<uint32_t> Tz(T); Tz.push_back(0u);   // the table as the persistent kernel keeps it in shared memory
   std::vector<uint32_t> filt(kFilterWords);
   int nq; const int E = build_accept_filter(T.data(), len, filt.data(), &nq);
   printf("len %d filter E %d nq %d\n", len, E, nq);
@@ -98,13 +101,14 @@ int main() {
         okref = dEref <= 0 || (dEref < len && u < T[dEref]);
         if (!okref) memcpy(ref, tile, sizeof(tile));
       } else if (it % 3 == 0) u = rng() % 4;
-      for (int variant = (cls == 2 ? 0 : 1); variant < 2; ++variant) {
+      for (int variant = (cls == 2 ? 0 : 1); variant < 3; ++variant) {
         uint32_t got[64]; memcpy(got, tile, sizeof(tile));
         int es = 0; unsigned na = 0;
         uint32_t* p = got + z * 8 + y;
         const char* cb = reinterpret_cast<const char*>(tab) + (it & 7) * 16;
-        if (variant == 0) run_trial<true>(bi, X, p, cb, filt.data(), T.data(), len, E, w, u, es, na);
-        else run_trial<false>(bi, X, p, cb, filt.data(), T.data(), len, E, w, u, es, na);
+        if (variant == 0) run_trial<kAcceptFilter>(bi, X, p, cb, filt.data(), T.data(), len, E, w, u, es, na);
+        else if (variant == 1) run_trial<kAcceptGlobal>(bi, X, p, cb, filt.data(), T.data(), len, E, w, u, es, na);
+        else run_trial<kAcceptDirect>(bi, X, p, cb, Tz.data(), T.data(), len, E, w, u, es, na);
         const bool same = memcmp(got, ref, sizeof(ref)) == 0;
         if (!same || na != (okref ? 1u : 0u) || es != (okref ? (int)dEref : 0)) {
           if (bad < 10) printf("MISMATCH variant %d bi %d X %d y %d z %d dir %d a %d b %d dEref %lld okref %d got es %d na %u same %d u %u\n",

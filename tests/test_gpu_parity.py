@@ -11,7 +11,8 @@ from smcx_inputs import get_config, make_accept_table, make_epi, scaled_config
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_THREAD_PER_CELL]
+KERNELS = [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_THREAD_PER_CELL, smcx.KERNEL_THREAD_PERSISTENT]
+KERNEL_IDS = ["warp", "thread", "persistent"]
 
 
 def _supported(cfg, kernel):
@@ -40,7 +41,7 @@ def _assert_sro(g, o):
     assert np.allclose(ga, oa, rtol=1e-9, atol=1e-9, equal_nan=True)
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
 def test_config1_full_run_species_after_every_sweep(kernel):
     cfg = get_config(1)
     g, o = _pair(cfg, kernel)
@@ -56,7 +57,7 @@ def test_config1_full_run_species_after_every_sweep(kernel):
     _assert_sro(g, o)
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
 def test_config2_anneal_prefix(kernel):
     """Config 2 with its per-sweep temperature table; SRO sampled every 10 sweeps here
     (every 100 over the full 2,000 in the slow test)."""
@@ -105,7 +106,7 @@ def test_config3_fcc_five_species_prefix():
     _assert_sro(g, o)
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
 def test_config4_shape_ragged_grid(kernel):
     """Config 4's species/EPI/kT on a non-cubic lattice whose cells per colour (13*11*9) fill
     neither a warp nor a block evenly."""
@@ -119,7 +120,7 @@ def test_config4_shape_ragged_grid(kernel):
     _assert_sro(g, o)
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
 def test_config4_full_size_invariants(kernel):
     """BCC 800^3 in the launch configuration bench.py times: conservation (P5), energy bookkeeping
     (P6: H recomputed by the reduction kernel == E0 + sum of accepted dE) and the species counts."""
@@ -180,7 +181,7 @@ def test_full_size_oracle_prefix(k, n):
     assert (g.energy_trace() == o.energy_trace()).all()
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
 def test_resume_and_determinism(kernel):
     cfg = scaled_config(1, (24, 16, 32))
     a = smcx.Lattice.from_config(cfg, kernel=kernel)
@@ -199,12 +200,14 @@ def test_thread_and_warp_kernels_agree():
     cfg = scaled_config(2, (40, 48, 56), n_sweeps=5)
     a = smcx.Lattice.from_config(cfg, kernel=smcx.KERNEL_WARP_PER_CELL)
     b = smcx.Lattice.from_config(cfg, kernel=smcx.KERNEL_THREAD_PER_CELL)
-    assert (a.storage, b.storage) == (smcx.STORAGE_U8, smcx.STORAGE_2BIT)
-    a.sweep(5)
-    b.sweep(5)
-    assert (a.species() == b.species()).all()
-    assert (a.energy_trace() == b.energy_trace()).all()
-    assert (a.sro()[1] == b.sro()[1]).all()
+    c = smcx.Lattice.from_config(cfg, kernel=smcx.KERNEL_THREAD_PERSISTENT)
+    assert (a.storage, b.storage, c.storage) == (smcx.STORAGE_U8, smcx.STORAGE_2BIT, smcx.STORAGE_2BIT)
+    for x in (a, b, c):
+        x.sweep(5)
+    for x in (b, c):
+        assert (a.species() == x.species()).all()
+        assert (a.energy_trace() == x.energy_trace()).all()
+        assert (a.sro()[1] == x.sro()[1]).all()
 
 
 @pytest.mark.parametrize("lat,dims,n_sp,n_shells,w", [
@@ -284,7 +287,7 @@ def test_energy_trace_ring_and_ranges():
         g.energy_trace(5, 3)       # beyond the sweeps done
 
 
-@pytest.mark.parametrize("kernel", KERNELS, ids=["warp", "thread"])
+@pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
 @pytest.mark.parametrize("kind", ["staircase", "short", "non_monotone", "long_kT"])
 def test_arbitrary_threshold_tables(kernel, kind):
     """The threshold table is input data: the library must take the same decisions as `u < T[dE]` for
