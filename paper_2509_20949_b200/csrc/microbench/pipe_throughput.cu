@@ -28,6 +28,10 @@ __global__ void k(uint32_t* out, uint32_t seed, uint32_t m) {
       if (OP == 9) { asm volatile("mul.hi.u32 %0, %0, %1;" : "+r"(a[i]) : "r"(c)); asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(c), "r"(seed)); }
       if (OP == 10) { asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a[i]) : "r"(c), "r"(seed)); asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(c), "r"(seed)); }
       if (OP == 11) { asm volatile("popc.b32 %0, %0;" : "+r"(a[i])); asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(c), "r"(seed)); asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(c), "r"(seed)); asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(c), "r"(seed));}
+      if (OP == 13) asm volatile("dp2a.lo.s32.u32 %0, %0, %1, %2;" : "+r"(a[i]) : "r"(c), "r"(seed));
+      if (OP == 14) asm volatile("dp4a.s32.u32 %0, %0, %1, %2;" : "+r"(a[i]) : "r"(c), "r"(seed));
+      if (OP == 15) { asm volatile("dp2a.hi.s32.u32 %0, %0, %1, %2;" : "+r"(a[i]) : "r"(c), "r"(seed)); asm volatile("lop3.b32 %0, %0, %1, %2, 0x96;" : "+r"(a[i]) : "r"(c), "r"(seed)); }
+      if (OP == 16) { asm volatile("dp2a.lo.s32.u32 %0, %0, %1, %2;" : "+r"(a[i]) : "r"(c), "r"(seed)); asm volatile("mad.lo.u32 %0, %0, %1, %2;" : "+r"(a[i]) : "r"(c), "r"(seed)); }
       if (OP == 12) { int p; asm volatile("{.reg .pred q; setp.lt.u32 q, %1, %2; selp.u32 %0, 1, 0, q;}" : "=r"(p) : "r"(a[i]), "r"(c)); a[i] += p; }
     }
   }
@@ -52,5 +56,6 @@ int main() {
   run<0>("mul.hi.u32", 1); run<1>("mul.wide.u32(+xor)", 2); run<2>("shr.u32", 1); run<3>("lop3", 1); run<4>("popc", 1);
   run<5>("prmt", 1); run<6>("mad.lo", 1); run<7>("add", 1); run<8>("shf.wrap", 1); run<9>("mul.hi+lop3", 2); run<10>("mad.lo+lop3", 2);
   run<11>("popc+3lop3", 4); run<12>("setp+selp+add", 3);
+  run<13>("dp2a.lo", 1); run<14>("dp4a", 1); run<15>("dp2a.hi+lop3", 2); run<16>("dp2a.lo+mad.lo", 2);
   return 0;
 }

@@ -84,6 +84,7 @@ struct Plan {
   int storage;
   int kernel;
   int coef_class;   // build_thread_coefficients: 2 = the filter variant of the thread kernel applies
+  bool coef_packed; // pack_thread_coefficients: the 16-bit coefficient rows are exact
   Layout lay;
 };
 
@@ -171,10 +172,13 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   // kernel / storage choice
   bool fast_ok = thread_kernel_supported(G);
   plan->coef_class = 0;
+  plan->coef_packed = false;
   if (fast_ok) {  // the packed kernel computes dE in int32 from a coefficient table: magnitudes must fit
     int32_t coef[16 * kCoefInts];
     plan->coef_class = build_thread_coefficients(p->epi, n, coef);
     fast_ok = plan->coef_class > 0;
+    int32_t pk[16 * 4];
+    plan->coef_packed = fast_ok && pack_thread_coefficients(coef, pk);
   }
   int kernel = p->kernel, storage = p->storage;
   if (kernel == SMCX_KERNEL_AUTO) {
@@ -199,7 +203,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   L.species = off;
   off += align_up(storage == SMCX_STORAGE_U8 ? (size_t)n_sites : (size_t)((n_sites + 15) / 16) * 4, 256);
   L.epi = off;     off += align_up((size_t)p->n_shells * n * n * sizeof(int32_t), 256);
-  L.coef = off;    off += align_up((size_t)16 * kCoefInts * sizeof(int32_t), 256);
+  L.coef = off;    off += align_up((size_t)16 * (kCoefInts + 4) * sizeof(int32_t), 256);
   L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
   L.filter = off;  off += align_up((size_t)kFilterWords * sizeof(uint32_t), 256);
   L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
@@ -362,8 +366,8 @@ int launch_colour_pass(smcx* h, int colour) {
   if (P.kernel == SMCX_KERNEL_THREAD_PERSISTENT) {
     const int warps = persist_warps_for(G.accept_len);
     if (warps > 0) {
-      const int rc = launch_thread_persistent(G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_coef(), h->d_accept(),
-                                              h->d_state(), colour, warps, h->sm_count, h->stream);
+      const int rc = launch_thread_persistent(G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_coef(), P.coef_packed,
+                                              h->d_accept(), h->d_state(), colour, warps, h->sm_count, h->stream);
       h->launches++;
       if (rc != 0) { h->err = "persistent thread-per-cell launch failed"; return SMCX_E_CUDA; }
       return SMCX_OK;
@@ -494,8 +498,11 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     DevState zero{};
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_state(), &zero, sizeof(zero), cudaMemcpyHostToDevice, h->stream));
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_epi(), h->epi.data(), h->epi.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
-    int32_t coef[16 * kCoefInts] = {0};
-    if (is_thread_kernel(h->plan.kernel)) build_thread_coefficients(h->epi.data(), h->plan.G.n_species, coef);
+    int32_t coef[16 * (kCoefInts + 4)] = {0};   // 32-bit rows, then the packed 16-bit rows
+    if (is_thread_kernel(h->plan.kernel)) {
+      build_thread_coefficients(h->epi.data(), h->plan.G.n_species, coef);
+      pack_thread_coefficients(coef, coef + 16 * kCoefInts);
+    }
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_coef(), coef, sizeof(coef), cudaMemcpyHostToDevice, h->stream));
     SMCX_CUDA(h, cudaMemsetAsync(h->d_trace(), 0, (size_t)h->plan.G.trace_capacity * sizeof(long long), h->stream));
     SMCX_CUDA(h, cudaStreamSynchronize(h->stream));  // &zero and epi must stay valid until copied

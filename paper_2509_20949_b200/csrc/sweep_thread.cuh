@@ -105,6 +105,22 @@ inline int build_thread_coefficients(const int32_t* epi, int n_species, int32_t*
   return cls;
 }
 
+// Host: the seven coefficients of every ordered pair as signed 16-bit halves, [a*4+b][4] int32:
+//   { cl0 | ch0' << 16, cb0 | cl1 << 16, ch1' | cb1 << 16, corr' } (all times kDEScale, as in coef),
+// the operand layout of dp2a (two 16-bit factors per word times two population counts packed in bytes).
+// Returns false if a coefficient does not fit 16 bits (the persistent kernel then takes the 32-bit rows).
+inline bool pack_thread_coefficients(const int32_t* coef /*16*8*/, int32_t* pk /*16*4*/) {
+  bool fits = true;
+  for (int e = 0; e < 16; ++e) {
+    const int32_t* c = coef + e * kCoefInts;
+    for (int k = 0; k < 6; ++k) fits = fits && c[k] >= -32768 && c[k] <= 32767;
+    for (int k = 0; k < 3; ++k)
+      pk[e * 4 + k] = (int32_t)(((uint32_t)c[2 * k] & 0xFFFFu) | ((uint32_t)c[2 * k + 1] << 16));
+    pk[e * 4 + 3] = c[6];
+  }
+  return fits;
+}
+
 // Host: two-level filter tables for a threshold table T (T[d] = 0 understood for d >= len).
 // Returns E >= 0 such that 0 <= T[d] - mulhi(Tq[d>>6], Tr[d&63]) <= E for all d <= kFilterDmax, or
 // -1 if no such small bound holds (then the kernel reads T[d] directly).  For
@@ -182,6 +198,16 @@ __host__ __device__ __forceinline__ uint32_t mad_u32(uint32_t a, uint32_t b, uin
   return d;
 #else
   return a * b + c;
+#endif
+}
+// c + lo16(a) * byte0(b) + hi16(a) * byte1(b), 16-bit halves signed, bytes unsigned: one IDP.2A (FMA pipe)
+__host__ __device__ __forceinline__ int dp2a_lo(uint32_t a, uint32_t b, int c) {
+#ifdef __CUDA_ARCH__
+  int d;
+  asm("dp2a.lo.s32.u32 %0, %1, %2, %3;" : "=r"(d) : "r"(a), "r"(b), "r"(c));
+  return d;
+#else
+  return c + (int)(int16_t)(a & 0xFFFFu) * (int)(b & 0xFFu) + (int)(int16_t)(a >> 16) * (int)((b >> 8) & 0xFFu);
 #endif
 }
 // Shared-memory tables are addressed on the device by 32-bit shared addresses formed with mad_u32.
@@ -289,7 +315,7 @@ inline void set_thread_masks(Geom& G) {
 // One trial (a4-a6).  p_i points at the tile row of site i (row stride STRIDE words).  ra / rb carry
 // two rows from one trial of an x-row to the next: a trial with bi == 0 takes rows y-1 and z-1 and
 // leaves y+1 and z+1 (which it cannot have modified), a trial with bi == 1 the other way round.
-template <int bi, int X, int MODE, int STRIDE>
+template <int bi, int X, int MODE, int STRIDE, bool PK = false>
 __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p_i, const TrialEnv& env, uint32_t w_dir,
                                                       uint32_t u, uint32_t& ra, uint32_t& rb, int& esum4,
                                                       unsigned& nacc) {
@@ -340,8 +366,17 @@ __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p
   const uint32_t a4 = (own_i >> K::shi) & 0x30u;
   const uint32_t b4 = (own_j >> mad_u32(dx, 4u, G.kc[kKcShj0 + slot])) & 0x30u;
   const smem_ptr_t crow = smem_index(smem_index(env.coef, a4, 32u), b4, 8u);
-  const int4 c0 = lds_int4(crow, 0), c1 = lds_int4(crow, 2048);
-  const int dE4 = c1.z + c0.x * pt1 + c0.y * ph1 + c0.z * pb1 + c0.w * pt2 + c1.x * ph2 + c1.y * pb2;   // 4 dE
+  int dE4;                                                   // 4 dE
+  if (PK) {
+    // 16-bit coefficient pairs: one LDS.128, three byte packs and three IDP.2A
+    const int4 c = lds_int4(crow, 0);
+    dE4 = dp2a_lo((uint32_t)c.x, mad_u32((uint32_t)ph1, 256u, (uint32_t)pt1), c.w);
+    dE4 = dp2a_lo((uint32_t)c.y, mad_u32((uint32_t)pt2, 256u, (uint32_t)pb1), dE4);
+    dE4 = dp2a_lo((uint32_t)c.z, mad_u32((uint32_t)pb2, 256u, (uint32_t)ph2), dE4);
+  } else {
+    const int4 c0 = lds_int4(crow, 0), c1 = lds_int4(crow, 2048);
+    dE4 = c1.z + c0.x * pt1 + c0.y * ph1 + c0.z * pb1 + c0.w * pt2 + c1.x * ph2 + c1.y * pb2;
+  }
   // Eq. 3 in integer form
   bool ok;
   if (MODE == kAcceptDirect) {
@@ -540,7 +575,7 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
       uint32_t ra = p_row[-NT], rb = p_row[-8 * NT];
 #define SMCX_TRIAL_PAIR(LX)                                                                                          \
       {                                                                                                              \
-        const Philox4 r = philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1);                                 \
+        const Philox4 r = philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1);                                \
         trial_thread<0, LX + 2, kFilter, NT>(G, p_row, env, r.x, r.y, ra, rb, esum, nacc);                                                \
         trial_thread<1, LX + 2, kFilter, NT>(G, p_row, env, r.z, r.w, ra, rb, esum, nacc);                                                \
       }
@@ -589,10 +624,10 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
 // and the staging / write-back of one overlaps the trial arithmetic of the others.  The shared memory
 // left over holds the whole threshold table T (kAcceptDirect), which turns the acceptance test into
 // one clamp, one load and two compares.
-constexpr int kPersistMaxWarps = 20;
+constexpr int kPersistMaxWarps = 20;   // a multiple of the four sub-partitions: 18 or 21 warps load them unevenly (measured)
 constexpr int kPersistMinWarps = 16;
 constexpr int kPersistTileBytes = kThreadTileWords * 32 * 4;             // per warp
-constexpr int kPersistSmemMax = 232448 - 1024;                           // 227 KB less the static part / reserve
+constexpr int kPersistSmemMax = 232448 - 512;                           // 227 KB less the static part / reserve
 
 // warps per block for a table of len entries, or 0 if the table does not fit next to 16 warps
 inline int persist_warps_for(int accept_len) {
@@ -605,6 +640,7 @@ inline size_t persist_smem(int warps, int accept_len) {
   return (size_t)warps * kPersistTileBytes + 2 * 16 * 8 * sizeof(int4) + (((size_t)accept_len + 1) * 4 + 15) / 16 * 16;
 }
 
+template <bool PK>
 __global__ void __launch_bounds__(kPersistMaxWarps * 32, 1)
 sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4* __restrict__ coef,
                         const uint32_t* __restrict__ accept, DevState* __restrict__ st, int colour) {
@@ -616,10 +652,15 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
   int4* s_coef1 = s_coef0 + 16 * 8;
   uint32_t* s_T = reinterpret_cast<uint32_t*>(s_coef1 + 16 * 8);
   __shared__ unsigned s_acc[kPersistMaxWarps];
+  // PK: coef points at the packed rows [16] int4; else at the 32-bit rows [16][2] int4
   for (int k = threadIdx.x; k < 128; k += blockDim.x) {
     const int ent = k >> 3;
-    s_coef0[k] = coef[ent * 2];
-    s_coef1[k] = coef[ent * 2 + 1];
+    if (PK) {
+      s_coef0[k] = coef[ent];
+    } else {
+      s_coef0[k] = coef[ent * 2];
+      s_coef1[k] = coef[ent * 2 + 1];
+    }
   }
   for (int k = threadIdx.x; k <= G.accept_len; k += blockDim.x) s_T[k] = k < G.accept_len ? accept[k] : 0u;
 
@@ -684,9 +725,9 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
         uint32_t ra = p_row[-NT], rb = p_row[-8 * NT];
 #define SMCX_TRIAL_PAIR(LX)                                                                                          \
         {                                                                                                            \
-          const Philox4 r = philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1);                               \
-          trial_thread<0, LX + 2, kAcceptDirect, NT>(G, p_row, env, r.x, r.y, ra, rb, esum, nacc);                   \
-          trial_thread<1, LX + 2, kAcceptDirect, NT>(G, p_row, env, r.z, r.w, ra, rb, esum, nacc);                   \
+          const Philox4 r = philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1);                              \
+          trial_thread<0, LX + 2, kAcceptDirect, NT, PK>(G, p_row, env, r.x, r.y, ra, rb, esum, nacc);               \
+          trial_thread<1, LX + 2, kAcceptDirect, NT, PK>(G, p_row, env, r.z, r.w, ra, rb, esum, nacc);               \
         }
         SMCX_TRIAL_PAIR(0) SMCX_TRIAL_PAIR(1) SMCX_TRIAL_PAIR(2) SMCX_TRIAL_PAIR(3)
 #undef SMCX_TRIAL_PAIR
@@ -727,18 +768,25 @@ inline size_t thread_kernel_smem() {
   return (size_t)kThreadTileWords * kThreadNT * 4 + 2 * 16 * 8 * sizeof(int4) + kFilterWords * 4;
 }
 
-inline int launch_thread_persistent(const Geom& G, uint32_t* lattice, const int32_t* d_coef, const uint32_t* accept,
+// d_coef: the 32-bit rows [16][8] int32 followed by the packed rows [16][4] int32
+inline int launch_thread_persistent(const Geom& G, uint32_t* lattice, const int32_t* d_coef, bool packed, const uint32_t* accept,
                                     DevState* st, int colour, int warps, int sm_count, cudaStream_t stream) {
   const unsigned n_batches = (G.cells_per_colour + 31u) / 32u;
   const unsigned want = (n_batches + warps - 1) / warps;
   const unsigned grid = want < (unsigned)sm_count ? want : (unsigned)sm_count;
-  sweep_thread_persistent<<<grid, warps * 32, persist_smem(warps, G.accept_len), stream>>>(
-      G, lattice, reinterpret_cast<const int4*>(d_coef), accept, st, colour);
+  if (packed)
+    sweep_thread_persistent<true><<<grid, warps * 32, persist_smem(warps, G.accept_len), stream>>>(
+        G, lattice, reinterpret_cast<const int4*>(d_coef + 16 * kCoefInts), accept, st, colour);
+  else
+    sweep_thread_persistent<false><<<grid, warps * 32, persist_smem(warps, G.accept_len), stream>>>(
+        G, lattice, reinterpret_cast<const int4*>(d_coef), accept, st, colour);
   return 0;
 }
 
 inline int configure_thread_per_cell() {
-  if (cudaFuncSetAttribute(sweep_thread_persistent, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  if (cudaFuncSetAttribute(sweep_thread_persistent<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                           kPersistSmemMax) != cudaSuccess) return -1;
+  if (cudaFuncSetAttribute(sweep_thread_persistent<false>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            kPersistSmemMax) != cudaSuccess) return -1;
   if (cudaFuncSetAttribute(sweep_thread_per_cell<true>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                            (int)thread_kernel_smem()) != cudaSuccess) return -1;

@@ -36,7 +36,7 @@ static long long local_energy(const uint32_t* tile, int px, int py, int pz, int 
 }
 
 // F: kAcceptGlobal / kAcceptFilter (filt = two-level tables) / kAcceptDirect (filt = T followed by one zero entry)
-template <int F>
+template <int F, bool PK = false>
 static void run_trial(int bi, int X, uint32_t* p, const char* cb, const uint32_t* filt, const uint32_t* T, int len, int E,
                       uint32_t w, uint32_t u, int& es, unsigned& na) {
   TrialEnv env; env.coef = smem_ptr(cb); env.filt = smem_ptr(filt); env.accept = T; env.accept_len = len; env.filter_E = E;
@@ -44,7 +44,7 @@ static void run_trial(int bi, int X, uint32_t* p, const char* cb, const uint32_t
   static Geom G; static bool init = false; if (!init) { G.key0 = 1; G.key1 = 2; set_thread_masks(G); init = true; }
   uint32_t ra = bi ? p[1] : p[-1], rb = bi ? p[8] : p[-8];
   const uint32_t era = bi ? p[-1] : p[1], erb = bi ? p[-8] : p[8];
-#define C(B, XX) if (bi == B && X == XX) { trial_thread<B, XX, F, 1>(G, p, env, w, u, ra, rb, es, na); if (ra != era || rb != erb) { printf("row carry mismatch\n"); exit(1);} es /= 4; return; }
+#define C(B, XX) if (bi == B && X == XX) { trial_thread<B, XX, F, 1, PK>(G, p, env, w, u, ra, rb, es, na); if (ra != era || rb != erb) { printf("row carry mismatch\n"); exit(1);} es /= 4; return; }
   C(0,2) C(0,3) C(0,4) C(0,5) C(1,2) C(1,3) C(1,4) C(1,5)
 #undef C
 }
@@ -59,7 +59,7 @@ int main() {
   std::vector<uint32_t> filt(kFilterWords);
   int nq; const int E = build_accept_filter(T.data(), len, filt.data(), &nq);
   printf("len %d filter E %d nq %d\n", len, E, nq);
-  long long n_over = 0, n_checked = 0, n_acc = 0, n_rare = 0, bad = 0;
+  long long n_packed = 0, n_over = 0, n_checked = 0, n_acc = 0, n_rare = 0, bad = 0;
   for (int rep = 0; rep < 400; ++rep) {
     const int nsp = 2 + rep % 3;
     for (int s = 0; s < 2; ++s) for (int a = 0; a < 4; ++a) for (int b = a; b < 4; ++b) {
@@ -76,6 +76,13 @@ int main() {
       tab[(ent * 8 + slot) * 4 + k] = coef[ent * 8 + k];
       tab[512 + (ent * 8 + slot) * 4 + k] = coef[ent * 8 + 4 + k];
     }
+    // packed 16-bit rows of the persistent kernel: [ent][8 slots] int4
+    int32_t pk[16 * 4];
+    const bool packable = pack_thread_coefficients(coef, pk);
+    alignas(16) static int32_t tabpk[16 * 8 * 4];
+    for (int ent = 0; ent < 16; ++ent) for (int slot = 0; slot < 8; ++slot) for (int k = 0; k < 4; ++k)
+      tabpk[(ent * 8 + slot) * 4 + k] = pk[ent * 4 + k];
+    if (packable) ++n_packed;
     uint32_t tile[64];
     for (auto& w : tile) { w = 0; for (int f = 0; f < 16; ++f) w |= (uint32_t)(rng() % nsp) << (2 * f); }
     for (int it = 0; it < 3000; ++it) {
@@ -101,14 +108,15 @@ int main() {
         okref = dEref <= 0 || (dEref < len && u < T[dEref]);
         if (!okref) memcpy(ref, tile, sizeof(tile));
       } else if (it % 3 == 0) u = rng() % 4;
-      for (int variant = (cls == 2 ? 0 : 1); variant < 3; ++variant) {
+      for (int variant = (cls == 2 ? 0 : 1); variant < (packable ? 4 : 3); ++variant) {
         uint32_t got[64]; memcpy(got, tile, sizeof(tile));
         int es = 0; unsigned na = 0;
         uint32_t* p = got + z * 8 + y;
         const char* cb = reinterpret_cast<const char*>(tab) + (it & 7) * 16;
         if (variant == 0) run_trial<kAcceptFilter>(bi, X, p, cb, filt.data(), T.data(), len, E, w, u, es, na);
         else if (variant == 1) run_trial<kAcceptGlobal>(bi, X, p, cb, filt.data(), T.data(), len, E, w, u, es, na);
-        else run_trial<kAcceptDirect>(bi, X, p, cb, Tz.data(), T.data(), len, E, w, u, es, na);
+        else if (variant == 2) run_trial<kAcceptDirect>(bi, X, p, cb, Tz.data(), T.data(), len, E, w, u, es, na);
+        else run_trial<kAcceptDirect, true>(bi, X, p, reinterpret_cast<const char*>(tabpk) + (it & 7) * 16, Tz.data(), T.data(), len, E, w, u, es, na);
         const bool same = memcmp(got, ref, sizeof(ref)) == 0;
         if (!same || na != (okref ? 1u : 0u) || es != (okref ? (int)dEref : 0)) {
           if (bad < 10) printf("MISMATCH variant %d bi %d X %d y %d z %d dir %d a %d b %d dEref %lld okref %d got es %d na %u same %d u %u\n",
@@ -120,7 +128,7 @@ int main() {
       ++n_checked; n_acc += okref;
     }
   }
-  printf("coef-overflow reps %lld; checked %lld trials, accepted %lld, forced-near-threshold %lld, mismatches %lld\n", n_over, n_checked, n_acc, n_rare, bad);
+  printf("packed-coefficient reps %lld, coef-overflow reps %lld; checked %lld trials, accepted %lld, forced-near-threshold %lld, mismatches %lld\n", n_packed, n_over, n_checked, n_acc, n_rare, bad);
   return bad != 0;
 }
 #endif

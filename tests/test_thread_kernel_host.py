@@ -22,7 +22,7 @@ def _nvcc():
 @pytest.mark.skipif(_nvcc() is None, reason="nvcc not available")
 def test_trial_arithmetic_matches_brute_force(tmp_path):
     exe = str(tmp_path / "thread_trial_check")
-    build = subprocess.run([_nvcc(), "-O1", "-std=c++17", "-Wno-deprecated-gpu-targets", "-o", exe, SRC],
+    build = subprocess.run([_nvcc(), "-O1", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-o", exe, SRC],
                            capture_output=True, text=True, timeout=600)
     assert build.returncode == 0, build.stdout + build.stderr
     run = subprocess.run([exe], capture_output=True, text=True, timeout=600)
