@@ -50,6 +50,25 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback"
 
 
+# What binds the thread-per-cell kernels is the integer ALU pipe: instructions per trial on that
+# pipe from the SASS of the trial loop plus the share of the staging / write-back code (profiles/), the cycles an
+# IMAD.WIDE / POPC holds the pipe from profiles/r1_pipe_microbench.md.
+ALU_PIPE = {2: {"alu_inst": 59.0, "wide": 9.0, "popc": 6.0}, 3: {"alu_inst": 51.0, "wide": 8.0, "popc": 6.0}}
+
+
+def alu_view(kernel: int, trials_per_s: float, clocks: dict):
+    if kernel not in ALU_PIPE:
+        return None
+    k = ALU_PIPE[kernel]
+    mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+    peak = 148 * 4 * mhz * 1e6 / 2.0                      # ALU-pipe warp-instructions/s: 1 per 2 cycles per sub-partition
+    inst = trials_per_s / 32.0 * k["alu_inst"]
+    busy = trials_per_s / 32.0 * (2.0 * k["alu_inst"] + 2.6 * k["wide"] + 1.0 * k["popc"]) / (148 * 4 * mhz * 1e6)
+    return {"bound": "alu", "achieved": inst, "peak": peak, "unit": "warp-inst/s", "frac": inst / peak,
+            "alu_inst_per_trial": k["alu_inst"], "pipe_busy_frac_with_wide_and_popc": busy,
+            "note": "whole-step trials/s; counts from SASS + ncu in profiles/"}
+
+
 def workload_string(cfg) -> str:
     lat = "BCC" if cfg.lattice == 0 else "FCC"
     return (f"{lat} {cfg.dims[0]}x{cfg.dims[1]}x{cfg.dims[2]} conventional cells ({cfg.n_sites} sites), "
@@ -326,6 +345,7 @@ def run_cuda(args, cfg, rank, world, local_rank):
                          "traffic": traffic, "peak_kind": peak_kind,
                          "kernel": {1: "sweep_warp_per_cell", 2: "sweep_thread_per_cell", 3: "sweep_thread_persistent"}[lat.kernel],
                          "algorithmic_bytes_per_trial": ALGO_BYTES_PER_TRIAL, "launch_ms": launch_ms},
+            "alu_view": alu_view(lat.kernel, value / world, clocks),
             "e2e": {"value": e2e_value, "unit": "trial swaps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps,
                     "what": "smcx_set_species(host) + steps x (smcx_set_temperature(host table) + smcx_sweep(1) + "
