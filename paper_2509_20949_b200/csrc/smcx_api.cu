@@ -290,7 +290,11 @@ int run_pair_counts(smcx* h, std::vector<unsigned long long>& host_M) {
   const long long n_conv = (long long)G.Lx * G.Ly * G.Lz;
   const int grid = grid_for(h, n_conv, 256);
   const size_t sm = (size_t)n_hist * sizeof(unsigned);
-  if (P.storage == SMCX_STORAGE_U8) {
+  if (P.storage == SMCX_STORAGE_2BIT && G.lattice == SMCX_BCC && G.n_shells == 2) {
+    // bit-parallel reduction: one thread per packed word (16 sites)
+    const int gridw = grid_for(h, n_conv / 8, 256);
+    pair_count_bcc2_kernel<<<gridw, 256, 0, h->stream>>>(G, reinterpret_cast<const uint32_t*>(h->d_species()), h->d_counts());
+  } else if (P.storage == SMCX_STORAGE_U8) {
     if (G.B == 2) pair_count_kernel<StoreU8, 2><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
     else          pair_count_kernel<StoreU8, 4><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
   } else {
