@@ -66,6 +66,9 @@ def _load():
         "oracle_get_visits": (None, [C.c_void_p, u32p]),
         "oracle_pair_counts": (None, [C.c_void_p, i64p]),
         "oracle_sro": (None, [C.c_void_p, f64p, i64p]),
+        "oracle_exchange_delta": (C.c_double, [C.c_int64, C.c_int64, C.c_int32, C.c_int32]),
+        "oracle_exchange_accept": (C.c_int, [C.c_int64, C.c_int64, C.c_int32, C.c_int32, C.c_uint32]),
+        "oracle_exchange_draw": (C.c_uint32, [C.c_uint64, C.c_uint64, C.c_uint32]),
     }
     for name, (res, args) in sig.items():
         fn = getattr(lib, name)
@@ -94,6 +97,42 @@ def shell(lattice: int, s: int) -> np.ndarray:
     buf = np.zeros((512, 3), dtype=np.int32)
     n = lib.oracle_shell(lattice, s, _ptr(buf, C.c_int32), 512)
     return buf[:n].copy()
+
+
+def exchange_delta(E_i: int, E_j: int, kT_i: int, kT_j: int) -> float:
+    """Delta of Eq. 6 for integer energies and temperatures in 0.1 meV."""
+    return float(_load().oracle_exchange_delta(int(E_i), int(E_j), int(kT_i), int(kT_j)))
+
+
+def exchange_accept(E_i: int, E_j: int, kT_i: int, kT_j: int, u: int) -> bool:
+    """Eq. 5 in integer form: accept iff Delta >= 0 or u < floor(exp(Delta) 2^32)."""
+    return bool(_load().oracle_exchange_accept(int(E_i), int(E_j), int(kT_i), int(kT_j), int(u)))
+
+
+def exchange_draw(seed: int, rnd: int, p: int) -> int:
+    return int(_load().oracle_exchange_draw(C.c_uint64(int(seed)), C.c_uint64(int(rnd)), int(p)))
+
+
+def replica_exchange(replicas: list, kT: list, tables: list, parity: int, seed: int, rnd: int,
+                     energy=lambda o: o.running_energy()) -> list:
+    """One round of replica exchange (S9; Eq. 5-6) over temperature slots.
+
+    ``replicas[p]`` is the Oracle running at slot p (temperature ``kT[p]``, threshold table
+    ``tables[p]``).  Slots p, p + 1 with p = parity, parity + 2, ... attempt an exchange; when it is
+    accepted the two configurations change slots (the list is permuted in place and each Oracle is
+    given the table of its new slot).  Returns the list of accept flags, one per slot pair (0 for the
+    pairs not attempted in this round).
+    """
+    n = len(replicas)
+    flags = [0] * max(0, n - 1)
+    for p in range(parity & 1, n - 1, 2):
+        u = exchange_draw(seed, rnd, p)
+        if exchange_accept(energy(replicas[p]), energy(replicas[p + 1]), kT[p], kT[p + 1], u):
+            replicas[p], replicas[p + 1] = replicas[p + 1], replicas[p]
+            replicas[p].set_temperature(tables[p])
+            replicas[p + 1].set_temperature(tables[p + 1])
+            flags[p] = 1
+    return flags
 
 
 class Oracle:

@@ -39,7 +39,7 @@
 namespace {
 
 enum { LAT_BCC = 0, LAT_FCC = 1 };
-enum { TAG_SHIFT = 1, TAG_TRIAL = 2, TAG_INIT = 3, TAG_SEQ = 5 };
+enum { TAG_SHIFT = 1, TAG_TRIAL = 2, TAG_INIT = 3, TAG_SEQ = 5, TAG_EXCHANGE = 6 };
 
 // ---------------------------------------------------------------------------------------
 // Philox4x32-10, Salmon, Moraes, Dror, Shaw, SC'11 (reading Q5 / S4).
@@ -420,6 +420,39 @@ extern "C" {
 
 void oracle_philox4x32_10(const uint32_t* ctr, const uint32_t* key, uint32_t* out) {
   philox4x32_10(ctr, key, out);
+}
+
+// ---------------------------------------------------------------------------------------
+// S9 replica exchange (parallel tempering), Eq. 5-6, PAPER.md:89-97:
+//   P_swap = min(1, exp(Delta)),  Delta = (1/kT_i - 1/kT_j)(E_i - E_j).
+// Energies are the integer H (0.1 meV), temperatures kT in the same units, so Delta is a pure
+// number.  Integer form of the decision, like Eq. 3: accept iff Delta >= 0 or u < T, with
+//   Delta = (double)(kT_j - kT_i) * (double)(E_i - E_j) / ((double)kT_i * (double)kT_j),
+//   T = min(floor(exp(Delta) * 2^32), 2^32 - 1), u a 32-bit Philox word.
+// ---------------------------------------------------------------------------------------
+double oracle_exchange_delta(int64_t E_i, int64_t E_j, int32_t kT_i, int32_t kT_j) {
+  const double a = (double)(kT_j - kT_i);
+  const double c = (double)(E_i - E_j);
+  const double b = (double)kT_i * (double)kT_j;
+  return a * c / b;
+}
+
+int oracle_exchange_accept(int64_t E_i, int64_t E_j, int32_t kT_i, int32_t kT_j, uint32_t u) {
+  const double delta = oracle_exchange_delta(E_i, E_j, kT_i, kT_j);
+  if (delta >= 0.0) return 1;
+  const double x = std::exp(delta) * 4294967296.0;
+  const uint32_t T = x >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)std::floor(x);
+  return u < T ? 1 : 0;
+}
+
+// The draw of the exchange attempt between temperature slots p and p + 1 in round r:
+// philox(ctr = (p, r_hi, r_lo, TAG_EXCHANGE), key = seed)[0].
+uint32_t oracle_exchange_draw(uint64_t seed, uint64_t round, uint32_t p) {
+  const uint32_t ctr[4] = {p, (uint32_t)(round >> 32), (uint32_t)(round & 0xffffffffull), (uint32_t)TAG_EXCHANGE};
+  const uint32_t key[2] = {(uint32_t)(seed & 0xffffffffull), (uint32_t)(seed >> 32)};
+  uint32_t out[4];
+  philox4x32_10(ctr, key, out);
+  return out[0];
 }
 
 // Writes up to max_out offsets (dx,dy,dz triples) of shell s; returns the shell size.

@@ -21,5 +21,6 @@ from .tables import (  # noqa: F401
     make_accept_table,
     accept_table_len,
     anneal_kT_units,
+    replica_ladder,
 )
 from .configs import Config, CONFIGS, get_config, scaled_config  # noqa: F401

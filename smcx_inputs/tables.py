@@ -66,3 +66,10 @@ def anneal_kT_units(t: int, n_sweeps: int = 2000, kT_hi: int = 1720, kT_lo: int 
     if n_sweeps <= 1:
         return kT_hi
     return kT_hi - ((kT_hi - kT_lo) * t) // (n_sweeps - 1)
+
+
+def replica_ladder(kT_lo: int, n_replicas: int, n_sites: int, coeff: float) -> list:
+    """Temperatures of a replica-exchange ladder spaced as Eq. 7 asks:
+    delta kT = coeff / sqrt(n_sites) (0.1 meV units, rounded to integers, at least 1 apart)."""
+    step = max(1, int(round(coeff / math.sqrt(float(n_sites)))))
+    return [int(kT_lo) + r * step for r in range(n_replicas)]
