@@ -152,6 +152,54 @@ int smcx_shell_offsets(smcx_t *h, int32_t shell, int32_t *xyz, int32_t max_offse
 int smcx_get_config(smcx_t *h, int32_t *storage, int32_t *kernel, int64_t *n_sites, int64_t *n_cells);
 int64_t smcx_kernel_launches(smcx_t *h); /* kernels launched by this handle so far */
 
+/* ---- Temperature parallelism on one GPU: replica ensemble and replica exchange -----------------
+ * "multiple replicas of the same system are simulated concurrently at different
+ * temperatures.  Configurations between replicas are periodically exchanged according to a
+ * Metropolis criterion", P_swap = min(1, exp(Delta)) (Eq. 5),
+ * Delta = (1/kT_i - 1/kT_j)(E_i - E_j) (Eq. 6); the ladder spacing follows Eq. 7 (PAPER.md:99-102,
+ * chosen by the caller).  Reading S9: in exchange round r the neighbouring slots
+ * (p, p+1), p = parity, parity+2, ..., attempt an exchange; Delta is evaluated in fp64 from the
+ * integer running energies and integer kT; accept iff Delta >= 0 or
+ * u < min(floor(exp(Delta) 2^32), 2^32-1), u = philox4x32_10(ctr = (p, r_hi, r_lo, 6), key =
+ * exchange_seed)[0].  An accepted exchange swaps the temperatures of the two replicas (each keeps
+ * its lattice, seed, sweep counter and trace and gets the threshold table of its new slot), which is
+ * the same Markov chain as swapping the configurations.  Decision and table switch run in kernels on
+ * the device: no call below synchronises with the host except smcx_ensemble_state.
+ *
+ * An ensemble owns n_replicas handles, one CUDA stream each (so small lattices run concurrently),
+ * all forked from / joined to the stream of `base` around every call: seen from that stream the
+ * calls execute in order.  Replica r is created like smcx_create(base) with seed seeds[r] and starts
+ * in slot r.  Every table is zero-padded to the longest one (T[d] = 0 for d >= len is the
+ * definition of the table, so no decision changes). */
+typedef struct smcx_ensemble smcx_ensemble_t;
+
+/* kT_units, accept, accept_len, seeds: host arrays of n_replicas entries (accept[p] is the host
+ * table of slot p, kT_units strictly positive).  base->accept / accept_len / seed / kT_units /
+ * d_workspace are ignored (the library allocates device memory).  2 <= n_replicas <= 1024. */
+int smcx_ensemble_create(smcx_ensemble_t **out, const smcx_params_t *base, int32_t n_replicas,
+                         const int32_t *kT_units, const uint32_t *const *accept, const int32_t *accept_len,
+                         const uint64_t *seeds, uint64_t exchange_seed);
+void smcx_ensemble_destroy(smcx_ensemble_t *e);
+/* Borrowed handle of replica r (valid until the ensemble is destroyed; do not smcx_destroy it, do
+ * not call smcx_set_temperature on it).  Reading calls (smcx_species, smcx_energy, smcx_sro,
+ * smcx_energy_trace, smcx_stats) are fine and synchronise that replica's stream only. */
+smcx_t *smcx_ensemble_replica(smcx_ensemble_t *e, int32_t r);
+/* n sweeps on every replica, each on its own stream.  Asynchronous. */
+int smcx_ensemble_sweep(smcx_ensemble_t *e, int64_t n);
+/* One exchange round with the given parity (0: pairs (0,1),(2,3),...; 1: (1,2),(3,4),...).
+ * Asynchronous: decision kernel + table switch on the device. */
+int smcx_ensemble_exchange(smcx_ensemble_t *e, int32_t parity);
+/* rounds x (sweeps_per_round sweeps on every replica, then one exchange round whose parity is the
+ * low bit of the ensemble's round counter).  Asynchronous. */
+int smcx_ensemble_run(smcx_ensemble_t *e, int64_t rounds, int64_t sweeps_per_round);
+/* Synchronises and reports (every pointer may be NULL): replica_at_slot[n], energy_at_slot[n]
+ * (running energy of the replica in that slot), attempted[n-1] / accepted[n-1] per slot pair,
+ * last_flags[n-1] (accept flags of the last round, 0 for pairs not attempted), rounds done. */
+int smcx_ensemble_state(smcx_ensemble_t *e, int32_t *replica_at_slot, int64_t *energy_at_slot,
+                        int64_t *attempted, int64_t *accepted, int32_t *last_flags, int64_t *rounds);
+int smcx_ensemble_synchronize(smcx_ensemble_t *e);
+int64_t smcx_ensemble_kernel_launches(smcx_ensemble_t *e); /* ensemble kernels + those of all replicas */
+
 const char *smcx_last_error(smcx_t *h); /* text of the last CUDA error seen by this handle */
 const char *smcx_strerror(int code);
 const char *smcx_version(void);

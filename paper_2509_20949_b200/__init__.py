@@ -9,5 +9,5 @@ from .binding import (  # noqa: F401
     BCC, FCC,
     STORAGE_AUTO, STORAGE_2BIT, STORAGE_U8,
     KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT,
-    SmcxError, Lattice, load_library, library_path, exported_symbols,
+    SmcxError, Lattice, Ensemble, load_library, library_path, exported_symbols,
 )

@@ -79,6 +79,16 @@ def load_library(build_if_missing: bool = True):
         "smcx_shell_offsets": (C.c_int, [vp, C.c_int32, i32p, C.c_int32, i32p]),
         "smcx_get_config": (C.c_int, [vp, i32p, i32p, i64p, i64p]),
         "smcx_kernel_launches": (C.c_int64, [vp]),
+        "smcx_ensemble_create": (C.c_int, [C.POINTER(vp), C.POINTER(_Params), C.c_int32, i32p,
+                                           C.POINTER(C.POINTER(C.c_uint32)), i32p, C.POINTER(C.c_uint64), C.c_uint64]),
+        "smcx_ensemble_destroy": (None, [vp]),
+        "smcx_ensemble_replica": (vp, [vp, C.c_int32]),
+        "smcx_ensemble_sweep": (C.c_int, [vp, C.c_int64]),
+        "smcx_ensemble_exchange": (C.c_int, [vp, C.c_int32]),
+        "smcx_ensemble_run": (C.c_int, [vp, C.c_int64, C.c_int64]),
+        "smcx_ensemble_state": (C.c_int, [vp, i32p, i64p, i64p, i64p, i32p, i64p]),
+        "smcx_ensemble_synchronize": (C.c_int, [vp]),
+        "smcx_ensemble_kernel_launches": (C.c_int64, [vp]),
         "smcx_last_error": (C.c_char_p, [vp]),
         "smcx_strerror": (C.c_char_p, [C.c_int]),
         "smcx_version": (C.c_char_p, []),
@@ -151,6 +161,23 @@ class Lattice:
         self.storage, self.kernel, self.n_sites, self.n_cells = st.value, kn.value, ns.value, nc.value
 
     @classmethod
+    def _borrowed(cls, handle, owner, lattice, dims, n_species, n_shells, device):
+        """Wrap a handle owned by an Ensemble (smcx_ensemble_replica): never destroyed from here."""
+        import torch
+        self = cls.__new__(cls)
+        self._lib = load_library()
+        self._h = C.c_void_p(handle)
+        self._owner, self._borrowed_handle = owner, True
+        self._workspace = None
+        self.device = torch.device("cuda", int(device))
+        self.lattice, self.dims = int(lattice), tuple(int(d) for d in dims)
+        self.n_species, self.n_shells = int(n_species), int(n_shells)
+        st, kn, ns, nc = C.c_int32(), C.c_int32(), C.c_int64(), C.c_int64()
+        self._check(self._lib.smcx_get_config(self._h, C.byref(st), C.byref(kn), C.byref(ns), C.byref(nc)), "smcx_get_config")
+        self.storage, self.kernel, self.n_sites, self.n_cells = st.value, kn.value, ns.value, nc.value
+        return self
+
+    @classmethod
     def from_config(cls, cfg, **over):
         kw = dict(lattice=cfg.lattice, dims=cfg.dims, n_species=cfg.n_species, n_shells=cfg.n_shells, epi=cfg.epi(),
                   accept=cfg.accept_table(0), seed=cfg.seed, link_cell=cfg.link_cell, kT_units=cfg.kT_at(0))
@@ -164,6 +191,9 @@ class Lattice:
             raise SmcxError(rc, what, detail)
 
     def close(self):
+        if getattr(self, "_borrowed_handle", False):
+            self._h = None
+            return
         if getattr(self, "_h", None):
             self._lib.smcx_destroy(self._h)
             self._h = None
@@ -252,6 +282,91 @@ class Lattice:
     @property
     def kernel_launches(self) -> int:
         return int(self._lib.smcx_kernel_launches(self._h))
+
+
+class Ensemble:
+    """One smcx_ensemble_t: replicas of one system on a temperature ladder with replica exchange on
+    the device (include/smcx.h, "Temperature parallelism on one GPU").  Methods mirror the C calls."""
+
+    def __init__(self, lattice, dims, n_species, n_shells, epi, kT_units, accept_tables, seeds, exchange_seed,
+                 link_cell=4, storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2509_20949_b200 needs a CUDA device; there is no CPU fallback")
+        self._lib = lib = load_library()
+        self._e = None
+        n = len(kT_units)
+        if not (len(accept_tables) == n and len(seeds) == n):
+            raise ValueError("kT_units, accept_tables and seeds must have one entry per replica")
+        tabs = [np.ascontiguousarray(t, dtype=np.uint32) for t in accept_tables]
+        p, keep = _make_params(lattice, dims, n_species, n_shells, epi, tabs[0], 0, link_cell, 0, storage, kernel,
+                               device, trace_capacity)
+        self.device = torch.device("cuda", int(device))
+        with torch.cuda.device(self.device):
+            self._stream = torch.cuda.current_stream(self.device)
+        p.stream = C.c_void_p(self._stream.cuda_stream)
+        kT = (C.c_int32 * n)(*[int(k) for k in kT_units])
+        ptrs = (C.POINTER(C.c_uint32) * n)(*[t.ctypes.data_as(C.POINTER(C.c_uint32)) for t in tabs])
+        lens = (C.c_int32 * n)(*[int(t.size) for t in tabs])
+        sd = (C.c_uint64 * n)(*[int(s) for s in seeds])
+        e = C.c_void_p()
+        rc = lib.smcx_ensemble_create(C.byref(e), C.byref(p), n, kT, ptrs, lens, sd, C.c_uint64(int(exchange_seed)))
+        if rc != 0:
+            raise SmcxError(rc, "smcx_ensemble_create")
+        self._e = e
+        del keep
+        self.n_replicas = n
+        self.kT_units = [int(k) for k in kT_units]
+        self.replicas = [Lattice._borrowed(lib.smcx_ensemble_replica(e, r), self, lattice, dims, n_species, n_shells,
+                                           device) for r in range(n)]
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise SmcxError(rc, what)
+
+    def close(self):
+        if getattr(self, "_e", None):
+            for r in self.replicas:
+                r.close()
+            self._lib.smcx_ensemble_destroy(self._e)
+            self._e = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def sweep(self, n=1):
+        self._check(self._lib.smcx_ensemble_sweep(self._e, int(n)), "smcx_ensemble_sweep")
+
+    def exchange(self, parity):
+        self._check(self._lib.smcx_ensemble_exchange(self._e, int(parity)), "smcx_ensemble_exchange")
+
+    def run(self, rounds, sweeps_per_round):
+        self._check(self._lib.smcx_ensemble_run(self._e, int(rounds), int(sweeps_per_round)), "smcx_ensemble_run")
+
+    def synchronize(self):
+        self._check(self._lib.smcx_ensemble_synchronize(self._e), "smcx_ensemble_synchronize")
+
+    def state(self) -> dict:
+        n = self.n_replicas
+        ras = np.zeros(n, dtype=np.int32)
+        en = np.zeros(n, dtype=np.int64)
+        att, acc = np.zeros(n - 1, dtype=np.int64), np.zeros(n - 1, dtype=np.int64)
+        flg = np.zeros(n - 1, dtype=np.int32)
+        rounds = C.c_int64()
+        i32p, i64p = C.POINTER(C.c_int32), C.POINTER(C.c_int64)
+        self._check(self._lib.smcx_ensemble_state(self._e, ras.ctypes.data_as(i32p), en.ctypes.data_as(i64p),
+                                                  att.ctypes.data_as(i64p), acc.ctypes.data_as(i64p),
+                                                  flg.ctypes.data_as(i32p), C.byref(rounds)), "smcx_ensemble_state")
+        return dict(replica_at_slot=ras, energy_at_slot=en, attempted=att, accepted=acc, last_flags=flg,
+                    rounds=rounds.value)
+
+    @property
+    def kernel_launches(self) -> int:
+        return int(self._lib.smcx_ensemble_kernel_launches(self._e))
 
 
 def workspace_bytes(**kw) -> int:

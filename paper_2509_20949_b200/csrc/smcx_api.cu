@@ -13,6 +13,7 @@
 #include <string>
 #include <vector>
 
+#include "ensemble_kernels.cuh"
 #include "lattice_kernels.cuh"
 #include "smcx_common.cuh"
 #include "sweep_thread.cuh"
@@ -778,3 +779,5 @@ int smcx_get_config(smcx_t* h, int32_t* storage, int32_t* kernel, int64_t* n_sit
 int64_t smcx_kernel_launches(smcx_t* h) { return h ? h->launches : 0; }
 
 }  // extern "C"
+
+#include "ensemble_api.inc"

@@ -1,0 +1,113 @@
+"""Replica ensemble + replica exchange on the GPU against the oracle (pytest -m gpu), through the C ABI:
+which replica sits in which temperature slot, the accept flags of every round, the running energies and
+the species arrays of every slot must be identical (S9; Eq. 5-6)."""
+import numpy as np
+import pytest
+
+import oracle
+import paper_2509_20949_b200 as smcx
+from smcx_inputs import make_accept_table, replica_ladder, scaled_config
+
+pytestmark = pytest.mark.gpu
+
+KERNELS = [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_THREAD_PER_CELL, smcx.KERNEL_THREAD_PERSISTENT]
+KERNEL_IDS = ["warp", "thread", "persistent"]
+
+
+def _ensemble(cfg, kTs, seeds, xseed, kernel):
+    tables = [make_accept_table(k) for k in kTs]
+    g = smcx.Ensemble(cfg.lattice, cfg.dims, cfg.n_species, cfg.n_shells, cfg.epi(), kTs, tables, seeds, xseed,
+                      link_cell=cfg.link_cell, kernel=kernel)
+    reps = [oracle.Oracle.from_config(cfg, seed=seeds[r], accept=tables[r]) for r in range(len(kTs))]
+    return g, reps, tables
+
+
+def _assert_slots_equal(g, o_at_slot, o_ids):
+    st = g.state()
+    assert st["replica_at_slot"].tolist() == o_ids
+    assert st["energy_at_slot"].tolist() == [o.running_energy() for o in o_at_slot]
+    for p, o in enumerate(o_at_slot):
+        r = int(st["replica_at_slot"][p])
+        assert (g.replicas[r].species() == o.species()).all(), f"slot {p}"
+        assert g.replicas[r].energy() == o.energy()
+        assert g.replicas[r].stats() == o.stats()
+    return st
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
+def test_exchange_rounds_match_the_oracle(kernel):
+    """Five replicas of the 16^3 BCC config on a ladder with a mixed accept/reject history: step by
+    step (sweeps, then one exchange round of alternating parity) against the oracle."""
+    cfg = scaled_config(1, (16, 16, 16))
+    kTs = replica_ladder(700, 5, cfg.n_sites, 30.0 * np.sqrt(cfg.n_sites))
+    assert kTs == [700, 730, 760, 790, 820]
+    seeds = [9100 + 17 * r for r in range(5)]
+    g, reps, tables = _ensemble(cfg, kTs, seeds, 4242, kernel)
+    for o in reps:
+        o.tag = reps.index(o)
+    n_acc = np.zeros(4, dtype=np.int64)
+    n_att = np.zeros(4, dtype=np.int64)
+    for rnd in range(12):
+        g.sweep(2)
+        for o in reps:
+            o.sweep(2)
+        g.exchange(rnd & 1)
+        flags = oracle.replica_exchange(reps, kTs, tables, rnd & 1, 4242, rnd)
+        n_acc += np.array(flags)
+        n_att[(rnd & 1)::2] += 1
+        st = g.state()
+        assert st["last_flags"].tolist() == flags, rnd
+        assert st["rounds"] == rnd + 1
+        assert st["replica_at_slot"].tolist() == [o.tag for o in reps]
+    st = _assert_slots_equal(g, reps, [o.tag for o in reps])
+    assert st["accepted"].tolist() == n_acc.tolist() and st["attempted"].tolist() == n_att.tolist()
+    assert 0 < n_acc.sum() < n_att.sum()            # both outcomes occurred
+    # after the exchanges every replica sweeps at the temperature of its new slot
+    g.sweep(3)
+    for o in reps:
+        o.sweep(3)
+    _assert_slots_equal(g, reps, [o.tag for o in reps])
+    for p, o in enumerate(reps):
+        r = o.tag
+        assert (g.replicas[r].energy_trace() == o.energy_trace()).all()
+    g.close()
+
+
+def test_run_is_the_same_as_step_by_step():
+    """smcx_ensemble_run(rounds, k) == rounds x (sweep(k); exchange(round parity)), enqueued without
+    any host synchronisation in between; also the anneal-length tables (different lengths per slot)."""
+    cfg = scaled_config(1, (16, 16, 24))
+    kTs = [430, 520, 610, 860]
+    seeds = [77, 78, 79, 80]
+    g, reps, tables = _ensemble(cfg, kTs, seeds, 5, smcx.KERNEL_AUTO)
+    assert len({t.size for t in tables}) == 4
+    for o in reps:
+        o.tag = reps.index(o)
+    g.run(9, 3)
+    for rnd in range(9):
+        for o in reps:
+            o.sweep(3)
+        oracle.replica_exchange(reps, kTs, tables, rnd & 1, 5, rnd)
+    st = _assert_slots_equal(g, reps, [o.tag for o in reps])
+    assert st["rounds"] == 9
+    g.close()
+
+
+def test_two_replicas_parity_one_is_a_no_op():
+    cfg = scaled_config(1, (16, 16, 16))
+    kTs = [600, 640]
+    g, reps, tables = _ensemble(cfg, kTs, [1, 2], 3, smcx.KERNEL_AUTO)
+    g.sweep(1)
+    g.exchange(1)                                   # no pair (1,2) with two replicas
+    st = g.state()
+    assert st["attempted"].tolist() == [0] and st["rounds"] == 1 and st["replica_at_slot"].tolist() == [0, 1]
+    g.close()
+
+
+def test_ensemble_argument_checks():
+    cfg = scaled_config(1, (16, 16, 16))
+    t = make_accept_table(600)
+    with pytest.raises(smcx.SmcxError):
+        smcx.Ensemble(cfg.lattice, cfg.dims, cfg.n_species, cfg.n_shells, cfg.epi(), [600], [t], [1], 1)
+    with pytest.raises(smcx.SmcxError):
+        smcx.Ensemble(cfg.lattice, cfg.dims, cfg.n_species, cfg.n_shells, cfg.epi(), [600, 0], [t, t], [1, 2], 1)

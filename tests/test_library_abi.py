@@ -78,6 +78,15 @@ def test_null_arguments_are_rejected_not_dereferenced():
     assert lib.smcx_sweep(None, 1) == E["NULL_ARG"]
     assert lib.smcx_energy(None, None) == E["NULL_ARG"]
     lib.smcx_destroy(None)
+    # replica ensemble
+    assert lib.smcx_ensemble_create(None, None, 2, None, None, None, None, 0) == E["NULL_ARG"]
+    assert lib.smcx_ensemble_sweep(None, 1) == E["NULL_ARG"]
+    assert lib.smcx_ensemble_exchange(None, 0) == E["NULL_ARG"]
+    assert lib.smcx_ensemble_run(None, 1, 1) == E["NULL_ARG"]
+    assert lib.smcx_ensemble_state(None, None, None, None, None, None, None) == E["NULL_ARG"]
+    assert lib.smcx_ensemble_replica(None, 0) is None
+    assert lib.smcx_ensemble_kernel_launches(None) == 0
+    lib.smcx_ensemble_destroy(None)
 
 
 def test_no_cpu_fallback_without_a_device():
