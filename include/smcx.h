@@ -59,7 +59,10 @@ enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
  * colour, the whole threshold table in shared memory.  While the current table is too long for that
  * (more than about 16,000 entries next to 20 warps, 32,000 next to 16) passes run the THREAD_PER_CELL
  * kernel instead.
- * AUTO picks THREAD_PERSISTENT when the parameters allow it.  Results never depend on it. */
+ * AUTO picks, when the parameters allow a thread kernel, THREAD_PERSISTENT for lattices that give every
+ * warp of every SM a batch of cells (>= 148*20*32 link cells per colour) and THREAD_PER_CELL below that
+ * (same speed there, and concurrent lattices of a replica ensemble overlap freely).  Results never
+ * depend on it. */
 enum { SMCX_KERNEL_AUTO = 0, SMCX_KERNEL_WARP_PER_CELL = 1, SMCX_KERNEL_THREAD_PER_CELL = 2,
        SMCX_KERNEL_THREAD_PERSISTENT = 3 };
 

@@ -39,8 +39,10 @@ struct EnsembleDev {
 
 // One block; thread k decides the pair (p, p + 1), p = parity + 2 k.  Pairs are disjoint, so the
 // decisions of a round are independent of each other.
+// parity < 0: the low bit of the round counter (smcx_ensemble_run; lets one captured graph serve every round).
 __global__ void replica_exchange_kernel(const EnsembleDev E, int parity, uint32_t key0, uint32_t key1) {
   const unsigned long long r = *E.round;
+  if (parity < 0) parity = (int)(r & 1ull);
   for (int p = threadIdx.x; p < E.n - 1; p += blockDim.x) E.last_flags[p] = 0;
   __syncthreads();
   for (int k = threadIdx.x; ; k += blockDim.x) {

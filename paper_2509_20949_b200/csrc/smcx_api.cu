@@ -9,6 +9,7 @@
 #include <cstdlib>
 #include <cstring>
 #include <limits>
+#include <map>
 #include <new>
 #include <string>
 #include <vector>
@@ -184,7 +185,13 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   int kernel = p->kernel, storage = p->storage;
   if (kernel == SMCX_KERNEL_AUTO) {
     if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_WARP_PER_CELL;
-    else kernel = fast_ok ? SMCX_KERNEL_THREAD_PERSISTENT : SMCX_KERNEL_WARP_PER_CELL;
+    else if (!fast_ok) kernel = SMCX_KERNEL_WARP_PER_CELL;
+    // The persistent kernel (one block of 20 warps and ~220 KB of shared memory per SM) pays off once
+    // every warp of every SM gets a batch of 32 cells.  Below that a colour pass is as long as one
+    // cell's chain of trials with either kernel, and concurrent launches of the persistent kernel
+    // (replica ensembles) cost ~20 us each where those of the block kernel overlap freely (measured:
+    // 32 replicas of BCC 64^3, 0.416 ms against 0.238 ms per sweep of all replicas).
+    else kernel = n_cells / 8 >= 148ll * kPersistMaxWarps * 32 ? SMCX_KERNEL_THREAD_PERSISTENT : SMCX_KERNEL_THREAD_PER_CELL;
   }
   if (kernel == SMCX_KERNEL_THREAD_PER_CELL || kernel == SMCX_KERNEL_THREAD_PERSISTENT) {
     if (!fast_ok) return SMCX_E_UNSUPPORTED;
@@ -484,6 +491,17 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     if (cudaEventCreateWithFlags(&h->staging_ev[s], cudaEventDisableTiming) != cudaSuccess) return fail(SMCX_E_CUDA);
   }
   if (configure_thread_per_cell() != 0) return fail(SMCX_E_CUDA);
+  // every kernel of a sweep prefers the largest shared-memory carve-out: an SM whose carve-out must
+  // change drains first, which serialises lattices that run concurrently (replica ensembles:
+  // measured 45 us instead of 28 us per colour pass when the one-thread epilogue asked for the default)
+  cudaFuncSetAttribute(sweep_epilogue, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(replica_exchange_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(replica_apply_tables_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(sweep_thread_per_cell<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(sweep_thread_per_cell<false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(sweep_warp_per_cell<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(sweep_warp_per_cell<4>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaGetLastError();
   if (cudaStreamCreateWithFlags(&h->capture_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); h->capture_stream = nullptr; }
   {
     const Geom& G = h->plan.G;
