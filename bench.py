@@ -213,6 +213,51 @@ def replica_seed(base_seed: int, rank: int) -> int:
 # --------------------------------------------------------------------------------------------
 # the CUDA arm
 # --------------------------------------------------------------------------------------------
+def run_ensemble(n_replicas: int, rounds: int = 20, sweeps_per_round: int = 10):
+    """Temperature parallelism on one GPU: n_replicas of BASELINE.json config 2's lattice
+    (BCC 64^3) on a ladder spaced as Eq. 7, rounds x (sweeps, replica-exchange round), device-timed."""
+    import numpy as np
+    import torch
+    import paper_2509_20949_b200 as smcx
+    from smcx_inputs import get_config, make_accept_table, replica_ladder
+
+    cfg = get_config(2)
+    kTs = replica_ladder(600, n_replicas, cfg.n_sites, 2.0 * float(np.sqrt(cfg.n_sites)))
+    tabs = [make_accept_table(k) for k in kTs]
+    ens = smcx.Ensemble(cfg.lattice, cfg.dims, cfg.n_species, cfg.n_shells, cfg.epi(), kTs, tabs,
+                        [cfg.seed + 7919 * r for r in range(n_replicas)], cfg.seed)
+    ens.run(rounds, sweeps_per_round)          # warm-up: captures the round graph
+    ens.synchronize()
+    l0 = ens.kernel_launches
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    ens.run(rounds, sweeps_per_round)
+    b.record()
+    ens.synchronize()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b)
+    st = ens.state()
+    single = smcx.Lattice.from_config(cfg)
+    single.sweep(rounds * sweeps_per_round)
+    single.synchronize()
+    a.record()
+    single.sweep(rounds * sweeps_per_round)
+    b.record()
+    single.synchronize()
+    torch.cuda.synchronize()
+    ms1 = a.elapsed_time(b)
+    n_sw = rounds * sweeps_per_round
+    out = {"workload": f"{n_replicas} replicas of BCC 64^3 (524288 sites each), kT ladder {kTs[0]}..{kTs[-1]} (0.1 meV), "
+                       f"{rounds} rounds x ({sweeps_per_round} sweeps + 1 exchange round)",
+           "value": cfg.n_sites * n_replicas * n_sw / (ms * 1e-3), "unit": "trial swaps/s (all replicas)",
+           "one_lattice_alone": cfg.n_sites * n_sw / (ms1 * 1e-3), "ms_per_round": ms / rounds,
+           "exchange_accept_rate": float(st["accepted"].sum()) / max(1, int(st["attempted"].sum())),
+           "gpu_launches": int(ens.kernel_launches - l0)}
+    single.close()
+    ens.close()
+    return out
+
+
 def run_cuda(args, cfg, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -359,6 +404,9 @@ def run_cuda(args, cfg, rank, world, local_rank):
             v, desc = timer.sample.n_sites * n_or / dt, timer.describe(n_or)
             out["cpu_baseline"] = {"value": v, "unit": "trial swaps/s", "cores": 1, "kind": "oracle", "sample": desc,
                                    "host_cores_available": os.cpu_count()}
+        if args.ensemble > 1 and world == 1:
+            lat.close()
+            out["temperature_parallel"] = run_ensemble(args.ensemble)
         print(json.dumps(out))
     lat.close()
     if world > 1:
@@ -376,6 +424,8 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 warp-per-cell, 2 thread-per-cell, 3 thread-per-cell persistent")
     ap.add_argument("--storage", type=int, default=0, help="0 auto, 2 packed 2-bit, 8 uint8")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ensemble", type=int, default=128,
+                    help="also time a replica-exchange ensemble of this many BCC 64^3 replicas (0: skip)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     rank = int(os.environ.get("RANK", "0"))

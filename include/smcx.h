@@ -53,6 +53,9 @@ enum { SMCX_BCC = 0, SMCX_FCC = 1 };
 enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
 
 /* Which sweep kernel runs.  WARP_PER_CELL: any lattice/shell list, U8 storage.
+ * GROUP_PER_CELL: the same generality with 4, 8, 16 or 32 lanes per link cell (as few as still give
+ * every SM about eight warps; the environment variable SMCX_GROUP_LANES overrides the choice) and a
+ * per-pair difference table in shared memory; what AUTO picks whenever a thread kernel does not apply.
  * THREAD_PER_CELL: BCC, first two shells, link_cell = 4, n_species <= 4, 2BIT storage; one block per
  * 128 cells, two-level acceptance filter in shared memory.
  * THREAD_PERSISTENT: same restrictions; one block per SM whose warps walk over the cells of the
@@ -64,7 +67,7 @@ enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
  * (same speed there, and concurrent lattices of a replica ensemble overlap freely).  Results never
  * depend on it. */
 enum { SMCX_KERNEL_AUTO = 0, SMCX_KERNEL_WARP_PER_CELL = 1, SMCX_KERNEL_THREAD_PER_CELL = 2,
-       SMCX_KERNEL_THREAD_PERSISTENT = 3 };
+       SMCX_KERNEL_THREAD_PERSISTENT = 3, SMCX_KERNEL_GROUP_PER_CELL = 4 };
 
 enum {
   SMCX_OK = 0,

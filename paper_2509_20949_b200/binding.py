@@ -14,7 +14,7 @@ _lib = None
 
 BCC, FCC = 0, 1
 STORAGE_AUTO, STORAGE_2BIT, STORAGE_U8 = 0, 2, 8
-KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT = 0, 1, 2, 3
+KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT, KERNEL_GROUP_PER_CELL = 0, 1, 2, 3, 4
 
 
 class SmcxError(RuntimeError):

@@ -17,6 +17,7 @@
 #include "ensemble_kernels.cuh"
 #include "lattice_kernels.cuh"
 #include "smcx_common.cuh"
+#include "sweep_group.cuh"
 #include "sweep_thread.cuh"
 #include "sweep_warp.cuh"
 
@@ -85,6 +86,7 @@ struct Plan {
   long long n_cells;
   int storage;
   int kernel;
+  int group_lanes;  // lanes per cell of the sub-warp kernel
   int coef_class;   // build_thread_coefficients: 2 = the filter variant of the thread kernel applies
   bool coef_packed; // pack_thread_coefficients: the 16-bit coefficient rows are exact
   Layout lay;
@@ -184,8 +186,8 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   }
   int kernel = p->kernel, storage = p->storage;
   if (kernel == SMCX_KERNEL_AUTO) {
-    if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_WARP_PER_CELL;
-    else if (!fast_ok) kernel = SMCX_KERNEL_WARP_PER_CELL;
+    if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_GROUP_PER_CELL;
+    else if (!fast_ok) kernel = SMCX_KERNEL_GROUP_PER_CELL;
     // The persistent kernel (one block of 20 warps and ~220 KB of shared memory per SM) pays off once
     // every warp of every SM gets a batch of 32 cells.  Below that a colour pass is as long as one
     // cell's chain of trials with either kernel, and concurrent launches of the persistent kernel
@@ -197,7 +199,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     if (!fast_ok) return SMCX_E_UNSUPPORTED;
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_2BIT;
     if (storage != SMCX_STORAGE_2BIT) return SMCX_E_UNSUPPORTED;
-  } else if (kernel == SMCX_KERNEL_WARP_PER_CELL) {
+  } else if (kernel == SMCX_KERNEL_WARP_PER_CELL || kernel == SMCX_KERNEL_GROUP_PER_CELL) {
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_U8;
     if (storage != SMCX_STORAGE_U8) return SMCX_E_UNSUPPORTED;
   } else {
@@ -205,6 +207,19 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   }
   plan->kernel = kernel;
   plan->storage = storage;
+  // sub-warp kernel: the fewest lanes per cell that still give every SM about eight warps of cells,
+  // and whose block (8 warps of tiles + tables) fits the shared memory of an SM
+  plan->group_lanes = 32;
+  for (int lanes = 4; lanes <= 32; lanes *= 2) {
+    if (group_smem_layout(G, lanes).total > 227 * 1024) continue;
+    if ((long long)G.cells_per_colour * lanes / 32 >= 148ll * 8 || lanes == 32) { plan->group_lanes = lanes; break; }
+  }
+  if (const char* env = std::getenv("SMCX_GROUP_LANES")) {
+    const int v = std::atoi(env);
+    if ((v == 4 || v == 8 || v == 16 || v == 32) && group_smem_layout(G, v).total <= 227 * 1024) plan->group_lanes = v;
+  }
+  if (kernel == SMCX_KERNEL_GROUP_PER_CELL && group_smem_layout(G, plan->group_lanes).total > 227 * 1024)
+    return SMCX_E_LINK_CELL_TOO_SMALL;
 
   Layout& L = plan->lay;
   size_t off = 0;
@@ -222,6 +237,11 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
 }
 
 }  // namespace
+
+// kernels that read the two-level acceptance filter tables
+inline bool uses_filter(const Plan& P) {
+  return (is_thread_kernel(P.kernel) && P.coef_class == 2) || P.kernel == SMCX_KERNEL_GROUP_PER_CELL;
+}
 
 struct smcx {
   Plan plan;
@@ -350,10 +370,10 @@ int upload_table(smcx* h, const uint32_t* accept, int len) {
                                cudaMemcpyHostToDevice, h->stream));
   h->plan.G.filter_E = -1;
   h->plan.G.filter_nq = 0;
-  if (is_thread_kernel(h->plan.kernel)) {
+  if (uses_filter(h->plan)) {
     uint32_t* filt = h->staging[slot] + kAcceptCapacity;
     int nq = 0;
-    const int E = h->plan.coef_class == 2 ? build_accept_filter(accept, len, filt, &nq) : -1;
+    const int E = build_accept_filter(accept, len, filt, &nq);
     if (E >= 0) {
       SMCX_CUDA(h, cudaMemcpyAsync(h->d_filter(), filt, (size_t)kFilterWords * sizeof(uint32_t),
                                    cudaMemcpyHostToDevice, h->stream));
@@ -390,6 +410,11 @@ int launch_colour_pass(smcx* h, int colour) {
                                           h->d_filter(), h->d_state(), colour, h->stream);
     h->launches++;
     if (rc != 0) { h->err = "thread-per-cell launch failed"; return SMCX_E_CUDA; }
+    return SMCX_OK;
+  }
+  if (P.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
+    launch_group_per_cell(G, P.group_lanes, h->d_species(), h->d_epi(), h->d_accept(), h->d_filter(), h->d_state(), colour, h->stream);
+    h->launches++;
     return SMCX_OK;
   }
   const int n2 = G.n_species * G.n_species;
@@ -508,6 +533,10 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     const int n2 = G.n_species * G.n_species;
     const size_t sm = (size_t)((G.n_shells * n2 * 4 + G.B * G.ZT * 2 + G.ZT + 15) & ~15) +
                       (size_t)kWarpsPerBlock * ((G.TW * G.TW * G.TW * G.B + 15) & ~15);
+    if (h->plan.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
+      const cudaError_t e = configure_group_per_cell(G, h->plan.group_lanes);
+      if (e != cudaSuccess) { h->err = cudaGetErrorString(e); return fail(SMCX_E_CUDA); }
+    }
     if (h->plan.kernel == SMCX_KERNEL_WARP_PER_CELL) {
       if (sm > 227 * 1024) return fail(SMCX_E_LINK_CELL_TOO_SMALL);
       cudaError_t e = G.B == 2

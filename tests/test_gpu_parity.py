@@ -11,12 +11,13 @@ from smcx_inputs import get_config, make_accept_table, make_epi, scaled_config
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_THREAD_PER_CELL, smcx.KERNEL_THREAD_PERSISTENT]
-KERNEL_IDS = ["warp", "thread", "persistent"]
+KERNELS = [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_GROUP_PER_CELL, smcx.KERNEL_THREAD_PER_CELL,
+           smcx.KERNEL_THREAD_PERSISTENT]
+KERNEL_IDS = ["warp", "group", "thread", "persistent"]
 
 
 def _supported(cfg, kernel):
-    if kernel == smcx.KERNEL_WARP_PER_CELL:
+    if kernel in (smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_GROUP_PER_CELL):
         return True
     return cfg.lattice == 0 and cfg.n_shells == 2 and cfg.link_cell == 4 and cfg.n_species <= 4
 
@@ -94,9 +95,10 @@ def test_config2_anneal_full_length():
     assert (g.energy_trace() == o.energy_trace()).all()
 
 
-def test_config3_fcc_five_species_prefix():
+@pytest.mark.parametrize("kernel", [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_GROUP_PER_CELL], ids=["warp", "group"])
+def test_config3_fcc_five_species_prefix(kernel):
     cfg = get_config(3)
-    g, o = _pair(cfg)
+    g, o = _pair(cfg, kernel)
     _assert_same_state(g, o)
     g.sweep(2)
     o.sweep(2)
@@ -219,11 +221,19 @@ def test_thread_and_warp_kernels_agree():
     (1, (16, 8, 8), 5, 3, 4),      # FCC three shells
     (1, (16, 16, 16), 16, 2, 4),   # maximum species count
 ])
-def test_edge_geometries(lat, dims, n_sp, n_shells, w):
+@pytest.mark.parametrize("kernel,lanes", [(smcx.KERNEL_WARP_PER_CELL, 0), (smcx.KERNEL_GROUP_PER_CELL, 4),
+                                          (smcx.KERNEL_GROUP_PER_CELL, 8), (smcx.KERNEL_GROUP_PER_CELL, 16),
+                                          (smcx.KERNEL_GROUP_PER_CELL, 32), (smcx.KERNEL_AUTO, 0)],
+                         ids=["warp", "group4", "group8", "group16", "group32", "auto"])
+def test_edge_geometries(lat, dims, n_sp, n_shells, w, kernel, lanes, monkeypatch):
     amplitude, kT, seed = 350, 500, 4711
     epi = make_epi(n_shells, n_sp, amplitude, seed)
     table = make_accept_table(kT)
-    g = smcx.Lattice(lat, dims, n_sp, n_shells, epi, table, seed, link_cell=w, kT_units=kT)
+    if lanes:
+        monkeypatch.setenv("SMCX_GROUP_LANES", str(lanes))   # lanes per cell of the sub-warp kernel
+    else:
+        monkeypatch.delenv("SMCX_GROUP_LANES", raising=False)
+    g = smcx.Lattice(lat, dims, n_sp, n_shells, epi, table, seed, link_cell=w, kT_units=kT, kernel=kernel)
     o = oracle.Oracle(lat, dims, n_sp, n_shells, epi, w, table, seed)
     assert o.lc_valid()
     for s in range(n_shells):
