@@ -379,7 +379,7 @@ def run_cuda(args, cfg, rank, world, local_rank):
                 "workload": workload_string(cfg), "config_id": args.config,
                 "step": f"1 sweep = 8 colour-pass launches + trace; pair-count/SRO reduction every {sro_every} sweeps "
                         f"and once at the end ({n_sro} inside the timed region)",
-                "kernel": {1: "warp_per_cell/u8", 2: "thread_per_cell/2bit", 3: "thread_persistent/2bit"}[lat.kernel],
+                "kernel": {1: "warp_per_cell/u8", 2: "thread_per_cell/2bit", 3: "thread_persistent/2bit", 4: "group_per_cell/u8"}[lat.kernel],
                 "l2": "lattice (%.0f MB in device storage) larger than the 126 MB L2; no flush" %
                       (cfg.n_sites * (0.25 if lat.storage == 2 else 1.0) / 1e6),
                 "parallelism": "replicas only" if world > 1 else "single GPU",
@@ -388,7 +388,7 @@ def run_cuda(args, cfg, rank, world, local_rank):
             "sweep_ms": sweep_ms / args.steps, "sro_ms_each": sro_ms / max(1, n_sro),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                          "traffic": traffic, "peak_kind": peak_kind,
-                         "kernel": {1: "sweep_warp_per_cell", 2: "sweep_thread_per_cell", 3: "sweep_thread_persistent"}[lat.kernel],
+                         "kernel": {1: "sweep_warp_per_cell", 2: "sweep_thread_per_cell", 3: "sweep_thread_persistent", 4: "sweep_group_per_cell"}[lat.kernel],
                          "algorithmic_bytes_per_trial": ALGO_BYTES_PER_TRIAL, "launch_ms": launch_ms},
             "alu_view": alu_view(lat.kernel, value / world, clocks),
             "e2e": {"value": e2e_value, "unit": "trial swaps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
@@ -421,7 +421,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default: 4, the graded one)")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 warp-per-cell, 2 thread-per-cell, 3 thread-per-cell persistent")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 warp-per-cell, 2 thread-per-cell, 3 thread-per-cell persistent, 4 sub-warp group per cell")
     ap.add_argument("--storage", type=int, default=0, help="0 auto, 2 packed 2-bit, 8 uint8")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--ensemble", type=int, default=128,

@@ -207,12 +207,13 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   }
   plan->kernel = kernel;
   plan->storage = storage;
-  // sub-warp kernel: the fewest lanes per cell that still give every SM about eight warps of cells,
+  // sub-warp kernel: the fewest lanes per cell that still give every SM about sixteen warps of cells
+  // (with fewer cells a pass is as long as one cell's chain of trials, which more lanes shorten),
   // and whose block (8 warps of tiles + tables) fits the shared memory of an SM
   plan->group_lanes = 32;
   for (int lanes = 4; lanes <= 32; lanes *= 2) {
     if (group_smem_layout(G, lanes).total > 227 * 1024) continue;
-    if ((long long)G.cells_per_colour * lanes / 32 >= 148ll * 8 || lanes == 32) { plan->group_lanes = lanes; break; }
+    if ((long long)G.cells_per_colour * lanes / 32 >= 148ll * 16 || lanes == 32) { plan->group_lanes = lanes; break; }
   }
   if (const char* env = std::getenv("SMCX_GROUP_LANES")) {
     const int v = std::atoi(env);
