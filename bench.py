@@ -288,8 +288,11 @@ def run_cuda(args, cfg, rank, world, local_rank):
             lat.set_temperature(kT, tab)
         lat.sweep(1)
 
-    for t in range(args.warmup):
-        one_step(t)
+    if tables is None:
+        lat.sweep(args.warmup)        # same call as the timed region: the sweep graph is captured here, not there
+    else:
+        for t in range(args.warmup):
+            one_step(t)
     lat.sro()
     barrier()
 
