@@ -49,6 +49,7 @@ def _load():
         "oracle_n_sites": (C.c_int64, [C.c_void_p]),
         "oracle_init_species": (None, [C.c_void_p]),
         "oracle_init_permutation": (C.c_uint64, [C.c_void_p, C.c_uint64]),
+        "oracle_init_composition": (C.c_int, [C.c_void_p, C.POINTER(C.c_int64)]),
         "oracle_set_species": (C.c_int, [C.c_void_p, u8p]),
         "oracle_get_species": (None, [C.c_void_p, u8p]),
         "oracle_set_temperature": (None, [C.c_void_p, u32p, C.c_int]),
@@ -173,6 +174,13 @@ class Oracle:
 
     def init_species(self):
         self._lib.oracle_init_species(self._h)
+
+    def init_composition(self, counts):
+        """S10: exactly counts[p] sites of species p, placed by the permutation of S6."""
+        c = np.ascontiguousarray(counts, dtype=np.int64)
+        assert c.size == self.n_species
+        if self._lib.oracle_init_composition(self._h, _ptr(c, C.c_int64)) != 0:
+            raise ValueError("counts must be non-negative and sum to n_sites")
 
     def init_permutation(self, i: int) -> int:
         return int(self._lib.oracle_init_permutation(self._h, C.c_uint64(i)))

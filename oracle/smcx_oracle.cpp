@@ -376,6 +376,30 @@ void init_species(Oracle& o) {
   o.E_valid = false;
 }
 
+// S10: a given composition (the paper's alloy is Fe29Co29Ni28Al7Ti7, not
+// equiatomic): counts n_0..n_{n-1} with sum N; sigma_i = p for cum_p <= pi(i) < cum_{p+1}, cum_p =
+// n_0 + ... + n_{p-1}, pi the permutation of S6.  Exactly n_p sites of species p, placed uniformly
+// at random.  Returns false (state unchanged) if the counts do not sum to N or one is negative.
+bool init_composition(Oracle& o, const int64_t* counts) {
+  int64_t sum = 0;
+  for (int p = 0; p < o.n_species; ++p) {
+    if (counts[p] < 0) return false;
+    sum += counts[p];
+  }
+  if (sum != o.N) return false;
+  int h = 1;
+  while ((1ull << (2 * h)) < (uint64_t)o.N) ++h;
+  for (int64_t i = 0; i < o.N; ++i) {
+    const int64_t r = (int64_t)feistel_permute(o, (uint64_t)i, h);
+    int p = 0;
+    int64_t cum = counts[0];
+    while (r >= cum) cum += counts[++p];
+    o.sigma[i] = (uint8_t)p;
+  }
+  o.E_valid = false;
+  return true;
+}
+
 // S7: ordered pair counts N_s(p',p) = sum_i [sigma_i=p'] sum_{d in O_s} [sigma_{i+d}=p].
 void pair_counts(const Oracle& o, int64_t* counts) {
   const int n = o.n_species;
@@ -494,6 +518,8 @@ void oracle_destroy(void* h) { delete (Oracle*)h; }
 int64_t oracle_n_sites(void* h) { return ((Oracle*)h)->N; }
 
 void oracle_init_species(void* h) { init_species(*(Oracle*)h); }
+
+int oracle_init_composition(void* h, const int64_t* counts) { return init_composition(*(Oracle*)h, counts) ? 0 : -1; }
 
 // pi(i) itself, for the bijection pin.
 uint64_t oracle_init_permutation(void* h, uint64_t i) {

@@ -22,5 +22,7 @@ from .tables import (  # noqa: F401
     accept_table_len,
     anneal_kT_units,
     replica_ladder,
+    composition_counts,
+    cooling_stages,
 )
 from .configs import Config, CONFIGS, get_config, scaled_config  # noqa: F401

@@ -73,3 +73,25 @@ def replica_ladder(kT_lo: int, n_replicas: int, n_sites: int, coeff: float) -> l
     delta kT = coeff / sqrt(n_sites) (0.1 meV units, rounded to integers, at least 1 apart)."""
     step = max(1, int(round(coeff / math.sqrt(float(n_sites)))))
     return [int(kT_lo) + r * step for r in range(n_replicas)]
+
+
+def composition_counts(n_sites: int, parts) -> list:
+    """Integer species counts for a composition given in parts (e.g. (29, 29, 28, 7, 7) for the paper's
+    Fe29Co29Ni28Al7Ti7): floor(n_sites * part / sum), the remainder handed out one site at a
+    time to the species with the largest fractional part (ties: lower index first).  Sums to n_sites."""
+    total = int(sum(parts))
+    base = [int(n_sites) * int(p) // total for p in parts]
+    rem = [int(n_sites) * int(p) % total for p in parts]
+    left = int(n_sites) - sum(base)
+    for p in sorted(range(len(parts)), key=lambda q: (-rem[q], q))[:left]:
+        base[p] += 1
+    return base
+
+
+def cooling_stages(kT_hi: int, kT_lo: int, n_stages: int) -> list:
+    """Stage-wise cooling as the paper runs it ("decrease the temperature from 2000 K to 1000 K, with tens of
+    thousands of MC steps at each temperature"): n_stages equally spaced temperatures from
+    kT_hi down to kT_lo inclusive, in 0.1 meV units (integers)."""
+    if n_stages <= 1:
+        return [int(kT_hi)]
+    return [int(kT_hi) - ((int(kT_hi) - int(kT_lo)) * s) // (n_stages - 1) for s in range(n_stages)]

@@ -10,8 +10,9 @@ from smcx_inputs import make_accept_table, replica_ladder, scaled_config
 
 pytestmark = pytest.mark.gpu
 
-KERNELS = [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_THREAD_PER_CELL, smcx.KERNEL_THREAD_PERSISTENT]
-KERNEL_IDS = ["warp", "thread", "persistent"]
+KERNELS = [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_GROUP_PER_CELL, smcx.KERNEL_THREAD_PER_CELL,
+           smcx.KERNEL_THREAD_PERSISTENT]
+KERNEL_IDS = ["warp", "group", "thread", "persistent"]
 
 
 def _ensemble(cfg, kTs, seeds, xseed, kernel):
@@ -90,6 +91,29 @@ def test_run_is_the_same_as_step_by_step():
         oracle.replica_exchange(reps, kTs, tables, rnd & 1, 5, rnd)
     st = _assert_slots_equal(g, reps, [o.tag for o in reps])
     assert st["rounds"] == 9
+    g.close()
+
+
+def test_fcc_five_species_ensemble_with_the_sub_warp_kernel():
+    """FCC, 5 species, 3 shells (the shape of config 3, and of the paper's alloy): the ensemble runs the
+    sub-warp kernel; slots, energies and species against the oracle after graph-replayed rounds."""
+    from smcx_inputs import make_epi
+    lat, dims, n_sp, n_sh, w = 1, (16, 16, 8), 5, 3, 4
+    epi = make_epi(n_sh, n_sp, 400, 1003)
+    kTs = [650, 690, 730]
+    tables = [make_accept_table(k) for k in kTs]
+    seeds = [31, 32, 33]
+    g = smcx.Ensemble(lat, dims, n_sp, n_sh, epi, kTs, tables, seeds, 99, link_cell=w)
+    assert g.replicas[0].kernel == smcx.KERNEL_GROUP_PER_CELL
+    reps = [oracle.Oracle(lat, dims, n_sp, n_sh, epi, w, tables[r], seeds[r]) for r in range(3)]
+    for o in reps:
+        o.tag = reps.index(o)
+    g.run(6, 2)
+    for rnd in range(6):
+        for o in reps:
+            o.sweep(2)
+        oracle.replica_exchange(reps, kTs, tables, rnd & 1, 99, rnd)
+    _assert_slots_equal(g, reps, [o.tag for o in reps])
     g.close()
 
 
