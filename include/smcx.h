@@ -125,6 +125,13 @@ void smcx_destroy(smcx_t *h);
 int smcx_set_species(smcx_t *h, const uint8_t *host_src);
 int smcx_set_species_device(smcx_t *h, const void *d_src);
 
+/* Replace the lattice state by a seeded random solid solution of a given composition (reading S10;
+ * the paper's alloy is Fe29Co29Ni28Al7Ti7): counts[p] >= 0 sites of species p,
+ * p < n_species, summing to N; site i holds the species p with cum_p <= pi(i) < cum_{p+1}, pi the
+ * permutation of S6 keyed by the handle's seed.  Host array.  SMCX_E_BAD_STATE if the counts are negative
+ * or do not sum to N.  The running energy is recomputed; the sweep counter and trace are kept. */
+int smcx_init_composition(smcx_t *h, const int64_t *counts);
+
 /* New acceptance table (a new temperature) for the following sweeps.  Asynchronous with respect
  * to the host: the table is copied into library-owned pinned memory before the call returns. */
 int smcx_set_temperature(smcx_t *h, int32_t kT_units, const uint32_t *accept, int32_t accept_len);

@@ -67,6 +67,7 @@ def load_library(build_if_missing: bool = True):
         "smcx_set_species": (C.c_int, [vp, C.POINTER(C.c_uint8)]),
         "smcx_set_species_device": (C.c_int, [vp, vp]),
         "smcx_set_temperature": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_uint32), C.c_int32]),
+        "smcx_init_composition": (C.c_int, [vp, i64p]),
         "smcx_sweep": (C.c_int, [vp, C.c_int64]),
         "smcx_energy": (C.c_int, [vp, i64p]),
         "smcx_running_energy": (C.c_int, [vp, i64p]),
@@ -215,6 +216,12 @@ class Lattice:
     def set_species_device(self, tensor):
         assert tensor.is_cuda and tensor.dtype.itemsize == 1 and tensor.numel() == self.n_sites and tensor.is_contiguous()
         self._check(self._lib.smcx_set_species_device(self._h, C.c_void_p(tensor.data_ptr())), "smcx_set_species_device")
+
+    def init_composition(self, counts):
+        c = np.ascontiguousarray(counts, dtype=np.int64)
+        if c.size != self.n_species:
+            raise ValueError("counts must have n_species entries")
+        self._check(self._lib.smcx_init_composition(self._h, c.ctypes.data_as(C.POINTER(C.c_int64))), "smcx_init_composition")
 
     def set_temperature(self, kT_units, accept):
         a = np.ascontiguousarray(accept, dtype=np.uint32)

@@ -70,6 +70,42 @@ __global__ void init_species_kernel(void* __restrict__ species, long long n_site
   }
 }
 
+// S10: composition initial state.  cum[p] = n_0 + ... + n_p; site i holds the species whose range
+// contains pi(i).  One thread per 16 consecutive sites, like init_species_kernel.
+struct CompositionCum { long long cum[kMaxSpecies]; };
+
+template <class Store>
+__global__ void init_composition_kernel(void* __restrict__ species, long long n_sites, int n_species, int h,
+                                        uint32_t k0, uint32_t k1, const CompositionCum C) {
+  const long long n_groups = (n_sites + 15) >> 4;
+  for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
+       g += (long long)gridDim.x * blockDim.x) {
+    uint32_t packed = 0;
+    uint32_t bytes[4] = {0, 0, 0, 0};
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const long long i = g * 16 + k;
+      uint32_t s = 0;
+      if (i < n_sites) {
+        const long long r = (long long)feistel_permute((unsigned long long)i, h, (unsigned long long)n_sites, k0, k1);
+        for (int p = 0; p < n_species - 1; ++p) s += r >= C.cum[p] ? 1u : 0u;
+      }
+      packed |= s << (2 * k);
+      bytes[k >> 2] |= s << (8 * (k & 3));
+    }
+    if (Store::kBits == 2) {
+      reinterpret_cast<uint32_t*>(species)[g] = packed;
+    } else {
+      uint8_t* p = reinterpret_cast<uint8_t*>(species) + g * 16;
+      if (g * 16 + 16 <= n_sites) {
+        *reinterpret_cast<uint4*>(p) = make_uint4(bytes[0], bytes[1], bytes[2], bytes[3]);
+      } else {
+        for (int k = 0; k < 16 && g * 16 + k < n_sites; ++k) p[k] = (uint8_t)((bytes[k >> 2] >> (8 * (k & 3))) & 0xff);
+      }
+    }
+  }
+}
+
 // ---- storage conversion: uint8 site-id order <-> packed 2-bit ------------------------------
 __global__ void pack2_kernel(const uint8_t* __restrict__ src, uint32_t* __restrict__ dst, long long first_site,
                              long long n_sites_chunk) {

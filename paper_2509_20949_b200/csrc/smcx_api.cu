@@ -628,6 +628,29 @@ int smcx_set_species(smcx_t* h, const uint8_t* host_src) {
   return reset_running_energy(h);
 }
 
+int smcx_init_composition(smcx_t* h, const int64_t* counts) {
+  if (!h || !counts) return SMCX_E_NULL_ARG;
+  const Plan& P = h->plan;
+  CompositionCum C{};
+  long long sum = 0;
+  for (int p = 0; p < P.G.n_species; ++p) {
+    if (counts[p] < 0) return SMCX_E_BAD_STATE;
+    sum += counts[p];
+    C.cum[p] = sum;
+  }
+  if (sum != P.n_sites) return SMCX_E_BAD_STATE;
+  int hh = 1;
+  while ((1ull << (2 * hh)) < (unsigned long long)P.n_sites) ++hh;
+  const int grid = grid_for(h, (P.n_sites + 15) / 16, 256);
+  if (P.storage == SMCX_STORAGE_U8)
+    init_composition_kernel<StoreU8><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh, P.G.key0, P.G.key1, C);
+  else
+    init_composition_kernel<Store2><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh, P.G.key0, P.G.key1, C);
+  h->launches++;
+  SMCX_CUDA(h, cudaGetLastError());
+  return reset_running_energy(h);
+}
+
 int smcx_set_temperature(smcx_t* h, int32_t kT_units, const uint32_t* accept, int32_t accept_len) {
   if (!h) return SMCX_E_NULL_ARG;
   const int rc = upload_table(h, accept, accept_len);

@@ -344,3 +344,46 @@ def test_large_epi_values_thread_kernel():
         o.sweep(3)
         _assert_same_state(g, o)
         assert (g.energy_trace() == o.energy_trace()).all()
+
+
+def test_paper_alloy_composition_and_stagewise_cooling():
+    """S10 + the paper's protocol in small: FCC, five species in the proportions
+    29/29/28/7/7, three shells, cooled through temperature stages; initial state, every stage's species,
+    trace and SRO against the oracle."""
+    from smcx_inputs import composition_counts, cooling_stages
+    lat, dims, n_sp, n_sh, w, seed = 1, (16, 16, 16), 5, 3, 4, 2029
+    epi = make_epi(n_sh, n_sp, 400, seed)
+    stages = cooling_stages(1720, 860, 4)
+    tables = [make_accept_table(k) for k in stages]
+    g = smcx.Lattice(lat, dims, n_sp, n_sh, epi, tables[0], seed, link_cell=w, kT_units=stages[0])
+    o = oracle.Oracle(lat, dims, n_sp, n_sh, epi, w, tables[0], seed)
+    counts = composition_counts(g.n_sites, (29, 29, 28, 7, 7))
+    g.init_composition(counts)
+    o.init_composition(counts)
+    _assert_same_state(g, o)
+    assert np.bincount(g.species(), minlength=n_sp).tolist() == counts
+    assert g.energy() == o.energy() == g.running_energy()
+    for kT, tab in zip(stages, tables):
+        g.set_temperature(kT, tab)
+        o.set_temperature(tab)
+        g.sweep(3)
+        o.sweep(3)
+        _assert_same_state(g, o)
+        _assert_sro(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.stats() == o.stats()
+    with pytest.raises(smcx.SmcxError):
+        g.init_composition([1, 1, 1, 1, 1])
+
+
+def test_composition_on_packed_storage():
+    cfg = scaled_config(4, (32, 24, 16))
+    g, o = _pair(cfg, smcx.KERNEL_THREAD_PERSISTENT)
+    counts = [cfg.n_sites // 2, cfg.n_sites // 4, cfg.n_sites // 8, cfg.n_sites // 8]
+    g.init_composition(counts)
+    o.init_composition(counts)
+    _assert_same_state(g, o)
+    g.sweep(3)
+    o.sweep(3)
+    _assert_same_state(g, o)
+    assert g.energy() == o.energy() == g.running_energy()
