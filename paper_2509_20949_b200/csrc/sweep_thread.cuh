@@ -617,6 +617,45 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
 }
 
 
+// ---- Philox4x32-10 of a trial pair with the counter structure (cell_id, q, t, tag) factored -------------
+// Rounds 1-3 contain six 32 x 32 -> 64 products; with ctr = (cell, q, sweep, tag) five of them do not depend
+// on (cell, q) jointly: M1*t is uniform, M0*cell, B = M1*c2' and C = M0*c0'' depend on the cell only (once per
+// cell), A_q = M0*(hi(M1*t) ^ q ^ k0) on q only (once per block, table in shared memory).  Per call that leaves
+// one product and three XORs for rounds 1-3 instead of six and six.  Same function, same bits.
+#ifndef SMCX_OPT_PHILOX_FACTORED
+#define SMCX_OPT_PHILOX_FACTORED 1
+#endif
+struct PhiloxCell { uint32_t l0, lB, hCk, lC; };   // per-cell constants (hCk = hi(C) ^ rk1[2])
+
+__device__ __forceinline__ void mulwide(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo) {
+  const uint64_t p = (uint64_t)a * b;
+  hi = (uint32_t)(p >> 32); lo = (uint32_t)p;
+}
+// Table entry q: (hi(A_q) ^ rk1[1], lo(A_q)); filled once per block for q < 64.
+__device__ __forceinline__ uint2 philox_slot_entry(uint32_t q, uint32_t t, const uint32_t* rk0, const uint32_t* rk1) {
+  uint32_t h1, l1, hA, lA;
+  mulwide(0xCD9E8D57u, t, h1, l1);
+  mulwide(0xD2511F53u, h1 ^ q ^ rk0[0], hA, lA);
+  return make_uint2(hA ^ rk1[1], lA);
+}
+__device__ __forceinline__ PhiloxCell philox_cell_setup(uint32_t cell_id, uint32_t t, uint32_t ctr3, const uint32_t* rk0,
+                                                        const uint32_t* rk1) {
+  uint32_t h0, l0, h1, l1, hB, lB, hC, lC;
+  mulwide(0xD2511F53u, cell_id, h0, l0);
+  mulwide(0xCD9E8D57u, t, h1, l1);
+  mulwide(0xCD9E8D57u, h0 ^ ctr3 ^ rk1[0], hB, lB);
+  mulwide(0xD2511F53u, hB ^ l1 ^ rk0[1], hC, lC);
+  return PhiloxCell{l0, lB, hC ^ rk1[2], lC};
+}
+__device__ __forceinline__ Philox4 philox_factored(const PhiloxCell& pc, uint2 slot, const uint32_t* rk0, const uint32_t* rk1) {
+  uint32_t hD, lD;
+  mulwide(0xCD9E8D57u, slot.x ^ pc.l0, hD, lD);                 // round 3: M1 * c2'' , c2'' = hi(A_q) ^ l0 ^ rk1[1]
+  uint32_t c0 = hD ^ pc.lB ^ rk0[2], c1 = lD, c2 = pc.hCk ^ slot.y, c3 = pc.lC;
+#pragma unroll
+  for (int r = 3; r < 10; ++r) philox_round(c0, c1, c2, c3, rk0[r], rk1[r]);
+  return Philox4{c0, c1, c2, c3};
+}
+
 // ---- persistent variant ---------------------------------------------------------------------------
 // One block of kPersistWarps warps per SM for the whole colour pass.  Every warp owns an 8 KB tile
 // area (32 cells, row r of lane l at word r * 32 + l) and walks over batches of 32 consecutive cells
@@ -627,7 +666,7 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
 constexpr int kPersistMaxWarps = 20;   // a multiple of the four sub-partitions: 18 or 21 warps load them unevenly (measured)
 constexpr int kPersistMinWarps = 16;
 constexpr int kPersistTileBytes = kThreadTileWords * 32 * 4;             // per warp
-constexpr int kPersistSmemMax = 232448 - 512;                           // 227 KB less the static part / reserve
+constexpr int kPersistSmemMax = 232448 - 1024;                          // 227 KB less the static part / reserve
 
 // warps per block for a table of len entries, or 0 if the table does not fit next to 16 warps
 inline int persist_warps_for(int accept_len) {
@@ -652,6 +691,9 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
   int4* s_coef1 = s_coef0 + 16 * 8;
   uint32_t* s_T = reinterpret_cast<uint32_t*>(s_coef1 + 16 * 8);
   __shared__ unsigned s_acc[kPersistMaxWarps];
+#if SMCX_OPT_PHILOX_FACTORED
+  __shared__ uint2 s_slot[64];                                  // Philox round-2 products that depend on the slot pair only
+#endif
   // PK: coef points at the packed rows [16] int4; else at the 32-bit rows [16][2] int4
   for (int k = threadIdx.x; k < 128; k += blockDim.x) {
     const int ent = k >> 3;
@@ -665,6 +707,9 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
   for (int k = threadIdx.x; k <= G.accept_len; k += blockDim.x) s_T[k] = k < G.accept_len ? accept[k] : 0u;
 
   const uint32_t t = (uint32_t)st->sweep;
+#if SMCX_OPT_PHILOX_FACTORED
+  if (threadIdx.x < 64) s_slot[threadIdx.x] = philox_slot_entry(threadIdx.x, t, G.rk0, G.rk1);
+#endif
   int ox, oy, oz;
   sweep_origin(G, t, ox, oy, oz);
   int esum = 0;                                                 // kDEScale * sum of accepted dE of this thread
@@ -718,6 +763,12 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
         }
       }
       const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
+#if SMCX_OPT_PHILOX_FACTORED
+      const PhiloxCell pc = philox_cell_setup(cell_id, t, ctr3, G.rk0, G.rk1);
+#define SMCX_PHILOX_PAIR(LX) philox_factored(pc, s_slot[q0 + LX], G.rk0, G.rk1)
+#else
+#define SMCX_PHILOX_PAIR(LX) philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1)
+#endif
 #pragma unroll 1
       for (int lzy = 0; lzy < 16; ++lzy) {
         uint32_t* p_row = tile + (((lzy >> 2) + 2) * 8 + (lzy & 3) + 2) * NT;
@@ -725,12 +776,13 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
         uint32_t ra = p_row[-NT], rb = p_row[-8 * NT];
 #define SMCX_TRIAL_PAIR(LX)                                                                                          \
         {                                                                                                            \
-          const Philox4 r = philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1);                              \
+          const Philox4 r = SMCX_PHILOX_PAIR(LX);                                                                    \
           trial_thread<0, LX + 2, kAcceptDirect, NT, PK>(G, p_row, env, r.x, r.y, ra, rb, esum, nacc);               \
           trial_thread<1, LX + 2, kAcceptDirect, NT, PK>(G, p_row, env, r.z, r.w, ra, rb, esum, nacc);               \
         }
         SMCX_TRIAL_PAIR(0) SMCX_TRIAL_PAIR(1) SMCX_TRIAL_PAIR(2) SMCX_TRIAL_PAIR(3)
 #undef SMCX_TRIAL_PAIR
+#undef SMCX_PHILOX_PAIR
       }
       switch (x0 & 7) {
         case 0: write_back_tile<0, NT>(G, tile, lattice, wlo, dwh, t0y, t0z, rw, zstride); break;
