@@ -29,7 +29,7 @@
 
 namespace smcxk {
 
-constexpr int kGroupWarpsPerBlock = 8;
+constexpr int kGroupWarpsPerBlock = 8;    // at most; group_warps_per_block() picks fewer when that lets more blocks share an SM
 // Tile layout in shared memory (bytes): position (pz, py, px) at pz * zpitch + py * ypitch + px with
 // ypitch = 2 TW rounded up to a multiple of 4 and zpitch = 2 TW * ypitch + kGroupZPad.  Without the pad a
 // step in z is a multiple of 32 words and neighbours that differ in z only share a bank.  The tiles of
@@ -48,7 +48,7 @@ struct GroupSmem {
 };
 
 // Difference table row of the ordered pair (a,b): [s * n + x] for the shells, then corr(a,b), then n zeros.
-inline GroupSmem group_smem_layout(const Geom& G, int lanes) {
+inline GroupSmem group_smem_layout(const Geom& G, int lanes, int warps = kGroupWarpsPerBlock) {
   GroupSmem L;
   const int n = G.n_species;
   int stride = G.n_shells * n + 1 + n;
@@ -57,7 +57,7 @@ inline GroupSmem group_smem_layout(const Geom& G, int lanes) {
   L.d_bytes = (n * n * stride * 4 + 15) & ~15;
   L.nb_bytes = (G.ZT * 4 + 15) & ~15;     // per neighbour: (step & 0xffff) | row << 16
   L.tile_bytes = ((2 * G.TW * group_zpitch(G.TW) + 127) & ~127) + kGroupSkew;
-  const int cells_per_block = kGroupWarpsPerBlock * (32 / lanes);
+  const int cells_per_block = warps * (32 / lanes);
   L.filt_bytes = kFilterWords * 4;
   L.total = (L.d_bytes + L.nb_bytes + L.filt_bytes + cells_per_block * L.tile_bytes + 15) & ~15;
   return L;
@@ -122,7 +122,8 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   const uint32_t t = (uint32_t)st->sweep;
   int ox, oy, oz;
   sweep_origin(G, t, ox, oy, oz);
-  const uint32_t m = (blockIdx.x * kGroupWarpsPerBlock + warp) * CPW + grp;
+  const int n_warps = blockDim.x >> 5;
+  const uint32_t m = (blockIdx.x * n_warps + warp) * CPW + grp;
   const bool active = m < G.cells_per_colour;
   long long sum_dE = 0;
   unsigned n_acc = 0;
@@ -273,7 +274,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   __syncthreads();
   if (threadIdx.x == 0) {
     long long e = 0; unsigned a = 0;
-    for (int i = 0; i < kGroupWarpsPerBlock; ++i) { e += s_dE[i]; a += s_acc[i]; }
+    for (int i = 0; i < n_warps; ++i) { e += s_dE[i]; a += s_acc[i]; }
     if (a) {
       atomicAdd(reinterpret_cast<unsigned long long*>(&st->e_run), (unsigned long long)e);
       atomicAdd(&st->accepted, (unsigned long long)a);
@@ -307,8 +308,20 @@ inline int group_nit(const Geom& G, int lanes) {
 #define SMCX_GROUP_DISPATCH(Bv, lanes, nit, ...)              \
   if ((Bv) == 2) { SMCX_GROUP_DISPATCH_L(2, lanes, nit, __VA_ARGS__) } else { SMCX_GROUP_DISPATCH_L(4, lanes, nit, __VA_ARGS__) }
 
+// Warps per block: 8, or 4 / 2 when a block of 8 warps of tiles would leave an SM with fewer than three
+// blocks (large tiles with few lanes per cell); SMCX_GROUP_WARPS overrides it for experiments.
+inline int group_warps_per_block(const Geom& G, int lanes) {
+  int warps = kGroupWarpsPerBlock;
+  while (warps > 2 && 3 * group_smem_layout(G, lanes, warps).total > 227 * 1024) warps >>= 1;
+  if (const char* env = std::getenv("SMCX_GROUP_WARPS")) {
+    const int v = std::atoi(env);
+    if ((v == 1 || v == 2 || v == 4 || v == 8) && group_smem_layout(G, lanes, v).total <= 227 * 1024) warps = v;
+  }
+  return warps;
+}
+
 inline cudaError_t configure_group_per_cell(const Geom& G, int lanes) {
-  const int sm = group_smem_layout(G, lanes).total;
+  const int sm = group_smem_layout(G, lanes, group_warps_per_block(G, lanes)).total;
   const int nit = group_nit(G, lanes);
   cudaError_t e = cudaSuccess;
   SMCX_GROUP_DISPATCH(G.B, lanes, nit, {
@@ -322,10 +335,11 @@ inline cudaError_t configure_group_per_cell(const Geom& G, int lanes) {
 
 inline void launch_group_per_cell(const Geom& G, int lanes, uint8_t* species, const int32_t* epi, const uint32_t* accept,
                                   const uint32_t* filt, DevState* st, int colour, cudaStream_t stream) {
-  const GroupSmem S = group_smem_layout(G, lanes);
-  const unsigned cpb = kGroupWarpsPerBlock * (32 / lanes);
+  const int warps = group_warps_per_block(G, lanes);
+  const GroupSmem S = group_smem_layout(G, lanes, warps);
+  const unsigned cpb = warps * (32 / lanes);
   const unsigned grid = (G.cells_per_colour + cpb - 1) / cpb;
-  const int nt = kGroupWarpsPerBlock * 32;
+  const int nt = warps * 32;
   const int nit = group_nit(G, lanes);
   SMCX_GROUP_DISPATCH(G.B, lanes, nit, {
     sweep_group_per_cell<B_, L_, N_><<<grid, nt, S.total, stream>>>(G, species, epi, accept, filt, st, colour, S.d_stride,
