@@ -132,6 +132,13 @@ int smcx_set_species_device(smcx_t *h, const void *d_src);
  * or do not sum to N.  The running energy is recomputed; the sweep counter and trace are kept. */
 int smcx_init_composition(smcx_t *h, const int64_t *counts);
 
+/* Resume from a checkpoint.  The state of a run is (species array, sweep counter, seed, threshold
+ * table); the random numbers depend on counters only (reading S4), so a handle created with the same
+ * parameters, given the saved species (smcx_set_species) and the saved counter, continues the run bit for
+ * bit (3-million-step runs as in PAPER.md:165 need this).  The next sweep is sweep t, 0 <= t < 2^32; the
+ * energy trace restarts at t.  Synchronises. */
+int smcx_set_sweep_counter(smcx_t *h, int64_t t);
+
 /* New acceptance table (a new temperature) for the following sweeps.  Asynchronous with respect
  * to the host: the table is copied into library-owned pinned memory before the call returns. */
 int smcx_set_temperature(smcx_t *h, int32_t kT_units, const uint32_t *accept, int32_t accept_len);

@@ -63,6 +63,7 @@ def _load():
         "oracle_shift": (None, [C.c_void_p, C.c_uint32, i32p]),
         "oracle_stats": (None, [C.c_void_p, i64p, i64p, i64p]),
         "oracle_trace": (C.c_int64, [C.c_void_p, C.c_int64, C.c_int64, i64p]),
+        "oracle_set_sweep_counter": (C.c_int, [C.c_void_p, C.c_int64]),
         "oracle_count_visits": (None, [C.c_void_p, C.c_int]),
         "oracle_get_visits": (None, [C.c_void_p, u32p]),
         "oracle_pair_counts": (None, [C.c_void_p, i64p]),
@@ -232,6 +233,11 @@ class Oracle:
         a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
         self._lib.oracle_stats(self._h, C.byref(a), C.byref(b), C.byref(c))
         return a.value, b.value, c.value
+
+    def set_sweep_counter(self, t: int):
+        """Resume from a checkpoint: the next sweep is sweep t; the trace restarts there."""
+        if self._lib.oracle_set_sweep_counter(self._h, int(t)) != 0:
+            raise ValueError("sweep counter out of range")
 
     def energy_trace(self, first: int = 0, count: int | None = None) -> np.ndarray:
         if count is None:

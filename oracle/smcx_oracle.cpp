@@ -88,7 +88,8 @@ struct Oracle {
   int64_t accepted = 0;
   int64_t E_run = 0;
   bool E_valid = false;
-  std::vector<int64_t> trace;           // E_run after each sweep
+  std::vector<int64_t> trace;           // E_run after each sweep, from sweep trace_first on
+  int64_t trace_first = 0;              // resume (checkpointing): the sweep counter was set to this value
 };
 
 // S0: basis positions in half-lattice units.
@@ -615,10 +616,22 @@ void oracle_stats(void* h, int64_t* sweeps, int64_t* trials, int64_t* accepted) 
   *sweeps = o.sweeps_done; *trials = o.trials; *accepted = o.accepted;
 }
 
+// Resume from a checkpoint (state = species array, sweep counter, seed; the RNG is counter-based, so the
+// continuation is exact): the next sweep is sweep t.  The trace restarts there.
+int oracle_set_sweep_counter(void* h, int64_t t) {
+  Oracle& o = *(Oracle*)h;
+  if (t < 0 || t > 0xffffffffll) return -1;
+  o.sweeps_done = t;
+  o.trials = t * o.N;
+  o.trace.clear();
+  o.trace_first = t;
+  return 0;
+}
+
 int64_t oracle_trace(void* h, int64_t first, int64_t count, int64_t* dst) {
   Oracle& o = *(Oracle*)h;
-  if (first < 0 || first + count > (int64_t)o.trace.size()) return -1;
-  for (int64_t k = 0; k < count; ++k) dst[k] = o.trace[(size_t)(first + k)];
+  if (first < o.trace_first || first - o.trace_first + count > (int64_t)o.trace.size()) return -1;
+  for (int64_t k = 0; k < count; ++k) dst[k] = o.trace[(size_t)(first - o.trace_first + k)];
   return count;
 }
 

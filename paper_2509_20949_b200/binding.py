@@ -68,6 +68,7 @@ def load_library(build_if_missing: bool = True):
         "smcx_set_species_device": (C.c_int, [vp, vp]),
         "smcx_set_temperature": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_uint32), C.c_int32]),
         "smcx_init_composition": (C.c_int, [vp, i64p]),
+        "smcx_set_sweep_counter": (C.c_int, [vp, C.c_int64]),
         "smcx_sweep": (C.c_int, [vp, C.c_int64]),
         "smcx_energy": (C.c_int, [vp, i64p]),
         "smcx_running_energy": (C.c_int, [vp, i64p]),
@@ -222,6 +223,9 @@ class Lattice:
         if c.size != self.n_species:
             raise ValueError("counts must have n_species entries")
         self._check(self._lib.smcx_init_composition(self._h, c.ctypes.data_as(C.POINTER(C.c_int64))), "smcx_init_composition")
+
+    def set_sweep_counter(self, t):
+        self._check(self._lib.smcx_set_sweep_counter(self._h, int(t)), "smcx_set_sweep_counter")
 
     def set_temperature(self, kT_units, accept):
         a = np.ascontiguousarray(accept, dtype=np.uint32)

@@ -257,6 +257,7 @@ struct smcx {
   int staging_next = 0;
   uint8_t* bounce = nullptr;  // device, kChunkSites bytes, lazily allocated
   long long sweeps_enqueued = 0;
+  long long trace_first = 0;  // first sweep whose energy the trace holds (smcx_set_sweep_counter moves it)
   long long launches = 0;
   // one sweep (8 colour passes + epilogue) captured as a CUDA graph; re-captured when the kernel
   // parameters change (new threshold table)
@@ -650,6 +651,17 @@ int smcx_init_composition(smcx_t* h, const int64_t* counts) {
   return reset_running_energy(h);
 }
 
+int smcx_set_sweep_counter(smcx_t* h, int64_t t) {
+  if (!h) return SMCX_E_NULL_ARG;
+  if (t < 0 || t > 0xffffffffll) return SMCX_E_RANGE;
+  const unsigned long long v = (unsigned long long)t;
+  SMCX_CUDA(h, cudaMemcpyAsync(&h->d_state()->sweep, &v, sizeof(v), cudaMemcpyHostToDevice, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  h->sweeps_enqueued = t;
+  h->trace_first = t;
+  return SMCX_OK;
+}
+
 int smcx_set_temperature(smcx_t* h, int32_t kT_units, const uint32_t* accept, int32_t accept_len) {
   if (!h) return SMCX_E_NULL_ARG;
   const int rc = upload_table(h, accept, accept_len);
@@ -726,7 +738,7 @@ int smcx_running_energy(smcx_t* h, int64_t* E) {
 int smcx_energy_trace(smcx_t* h, int64_t first_sweep, int64_t count, int64_t* dst) {
   if (!h || (!dst && count > 0)) return SMCX_E_NULL_ARG;
   const long long cap = h->plan.G.trace_capacity;
-  if (first_sweep < 0 || count < 0 || first_sweep + count > h->sweeps_enqueued ||
+  if (first_sweep < h->trace_first || count < 0 || first_sweep + count > h->sweeps_enqueued ||
       h->sweeps_enqueued - first_sweep > cap)
     return SMCX_E_RANGE;
   SMCX_CUDA(h, cudaStreamSynchronize(h->stream));

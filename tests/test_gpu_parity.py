@@ -387,3 +387,29 @@ def test_composition_on_packed_storage():
     o.sweep(3)
     _assert_same_state(g, o)
     assert g.energy() == o.energy() == g.running_energy()
+
+
+@pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
+def test_checkpoint_and_resume_in_a_new_handle(kernel):
+    """State = (species, sweep counter, seed): a new handle given both continues bit for bit, and agrees with
+    an oracle resumed the same way."""
+    cfg = scaled_config(1, (16, 16, 24))
+    a = smcx.Lattice.from_config(cfg, kernel=kernel)
+    a.sweep(4)
+    saved, t = a.species().copy(), a.stats()[0]
+    a.sweep(5)
+    b = smcx.Lattice.from_config(cfg, kernel=kernel)
+    b.set_species(saved)
+    b.set_sweep_counter(t)
+    b.sweep(5)
+    assert (a.species() == b.species()).all()
+    assert (a.energy_trace(4, 5) == b.energy_trace(4, 5)).all()
+    assert a.stats()[:2] == b.stats()[:2] and a.energy() == b.energy() == b.running_energy()
+    with pytest.raises(smcx.SmcxError):
+        b.energy_trace(0, 1)
+    o = oracle.Oracle.from_config(cfg)
+    o.set_species(saved)
+    o.set_sweep_counter(t)
+    o.sweep(5)
+    _assert_same_state(b, o)
+    assert (b.energy_trace(4, 5) == o.energy_trace(4, 5)).all()

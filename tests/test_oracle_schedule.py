@@ -191,3 +191,26 @@ def test_s6_equiatomic_counts_config3_remainder():
     N = cfg.n_sites
     assert N % 5 == 3
     assert [N // 5 + (p < 3) for p in range(5)] == [1677722] * 3 + [1677721] * 2
+
+
+def test_resume_from_a_checkpoint_is_exact():
+    """Checkpoint = (species array, sweep counter, seed): a fresh oracle given both continues the run bit for
+    bit (the draws depend on the counters only), while a wrong counter gives a different trajectory."""
+    cfg = scaled_config(1, (16, 16, 16))
+    a = oracle.Oracle.from_config(cfg)
+    a.sweep(4)
+    saved, t = a.species().copy(), a.stats()[0]
+    a.sweep(3)
+    b = oracle.Oracle.from_config(cfg)
+    b.set_species(saved)
+    b.set_sweep_counter(t)
+    b.sweep(3)
+    assert (a.species() == b.species()).all()
+    assert (a.energy_trace(4, 3) == b.energy_trace(4, 3)).all() and b.stats()[:2] == a.stats()[:2]
+    with pytest.raises(IndexError):
+        b.energy_trace(0, 1)                      # the trace restarts at the resume point
+    c = oracle.Oracle.from_config(cfg)
+    c.set_species(saved)
+    c.set_sweep_counter(t + 1)
+    c.sweep(3)
+    assert (a.species() != c.species()).any()
