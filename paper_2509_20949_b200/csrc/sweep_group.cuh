@@ -70,6 +70,15 @@ __device__ __forceinline__ int group_basis_pos(int b, int a) {
   return a == 0 ? ((b >> 1) & 1) : a == 1 ? (b & 1) : ((b == 1 || b == 2) ? 1 : 0);
 }
 
+// idx = (tz * TW + ty) * TW + tx -> (tx, ty, tz) without integer division: (idx + 0.5) / TW is at least
+// 0.5 / TW away from an integer, far more than the rounding error of the float product for idx < 2^20.
+__device__ __forceinline__ void group_split_index(int idx, int TW, float inv_TW, int& tx, int& ty, int& tz) {
+  const int row = (int)(((float)idx + 0.5f) * inv_TW);
+  tx = idx - row * TW;
+  tz = (int)(((float)row + 0.5f) * inv_TW);
+  ty = row - tz * TW;
+}
+
 // NIT > 0: every lane visits exactly NIT neighbours per site, their steps and rows in registers (NIT >=
 // ceil(ZT / L); surplus visits read the zero entries of the row).  NIT == 0: any ZT, steps from shared memory.
 template <int B, int L, int NIT>
@@ -130,6 +139,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   int cx = 0, cy = 0, cz = 0, t0x = 0, t0y = 0, t0z = 0;
   const int TW = G.TW, H = G.H, w = G.w;
   const int n_conv = TW * TW * TW;
+  const float inv_TW = 1.0f / (float)TW;
   if (active) {
     colour_cell(G, m, colour, cx, cy, cz);
     t0x = (ox + cx * w - H + G.Lx) % G.Lx;
@@ -144,7 +154,8 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
 #pragma unroll
     for (int q = 0; q < 4; ++q) {
       const int idx = idx0 + q * L;
-      const int tx = idx % TW, ty = (idx / TW) % TW, tz = idx / (TW * TW);
+      int tx, ty, tz;
+      group_split_index(idx, TW, inv_TW, tx, ty, tz);
       v[q] = 0;
       at[q] = idx < n_conv ? 2 * tz * zpitch + 2 * ty * ypitch + 2 * tx : -1;
       if (active && idx < n_conv) {
@@ -250,7 +261,8 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     // a7: write back the sites a swap can have touched: positions within r0 of the cell
     const int lo = 2 * H - G.r0, hi = 2 * (H + w) - 1 + G.r0;  // tile positions, inclusive
     for (int idx = g; idx < n_conv; idx += L) {
-      const int tx = idx % TW, ty = (idx / TW) % TW, tz = idx / (TW * TW);
+      int tx, ty, tz;
+      group_split_index(idx, TW, inv_TW, tx, ty, tz);
       int gx = t0x + tx; if (gx >= G.Lx) gx -= G.Lx;
       int gy = t0y + ty; if (gy >= G.Ly) gy -= G.Ly;
       int gz = t0z + tz; if (gz >= G.Lz) gz -= G.Lz;
