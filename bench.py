@@ -342,7 +342,7 @@ def run_cuda(args, cfg, rank, world, local_rank):
     # table, sweep, read the sweep's energy back), download the lattice, SRO.
     host_species = torch.empty(cfg.n_sites, dtype=torch.uint8).pin_memory().numpy()
     lat.species(out=host_species)
-    e2e_steps = min(args.steps, 20)
+    e2e_steps = min(args.steps, 200)   # one job: the lattice goes up and comes back once, the steps in between
     table = cfg.accept_table(0)
     barrier()
     t0 = time.perf_counter()
