@@ -111,6 +111,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
 
   Geom& G = plan->G;
   std::memset(&G, 0, sizeof(G));
+  G.gzpad = 8; G.gskew = 64;   // defaults until group_tune_layout() has run
   G.lattice = p->lattice;
   G.B = p->lattice == SMCX_BCC ? 2 : 4;
   G.n_species = n;
@@ -207,17 +208,19 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   }
   plan->kernel = kernel;
   plan->storage = storage;
-  // sub-warp kernel: 16 lanes per cell when that gives every SM about sixteen warps of cells, else 32 (with
+  // sub-warp kernel: 16 lanes per cell when that gives every SM about twelve warps of cells, else 32 (with
   // fewer cells a pass is as long as one cell's chain of trials, which more lanes shorten).  Measured on FCC,
-  // 5 species, 3 shells: 128^3 1.02 / 1.04 ms per sweep with 16 / 32 lanes; 400^3 (2.56e8 sites) 31.8 / 20.4 /
-  // 23.2 ms with 8 / 16 / 32 lanes (8 lanes: one block of 139 KB per SM).  4 and 8 lanes stay selectable.
+  // 5 species, 3 shells: 128^3 (2,048 warps at 16 lanes) 0.92 / 1.00 ms per sweep with 16 / 32 lanes; 400^3
+  // (2.56e8 sites) 31.8 / 20.4 / 23.2 ms with 8 / 16 / 32 lanes (8 lanes: one block of 139 KB per SM).
+  // 4 and 8 lanes stay selectable.
   plan->group_lanes = 32;
-  if (group_smem_layout(G, 16, 2).total <= 227 * 1024 && (long long)G.cells_per_colour * 16 / 32 >= 148ll * 16)
+  if (group_smem_layout(G, 16, 2).total <= 227 * 1024 && (long long)G.cells_per_colour * 16 / 32 >= 148ll * 12)
     plan->group_lanes = 16;
   if (const char* env = std::getenv("SMCX_GROUP_LANES")) {
     const int v = std::atoi(env);
     if ((v == 4 || v == 8 || v == 16 || v == 32) && group_smem_layout(G, v, 2).total <= 227 * 1024) plan->group_lanes = v;
   }
+  group_tune_layout(G, plan->group_lanes);
   if (kernel == SMCX_KERNEL_GROUP_PER_CELL && group_smem_layout(G, plan->group_lanes, 2).total > 227 * 1024)
     return SMCX_E_LINK_CELL_TOO_SMALL;
 

@@ -12,6 +12,7 @@ enum : uint32_t { TAG_SHIFT = 1u, TAG_TRIAL = 2u, TAG_INIT = 3u };
 constexpr int kMaxShells = 5;
 constexpr int kMaxNeighbours = 80;  // FCC, 5 shells: 12+6+24+12+24 = 78
 constexpr int kMaxSpecies = 16;
+constexpr int kMaxGroupSlots = 128;  // neighbour slots of the sub-warp kernel: lanes * visits >= neighbours
 
 // Philox4x32-10 (Salmon et al., SC'11).  Round keys are recomputed from the key each call; the
 // additions fold into immediates when the key is a kernel parameter.
@@ -99,6 +100,11 @@ struct Geom {
   unsigned char half_idx[kMaxNeighbours / 2];  // indices (into off) of the positive half
   // tile-linear index delta of neighbour m for a site with basis index b, and its basis index
   short delta[4][kMaxNeighbours];
+  // sub-warp kernel (sweep_group.cuh), chosen on the host by a model of the shared-memory banks:
+  // gslot[slot] = neighbour visited by lane (slot % lanes) in its visit (slot / lanes), 255 = none;
+  // gzpad / gskew = padding of the tile's z pitch / extra distance between the tiles of a warp (bytes)
+  unsigned char gslot[kMaxGroupSlots];
+  short gzpad, gskew;
 };
 
 }  // namespace smcxk

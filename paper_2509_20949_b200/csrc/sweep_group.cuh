@@ -23,6 +23,8 @@
 //    sweep_thread.cuh; the exact table in global memory only when u falls within E of the bound).
 // Results are bit-identical to the other kernels (tests/test_gpu_parity.py).
 #pragma once
+#include <mutex>
+#include <vector>
 #include "smcx_common.cuh"
 #include "sweep_thread.cuh"   // two-level acceptance filter (kFilterTr, kFilterWords, build_accept_filter)
 #include "sweep_warp.cuh"
@@ -31,19 +33,131 @@ namespace smcxk {
 
 constexpr int kGroupWarpsPerBlock = 8;    // at most; group_warps_per_block() picks fewer when that lets more blocks share an SM
 // Tile layout in shared memory (bytes): position (pz, py, px) at pz * zpitch + py * ypitch + px with
-// ypitch = 2 TW rounded up to a multiple of 4 and zpitch = 2 TW * ypitch + kGroupZPad.  Without the pad a
-// step in z is a multiple of 32 words and neighbours that differ in z only share a bank.  The tiles of
-// the cells of a warp are kGroupSkew bytes further apart than a multiple of 128 bytes, so that the same
-// site of different cells lies in different banks (ncu, FCC 128^3 before either: 71 % of the
-// shared-memory wavefronts were bank conflicts).
-constexpr int kGroupZPad = 12;
-constexpr int kGroupSkew = 4;
-constexpr int kGroupMaxIt = 6;          // neighbour visits per lane and site held in registers
+// ypitch = 2 TW rounded up to a multiple of 4 and zpitch = 2 TW * ypitch + G.gzpad; the tiles of the cells
+// of a warp are G.gskew bytes further apart than a multiple of 128 bytes.  Pad, skew and the assignment of
+// neighbours to (lane, visit) slots (G.gslot) are chosen on the host by group_tune_layout() below from a
+// model of the 32 banks: ncu on FCC 128^3 showed 71 % of the shared-memory wavefronts to be bank conflicts
+// with an unpadded tile, 3.0 / 2.5 / 2.5 wavefronts per neighbour load with pad 12 / skew 4 and neighbours
+// dealt to the lanes in shell order; the tuned layout brings the model's figure from 8.0 to about 4.
 __host__ __device__ inline int group_ypitch(int TW) { return (2 * TW + 3) & ~3; }
-__host__ __device__ inline int group_zpitch(int TW) { return 2 * TW * group_ypitch(TW) + kGroupZPad; }
+__host__ __device__ inline int group_zpitch(int TW, int zpad) { return 2 * TW * group_ypitch(TW) + zpad; }
+inline int group_tile_bytes(int TW, int zpad, int skew) { return ((2 * TW * group_zpitch(TW, zpad) + 127) & ~127) + skew; }
+
+// Register-resident neighbour lists exist for 2, 3 and 6 visits per lane (FCC with three shells: 42
+// neighbours over 32 / 16 / 8 lanes; BCC with two shells: 14 over 8 / 16 / 32); anything else takes the
+// variant that reads the steps from shared memory.
+inline int group_nit(const Geom& G, int lanes) {
+  const int need = (G.ZT + lanes - 1) / lanes;
+  return need <= 2 ? 2 : need <= 3 ? 3 : need <= 6 ? 6 : 0;
+}
+inline int group_visits(const Geom& G, int lanes) {
+  const int nit = group_nit(G, lanes);
+  return nit > 0 ? nit : (G.ZT + lanes - 1) / lanes;
+}
+
+// Bank model: one neighbour load of a warp = for every cell of the warp (bank shift c * tile words) the
+// lanes' steps from a common site address A; wavefronts = the largest number of distinct words that fall
+// into one bank.  Summed over the visits and averaged over A mod 4 (all that matters of A).
+inline double group_bank_cost(const int* step, const unsigned char* slot, int lanes, int visits, int tile_words) {
+  const int cells = 32 / lanes;
+  int total = 0;
+  for (int a = 0; a < 4; ++a)
+    for (int v = 0; v < visits; ++v) {
+      int words[32], banks[32], nw = 0, worst = 0;
+      for (int c = 0; c < cells; ++c)
+        for (int l = 0; l < lanes; ++l) {
+          const int m = slot[v * lanes + l];
+          const int st = m == 255 ? 0 : step[m];
+          const int w = ((a + st + (1 << 20)) >> 2) + c * tile_words + c * (1 << 22);   // distinct words per cell
+          bool seen = false;
+          for (int k = 0; k < nw; ++k) seen = seen || words[k] == w;
+          if (!seen) { words[nw] = w; banks[nw] = (w - c * (1 << 22)) & 31; ++nw; }
+        }
+      for (int k = 0; k < nw; ++k) {
+        int cnt = 0;
+        for (int j = 0; j < nw; ++j) cnt += banks[j] == banks[k];
+        worst = cnt > worst ? cnt : worst;
+      }
+      total += worst;
+    }
+  return total / 4.0;
+}
+
+// Chooses G.gzpad, G.gskew and G.gslot for this lane count: every (pad, skew) with the neighbours in
+// shell order first, then a deterministic local search (swaps of two slots) on the best few.
+inline void group_tune_layout_search(Geom& G, int lanes) {
+  const int visits = group_visits(G, lanes), slots = visits * lanes, ZT = G.ZT;
+  unsigned char ident[kMaxGroupSlots];
+  for (int s = 0; s < kMaxGroupSlots; ++s) ident[s] = s < ZT ? (unsigned char)s : (unsigned char)255;
+  G.gzpad = 8; G.gskew = 64;
+  for (int s = 0; s < kMaxGroupSlots; ++s) G.gslot[s] = ident[s];
+  if (slots > kMaxGroupSlots || lanes > 32) return;
+  const int yp = group_ypitch(G.TW);
+  struct Cand { double cost; int pad, skew; } best[4] = {{1e30, 8, 64}, {1e30, 8, 64}, {1e30, 8, 64}, {1e30, 8, 64}};
+  int step[kMaxNeighbours];
+  // a layout must not cost a resident block: blocks per SM as with the smallest tile (tables ~ 8 KB)
+  const int cells_per_block = kGroupWarpsPerBlock * (32 / lanes);
+  const int blocks_min_tile = (227 * 1024) / (8192 + cells_per_block * group_tile_bytes(G.TW, 0, 4));
+  for (int pad = 0; pad < 32; pad += 4) {
+    const int zp = group_zpitch(G.TW, pad);
+    for (int m = 0; m < ZT; ++m) step[m] = G.off[m][2] * zp + G.off[m][1] * yp + G.off[m][0];
+    for (int skew = 4; skew < 128; skew += 4) {
+      if (blocks_min_tile > 0 &&
+          (227 * 1024) / (8192 + cells_per_block * group_tile_bytes(G.TW, pad, skew)) < blocks_min_tile) continue;
+      const double c = group_bank_cost(step, ident, lanes, visits, group_tile_bytes(G.TW, pad, skew) / 4);
+      for (int k = 0; k < 4; ++k)
+        if (c < best[k].cost) { for (int j = 3; j > k; --j) best[j] = best[j - 1]; best[k] = {c, pad, skew}; break; }
+      if (lanes == 32) break;   // one cell per warp: the skew does not matter
+    }
+  }
+  double best_cost = 1e30;
+  for (int k = 0; k < 4; ++k) {
+    const int pad = best[k].pad, skew = best[k].skew, zp = group_zpitch(G.TW, pad);
+    const int tw = group_tile_bytes(G.TW, pad, skew) / 4;
+    for (int m = 0; m < ZT; ++m) step[m] = G.off[m][2] * zp + G.off[m][1] * yp + G.off[m][0];
+    unsigned char slot[kMaxGroupSlots];
+    for (int s = 0; s < kMaxGroupSlots; ++s) slot[s] = ident[s];
+    double c = group_bank_cost(step, slot, lanes, visits, tw);
+    uint32_t rng = 12345u + (uint32_t)k;
+    for (int iter = 0; iter < 2500 && c > visits; ++iter) {
+      rng = rng * 1664525u + 1013904223u; const int s1 = (int)((rng >> 8) % (uint32_t)slots);
+      rng = rng * 1664525u + 1013904223u; const int s2 = (int)((rng >> 8) % (uint32_t)slots);
+      if (s1 / lanes == s2 / lanes || slot[s1] == slot[s2]) continue;
+      const unsigned char t1 = slot[s1]; slot[s1] = slot[s2]; slot[s2] = t1;
+      const double c2 = group_bank_cost(step, slot, lanes, visits, tw);
+      if (c2 <= c) c = c2; else { slot[s2] = slot[s1]; slot[s1] = t1; }
+    }
+    if (c < best_cost) {
+      best_cost = c; G.gzpad = (short)pad; G.gskew = (short)skew;
+      for (int s = 0; s < kMaxGroupSlots; ++s) G.gslot[s] = slot[s];
+    }
+  }
+}
+
+struct GroupTuneEntry { int lattice, n_shells, TW, lanes; short zpad, skew; unsigned char slot[kMaxGroupSlots]; };
+inline void group_tune_layout(Geom& G, int lanes) {
+  // the result depends on (lattice, shells, tile edge, lanes) only: computed once per process
+  static std::mutex mu;
+  static std::vector<GroupTuneEntry> cache;
+  {
+    std::lock_guard<std::mutex> lock(mu);
+    for (const GroupTuneEntry& e : cache)
+      if (e.lattice == G.lattice && e.n_shells == G.n_shells && e.TW == G.TW && e.lanes == lanes) {
+        G.gzpad = e.zpad; G.gskew = e.skew;
+        for (int s = 0; s < kMaxGroupSlots; ++s) G.gslot[s] = e.slot[s];
+        return;
+      }
+  }
+  group_tune_layout_search(G, lanes);
+  GroupTuneEntry e{G.lattice, G.n_shells, G.TW, lanes, G.gzpad, G.gskew, {}};
+  for (int s = 0; s < kMaxGroupSlots; ++s) e.slot[s] = G.gslot[s];
+  std::lock_guard<std::mutex> lock(mu);
+  cache.push_back(e);
+}
 
 struct GroupSmem {
   int d_stride;        // ints per ordered pair in the difference table (odd: spreads the pairs over the banks)
+  int d_copies;        // copies of the difference table (one per cell of a warp when rows fit 32 words)
   int d_bytes, nb_bytes, filt_bytes, tile_bytes, total;
 };
 
@@ -53,10 +167,12 @@ inline GroupSmem group_smem_layout(const Geom& G, int lanes, int warps = kGroupW
   const int n = G.n_species;
   int stride = G.n_shells * n + 1 + n;
   if ((stride & 1) == 0) ++stride;
+  L.d_copies = 1;   // per-cell copies with rows 32 words apart were measured: FCC 128^3 0.912 -> 0.892 ms per sweep, but the
+                    // 4 KB more per block cost FCC 400^3 a resident block (18.3 -> 19.6 ms): not used
   L.d_stride = stride;
-  L.d_bytes = (n * n * stride * 4 + 15) & ~15;
+  L.d_bytes = ((n * n * stride * L.d_copies + 32) * 4 + 15) & ~15;
   L.nb_bytes = (G.ZT * 4 + 15) & ~15;     // per neighbour: (step & 0xffff) | row << 16
-  L.tile_bytes = ((2 * G.TW * group_zpitch(G.TW) + 127) & ~127) + kGroupSkew;
+  L.tile_bytes = group_tile_bytes(G.TW, G.gzpad, G.gskew);
   const int cells_per_block = warps * (32 / lanes);
   L.filt_bytes = kFilterWords * 4;
   L.total = (L.d_bytes + L.nb_bytes + L.filt_bytes + cells_per_block * L.tile_bytes + 15) & ~15;
@@ -99,7 +215,11 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
 
   const int n = G.n_species, ZT = G.ZT;
   const int corr_at = G.n_shells * n, zero_at = corr_at + 1;
-  for (int k = threadIdx.x; k < n * n * d_stride; k += blockDim.x) {
+  // d_stride == 32 with fewer than 32 lanes: CPW copies, copy c at word c * (n n 32 + L)
+  const int d_copy_words = n * n * d_stride + L;
+  const int d_copies = (L < 32 && d_stride == 32) ? CPW : 1;
+  for (int k0 = threadIdx.x; k0 < n * n * d_stride * d_copies; k0 += blockDim.x) {
+    const int copy = k0 / (n * n * d_stride), k = k0 - copy * (n * n * d_stride);
     const int pair = k / d_stride, e = k % d_stride;
     const int a = pair / n, b = pair % n;
     int v = 0;
@@ -109,11 +229,12 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     } else if (e == corr_at) {
       v = 2 * epi[a * n + b] - epi[a * n + a] - epi[b * n + b];
     }
-    s_D[k] = v;
+    s_D[copy * d_copy_words + k] = v;
   }
+  const int32_t* s_Dg = s_D + (d_copies > 1 ? grp * d_copy_words : 0);   // this cell's copy
   if (G.filter_E >= 0)
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
-  const int ypitch = group_ypitch(G.TW), zpitch = group_zpitch(G.TW);
+  const int ypitch = group_ypitch(G.TW), zpitch = group_zpitch(G.TW, G.gzpad);
   for (int k = threadIdx.x; k < ZT; k += blockDim.x) {
     const int step = G.off[k][2] * zpitch + G.off[k][1] * ypitch + G.off[k][0];
     s_nb[k] = ((uint32_t)(uint16_t)(short)step) | ((uint32_t)(G.shell_of[k] * n) << 16);
@@ -122,8 +243,8 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   int nstep[NIT > 0 ? NIT : 1], nrow[NIT > 0 ? NIT : 1];
 #pragma unroll
   for (int it = 0; it < NIT; ++it) {
-    const int mm = g + it * L;
-    const bool valid = mm < ZT;
+    const int mm = G.gslot[g + it * L];
+    const bool valid = mm != 255;
     nstep[it] = valid ? G.off[mm][2] * zpitch + G.off[mm][1] * ypitch + G.off[mm][0] : 0;
     nrow[it] = valid ? G.shell_of[mm] * n : zero_at;
   }
@@ -208,7 +329,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
             const int sa = *p_i, sb = *p_j;
             // a5: partial sums over this lane's neighbours of i (a -> b) and of j (b -> a); a trial between
             // equal species runs through the same code (its row of D is all zeros) and is masked below
-            const int32_t* Drow = s_D + (sa * n + sb) * d_stride;
+            const int32_t* Drow = s_Dg + (sa * n + sb) * d_stride;
             int part = 0;
             if (NIT > 0) {
 #pragma unroll
@@ -217,8 +338,8 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
             } else {
 #pragma unroll 2
               for (int it = 0; it < nit; ++it) {
-                const int mm = g + it * L;
-                const bool valid = mm < ZT;
+                const int mm = G.gslot[g + it * L];
+                const bool valid = mm != 255;
                 const uint32_t e = s_nb[valid ? mm : 0];
                 const int step = (int)(short)(e & 0xffffu), row = valid ? (int)(e >> 16) : zero_at;
                 part += Drow[row + p_i[step]] - Drow[row + p_j[step]];
@@ -292,14 +413,6 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
       atomicAdd(&st->accepted, (unsigned long long)a);
     }
   }
-}
-
-// Register-resident neighbour lists exist for 2, 3 and 6 visits per lane (FCC with three shells: 42
-// neighbours over 32 / 16 / 8 lanes; BCC with two shells: 14 over 8 / 16 / 32); anything else takes the
-// variant that reads the steps from shared memory.
-inline int group_nit(const Geom& G, int lanes) {
-  const int need = (G.ZT + lanes - 1) / lanes;
-  return need <= 2 ? 2 : need <= 3 ? 3 : need <= 6 ? 6 : 0;
 }
 
 // f<B, L, NIT>() for the runtime (B, lanes, nit)
