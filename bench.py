@@ -258,6 +258,34 @@ def run_ensemble(n_replicas: int, rounds: int = 20, sweeps_per_round: int = 10):
     return out
 
 
+def run_paper_shaped_fcc(edge: int = 400, sweeps: int = 10):
+    """A lattice of the paper's own shape: FCC, five species in the proportions
+    29/29/28/7/7 (reading S10), three shells, kT = 86 meV, synthetic EPI; the sub-warp kernel, device-timed."""
+    import torch
+    import paper_2509_20949_b200 as smcx
+    from smcx_inputs import composition_counts, make_accept_table, make_epi
+
+    dims = (edge, edge, edge)
+    lat = smcx.Lattice(smcx.FCC, dims, 5, 3, make_epi(3, 5, 400, 1006), make_accept_table(860), 1006, link_cell=4,
+                       kT_units=860)
+    lat.init_composition(composition_counts(lat.n_sites, (29, 29, 28, 7, 7)))
+    lat.sweep(3)
+    lat.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    lat.sweep(sweeps)
+    b.record()
+    lat.synchronize()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / sweeps
+    out = {"workload": f"FCC {edge}^3 conventional cells ({lat.n_sites} sites), 5 species 29/29/28/7/7, 3-shell int32 EPI in "
+                       f"[-400,400], kT=86 meV, link cell 4, seed 1006", "kernel": "sweep_group_per_cell/u8",
+           "value": lat.n_sites / (ms * 1e-3), "unit": "trial swaps/s", "sweep_ms": ms,
+           "paper_h800_per_gpu": 3.5e9, "paper_note": "PAPER.md:130, EPI model on H800; other hardware and interactions: context"}
+    lat.close()
+    return out
+
+
 def run_cuda(args, cfg, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -410,6 +438,8 @@ def run_cuda(args, cfg, rank, world, local_rank):
         if args.ensemble > 1 and world == 1:
             lat.close()
             out["temperature_parallel"] = run_ensemble(args.ensemble)
+            if args.fcc_edge > 0:
+                out["paper_shaped_fcc"] = run_paper_shaped_fcc(args.fcc_edge)
         print(json.dumps(out))
     lat.close()
     if world > 1:
@@ -427,6 +457,9 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 warp-per-cell, 2 thread-per-cell, 3 thread-per-cell persistent, 4 sub-warp group per cell")
     ap.add_argument("--storage", type=int, default=0, help="0 auto, 2 packed 2-bit, 8 uint8")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--fcc-edge", type=int, default=400,
+                    help="with --ensemble: also time the sub-warp kernel on an FCC lattice of the paper's shape, this many "
+                         "conventional cells per edge (0: skip)")
     ap.add_argument("--ensemble", type=int, default=128,
                     help="also time a replica-exchange ensemble of this many BCC 64^3 replicas (0: skip)")
     args = ap.parse_args()
