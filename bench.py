@@ -53,7 +53,7 @@ def measured_peak():
 # What binds the thread-per-cell kernels is the integer ALU pipe: instructions per trial on that
 # pipe from the SASS of the trial loop plus the share of the staging / write-back code (profiles/), the cycles an
 # IMAD.WIDE / POPC holds the pipe from profiles/r1_pipe_microbench.md.
-ALU_PIPE = {2: {"alu_inst": 59.0, "wide": 9.0, "popc": 6.0}, 3: {"alu_inst": 51.0, "wide": 8.0, "popc": 6.0}}
+ALU_PIPE = {2: {"alu_inst": 59.0, "wide": 9.0, "popc": 6.0}, 3: {"alu_inst": 50.5, "wide": 7.5, "popc": 6.0}}   # session 7 SASS: 47.4 in the trial loop + ~3 outside
 
 
 def alu_view(kernel: int, trials_per_s: float, clocks: dict):
