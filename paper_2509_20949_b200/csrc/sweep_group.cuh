@@ -18,7 +18,8 @@
 //    time, looks the tile step of the drawn direction up right away (off the chain of dependent trials)
 //    and hands step and acceptance draw round with group-wide shuffles;
 //  * control flow is uniform over the warp (a trial between equal species is computed and masked; a lane
-//    with fewer neighbours than the others visits a row of zeros), so the 32 / L cells of a warp never
+//    with fewer neighbours than the others visits the position one step in x from both sites, which is never a
+//    lattice site and always holds 0: the two table terms cancel), so the 32 / L cells of a warp never
 //    serialise, and the acceptance test reads the two-level filter tables in shared memory (see
 //    sweep_thread.cuh; the exact table in global memory only when u falls within E of the bound).
 // Results are bit-identical to the other kernels (tests/test_gpu_parity.py).
@@ -156,21 +157,22 @@ inline void group_tune_layout(Geom& G, int lanes) {
 }
 
 struct GroupSmem {
-  int d_stride;        // ints per ordered pair in the difference table (odd: spreads the pairs over the banks)
-  int d_copies;        // copies of the difference table (one per cell of a warp when rows fit 32 words)
+  int d_stride;        // ints per ordered pair in the difference table
+  int d_copies;        // 2: every 32-word stripe holds the pair's row twice, cells with odd index in their warp read the upper half
   int d_bytes, nb_bytes, filt_bytes, tile_bytes, total;
 };
 
-// Difference table row of the ordered pair (a,b): [s * n + x] for the shells, then corr(a,b), then n zeros.
+// Difference table row of the ordered pair (a,b): [s * n + x] for the shells, then corr(a,b).  When a row fits
+// 16 words and a warp holds several cells, rows are 32 words apart and stored twice (words 0..15 and 16..31):
+// the rows two cells of a warp read at the same time then lie in different halves of the banks whatever the pairs
+// (ncu, FCC 256^3, 16 lanes: 1.3-1.5 wavefronts per table load with one copy and a row stride of 21).
 inline GroupSmem group_smem_layout(const Geom& G, int lanes, int warps = kGroupWarpsPerBlock) {
   GroupSmem L;
   const int n = G.n_species;
-  int stride = G.n_shells * n + 1 + n;
-  if ((stride & 1) == 0) ++stride;
-  L.d_copies = 1;   // per-cell copies with rows 32 words apart were measured: FCC 128^3 0.912 -> 0.892 ms per sweep, but the
-                    // 4 KB more per block cost FCC 400^3 a resident block (18.3 -> 19.6 ms): not used
-  L.d_stride = stride;
-  L.d_bytes = ((n * n * stride * L.d_copies + 32) * 4 + 15) & ~15;
+  const int row = G.n_shells * n + 1;
+  if (lanes < 32 && row <= 16) { L.d_stride = 32; L.d_copies = 2; }
+  else { L.d_stride = row | 1; L.d_copies = 1; }
+  L.d_bytes = (n * n * L.d_stride * 4 + 15) & ~15;
   L.nb_bytes = (G.ZT * 4 + 15) & ~15;     // per neighbour: (step & 0xffff) | row << 16
   L.tile_bytes = group_tile_bytes(G.TW, G.gzpad, G.gskew);
   const int cells_per_block = warps * (32 / lanes);
@@ -196,7 +198,7 @@ __device__ __forceinline__ void group_split_index(int idx, int TW, float inv_TW,
 }
 
 // NIT > 0: every lane visits exactly NIT neighbours per site, their steps and rows in registers (NIT >=
-// ceil(ZT / L); surplus visits read the zero entries of the row).  NIT == 0: any ZT, steps from shared memory.
+// ceil(ZT / L); surplus visits cancel, see above).  NIT == 0: any ZT, steps from shared memory.
 template <int B, int L, int NIT>
 __global__ void __launch_bounds__(kGroupWarpsPerBlock * 32)
 sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t* __restrict__ epi,
@@ -214,13 +216,10 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   __shared__ unsigned s_acc[kGroupWarpsPerBlock];
 
   const int n = G.n_species, ZT = G.ZT;
-  const int corr_at = G.n_shells * n, zero_at = corr_at + 1;
-  // d_stride == 32 with fewer than 32 lanes: CPW copies, copy c at word c * (n n 32 + L)
-  const int d_copy_words = n * n * d_stride + L;
-  const int d_copies = (L < 32 && d_stride == 32) ? CPW : 1;
-  for (int k0 = threadIdx.x; k0 < n * n * d_stride * d_copies; k0 += blockDim.x) {
-    const int copy = k0 / (n * n * d_stride), k = k0 - copy * (n * n * d_stride);
-    const int pair = k / d_stride, e = k % d_stride;
+  const int corr_at = G.n_shells * n;
+  const bool d_twice = L < 32 && d_stride == 32;                // see group_smem_layout
+  for (int k = threadIdx.x; k < n * n * d_stride; k += blockDim.x) {
+    const int pair = k / d_stride, e = d_twice ? ((k % d_stride) & 15) : k % d_stride;
     const int a = pair / n, b = pair % n;
     int v = 0;
     if (e < corr_at) {
@@ -229,9 +228,9 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     } else if (e == corr_at) {
       v = 2 * epi[a * n + b] - epi[a * n + a] - epi[b * n + b];
     }
-    s_D[copy * d_copy_words + k] = v;
+    s_D[k] = v;
   }
-  const int32_t* s_Dg = s_D + (d_copies > 1 ? grp * d_copy_words : 0);   // this cell's copy
+  const int32_t* s_Dg = s_D + (d_twice ? (grp & 1) * 16 : 0);   // this cell's half of the stripes
   if (G.filter_E >= 0)
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
   const int ypitch = group_ypitch(G.TW), zpitch = group_zpitch(G.TW, G.gzpad);
@@ -245,8 +244,8 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   for (int it = 0; it < NIT; ++it) {
     const int mm = G.gslot[g + it * L];
     const bool valid = mm != 255;
-    nstep[it] = valid ? G.off[mm][2] * zpitch + G.off[mm][1] * ypitch + G.off[mm][0] : 0;
-    nrow[it] = valid ? G.shell_of[mm] * n : zero_at;
+    nstep[it] = valid ? G.off[mm][2] * zpitch + G.off[mm][1] * ypitch + G.off[mm][0] : 1;
+    nrow[it] = valid ? G.shell_of[mm] * n : 0;
   }
 
   const uint32_t t = (uint32_t)st->sweep;
@@ -267,6 +266,9 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     t0y = (oy + cy * w - H + G.Ly) % G.Ly;
     t0z = (oz + cz * w - H + G.Lz) % G.Lz;
   }
+  // positions that are not lattice sites must read 0 (empty neighbour slots visit them): clear the tile first
+  for (int k = g; k < tile_bytes / 4; k += L) reinterpret_cast<uint32_t*>(tile)[k] = 0u;
+  __syncwarp();
   // a3: stage the tile, four conventional cells per lane in flight (a group without a cell stages species
   // 0 everywhere: all its trials are no-ops)
   for (int idx0 = g; idx0 < n_conv; idx0 += 4 * L) {
@@ -341,7 +343,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
                 const int mm = G.gslot[g + it * L];
                 const bool valid = mm != 255;
                 const uint32_t e = s_nb[valid ? mm : 0];
-                const int step = (int)(short)(e & 0xffffu), row = valid ? (int)(e >> 16) : zero_at;
+                const int step = valid ? (int)(short)(e & 0xffffu) : 1, row = valid ? (int)(e >> 16) : 0;
                 part += Drow[row + p_i[step]] - Drow[row + p_j[step]];
               }
             }
