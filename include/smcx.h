@@ -53,8 +53,8 @@ enum { SMCX_BCC = 0, SMCX_FCC = 1 };
 enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
 
 /* Which sweep kernel runs.  WARP_PER_CELL: any lattice/shell list, U8 storage.
- * GROUP_PER_CELL: the same generality with 4, 8, 16 or 32 lanes per link cell (16 if that still gives
- * every SM about twelve warps, else 32; the environment variable SMCX_GROUP_LANES overrides the choice) and a
+ * GROUP_PER_CELL: the same generality with 4, 8, 16 or 32 lanes per link cell (8, 16 or 32 by the number of
+ * cells per colour; the environment variable SMCX_GROUP_LANES overrides the choice) and a
  * per-pair difference table in shared memory; what AUTO picks whenever a thread kernel does not apply.
  * THREAD_PER_CELL: BCC, first two shells, link_cell = 4, n_species <= 4, 2BIT storage; one block per
  * 128 cells, two-level acceptance filter in shared memory.

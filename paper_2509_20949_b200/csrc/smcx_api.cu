@@ -111,7 +111,6 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
 
   Geom& G = plan->G;
   std::memset(&G, 0, sizeof(G));
-  G.gzpad = 8; G.gskew = 64;   // defaults until group_tune_layout() has run
   G.lattice = p->lattice;
   G.B = p->lattice == SMCX_BCC ? 2 : 4;
   G.n_species = n;
@@ -139,6 +138,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   if (2 * w < 2 * r0 + R) return SMCX_E_LINK_CELL_TOO_SMALL;
   G.H = (r0 + R + 1) / 2;
   G.TW = w + 2 * G.H;
+  group_default_layout(G);     // until group_tune_layout() has run
   long long n_sites = G.B;
   for (int a = 0; a < 3; ++a) {
     const int L = p->dims[a];
@@ -208,14 +208,15 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   }
   plan->kernel = kernel;
   plan->storage = storage;
-  // sub-warp kernel: 16 lanes per cell when that gives every SM about twelve warps of cells, else 32 (with
-  // fewer cells a pass is as long as one cell's chain of trials, which more lanes shorten).  Measured on FCC,
-  // 5 species, 3 shells: 128^3 (2,048 warps at 16 lanes) 0.92 / 1.00 ms per sweep with 16 / 32 lanes; 400^3
-  // (2.56e8 sites) 31.8 / 20.4 / 23.2 ms with 8 / 16 / 32 lanes (8 lanes: one block of 139 KB per SM).
-  // 4 and 8 lanes stay selectable.
+  // sub-warp kernel: lanes per cell by the number of cells of a colour.  With few cells a pass is as long as
+  // one cell's chain of trials, which more lanes shorten; with many, fewer lanes mean less replicated work.
+  // Measured on FCC, 5 species, 3 shells (ms per sweep with 8 / 16 / 32 lanes): 128^3 (4,096 cells per colour)
+  // 0.99 / 0.87 / 1.00; 400^3 (125,000 cells per colour) 14.9 / 15.5 / 21.9.
   plan->group_lanes = 32;
   if (group_smem_layout(G, 16, 2).total <= 227 * 1024 && (long long)G.cells_per_colour * 16 / 32 >= 148ll * 12)
     plan->group_lanes = 16;
+  if (group_smem_layout(G, 8, 2).total <= 227 * 1024 && (long long)G.cells_per_colour * 8 / 32 >= 148ll * 48)
+    plan->group_lanes = 8;
   if (const char* env = std::getenv("SMCX_GROUP_LANES")) {
     const int v = std::atoi(env);
     if ((v == 4 || v == 8 || v == 16 || v == 32) && group_smem_layout(G, v, 2).total <= 227 * 1024) plan->group_lanes = v;

@@ -102,9 +102,12 @@ struct Geom {
   short delta[4][kMaxNeighbours];
   // sub-warp kernel (sweep_group.cuh), chosen on the host by a model of the shared-memory banks:
   // gslot[slot] = neighbour visited by lane (slot % lanes) in its visit (slot / lanes), 255 = none;
-  // gzpad / gskew = padding of the tile's z pitch / extra distance between the tiles of a warp (bytes)
+  // tile index of position (px, py, pz) (units of a/2) = (px + gA py + gB pz) >> gshift: gshift 0 is a plain
+  // pitched byte grid, gshift 1 a compact linear index over the lattice sites only; gskew = extra distance
+  // between the tiles of a warp, gtile = bytes of one tile without the skew
   unsigned char gslot[kMaxGroupSlots];
-  short gzpad, gskew;
+  int gA, gB, gtile;
+  short gshift, gskew;
 };
 
 }  // namespace smcxk

@@ -6,9 +6,9 @@
 // by the latency of one cell's chain of 256 dependent trials):
 //  * the serial part of a trial (slot -> site, direction, species of i and j, acceptance) is replicated
 //    over L lanes instead of 32, and 32 / L cells share a warp;
-//  * the tile is indexed by POSITION in units of a/2 (a (2 TW)^3 byte grid of which a BCC / FCC lattice
-//    uses a quarter / a half), so the tile-index step to neighbour m is the same for every site whatever
-//    its basis: lane g keeps the steps and the table rows of its neighbours g, g + L, ... in registers,
+//  * the tile index of a site is LINEAR in its position, (px + A py + B pz) >> shift in units of a/2 (see
+//    below), so the tile-index step to neighbour m is the same for every site whatever its basis: lane g
+//    keeps the steps and the table rows of its neighbours (slots g, g + L, ... of G.gslot) in registers,
 //    and a neighbour visit is one add, the species load, one add and the load of
 //    D[(a,b)][s][x] = V_s(b,x) - V_s(a,x) from a table built in shared memory when the block starts.
 //    The sums over the neighbours of i and of j both include the i-j bond;
@@ -18,8 +18,8 @@
 //    time, looks the tile step of the drawn direction up right away (off the chain of dependent trials)
 //    and hands step and acceptance draw round with group-wide shuffles;
 //  * control flow is uniform over the warp (a trial between equal species is computed and masked; a lane
-//    with fewer neighbours than the others visits the position one step in x from both sites, which is never a
-//    lattice site and always holds 0: the two table terms cancel), so the 32 / L cells of a warp never
+//    with fewer neighbours than the others visits the two sites themselves with the row of shell 0: a term that
+//    depends on the pair (a,b) only and is taken out of corr(a,b) when the table is built), so the 32 / L cells of a warp never
 //    serialise, and the acceptance test reads the two-level filter tables in shared memory (see
 //    sweep_thread.cuh; the exact table in global memory only when u falls within E of the bound).
 // Results are bit-identical to the other kernels (tests/test_gpu_parity.py).
@@ -33,20 +33,58 @@
 namespace smcxk {
 
 constexpr int kGroupWarpsPerBlock = 8;    // at most; group_warps_per_block() picks fewer when that lets more blocks share an SM
-// Tile layout in shared memory (bytes): position (pz, py, px) at pz * zpitch + py * ypitch + px with
-// ypitch = 2 TW rounded up to a multiple of 4 and zpitch = 2 TW * ypitch + G.gzpad; the tiles of the cells
-// of a warp are G.gskew bytes further apart than a multiple of 128 bytes.  Pad, skew and the assignment of
-// neighbours to (lane, visit) slots (G.gslot) are chosen on the host by group_tune_layout() below from a
-// model of the 32 banks: ncu on FCC 128^3 showed 71 % of the shared-memory wavefronts to be bank conflicts
-// with an unpadded tile, 3.0 / 2.5 / 2.5 wavefronts per neighbour load with pad 12 / skew 4 and neighbours
-// dealt to the lanes in shell order; the tuned layout brings the model's figure from 8.0 to about 4.
-__host__ __device__ inline int group_ypitch(int TW) { return (2 * TW + 3) & ~3; }
-__host__ __device__ inline int group_zpitch(int TW, int zpad) { return 2 * TW * group_ypitch(TW) + zpad; }
-inline int group_tile_bytes(int TW, int zpad, int skew) { return ((2 * TW * group_zpitch(TW, zpad) + 127) & ~127) + skew; }
+// Tile layout in shared memory: the species of the site at position (px, py, pz) (units of a/2, tile-relative)
+// is the byte at index (px + A py + B pz) >> shift.  The index is LINEAR in the position, so the step to
+// neighbour m is the same number for every site whatever its basis, and lane g keeps its steps in registers.
+// shift = 1 with suitable odd / even A, B enumerates the lattice sites only (every lattice vector has an even
+// px + A py + B pz), about 2.2 KB per FCC cell at w = 4 and 1.1 KB per BCC cell, where a plain pitched grid
+// over all positions (shift = 0) takes 4.3 KB.  The tiles of the cells of a warp are G.gskew bytes further
+// apart than a multiple of 128 bytes.  A, B, skew and the assignment of neighbours to (lane, visit) slots
+// (G.gslot) are chosen on the host by group_tune_layout() from a model of the 32 banks: ncu on FCC 128^3
+// showed 71 % of the shared-memory wavefronts to be bank conflicts with an unpadded grid and 2.5-3.0
+// wavefronts per neighbour load with a fixed pad and neighbours dealt to the lanes in shell order.
+__host__ __device__ inline int group_index(int px, int py, int pz, int A, int B, int sh) { return (px + A * py + B * pz) >> sh; }
+
+inline void group_basis_pos_host(int Bsites, int b, int p[3]) {
+  if (Bsites == 2) { p[0] = p[1] = p[2] = b; return; }
+  p[0] = (b >> 1) & 1; p[1] = b & 1; p[2] = (b == 1 || b == 2) ? 1 : 0;
+}
+
+// Bytes of a tile (largest site index + 1, rounded up to 128) if every site of the TW^3 conventional cells
+// gets an integral index of its own, else 0.
+inline int group_layout_extent(const Geom& G, int A, int B, int sh) {
+  const int P = 2 * G.TW;
+  const long long top = ((long long)(P - 1) * (1 + A + B)) >> sh;
+  if (A <= 0 || B <= 0 || top > 60000) return 0;
+  std::vector<unsigned char> seen((size_t)top + 1, 0);
+  for (int tz = 0; tz < G.TW; ++tz)
+    for (int ty = 0; ty < G.TW; ++ty)
+      for (int tx = 0; tx < G.TW; ++tx)
+        for (int b = 0; b < G.B; ++b) {
+          int bp[3];
+          group_basis_pos_host(G.B, b, bp);
+          const int num = (2 * tx + bp[0]) + A * (2 * ty + bp[1]) + B * (2 * tz + bp[2]);
+          if (num & ((1 << sh) - 1)) return 0;
+          const int idx = num >> sh;
+          if (seen[(size_t)idx]) return 0;
+          seen[(size_t)idx] = 1;
+        }
+  return ((int)top + 1 + 127) & ~127;
+}
+
+inline void group_default_layout(Geom& G) {   // plain pitched grid over all positions
+  G.gshift = 0;
+  G.gA = (2 * G.TW + 3) & ~3;
+  G.gB = 2 * G.TW * G.gA + 8;
+  G.gskew = 64;
+  G.gtile = ((2 * G.TW * G.gB + 127) & ~127);
+  for (int s = 0; s < kMaxGroupSlots; ++s) G.gslot[s] = s < G.ZT ? (unsigned char)s : (unsigned char)255;
+}
 
 // Register-resident neighbour lists exist for 2, 3 and 6 visits per lane (FCC with three shells: 42
 // neighbours over 32 / 16 / 8 lanes; BCC with two shells: 14 over 8 / 16 / 32); anything else takes the
-// variant that reads the steps from shared memory.
+// variant that reads the steps from shared memory (11 visits in registers, FCC with 4 lanes, was measured: 23 ms
+// per sweep of FCC 400^3 against 15 ms with 8 lanes).
 inline int group_nit(const Geom& G, int lanes) {
   const int need = (G.ZT + lanes - 1) / lanes;
   return need <= 2 ? 2 : need <= 3 ? 3 : need <= 6 ? 6 : 0;
@@ -84,40 +122,53 @@ inline double group_bank_cost(const int* step, const unsigned char* slot, int la
   return total / 4.0;
 }
 
-// Chooses G.gzpad, G.gskew and G.gslot for this lane count: every (pad, skew) with the neighbours in
-// shell order first, then a deterministic local search (swaps of two slots) on the best few.
+// Chooses the layout (G.gA, G.gB, G.gshift, G.gtile, G.gskew) and G.gslot for this lane count: candidate
+// index maps (the pitched grid with a few paddings; compact maps with shift 1, the smallest B for every A in
+// a range) no more than 8 % above the smallest tile, every skew, neighbours in shell order first; then a
+// deterministic local search (swaps of two slots) on the best few.
 inline void group_tune_layout_search(Geom& G, int lanes) {
-  const int visits = group_visits(G, lanes), slots = visits * lanes, ZT = G.ZT;
-  unsigned char ident[kMaxGroupSlots];
-  for (int s = 0; s < kMaxGroupSlots; ++s) ident[s] = s < ZT ? (unsigned char)s : (unsigned char)255;
-  G.gzpad = 8; G.gskew = 64;
-  for (int s = 0; s < kMaxGroupSlots; ++s) G.gslot[s] = ident[s];
+  const int visits = group_visits(G, lanes), slots = visits * lanes, ZT = G.ZT, P = 2 * G.TW;
+  group_default_layout(G);
   if (slots > kMaxGroupSlots || lanes > 32) return;
-  const int yp = group_ypitch(G.TW);
-  struct Cand { double cost; int pad, skew; } best[4] = {{1e30, 8, 64}, {1e30, 8, 64}, {1e30, 8, 64}, {1e30, 8, 64}};
-  int step[kMaxNeighbours];
-  // a layout must not cost a resident block: blocks per SM as with the smallest tile (tables ~ 8 KB)
-  const int cells_per_block = kGroupWarpsPerBlock * (32 / lanes);
-  const int blocks_min_tile = (227 * 1024) / (8192 + cells_per_block * group_tile_bytes(G.TW, 0, 4));
+  struct Map { int A, B, sh, bytes; };
+  std::vector<Map> maps;
   for (int pad = 0; pad < 32; pad += 4) {
-    const int zp = group_zpitch(G.TW, pad);
-    for (int m = 0; m < ZT; ++m) step[m] = G.off[m][2] * zp + G.off[m][1] * yp + G.off[m][0];
+    const int A = (P + 3) & ~3, B = P * A + pad;
+    maps.push_back({A, B, 0, (P * B + 127) & ~127});
+  }
+  for (int A = P / 2; A <= 2 * P + 8; ++A) {
+    int found = 0;
+    for (int B = A * (P / 2); B <= A * (P + 2) + P + 2 && found < 2; ++B) {
+      const int bytes = group_layout_extent(G, A, B, 1);
+      if (bytes > 0) { maps.push_back({A, B, 1, bytes}); ++found; }
+    }
+  }
+  int min_bytes = 1 << 30;
+  for (const Map& m : maps) min_bytes = std::min(min_bytes, m.bytes);
+  struct Cand { double cost; Map m; int skew; };
+  Cand best[4];
+  for (int k = 0; k < 4; ++k) best[k] = {1e30, maps[0], 64};
+  int step[kMaxNeighbours];
+  for (const Map& m : maps) {
+    if (m.bytes > min_bytes + min_bytes / 12) continue;
+    for (int q = 0; q < ZT; ++q) step[q] = (G.off[q][0] + m.A * G.off[q][1] + m.B * G.off[q][2]) >> m.sh;
+    unsigned char ident[kMaxGroupSlots];
+    for (int s = 0; s < kMaxGroupSlots; ++s) ident[s] = s < ZT ? (unsigned char)s : (unsigned char)255;
     for (int skew = 4; skew < 128; skew += 4) {
-      if (blocks_min_tile > 0 &&
-          (227 * 1024) / (8192 + cells_per_block * group_tile_bytes(G.TW, pad, skew)) < blocks_min_tile) continue;
-      const double c = group_bank_cost(step, ident, lanes, visits, group_tile_bytes(G.TW, pad, skew) / 4);
+      const double c = group_bank_cost(step, ident, lanes, visits, (m.bytes + skew) / 4);
       for (int k = 0; k < 4; ++k)
-        if (c < best[k].cost) { for (int j = 3; j > k; --j) best[j] = best[j - 1]; best[k] = {c, pad, skew}; break; }
+        if (c < best[k].cost) { for (int j = 3; j > k; --j) best[j] = best[j - 1]; best[k] = {c, m, skew}; break; }
       if (lanes == 32) break;   // one cell per warp: the skew does not matter
     }
   }
   double best_cost = 1e30;
   for (int k = 0; k < 4; ++k) {
-    const int pad = best[k].pad, skew = best[k].skew, zp = group_zpitch(G.TW, pad);
-    const int tw = group_tile_bytes(G.TW, pad, skew) / 4;
-    for (int m = 0; m < ZT; ++m) step[m] = G.off[m][2] * zp + G.off[m][1] * yp + G.off[m][0];
+    if (best[k].cost >= 1e30) continue;
+    const Map m = best[k].m;
+    const int skew = best[k].skew, tw = (m.bytes + skew) / 4;
+    for (int q = 0; q < ZT; ++q) step[q] = (G.off[q][0] + m.A * G.off[q][1] + m.B * G.off[q][2]) >> m.sh;
     unsigned char slot[kMaxGroupSlots];
-    for (int s = 0; s < kMaxGroupSlots; ++s) slot[s] = ident[s];
+    for (int s = 0; s < kMaxGroupSlots; ++s) slot[s] = s < ZT ? (unsigned char)s : (unsigned char)255;
     double c = group_bank_cost(step, slot, lanes, visits, tw);
     uint32_t rng = 12345u + (uint32_t)k;
     for (int iter = 0; iter < 2500 && c > visits; ++iter) {
@@ -129,13 +180,14 @@ inline void group_tune_layout_search(Geom& G, int lanes) {
       if (c2 <= c) c = c2; else { slot[s2] = slot[s1]; slot[s1] = t1; }
     }
     if (c < best_cost) {
-      best_cost = c; G.gzpad = (short)pad; G.gskew = (short)skew;
+      best_cost = c;
+      G.gA = m.A; G.gB = m.B; G.gshift = (short)m.sh; G.gtile = m.bytes; G.gskew = (short)skew;
       for (int s = 0; s < kMaxGroupSlots; ++s) G.gslot[s] = slot[s];
     }
   }
 }
 
-struct GroupTuneEntry { int lattice, n_shells, TW, lanes; short zpad, skew; unsigned char slot[kMaxGroupSlots]; };
+struct GroupTuneEntry { int lattice, n_shells, TW, lanes, A, B, tile; short shift, skew; unsigned char slot[kMaxGroupSlots]; };
 inline void group_tune_layout(Geom& G, int lanes) {
   // the result depends on (lattice, shells, tile edge, lanes) only: computed once per process
   static std::mutex mu;
@@ -144,13 +196,13 @@ inline void group_tune_layout(Geom& G, int lanes) {
     std::lock_guard<std::mutex> lock(mu);
     for (const GroupTuneEntry& e : cache)
       if (e.lattice == G.lattice && e.n_shells == G.n_shells && e.TW == G.TW && e.lanes == lanes) {
-        G.gzpad = e.zpad; G.gskew = e.skew;
+        G.gA = e.A; G.gB = e.B; G.gtile = e.tile; G.gshift = e.shift; G.gskew = e.skew;
         for (int s = 0; s < kMaxGroupSlots; ++s) G.gslot[s] = e.slot[s];
         return;
       }
   }
   group_tune_layout_search(G, lanes);
-  GroupTuneEntry e{G.lattice, G.n_shells, G.TW, lanes, G.gzpad, G.gskew, {}};
+  GroupTuneEntry e{G.lattice, G.n_shells, G.TW, lanes, G.gA, G.gB, G.gtile, G.gshift, G.gskew, {}};
   for (int s = 0; s < kMaxGroupSlots; ++s) e.slot[s] = G.gslot[s];
   std::lock_guard<std::mutex> lock(mu);
   cache.push_back(e);
@@ -174,7 +226,7 @@ inline GroupSmem group_smem_layout(const Geom& G, int lanes, int warps = kGroupW
   else { L.d_stride = row | 1; L.d_copies = 1; }
   L.d_bytes = (n * n * L.d_stride * 4 + 15) & ~15;
   L.nb_bytes = (G.ZT * 4 + 15) & ~15;     // per neighbour: (step & 0xffff) | row << 16
-  L.tile_bytes = group_tile_bytes(G.TW, G.gzpad, G.gskew);
+  L.tile_bytes = G.gtile + G.gskew;
   const int cells_per_block = warps * (32 / lanes);
   L.filt_bytes = kFilterWords * 4;
   L.total = (L.d_bytes + L.nb_bytes + L.filt_bytes + cells_per_block * L.tile_bytes + 15) & ~15;
@@ -198,7 +250,7 @@ __device__ __forceinline__ void group_split_index(int idx, int TW, float inv_TW,
 }
 
 // NIT > 0: every lane visits exactly NIT neighbours per site, their steps and rows in registers (NIT >=
-// ceil(ZT / L); surplus visits cancel, see above).  NIT == 0: any ZT, steps from shared memory.
+// ceil(ZT / L); surplus visits are compensated in corr, see above).  NIT == 0: any ZT, steps from shared memory.
 template <int B, int L, int NIT>
 __global__ void __launch_bounds__(kGroupWarpsPerBlock * 32)
 sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t* __restrict__ epi,
@@ -217,6 +269,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
 
   const int n = G.n_species, ZT = G.ZT;
   const int corr_at = G.n_shells * n;
+  const int n_empty = (NIT > 0 ? NIT : (ZT + L - 1) / L) * L - ZT;   // neighbour slots without a neighbour
   const bool d_twice = L < 32 && d_stride == 32;                // see group_smem_layout
   for (int k = threadIdx.x; k < n * n * d_stride; k += blockDim.x) {
     const int pair = k / d_stride, e = d_twice ? ((k % d_stride) & 15) : k % d_stride;
@@ -226,16 +279,18 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
       const int s = e / n, x = e % n;
       v = epi[(s * n + b) * n + x] - epi[(s * n + a) * n + x];
     } else if (e == corr_at) {
-      v = 2 * epi[a * n + b] - epi[a * n + a] - epi[b * n + b];
+      // corr(a,b), less what the empty slots add: each reads D_0(sigma_i) - D_0(sigma_j) = D_0(a) - D_0(b)
+      v = 2 * epi[a * n + b] - epi[a * n + a] - epi[b * n + b] -
+          n_empty * ((epi[b * n + a] - epi[a * n + a]) - (epi[b * n + b] - epi[a * n + b]));
     }
     s_D[k] = v;
   }
   const int32_t* s_Dg = s_D + (d_twice ? (grp & 1) * 16 : 0);   // this cell's half of the stripes
   if (G.filter_E >= 0)
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
-  const int ypitch = group_ypitch(G.TW), zpitch = group_zpitch(G.TW, G.gzpad);
+  const int cA = G.gA, cB = G.gB, csh = G.gshift;
   for (int k = threadIdx.x; k < ZT; k += blockDim.x) {
-    const int step = G.off[k][2] * zpitch + G.off[k][1] * ypitch + G.off[k][0];
+    const int step = group_index(G.off[k][0], G.off[k][1], G.off[k][2], cA, cB, csh);
     s_nb[k] = ((uint32_t)(uint16_t)(short)step) | ((uint32_t)(G.shell_of[k] * n) << 16);
   }
   // this lane's neighbours
@@ -244,7 +299,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   for (int it = 0; it < NIT; ++it) {
     const int mm = G.gslot[g + it * L];
     const bool valid = mm != 255;
-    nstep[it] = valid ? G.off[mm][2] * zpitch + G.off[mm][1] * ypitch + G.off[mm][0] : 1;
+    nstep[it] = valid ? group_index(G.off[mm][0], G.off[mm][1], G.off[mm][2], cA, cB, csh) : 0;
     nrow[it] = valid ? G.shell_of[mm] * n : 0;
   }
 
@@ -266,9 +321,6 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     t0y = (oy + cy * w - H + G.Ly) % G.Ly;
     t0z = (oz + cz * w - H + G.Lz) % G.Lz;
   }
-  // positions that are not lattice sites must read 0 (empty neighbour slots visit them): clear the tile first
-  for (int k = g; k < tile_bytes / 4; k += L) reinterpret_cast<uint32_t*>(tile)[k] = 0u;
-  __syncwarp();
   // a3: stage the tile, four conventional cells per lane in flight (a group without a cell stages species
   // 0 everywhere: all its trials are no-ops)
   for (int idx0 = g; idx0 < n_conv; idx0 += 4 * L) {
@@ -280,7 +332,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
       int tx, ty, tz;
       group_split_index(idx, TW, inv_TW, tx, ty, tz);
       v[q] = 0;
-      at[q] = idx < n_conv ? 2 * tz * zpitch + 2 * ty * ypitch + 2 * tx : -1;
+      at[q] = idx < n_conv ? group_index(2 * tx, 2 * ty, 2 * tz, cA, cB, csh) : -1;
       if (active && idx < n_conv) {
         int gx = t0x + tx; if (gx >= G.Lx) gx -= G.Lx;
         int gy = t0y + ty; if (gy >= G.Ly) gy -= G.Ly;
@@ -295,7 +347,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
       unsigned char* dst = tile + at[q];
 #pragma unroll
       for (int b = 0; b < B; ++b)
-        dst[group_basis_pos<B>(b, 2) * zpitch + group_basis_pos<B>(b, 1) * ypitch + group_basis_pos<B>(b, 0)] =
+        dst[group_index(group_basis_pos<B>(b, 0), group_basis_pos<B>(b, 1), group_basis_pos<B>(b, 2), cA, cB, csh)] =
             (unsigned char)(v[q] >> (8 * b));
     }
   }
@@ -312,7 +364,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     for (int lz = 0; lz < w; ++lz)
       for (int ly = 0; ly < w; ++ly)
         for (int lx = 0; lx < w; ++lx) {
-          const int conv = 2 * (lz + H) * zpitch + 2 * (ly + H) * ypitch + 2 * (lx + H);   // position (0,0,0) of the conventional cell
+          const int conv = group_index(2 * (lx + H), 2 * (ly + H), 2 * (lz + H), cA, cB, csh);   // position (0,0,0) of the conventional cell
 #pragma unroll
           for (int b = 0; b < B; ++b, ++k) {
             if ((k & (2 * L - 1)) == 0) {  // a4: the L Philox calls of a group cover the next 2 L slots
@@ -325,8 +377,8 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
             const int src = (k >> 1) & (L - 1);
             const int step_j = __shfl_sync(0xffffffffu, (k & 1) ? r_step_odd : r_step_even, src, L);
             const uint32_t u = __shfl_sync(0xffffffffu, (k & 1) ? r_u_odd : r_u_even, src, L);
-            const unsigned char* p_i = tile + conv + group_basis_pos<B>(b, 2) * zpitch + group_basis_pos<B>(b, 1) * ypitch +
-                                       group_basis_pos<B>(b, 0);
+            const unsigned char* p_i = tile + conv + group_index(group_basis_pos<B>(b, 0), group_basis_pos<B>(b, 1),
+                                                                 group_basis_pos<B>(b, 2), cA, cB, csh);
             const unsigned char* p_j = p_i + step_j;
             const int sa = *p_i, sb = *p_j;
             // a5: partial sums over this lane's neighbours of i (a -> b) and of j (b -> a); a trial between
@@ -343,7 +395,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
                 const int mm = G.gslot[g + it * L];
                 const bool valid = mm != 255;
                 const uint32_t e = s_nb[valid ? mm : 0];
-                const int step = valid ? (int)(short)(e & 0xffffu) : 1, row = valid ? (int)(e >> 16) : 0;
+                const int step = valid ? (int)(short)(e & 0xffffu) : 0, row = valid ? (int)(e >> 16) : 0;
                 part += Drow[row + p_i[step]] - Drow[row + p_j[step]];
               }
             }
@@ -395,7 +447,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
         const int px = 2 * tx + group_basis_pos<B>(b, 0), py = 2 * ty + group_basis_pos<B>(b, 1),
                   pz = 2 * tz + group_basis_pos<B>(b, 2);
         if (px >= lo && px <= hi && py >= lo && py <= hi && pz >= lo && pz <= hi)
-          species[gi + b] = tile[pz * zpitch + py * ypitch + px];
+          species[gi + b] = tile[group_index(px, py, pz, cA, cB, csh)];
       }
     }
   }
@@ -435,14 +487,15 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
 #define SMCX_GROUP_DISPATCH(Bv, lanes, nit, ...)              \
   if ((Bv) == 2) { SMCX_GROUP_DISPATCH_L(2, lanes, nit, __VA_ARGS__) } else { SMCX_GROUP_DISPATCH_L(4, lanes, nit, __VA_ARGS__) }
 
-// Warps per block: 8, or 4 / 2 when a block of 8 warps of tiles would leave an SM with fewer than three
-// blocks (large tiles with few lanes per cell); SMCX_GROUP_WARPS overrides it for experiments.
+// Warps per block: 8, or 4 / 2 when a block of 8 warps of tiles would leave an SM with fewer than four
+// blocks (measured, FCC 400^3, 8 lanes: 16.8 / 14.9 / 16.5 ms per sweep with 8 / 4 / 2 warps per block);
+// SMCX_GROUP_WARPS overrides it for experiments.
 inline int group_warps_per_block(const Geom& G, int lanes) {
   int warps = kGroupWarpsPerBlock;
-  while (warps > 2 && 3 * group_smem_layout(G, lanes, warps).total > 227 * 1024) warps >>= 1;
+  while (warps > 2 && 4 * group_smem_layout(G, lanes, warps).total > 227 * 1024) warps >>= 1;
   if (const char* env = std::getenv("SMCX_GROUP_WARPS")) {
     const int v = std::atoi(env);
-    if ((v == 1 || v == 2 || v == 4 || v == 8) && group_smem_layout(G, lanes, v).total <= 227 * 1024) warps = v;
+    if (v >= 1 && v <= 8 && group_smem_layout(G, lanes, v).total <= 227 * 1024) warps = v;
   }
   return warps;
 }
