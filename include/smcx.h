@@ -171,6 +171,13 @@ int smcx_synchronize(smcx_t *h);
 int smcx_shell_offsets(smcx_t *h, int32_t shell, int32_t *xyz, int32_t max_offsets, int32_t *n_offsets);
 int smcx_get_config(smcx_t *h, int32_t *storage, int32_t *kernel, int64_t *n_sites, int64_t *n_cells);
 int64_t smcx_kernel_launches(smcx_t *h); /* kernels launched by this handle so far */
+/* Shared-memory tile layout the host chose for the GROUP_PER_CELL kernel with these parameters (needs no
+ * GPU): lanes per cell; the tile index of the site at tile position (px, py, pz), units of a/2, is
+ * (px + A py + B pz) >> shift; tile_bytes per cell plus skew bytes between the tiles of a warp;
+ * slots[k] = neighbour (index into the concatenated shell list) that lane k % lanes visits in its visit
+ * k / lanes, 255 = none, k < 128.  Every pointer may be NULL. */
+int smcx_group_layout(const smcx_params_t *p, int32_t *lanes, int32_t *A, int32_t *B, int32_t *shift,
+                      int32_t *tile_bytes, int32_t *skew, uint8_t *slots);
 
 /* ---- Temperature parallelism on one GPU: replica ensemble and replica exchange -----------------
  * "multiple replicas of the same system are simulated concurrently at different

@@ -81,6 +81,7 @@ def load_library(build_if_missing: bool = True):
         "smcx_shell_offsets": (C.c_int, [vp, C.c_int32, i32p, C.c_int32, i32p]),
         "smcx_get_config": (C.c_int, [vp, i32p, i32p, i64p, i64p]),
         "smcx_kernel_launches": (C.c_int64, [vp]),
+        "smcx_group_layout": (C.c_int, [C.POINTER(_Params), i32p, i32p, i32p, i32p, i32p, i32p, C.POINTER(C.c_uint8)]),
         "smcx_ensemble_create": (C.c_int, [C.POINTER(vp), C.POINTER(_Params), C.c_int32, i32p,
                                            C.POINTER(C.POINTER(C.c_uint32)), i32p, C.POINTER(C.c_uint64), C.c_uint64]),
         "smcx_ensemble_destroy": (None, [vp]),
@@ -378,6 +379,23 @@ class Ensemble:
     @property
     def kernel_launches(self) -> int:
         return int(self._lib.smcx_ensemble_kernel_launches(self._e))
+
+
+def group_layout(**kw) -> dict:
+    """smcx_group_layout: the tile layout the host picks for the sub-warp kernel (no GPU needed)."""
+    lib = load_library()
+    defaults = dict(link_cell=4, kT_units=0, storage=0, kernel=0, device=0, trace_capacity=0)
+    defaults.update(kw)
+    p, _keep = _make_params(**defaults)
+    v = [C.c_int32() for _ in range(6)]
+    slots = (C.c_uint8 * 128)()
+    rc = lib.smcx_group_layout(C.byref(p), *[C.byref(x) for x in v], slots)
+    if rc != 0:
+        raise SmcxError(rc, "smcx_group_layout")
+    names = ("lanes", "A", "B", "shift", "tile_bytes", "skew")
+    out = {k: x.value for k, x in zip(names, v)}
+    out["slots"] = np.frombuffer(bytes(slots), dtype=np.uint8).copy()
+    return out
 
 
 def workspace_bytes(**kw) -> int:

@@ -864,6 +864,23 @@ int smcx_get_config(smcx_t* h, int32_t* storage, int32_t* kernel, int64_t* n_sit
 
 int64_t smcx_kernel_launches(smcx_t* h) { return h ? h->launches : 0; }
 
+int smcx_group_layout(const smcx_params_t* p, int32_t* lanes, int32_t* A, int32_t* B, int32_t* shift,
+                      int32_t* tile_bytes, int32_t* skew, uint8_t* slots) {
+  if (!p) return SMCX_E_NULL_ARG;
+  Plan plan;
+  const int rc = make_plan(p, &plan);
+  if (rc != SMCX_OK) return rc;
+  const Geom& G = plan.G;
+  if (lanes) *lanes = plan.group_lanes;
+  if (A) *A = G.gA;
+  if (B) *B = G.gB;
+  if (shift) *shift = G.gshift;
+  if (tile_bytes) *tile_bytes = G.gtile;
+  if (skew) *skew = G.gskew;
+  if (slots) std::memcpy(slots, G.gslot, kMaxGroupSlots);
+  return SMCX_OK;
+}
+
 }  // extern "C"
 
 #include "ensemble_api.inc"

@@ -102,3 +102,45 @@ def test_no_cpu_fallback_without_a_device():
     h = C.c_void_p()
     assert lib.smcx_create(C.byref(h), C.byref(p)) == -11
     assert not h.value
+
+
+@pytest.mark.parametrize("lat,dims,n_sp,n_shells,w", [
+    (1, (128, 128, 128), 5, 3, 4),   # config 3
+    (1, (400, 400, 400), 5, 3, 4),   # paper-shaped lattice (8 lanes)
+    (0, (64, 64, 64), 5, 2, 4),      # BCC the thread kernels do not take
+    (0, (24, 24, 24), 4, 4, 3),      # four shells, odd link cell
+    (1, (16, 16, 16), 16, 5, 4),     # 78 neighbours, 16 species
+])
+def test_sub_warp_tile_layout_is_a_valid_one(lat, dims, n_sp, n_shells, w):
+    """The layout group_tune_layout() picks on the host: every site of the (w + 2H)^3 tile gets an integral byte
+    index of its own inside the tile, every neighbour sits in exactly one (lane, visit) slot, and the steps fit
+    the 16 bits they are stored in."""
+    from paper_2509_20949_b200.binding import group_layout
+    from pygeom import shells
+    L = group_layout(lattice=lat, dims=dims, n_species=n_sp, n_shells=n_shells, epi=make_epi(n_shells, n_sp, 300, 1),
+                     accept=make_accept_table(600), seed=1, link_cell=w, storage=smcx.STORAGE_U8)
+    assert L["lanes"] in (4, 8, 16, 32) and L["shift"] in (0, 1) and L["skew"] % 4 == 0
+    sh, _ = shells(lat, n_shells)
+    offs = np.concatenate(sh)                                              # (dx, dy, dz) per neighbour
+    ZT = len(offs)
+    slots = L["slots"]
+    used = slots[slots != 255]
+    assert sorted(used.tolist()) == list(range(ZT))
+    visits = -(-ZT // L["lanes"])
+    assert (slots[max(visits, 2 if visits <= 2 else 3 if visits <= 3 else 6 if visits <= 6 else visits) * L["lanes"]:] == 255).all()
+    reach0 = np.abs(sh[0]).max()
+    reach = np.abs(offs).max()
+    H = (reach0 + reach + 1) // 2
+    TW = w + 2 * H
+    basis = [(0, 0, 0), (1, 1, 1)] if lat == 0 else [(0, 0, 0), (0, 1, 1), (1, 0, 1), (1, 1, 0)]
+    t = np.arange(TW)
+    tz, ty, tx = np.meshgrid(t, t, t, indexing="ij")
+    idx = []
+    for (bx, by, bz) in basis:
+        num = (2 * tx + bx) + L["A"] * (2 * ty + by) + L["B"] * (2 * tz + bz)
+        assert (num % (1 << L["shift"]) == 0).all()
+        idx.append((num >> L["shift"]).ravel())
+    idx = np.concatenate(idx)
+    assert idx.min() >= 0 and idx.max() < L["tile_bytes"] and len(np.unique(idx)) == idx.size
+    steps = (offs[:, 0] + L["A"] * offs[:, 1] + L["B"] * offs[:, 2])
+    assert (steps % (1 << L["shift"]) == 0).all() and np.abs(steps >> L["shift"]).max() < 32768
