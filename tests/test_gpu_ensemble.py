@@ -135,3 +135,24 @@ def test_ensemble_argument_checks():
         smcx.Ensemble(cfg.lattice, cfg.dims, cfg.n_species, cfg.n_shells, cfg.epi(), [600], [t], [1], 1)
     with pytest.raises(smcx.SmcxError):
         smcx.Ensemble(cfg.lattice, cfg.dims, cfg.n_species, cfg.n_shells, cfg.epi(), [600, 0], [t, t], [1, 2], 1)
+
+
+@pytest.mark.skipif(not __import__("os").environ.get("SMCX_SLOW"), reason="long run; set SMCX_SLOW=1")
+def test_long_exchange_run_slow():
+    """Eight replicas, 300 graph-replayed rounds of (2 sweeps + exchange): slots, counters, energies and species
+    against the oracle at the end (dozens of accepted exchanges in between)."""
+    cfg = scaled_config(1, (16, 16, 16))
+    kTs = replica_ladder(600, 8, cfg.n_sites, 25.0 * np.sqrt(cfg.n_sites))
+    seeds = [500 + r for r in range(8)]
+    g, reps, tables = _ensemble(cfg, kTs, seeds, 2024, smcx.KERNEL_AUTO)
+    for o in reps:
+        o.tag = reps.index(o)
+    g.run(300, 2)
+    n_acc = np.zeros(7, dtype=np.int64)
+    for rnd in range(300):
+        for o in reps:
+            o.sweep(2)
+        n_acc += np.array(oracle.replica_exchange(reps, kTs, tables, rnd & 1, 2024, rnd))
+    st = _assert_slots_equal(g, reps, [o.tag for o in reps])
+    assert st["accepted"].tolist() == n_acc.tolist() and n_acc.sum() > 30
+    g.close()
