@@ -14,6 +14,8 @@
 #include <string>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>   // header-only; ranges cost nothing without a profiler attached
+
 #include "ensemble_kernels.cuh"
 #include "lattice_kernels.cuh"
 #include "smcx_common.cuh"
@@ -437,12 +439,18 @@ int launch_colour_pass(smcx* h, int colour) {
 
 // One sweep on h->stream: 8 colour passes and the trace/counter epilogue.
 int enqueue_sweep(smcx* h) {
+  static const char* const kPassName[8] = {"smcx colour 0", "smcx colour 1", "smcx colour 2", "smcx colour 3",
+                                           "smcx colour 4", "smcx colour 5", "smcx colour 6", "smcx colour 7"};
+  nvtxRangePushA("smcx sweep");
   for (int colour = 0; colour < 8; ++colour) {
+    nvtxRangePushA(kPassName[colour]);
     const int rc = launch_colour_pass(h, colour);
-    if (rc != SMCX_OK) return rc;
+    nvtxRangePop();
+    if (rc != SMCX_OK) { nvtxRangePop(); return rc; }
   }
   sweep_epilogue<<<1, 1, 0, h->stream>>>(h->d_state(), h->d_trace(), h->plan.G.trace_capacity);
   h->launches++;
+  nvtxRangePop();
   return SMCX_OK;
 }
 
