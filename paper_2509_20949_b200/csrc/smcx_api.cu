@@ -223,6 +223,15 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     const int v = std::atoi(env);
     if ((v == 4 || v == 8 || v == 16 || v == 32) && group_smem_layout(G, v, 2).total <= 227 * 1024) plan->group_lanes = v;
   }
+  {
+    long long max_d = 0;   // largest |V_s(b,x) - V_s(a,x)|
+    for (int s = 0; s < p->n_shells; ++s)
+      for (int a = 0; a < n; ++a)
+        for (int b = 0; b < n; ++b)
+          for (int x = 0; x < n; ++x)
+            max_d = std::max(max_d, std::llabs((long long)p->epi[(s * n + b) * n + x] - (long long)p->epi[(s * n + a) * n + x]));
+    G.gd16 = max_d <= 32767 ? 1 : 0;
+  }
   group_tune_layout(G, plan->group_lanes);
   if (kernel == SMCX_KERNEL_GROUP_PER_CELL && group_smem_layout(G, plan->group_lanes, 2).total > 227 * 1024)
     return SMCX_E_LINK_CELL_TOO_SMALL;

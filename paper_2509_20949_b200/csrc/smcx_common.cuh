@@ -108,6 +108,7 @@ struct Geom {
   unsigned char gslot[kMaxGroupSlots];
   int gA, gB, gtile;
   short gshift, gskew;
+  int gd16;   // every difference V_s(b,x) - V_s(a,x) fits a signed 16-bit word (table of the sub-warp kernel)
 };
 
 }  // namespace smcxk

@@ -210,7 +210,8 @@ inline void group_tune_layout(Geom& G, int lanes) {
 
 struct GroupSmem {
   int d_stride;        // ints per ordered pair in the difference table
-  int d_copies;        // 2: every 32-word stripe holds the pair's row twice, cells with odd index in their warp read the upper half
+  int d_copies;        // 2: every 32-word stripe holds the pair's row twice, cells with odd index in their warp read the upper
+                       // half; 4: 16-bit rows, four per stripe (one per cell of a warp), corr in a table of its own
   int d_bytes, nb_bytes, filt_bytes, tile_bytes, total;
 };
 
@@ -222,9 +223,18 @@ inline GroupSmem group_smem_layout(const Geom& G, int lanes, int warps = kGroupW
   GroupSmem L;
   const int n = G.n_species;
   const int row = G.n_shells * n + 1;
-  if (lanes < 32 && row <= 16) { L.d_stride = 32; L.d_copies = 2; }
-  else { L.d_stride = row | 1; L.d_copies = 1; }
-  L.d_bytes = (n * n * L.d_stride * 4 + 15) & ~15;
+  if (lanes == 8 && G.gd16 && row - 1 <= 16) {
+    // four cells per warp and differences that fit 16 bits: rows of 16 halfwords (8 words), one 8-bank window
+    // of every 32-word stripe per cell of the warp, so that the four rows a warp reads at the same time never
+    // share a bank (ncu, FCC 256^3, 8 lanes, doubled 32-bit rows: 1.87 wavefronts per table load); corr(a,b)
+    // stays 32-bit in a table of its own behind the stripes
+    L.d_stride = 32; L.d_copies = 4;
+    L.d_bytes = ((n * n * 32 + n * n) * 4 + 15) & ~15;
+  } else {
+    if (lanes < 32 && row <= 16) { L.d_stride = 32; L.d_copies = 2; }
+    else { L.d_stride = row | 1; L.d_copies = 1; }
+    L.d_bytes = (n * n * L.d_stride * 4 + 15) & ~15;
+  }
   L.nb_bytes = (G.ZT * 4 + 15) & ~15;     // per neighbour: (step & 0xffff) | row << 16
   L.tile_bytes = G.gtile + G.gskew;
   const int cells_per_block = warps * (32 / lanes);
@@ -255,7 +265,7 @@ template <int B, int L, int NIT>
 __global__ void __launch_bounds__(kGroupWarpsPerBlock * 32)
 sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t* __restrict__ epi,
                      const uint32_t* __restrict__ accept, const uint32_t* __restrict__ filt, DevState* __restrict__ st,
-                     int colour, int d_stride, int d_bytes, int nb_bytes, int tile_bytes) {
+                     int colour, int d_stride, int d_copies, int d_bytes, int nb_bytes, int tile_bytes) {
   constexpr int CPW = 32 / L;                                   // cells per warp
   extern __shared__ __align__(16) unsigned char smem[];
   int32_t* s_D = reinterpret_cast<int32_t*>(smem);              // [a * n + b][d_stride]
@@ -270,9 +280,22 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   const int n = G.n_species, ZT = G.ZT;
   const int corr_at = G.n_shells * n;
   const int n_empty = (NIT > 0 ? NIT : (ZT + L - 1) / L) * L - ZT;   // neighbour slots without a neighbour
-  const bool d_twice = L < 32 && d_stride == 32;                // see group_smem_layout
-  for (int k = threadIdx.x; k < n * n * d_stride; k += blockDim.x) {
-    const int pair = k / d_stride, e = d_twice ? ((k % d_stride) & 15) : k % d_stride;
+  const bool d_twice = d_copies == 2, d_half = L == 8 && d_copies == 4;   // see group_smem_layout (d_half: 8 lanes only, compile-time false elsewhere)
+  if (d_half) {
+    short* s_D16 = reinterpret_cast<short*>(s_D);
+    for (int k = threadIdx.x; k < n * n * 64; k += blockDim.x) {
+      const int pair = k >> 6, e = k & 15;
+      const int a = pair / n, b = pair % n;
+      int v = 0;
+      if (e < corr_at) {
+        const int s = e / n, x = e % n;
+        v = epi[(s * n + b) * n + x] - epi[(s * n + a) * n + x];
+      }
+      s_D16[k] = (short)v;
+    }
+  }
+  for (int k = threadIdx.x; k < (d_half ? n * n : n * n * d_stride); k += blockDim.x) {
+    const int pair = d_half ? k : k / d_stride, e = d_half ? corr_at : (d_twice ? ((k % d_stride) & 15) : k % d_stride);
     const int a = pair / n, b = pair % n;
     int v = 0;
     if (e < corr_at) {
@@ -283,9 +306,10 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
       v = 2 * epi[a * n + b] - epi[a * n + a] - epi[b * n + b] -
           n_empty * ((epi[b * n + a] - epi[a * n + a]) - (epi[b * n + b] - epi[a * n + b]));
     }
-    s_D[k] = v;
+    s_D[d_half ? n * n * 32 + k : k] = v;
   }
   const int32_t* s_Dg = s_D + (d_twice ? (grp & 1) * 16 : 0);   // this cell's half of the stripes
+  const short* s_Dh = reinterpret_cast<const short*>(s_D) + grp * 16;   // d_half: this cell's window
   if (G.filter_E >= 0)
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
   const int cA = G.gA, cB = G.gB, csh = G.gshift;
@@ -383,12 +407,15 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
             const int sa = *p_i, sb = *p_j;
             // a5: partial sums over this lane's neighbours of i (a -> b) and of j (b -> a); a trial between
             // equal species runs through the same code (its row of D is all zeros) and is masked below
-            const int32_t* Drow = s_Dg + (sa * n + sb) * d_stride;
+            const int pair = sa * n + sb;
+            const int32_t* Drow = s_Dg + pair * d_stride;
+            const short* Dh = s_Dh + pair * 64;
             int part = 0;
             if (NIT > 0) {
 #pragma unroll
               for (int it = 0; it < NIT; ++it)
-                part += Drow[nrow[it] + p_i[nstep[it]]] - Drow[nrow[it] + p_j[nstep[it]]];
+                part += d_half ? (int)Dh[nrow[it] + p_i[nstep[it]]] - (int)Dh[nrow[it] + p_j[nstep[it]]]
+                               : Drow[nrow[it] + p_i[nstep[it]]] - Drow[nrow[it] + p_j[nstep[it]]];
             } else {
 #pragma unroll 2
               for (int it = 0; it < nit; ++it) {
@@ -396,7 +423,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
                 const bool valid = mm != 255;
                 const uint32_t e = s_nb[valid ? mm : 0];
                 const int step = valid ? (int)(short)(e & 0xffffu) : 0, row = valid ? (int)(e >> 16) : 0;
-                part += Drow[row + p_i[step]] - Drow[row + p_j[step]];
+                part += d_half ? (int)Dh[row + p_i[step]] - (int)Dh[row + p_j[step]] : Drow[row + p_i[step]] - Drow[row + p_j[step]];
               }
             }
             // sum over the lanes of the group: one REDUX for a whole warp; a shuffle tree for smaller groups
@@ -407,7 +434,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
 #pragma unroll
               for (int o = L >> 1; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o, L);
             }
-            const int dE = part + Drow[corr_at];
+            const int dE = part + (d_half ? s_D[n * n * 32 + pair] : Drow[corr_at]);
             // a6: Eq. 3 in integer form.  ta <= T[dE] <= ta + E (host-verified); dE <= 0 maps to entry 0.
             bool ok;
             if (filter_E >= 0) {
@@ -522,7 +549,7 @@ inline void launch_group_per_cell(const Geom& G, int lanes, uint8_t* species, co
   const int nt = warps * 32;
   const int nit = group_nit(G, lanes);
   SMCX_GROUP_DISPATCH(G.B, lanes, nit, {
-    sweep_group_per_cell<B_, L_, N_><<<grid, nt, S.total, stream>>>(G, species, epi, accept, filt, st, colour, S.d_stride,
+    sweep_group_per_cell<B_, L_, N_><<<grid, nt, S.total, stream>>>(G, species, epi, accept, filt, st, colour, S.d_stride, S.d_copies,
                                                                      S.d_bytes, S.nb_bytes, S.tile_bytes);
   })
 }

@@ -413,3 +413,22 @@ def test_checkpoint_and_resume_in_a_new_handle(kernel):
     o.sweep(5)
     _assert_same_state(b, o)
     assert (b.energy_trace(4, 5) == o.energy_trace(4, 5)).all()
+
+
+@pytest.mark.parametrize("lanes", [8, 16, 32])
+@pytest.mark.parametrize("amplitude,kT", [(400, 690), (30_000, 20_000)], ids=["d16", "d32"])
+def test_sub_warp_kernel_table_formats(lanes, amplitude, kT, monkeypatch):
+    """FCC, 5 species, 3 shells with differences that fit 16 bits (8 lanes: halfword rows, one bank window per
+    cell of the warp) and with differences that do not (32-bit rows everywhere), for every lane count."""
+    monkeypatch.setenv("SMCX_GROUP_LANES", str(lanes))
+    lat, dims, n_sp, n_sh, w, seed = 1, (16, 16, 8), 5, 3, 4, 91
+    epi = make_epi(n_sh, n_sp, amplitude, seed)
+    assert (np.abs(epi).max() * 2 > 32767) == (amplitude > 16384)
+    table = make_accept_table(kT)
+    g = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, seed, link_cell=w, kT_units=kT, kernel=smcx.KERNEL_GROUP_PER_CELL)
+    o = oracle.Oracle(lat, dims, n_sp, n_sh, epi, w, table, seed)
+    g.sweep(4)
+    o.sweep(4)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all() and g.stats() == o.stats()
+    assert g.stats()[2] > 0
