@@ -32,6 +32,9 @@
 
 namespace smcxk {
 
+#ifndef SMCX_GROUP_REDUX_MIN_LANES
+#define SMCX_GROUP_REDUX_MIN_LANES 16   // measured: 16 lanes 0.866 -> 0.772 ms per sweep of FCC 128^3, 8 lanes 0.949 -> 1.003
+#endif
 constexpr int kGroupWarpsPerBlock = 8;    // at most; group_warps_per_block() picks fewer when that lets more blocks share an SM
 // Tile layout in shared memory: the species of the site at position (px, py, pz) (units of a/2, tile-relative)
 // is the byte at index (px + A py + B pz) >> shift.  The index is LINEAR in the position, so the step to
@@ -430,6 +433,16 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
             // (a REDUX per member mask was measured slower: FCC 128^3, 8 lanes, 1.49 against 1.26 ms per sweep)
             if (L == 32) {
               part = __reduce_add_sync(0xffffffffu, part);
+            } else if (L >= SMCX_GROUP_REDUX_MIN_LANES) {
+              // one whole-warp REDUX per cell of the warp, the other cells' lanes contributing 0: CPW independent
+              // instructions instead of a chain of log2(L) shuffles and adds
+              int sum = 0;
+#pragma unroll
+              for (int c = 0; c < CPW; ++c) {
+                const int r = __reduce_add_sync(0xffffffffu, grp == c ? part : 0);
+                sum = grp == c ? r : sum;
+              }
+              part = sum;
             } else {
 #pragma unroll
               for (int o = L >> 1; o > 0; o >>= 1) part += __shfl_xor_sync(0xffffffffu, part, o, L);
