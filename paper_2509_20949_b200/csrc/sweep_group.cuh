@@ -387,14 +387,16 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     const int filter_E = G.filter_E;
     uint32_t r_u_even = 0, r_u_odd = 0;
     int r_step_even = 0, r_step_odd = 0;
-    int k = 0;
+    int kc = 0;   // conventional cells of the link cell done so far: slot k = kc * B + b, so k & 1 = b & 1 at compile time
     for (int lz = 0; lz < w; ++lz)
       for (int ly = 0; ly < w; ++ly)
         for (int lx = 0; lx < w; ++lx) {
           const int conv = group_index(2 * (lx + H), 2 * (ly + H), 2 * (lz + H), cA, cB, csh);   // position (0,0,0) of the conventional cell
 #pragma unroll
-          for (int b = 0; b < B; ++b, ++k) {
-            if ((k & (2 * L - 1)) == 0) {  // a4: the L Philox calls of a group cover the next 2 L slots
+          for (int b = 0; b < B; ++b) {
+            const int k = kc * B + b;
+            // a4: the L Philox calls of a group cover the next 2 L slots (2 L is a multiple of B: only b == 0 can start a batch)
+            if ((2 * L) % B == 0 ? (b == 0 && (kc & (2 * L / B - 1)) == 0) : ((k & (2 * L - 1)) == 0)) {
               const Philox4 r = philox4x32_10(cell_id, (uint32_t)(k >> 1) + g, t, ctr3, G.key0, G.key1);
               // direction -> tile step of the partner, looked up here, off the chain of dependent trials
               r_step_even = (int)(short)(s_nb[mulhi_u32(r.x, (uint32_t)G.Z0)] & 0xffffu);
@@ -402,8 +404,8 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
               r_u_even = r.y; r_u_odd = r.w;
             }
             const int src = (k >> 1) & (L - 1);
-            const int step_j = __shfl_sync(0xffffffffu, (k & 1) ? r_step_odd : r_step_even, src, L);
-            const uint32_t u = __shfl_sync(0xffffffffu, (k & 1) ? r_u_odd : r_u_even, src, L);
+            const int step_j = __shfl_sync(0xffffffffu, (b & 1) ? r_step_odd : r_step_even, src, L);
+            const uint32_t u = __shfl_sync(0xffffffffu, (b & 1) ? r_u_odd : r_u_even, src, L);
             const unsigned char* p_i = tile + conv + group_index(group_basis_pos<B>(b, 0), group_basis_pos<B>(b, 1),
                                                                  group_basis_pos<B>(b, 2), cA, cB, csh);
             const unsigned char* p_j = p_i + step_j;
@@ -470,6 +472,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
             }
             __syncwarp();
           }
+          ++kc;
         }
   }
   if (active) {
