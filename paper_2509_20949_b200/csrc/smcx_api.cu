@@ -79,7 +79,7 @@ inline int floor_div2(int v) { return v >= 0 ? v / 2 : -((-v + 1) / 2); }
 inline bool is_thread_kernel(int k) { return k == SMCX_KERNEL_THREAD_PER_CELL || k == SMCX_KERNEL_THREAD_PERSISTENT; }
 
 struct Layout {
-  size_t species, epi, coef, accept, filter, trace, state, counts, total;
+  size_t species, epi, coef, gtable, accept, filter, trace, state, counts, total;
 };
 
 struct Plan {
@@ -242,6 +242,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   off += align_up(storage == SMCX_STORAGE_U8 ? (size_t)n_sites : (size_t)((n_sites + 15) / 16) * 4, 256);
   L.epi = off;     off += align_up((size_t)p->n_shells * n * n * sizeof(int32_t), 256);
   L.coef = off;    off += align_up((size_t)16 * (kCoefInts + 4) * sizeof(int32_t), 256);
+  L.gtable = off;  off += align_up((size_t)group_smem_layout(G, plan->group_lanes).d_bytes, 256);   // sub-warp kernel's difference table
   L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
   L.filter = off;  off += align_up((size_t)kFilterWords * sizeof(uint32_t), 256);
   L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
@@ -286,6 +287,7 @@ struct smcx {
   uint8_t* d_species() const { return reinterpret_cast<uint8_t*>(ws + plan.lay.species); }
   int32_t* d_epi() const { return reinterpret_cast<int32_t*>(ws + plan.lay.epi); }
   int32_t* d_coef() const { return reinterpret_cast<int32_t*>(ws + plan.lay.coef); }
+  int32_t* d_gtable() const { return reinterpret_cast<int32_t*>(ws + plan.lay.gtable); }
   uint32_t* d_accept() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.accept); }
   uint32_t* d_filter() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.filter); }
   long long* d_trace() const { return reinterpret_cast<long long*>(ws + plan.lay.trace); }
@@ -429,7 +431,7 @@ int launch_colour_pass(smcx* h, int colour) {
     return SMCX_OK;
   }
   if (P.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
-    launch_group_per_cell(G, P.group_lanes, h->d_species(), h->d_epi(), h->d_accept(), h->d_filter(), h->d_state(), colour, h->stream);
+    launch_group_per_cell(G, P.group_lanes, h->d_species(), h->d_gtable(), h->d_accept(), h->d_filter(), h->d_state(), colour, h->stream);
     h->launches++;
     return SMCX_OK;
   }
@@ -578,6 +580,11 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
       pack_thread_coefficients(coef, coef + 16 * kCoefInts);
     }
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_coef(), coef, sizeof(coef), cudaMemcpyHostToDevice, h->stream));
+    std::vector<int32_t> gtab;
+    if (h->plan.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
+      group_build_table(h->plan.G, h->plan.group_lanes, h->epi.data(), gtab);
+      SMCX_CUDA(h, cudaMemcpyAsync(h->d_gtable(), gtab.data(), gtab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+    }
     SMCX_CUDA(h, cudaMemsetAsync(h->d_trace(), 0, (size_t)h->plan.G.trace_capacity * sizeof(long long), h->stream));
     SMCX_CUDA(h, cudaStreamSynchronize(h->stream));  // &zero and epi must stay valid until copied
     int r = upload_table(h, p->accept, p->accept_len);

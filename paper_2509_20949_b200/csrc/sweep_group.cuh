@@ -246,6 +246,36 @@ inline GroupSmem group_smem_layout(const Geom& G, int lanes, int warps = kGroupW
   return L;
 }
 
+// The difference table of a handle in the layout group_smem_layout() describes, built once on the host:
+// D[(a,b)][s][x] = V_s(b,x) - V_s(a,x) and corr(a,b) = 2 V_0(a,b) - V_0(a,a) - V_0(b,b) less what the empty
+// neighbour slots add (each reads D_0(a) - D_0(b), see the kernel).
+inline void group_build_table(const Geom& G, int lanes, const int32_t* epi, std::vector<int32_t>& tab) {
+  const GroupSmem S = group_smem_layout(G, lanes);
+  const int n = G.n_species, corr_at = G.n_shells * n;
+  const int n_empty = group_visits(G, lanes) * lanes - G.ZT;
+  tab.assign((size_t)S.d_bytes / 4, 0);
+  auto D = [&](int s, int a, int b, int x) { return epi[(s * n + b) * n + x] - epi[(s * n + a) * n + x]; };
+  auto corr = [&](int a, int b) {
+    return 2 * epi[a * n + b] - epi[a * n + a] - epi[b * n + b] - n_empty * (D(0, a, b, a) - D(0, a, b, b));
+  };
+  for (int a = 0; a < n; ++a)
+    for (int b = 0; b < n; ++b) {
+      const int pair = a * n + b;
+      if (S.d_copies == 4) {                       // halfword rows, four windows of 16 per stripe; corr behind the stripes
+        int16_t* h = reinterpret_cast<int16_t*>(tab.data()) + (size_t)pair * 64;
+        for (int c = 0; c < 4; ++c)
+          for (int e = 0; e < corr_at; ++e) h[c * 16 + e] = (int16_t)D(e / n, a, b, e % n);
+        tab[(size_t)n * n * 32 + pair] = corr(a, b);
+      } else {
+        int32_t* r = tab.data() + (size_t)pair * S.d_stride;
+        for (int c = 0; c < (S.d_copies == 2 ? 2 : 1); ++c) {
+          for (int e = 0; e < corr_at; ++e) r[c * 16 + e] = D(e / n, a, b, e % n);
+          r[c * 16 + corr_at] = corr(a, b);
+        }
+      }
+    }
+}
+
 // basis position (units of a/2) of basis index b along axis a (0 = x, 1 = y, 2 = z); S0
 template <int B>
 __device__ __forceinline__ int group_basis_pos(int b, int a) {
@@ -266,7 +296,7 @@ __device__ __forceinline__ void group_split_index(int idx, int TW, float inv_TW,
 // ceil(ZT / L); surplus visits are compensated in corr, see above).  NIT == 0: any ZT, steps from shared memory.
 template <int B, int L, int NIT>
 __global__ void __launch_bounds__(kGroupWarpsPerBlock * 32)
-sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t* __restrict__ epi,
+sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t* __restrict__ table,
                      const uint32_t* __restrict__ accept, const uint32_t* __restrict__ filt, DevState* __restrict__ st,
                      int colour, int d_stride, int d_copies, int d_bytes, int nb_bytes, int tile_bytes) {
   constexpr int CPW = 32 / L;                                   // cells per warp
@@ -282,35 +312,9 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
 
   const int n = G.n_species, ZT = G.ZT;
   const int corr_at = G.n_shells * n;
-  const int n_empty = (NIT > 0 ? NIT : (ZT + L - 1) / L) * L - ZT;   // neighbour slots without a neighbour
   const bool d_twice = d_copies == 2, d_half = L == 8 && d_copies == 4;   // see group_smem_layout (d_half: 8 lanes only, compile-time false elsewhere)
-  if (d_half) {
-    short* s_D16 = reinterpret_cast<short*>(s_D);
-    for (int k = threadIdx.x; k < n * n * 64; k += blockDim.x) {
-      const int pair = k >> 6, e = k & 15;
-      const int a = pair / n, b = pair % n;
-      int v = 0;
-      if (e < corr_at) {
-        const int s = e / n, x = e % n;
-        v = epi[(s * n + b) * n + x] - epi[(s * n + a) * n + x];
-      }
-      s_D16[k] = (short)v;
-    }
-  }
-  for (int k = threadIdx.x; k < (d_half ? n * n : n * n * d_stride); k += blockDim.x) {
-    const int pair = d_half ? k : k / d_stride, e = d_half ? corr_at : (d_twice ? ((k % d_stride) & 15) : k % d_stride);
-    const int a = pair / n, b = pair % n;
-    int v = 0;
-    if (e < corr_at) {
-      const int s = e / n, x = e % n;
-      v = epi[(s * n + b) * n + x] - epi[(s * n + a) * n + x];
-    } else if (e == corr_at) {
-      // corr(a,b), less what the empty slots add: each reads D_0(sigma_i) - D_0(sigma_j) = D_0(a) - D_0(b)
-      v = 2 * epi[a * n + b] - epi[a * n + a] - epi[b * n + b] -
-          n_empty * ((epi[b * n + a] - epi[a * n + a]) - (epi[b * n + b] - epi[a * n + b]));
-    }
-    s_D[d_half ? n * n * 32 + k : k] = v;
-  }
+  // the difference table comes ready-made from the host (group_build_table): a plain copy
+  for (int k = threadIdx.x; k < d_bytes / 4; k += blockDim.x) s_D[k] = table[k];
   const int32_t* s_Dg = s_D + (d_twice ? (grp & 1) * 16 : 0);   // this cell's half of the stripes
   const short* s_Dh = reinterpret_cast<const short*>(s_D) + grp * 16;   // d_half: this cell's window
   if (G.filter_E >= 0)
@@ -556,7 +560,7 @@ inline cudaError_t configure_group_per_cell(const Geom& G, int lanes) {
   return e;
 }
 
-inline void launch_group_per_cell(const Geom& G, int lanes, uint8_t* species, const int32_t* epi, const uint32_t* accept,
+inline void launch_group_per_cell(const Geom& G, int lanes, uint8_t* species, const int32_t* table, const uint32_t* accept,
                                   const uint32_t* filt, DevState* st, int colour, cudaStream_t stream) {
   const int warps = group_warps_per_block(G, lanes);
   const GroupSmem S = group_smem_layout(G, lanes, warps);
@@ -565,7 +569,7 @@ inline void launch_group_per_cell(const Geom& G, int lanes, uint8_t* species, co
   const int nt = warps * 32;
   const int nit = group_nit(G, lanes);
   SMCX_GROUP_DISPATCH(G.B, lanes, nit, {
-    sweep_group_per_cell<B_, L_, N_><<<grid, nt, S.total, stream>>>(G, species, epi, accept, filt, st, colour, S.d_stride, S.d_copies,
+    sweep_group_per_cell<B_, L_, N_><<<grid, nt, S.total, stream>>>(G, species, table, accept, filt, st, colour, S.d_stride, S.d_copies,
                                                                      S.d_bytes, S.nb_bytes, S.tile_bytes);
   })
 }
