@@ -480,21 +480,45 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
         }
   }
   if (active) {
-    // a7: write back the sites a swap can have touched: positions within r0 of the cell
+    // a7: write back the sites a swap can have touched: positions within r0 of the cell.  Only the conventional
+    // cells that hold such a position are visited (6^3 of the 8^3 of the tile at w = 4), two per lane in flight.
     const int lo = 2 * H - G.r0, hi = 2 * (H + w) - 1 + G.r0;  // tile positions, inclusive
-    for (int idx = g; idx < n_conv; idx += L) {
-      int tx, ty, tz;
-      group_split_index(idx, TW, inv_TW, tx, ty, tz);
-      int gx = t0x + tx; if (gx >= G.Lx) gx -= G.Lx;
-      int gy = t0y + ty; if (gy >= G.Ly) gy -= G.Ly;
-      int gz = t0z + tz; if (gz >= G.Lz) gz -= G.Lz;
-      const long long gi = (((long long)gz * G.Ly + gy) * G.Lx + gx) * B;
+    const int c0 = lo >> 1, WB = (hi >> 1) - c0 + 1, n_wb = WB * WB * WB;
+    const float inv_WB = 1.0f / (float)WB;
+    for (int idx0 = g; idx0 < n_wb; idx0 += 2 * L) {
+      uint32_t val[2];
+      uint32_t keep[2];          // bit b: site b of the conventional cell lies in the written range
+      long long gi[2];
 #pragma unroll
-      for (int b = 0; b < B; ++b) {
-        const int px = 2 * tx + group_basis_pos<B>(b, 0), py = 2 * ty + group_basis_pos<B>(b, 1),
-                  pz = 2 * tz + group_basis_pos<B>(b, 2);
-        if (px >= lo && px <= hi && py >= lo && py <= hi && pz >= lo && pz <= hi)
-          species[gi + b] = tile[group_index(px, py, pz, cA, cB, csh)];
+      for (int q = 0; q < 2; ++q) {
+        const int idx = idx0 + q * L;
+        int tx, ty, tz;
+        group_split_index(idx < n_wb ? idx : 0, WB, inv_WB, tx, ty, tz);
+        tx += c0; ty += c0; tz += c0;
+        int gx = t0x + tx; if (gx >= G.Lx) gx -= G.Lx;
+        int gy = t0y + ty; if (gy >= G.Ly) gy -= G.Ly;
+        int gz = t0z + tz; if (gz >= G.Lz) gz -= G.Lz;
+        gi[q] = (((long long)gz * G.Ly + gy) * G.Lx + gx) * B;
+        val[q] = 0; keep[q] = 0;
+#pragma unroll
+        for (int b = 0; b < B; ++b) {
+          const int px = 2 * tx + group_basis_pos<B>(b, 0), py = 2 * ty + group_basis_pos<B>(b, 1),
+                    pz = 2 * tz + group_basis_pos<B>(b, 2);
+          const bool in = idx < n_wb && px >= lo && px <= hi && py >= lo && py <= hi && pz >= lo && pz <= hi;
+          val[q] |= (uint32_t)tile[group_index(px, py, pz, cA, cB, csh)] << (8 * b);
+          keep[q] |= in ? 1u << b : 0u;
+        }
+      }
+#pragma unroll
+      for (int q = 0; q < 2; ++q) {
+        if (keep[q] == (1u << B) - 1u) {          // whole conventional cell: one store
+          if (B == 2) *reinterpret_cast<uint16_t*>(species + gi[q]) = (uint16_t)val[q];
+          else        *reinterpret_cast<uint32_t*>(species + gi[q]) = val[q];
+        } else {
+#pragma unroll
+          for (int b = 0; b < B; ++b)
+            if (keep[q] >> b & 1u) species[gi[q] + b] = (unsigned char)(val[q] >> (8 * b));
+        }
       }
     }
   }
