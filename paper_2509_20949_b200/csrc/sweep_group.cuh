@@ -352,13 +352,13 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     t0y = (oy + cy * w - H + G.Ly) % G.Ly;
     t0z = (oz + cz * w - H + G.Lz) % G.Lz;
   }
-  // a3: stage the tile, four conventional cells per lane in flight (a group without a cell stages species
+  // a3: stage the tile, eight conventional cells per lane in flight (a group without a cell stages species
   // 0 everywhere: all its trials are no-ops)
-  for (int idx0 = g; idx0 < n_conv; idx0 += 4 * L) {
-    uint32_t v[4];
-    int at[4];
+  for (int idx0 = g; idx0 < n_conv; idx0 += 8 * L) {
+    uint32_t v[8];
+    int at[8];
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < 8; ++q) {
       const int idx = idx0 + q * L;
       int tx, ty, tz;
       group_split_index(idx, TW, inv_TW, tx, ty, tz);
@@ -373,7 +373,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
       }
     }
 #pragma unroll
-    for (int q = 0; q < 4; ++q) {
+    for (int q = 0; q < 8; ++q) {
       if (at[q] < 0) continue;
       unsigned char* dst = tile + at[q];
 #pragma unroll
