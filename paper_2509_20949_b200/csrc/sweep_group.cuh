@@ -314,11 +314,14 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   const int corr_at = G.n_shells * n;
   const bool d_twice = d_copies == 2, d_half = L == 8 && d_copies == 4;   // see group_smem_layout (d_half: 8 lanes only, compile-time false elsewhere)
   // the difference table comes ready-made from the host (group_build_table): a plain copy
+#pragma unroll 4
   for (int k = threadIdx.x; k < d_bytes / 4; k += blockDim.x) s_D[k] = table[k];
   const int32_t* s_Dg = s_D + (d_twice ? (grp & 1) * 16 : 0);   // this cell's half of the stripes
   const short* s_Dh = reinterpret_cast<const short*>(s_D) + grp * 16;   // d_half: this cell's window
-  if (G.filter_E >= 0)
+  if (G.filter_E >= 0) {
+#pragma unroll 5
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
+  }
   const int cA = G.gA, cB = G.gB, csh = G.gshift;
   for (int k = threadIdx.x; k < ZT; k += blockDim.x) {
     const int step = group_index(G.off[k][0], G.off[k][1], G.off[k][2], cA, cB, csh);
