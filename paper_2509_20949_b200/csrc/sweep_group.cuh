@@ -10,10 +10,12 @@
 //    below), so the tile-index step to neighbour m is the same for every site whatever its basis: lane g
 //    keeps the steps and the table rows of its neighbours (slots g, g + L, ... of G.gslot) in registers,
 //    and a neighbour visit is one add, the species load, one add and the load of
-//    D[(a,b)][s][x] = V_s(b,x) - V_s(a,x) from a table built in shared memory when the block starts.
+//    D[(a,b)][s][x] = V_s(b,x) - V_s(a,x) from a table the host builds once (group_build_table) and every
+//    block copies into shared memory.
 //    The sums over the neighbours of i and of j both include the i-j bond;
 //    corr(a,b) = 2 V_0(a,b) - V_0(a,a) - V_0(b,b) takes it out again (exact integer identity);
-//  * one xor-shuffle tree over the group (one REDUX when the group is a whole warp) sums the partial dE;
+//  * the partial dE of the lanes are summed by one whole-warp REDUX per cell of the warp with 16 or 32 lanes
+//    (the other cells' lanes contribute 0), by an xor-shuffle tree with fewer;
 //  * Philox: lane g of a group computes the call of slot pair q0 + g, so a group draws 2 L slots at a
 //    time, looks the tile step of the drawn direction up right away (off the chain of dependent trials)
 //    and hands step and acceptance draw round with group-wide shuffles;
