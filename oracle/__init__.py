@@ -28,7 +28,7 @@ def build(force: bool = False) -> str:
         if force or stale:
             tmp = _LIB + f".tmp{os.getpid()}"
             subprocess.check_call(
-                ["g++", "-O2", "-std=c++17", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC])
+                ["g++", "-O2", "-std=c++17", "-fopenmp", "-fPIC", "-shared", "-Wall", "-Wextra", "-o", tmp, _SRC])
             os.replace(tmp, _LIB)
     return _LIB
 
@@ -60,6 +60,7 @@ def _load():
         "oracle_lc_valid": (C.c_int, [C.c_void_p]),
         "oracle_sweep_lc": (C.c_int, [C.c_void_p, C.c_int64, C.c_int, C.c_uint32]),
         "oracle_sweep_seq": (None, [C.c_void_p, C.c_int64]),
+        "oracle_set_threads": (C.c_int, [C.c_void_p, C.c_int]),
         "oracle_shift": (None, [C.c_void_p, C.c_uint32, i32p]),
         "oracle_stats": (None, [C.c_void_p, i64p, i64p, i64p]),
         "oracle_trace": (C.c_int64, [C.c_void_p, C.c_int64, C.c_int64, i64p]),
@@ -141,7 +142,7 @@ class Oracle:
     """One lattice + schedule state.  Method names follow include/smcx.h where they overlap."""
 
     def __init__(self, lattice, dims, n_species, n_shells, epi, link_cell, accept, seed,
-                 init: bool = True):
+                 init: bool = True, threads: int = 1):
         lib = _load()
         self._lib = lib
         self.lattice, self.dims = int(lattice), tuple(int(d) for d in dims)
@@ -156,15 +157,22 @@ class Oracle:
         if not self._h:
             raise ValueError("oracle_create rejected the parameters")
         self.n_sites = int(lib.oracle_n_sites(self._h))
+        self.threads = int(lib.oracle_set_threads(self._h, int(threads)))
         if init:
             lib.oracle_init_species(self._h)
 
     @classmethod
-    def from_config(cls, cfg, init: bool = True, **over):
+    def from_config(cls, cfg, init: bool = True, threads: int = 1, **over):
         kw = dict(lattice=cfg.lattice, dims=cfg.dims, n_species=cfg.n_species, n_shells=cfg.n_shells,
                   epi=cfg.epi(), link_cell=cfg.link_cell, accept=cfg.accept_table(0), seed=cfg.seed)
         kw.update(over)
-        return cls(init=init, **kw)
+        return cls(init=init, threads=threads, **kw)
+
+    def set_threads(self, n: int) -> int:
+        """OpenMP threads over the cells of a colour (and over sites in the init / energy / pair-count
+        loops); 1 = the plain single-threaded loops.  Results never depend on it (pinned)."""
+        self.threads = int(self._lib.oracle_set_threads(self._h, int(n)))
+        return self.threads
 
     def close(self):
         if getattr(self, "_h", None):

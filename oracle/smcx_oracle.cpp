@@ -25,6 +25,11 @@
 // numbers; closed-form energies (single species, B2); dE against full recomputation;
 // conservation; energy bookkeeping; order independence of same-colour cells and its failure
 // for w=1; exact Boltzmann histogram on 16 sites; B2 SRO values and sum rules.
+// Threads: single-threaded unless oracle_set_threads(n > 1) is called; then the cells of one colour
+// (which commute, pin P7; the paper's own CPU mapping spreads link cells over OpenMP threads,
+// PAPER.md:114) are spread over n OpenMP threads, each with its own tally of trials / accepted / sum dE
+// added up after the loop.  Same arithmetic, same order inside a cell; pinned bit for bit against the
+// one-thread run (tests/test_oracle_schedule.py).
 // Parity unpinned: the authors' own trajectories and Fig. 6 curves (their EPI values and
 // code are not available).
 #include <algorithm>
@@ -90,6 +95,13 @@ struct Oracle {
   bool E_valid = false;
   std::vector<int64_t> trace;           // E_run after each sweep, from sweep trace_first on
   int64_t trace_first = 0;              // resume (checkpointing): the sweep counter was set to this value
+  int threads = 1;                      // OpenMP threads over the cells of a colour (1 = plain loop)
+};
+
+// What a run of trials adds to the bookkeeping; one per thread when the cells of a colour are spread
+// over threads, summed into the Oracle after the loop.
+struct Tally {
+  int64_t trials = 0, accepted = 0, dE = 0;
 };
 
 // S0: basis positions in half-lattice units.
@@ -196,6 +208,8 @@ int64_t total_energy(const Oracle& o) {
   for (int s = 0; s < o.n_shells; ++s)
     for (const Vec3& d : o.shell[s]) {
       if (!in_positive_half(d)) continue;
+      // an exact integer sum over sites: the threads' partial sums add up to the same H
+#pragma omp parallel for reduction(+ : H) schedule(static) num_threads(o.threads) if (o.threads > 1)
       for (int64_t i = 0; i < o.N; ++i) H += V(o, s, o.sigma[i], o.sigma[neighbour(o, i, d)]);
     }
   return H;
@@ -246,11 +260,11 @@ int64_t swap_delta(Oracle& o, int64_t i, int64_t j) {
 }
 
 // S4: one trial with primary site i, direction word w_dir and acceptance word u.
-void trial(Oracle& o, int64_t i, uint32_t w_dir, uint32_t u) {
+void trial(Oracle& o, Tally& tally, int64_t i, uint32_t w_dir, uint32_t u) {
   const std::vector<Vec3>& nn = o.shell[0];
   const uint32_t dir = mulhi32(w_dir, (uint32_t)nn.size());
   const int64_t j = neighbour(o, i, nn[dir]);
-  o.trials++;
+  tally.trials++;
   if (o.count_visits) o.visits[i]++;
   const uint8_t a = o.sigma[i], b = o.sigma[j];
   if (a == b) return;  // Q8: same species, nothing changes
@@ -259,15 +273,51 @@ void trial(Oracle& o, int64_t i, uint32_t w_dir, uint32_t u) {
   const bool ok = dE <= 0 || (dE < (int64_t)o.accept.size() && u < o.accept[(size_t)dE]);
   if (ok) {
     std::swap(o.sigma[i], o.sigma[j]);
-    o.E_run += dE;
-    o.accepted++;
+    tally.dE += dE;
+    tally.accepted++;
   }
+}
+
+void add_tally(Oracle& o, const Tally& tally) {
+  o.trials += tally.trials;
+  o.accepted += tally.accepted;
+  o.E_run += tally.dE;
 }
 
 void ensure_energy(Oracle& o) {
   if (!o.E_valid) {
     o.E_run = total_energy(o);
     o.E_valid = true;
+  }
+}
+
+// S3.2 + S4: the S = w^3 B trials of one link cell, slot by slot.
+void run_cell(Oracle& o, Tally& tally, uint32_t cell_id, int colour, uint32_t t, int ox, int oy, int oz) {
+  const uint32_t key[2] = {(uint32_t)(o.seed & 0xffffffffu), (uint32_t)(o.seed >> 32)};
+  const int w = o.w;
+  const int ncx = o.L[0] / w, ncy = o.L[1] / w;
+  const int S = w * w * w * o.B;
+  const int cx = (int)(cell_id % (uint32_t)ncx);
+  const int cy = (int)((cell_id / (uint32_t)ncx) % (uint32_t)ncy);
+  const int cz = (int)(cell_id / (uint32_t)(ncx * ncy));
+  uint32_t r[4];
+  for (int k = 0; k < S; ++k) {
+    // S3.2: slot k -> local site ((lz*w + ly)*w + lx)*B + b.
+    const int b = k % o.B;
+    int rest = k / o.B;
+    const int lx = rest % w; rest /= w;
+    const int ly = rest % w; rest /= w;
+    const int lz = rest;
+    const int x = (ox + cx * w + lx) % o.L[0];
+    const int y = (oy + cy * w + ly) % o.L[1];
+    const int z = (oz + cz * w + lz) % o.L[2];
+    const int64_t i = (((int64_t)z * o.L[1] + y) * o.L[0] + x) * o.B + b;
+    // S4: one Philox call serves two consecutive slots.
+    const uint32_t q = (uint32_t)(k >> 1);
+    const uint32_t ct[4] = {cell_id, q, t, (uint32_t)TAG_TRIAL | ((uint32_t)colour << 8)};
+    philox4x32_10(ct, key, r);
+    if (k & 1) trial(o, tally, i, r[2], r[3]);
+    else       trial(o, tally, i, r[0], r[1]);
   }
 }
 
@@ -286,7 +336,6 @@ void sweep_lc(Oracle& o, int order_mode, uint32_t order_seed) {
   const int oy = (int)mulhi32(r[1], (uint32_t)w);
   const int oz = (int)mulhi32(r[2], (uint32_t)w);
   const int ncx = o.L[0] / w, ncy = o.L[1] / w, ncz = o.L[2] / w;
-  const int S = w * w * w * o.B;
   std::vector<uint32_t> cells;
   for (int colour = 0; colour < 8; ++colour) {
     // S2: cells of this colour.
@@ -301,29 +350,27 @@ void sweep_lc(Oracle& o, int order_mode, uint32_t order_seed) {
       std::mt19937 g(order_seed + (uint32_t)colour + 8u * t);
       std::shuffle(cells.begin(), cells.end(), g);
     }
-    for (uint32_t cell_id : cells) {
-      const int cx = (int)(cell_id % (uint32_t)ncx);
-      const int cy = (int)((cell_id / (uint32_t)ncx) % (uint32_t)ncy);
-      const int cz = (int)(cell_id / (uint32_t)(ncx * ncy));
-      for (int k = 0; k < S; ++k) {
-        // S3.2: slot k -> local site ((lz*w + ly)*w + lx)*B + b.
-        const int b = k % o.B;
-        int rest = k / o.B;
-        const int lx = rest % w; rest /= w;
-        const int ly = rest % w; rest /= w;
-        const int lz = rest;
-        const int x = (ox + cx * w + lx) % o.L[0];
-        const int y = (oy + cy * w + ly) % o.L[1];
-        const int z = (oz + cz * w + lz) % o.L[2];
-        const int64_t i = (((int64_t)z * o.L[1] + y) * o.L[0] + x) * o.B + b;
-        // S4: one Philox call serves two consecutive slots.
-        const uint32_t q = (uint32_t)(k >> 1);
-        const uint32_t ct[4] = {cell_id, q, t, (uint32_t)TAG_TRIAL | ((uint32_t)colour << 8)};
-        philox4x32_10(ct, key, r);
-        if (k & 1) trial(o, i, r[2], r[3]);
-        else       trial(o, i, r[0], r[1]);
+    // The cells of one colour, in the order of `cells`: a plain loop, or spread over o.threads OpenMP
+    // threads (same-colour cells touch disjoint sites, S2, so they commute: pin P7).
+    Tally total;
+    const int64_t n_cells = (int64_t)cells.size();
+    if (o.threads <= 1) {
+      for (int64_t c = 0; c < n_cells; ++c) run_cell(o, total, cells[(size_t)c], colour, t, ox, oy, oz);
+    } else {
+#ifdef _OPENMP
+#pragma omp parallel num_threads(o.threads)
+      {
+        Tally mine;
+#pragma omp for schedule(static)
+        for (int64_t c = 0; c < n_cells; ++c) run_cell(o, mine, cells[(size_t)c], colour, t, ox, oy, oz);
+#pragma omp critical
+        { total.trials += mine.trials; total.accepted += mine.accepted; total.dE += mine.dE; }
       }
+#else
+      for (int64_t c = 0; c < n_cells; ++c) run_cell(o, total, cells[(size_t)c], colour, t, ox, oy, oz);
+#endif
     }
+    add_tally(o, total);
   }
   // S3.3
   o.trace.push_back(o.E_run);
@@ -337,12 +384,14 @@ void sweep_seq(Oracle& o) {
   const uint32_t key[2] = {(uint32_t)(o.seed & 0xffffffffu), (uint32_t)(o.seed >> 32)};
   const uint32_t t = (uint32_t)o.sweeps_done;
   uint32_t r[4];
+  Tally tally;
   for (int64_t i = 0; i < o.N; ++i) {
     const uint32_t ct[4] = {(uint32_t)((uint64_t)i & 0xffffffffu), (uint32_t)((uint64_t)i >> 32), t,
                             (uint32_t)TAG_SEQ};
     philox4x32_10(ct, key, r);
-    trial(o, i, r[0], r[1]);
+    trial(o, tally, i, r[0], r[1]);
   }
+  add_tally(o, tally);
   o.trace.push_back(o.E_run);
   o.sweeps_done++;
 }
@@ -372,6 +421,7 @@ uint64_t feistel_permute(const Oracle& o, uint64_t v, int h) {
 void init_species(Oracle& o) {
   int h = 1;
   while ((1ull << (2 * h)) < (uint64_t)o.N) ++h;
+#pragma omp parallel for schedule(static) num_threads(o.threads) if (o.threads > 1)   // sites are independent
   for (int64_t i = 0; i < o.N; ++i)
     o.sigma[i] = (uint8_t)(feistel_permute(o, (uint64_t)i, h) % (uint64_t)o.n_species);
   o.E_valid = false;
@@ -390,6 +440,7 @@ bool init_composition(Oracle& o, const int64_t* counts) {
   if (sum != o.N) return false;
   int h = 1;
   while ((1ull << (2 * h)) < (uint64_t)o.N) ++h;
+#pragma omp parallel for schedule(static) num_threads(o.threads) if (o.threads > 1)   // sites are independent
   for (int64_t i = 0; i < o.N; ++i) {
     const int64_t r = (int64_t)feistel_permute(o, (uint64_t)i, h);
     int p = 0;
@@ -406,12 +457,16 @@ void pair_counts(const Oracle& o, int64_t* counts) {
   const int n = o.n_species;
   std::fill(counts, counts + (size_t)o.n_shells * n * n, (int64_t)0);
   for (int s = 0; s < o.n_shells; ++s)
-    for (const Vec3& d : o.shell[s])
+    for (const Vec3& d : o.shell[s]) {
+      int64_t* row = counts + (size_t)s * n * n;
+      // exact integer histogram: per-thread copies of the n x n counters are added up by the reduction
+#pragma omp parallel for reduction(+ : row[: n * n]) schedule(static) num_threads(o.threads) if (o.threads > 1)
       for (int64_t i = 0; i < o.N; ++i) {
         const int pc = o.sigma[i];
         const int pn = o.sigma[neighbour(o, i, d)];
-        counts[((size_t)s * n + pc) * n + pn]++;
+        row[(size_t)pc * n + pn]++;
       }
+    }
 }
 
 // Eq. 8: alpha_s^{pp'} = 1 - P_s(p | p') / c_p with
@@ -594,6 +649,19 @@ int oracle_sweep_lc(void* h, int64_t n, int order_mode, uint32_t order_seed) {
     if (o.L[a] % (2 * o.w)) return -1;
   for (int64_t s = 0; s < n; ++s) sweep_lc(o, order_mode, order_seed);
   return 0;
+}
+
+// Threads over the cells of a colour for the following oracle_sweep_lc calls (1 = plain loop).  Returns
+// the number that will be used: 1 when the library was built without OpenMP.
+int oracle_set_threads(void* h, int n) {
+  Oracle& o = *(Oracle*)h;
+#ifdef _OPENMP
+  o.threads = n < 1 ? 1 : n;
+#else
+  (void)n;
+  o.threads = 1;
+#endif
+  return o.threads;
 }
 
 void oracle_sweep_seq(void* h, int64_t n) {

@@ -214,3 +214,37 @@ def test_resume_from_a_checkpoint_is_exact():
     c.set_sweep_counter(t + 1)
     c.sweep(3)
     assert (a.species() != c.species()).any()
+
+
+@pytest.mark.parametrize("cfg_id,dims,threads", [(1, (16, 16, 16), 2), (1, (24, 16, 32), 5), (3, (16, 8, 16), 4),
+                                                 (3, (8, 8, 8), 16)])
+def test_p7_threads_over_the_cells_of_a_colour_change_nothing(cfg_id, dims, threads):
+    """Multi-thread twin of P7 (the OpenMP pragma on the per-colour cell loop "must reproduce
+    the 1-thread result bit for bit"): initial state, species after every sweep, trace, counters, visit counts,
+    recomputed energy and pair counts are those of the plain loop, also with more threads than cells of a colour
+    (FCC 8^3 has one) and with the shuffled cell order."""
+    cfg = scaled_config(cfg_id, dims)
+    one = oracle.Oracle.from_config(cfg)
+    many = oracle.Oracle.from_config(cfg, threads=threads)
+    assert one.threads == 1 and many.threads == threads
+    assert (one.species() == many.species()).all()                  # S6 under threads
+    assert one.energy() == many.energy()
+    many.count_visits(True)
+    for t in range(4):
+        one.sweep(1)
+        many.sweep(1, order_mode=2 if t & 1 else 0, order_seed=7)
+        assert (one.species() == many.species()).all()
+    assert (many.visits() == 4).all()
+    assert (one.energy_trace() == many.energy_trace()).all()
+    assert one.stats() == many.stats()
+    assert one.energy() == many.energy() == many.running_energy()
+    assert (one.sro()[1] == many.sro()[1]).all()
+    counts = [cfg.n_sites - 3 * (cfg.n_sites // 5)] + [cfg.n_sites // 5] * 3 + [0] * (cfg.n_species - 4)
+    one.init_composition(counts)
+    many.init_composition(counts)
+    assert (one.species() == many.species()).all()                  # S10 under threads
+    many.set_threads(1)
+    one.set_threads(3)
+    one.sweep(2)
+    many.sweep(2)
+    assert (one.species() == many.species()).all() and one.running_energy() == many.running_energy()
