@@ -54,13 +54,13 @@ enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
 
 /* Which sweep kernel runs.  WARP_PER_CELL: any lattice/shell list, U8 storage.
  * GROUP_PER_CELL: the same generality with 4, 8, 16 or 32 lanes per link cell (8, 16 or 32 by the number of
- * cells per colour; the environment variable SMCX_GROUP_LANES overrides the choice) and a
+ * cells per colour; smcx_params_t::group_lanes overrides the choice) and a
  * per-pair difference table in shared memory; what AUTO picks whenever a thread kernel does not apply.
  * THREAD_PER_CELL: BCC, first two shells, link_cell = 4, n_species <= 4, 2BIT storage; one block per
  * 128 cells, two-level acceptance filter in shared memory.
  * THREAD_PERSISTENT: same restrictions; one block per SM whose warps walk over the cells of the
  * colour, the whole threshold table in shared memory.  While the current table is too long for that
- * (more than about 16,000 entries next to 20 warps, 32,000 next to 16) passes run the THREAD_PER_CELL
+ * (more than 15,871 entries next to 20 warps, 24,063 next to 16) passes run the THREAD_PER_CELL
  * kernel instead.
  * AUTO picks, when the parameters allow a thread kernel, THREAD_PERSISTENT for lattices that give every
  * warp of every SM a batch of cells (>= 148*20*32 link cells per colour) and THREAD_PER_CELL below that
@@ -84,7 +84,8 @@ enum {
   SMCX_E_NO_MEMORY = -10,          /* host or device allocation failed / workspace too small */
   SMCX_E_CUDA = -11,               /* CUDA error; text via smcx_last_error */
   SMCX_E_UNSUPPORTED = -12,        /* storage/kernel choice not valid for these parameters */
-  SMCX_E_RANGE = -13               /* trace range not retained, sweep counter overflow */
+  SMCX_E_RANGE = -13,              /* trace range not retained, sweep counter overflow */
+  SMCX_E_EPI_RANGE = -14           /* EPI magnitudes so large that the int32 dE of a trial could overflow */
 };
 
 typedef struct {
@@ -98,7 +99,7 @@ typedef struct {
   const uint32_t *accept;   /* host, thresholds T[0..accept_len): a trial with dE = d > 0 is
                                accepted iff d < accept_len and u < T[d], u a 32-bit Philox word
                                (Eq. 3 in integer form); the library never evaluates exp() */
-  int32_t accept_len;       /* 1 .. 2^22 */
+  int32_t accept_len;       /* 1 .. 2^20 (entries reserved on the device); longer tables: SMCX_E_BAD_TABLE */
   uint64_t seed;            /* Philox key */
   int32_t storage;          /* SMCX_STORAGE_* */
   int32_t kernel;           /* SMCX_KERNEL_* */
@@ -107,6 +108,9 @@ typedef struct {
   void *stream;             /* cudaStream_t (e.g. torch.cuda.current_stream().cuda_stream); NULL = legacy default */
   void *d_workspace;        /* device, caller-owned, >= smcx_workspace_bytes(); NULL = library allocates */
   size_t workspace_bytes;   /* size of d_workspace */
+  int32_t group_lanes;      /* GROUP_PER_CELL: lanes per link cell, 4 | 8 | 16 | 32; 0 = chosen from the cells per colour.
+                               A value whose tiles do not fit shared memory is ignored (auto). */
+  int32_t group_warps;      /* GROUP_PER_CELL: warps per block, 1..8; 0 = as many as leave room for four blocks per SM */
 } smcx_params_t;
 
 /* Bytes of device workspace a handle with these parameters needs (species array in its storage
@@ -152,10 +156,15 @@ int smcx_sweep(smcx_t *h, int64_t n);
 int smcx_energy(smcx_t *h, int64_t *E);
 /* Running energy E_0 + sum of accepted dE as kept by the sweep kernels.  Synchronises. */
 int smcx_running_energy(smcx_t *h, int64_t *E);
-/* dst[k] = running energy after sweep first_sweep + k, k < count.  Synchronises. */
+/* Energy after every Monte Carlo step (the quantity a warm-up / measurement protocol watches, PAPER.md:65;
+ * E_i of Eq. 6 for replica exchange): dst[k] = running energy after sweep first_sweep + k,
+ * k < count.  SMCX_E_RANGE if a sweep is no longer (or not yet) in the ring of trace_capacity entries.
+ * Synchronises. */
 int smcx_energy_trace(smcx_t *h, int64_t first_sweep, int64_t count, int64_t *dst);
 
-/* Species, N bytes, one per site in site-id order whatever the device storage.  Synchronises. */
+/* The configuration sigma itself (what the paper stores and post-processes: "configurations" for the SRO
+ * average PAPER.md:163 and the atom-probe comparison PAPER.md:185; lattice order nx*ny*nz*basis):
+ * N bytes, one species per site in site-id order whatever the device storage.  Synchronises. */
 int smcx_species(smcx_t *h, uint8_t *host_dst);
 int smcx_species_device(smcx_t *h, void *d_dst); /* asynchronous, on the handle's stream */
 
@@ -164,6 +173,9 @@ int smcx_species_device(smcx_t *h, void *d_dst); /* asynchronous, on the handle'
  * sigma_{i+d} = p} (int64).  NaN where a species is absent.  pair_counts may be NULL.  Synchronises. */
 int smcx_sro(smcx_t *h, double *alpha, int64_t *pair_counts);
 
+/* Bookkeeping of the run: Monte Carlo steps done, trial moves made (= steps x N: one trial per site per step,
+ * PAPER.md:65; the paper's throughput unit "atom step") and trials accepted by Eq. 3
+ * (PAPER.md:60-63).  Every pointer may be NULL.  Synchronises. */
 int smcx_stats(smcx_t *h, int64_t *sweeps_done, int64_t *trials, int64_t *accepted);
 int smcx_synchronize(smcx_t *h);
 

@@ -30,6 +30,7 @@ class _Params(C.Structure):
         ("accept", C.POINTER(C.c_uint32)), ("accept_len", C.c_int32), ("seed", C.c_uint64),
         ("storage", C.c_int32), ("kernel", C.c_int32), ("device", C.c_int32), ("trace_capacity", C.c_int32),
         ("stream", C.c_void_p), ("d_workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
+        ("group_lanes", C.c_int32), ("group_warps", C.c_int32),
     ]
 
 
@@ -111,7 +112,7 @@ def _strerror(code: int) -> str:
 
 
 def _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage, kernel,
-                 device, trace_capacity):
+                 device, trace_capacity, group_lanes=0, group_warps=0):
     epi = np.ascontiguousarray(epi, dtype=np.int32)
     accept = np.ascontiguousarray(accept, dtype=np.uint32)
     p = _Params()
@@ -124,6 +125,7 @@ def _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cel
     p.accept_len = int(accept.size)
     p.seed = int(seed)
     p.storage, p.kernel, p.device, p.trace_capacity = int(storage), int(kernel), int(device), int(trace_capacity)
+    p.group_lanes, p.group_warps = int(group_lanes), int(group_warps)
     return p, (epi, accept)
 
 
@@ -131,7 +133,7 @@ class Lattice:
     """One smcx_t handle.  Methods mirror the C entry points of include/smcx.h."""
 
     def __init__(self, lattice, dims, n_species, n_shells, epi, accept, seed, link_cell=4, kT_units=0,
-                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0):
+                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0, group_lanes=0, group_warps=0):
         import torch  # device memory + stream only
 
         if not torch.cuda.is_available():
@@ -139,7 +141,7 @@ class Lattice:
         self._lib = lib = load_library()
         self._h = None
         p, keep = _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage,
-                               kernel, device, trace_capacity)
+                               kernel, device, trace_capacity, group_lanes, group_warps)
         need = C.c_size_t(0)
         rc = lib.smcx_workspace_bytes(C.byref(p), C.byref(need))
         if rc != 0:

@@ -89,6 +89,7 @@ struct Plan {
   int storage;
   int kernel;
   int group_lanes;  // lanes per cell of the sub-warp kernel
+  int group_warps;  // its warps per block
   int coef_class;   // build_thread_coefficients: 2 = the filter variant of the thread kernel applies
   bool coef_packed; // pack_thread_coefficients: the 16-bit coefficient rows are exact
   Layout lay;
@@ -219,11 +220,14 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     plan->group_lanes = 16;
   if (group_smem_layout(G, 8, 2).total <= 227 * 1024 && (long long)G.cells_per_colour * 8 / 32 >= 148ll * 48)
     plan->group_lanes = 8;
-  if (const char* env = std::getenv("SMCX_GROUP_LANES")) {
-    const int v = std::atoi(env);
-    if ((v == 4 || v == 8 || v == 16 || v == 32) && group_smem_layout(G, v, 2).total <= 227 * 1024) plan->group_lanes = v;
+  if (p->group_lanes != 0) {
+    const int v = p->group_lanes;
+    if (v != 4 && v != 8 && v != 16 && v != 32) return SMCX_E_UNSUPPORTED;
+    if (group_smem_layout(G, v, 2).total <= 227 * 1024) plan->group_lanes = v;
   }
+  if (p->group_warps < 0 || p->group_warps > kGroupWarpsPerBlock) return SMCX_E_UNSUPPORTED;
   {
+    // the generic kernels compute dE = sum over 2 ZT neighbours of D_s(x) + corr(a,b) in int32
     long long max_d = 0;   // largest |V_s(b,x) - V_s(a,x)|
     for (int s = 0; s < p->n_shells; ++s)
       for (int a = 0; a < n; ++a)
@@ -231,8 +235,10 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
           for (int x = 0; x < n; ++x)
             max_d = std::max(max_d, std::llabs((long long)p->epi[(s * n + b) * n + x] - (long long)p->epi[(s * n + a) * n + x]));
     G.gd16 = max_d <= 32767 ? 1 : 0;
+    if ((2ll * G.ZT + 2 * kMaxGroupSlots + 4) * max_d >= (1ll << 31)) return SMCX_E_EPI_RANGE;
   }
   group_tune_layout(G, plan->group_lanes);
+  plan->group_warps = group_warps_per_block(G, plan->group_lanes, p->group_warps);
   if (kernel == SMCX_KERNEL_GROUP_PER_CELL && group_smem_layout(G, plan->group_lanes, 2).total > 227 * 1024)
     return SMCX_E_LINK_CELL_TOO_SMALL;
 
@@ -305,6 +311,20 @@ namespace {
       return SMCX_E_CUDA;                                                         \
     }                                                                             \
   } while (0)
+
+// Every entry point that touches CUDA runs on the handle's device whatever device the caller has made current
+// (a process that drives several GPUs switches devices between calls) and restores the caller's device on return.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  explicit DeviceGuard(int device) {
+    if (cudaGetDevice(&prev) == cudaSuccess && prev != device) switched = cudaSetDevice(device) == cudaSuccess;
+    else cudaGetLastError();
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+  DeviceGuard(const DeviceGuard&) = delete;
+  DeviceGuard& operator=(const DeviceGuard&) = delete;
+};
 
 int grid_for(const smcx* h, long long work_items, int block) {
   const long long want = (work_items + block - 1) / block;
@@ -431,8 +451,9 @@ int launch_colour_pass(smcx* h, int colour) {
     return SMCX_OK;
   }
   if (P.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
-    launch_group_per_cell(G, P.group_lanes, h->d_species(), h->d_gtable(), h->d_accept(), h->d_filter(), h->d_state(), colour, h->stream);
+    launch_group_per_cell(G, P.group_lanes, P.group_warps, h->d_species(), h->d_gtable(), h->d_accept(), h->d_filter(), h->d_state(), colour, h->stream);
     h->launches++;
+    SMCX_CUDA(h, cudaGetLastError());
     return SMCX_OK;
   }
   const int n2 = G.n_species * G.n_species;
@@ -487,6 +508,7 @@ const char* smcx_strerror(int code) {
     case SMCX_E_CUDA: return "CUDA error (see smcx_last_error)";
     case SMCX_E_UNSUPPORTED: return "storage/kernel choice not valid for these parameters";
     case SMCX_E_RANGE: return "range not available";
+    case SMCX_E_EPI_RANGE: return "EPI magnitudes too large: the int32 energy change of a trial could overflow";
     default: return "unknown error";
   }
 }
@@ -520,7 +542,9 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     cudaGetLastError();
     return fail(SMCX_E_CUDA);
   }
-  if (cudaSetDevice(p->device) != cudaSuccess) return fail(SMCX_E_CUDA);
+  DeviceGuard on_device(p->device);     // the caller's current device is restored on return
+  int now = -1;
+  if (cudaGetDevice(&now) != cudaSuccess || now != p->device) return fail(SMCX_E_CUDA);
   cudaDeviceProp prop;
   if (cudaGetDeviceProperties(&prop, p->device) != cudaSuccess) return fail(SMCX_E_CUDA);
   h->sm_count = prop.multiProcessorCount;
@@ -558,7 +582,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     const size_t sm = (size_t)((G.n_shells * n2 * 4 + G.B * G.ZT * 2 + G.ZT + 15) & ~15) +
                       (size_t)kWarpsPerBlock * ((G.TW * G.TW * G.TW * G.B + 15) & ~15);
     if (h->plan.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
-      const cudaError_t e = configure_group_per_cell(G, h->plan.group_lanes);
+      const cudaError_t e = configure_group_per_cell(G, h->plan.group_lanes, h->plan.group_warps);
       if (e != cudaSuccess) { h->err = cudaGetErrorString(e); return fail(SMCX_E_CUDA); }
     }
     if (h->plan.kernel == SMCX_KERNEL_WARP_PER_CELL) {
@@ -600,6 +624,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
 
 void smcx_destroy(smcx_t* h) {
   if (!h) return;
+  DeviceGuard on_device(h->device);
   if (h->stream || h->ws) cudaStreamSynchronize(h->stream);
   for (int s = 0; s < kStagingSlots; ++s) {
     if (h->staging[s]) cudaFreeHost(h->staging[s]);
@@ -615,6 +640,7 @@ void smcx_destroy(smcx_t* h) {
 
 int smcx_set_species_device(smcx_t* h, const void* d_src) {
   if (!h || !d_src) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   const uint8_t* src = reinterpret_cast<const uint8_t*>(d_src);
   unsigned long long zero = 0;
@@ -637,6 +663,7 @@ int smcx_set_species_device(smcx_t* h, const void* d_src) {
 
 int smcx_set_species(smcx_t* h, const uint8_t* host_src) {
   if (!h || !host_src) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   for (long long i = 0; i < P.n_sites; ++i)
     if (host_src[i] >= P.G.n_species) return SMCX_E_BAD_STATE;
@@ -658,6 +685,7 @@ int smcx_set_species(smcx_t* h, const uint8_t* host_src) {
 
 int smcx_init_composition(smcx_t* h, const int64_t* counts) {
   if (!h || !counts) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   CompositionCum C{};
   long long sum = 0;
@@ -681,6 +709,7 @@ int smcx_init_composition(smcx_t* h, const int64_t* counts) {
 
 int smcx_set_sweep_counter(smcx_t* h, int64_t t) {
   if (!h) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   if (t < 0 || t > 0xffffffffll) return SMCX_E_RANGE;
   const unsigned long long v = (unsigned long long)t;
   SMCX_CUDA(h, cudaMemcpyAsync(&h->d_state()->sweep, &v, sizeof(v), cudaMemcpyHostToDevice, h->stream));
@@ -692,6 +721,7 @@ int smcx_set_sweep_counter(smcx_t* h, int64_t t) {
 
 int smcx_set_temperature(smcx_t* h, int32_t kT_units, const uint32_t* accept, int32_t accept_len) {
   if (!h) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   const int rc = upload_table(h, accept, accept_len);
   if (rc == SMCX_OK) h->kT_units = kT_units;
   return rc;
@@ -699,6 +729,7 @@ int smcx_set_temperature(smcx_t* h, int32_t kT_units, const uint32_t* accept, in
 
 int smcx_sweep(smcx_t* h, int64_t n) {
   if (!h) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   if (n < 0 || h->sweeps_enqueued + n > 0xffffffffll) return SMCX_E_RANGE;  // t is a 32-bit counter word
   // Runs of sweeps at fixed parameters are replayed from a captured graph of one sweep (the kernels
   // read the sweep counter from device memory, so the same graph serves every sweep).
@@ -741,12 +772,14 @@ int smcx_sweep(smcx_t* h, int64_t n) {
 
 int smcx_synchronize(smcx_t* h) {
   if (!h) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
   return SMCX_OK;
 }
 
 int smcx_energy(smcx_t* h, int64_t* E) {
   if (!h || !E) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   std::vector<unsigned long long> M;
   const int rc = run_pair_counts(h, M);
   if (rc != SMCX_OK) return rc;
@@ -756,6 +789,7 @@ int smcx_energy(smcx_t* h, int64_t* E) {
 
 int smcx_running_energy(smcx_t* h, int64_t* E) {
   if (!h || !E) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   long long e = 0;
   SMCX_CUDA(h, cudaMemcpyAsync(&e, &h->d_state()->e_run, sizeof(e), cudaMemcpyDeviceToHost, h->stream));
   SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
@@ -765,6 +799,7 @@ int smcx_running_energy(smcx_t* h, int64_t* E) {
 
 int smcx_energy_trace(smcx_t* h, int64_t first_sweep, int64_t count, int64_t* dst) {
   if (!h || (!dst && count > 0)) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   const long long cap = h->plan.G.trace_capacity;
   if (first_sweep < h->trace_first || count < 0 || first_sweep + count > h->sweeps_enqueued ||
       h->sweeps_enqueued - first_sweep > cap)
@@ -782,6 +817,7 @@ int smcx_energy_trace(smcx_t* h, int64_t first_sweep, int64_t count, int64_t* ds
 
 int smcx_species_device(smcx_t* h, void* d_dst) {
   if (!h || !d_dst) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   if (P.storage == SMCX_STORAGE_U8) {
     SMCX_CUDA(h, cudaMemcpyAsync(d_dst, h->d_species(), (size_t)P.n_sites, cudaMemcpyDeviceToDevice, h->stream));
@@ -796,6 +832,7 @@ int smcx_species_device(smcx_t* h, void* d_dst) {
 
 int smcx_species(smcx_t* h, uint8_t* host_dst) {
   if (!h || !host_dst) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   if (P.storage == SMCX_STORAGE_U8) {
     SMCX_CUDA(h, cudaMemcpyAsync(host_dst, h->d_species(), (size_t)P.n_sites, cudaMemcpyDeviceToHost, h->stream));
@@ -818,6 +855,7 @@ int smcx_species(smcx_t* h, uint8_t* host_dst) {
 
 int smcx_sro(smcx_t* h, double* alpha, int64_t* pair_counts) {
   if (!h || !alpha) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   std::vector<unsigned long long> M;
   const int rc = run_pair_counts(h, M);
   if (rc != SMCX_OK) return rc;
@@ -854,6 +892,7 @@ int smcx_sro(smcx_t* h, double* alpha, int64_t* pair_counts) {
 
 int smcx_stats(smcx_t* h, int64_t* sweeps_done, int64_t* trials, int64_t* accepted) {
   if (!h) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   DevState st;
   SMCX_CUDA(h, cudaMemcpyAsync(&st, h->d_state(), sizeof(st), cudaMemcpyDeviceToHost, h->stream));
   SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
@@ -865,6 +904,7 @@ int smcx_stats(smcx_t* h, int64_t* sweeps_done, int64_t* trials, int64_t* accept
 
 int smcx_shell_offsets(smcx_t* h, int32_t shell, int32_t* xyz, int32_t max_offsets, int32_t* n_offsets) {
   if (!h || !n_offsets) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   const Geom& G = h->plan.G;
   if (shell < 0 || shell >= G.n_shells) return SMCX_E_BAD_SHELLS;
   int k = 0;
@@ -879,6 +919,7 @@ int smcx_shell_offsets(smcx_t* h, int32_t shell, int32_t* xyz, int32_t max_offse
 
 int smcx_get_config(smcx_t* h, int32_t* storage, int32_t* kernel, int64_t* n_sites, int64_t* n_cells) {
   if (!h) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
   if (storage) *storage = h->plan.storage;
   if (kernel) *kernel = h->plan.kernel;
   if (n_sites) *n_sites = h->plan.n_sites;

@@ -565,19 +565,17 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
 
 // Warps per block: 8, or 4 / 2 when a block of 8 warps of tiles would leave an SM with fewer than four
 // blocks (measured, FCC 400^3, 8 lanes: 16.8 / 14.9 / 16.5 ms per sweep with 8 / 4 / 2 warps per block);
-// SMCX_GROUP_WARPS overrides it for experiments.
-inline int group_warps_per_block(const Geom& G, int lanes) {
+// `requested` (smcx_params_t::group_warps, 0 = auto) overrides it when that many warps of tiles fit.
+inline int group_warps_per_block(const Geom& G, int lanes, int requested) {
   int warps = kGroupWarpsPerBlock;
   while (warps > 2 && 4 * group_smem_layout(G, lanes, warps).total > 227 * 1024) warps >>= 1;
-  if (const char* env = std::getenv("SMCX_GROUP_WARPS")) {
-    const int v = std::atoi(env);
-    if (v >= 1 && v <= 8 && group_smem_layout(G, lanes, v).total <= 227 * 1024) warps = v;
-  }
+  if (requested >= 1 && requested <= kGroupWarpsPerBlock && group_smem_layout(G, lanes, requested).total <= 227 * 1024)
+    warps = requested;
   return warps;
 }
 
-inline cudaError_t configure_group_per_cell(const Geom& G, int lanes) {
-  const int sm = group_smem_layout(G, lanes, group_warps_per_block(G, lanes)).total;
+inline cudaError_t configure_group_per_cell(const Geom& G, int lanes, int warps) {
+  const int sm = group_smem_layout(G, lanes, warps).total;
   const int nit = group_nit(G, lanes);
   cudaError_t e = cudaSuccess;
   SMCX_GROUP_DISPATCH(G.B, lanes, nit, {
@@ -589,9 +587,8 @@ inline cudaError_t configure_group_per_cell(const Geom& G, int lanes) {
   return e;
 }
 
-inline void launch_group_per_cell(const Geom& G, int lanes, uint8_t* species, const int32_t* table, const uint32_t* accept,
+inline void launch_group_per_cell(const Geom& G, int lanes, int warps, uint8_t* species, const int32_t* table, const uint32_t* accept,
                                   const uint32_t* filt, DevState* st, int colour, cudaStream_t stream) {
-  const int warps = group_warps_per_block(G, lanes);
   const GroupSmem S = group_smem_layout(G, lanes, warps);
   const unsigned cpb = warps * (32 / lanes);
   const unsigned grid = (G.cells_per_colour + cpb - 1) / cpb;

@@ -32,26 +32,12 @@
 
 namespace smcxk {
 
-#ifndef SMCX_NT
-#define SMCX_NT 128
-#endif
-#ifndef SMCX_BLOCKS_PER_SM
-#define SMCX_BLOCKS_PER_SM 5
-#endif
-#ifndef SMCX_OPT_DXMAD
-#define SMCX_OPT_DXMAD 1     // x bit of the direction by multiply-add instead of a mask
-#endif
-#ifndef SMCX_OPT_ATOMSWAP
-#define SMCX_OPT_ATOMSWAP 1  // swap by two shared-memory atomic adds instead of two stores
-#endif
-#ifndef SMCX_OPT_XORSWAP
-#define SMCX_OPT_XORSWAP 1   // swap by two predicated shared-memory atomic XORs of (a ^ b)
-#endif
 // Acceptance variants of trial_thread (template parameter MODE)
 constexpr int kAcceptGlobal = 0;   // explicit a != b test, T[dE] from global memory
 constexpr int kAcceptFilter = 1;   // two-level filter tables in shared memory, rare exact look-up
 constexpr int kAcceptDirect = 2;   // the whole table T (plus one zero entry) in shared memory
-constexpr int kThreadNT = SMCX_NT;      // threads (= cells) per block
+constexpr int kThreadNT = 128;          // threads (= cells) per block of sweep_thread_per_cell
+constexpr int kThreadBlocksPerSM = 5;   // 128 x 5 measured best (profiles/README.md, block shapes)
 constexpr int kThreadTileWords = 64;    // 8 x 8 rows of one word
 constexpr int kCoefInts = 8;            // per (a,b): cl0 ch0' cb0 cl1 | ch1' cb1 corr' pad
 constexpr int kFilterTr = 64;           // Tr[r] = T[r], r < 64
@@ -73,7 +59,8 @@ inline bool thread_kernel_supported(const Geom& G) {
 //   corr' = corr - sum_s Z_s (cl_s + ch_s + cb_s).
 // The table holds kDEScale times these values.  Entries with a == b hold kSameSpecies in corr' and
 // zeros elsewhere.  Returns, from the bound |dE| <= 2 sum_s Z_s max_x |D_s(x)| + |corr|:
-//   0  kDEScale dE could overflow int32: the kernel cannot be used;
+//   0  the sum of kDEScale dE over the 128 trials of a cell could overflow the int32 a thread accumulates it in
+//      (bound >= 2^22): the kernel cannot be used;
 //   1  exact, but dE can reach kSameSpecies: only the variant without the filter tables applies;
 //   2  every dE of a trial between different species is below kSameSpecies: the filter variant applies.
 inline int build_thread_coefficients(const int32_t* epi, int n_species, int32_t* coef /*16*8*/) {
@@ -100,7 +87,7 @@ inline int build_thread_coefficients(const int32_t* epi, int n_species, int32_t*
       }
       c[6] = (int32_t)(kDEScale * corr);
       if (bound >= kSameSpecies) cls = std::min(cls, 1);
-      if (bound >= (1ll << 28)) cls = 0;
+      if (bound >= (1ll << 22)) cls = 0;
     }
   return cls;
 }
@@ -324,14 +311,9 @@ __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p
   constexpr int slot = bi * 4 + X - 2;
   // direction: top three bits of the draw (= mulhi(w_dir, 8)); dx = bit 0, dy = bit 1, dz = bit 2.
   // row_j - row_i = (dy - 1 + bi) + 8 (dz - 1 + bi): byte (dy + 2 dz) of 0x09080100, less 9 if bi == 0
-#if SMCX_OPT_DXMAD
   const uint32_t t1 = w_dir >> 30;
   const uint32_t dx = mad_u32(t1, 0xFFFFFFFEu, w_dir >> 29);   // dir - 2 (dir >> 1), on the FMA pipe
   const uint32_t rdp = prmt(0x09080100u, 0u, t1);
-#else
-  const uint32_t dx = (w_dir >> 29) & 1u;
-  const uint32_t rdp = prmt(0x09080100u, 0u, w_dir >> 30);
-#endif
   uint32_t* p_j = p_i - 9 * (1 - bi) * NT + rdp * NT;
   // rows around i and j
   const uint32_t own_i = p_i[0];
@@ -385,7 +367,7 @@ __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p
     // construction) all clamp to that entry and are decided by the sign test alone
     const uint32_t i4 = min((uint32_t)dE4, env.tmax4);
     const uint32_t thr = lds_u32(env.filt, i4);
-#if defined(__CUDA_ARCH__) && SMCX_OPT_XORSWAP
+#if defined(__CUDA_ARCH__)
     // decision without a branch or a 0/1 value: reject = dE > 0 and u >= T.  A rejected trial XORs
     // zeros (ptxas would wrap a predicated shared-memory atomic in a branch of its own).
     uint32_t xm;
@@ -436,7 +418,7 @@ __host__ __device__ __forceinline__ void trial_thread(const Geom& G, uint32_t* p
   // rejected trial stores the rows back unchanged (no branch)
   const uint32_t oki = ok ? 1u : 0u;
   const uint32_t od = mad_u32(oki, b4 - a4, 0u);
-#if SMCX_OPT_ATOMSWAP && defined(__CUDA_ARCH__)
+#if defined(__CUDA_ARCH__)
   atomicAdd(p_i, od * (1u << K::shi));                       // shared-memory adds: i and j may share a row
   atomicAdd(p_j, od * ((0u - (1u << K::shj0)) * mul));
 #else
@@ -495,7 +477,7 @@ __device__ __forceinline__ void write_back_tile(const Geom& G, const uint32_t* t
 
 #ifdef __CUDACC__
 template <int kFilter>
-__global__ void __launch_bounds__(kThreadNT, SMCX_BLOCKS_PER_SM)
+__global__ void __launch_bounds__(kThreadNT, kThreadBlocksPerSM)
 sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* __restrict__ coef,
                       const uint32_t* __restrict__ accept, const uint32_t* __restrict__ filt,
                       DevState* __restrict__ st, int colour) {
@@ -505,7 +487,7 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
   int4* s_coef0 = reinterpret_cast<int4*>(smem_w + kThreadTileWords * NT);   // [16][8 slots]
   int4* s_coef1 = s_coef0 + 16 * 8;
   uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_coef1 + 16 * 8);
-  __shared__ int s_dE[NT / 32];
+  __shared__ long long s_dE[NT / 32];
   __shared__ unsigned s_acc[NT / 32];
   // coefficient rows replicated over the 8 lane slots of a quarter warp: conflict-free LDS.128
   for (int k = threadIdx.x; k < 128; k += NT) {
@@ -598,13 +580,14 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
       }
     }
   }
-  // a8: block reduction, one atomic pair per block (the trials accumulated kDEScale dE)
-  esum /= kDEScale;
+  // a8: block reduction, one atomic pair per block (the trials accumulated kDEScale dE: exact in int32 per
+  // cell by build_thread_coefficients' bound, summed over cells in 64 bits)
+  long long esum64 = esum / kDEScale;
   for (int o = 16; o > 0; o >>= 1) {
-    esum += __shfl_down_sync(0xffffffffu, esum, o);
+    esum64 += __shfl_down_sync(0xffffffffu, esum64, o);
     nacc += __shfl_down_sync(0xffffffffu, nacc, o);
   }
-  if ((threadIdx.x & 31) == 0) { s_dE[threadIdx.x >> 5] = esum; s_acc[threadIdx.x >> 5] = nacc; }
+  if ((threadIdx.x & 31) == 0) { s_dE[threadIdx.x >> 5] = esum64; s_acc[threadIdx.x >> 5] = nacc; }
   __syncthreads();
   if (threadIdx.x == 0) {
     long long e = 0; unsigned a = 0;
@@ -622,9 +605,6 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
 // on (cell, q) jointly: M1*t is uniform, M0*cell, B = M1*c2' and C = M0*c0'' depend on the cell only (once per
 // cell), A_q = M0*(hi(M1*t) ^ q ^ k0) on q only (once per block, table in shared memory).  Per call that leaves
 // one product and three XORs for rounds 1-3 instead of six and six.  Same function, same bits.
-#ifndef SMCX_OPT_PHILOX_FACTORED
-#define SMCX_OPT_PHILOX_FACTORED 1
-#endif
 struct PhiloxCell { uint32_t l0, lB, hCk, lC; };   // per-cell constants (hCk = hi(C) ^ rk1[2])
 
 __device__ __forceinline__ void mulwide(uint32_t a, uint32_t b, uint32_t& hi, uint32_t& lo) {
@@ -691,9 +671,7 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
   int4* s_coef1 = s_coef0 + 16 * 8;
   uint32_t* s_T = reinterpret_cast<uint32_t*>(s_coef1 + 16 * 8);
   __shared__ unsigned s_acc[kPersistMaxWarps];
-#if SMCX_OPT_PHILOX_FACTORED
   __shared__ uint2 s_slot[64];                                  // Philox round-2 products that depend on the slot pair only
-#endif
   // PK: coef points at the packed rows [16] int4; else at the 32-bit rows [16][2] int4
   for (int k = threadIdx.x; k < 128; k += blockDim.x) {
     const int ent = k >> 3;
@@ -707,9 +685,7 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
   for (int k = threadIdx.x; k <= G.accept_len; k += blockDim.x) s_T[k] = k < G.accept_len ? accept[k] : 0u;
 
   const uint32_t t = (uint32_t)st->sweep;
-#if SMCX_OPT_PHILOX_FACTORED
   if (threadIdx.x < 64) s_slot[threadIdx.x] = philox_slot_entry(threadIdx.x, t, G.rk0, G.rk1);
-#endif
   int ox, oy, oz;
   sweep_origin(G, t, ox, oy, oz);
   int esum = 0;                                                 // kDEScale * sum of accepted dE of this thread
@@ -763,12 +739,8 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
         }
       }
       const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
-#if SMCX_OPT_PHILOX_FACTORED
       const PhiloxCell pc = philox_cell_setup(cell_id, t, ctr3, G.rk0, G.rk1);
 #define SMCX_PHILOX_PAIR(LX) philox_factored(pc, s_slot[q0 + LX], G.rk0, G.rk1)
-#else
-#define SMCX_PHILOX_PAIR(LX) philox4x32_10_rk(cell_id, q0 + LX, t, ctr3, G.rk0, G.rk1)
-#endif
 #pragma unroll 1
       for (int lzy = 0; lzy < 16; ++lzy) {
         uint32_t* p_row = tile + (((lzy >> 2) + 2) * 8 + (lzy & 3) + 2) * NT;
@@ -832,7 +804,7 @@ inline int launch_thread_persistent(const Geom& G, uint32_t* lattice, const int3
   else
     sweep_thread_persistent<false><<<grid, warps * 32, persist_smem(warps, G.accept_len), stream>>>(
         G, lattice, reinterpret_cast<const int4*>(d_coef), accept, st, colour);
-  return 0;
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 
 inline int configure_thread_per_cell() {
@@ -856,7 +828,7 @@ inline int launch_thread_per_cell(const Geom& G, uint32_t* lattice, const int32_
   else
     sweep_thread_per_cell<false><<<grid, kThreadNT, thread_kernel_smem(), stream>>>(
         G, lattice, reinterpret_cast<const int4*>(d_coef), accept, d_filter, st, colour);
-  return 0;
+  return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 #endif  // __CUDACC__
 

@@ -156,3 +156,48 @@ def test_long_exchange_run_slow():
     st = _assert_slots_equal(g, reps, [o.tag for o in reps])
     assert st["accepted"].tolist() == n_acc.tolist() and n_acc.sum() > 30
     g.close()
+
+
+def _ladder_hitting(T_target, dE, kT_hi=2_100_000_000):
+    """Integer temperatures (kT_0 < kT_1) for which floor(exp(Delta) 2^32) == T_target with the fractional part of
+    exp(Delta) 2^32 well inside (0.25, 0.75), Delta = (kT_1 - kT_0) dE / (kT_0 kT_1), dE = E_0 - E_1 < 0: for kT_1
+    near 2^31 one unit of kT_0 moves the threshold by a fraction of a unit, so a scan over kT_1 finds one quickly."""
+    want = np.log((T_target + 0.5) / 4294967296.0)                 # Delta* < 0
+    for kT1 in range(kT_hi, kT_hi - 4000, -1):
+        kT0 = int(round(1.0 / (1.0 / kT1 + want / dE)))            # 1/kT0 - 1/kT1 = Delta*/dE
+        if not 0 < kT0 < kT1:
+            continue
+        x = np.exp(oracle.exchange_delta(0, -dE, kT0, kT1)) * 4294967296.0
+        if int(np.floor(x)) == T_target and 0.25 < x - np.floor(x) < 0.75:
+            return kT0, kT1
+    raise AssertionError("no ladder found")
+
+
+@pytest.mark.parametrize("offset,expect", [(+1, 1), (0, 0), (-1, 0)], ids=["u=T-1", "u=T", "u=T+1"])
+def test_exchange_decision_at_the_threshold(offset, expect):
+    """S9's integer decision `u < floor(exp(Delta) 2^32)` exactly at its edge (Eq. 5): the two
+    temperatures are constructed so that the threshold T is the Philox draw of the round plus 1, plus 0 and minus 1
+    -- accept, reject, reject -- with exp(Delta) 2^32 far enough from an integer that CUDA's exp and libm's cannot
+    round to different sides.  Energies: replica 0 a pure crystal (E = 0), replica 1 the B2 state (E = 4 N v)."""
+    lat, dims, v = 0, (16, 16, 16), 15_000
+    N = 2 * 16 ** 3
+    epi = np.array([[[0, v], [v, 0]]], dtype=np.int32)
+    dE = -4 * N * v                                                  # E_0 - E_1
+    xseed = next(s for s in range(10_000, 20_000) if oracle.exchange_draw(s, 0, 0) > 0.90 * 2 ** 32
+                 and oracle.exchange_draw(s, 0, 0) < 0.99 * 2 ** 32)
+    u = oracle.exchange_draw(xseed, 0, 0)
+    kT0, kT1 = _ladder_hitting(u + offset, dE)
+    assert bool(oracle.exchange_accept(0, -dE, kT0, kT1, u)) == bool(expect)
+    tiny = np.array([0xFFFFFFFF, 0], dtype=np.uint32)               # no sweeps are run: any table will do
+    g = smcx.Ensemble(lat, dims, 2, 1, epi, [kT0, kT1], [tiny, tiny], [1, 2], xseed)
+    s0 = np.zeros(N, np.uint8)
+    s1 = np.zeros(N, np.uint8)
+    s1[1::2] = 1
+    g.replicas[0].set_species(s0)
+    g.replicas[1].set_species(s1)
+    assert g.replicas[0].running_energy() == 0 and g.replicas[1].running_energy() == -dE
+    g.exchange(0)
+    st = g.state()
+    assert st["last_flags"].tolist() == [expect] and st["attempted"].tolist() == [1]
+    assert st["replica_at_slot"].tolist() == ([1, 0] if expect else [0, 1])
+    g.close()

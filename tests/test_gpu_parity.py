@@ -1,6 +1,7 @@
 """GPU-vs-oracle parity through the C ABI (pytest -m gpu): species arrays, energy traces and pair
 counts bit-exact, fp64 SRO within 1e-9 relative (BASELINE.json north_star)."""
 import os
+import time
 
 import numpy as np
 import pytest
@@ -22,9 +23,15 @@ def _supported(cfg, kernel):
     return cfg.lattice == 0 and cfg.n_shells == 2 and cfg.link_cell == 4 and cfg.n_species <= 4
 
 
-def _pair(cfg, kernel=smcx.KERNEL_AUTO, **over):
+# The full-size oracle runs spread the cells of a colour over all host cores (oracle pin
+# test_p7_threads_over_the_cells_of_a_colour_change_nothing: bit-identical to the one-thread oracle).
+ALL_CORES = max(1, os.cpu_count() or 1)
+
+
+def _pair(cfg, kernel=smcx.KERNEL_AUTO, threads=1, **over):
     g = smcx.Lattice.from_config(cfg, kernel=kernel, **over)
-    o = oracle.Oracle.from_config(cfg, **{k: v for k, v in over.items() if k in ("seed", "link_cell", "epi", "accept")})
+    o = oracle.Oracle.from_config(cfg, threads=threads,
+                                  **{k: v for k, v in over.items() if k in ("seed", "link_cell", "epi", "accept")})
     return g, o
 
 
@@ -61,7 +68,7 @@ def test_config1_full_run_species_after_every_sweep(kernel):
 @pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
 def test_config2_anneal_prefix(kernel):
     """Config 2 with its per-sweep temperature table; SRO sampled every 10 sweeps here
-    (every 100 over the full 2,000 in the slow test)."""
+    (every 100 over the full 2,000 sweeps in test_config2_anneal_full_length)."""
     cfg = get_config(2)
     n = 30
     g, o = _pair(cfg, kernel)
@@ -79,10 +86,11 @@ def test_config2_anneal_prefix(kernel):
     assert g.stats() == o.stats()
 
 
-@pytest.mark.slow
 def test_config2_anneal_full_length():
+    """BASELINE.json configs[1] at SURVEY.md 8(d)'s extent: all 2,000 sweeps of the anneal, species + SRO at the 20
+    sample points, the full trace."""
     cfg = get_config(2)
-    g, o = _pair(cfg)
+    g, o = _pair(cfg, threads=ALL_CORES)
     for t in range(cfg.n_sweeps):
         table = cfg.accept_table(t)
         g.set_temperature(cfg.kT_at(t), table)
@@ -144,20 +152,18 @@ def test_config4_full_size_invariants(kernel):
     assert int((cfg.epi().astype(np.int64) * c1).sum()) == 2 * g.energy()
 
 
-@pytest.mark.slow
 def test_config5_shape_at_400_cubed():
     """Config 5's parameters on 400^3 cells (1.28e8 sites): the oracle cannot reach 1.6e10 sites in
     reasonable time, so parity is checked on the same build at this size and invariants at full
     size (test_config5_full_size_invariants)."""
     cfg = scaled_config(5, (400, 400, 400))
-    g, o = _pair(cfg)
+    g, o = _pair(cfg, threads=ALL_CORES)
     g.sweep(1)
     o.sweep(1)
     _assert_same_state(g, o)
     assert (g.energy_trace() == o.energy_trace()).all()
 
 
-@pytest.mark.slow
 def test_config5_full_size_invariants():
     cfg = get_config(5)
     g = smcx.Lattice.from_config(cfg)
@@ -172,18 +178,54 @@ def test_config5_full_size_invariants():
     assert int((cfg.epi().astype(np.int64) * c1).sum()) == 2 * g.energy()
 
 
-@pytest.mark.slow
-@pytest.mark.parametrize("k,n", [(4, 1), (3, 20)])
-def test_full_size_oracle_prefix(k, n):
-    """SMCX_C3_SWEEPS lengthens the config-3 prefix (its full 1,000 sweeps take the oracle about an hour)."""
-    if k == 3:
-        n = int(os.environ.get("SMCX_C3_SWEEPS", n))
-    cfg = get_config(k)
-    g, o = _pair(cfg)
-    g.sweep(n)
-    o.sweep(n)
+def test_config4_full_size_oracle_two_sweeps():
+    """BASELINE.json configs[3] (BCC 800^3, 1.024e9 sites, the graded configuration) in the launch configuration
+    bench.py times, at SURVEY.md 8(d)'s extent: initial state, species after 2 sweeps and the trace against the
+    oracle (all host cores)."""
+    cfg = get_config(4)
+    g, o = _pair(cfg, threads=ALL_CORES)
+    assert g.kernel == smcx.KERNEL_THREAD_PERSISTENT and g.storage == smcx.STORAGE_2BIT
+    _assert_same_state(g, o)
+    g.sweep(2)
+    o.sweep(2)
     _assert_same_state(g, o)
     assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.stats() == o.stats()
+    assert g.running_energy() == o.running_energy()
+
+
+def test_config3_full_length():
+    """BASELINE.json configs[2] (FCC 128^3, 5 species, 3 shells): all 1,000 sweeps, the trace compared every 100
+    sweeps and the species at the end.  SMCX_C3_BUDGET_S (default 600) bounds the oracle's wall
+    clock on hosts with few cores: the run then stops at a multiple of 100 sweeps, never below 200, and the
+    test prints how far it got."""
+    cfg = get_config(3)
+    budget = float(os.environ.get("SMCX_C3_BUDGET_S", "600"))
+    g, o = _pair(cfg, threads=ALL_CORES)
+    t0, done = time.time(), 0
+    while done < cfg.n_sweeps and (done < 200 or time.time() - t0 < budget):
+        g.sweep(100)
+        o.sweep(100)
+        done += 100
+        assert (g.energy_trace(done - 100, 100) == o.energy_trace(done - 100, 100)).all()
+    _assert_same_state(g, o)
+    assert g.stats() == o.stats()
+    _assert_sro(g, o)
+    print(f"config 3: {done} of {cfg.n_sweeps} sweeps bit-exact with the oracle in {time.time() - t0:.0f} s "
+          f"({ALL_CORES} oracle threads)")
+    assert done == cfg.n_sweeps or time.time() - t0 >= budget
+
+
+@pytest.mark.slow
+def test_config5_full_size_oracle_first_sweep():
+    """BASELINE.json configs[4] (BCC 2000^3, 1.6e10 sites) against the oracle on sweep 0 (needs
+    16 GB of host memory for the oracle's array and as much for the copy of the device's).  SMCX_SLOW=1."""
+    cfg = get_config(5)
+    g, o = _pair(cfg, threads=ALL_CORES)
+    g.sweep(1)
+    o.sweep(1)
+    assert g.energy_trace()[0] == o.energy_trace()[0] and g.stats() == o.stats()
+    _assert_same_state(g, o)
 
 
 @pytest.mark.parametrize("kernel", KERNELS, ids=KERNEL_IDS)
@@ -228,15 +270,12 @@ def test_thread_and_warp_kernels_agree():
                                           (smcx.KERNEL_GROUP_PER_CELL, 8), (smcx.KERNEL_GROUP_PER_CELL, 16),
                                           (smcx.KERNEL_GROUP_PER_CELL, 32), (smcx.KERNEL_AUTO, 0)],
                          ids=["warp", "group4", "group8", "group16", "group32", "auto"])
-def test_edge_geometries(lat, dims, n_sp, n_shells, w, kernel, lanes, monkeypatch):
+def test_edge_geometries(lat, dims, n_sp, n_shells, w, kernel, lanes):
     amplitude, kT, seed = 350, 500, 4711
     epi = make_epi(n_shells, n_sp, amplitude, seed)
     table = make_accept_table(kT)
-    if lanes:
-        monkeypatch.setenv("SMCX_GROUP_LANES", str(lanes))   # lanes per cell of the sub-warp kernel
-    else:
-        monkeypatch.delenv("SMCX_GROUP_LANES", raising=False)
-    g = smcx.Lattice(lat, dims, n_sp, n_shells, epi, table, seed, link_cell=w, kT_units=kT, kernel=kernel)
+    g = smcx.Lattice(lat, dims, n_sp, n_shells, epi, table, seed, link_cell=w, kT_units=kT, kernel=kernel,
+                     group_lanes=lanes)                      # lanes per cell of the sub-warp kernel (0 = auto)
     o = oracle.Oracle(lat, dims, n_sp, n_shells, epi, w, table, seed)
     assert o.lc_valid()
     for s in range(n_shells):
@@ -420,15 +459,15 @@ def test_checkpoint_and_resume_in_a_new_handle(kernel):
 
 @pytest.mark.parametrize("lanes", [8, 16, 32])
 @pytest.mark.parametrize("amplitude,kT", [(400, 690), (30_000, 20_000)], ids=["d16", "d32"])
-def test_sub_warp_kernel_table_formats(lanes, amplitude, kT, monkeypatch):
+def test_sub_warp_kernel_table_formats(lanes, amplitude, kT):
     """FCC, 5 species, 3 shells with differences that fit 16 bits (8 lanes: halfword rows, one bank window per
     cell of the warp) and with differences that do not (32-bit rows everywhere), for every lane count."""
-    monkeypatch.setenv("SMCX_GROUP_LANES", str(lanes))
     lat, dims, n_sp, n_sh, w, seed = 1, (16, 16, 8), 5, 3, 4, 91
     epi = make_epi(n_sh, n_sp, amplitude, seed)
     assert (np.abs(epi).max() * 2 > 32767) == (amplitude > 16384)
     table = make_accept_table(kT)
-    g = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, seed, link_cell=w, kT_units=kT, kernel=smcx.KERNEL_GROUP_PER_CELL)
+    g = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, seed, link_cell=w, kT_units=kT, kernel=smcx.KERNEL_GROUP_PER_CELL,
+                     group_lanes=lanes, group_warps=2 if lanes == 8 else 0)
     o = oracle.Oracle(lat, dims, n_sp, n_sh, epi, w, table, seed)
     g.sweep(4)
     o.sweep(4)

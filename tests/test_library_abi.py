@@ -10,7 +10,7 @@ from paper_2509_20949_b200.binding import SmcxError, workspace_bytes
 from smcx_inputs import get_config, make_accept_table, make_epi
 
 E = dict(NULL_ARG=-1, BAD_LATTICE=-2, BAD_DIMS=-3, BAD_SPECIES=-4, BAD_SHELLS=-5, EPI_NOT_SYMMETRIC=-6,
-         LINK_CELL_TOO_SMALL=-7, BAD_TABLE=-8, UNSUPPORTED=-12)
+         LINK_CELL_TOO_SMALL=-7, BAD_TABLE=-8, UNSUPPORTED=-12, EPI_RANGE=-14)
 
 
 def test_library_loads_and_exports_every_declared_symbol():
@@ -64,6 +64,18 @@ def test_parameter_validation_codes():
     assert _code(accept=np.zeros(0, np.uint32)) == E["BAD_TABLE"]
     assert _code(storage=smcx.STORAGE_2BIT, kernel=smcx.KERNEL_WARP_PER_CELL) == E["UNSUPPORTED"]
     assert _code(lattice=1, n_shells=3, epi=make_epi(3, 4, 300, 1), kernel=smcx.KERNEL_THREAD_PER_CELL) == E["UNSUPPORTED"]
+    # explicit launch shape of the sub-warp kernel (smcx_params_t::group_lanes / group_warps; 0 = auto)
+    assert _code(kernel=smcx.KERNEL_GROUP_PER_CELL, group_lanes=5) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_GROUP_PER_CELL, group_lanes=64) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_GROUP_PER_CELL, group_warps=9) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_GROUP_PER_CELL, group_warps=-1) == E["UNSUPPORTED"]
+    for lanes in (0, 4, 8, 16, 32):
+        assert workspace_bytes(**_kw(kernel=smcx.KERNEL_GROUP_PER_CELL, group_lanes=lanes, group_warps=lanes // 8)) > 0
+    # interactions so large that a trial's int32 dE could overflow
+    huge = make_epi(2, 4, 300, 1) * 400_000
+    assert _code(epi=huge) == E["EPI_RANGE"]
+    assert _code(epi=huge, kernel=smcx.KERNEL_WARP_PER_CELL) == E["EPI_RANGE"]
+    assert smcx.load_library().smcx_strerror(E["EPI_RANGE"]) != smcx.load_library().smcx_strerror(-99)
     # valid combinations pass
     assert workspace_bytes(**_kw()) > 0
     assert workspace_bytes(**_kw(n_shells=4, epi=make_epi(4, 4, 300, 1), link_cell=4, dims=(24, 16, 16))) > 0
@@ -117,6 +129,9 @@ def test_sub_warp_tile_layout_is_a_valid_one(lat, dims, n_sp, n_shells, w):
     the 16 bits they are stored in."""
     from paper_2509_20949_b200.binding import group_layout
     from pygeom import shells
+    forced = group_layout(lattice=lat, dims=dims, n_species=n_sp, n_shells=n_shells, epi=make_epi(n_shells, n_sp, 300, 1),
+                          accept=make_accept_table(600), seed=1, link_cell=w, storage=smcx.STORAGE_U8, group_lanes=32)
+    assert forced["lanes"] == 32                                            # the field is honoured
     L = group_layout(lattice=lat, dims=dims, n_species=n_sp, n_shells=n_shells, epi=make_epi(n_shells, n_sp, 300, 1),
                      accept=make_accept_table(600), seed=1, link_cell=w, storage=smcx.STORAGE_U8)
     assert L["lanes"] in (4, 8, 16, 32) and L["shift"] in (0, 1) and L["skew"] % 4 == 0
