@@ -48,9 +48,13 @@ typedef struct smcx smcx_t; /* opaque; one per (GPU, stream) */
 
 enum { SMCX_BCC = 0, SMCX_FCC = 1 };
 
-/* Device storage of the species array. U8: one byte per site in site-id order.
- * 2BIT: 16 sites per 32-bit word in site-id order (n_species <= 4).  Results never depend on it. */
-enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
+/* Device storage of the species array.  U8: one byte per site in site-id order.
+ * 2BIT: 16 sites per 32-bit word in site-id order (n_species <= 4).
+ * 4BIT: 8 sites per 32-bit word (n_species <= 16), sublattice-planar in groups of 8 conventional cells along x
+ * (dims[0] must be a multiple of 8): group g = c >> 3 of conventional cell c = (z Ly + y) Lx + x holds B words
+ * (B = 2 BCC, 4 FCC), word b = the sites with basis index b of its 8 cells, cell c & 7 in bits 4 (c & 7) .. + 3.
+ * Results never depend on the storage (smcx_species always returns one byte per site in site-id order). */
+enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_4BIT = 4, SMCX_STORAGE_U8 = 8 };
 
 /* Which sweep kernel runs.  WARP_PER_CELL: any lattice/shell list, U8 storage.
  * GROUP_PER_CELL: the same generality with 4, 8, 16 or 32 lanes per link cell (8, 16 or 32 by the number of
@@ -62,12 +66,17 @@ enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_U8 = 8 };
  * colour, the whole threshold table in shared memory.  While the current table is too long for that
  * (more than 15,871 entries next to 20 warps, 24,063 next to 16) passes run the THREAD_PER_CELL
  * kernel instead.
+ * FCC_THREAD: FCC, the first 1..3 shells, link_cell = 4, n_species <= 8, 4BIT storage, every
+ * |V_s(b,x) - V_s(a,x)| < 32768: one thread per link cell on a packed tile (one 32-bit word per sublattice row of 8
+ * cells), neighbours gathered by rotations and bit-selects, the EPI differences applied four neighbours at a time by
+ * byte-permute look-ups (PRMT) and byte dot products (sweep_fcc.cuh).  What AUTO picks for such lattices when
+ * a colour has at least 148 * 6 * 32 link cells (below that the sub-warp kernel's shorter chain per trial wins).
  * AUTO picks, when the parameters allow a thread kernel, THREAD_PERSISTENT for lattices that give every
  * warp of every SM a batch of cells (>= 148*20*32 link cells per colour) and THREAD_PER_CELL below that
  * (same speed there, and concurrent lattices of a replica ensemble overlap freely).  Results never
  * depend on it. */
 enum { SMCX_KERNEL_AUTO = 0, SMCX_KERNEL_WARP_PER_CELL = 1, SMCX_KERNEL_THREAD_PER_CELL = 2,
-       SMCX_KERNEL_THREAD_PERSISTENT = 3, SMCX_KERNEL_GROUP_PER_CELL = 4 };
+       SMCX_KERNEL_THREAD_PERSISTENT = 3, SMCX_KERNEL_GROUP_PER_CELL = 4, SMCX_KERNEL_FCC_THREAD = 5 };
 
 enum {
   SMCX_OK = 0,
@@ -123,11 +132,23 @@ int smcx_workspace_bytes(const smcx_params_t *p, size_t *bytes);
 int smcx_create(smcx_t **out, const smcx_params_t *p);
 void smcx_destroy(smcx_t *h);
 
-/* Replace the lattice state.  host_src / d_src: N bytes, one species per site in site-id order.
- * Returns SMCX_E_BAD_STATE (state unchanged on the host path) if a value is >= n_species.
- * The running energy is recomputed; the sweep counter and trace are kept. */
+/* Replace the lattice state (the configuration sigma of Eq. 1-2).  host_src / d_src: N bytes, one
+ * species per site in site-id order.  Values are validated on the device (no pass over the array on the host):
+ * SMCX_E_BAD_STATE if one is >= n_species -- the device path then leaves the lattice unchanged, the host path has
+ * overwritten it with the low bits of the rejected array and it must be set again.  Host memory may be pageable
+ * or pinned (pinned: the copy of one 2^26-site chunk overlaps the packing of the previous one).
+ * The running energy is recomputed; the sweep counter and trace are kept.  Synchronises. */
 int smcx_set_species(smcx_t *h, const uint8_t *host_src);
 int smcx_set_species_device(smcx_t *h, const void *d_src);
+
+/* The species array in the handle's device storage format, for checkpoints that move 1/4 (2BIT) or 1/2 (4BIT) byte
+ * per site (3-million-step runs): smcx_storage_bytes() bytes of host memory, layout as
+ * described at SMCX_STORAGE_*.  A packed checkpoint can only be loaded into a handle with the same storage, lattice
+ * and dims.  smcx_set_species_packed validates like smcx_set_species (SMCX_E_BAD_STATE: set the state again),
+ * recomputes the running energy and keeps the sweep counter.  Both synchronise. */
+int smcx_storage_bytes(smcx_t *h, size_t *bytes);
+int smcx_species_packed(smcx_t *h, void *host_dst);
+int smcx_set_species_packed(smcx_t *h, const void *host_src);
 
 /* Replace the lattice state by a seeded random solid solution of a given composition (reading S10;
  * the paper's alloy is Fe29Co29Ni28Al7Ti7): counts[p] >= 0 sites of species p,

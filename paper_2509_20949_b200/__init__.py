@@ -7,7 +7,8 @@ and a CUDA device and raises otherwise.
 """
 from .binding import (  # noqa: F401
     BCC, FCC,
-    STORAGE_AUTO, STORAGE_2BIT, STORAGE_U8,
+    STORAGE_AUTO, STORAGE_2BIT, STORAGE_4BIT, STORAGE_U8,
     KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT, KERNEL_GROUP_PER_CELL,
+    KERNEL_FCC_THREAD,
     SmcxError, Lattice, Ensemble, load_library, library_path, exported_symbols,
 )

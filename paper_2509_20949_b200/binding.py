@@ -13,8 +13,9 @@ _HEADER = os.path.join(os.path.dirname(_HERE), "include", "smcx.h")
 _lib = None
 
 BCC, FCC = 0, 1
-STORAGE_AUTO, STORAGE_2BIT, STORAGE_U8 = 0, 2, 8
+STORAGE_AUTO, STORAGE_2BIT, STORAGE_4BIT, STORAGE_U8 = 0, 2, 4, 8
 KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT, KERNEL_GROUP_PER_CELL = 0, 1, 2, 3, 4
+KERNEL_FCC_THREAD = 5
 
 
 class SmcxError(RuntimeError):
@@ -67,6 +68,9 @@ def load_library(build_if_missing: bool = True):
         "smcx_destroy": (None, [vp]),
         "smcx_set_species": (C.c_int, [vp, C.POINTER(C.c_uint8)]),
         "smcx_set_species_device": (C.c_int, [vp, vp]),
+        "smcx_storage_bytes": (C.c_int, [vp, C.POINTER(C.c_size_t)]),
+        "smcx_species_packed": (C.c_int, [vp, vp]),
+        "smcx_set_species_packed": (C.c_int, [vp, vp]),
         "smcx_set_temperature": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_uint32), C.c_int32]),
         "smcx_init_composition": (C.c_int, [vp, i64p]),
         "smcx_set_sweep_counter": (C.c_int, [vp, C.c_int64]),
@@ -220,6 +224,26 @@ class Lattice:
     def set_species_device(self, tensor):
         assert tensor.is_cuda and tensor.dtype.itemsize == 1 and tensor.numel() == self.n_sites and tensor.is_contiguous()
         self._check(self._lib.smcx_set_species_device(self._h, C.c_void_p(tensor.data_ptr())), "smcx_set_species_device")
+
+    def storage_bytes(self) -> int:
+        n = C.c_size_t(0)
+        self._check(self._lib.smcx_storage_bytes(self._h, C.byref(n)), "smcx_storage_bytes")
+        return int(n.value)
+
+    def species_packed(self, out=None) -> np.ndarray:
+        """The species array in device storage format (smcx_species_packed), as bytes."""
+        n = self.storage_bytes()
+        if out is None:
+            out = np.empty(n, dtype=np.uint8)
+        assert out.dtype == np.uint8 and out.size == n and out.flags.c_contiguous
+        self._check(self._lib.smcx_species_packed(self._h, C.c_void_p(out.ctypes.data)), "smcx_species_packed")
+        return out
+
+    def set_species_packed(self, packed):
+        a = np.ascontiguousarray(packed, dtype=np.uint8)
+        if a.size != self.storage_bytes():
+            raise ValueError("packed array must have storage_bytes() bytes")
+        self._check(self._lib.smcx_set_species_packed(self._h, C.c_void_p(a.ctypes.data)), "smcx_set_species_packed")
 
     def init_composition(self, counts):
         c = np.ascontiguousarray(counts, dtype=np.int64)

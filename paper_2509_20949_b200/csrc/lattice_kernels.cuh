@@ -5,17 +5,66 @@
 
 namespace smcxk {
 
-// ---- species accessors for the two device storage formats --------------------------------
+// ---- species accessors for the device storage formats -------------------------------------
+// load(): species of site i.  store16(): the 16 consecutive sites 16 g .. 16 g + 15 (vals[k] = species of site
+// 16 g + k; sites >= n_sites are not written).
 struct StoreU8 {
   static constexpr int kBits = 8;
   __device__ static __forceinline__ int load(const void* p, long long i) {
     return reinterpret_cast<const uint8_t*>(p)[i];
+  }
+  __device__ static __forceinline__ void store16(void* species, long long g, long long n_sites, const uint32_t* vals) {
+    uint8_t* p = reinterpret_cast<uint8_t*>(species) + g * 16;
+    if (g * 16 + 16 <= n_sites) {
+      uint32_t w[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+      for (int k = 0; k < 16; ++k) w[k >> 2] |= vals[k] << (8 * (k & 3));
+      *reinterpret_cast<uint4*>(p) = make_uint4(w[0], w[1], w[2], w[3]);
+    } else {
+      for (int k = 0; k < 16 && g * 16 + k < n_sites; ++k) p[k] = (uint8_t)vals[k];
+    }
   }
 };
 struct Store2 {
   static constexpr int kBits = 2;
   __device__ static __forceinline__ int load(const void* p, long long i) {
     return (int)((reinterpret_cast<const uint32_t*>(p)[i >> 4] >> (2 * (int)(i & 15))) & 3u);
+  }
+  __device__ static __forceinline__ void store16(void* species, long long g, long long, const uint32_t* vals) {
+    uint32_t packed = 0;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) packed |= vals[k] << (2 * k);
+    reinterpret_cast<uint32_t*>(species)[g] = packed;
+  }
+};
+// SMCX_STORAGE_4BIT: 4 bits per site, sublattice-planar in groups of 8 conventional cells along x (Lx is a multiple
+// of 8): group G = c >> 3 of conventional cell c = (z Ly + y) Lx + x holds B words, word b = the sites of basis
+// index b of its 8 cells, cell (c & 7) in nibble (c & 7).  A row of 8 cells of one sublattice is then one 32-bit
+// word, which is what the packed FCC kernel (sweep_fcc.cuh) gathers neighbours from.
+template <int B>
+struct Store4 {
+  static constexpr int kBits = 4;
+  __device__ static __forceinline__ int load(const void* p, long long i) {
+    const long long c = i / B;
+    const int b = (int)(i - c * B);
+    return (int)((reinterpret_cast<const uint32_t*>(p)[(c >> 3) * B + b] >> (4 * (int)(c & 7))) & 15u);
+  }
+  __device__ static __forceinline__ void store16(void* species, long long g, long long, const uint32_t* vals) {
+    if (B == 2) {             // 16 sites = 8 conventional cells = one group of two words
+      uint32_t w0 = 0, w1 = 0;
+#pragma unroll
+      for (int x = 0; x < 8; ++x) { w0 |= vals[2 * x] << (4 * x); w1 |= vals[2 * x + 1] << (4 * x); }
+      reinterpret_cast<uint2*>(species)[g] = make_uint2(w0, w1);
+    } else {                  // 16 sites = 4 conventional cells = half of each of the group's four words
+      uint16_t* h = reinterpret_cast<uint16_t*>(species) + (g >> 1) * 8 + (g & 1);
+#pragma unroll
+      for (int b = 0; b < 4; ++b) {
+        uint32_t v = 0;
+#pragma unroll
+        for (int x = 0; x < 4; ++x) v |= vals[4 * x + b] << (4 * x);
+        h[2 * b] = (uint16_t)v;
+      }
+    }
   }
 };
 
@@ -45,28 +94,16 @@ __global__ void init_species_kernel(void* __restrict__ species, long long n_site
   const long long n_groups = (n_sites + 15) >> 4;
   for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
        g += (long long)gridDim.x * blockDim.x) {
-    uint32_t packed = 0;
-    uint32_t bytes[4] = {0, 0, 0, 0};
+    uint32_t vals[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
       const long long i = g * 16 + k;
-      uint32_t s = 0;
+      vals[k] = 0;
       if (i < n_sites)
-        s = (uint32_t)(feistel_permute((unsigned long long)i, h, (unsigned long long)n_sites, k0, k1) %
-                       (unsigned long long)n_species);
-      packed |= s << (2 * k);
-      bytes[k >> 2] |= s << (8 * (k & 3));
+        vals[k] = (uint32_t)(feistel_permute((unsigned long long)i, h, (unsigned long long)n_sites, k0, k1) %
+                             (unsigned long long)n_species);
     }
-    if (Store::kBits == 2) {
-      reinterpret_cast<uint32_t*>(species)[g] = packed;
-    } else {
-      uint8_t* p = reinterpret_cast<uint8_t*>(species) + g * 16;
-      if (g * 16 + 16 <= n_sites) {
-        *reinterpret_cast<uint4*>(p) = make_uint4(bytes[0], bytes[1], bytes[2], bytes[3]);
-      } else {
-        for (int k = 0; k < 16 && g * 16 + k < n_sites; ++k) p[k] = (uint8_t)((bytes[k >> 2] >> (8 * (k & 3))) & 0xff);
-      }
-    }
+    Store::store16(species, g, n_sites, vals);
   }
 }
 
@@ -80,8 +117,7 @@ __global__ void init_composition_kernel(void* __restrict__ species, long long n_
   const long long n_groups = (n_sites + 15) >> 4;
   for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
        g += (long long)gridDim.x * blockDim.x) {
-    uint32_t packed = 0;
-    uint32_t bytes[4] = {0, 0, 0, 0};
+    uint32_t vals[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
       const long long i = g * 16 + k;
@@ -90,50 +126,77 @@ __global__ void init_composition_kernel(void* __restrict__ species, long long n_
         const long long r = (long long)feistel_permute((unsigned long long)i, h, (unsigned long long)n_sites, k0, k1);
         for (int p = 0; p < n_species - 1; ++p) s += r >= C.cum[p] ? 1u : 0u;
       }
-      packed |= s << (2 * k);
-      bytes[k >> 2] |= s << (8 * (k & 3));
+      vals[k] = s;
     }
-    if (Store::kBits == 2) {
-      reinterpret_cast<uint32_t*>(species)[g] = packed;
+    Store::store16(species, g, n_sites, vals);
+  }
+}
+
+// ---- storage conversion: uint8 site-id order <-> device storage ------------------------------
+// One thread per 16 consecutive sites.  src / dst point at a chunk of n_sites_chunk sites that starts at site
+// first_site (a multiple of 32) of the lattice; `lattice` is the whole array in device storage.  Validation is
+// fused into the packing: any source value >= n_species raises st->bad_state (the caller reads it once, after the
+// last chunk).
+template <class Store>
+__global__ void pack_kernel(const uint8_t* __restrict__ src, void* __restrict__ lattice, long long first_site,
+                            long long n_sites_chunk, int n_species, DevState* __restrict__ st) {
+  const long long n_groups = (n_sites_chunk + 15) >> 4;
+  bool bad = false;
+  for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
+       g += (long long)gridDim.x * blockDim.x) {
+    uint32_t vals[16];
+    if (g * 16 + 16 <= n_sites_chunk) {
+      const uint4 v = *reinterpret_cast<const uint4*>(src + g * 16);
+      const uint32_t w[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+      for (int k = 0; k < 16; ++k) vals[k] = (w[k >> 2] >> (8 * (k & 3))) & 0xffu;
     } else {
-      uint8_t* p = reinterpret_cast<uint8_t*>(species) + g * 16;
-      if (g * 16 + 16 <= n_sites) {
-        *reinterpret_cast<uint4*>(p) = make_uint4(bytes[0], bytes[1], bytes[2], bytes[3]);
-      } else {
-        for (int k = 0; k < 16 && g * 16 + k < n_sites; ++k) p[k] = (uint8_t)((bytes[k >> 2] >> (8 * (k & 3))) & 0xff);
-      }
+      for (int k = 0; k < 16; ++k) vals[k] = g * 16 + k < n_sites_chunk ? src[g * 16 + k] : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      bad |= vals[k] >= (uint32_t)n_species;
+      vals[k] &= (1u << Store::kBits) - 1u;
+    }
+    Store::store16(lattice, (first_site >> 4) + g, first_site + n_sites_chunk, vals);
+  }
+  if (bad) atomicOr(&st->bad_state, 1ull);
+}
+
+template <class Store>
+__global__ void unpack_kernel(const void* __restrict__ lattice, uint8_t* __restrict__ dst, long long first_site,
+                              long long n_sites_chunk) {
+  const long long n_groups = (n_sites_chunk + 15) >> 4;
+  for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
+       g += (long long)gridDim.x * blockDim.x) {
+    uint32_t vals[16];
+    if (Store::kBits == 2) {
+      const uint32_t packed = reinterpret_cast<const uint32_t*>(lattice)[(first_site >> 4) + g];
+#pragma unroll
+      for (int k = 0; k < 16; ++k) vals[k] = (packed >> (2 * k)) & 3u;
+    } else {
+#pragma unroll
+      for (int k = 0; k < 16; ++k) vals[k] = (uint32_t)Store::load(lattice, first_site + g * 16 + k);
+    }
+    if (g * 16 + 16 <= n_sites_chunk) {
+      uint32_t w[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+      for (int k = 0; k < 16; ++k) w[k >> 2] |= vals[k] << (8 * (k & 3));
+      *reinterpret_cast<uint4*>(dst + g * 16) = make_uint4(w[0], w[1], w[2], w[3]);
+    } else {
+      for (int k = 0; k < 16; ++k)
+        if (g * 16 + k < n_sites_chunk) dst[g * 16 + k] = (uint8_t)vals[k];
     }
   }
 }
 
-// ---- storage conversion: uint8 site-id order <-> packed 2-bit ------------------------------
-__global__ void pack2_kernel(const uint8_t* __restrict__ src, uint32_t* __restrict__ dst, long long first_site,
-                             long long n_sites_chunk) {
-  // first_site is a multiple of 16; src points at the chunk, dst at the whole packed array.
-  const long long n_groups = (n_sites_chunk + 15) >> 4;
-  for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
-       g += (long long)gridDim.x * blockDim.x) {
-    uint32_t packed = 0;
-    for (int k = 0; k < 16; ++k) {
-      const long long i = g * 16 + k;
-      const uint32_t s = i < n_sites_chunk ? src[i] : 0u;
-      packed |= (s & 3u) << (2 * k);
-    }
-    dst[(first_site >> 4) + g] = packed;
-  }
-}
-
-__global__ void unpack2_kernel(const uint32_t* __restrict__ src, uint8_t* __restrict__ dst, long long first_site,
-                               long long n_sites_chunk) {
-  const long long n_groups = (n_sites_chunk + 15) >> 4;
-  for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
-       g += (long long)gridDim.x * blockDim.x) {
-    const uint32_t packed = src[(first_site >> 4) + g];
-    for (int k = 0; k < 16; ++k) {
-      const long long i = g * 16 + k;
-      if (i < n_sites_chunk) dst[i] = (uint8_t)((packed >> (2 * k)) & 3u);
-    }
-  }
+// Flags any field >= n_species in an array in device storage (smcx_set_species_packed).
+template <class Store>
+__global__ void validate_storage_kernel(const void* __restrict__ lattice, long long n_sites, int n_species, DevState* st) {
+  bool bad = false;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n_sites; i += (long long)gridDim.x * blockDim.x)
+    bad |= Store::load(lattice, i) >= n_species;
+  if (bad) atomicOr(&st->bad_state, 1ull);
 }
 
 // Flags any byte >= n_species.

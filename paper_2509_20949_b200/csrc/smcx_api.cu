@@ -19,6 +19,7 @@
 #include "ensemble_kernels.cuh"
 #include "lattice_kernels.cuh"
 #include "smcx_common.cuh"
+#include "sweep_fcc.cuh"
 #include "sweep_group.cuh"
 #include "sweep_thread.cuh"
 #include "sweep_warp.cuh"
@@ -79,7 +80,7 @@ inline int floor_div2(int v) { return v >= 0 ? v / 2 : -((-v + 1) / 2); }
 inline bool is_thread_kernel(int k) { return k == SMCX_KERNEL_THREAD_PER_CELL || k == SMCX_KERNEL_THREAD_PERSISTENT; }
 
 struct Layout {
-  size_t species, epi, coef, gtable, accept, filter, trace, state, counts, total;
+  size_t species, epi, coef, gtable, fcc_lut, fcc_corr, accept, filter, trace, state, counts, total;
 };
 
 struct Plan {
@@ -92,10 +93,19 @@ struct Plan {
   int group_warps;  // its warps per block
   int coef_class;   // build_thread_coefficients: 2 = the filter variant of the thread kernel applies
   bool coef_packed; // pack_thread_coefficients: the 16-bit coefficient rows are exact
+  int fcc_rep;      // sweep_fcc_thread: replicas of the look-up rows in shared memory
+  FccTables fcc_tables;
   Layout lay;
 };
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+size_t storage_bytes(int storage, long long n_sites) {
+  if (storage == SMCX_STORAGE_U8) return (size_t)n_sites;
+  if (storage == SMCX_STORAGE_2BIT) return (size_t)((n_sites + 15) / 16) * 4;
+  return (size_t)((n_sites + 7) / 8) * 4;   // 4BIT
+}
+
 
 int make_plan(const smcx_params_t* p, Plan* plan) {
   if (!p || !plan) return SMCX_E_NULL_ARG;
@@ -188,9 +198,22 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     int32_t pk[16 * 4];
     plan->coef_packed = fast_ok && pack_thread_coefficients(coef, pk);
   }
+  // packed FCC kernel: geometry, and every EPI difference must fit the 16-bit look-up
+  bool fcc_ok = fcc_kernel_supported(G);
+  plan->fcc_rep = 1;
+  if (fcc_ok) {
+    std::vector<uint32_t> lut;
+    std::vector<int32_t> corr;
+    fcc_ok = fcc_build_lut(p->epi, n, p->n_shells, 1, lut, corr) && fcc_build_tables<32>(G, plan->fcc_tables);
+    plan->fcc_rep = fcc_lut_rep(n);
+  }
   int kernel = p->kernel, storage = p->storage;
   if (kernel == SMCX_KERNEL_AUTO) {
-    if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_GROUP_PER_CELL;
+    // FCC: the packed thread-per-cell kernel once every warp of every SM gets a batch of 32 cells; below that a pass
+    // lasts as long as one cell's chain of trials, which is shorter with several lanes per cell
+    if (fcc_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && n_cells / 8 >= 148ll * kFccWarps * 32)))
+      kernel = SMCX_KERNEL_FCC_THREAD;
+    else if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_GROUP_PER_CELL;
     else if (!fast_ok) kernel = SMCX_KERNEL_GROUP_PER_CELL;
     // The persistent kernel (one block of 20 warps and ~220 KB of shared memory per SM) pays off once
     // every warp of every SM gets a batch of 32 cells.  Below that a colour pass is as long as one
@@ -203,12 +226,17 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     if (!fast_ok) return SMCX_E_UNSUPPORTED;
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_2BIT;
     if (storage != SMCX_STORAGE_2BIT) return SMCX_E_UNSUPPORTED;
+  } else if (kernel == SMCX_KERNEL_FCC_THREAD) {
+    if (!fcc_ok) return SMCX_E_UNSUPPORTED;
+    if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_4BIT;
+    if (storage != SMCX_STORAGE_4BIT) return SMCX_E_UNSUPPORTED;
   } else if (kernel == SMCX_KERNEL_WARP_PER_CELL || kernel == SMCX_KERNEL_GROUP_PER_CELL) {
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_U8;
     if (storage != SMCX_STORAGE_U8) return SMCX_E_UNSUPPORTED;
   } else {
     return SMCX_E_UNSUPPORTED;
   }
+  if (storage == SMCX_STORAGE_4BIT && (G.Lx & 7) != 0) return SMCX_E_UNSUPPORTED;
   plan->kernel = kernel;
   plan->storage = storage;
   // sub-warp kernel: lanes per cell by the number of cells of a colour.  With few cells a pass is as long as
@@ -245,10 +273,12 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   Layout& L = plan->lay;
   size_t off = 0;
   L.species = off;
-  off += align_up(storage == SMCX_STORAGE_U8 ? (size_t)n_sites : (size_t)((n_sites + 15) / 16) * 4, 256);
+  off += align_up(storage_bytes(storage, n_sites), 256);
   L.epi = off;     off += align_up((size_t)p->n_shells * n * n * sizeof(int32_t), 256);
   L.coef = off;    off += align_up((size_t)16 * (kCoefInts + 4) * sizeof(int32_t), 256);
   L.gtable = off;  off += align_up((size_t)group_smem_layout(G, plan->group_lanes).d_bytes, 256);   // sub-warp kernel's difference table
+  L.fcc_lut = off; off += align_up((size_t)64 * 3 * 8 * 16, 256);                                   // packed FCC kernel's look-up rows
+  L.fcc_corr = off; off += align_up((size_t)64 * sizeof(int32_t), 256);
   L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
   L.filter = off;  off += align_up((size_t)kFilterWords * sizeof(uint32_t), 256);
   L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
@@ -262,7 +292,8 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
 
 // kernels that read the two-level acceptance filter tables
 inline bool uses_filter(const Plan& P) {
-  return (is_thread_kernel(P.kernel) && P.coef_class == 2) || P.kernel == SMCX_KERNEL_GROUP_PER_CELL;
+  return (is_thread_kernel(P.kernel) && P.coef_class == 2) || P.kernel == SMCX_KERNEL_GROUP_PER_CELL ||
+         P.kernel == SMCX_KERNEL_FCC_THREAD;
 }
 
 struct smcx {
@@ -277,7 +308,11 @@ struct smcx {
   cudaEvent_t staging_ev[kStagingSlots] = {nullptr, nullptr, nullptr, nullptr};
   size_t staging_cap = 0;
   int staging_next = 0;
-  uint8_t* bounce = nullptr;  // device, kChunkSites bytes, lazily allocated
+  // packed <-> uint8 host transfers: two device bounce buffers of kChunkSites bytes (lazily allocated), a copy
+  // stream, and per buffer the events "filled" / "free again"
+  uint8_t* bounce[2] = {nullptr, nullptr};
+  cudaStream_t copy_stream = nullptr;
+  cudaEvent_t bounce_full[2] = {nullptr, nullptr}, bounce_free[2] = {nullptr, nullptr};
   long long sweeps_enqueued = 0;
   long long trace_first = 0;  // first sweep whose energy the trace holds (smcx_set_sweep_counter moves it)
   long long launches = 0;
@@ -294,6 +329,8 @@ struct smcx {
   int32_t* d_epi() const { return reinterpret_cast<int32_t*>(ws + plan.lay.epi); }
   int32_t* d_coef() const { return reinterpret_cast<int32_t*>(ws + plan.lay.coef); }
   int32_t* d_gtable() const { return reinterpret_cast<int32_t*>(ws + plan.lay.gtable); }
+  uint32_t* d_fcc_lut() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.fcc_lut); }
+  int32_t* d_fcc_corr() const { return reinterpret_cast<int32_t*>(ws + plan.lay.fcc_corr); }
   uint32_t* d_accept() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.accept); }
   uint32_t* d_filter() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.filter); }
   long long* d_trace() const { return reinterpret_cast<long long*>(ws + plan.lay.trace); }
@@ -326,6 +363,15 @@ struct DeviceGuard {
   DeviceGuard& operator=(const DeviceGuard&) = delete;
 };
 
+// `Store` = accessor of the handle's device storage (lattice_kernels.cuh) inside the statement(s) given
+#define SMCX_STORE_DISPATCH(P, ...)                                                              \
+  do {                                                                                           \
+    if ((P).storage == SMCX_STORAGE_U8) { using Store = StoreU8; __VA_ARGS__; }                  \
+    else if ((P).storage == SMCX_STORAGE_2BIT) { using Store = Store2; __VA_ARGS__; }            \
+    else if ((P).G.B == 2) { using Store = Store4<2>; __VA_ARGS__; }                             \
+    else { using Store = Store4<4>; __VA_ARGS__; }                                               \
+  } while (0)
+
 int grid_for(const smcx* h, long long work_items, int block) {
   const long long want = (work_items + block - 1) / block;
   const long long cap = (long long)h->sm_count * 16;
@@ -337,10 +383,8 @@ int launch_init(smcx* h) {
   int hh = 1;
   while ((1ull << (2 * hh)) < (unsigned long long)P.n_sites) ++hh;
   const int grid = grid_for(h, (P.n_sites + 15) / 16, 256);
-  if (P.storage == SMCX_STORAGE_U8)
-    init_species_kernel<StoreU8><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh, P.G.key0, P.G.key1);
-  else
-    init_species_kernel<Store2><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh, P.G.key0, P.G.key1);
+  SMCX_STORE_DISPATCH(P, init_species_kernel<Store><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh,
+                                                                                   P.G.key0, P.G.key1));
   h->launches++;
   SMCX_CUDA(h, cudaGetLastError());
   return SMCX_OK;
@@ -360,12 +404,10 @@ int run_pair_counts(smcx* h, std::vector<unsigned long long>& host_M) {
     // bit-parallel reduction: one thread per packed word (16 sites)
     const int gridw = grid_for(h, n_conv / 8, 256);
     pair_count_bcc2_kernel<<<gridw, 256, 0, h->stream>>>(G, reinterpret_cast<const uint32_t*>(h->d_species()), h->d_counts());
-  } else if (P.storage == SMCX_STORAGE_U8) {
-    if (G.B == 2) pair_count_kernel<StoreU8, 2><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
-    else          pair_count_kernel<StoreU8, 4><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
+  } else if (G.B == 2) {
+    SMCX_STORE_DISPATCH(P, pair_count_kernel<Store, 2><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts()));
   } else {
-    if (G.B == 2) pair_count_kernel<Store2, 2><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
-    else          pair_count_kernel<Store2, 4><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts());
+    SMCX_STORE_DISPATCH(P, pair_count_kernel<Store, 4><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_counts()));
   }
   h->launches++;
   SMCX_CUDA(h, cudaGetLastError());
@@ -426,7 +468,13 @@ int upload_table(smcx* h, const uint32_t* accept, int len) {
 }
 
 int ensure_bounce(smcx* h) {
-  if (!h->bounce) SMCX_CUDA(h, cudaMalloc(&h->bounce, (size_t)kChunkSites));
+  const size_t chunk = (size_t)std::min<long long>(kChunkSites, h->plan.n_sites);
+  for (int k = 0; k < 2; ++k) {
+    if (!h->bounce[k]) SMCX_CUDA(h, cudaMalloc(&h->bounce[k], chunk));
+    if (!h->bounce_full[k]) SMCX_CUDA(h, cudaEventCreateWithFlags(&h->bounce_full[k], cudaEventDisableTiming));
+    if (!h->bounce_free[k]) SMCX_CUDA(h, cudaEventCreateWithFlags(&h->bounce_free[k], cudaEventDisableTiming));
+  }
+  if (!h->copy_stream) SMCX_CUDA(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
   return SMCX_OK;
 }
 
@@ -448,6 +496,13 @@ int launch_colour_pass(smcx* h, int colour) {
                                           h->d_filter(), h->d_state(), colour, h->stream);
     h->launches++;
     if (rc != 0) { h->err = "thread-per-cell launch failed"; return SMCX_E_CUDA; }
+    return SMCX_OK;
+  }
+  if (P.kernel == SMCX_KERNEL_FCC_THREAD) {
+    const int rc = launch_fcc_thread(G, P.fcc_tables, reinterpret_cast<uint32_t*>(h->d_species()), h->d_fcc_lut(), h->d_fcc_corr(),
+                                     P.fcc_rep, h->d_accept(), h->d_filter(), h->d_state(), colour, h->sm_count, h->stream);
+    h->launches++;
+    if (rc != 0) { h->err = "packed FCC thread-per-cell launch failed"; return SMCX_E_CUDA; }
     return SMCX_OK;
   }
   if (P.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
@@ -564,6 +619,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     if (cudaEventCreateWithFlags(&h->staging_ev[s], cudaEventDisableTiming) != cudaSuccess) return fail(SMCX_E_CUDA);
   }
   if (configure_thread_per_cell() != 0) return fail(SMCX_E_CUDA);
+  if (h->plan.kernel == SMCX_KERNEL_FCC_THREAD && configure_fcc_thread(h->plan.fcc_rep) != 0) return fail(SMCX_E_CUDA);
   // every kernel of a sweep prefers the largest shared-memory carve-out: an SM whose carve-out must
   // change drains first, which serialises lattices that run concurrently (replica ensembles:
   // measured 45 us instead of 28 us per colour pass when the one-thread epilogue asked for the default)
@@ -609,6 +665,13 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
       group_build_table(h->plan.G, h->plan.group_lanes, h->epi.data(), gtab);
       SMCX_CUDA(h, cudaMemcpyAsync(h->d_gtable(), gtab.data(), gtab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
     }
+    std::vector<uint32_t> flut;
+    std::vector<int32_t> fcorr;
+    if (h->plan.kernel == SMCX_KERNEL_FCC_THREAD) {
+      fcc_build_lut(h->epi.data(), h->plan.G.n_species, h->plan.G.n_shells, h->plan.fcc_rep, flut, fcorr);
+      SMCX_CUDA(h, cudaMemcpyAsync(h->d_fcc_lut(), flut.data(), flut.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, h->stream));
+      SMCX_CUDA(h, cudaMemcpyAsync(h->d_fcc_corr(), fcorr.data(), fcorr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+    }
     SMCX_CUDA(h, cudaMemsetAsync(h->d_trace(), 0, (size_t)h->plan.G.trace_capacity * sizeof(long long), h->stream));
     SMCX_CUDA(h, cudaStreamSynchronize(h->stream));  // &zero and epi must stay valid until copied
     int r = upload_table(h, p->accept, p->accept_len);
@@ -632,10 +695,27 @@ void smcx_destroy(smcx_t* h) {
   }
   if (h->sweep_graph) cudaGraphExecDestroy(h->sweep_graph);
   if (h->capture_stream) cudaStreamDestroy(h->capture_stream);
-  if (h->bounce) cudaFree(h->bounce);
+  for (int k = 0; k < 2; ++k) {
+    if (h->bounce[k]) cudaFree(h->bounce[k]);
+    if (h->bounce_full[k]) cudaEventDestroy(h->bounce_full[k]);
+    if (h->bounce_free[k]) cudaEventDestroy(h->bounce_free[k]);
+  }
+  if (h->copy_stream) cudaStreamDestroy(h->copy_stream);
   if (h->owns_ws && h->ws) cudaFree(h->ws);
   cudaGetLastError();
   delete h;
+}
+
+// Did a validation kernel flag a value >= n_species since clear_bad_state()?  Synchronises.
+static int clear_bad_state(smcx* h) {
+  SMCX_CUDA(h, cudaMemsetAsync(&h->d_state()->bad_state, 0, sizeof(unsigned long long), h->stream));
+  return SMCX_OK;
+}
+static int check_bad_state(smcx* h) {
+  unsigned long long bad = 0;
+  SMCX_CUDA(h, cudaMemcpyAsync(&bad, &h->d_state()->bad_state, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  return bad ? SMCX_E_BAD_STATE : SMCX_OK;
 }
 
 int smcx_set_species_device(smcx_t* h, const void* d_src) {
@@ -643,43 +723,89 @@ int smcx_set_species_device(smcx_t* h, const void* d_src) {
   DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   const uint8_t* src = reinterpret_cast<const uint8_t*>(d_src);
-  unsigned long long zero = 0;
-  SMCX_CUDA(h, cudaMemcpyAsync(&h->d_state()->bad_state, &zero, sizeof(zero), cudaMemcpyHostToDevice, h->stream));
+  int rc = clear_bad_state(h);
+  if (rc != SMCX_OK) return rc;
+  // validated before anything is written: on SMCX_E_BAD_STATE the lattice is unchanged
   validate_u8_kernel<<<grid_for(h, P.n_sites, 256), 256, 0, h->stream>>>(src, P.n_sites, P.G.n_species, h->d_state());
   h->launches++;
-  unsigned long long bad = 0;
-  SMCX_CUDA(h, cudaMemcpyAsync(&bad, &h->d_state()->bad_state, sizeof(bad), cudaMemcpyDeviceToHost, h->stream));
-  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
-  if (bad) return SMCX_E_BAD_STATE;
+  rc = check_bad_state(h);
+  if (rc != SMCX_OK) return rc;
   if (P.storage == SMCX_STORAGE_U8) {
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_species(), src, (size_t)P.n_sites, cudaMemcpyDeviceToDevice, h->stream));
   } else {
-    pack2_kernel<<<grid_for(h, (P.n_sites + 15) / 16, 256), 256, 0, h->stream>>>(src, reinterpret_cast<uint32_t*>(h->d_species()), 0, P.n_sites);
+    SMCX_STORE_DISPATCH(P, pack_kernel<Store><<<grid_for(h, (P.n_sites + 15) / 16, 256), 256, 0, h->stream>>>(
+                               src, h->d_species(), 0, P.n_sites, P.G.n_species, h->d_state()));
     h->launches++;
     SMCX_CUDA(h, cudaGetLastError());
   }
   return reset_running_energy(h);
 }
 
+// Host upload.  The values are validated on the device while they are packed (no pass over the array on the
+// host): on SMCX_E_BAD_STATE the lattice has been overwritten with the low bits of the rejected array and must
+// be set again.  Packed storage: chunks of 2^26 sites through two device bounce buffers, the copy of chunk k + 1
+// on the copy stream overlapping the packing of chunk k.
 int smcx_set_species(smcx_t* h, const uint8_t* host_src) {
   if (!h || !host_src) return SMCX_E_NULL_ARG;
   DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
-  for (long long i = 0; i < P.n_sites; ++i)
-    if (host_src[i] >= P.G.n_species) return SMCX_E_BAD_STATE;
+  int rc = clear_bad_state(h);
+  if (rc != SMCX_OK) return rc;
   if (P.storage == SMCX_STORAGE_U8) {
     SMCX_CUDA(h, cudaMemcpyAsync(h->d_species(), host_src, (size_t)P.n_sites, cudaMemcpyHostToDevice, h->stream));
+    validate_u8_kernel<<<grid_for(h, P.n_sites, 256), 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, h->d_state());
+    h->launches++;
   } else {
-    int rc = ensure_bounce(h);
+    rc = ensure_bounce(h);
     if (rc != SMCX_OK) return rc;
-    for (long long first = 0; first < P.n_sites; first += kChunkSites) {
+    SMCX_CUDA(h, cudaEventRecord(h->bounce_free[0], h->stream));   // the bounce buffers are free once earlier work is done
+    SMCX_CUDA(h, cudaEventRecord(h->bounce_free[1], h->stream));
+    int k = 0;
+    for (long long first = 0; first < P.n_sites; first += kChunkSites, k ^= 1) {
       const long long cnt = std::min(kChunkSites, P.n_sites - first);
-      SMCX_CUDA(h, cudaMemcpyAsync(h->bounce, host_src + first, (size_t)cnt, cudaMemcpyHostToDevice, h->stream));
-      pack2_kernel<<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(h->bounce, reinterpret_cast<uint32_t*>(h->d_species()), first, cnt);
+      SMCX_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->bounce_free[k], 0));
+      SMCX_CUDA(h, cudaMemcpyAsync(h->bounce[k], host_src + first, (size_t)cnt, cudaMemcpyHostToDevice, h->copy_stream));
+      SMCX_CUDA(h, cudaEventRecord(h->bounce_full[k], h->copy_stream));
+      SMCX_CUDA(h, cudaStreamWaitEvent(h->stream, h->bounce_full[k], 0));
+      SMCX_STORE_DISPATCH(P, pack_kernel<Store><<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(
+                                 h->bounce[k], h->d_species(), first, cnt, P.G.n_species, h->d_state()));
       h->launches++;
       SMCX_CUDA(h, cudaGetLastError());
+      SMCX_CUDA(h, cudaEventRecord(h->bounce_free[k], h->stream));
     }
   }
+  rc = check_bad_state(h);
+  if (rc != SMCX_OK) return rc;
+  return reset_running_energy(h);
+}
+
+int smcx_storage_bytes(smcx_t* h, size_t* bytes) {
+  if (!h || !bytes) return SMCX_E_NULL_ARG;
+  *bytes = storage_bytes(h->plan.storage, h->plan.n_sites);
+  return SMCX_OK;
+}
+
+int smcx_species_packed(smcx_t* h, void* host_dst) {
+  if (!h || !host_dst) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
+  SMCX_CUDA(h, cudaMemcpyAsync(host_dst, h->d_species(), storage_bytes(h->plan.storage, h->plan.n_sites),
+                               cudaMemcpyDeviceToHost, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  return SMCX_OK;
+}
+
+int smcx_set_species_packed(smcx_t* h, const void* host_src) {
+  if (!h || !host_src) return SMCX_E_NULL_ARG;
+  DeviceGuard on_device(h->device);
+  const Plan& P = h->plan;
+  int rc = clear_bad_state(h);
+  if (rc != SMCX_OK) return rc;
+  SMCX_CUDA(h, cudaMemcpyAsync(h->d_species(), host_src, storage_bytes(P.storage, P.n_sites), cudaMemcpyHostToDevice, h->stream));
+  SMCX_STORE_DISPATCH(P, validate_storage_kernel<Store><<<grid_for(h, P.n_sites, 256), 256, 0, h->stream>>>(
+                             h->d_species(), P.n_sites, P.G.n_species, h->d_state()));
+  h->launches++;
+  rc = check_bad_state(h);
+  if (rc != SMCX_OK) return rc;
   return reset_running_energy(h);
 }
 
@@ -698,10 +824,8 @@ int smcx_init_composition(smcx_t* h, const int64_t* counts) {
   int hh = 1;
   while ((1ull << (2 * hh)) < (unsigned long long)P.n_sites) ++hh;
   const int grid = grid_for(h, (P.n_sites + 15) / 16, 256);
-  if (P.storage == SMCX_STORAGE_U8)
-    init_composition_kernel<StoreU8><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh, P.G.key0, P.G.key1, C);
-  else
-    init_composition_kernel<Store2><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh, P.G.key0, P.G.key1, C);
+  SMCX_STORE_DISPATCH(P, init_composition_kernel<Store><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh,
+                                                                                       P.G.key0, P.G.key1, C));
   h->launches++;
   SMCX_CUDA(h, cudaGetLastError());
   return reset_running_energy(h);
@@ -822,14 +946,16 @@ int smcx_species_device(smcx_t* h, void* d_dst) {
   if (P.storage == SMCX_STORAGE_U8) {
     SMCX_CUDA(h, cudaMemcpyAsync(d_dst, h->d_species(), (size_t)P.n_sites, cudaMemcpyDeviceToDevice, h->stream));
   } else {
-    unpack2_kernel<<<grid_for(h, (P.n_sites + 15) / 16, 256), 256, 0, h->stream>>>(
-        reinterpret_cast<const uint32_t*>(h->d_species()), reinterpret_cast<uint8_t*>(d_dst), 0, P.n_sites);
+    SMCX_STORE_DISPATCH(P, unpack_kernel<Store><<<grid_for(h, (P.n_sites + 15) / 16, 256), 256, 0, h->stream>>>(
+                               h->d_species(), reinterpret_cast<uint8_t*>(d_dst), 0, P.n_sites));
     h->launches++;
     SMCX_CUDA(h, cudaGetLastError());
   }
   return SMCX_OK;
 }
 
+// Packed storage: chunk k is unpacked into bounce buffer k & 1 on the handle's stream and copied to the host on
+// the copy stream while chunk k + 1 is being unpacked; one synchronisation at the end.
 int smcx_species(smcx_t* h, uint8_t* host_dst) {
   if (!h || !host_dst) return SMCX_E_NULL_ARG;
   DeviceGuard on_device(h->device);
@@ -841,15 +967,23 @@ int smcx_species(smcx_t* h, uint8_t* host_dst) {
   }
   int rc = ensure_bounce(h);
   if (rc != SMCX_OK) return rc;
-  for (long long first = 0; first < P.n_sites; first += kChunkSites) {
+  SMCX_CUDA(h, cudaEventRecord(h->bounce_free[0], h->stream));
+  SMCX_CUDA(h, cudaEventRecord(h->bounce_free[1], h->stream));
+  int k = 0;
+  for (long long first = 0; first < P.n_sites; first += kChunkSites, k ^= 1) {
     const long long cnt = std::min(kChunkSites, P.n_sites - first);
-    unpack2_kernel<<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(
-        reinterpret_cast<const uint32_t*>(h->d_species()), h->bounce, first, cnt);
+    SMCX_CUDA(h, cudaStreamWaitEvent(h->stream, h->bounce_free[k], 0));
+    SMCX_STORE_DISPATCH(P, unpack_kernel<Store><<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(
+                               h->d_species(), h->bounce[k], first, cnt));
     h->launches++;
     SMCX_CUDA(h, cudaGetLastError());
-    SMCX_CUDA(h, cudaMemcpyAsync(host_dst + first, h->bounce, (size_t)cnt, cudaMemcpyDeviceToHost, h->stream));
-    SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+    SMCX_CUDA(h, cudaEventRecord(h->bounce_full[k], h->stream));
+    SMCX_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->bounce_full[k], 0));
+    SMCX_CUDA(h, cudaMemcpyAsync(host_dst + first, h->bounce[k], (size_t)cnt, cudaMemcpyDeviceToHost, h->copy_stream));
+    SMCX_CUDA(h, cudaEventRecord(h->bounce_free[k], h->copy_stream));
   }
+  SMCX_CUDA(h, cudaStreamSynchronize(h->copy_stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
   return SMCX_OK;
 }
 

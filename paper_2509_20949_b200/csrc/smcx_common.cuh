@@ -61,6 +61,7 @@ struct DevState {
   long long e_run;               // running energy E_0 + sum of accepted dE
   unsigned long long accepted;   // accepted swaps
   unsigned long long bad_state;  // set by validation kernels
+  unsigned work[8];              // per colour: batches of cells handed out so far in this sweep (sweep_fcc_thread); zeroed by sweep_epilogue
 };
 
 // Lattice + link-cell geometry and the shell-offset tables.  Passed to kernels by value, i.e. it

@@ -169,6 +169,7 @@ __global__ void sweep_epilogue(DevState* st, long long* trace, int trace_capacit
   const unsigned long long t = st->sweep;
   trace[t % (unsigned long long)trace_capacity] = st->e_run;
   st->sweep = t + 1ull;
+  for (int c = 0; c < 8; ++c) st->work[c] = 0u;
 }
 
 }  // namespace smcxk

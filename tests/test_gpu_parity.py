@@ -103,7 +103,8 @@ def test_config2_anneal_full_length():
     assert (g.energy_trace() == o.energy_trace()).all()
 
 
-@pytest.mark.parametrize("kernel", [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_GROUP_PER_CELL], ids=["warp", "group"])
+@pytest.mark.parametrize("kernel", [smcx.KERNEL_WARP_PER_CELL, smcx.KERNEL_GROUP_PER_CELL, smcx.KERNEL_FCC_THREAD],
+                         ids=["warp", "group", "fcc_thread"])
 def test_config3_fcc_five_species_prefix(kernel):
     cfg = get_config(3)
     g, o = _pair(cfg, kernel)
@@ -474,3 +475,129 @@ def test_sub_warp_kernel_table_formats(lanes, amplitude, kT):
     _assert_same_state(g, o)
     assert (g.energy_trace() == o.energy_trace()).all() and g.stats() == o.stats()
     assert g.stats()[2] > 0
+
+
+# ---- packed FCC kernel (SMCX_KERNEL_FCC_THREAD, SMCX_STORAGE_4BIT) -------------------------------------------------
+@pytest.mark.parametrize("dims,n_sp,n_sh,amp,kT", [
+    ((16, 16, 16), 5, 3, 400, 690),      # config 3's parameters in small
+    ((24, 16, 8), 8, 3, 400, 860),       # most species the look-up takes, one cell per colour along z
+    ((16, 8, 24), 2, 2, 300, 500),       # two shells: the third shell's rows are zero
+    ((40, 24, 16), 5, 3, 15_000, 9_000), # differences that need the high byte of the look-up in full
+    ((32, 32, 32), 3, 3, 400, 430),      # more than one batch of 32 cells per colour (64)
+])
+def test_packed_fcc_kernel_against_the_oracle(dims, n_sp, n_sh, amp, kT):
+    lat, w, seed = 1, 4, 515
+    epi = make_epi(n_sh, n_sp, amp, seed)
+    table = make_accept_table(kT)
+    g = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, seed, link_cell=w, kT_units=kT, kernel=smcx.KERNEL_FCC_THREAD)
+    assert g.storage == smcx.STORAGE_4BIT and g.kernel == smcx.KERNEL_FCC_THREAD
+    o = oracle.Oracle(lat, dims, n_sp, n_sh, epi, w, table, seed)
+    _assert_same_state(g, o)                       # S6 through Store4
+    assert g.energy() == o.energy() == g.running_energy()
+    for _ in range(4):
+        g.sweep(1)
+        o.sweep(1)
+        _assert_same_state(g, o)
+    g.sweep(3)                                     # graph replay
+    o.sweep(3)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.stats() == o.stats() and g.stats()[2] > 0
+    assert g.energy() == o.energy() == g.running_energy()
+    _assert_sro(g, o)                              # pair counts on 4-bit storage
+
+
+def test_p14_four_bit_and_uint8_storage_agree():
+    """P14: SMCX_STORAGE_4BIT (packed FCC kernel) and SMCX_STORAGE_U8 (sub-warp and warp kernels) give identical
+    smcx_species, traces and pair counts, on the paper's composition with stage-wise cooling."""
+    from smcx_inputs import composition_counts, cooling_stages
+    lat, dims, n_sp, n_sh, w, seed = 1, (32, 16, 16), 5, 3, 4, 77
+    epi = make_epi(n_sh, n_sp, 400, seed)
+    stages = cooling_stages(1720, 860, 3)
+    tables = [make_accept_table(k) for k in stages]
+    hs = [smcx.Lattice(lat, dims, n_sp, n_sh, epi, tables[0], seed, link_cell=w, kT_units=stages[0], kernel=k)
+          for k in (smcx.KERNEL_FCC_THREAD, smcx.KERNEL_GROUP_PER_CELL, smcx.KERNEL_WARP_PER_CELL)]
+    assert [h.storage for h in hs] == [smcx.STORAGE_4BIT, smcx.STORAGE_U8, smcx.STORAGE_U8]
+    counts = composition_counts(hs[0].n_sites, (29, 29, 28, 7, 7))
+    for h in hs:
+        h.init_composition(counts)
+    for kT, tab in zip(stages, tables):
+        for h in hs:
+            h.set_temperature(kT, tab)
+            h.sweep(3)
+        for h in hs[1:]:
+            assert (hs[0].species() == h.species()).all()
+            assert (hs[0].sro()[1] == h.sro()[1]).all()
+    for h in hs[1:]:
+        assert (hs[0].energy_trace() == h.energy_trace()).all() and hs[0].stats() == h.stats()
+
+
+@pytest.mark.parametrize("storage,lat,dims,n_sp,kernel", [
+    (smcx.STORAGE_2BIT, 0, (16, 24, 16), 4, smcx.KERNEL_THREAD_PER_CELL),
+    (smcx.STORAGE_4BIT, 1, (16, 16, 24), 7, smcx.KERNEL_FCC_THREAD),
+    (smcx.STORAGE_U8, 1, (16, 16, 8), 5, smcx.KERNEL_GROUP_PER_CELL),
+])
+def test_packed_checkpoint_roundtrip(storage, lat, dims, n_sp, kernel):
+    """smcx_species_packed / smcx_set_species_packed: the device storage format as a checkpoint (1/4, 1/2 or 1 byte per
+    site); a new handle given the packed array and the sweep counter continues bit for bit; invalid fields are refused."""
+    n_sh = 2 if lat == 0 else 3
+    epi = make_epi(n_sh, n_sp, 300, 9)
+    table = make_accept_table(600)
+    kw = dict(link_cell=4, kT_units=600, kernel=kernel)
+    a = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, 9, **kw)
+    assert a.storage == storage
+    assert a.storage_bytes() == a.n_sites * {2: 1, 4: 2, 8: 4}[storage] // 4
+    a.sweep(3)
+    packed, species, t = a.species_packed().copy(), a.species().copy(), a.stats()[0]
+    a.sweep(2)
+    b = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, 9, **kw)
+    b.set_species_packed(packed)
+    assert (b.species() == species).all() and b.energy() == b.running_energy()
+    b.set_sweep_counter(t)
+    b.sweep(2)
+    assert (a.species() == b.species()).all() and (a.energy_trace(3, 2) == b.energy_trace(3, 2)).all()
+    if storage != smcx.STORAGE_U8 and n_sp < (1 << storage):
+        packed[5] = 0xFF                             # fields 15 / 3 >= n_species
+        with pytest.raises(smcx.SmcxError) as ei:
+            b.set_species_packed(packed)
+        assert ei.value.code == -9
+    # uint8 upload / download through the same storage
+    rng = np.random.default_rng(1)
+    s = rng.integers(0, n_sp, a.n_sites).astype(np.uint8)
+    b.set_species(s)
+    assert (b.species() == s).all() and (b.species_device().cpu().numpy() == s).all()
+    s[11] = n_sp
+    with pytest.raises(smcx.SmcxError):
+        b.set_species(s)
+
+
+def test_paper_shaped_fcc_full_size_invariants():
+    """The lattice bench.py times as `paper_shaped_fcc` (FCC 400^3, 29/29/28/7/7, three shells) in the launch
+    configuration it is timed in (AUTO -> packed FCC kernel): conservation, energy bookkeeping, H = 1/2 sum V N; and the
+    same build against the oracle on a 96 x 80 x 64 box (ragged batches: 12 * 10 * 8 / 8 = 120 cells per colour)."""
+    from smcx_inputs import composition_counts
+    epi, table = make_epi(3, 5, 400, 1006), make_accept_table(860)
+    g = smcx.Lattice(smcx.FCC, (400, 400, 400), 5, 3, epi, table, 1006, link_cell=4, kT_units=860)
+    assert g.kernel == smcx.KERNEL_FCC_THREAD and g.storage == smcx.STORAGE_4BIT
+    counts = composition_counts(g.n_sites, (29, 29, 28, 7, 7))
+    g.init_composition(counts)
+    _, c0 = g.sro()
+    assert (c0[0].sum(axis=1) // 12 == np.array(counts)).all()
+    assert g.energy() == g.running_energy()
+    g.sweep(3)
+    _, c1 = g.sro()
+    assert (c1[0].sum(axis=1) // 12 == np.array(counts)).all() and (c1 == c1.transpose(0, 2, 1)).all()
+    assert g.energy() == g.running_energy() == g.energy_trace()[-1]
+    assert int((epi.astype(np.int64) * c1).sum()) == 2 * g.energy()
+    assert 0 < g.stats()[2] < g.stats()[1]
+    g.close()
+    dims = (96, 80, 64)
+    s = smcx.Lattice(smcx.FCC, dims, 5, 3, epi, table, 1006, link_cell=4, kT_units=860, kernel=smcx.KERNEL_FCC_THREAD)
+    o = oracle.Oracle(smcx.FCC, dims, 5, 3, epi, 4, table, 1006, threads=ALL_CORES)
+    cs = composition_counts(s.n_sites, (29, 29, 28, 7, 7))
+    s.init_composition(cs)
+    o.init_composition(cs)
+    s.sweep(3)
+    o.sweep(3)
+    _assert_same_state(s, o)
+    assert (s.energy_trace() == o.energy_trace()).all() and s.stats() == o.stats()

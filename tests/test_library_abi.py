@@ -64,6 +64,18 @@ def test_parameter_validation_codes():
     assert _code(accept=np.zeros(0, np.uint32)) == E["BAD_TABLE"]
     assert _code(storage=smcx.STORAGE_2BIT, kernel=smcx.KERNEL_WARP_PER_CELL) == E["UNSUPPORTED"]
     assert _code(lattice=1, n_shells=3, epi=make_epi(3, 4, 300, 1), kernel=smcx.KERNEL_THREAD_PER_CELL) == E["UNSUPPORTED"]
+    # 4-bit storage belongs to the packed FCC kernel
+    assert _code(storage=smcx.STORAGE_4BIT) == E["UNSUPPORTED"]                                  # BCC
+    fcc = dict(lattice=1, n_shells=3, n_species=5, epi=make_epi(3, 5, 400, 1))
+    assert _code(storage=smcx.STORAGE_4BIT, kernel=smcx.KERNEL_GROUP_PER_CELL, **fcc) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_FCC_THREAD, storage=smcx.STORAGE_U8, **fcc) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_FCC_THREAD, lattice=1, n_shells=3, n_species=9, epi=make_epi(3, 9, 400, 1)) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_FCC_THREAD, lattice=1, n_shells=3, n_species=5, epi=make_epi(3, 5, 20_000, 1)) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_FCC_THREAD, dims=(16, 16, 16), link_cell=2, **fcc) == E["UNSUPPORTED"]
+    n4 = workspace_bytes(**_kw(kernel=smcx.KERNEL_FCC_THREAD, dims=(32, 16, 16), **fcc))
+    n8 = workspace_bytes(**_kw(kernel=smcx.KERNEL_GROUP_PER_CELL, dims=(32, 16, 16), **fcc))
+    assert 0 < n8 - n4 <= 32 * 16 * 16 * 4 // 2 + 4096 and n4 >= 32 * 16 * 16 * 4 // 2
+    assert workspace_bytes(**_kw(storage=smcx.STORAGE_4BIT, **fcc)) > 0                        # AUTO kernel follows the storage
     # explicit launch shape of the sub-warp kernel (smcx_params_t::group_lanes / group_warps; 0 = auto)
     assert _code(kernel=smcx.KERNEL_GROUP_PER_CELL, group_lanes=5) == E["UNSUPPORTED"]
     assert _code(kernel=smcx.KERNEL_GROUP_PER_CELL, group_lanes=64) == E["UNSUPPORTED"]
