@@ -50,23 +50,60 @@ def measured_peak():
         return FALLBACK_HBM_GBS, "fallback"
 
 
-# What binds the thread-per-cell kernels is the integer ALU pipe: instructions per trial on that
-# pipe from the SASS of the trial loop plus the share of the staging / write-back code (profiles/), the cycles an
-# IMAD.WIDE / POPC holds the pipe from profiles/r1_pipe_microbench.md.
-ALU_PIPE = {2: {"alu_inst": 59.0, "wide": 9.0, "popc": 6.0}, 3: {"alu_inst": 50.5, "wide": 7.5, "popc": 6.0}}   # session 7 SASS: 47.4 in the trial loop + ~3 outside
+KERNEL_NAMES = {1: "sweep_warp_per_cell", 2: "sweep_thread_per_cell", 3: "sweep_thread_persistent", 4: "sweep_group_per_cell",
+                5: "sweep_fcc_thread"}
+STORAGE_NAMES = {2: "2bit", 4: "4bit", 8: "u8"}
+# Sources a kernel is compiled from: a number taken from an ncu capture (DRAM traffic, instruction counts per trial)
+# is only reported next to live timings while these files are what they were at the capture.
+KERNEL_SOURCES = {
+    1: ["sweep_warp.cuh", "smcx_common.cuh"],
+    2: ["sweep_thread.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
+    3: ["sweep_thread.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
+    4: ["sweep_group.cuh", "sweep_thread.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
+    5: ["sweep_fcc.cuh", "sweep_thread.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
+}
+CAPTURES = os.path.join(ROOT, "profiles", "dram_traffic.csv")
 
 
-def alu_view(kernel: int, trials_per_s: float, clocks: dict):
-    if kernel not in ALU_PIPE:
+def kernel_source_hash(kernel: int) -> str:
+    import hashlib
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES[kernel]:
+        with open(os.path.join(ROOT, "paper_2509_20949_b200", "csrc", name), "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:12]
+
+
+def load_capture(kernel: int, n_sites: int):
+    """The committed ncu capture of this kernel on this workload (profiles/dram_traffic.csv), or (None, why)."""
+    if not os.path.exists(CAPTURES):
+        return None, "no capture file"
+    want = kernel_source_hash(kernel)
+    stale = None
+    for line in open(CAPTURES):
+        f = [x.strip() for x in line.split(",")]
+        if len(f) < 8 or not f[0].isdigit() or int(f[0]) != kernel or int(f[1]) != n_sites:
+            continue
+        row = {"dram_bytes": float(f[2]), "source_hash": f[3], "alu_inst": float(f[4]), "wide": float(f[5]), "popc": float(f[6]),
+               "capture": f[7]}
+        if row["source_hash"] == want:
+            return row, None
+        stale = f"kernel sources changed since the capture {row['capture']} (hash {row['source_hash']} -> {want}): take a new one"
+    return None, stale or "no capture of this kernel on this workload"
+
+
+def alu_view(capture, trials_per_s: float, clocks: dict):
+    """The integer ALU pipe is what binds the thread-per-cell kernels: instructions per trial on that pipe
+    and the cycles an IMAD.WIDE / POPC holds it (profiles/r1_pipe_microbench.md), from the capture the sources match."""
+    if capture is None:
         return None
-    k = ALU_PIPE[kernel]
     mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
     peak = 148 * 4 * mhz * 1e6 / 2.0                      # ALU-pipe warp-instructions/s: 1 per 2 cycles per sub-partition
-    inst = trials_per_s / 32.0 * k["alu_inst"]
-    busy = trials_per_s / 32.0 * (2.0 * k["alu_inst"] + 2.6 * k["wide"] + 1.0 * k["popc"]) / (148 * 4 * mhz * 1e6)
+    inst = trials_per_s / 32.0 * capture["alu_inst"]
+    busy = trials_per_s / 32.0 * (2.0 * capture["alu_inst"] + 2.6 * capture["wide"] + 1.0 * capture["popc"]) / (148 * 4 * mhz * 1e6)
     return {"bound": "alu", "achieved": inst, "peak": peak, "unit": "warp-inst/s", "frac": inst / peak,
-            "alu_inst_per_trial": k["alu_inst"], "pipe_busy_frac_with_wide_and_popc": busy,
-            "note": "whole-step trials/s; counts from SASS + ncu in profiles/"}
+            "alu_inst_per_trial": capture["alu_inst"], "pipe_busy_frac_with_wide_and_popc": busy,
+            "note": f"whole-step trials/s; instruction counts from {capture['capture']}"}
 
 
 def workload_string(cfg) -> str:
@@ -258,18 +295,9 @@ def run_ensemble(n_replicas: int, rounds: int = 20, sweeps_per_round: int = 10):
     return out
 
 
-def run_paper_shaped_fcc(edge: int = 400, sweeps: int = 10):
-    """A lattice of the paper's own shape (PAPER.md:141, 163-165): FCC, five species in the proportions
-    29/29/28/7/7 (reading S10), three shells, kT = 86 meV, synthetic EPI; the sub-warp kernel, device-timed."""
+def _time_sweeps(lat, warm: int, sweeps: int) -> float:
     import torch
-    import paper_2509_20949_b200 as smcx
-    from smcx_inputs import composition_counts, make_accept_table, make_epi
-
-    dims = (edge, edge, edge)
-    lat = smcx.Lattice(smcx.FCC, dims, 5, 3, make_epi(3, 5, 400, 1006), make_accept_table(860), 1006, link_cell=4,
-                       kT_units=860)
-    lat.init_composition(composition_counts(lat.n_sites, (29, 29, 28, 7, 7)))
-    lat.sweep(3)
+    lat.sweep(warm)
     lat.synchronize()
     a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     a.record()
@@ -277,11 +305,51 @@ def run_paper_shaped_fcc(edge: int = 400, sweeps: int = 10):
     b.record()
     lat.synchronize()
     torch.cuda.synchronize()
-    ms = a.elapsed_time(b) / sweeps
-    out = {"workload": f"FCC {edge}^3 conventional cells ({lat.n_sites} sites), 5 species 29/29/28/7/7, 3-shell int32 EPI in "
-                       f"[-400,400], kT=86 meV, link cell 4, seed 1006", "kernel": "sweep_group_per_cell/u8",
-           "value": lat.n_sites / (ms * 1e-3), "unit": "trial swaps/s", "sweep_ms": ms,
-           "paper_h800_per_gpu": 3.5e9, "paper_note": "PAPER.md:130, EPI model on H800; other hardware and interactions: context"}
+    return a.elapsed_time(b) / sweeps
+
+
+def run_paper_shaped_fcc(edge: int = 400, sweeps: int = 10):
+    """A lattice of the paper's own shape (PAPER.md:141, 163-165): FCC, five species in the proportions
+    29/29/28/7/7 (reading S10), three shells, kT = 86 meV, synthetic EPI; the kernel AUTO picks (packed FCC kernel on
+    4-bit storage) and, beside it, the sub-warp kernel on uint8 storage; device-timed."""
+    import paper_2509_20949_b200 as smcx
+    from smcx_inputs import composition_counts, make_accept_table, make_epi
+
+    dims = (edge, edge, edge)
+    peak, _ = measured_peak()
+    out = {}
+    for key, kernel in (("auto", smcx.KERNEL_AUTO), ("sub_warp", smcx.KERNEL_GROUP_PER_CELL)):
+        lat = smcx.Lattice(smcx.FCC, dims, 5, 3, make_epi(3, 5, 400, 1006), make_accept_table(860), 1006, link_cell=4,
+                           kT_units=860, kernel=kernel)
+        lat.init_composition(composition_counts(lat.n_sites, (29, 29, 28, 7, 7)))
+        ms = _time_sweeps(lat, 3, sweeps)
+        out[key] = {"kernel": f"{KERNEL_NAMES[lat.kernel]}/{STORAGE_NAMES[lat.storage]}", "value": lat.n_sites / (ms * 1e-3),
+                    "sweep_ms": ms}
+        n_sites = lat.n_sites
+        lat.close()
+    v = out["auto"]["value"]
+    return {"workload": f"FCC {edge}^3 conventional cells ({n_sites} sites), 5 species 29/29/28/7/7, 3-shell int32 EPI in "
+                        f"[-400,400], kT=86 meV, link cell 4, seed 1006", "kernel": out["auto"]["kernel"],
+            "value": v, "unit": "trial swaps/s", "sweep_ms": out["auto"]["sweep_ms"],
+            "frac_of_hbm_roofline": v * ALGO_BYTES_PER_TRIAL / (peak * 1e9),
+            "algorithmic_bytes_per_trial": ALGO_BYTES_PER_TRIAL,
+            "device_bytes_per_trial_4bit": 8 * (0.5 + 0.5 * 36 / 64.0),
+            "sub_warp_kernel": out["sub_warp"],
+            "paper_h800_per_gpu": 3.5e9, "paper_note": "PAPER.md:130, EPI model on H800; other hardware and interactions: context"}
+
+
+def run_largest_single_gpu(sweeps: int = 20):
+    """BASELINE.json configs[4]: BCC 2000^3, 1.6e10 sites (4 GB in 2-bit storage), device-timed."""
+    import paper_2509_20949_b200 as smcx
+
+    cfg = get_config(5)
+    peak, _ = measured_peak()
+    lat = smcx.Lattice.from_config(cfg)
+    ms = _time_sweeps(lat, 3, sweeps)
+    v = cfg.n_sites / (ms * 1e-3)
+    out = {"workload": workload_string(cfg), "config_id": 5, "kernel": f"{KERNEL_NAMES[lat.kernel]}/{STORAGE_NAMES[lat.storage]}",
+           "sweeps": sweeps, "value": v, "unit": "trial swaps/s", "sweep_ms": ms,
+           "frac_of_hbm_roofline": v * ALGO_BYTES_PER_TRIAL / (peak * 1e9)}
     lat.close()
     return out
 
@@ -395,13 +463,12 @@ def run_cuda(args, cfg, rank, world, local_rank):
         # dominant kernel: one colour pass = n_sites/8 trials per launch, 8 launches per sweep
         launch_ms = sweep_ms / (8.0 * args.steps)
         achieved = ALGO_BYTES_PER_TRIAL * (cfg.n_sites / 8.0) / (launch_ms * 1e-3) / 1e9
-        traffic = None   # measured dram bytes per launch from the committed ncu capture, if it matches this run
-        tp = os.path.join(ROOT, "profiles", "dram_traffic.csv")
-        if os.path.exists(tp):
-            for line in open(tp):
-                f = line.strip().split(",")
-                if len(f) == 3 and f[0].isdigit() and int(f[0]) == lat.kernel and int(f[1]) == cfg.n_sites:
-                    traffic = float(f[2])
+        # DRAM bytes per launch and instruction counts come from an ncu capture: reported only while the kernel's
+        # sources are what they were when it was taken, null (with the reason) otherwise
+        capture, capture_note = load_capture(lat.kernel, cfg.n_sites)
+        traffic = capture["dram_bytes"] if capture else None
+        dev_bytes = cfg.n_sites * {2: 0.25, 4: 0.5, 8: 1.0}[lat.storage]
+        frac = achieved / peak
         out = {
             "metric": metric_name(), "value": value, "unit": "trial swaps/s", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak",
@@ -410,18 +477,27 @@ def run_cuda(args, cfg, rank, world, local_rank):
                 "workload": workload_string(cfg), "config_id": args.config,
                 "step": f"1 sweep = 8 colour-pass launches + trace; pair-count/SRO reduction every {sro_every} sweeps "
                         f"and once at the end ({n_sro} inside the timed region)",
-                "kernel": {1: "warp_per_cell/u8", 2: "thread_per_cell/2bit", 3: "thread_persistent/2bit", 4: "group_per_cell/u8"}[lat.kernel],
-                "l2": "lattice (%.0f MB in device storage) larger than the 126 MB L2; no flush" %
-                      (cfg.n_sites * (0.25 if lat.storage == 2 else 1.0) / 1e6),
+                "kernel": f"{KERNEL_NAMES[lat.kernel]}/{STORAGE_NAMES[lat.storage]}",
+                "l2": ("lattice (%.0f MB in device storage) larger than the 126 MB L2; no flush" % (dev_bytes / 1e6))
+                      if dev_bytes > 126e6 else
+                      ("lattice (%.1f MB in device storage) fits the 126 MB L2 and stays resident between sweeps; no flush: "
+                       "this configuration is latency-bound, not a bandwidth measurement" % (dev_bytes / 1e6)),
                 "parallelism": "replicas only" if world > 1 else "single GPU",
             },
             "pct_of_hbm_roofline": 100.0 * (value / world) * ALGO_BYTES_PER_TRIAL / (peak * 1e9),
             "sweep_ms": sweep_ms / args.steps, "sro_ms_each": sro_ms / max(1, n_sro),
-            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                         "traffic": traffic, "peak_kind": peak_kind,
-                         "kernel": {1: "sweep_warp_per_cell", 2: "sweep_thread_per_cell", 3: "sweep_thread_persistent", 4: "sweep_group_per_cell"}[lat.kernel],
-                         "algorithmic_bytes_per_trial": ALGO_BYTES_PER_TRIAL, "launch_ms": launch_ms},
-            "alu_view": alu_view(lat.kernel, value / world, clocks),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": frac,
+                         "traffic": traffic, "traffic_note": capture_note, "peak_kind": peak_kind,
+                         "kernel": KERNEL_NAMES[lat.kernel],
+                         "what": "achieved = ALGORITHMIC bytes (uint8, SURVEY.md 8(d)) per launch / measured launch time, as "
+                                 "north_star declares the roofline; the bytes the kernel really moves are in `dram`",
+                         "algorithmic_bytes_per_trial": ALGO_BYTES_PER_TRIAL, "launch_ms": launch_ms,
+                         "north_star_target_frac": 0.5, "target_met": bool(frac >= 0.5)},
+            # what the kernel moves (packed storage): measured DRAM bytes per launch / live launch time
+            "dram": ({"bytes_per_launch": traffic, "achieved_gbs": traffic / (launch_ms * 1e-3) / 1e9,
+                      "frac_of_peak": traffic / (launch_ms * 1e-3) / 1e9 / peak, "source": capture["capture"]}
+                     if capture else None),
+            "alu_view": alu_view(capture, value / world, clocks),
             "e2e": {"value": e2e_value, "unit": "trial swaps/s", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                     "steps": e2e_steps,
                     "what": "smcx_set_species(host) + steps x (smcx_set_temperature(host table) + smcx_sweep(1) + "
@@ -440,6 +516,8 @@ def run_cuda(args, cfg, rank, world, local_rank):
             out["temperature_parallel"] = run_ensemble(args.ensemble)
             if args.fcc_edge > 0:
                 out["paper_shaped_fcc"] = run_paper_shaped_fcc(args.fcc_edge)
+            if args.largest and args.config != 5:
+                out["largest_single_gpu"] = run_largest_single_gpu()
         print(json.dumps(out))
     lat.close()
     if world > 1:
@@ -454,15 +532,22 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="cuda", choices=["cuda", "reference"])
     ap.add_argument("--config", type=int, default=4, help="BASELINE.json config 1..5 (default: 4, the graded one)")
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 warp-per-cell, 2 thread-per-cell, 3 thread-per-cell persistent, 4 sub-warp group per cell")
-    ap.add_argument("--storage", type=int, default=0, help="0 auto, 2 packed 2-bit, 8 uint8")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 warp-per-cell, 2 thread-per-cell, 3 thread-per-cell persistent, 4 sub-warp group per cell, 5 packed FCC thread-per-cell")
+    ap.add_argument("--storage", type=int, default=0, help="0 auto, 2 packed 2-bit, 4 packed 4-bit, 8 uint8")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--fcc-edge", type=int, default=400,
                     help="with --ensemble: also time the sub-warp kernel on an FCC lattice of the paper's shape, this many "
                          "conventional cells per edge (0: skip)")
+    ap.add_argument("--no-largest", dest="largest", action="store_false",
+                    help="skip the BCC 2000^3 (1.6e10 sites) leg that the default run adds as `largest_single_gpu`")
+    ap.add_argument("--source-hash", action="store_true", help="print the source hash of every kernel (for profiles/dram_traffic.csv) and exit")
     ap.add_argument("--ensemble", type=int, default=128,
                     help="also time a replica-exchange ensemble of this many BCC 64^3 replicas (0: skip)")
     args = ap.parse_args()
+    if args.source_hash:
+        for k in sorted(KERNEL_SOURCES):
+            print(k, KERNEL_NAMES[k], kernel_source_hash(k))
+        return
     args.warmup = max(args.warmup, 3) if args.impl == "cuda" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
