@@ -60,6 +60,8 @@ def _load():
         "oracle_lc_valid": (C.c_int, [C.c_void_p]),
         "oracle_sweep_lc": (C.c_int, [C.c_void_p, C.c_int64, C.c_int, C.c_uint32]),
         "oracle_sweep_seq": (None, [C.c_void_p, C.c_int64]),
+        "oracle_sweep_lc_slabs": (C.c_int64, [C.c_void_p, C.c_int64, C.c_int, C.c_int, C.c_int, C.c_uint32]),
+        "oracle_slab_partition": (C.c_int, [C.c_void_p, C.c_int, i32p]),
         "oracle_set_threads": (C.c_int, [C.c_void_p, C.c_int]),
         "oracle_shift": (None, [C.c_void_p, C.c_uint32, i32p]),
         "oracle_stats": (None, [C.c_void_p, i64p, i64p, i64p]),
@@ -228,6 +230,23 @@ class Oracle:
     def sweep(self, n: int = 1, order_mode: int = 0, order_seed: int = 0):
         if self._lib.oracle_sweep_lc(self._h, int(n), int(order_mode), int(order_seed)) != 0:
             raise ValueError("lattice dimensions not divisible by 2*link_cell")
+
+    def sweep_slabs(self, n: int, n_slabs: int, ghost: int = 2, exchange: bool = True, order_seed: int = 0) -> int:
+        """S11: n link-cell sweeps with the lattice cut into n_slabs slabs along z, each holding
+        only its window (ghost layers included) and exchanging boundary layers after every colour pass.  Returns
+        the number of reads of sites a slab did not hold (0 when the protocol is right)."""
+        bad = int(self._lib.oracle_sweep_lc_slabs(self._h, int(n), int(n_slabs), int(ghost), 1 if exchange else 0,
+                                                  int(order_seed)))
+        if bad < 0:
+            raise ValueError("the lattice cannot be cut into that many slabs (pairs of link-cell rows)")
+        return bad
+
+    def slab_partition(self, n_slabs: int):
+        """[(first link-cell row, number of rows)] of the n_slabs slabs (reading S11)."""
+        rows = np.zeros(2 * int(n_slabs), dtype=np.int32)
+        if self._lib.oracle_slab_partition(self._h, int(n_slabs), _ptr(rows, C.c_int32)) != 0:
+            raise ValueError("the lattice cannot be cut into that many slabs")
+        return [(int(rows[2 * k]), int(rows[2 * k + 1])) for k in range(int(n_slabs))]
 
     def sweep_sequential(self, n: int = 1):
         self._lib.oracle_sweep_seq(self._h, int(n))

@@ -96,7 +96,10 @@ struct Oracle {
   std::vector<int64_t> trace;           // E_run after each sweep, from sweep trace_first on
   int64_t trace_first = 0;              // resume (checkpointing): the sweep counter was set to this value
   int threads = 1;                      // OpenMP threads over the cells of a colour (1 = plain loop)
+  mutable int64_t poison_reads = 0;     // S11: species values >= n_species met while evaluating energies
 };
+
+constexpr uint8_t kPoison = 255;
 
 // What a run of trials adds to the bookkeeping; one per thread when the cells of a colour are spread
 // over threads, summed into the Oracle after the loop.
@@ -192,6 +195,9 @@ inline int64_t neighbour(const Oracle& o, int64_t i, const Vec3& d) {
 }
 
 inline int32_t V(const Oracle& o, int s, int a, int b) {
+  // kPoison marks sites a slab of the decomposed sweep (S11) does not hold; reading one is a bug of the
+  // decomposition (ghost layer too thin, exchange missing), counted and answered with 0
+  if (a >= o.n_species || b >= o.n_species) { o.poison_reads++; return 0; }
   return o.epi[((size_t)s * o.n_species + a) * o.n_species + b];
 }
 
@@ -375,6 +381,149 @@ void sweep_lc(Oracle& o, int order_mode, uint32_t order_seed) {
   // S3.3
   o.trace.push_back(o.E_run);
   o.sweeps_done++;
+}
+
+// ---------------------------------------------------------------------------------------
+// S11: lattice parallelism (section "Distributed SMC-X": "the complete lattice is
+// partitioned across multiple GPUs, with a ghost layer used to exchange boundary information between
+// neighboring sublattices", Fig. 2; scaling and computation-communication overlap PAPER.md:147).
+// The paper gives no protocol.  Reading S11: the lattice is cut into D slabs along z on
+// boundaries of PAIRS of link-cell rows (so the colour of a row does not depend on the slab):
+//   pairs = (Lz / w) / 2;  slab k owns pairs/D + (k < pairs mod D) consecutive row pairs.
+// A slab owns link cells, not layers: in sweep t with origin oz its rows [r0, r1) cover the layers
+// [a, b) = [oz + r0 w, oz + r1 w) (mod Lz) and it holds a copy of the window [a - g, b + g), g = ghost
+// layers (conventional cells).  Every trial draws its random numbers from the GLOBAL cell id, slot, sweep
+// and colour (S4), so a decomposed sweep must reproduce the undivided one bit for bit; what the protocol
+// has to get right is only which copies are refreshed when:
+//   start of sweep t:  the window moves by oz(t) - oz(t-1); the layers that enter it are fetched from the
+//                      neighbour on that side (whose old window held them up to date);
+//   after colour pass c (rows of parity pz = (c >> 2) & 1 were active): a slab's bottom row (pz = 0)
+//                      modified layers [a - wr, a + w + wr), wr = layers a swap partner can lie outside its
+//                      cell = ceil(r0 / 2); the part inside the lower neighbour's window, [a - wr, a + g),
+//                      is sent down.  For pz = 1 the top row sends [b - g, b + wr) up.  One message per slab
+//                      and pass; no other row reaches a neighbour's window.
+// The implementation below keeps one full-size array per slab in which everything outside the slab's window is
+// kPoison, runs the slabs in a shuffled order inside every pass (they must commute), copies exactly the layers
+// named above, and counts reads of poisoned sites.  It is pinned against the undivided sweep (tests/
+// test_oracle_domains.py): equal arrays / traces / statistics and zero poison reads for g = H; poison reads or
+// different arrays for a thinner ghost layer or without the exchanges.
+// ---------------------------------------------------------------------------------------
+struct Slab {
+  int row_first = 0, row_count = 0;
+  std::vector<uint8_t> sig;     // N bytes; valid inside the window only
+};
+
+std::vector<Slab> slab_partition(const Oracle& o, int D) {
+  const int pairs = o.L[2] / o.w / 2;
+  std::vector<Slab> slabs((size_t)D);
+  int row = 0;
+  for (int k = 0; k < D; ++k) {
+    slabs[k].row_first = row;
+    slabs[k].row_count = 2 * (pairs / D + (k < pairs % D ? 1 : 0));
+    row += slabs[k].row_count;
+  }
+  return slabs;
+}
+
+inline int64_t layer_sites(const Oracle& o) { return (int64_t)o.L[0] * o.L[1] * o.B; }
+
+// copy `count` layers starting at global layer z0 (any integer; taken mod Lz) from src to dst
+void copy_layers(const Oracle& o, const std::vector<uint8_t>& src, std::vector<uint8_t>& dst, int z0, int count) {
+  const int64_t ls = layer_sites(o);
+  for (int k = 0; k < count; ++k) {
+    const int z = wrap(z0 + k, o.L[2]);
+    std::memcpy(dst.data() + (size_t)z * ls, src.data() + (size_t)z * ls, (size_t)ls);
+  }
+}
+
+// everything outside the window [lo, lo + count) of the slab becomes kPoison
+void poison_outside(const Oracle& o, Slab& s, int lo, int count) {
+  const int64_t ls = layer_sites(o);
+  std::vector<char> keep((size_t)o.L[2], 0);
+  for (int k = 0; k < count; ++k) keep[(size_t)wrap(lo + k, o.L[2])] = 1;
+  for (int z = 0; z < o.L[2]; ++z)
+    if (!keep[(size_t)z]) std::memset(s.sig.data() + (size_t)z * ls, kPoison, (size_t)ls);
+}
+
+void shift_origin(const Oracle& o, uint32_t t, int& ox, int& oy, int& oz) {
+  const uint32_t key[2] = {(uint32_t)(o.seed & 0xffffffffu), (uint32_t)(o.seed >> 32)};
+  const uint32_t cs[4] = {0u, 0u, t, (uint32_t)TAG_SHIFT};
+  uint32_t r[4];
+  philox4x32_10(cs, key, r);
+  ox = (int)mulhi32(r[0], (uint32_t)o.w);
+  oy = (int)mulhi32(r[1], (uint32_t)o.w);
+  oz = (int)mulhi32(r[2], (uint32_t)o.w);
+}
+
+// n sweeps of the state in o.sigma, decomposed into D slabs with `ghost` ghost layers; `exchange` = false leaves
+// the per-pass messages out (negative control).  The result is gathered back into o.sigma.  Returns the
+// number of poisoned reads, or -1 if the lattice cannot be cut into D slabs.
+int64_t sweep_lc_slabs(Oracle& o, int64_t n, int D, int ghost, bool exchange, uint32_t order_seed) {
+  const int w = o.w;
+  if (D < 2 || o.L[2] % (2 * w) || D > o.L[2] / w / 2 || ghost < 0) return -1;
+  ensure_energy(o);
+  int r0_reach = 0;
+  for (const Vec3& d : o.shell[0]) r0_reach = std::max(r0_reach, std::max(std::abs(d.x), std::max(std::abs(d.y), std::abs(d.z))));
+  const int wr = (r0_reach + 1) / 2;
+  std::vector<Slab> slabs = slab_partition(o, D);
+  const int ncx = o.L[0] / w, ncy = o.L[1] / w;
+  o.poison_reads = 0;
+  if (n <= 0) return 0;
+  int ox = 0, oy = 0, oz = 0, oz_prev = 0;
+  std::mt19937 order_rng(order_seed);
+  for (int64_t step = 0; step < n; ++step) {
+    const uint32_t t = (uint32_t)o.sweeps_done;
+    shift_origin(o, t, ox, oy, oz);
+    if (step == 0) {
+      // scatter: every slab gets its window of the first sweep and nothing else
+      for (Slab& s : slabs) {
+        s.sig = o.sigma;
+        poison_outside(o, s, oz + s.row_first * w - ghost, s.row_count * w + 2 * ghost);
+      }
+    } else if (oz != oz_prev) {
+      // the windows move by oz - oz_prev layers: fetch what enters them from the neighbour on that side
+      const int sh = oz - oz_prev;
+      for (int k = 0; k < D; ++k) {
+        Slab& s = slabs[(size_t)k];
+        const int a_old = oz_prev + s.row_first * w, b_old = a_old + s.row_count * w;
+        if (sh > 0) copy_layers(o, slabs[(size_t)((k + 1) % D)].sig, s.sig, b_old + ghost, sh);
+        else        copy_layers(o, slabs[(size_t)((k + D - 1) % D)].sig, s.sig, a_old - ghost + sh, -sh);
+      }
+      for (Slab& s : slabs) poison_outside(o, s, oz + s.row_first * w - ghost, s.row_count * w + 2 * ghost);
+    }
+    oz_prev = oz;
+    for (int colour = 0; colour < 8; ++colour) {
+      const int pz = (colour >> 2) & 1;
+      std::vector<int> order((size_t)D);
+      for (int k = 0; k < D; ++k) order[(size_t)k] = k;
+      std::shuffle(order.begin(), order.end(), order_rng);
+      Tally total;
+      for (int k : order) {
+        Slab& s = slabs[(size_t)k];
+        std::swap(o.sigma, s.sig);               // the slab's private copy is the lattice while its cells run
+        for (int cz = s.row_first; cz < s.row_first + s.row_count; ++cz)
+          for (int cy = 0; cy < ncy; ++cy)
+            for (int cx = 0; cx < ncx; ++cx)
+              if (((cx & 1) | ((cy & 1) << 1) | ((cz & 1) << 2)) == colour)
+                run_cell(o, total, (uint32_t)((cz * ncy + cy) * ncx + cx), colour, t, ox, oy, oz);
+        std::swap(o.sigma, s.sig);
+      }
+      add_tally(o, total);
+      if (!exchange) continue;
+      // one message per slab: the active boundary row's modified layers that lie in the neighbour's window
+      for (int k = 0; k < D; ++k) {
+        const Slab& s = slabs[(size_t)k];
+        const int a = oz + s.row_first * w, b = a + s.row_count * w;
+        if (pz == 0) copy_layers(o, s.sig, slabs[(size_t)((k + D - 1) % D)].sig, a - wr, wr + ghost);
+        else         copy_layers(o, s.sig, slabs[(size_t)((k + 1) % D)].sig, b - ghost, ghost + wr);
+      }
+    }
+    o.trace.push_back(o.E_run);
+    o.sweeps_done++;
+  }
+  // gather: every layer from the slab whose rows cover it under the last origin
+  for (const Slab& s : slabs) copy_layers(o, s.sig, o.sigma, oz + s.row_first * w, s.row_count * w);
+  return o.poison_reads;
 }
 
 // S8: plain single-site-sequential Metropolis (no link cells); used for the exact
@@ -662,6 +811,22 @@ int oracle_set_threads(void* h, int n) {
   o.threads = 1;
 #endif
   return o.threads;
+}
+
+// S11: n link-cell sweeps with the lattice cut into D slabs along z (ghost layers, exchanges after every colour
+// pass).  Returns the number of reads of sites a slab did not hold (0 for a correct protocol), -1 if the
+// lattice cannot be cut that way.
+int64_t oracle_sweep_lc_slabs(void* h, int64_t n, int D, int ghost, int exchange, uint32_t order_seed) {
+  return sweep_lc_slabs(*(Oracle*)h, n, D, ghost, exchange != 0, order_seed);
+}
+
+// The slab partition itself: rows[2 k] = first link-cell row of slab k, rows[2 k + 1] = its number of rows.
+int oracle_slab_partition(void* h, int D, int* rows) {
+  Oracle& o = *(Oracle*)h;
+  if (D < 1 || o.L[2] % (2 * o.w) || D > o.L[2] / o.w / 2) return -1;
+  const std::vector<Slab> slabs = slab_partition(o, D);
+  for (int k = 0; k < D; ++k) { rows[2 * k] = slabs[(size_t)k].row_first; rows[2 * k + 1] = slabs[(size_t)k].row_count; }
+  return 0;
 }
 
 void oracle_sweep_seq(void* h, int64_t n) {
