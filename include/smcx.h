@@ -120,6 +120,8 @@ typedef struct {
   int32_t group_lanes;      /* GROUP_PER_CELL: lanes per link cell, 4 | 8 | 16 | 32; 0 = chosen from the cells per colour.
                                A value whose tiles do not fit shared memory is ignored (auto). */
   int32_t group_warps;      /* GROUP_PER_CELL: warps per block, 1..8; 0 = as many as leave room for four blocks per SM */
+  int32_t domain_count;     /* 0 or 1: the handle holds the whole lattice.  Set by smcx_domain_create (>= 2: the handle holds */
+  int32_t domain_index;     /* slab domain_index of dims cut into domain_count slabs along z); leave both 0 otherwise */
 } smcx_params_t;
 
 /* Bytes of device workspace a handle with these parameters needs (species array in its storage
@@ -259,6 +261,113 @@ int smcx_ensemble_state(smcx_ensemble_t *e, int32_t *replica_at_slot, int64_t *e
                         int64_t *attempted, int64_t *accepted, int32_t *last_flags, int64_t *rounds);
 int smcx_ensemble_synchronize(smcx_ensemble_t *e);
 int64_t smcx_ensemble_kernel_launches(smcx_ensemble_t *e); /* ensemble kernels + those of all replicas */
+
+/* ---- Lattice parallelism: slabs with ghost layers, computation-communication overlap ---------------------------
+ * PAPER.md:85 (section "Distributed SMC-X"): "the complete lattice is partitioned across multiple GPUs, with a ghost
+ * layer used to exchange boundary information between neighboring sublattices" (Fig. 2); "We also
+ * implemented a computing-communication overlap for EPI_GPU" (strong scaling 0.339 -> 0.679 on 16 GPUs).  The paper
+ * gives no protocol; reading S11:
+ *   - the lattice is cut along z into n_domains slabs on boundaries of PAIRS of link-cell rows: with
+ *     pairs = dims[2] / link_cell / 2, slab k owns pairs / n + (k < pairs mod n) consecutive pairs (n <= pairs);
+ *   - a slab owns link cells, not layers: in a sweep with origin oz its rows [r0, r1) cover the layers
+ *     [a, b) = [oz + r0 w, oz + r1 w) (mod dims[2]).  It stores, without wrap, the layers r0 w - H .. r1 w + w - 2 + H
+ *     (H = 2 ghost layers: the LIZ+ reaches r0 + R = 3 half-units): every window [a - H, b + H) for oz < w;
+ *   - random numbers are keyed by the GLOBAL cell id, so the decomposed sweep reproduces the undivided one bit for bit;
+ *   - start of a sweep: the window moves by oz - oz_prev layers and the layers entering it are fetched from the
+ *     neighbour on that side; after colour pass c (rows of parity pz = (c >> 2) & 1 active) the slab's bottom row
+ *     (pz = 0) sends the layers [a - 1, a + H) down, its top row (pz = 1) sends [b - H, b + 1) up: one message per slab
+ *     and pass, H + 1 layers, contiguous in device storage (layers are the slowest index of every storage format);
+ *   - overlap: a pass is launched as the boundary row first, then the message leaves on a copy stream while the
+ *     other rows of the pass run.
+ * Two ways to run it.  smcx_domain_group_*: all slabs in one process, on one or several devices, messages as
+ * device-to-device / peer copies ordered by events -- no host synchronisation inside a sweep.  smcx_domain_*: one slab
+ * per handle (one process per GPU); the caller moves the messages (e.g. torch.distributed send/recv over NCCL on the
+ * byte ranges the message calls name) between smcx_domain_pass calls. */
+typedef struct smcx_domain smcx_domain_t;
+typedef struct smcx_domain_group smcx_domain_group_t;
+
+typedef struct {
+  int32_t n_domains, index;
+  int32_t lower, upper;          /* indices of the neighbouring slabs (periodic) */
+  int32_t row_first, row_count;  /* link-cell rows along z this slab owns (both even) */
+  int32_t z_base;                /* layer of the whole lattice held in storage layer 0 (mod dims[2]) */
+  int32_t z_layers;              /* storage layers = row_count w + w - 1 + 2 ghost */
+  int32_t ghost;                 /* H */
+  int32_t storage;               /* SMCX_STORAGE_* of the slab */
+  int64_t layer_bytes;           /* bytes of one layer in device storage */
+  int64_t owned_sites;           /* row_count w dims[0] dims[1] B */
+} smcx_domain_info_t;
+
+/* One message: `bytes` bytes at byte offset `offset` of this slab's species storage (smcx_domain_storage), to / from
+ * slab `peer`.  tag 0: the message travels downwards (to the lower neighbour), 1: upwards.  The message a slab sends
+ * with tag T is the one its peer receives with tag T.  bytes = 0: no message. */
+typedef struct { int32_t peer, tag; int64_t offset, bytes; } smcx_domain_msg_t;
+
+/* The partition alone (host arithmetic, no GPU): what slab `index` of `n_domains` holds.  storage / layer_bytes are
+ * those smcx_domain_create would choose.  SMCX_E_BAD_DIMS if dims[2] has fewer than n_domains pairs of rows. */
+int smcx_domain_partition(const smcx_params_t *p, int32_t n_domains, int32_t index, smcx_domain_info_t *info);
+/* The messages of a slab, from the seed and the sweep number alone (host arithmetic, no GPU): phase -1 = window shift at
+ * the start of sweep `sweep` (needs the origins of sweeps sweep - 1 and sweep; none for sweep == first_sweep, when every
+ * layer of a window is valid), phase 0..7 = after that colour pass. */
+int smcx_domain_plan_messages(const smcx_params_t *p, int32_t n_domains, int32_t index, int64_t sweep, int64_t first_sweep,
+                              int32_t phase, smcx_domain_msg_t *send, smcx_domain_msg_t *recv);
+
+/* One slab.  p describes the WHOLE lattice (dims, seed, tables ...); p->d_workspace, if given, must hold
+ * smcx_domain_workspace_bytes().  The initial state is the slab's part of the seeded state of the whole lattice. */
+int smcx_domain_workspace_bytes(const smcx_params_t *p, int32_t n_domains, int32_t index, size_t *bytes);
+int smcx_domain_create(smcx_domain_t **out, const smcx_params_t *p, int32_t n_domains, int32_t index);
+void smcx_domain_destroy(smcx_domain_t *d);
+int smcx_domain_info(smcx_domain_t *d, smcx_domain_info_t *info);
+void *smcx_domain_storage(smcx_domain_t *d);   /* device pointer of the species storage: z_layers * layer_bytes bytes */
+/* host arrays of the WHOLE lattice (N bytes, site-id order): the slab takes its window / fills in the layers it owns */
+int smcx_domain_set_species(smcx_domain_t *d, const uint8_t *host_whole);
+int smcx_domain_species(smcx_domain_t *d, uint8_t *host_whole);
+int smcx_domain_init_composition(smcx_domain_t *d, const int64_t *counts);
+int smcx_domain_set_temperature(smcx_domain_t *d, int32_t kT_units, const uint32_t *accept, int32_t accept_len);
+int smcx_domain_set_sweep_counter(smcx_domain_t *d, int64_t t);
+/* One sweep = begin_sweep, [move the shift messages], then for colour 0..7: pass (part 0 = every row of the colour;
+ * or part 1 = the boundary row, then part 2 = the others), [move the pass messages], and end_sweep.  The caller must
+ * have completed the incoming messages of a phase (and its own outgoing ones) on the slab's stream before the next
+ * smcx_domain_pass.  send / recv may be NULL.  All asynchronous on the slab's stream. */
+int smcx_domain_begin_sweep(smcx_domain_t *d, smcx_domain_msg_t *send, smcx_domain_msg_t *recv);
+int smcx_domain_pass(smcx_domain_t *d, int32_t colour, int32_t part);
+int smcx_domain_pass_messages(smcx_domain_t *d, int32_t colour, smcx_domain_msg_t *send, smcx_domain_msg_t *recv);
+int smcx_domain_end_sweep(smcx_domain_t *d);
+/* Partial results; their sums over the slabs are those of the whole lattice.  pair_counts: positive-half counts
+ * M[s][x][y] of the bonds of the layers the slab owns; running energy / trace: the slab's share of H at the start plus
+ * the dE its cells accepted.  Synchronise the slab's stream. */
+int smcx_domain_pair_counts(smcx_domain_t *d, int64_t *half_counts);
+int smcx_domain_running_energy(smcx_domain_t *d, int64_t *E);
+int smcx_domain_energy_trace(smcx_domain_t *d, int64_t first_sweep, int64_t count, int64_t *dst);
+int smcx_domain_stats(smcx_domain_t *d, int64_t *sweeps_done, int64_t *trials, int64_t *accepted);
+int smcx_domain_synchronize(smcx_domain_t *d);
+int64_t smcx_domain_kernel_launches(smcx_domain_t *d);
+/* Eq. 8 from the positive-half counts of the whole lattice (the sum of the slabs'): alpha and ordered pair counts as
+ * smcx_sro returns them.  Host arithmetic only. */
+int smcx_sro_from_counts(const smcx_params_t *p, const int64_t *half_counts, double *alpha, int64_t *pair_counts);
+
+/* All slabs in one process.  devices: n_domains device ordinals, or NULL = all on p->device (slabs of one GPU; what
+ * the tests run).  Slabs on different devices need peer access (NVLink): SMCX_E_CUDA if a device cannot reach its
+ * neighbours.  overlap != 0: boundary row first, message in flight while the other rows run (CCO).  p->stream orders
+ * the group's calls: they fork from it and join it.  p->d_workspace is ignored (the library allocates). */
+int smcx_domain_group_create(smcx_domain_group_t **out, const smcx_params_t *p, int32_t n_domains, const int32_t *devices,
+                             int32_t overlap);
+void smcx_domain_group_destroy(smcx_domain_group_t *g);
+smcx_domain_t *smcx_domain_group_member(smcx_domain_group_t *g, int32_t k);   /* borrowed */
+int smcx_domain_group_sweep(smcx_domain_group_t *g, int64_t n);               /* asynchronous */
+int smcx_domain_group_set_temperature(smcx_domain_group_t *g, int32_t kT_units, const uint32_t *accept, int32_t accept_len);
+int smcx_domain_group_set_species(smcx_domain_group_t *g, const uint8_t *host_whole);
+int smcx_domain_group_init_composition(smcx_domain_group_t *g, const int64_t *counts);
+int smcx_domain_group_set_sweep_counter(smcx_domain_group_t *g, int64_t t);
+int smcx_domain_group_species(smcx_domain_group_t *g, uint8_t *host_whole);
+int smcx_domain_group_energy(smcx_domain_group_t *g, int64_t *E);             /* recomputed from the slabs' pair counts */
+int smcx_domain_group_running_energy(smcx_domain_group_t *g, int64_t *E);
+int smcx_domain_group_energy_trace(smcx_domain_group_t *g, int64_t first_sweep, int64_t count, int64_t *dst);
+int smcx_domain_group_sro(smcx_domain_group_t *g, double *alpha, int64_t *pair_counts);
+int smcx_domain_group_stats(smcx_domain_group_t *g, int64_t *sweeps_done, int64_t *trials, int64_t *accepted);
+int smcx_domain_group_synchronize(smcx_domain_group_t *g);
+int64_t smcx_domain_group_kernel_launches(smcx_domain_group_t *g);
+int64_t smcx_domain_group_message_bytes(smcx_domain_group_t *g);              /* bytes moved between slabs so far */
 
 const char *smcx_last_error(smcx_t *h); /* text of the last CUDA error seen by this handle */
 const char *smcx_strerror(int code);

@@ -10,5 +10,6 @@ from .binding import (  # noqa: F401
     STORAGE_AUTO, STORAGE_2BIT, STORAGE_4BIT, STORAGE_U8,
     KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT, KERNEL_GROUP_PER_CELL,
     KERNEL_FCC_THREAD,
-    SmcxError, Lattice, Ensemble, load_library, library_path, exported_symbols,
+    SmcxError, Lattice, Ensemble, Domain, DomainGroup, load_library, library_path, exported_symbols,
+    domain_partition, domain_plan_messages, sro_from_counts,
 )

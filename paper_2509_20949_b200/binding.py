@@ -32,7 +32,28 @@ class _Params(C.Structure):
         ("storage", C.c_int32), ("kernel", C.c_int32), ("device", C.c_int32), ("trace_capacity", C.c_int32),
         ("stream", C.c_void_p), ("d_workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
         ("group_lanes", C.c_int32), ("group_warps", C.c_int32),
+        ("domain_count", C.c_int32), ("domain_index", C.c_int32),
     ]
+
+
+class DomainInfo(C.Structure):
+    """smcx_domain_info_t"""
+    _fields_ = [
+        ("n_domains", C.c_int32), ("index", C.c_int32), ("lower", C.c_int32), ("upper", C.c_int32),
+        ("row_first", C.c_int32), ("row_count", C.c_int32), ("z_base", C.c_int32), ("z_layers", C.c_int32),
+        ("ghost", C.c_int32), ("storage", C.c_int32), ("layer_bytes", C.c_int64), ("owned_sites", C.c_int64),
+    ]
+
+    def as_dict(self):
+        return {k: int(getattr(self, k)) for k, _ in self._fields_}
+
+
+class DomainMsg(C.Structure):
+    """smcx_domain_msg_t"""
+    _fields_ = [("peer", C.c_int32), ("tag", C.c_int32), ("offset", C.c_int64), ("bytes", C.c_int64)]
+
+    def as_tuple(self):
+        return (int(self.peer), int(self.tag), int(self.offset), int(self.bytes))
 
 
 def library_path() -> str:
@@ -97,6 +118,47 @@ def load_library(build_if_missing: bool = True):
         "smcx_ensemble_state": (C.c_int, [vp, i32p, i64p, i64p, i64p, i32p, i64p]),
         "smcx_ensemble_synchronize": (C.c_int, [vp]),
         "smcx_ensemble_kernel_launches": (C.c_int64, [vp]),
+        "smcx_domain_partition": (C.c_int, [C.POINTER(_Params), C.c_int32, C.c_int32, C.POINTER(DomainInfo)]),
+        "smcx_domain_plan_messages": (C.c_int, [C.POINTER(_Params), C.c_int32, C.c_int32, C.c_int64, C.c_int64, C.c_int32,
+                                                C.POINTER(DomainMsg), C.POINTER(DomainMsg)]),
+        "smcx_domain_workspace_bytes": (C.c_int, [C.POINTER(_Params), C.c_int32, C.c_int32, C.POINTER(C.c_size_t)]),
+        "smcx_domain_create": (C.c_int, [C.POINTER(vp), C.POINTER(_Params), C.c_int32, C.c_int32]),
+        "smcx_domain_destroy": (None, [vp]),
+        "smcx_domain_info": (C.c_int, [vp, C.POINTER(DomainInfo)]),
+        "smcx_domain_storage": (vp, [vp]),
+        "smcx_domain_set_species": (C.c_int, [vp, C.POINTER(C.c_uint8)]),
+        "smcx_domain_species": (C.c_int, [vp, C.POINTER(C.c_uint8)]),
+        "smcx_domain_init_composition": (C.c_int, [vp, i64p]),
+        "smcx_domain_set_temperature": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_uint32), C.c_int32]),
+        "smcx_domain_set_sweep_counter": (C.c_int, [vp, C.c_int64]),
+        "smcx_domain_begin_sweep": (C.c_int, [vp, C.POINTER(DomainMsg), C.POINTER(DomainMsg)]),
+        "smcx_domain_pass": (C.c_int, [vp, C.c_int32, C.c_int32]),
+        "smcx_domain_pass_messages": (C.c_int, [vp, C.c_int32, C.POINTER(DomainMsg), C.POINTER(DomainMsg)]),
+        "smcx_domain_end_sweep": (C.c_int, [vp]),
+        "smcx_domain_pair_counts": (C.c_int, [vp, i64p]),
+        "smcx_domain_running_energy": (C.c_int, [vp, i64p]),
+        "smcx_domain_energy_trace": (C.c_int, [vp, C.c_int64, C.c_int64, i64p]),
+        "smcx_domain_stats": (C.c_int, [vp, i64p, i64p, i64p]),
+        "smcx_domain_synchronize": (C.c_int, [vp]),
+        "smcx_domain_kernel_launches": (C.c_int64, [vp]),
+        "smcx_sro_from_counts": (C.c_int, [C.POINTER(_Params), i64p, C.POINTER(C.c_double), i64p]),
+        "smcx_domain_group_create": (C.c_int, [C.POINTER(vp), C.POINTER(_Params), C.c_int32, i32p, C.c_int32]),
+        "smcx_domain_group_destroy": (None, [vp]),
+        "smcx_domain_group_member": (vp, [vp, C.c_int32]),
+        "smcx_domain_group_sweep": (C.c_int, [vp, C.c_int64]),
+        "smcx_domain_group_set_temperature": (C.c_int, [vp, C.c_int32, C.POINTER(C.c_uint32), C.c_int32]),
+        "smcx_domain_group_set_species": (C.c_int, [vp, C.POINTER(C.c_uint8)]),
+        "smcx_domain_group_init_composition": (C.c_int, [vp, i64p]),
+        "smcx_domain_group_set_sweep_counter": (C.c_int, [vp, C.c_int64]),
+        "smcx_domain_group_species": (C.c_int, [vp, C.POINTER(C.c_uint8)]),
+        "smcx_domain_group_energy": (C.c_int, [vp, i64p]),
+        "smcx_domain_group_running_energy": (C.c_int, [vp, i64p]),
+        "smcx_domain_group_energy_trace": (C.c_int, [vp, C.c_int64, C.c_int64, i64p]),
+        "smcx_domain_group_sro": (C.c_int, [vp, C.POINTER(C.c_double), i64p]),
+        "smcx_domain_group_stats": (C.c_int, [vp, i64p, i64p, i64p]),
+        "smcx_domain_group_synchronize": (C.c_int, [vp]),
+        "smcx_domain_group_kernel_launches": (C.c_int64, [vp]),
+        "smcx_domain_group_message_bytes": (C.c_int64, [vp]),
         "smcx_last_error": (C.c_char_p, [vp]),
         "smcx_strerror": (C.c_char_p, [C.c_int]),
         "smcx_version": (C.c_char_p, []),
@@ -434,3 +496,330 @@ def workspace_bytes(**kw) -> int:
     if rc != 0:
         raise SmcxError(rc, "smcx_workspace_bytes")
     return int(need.value)
+
+
+# ---- lattice parallelism (include/smcx.h, "Lattice parallelism: slabs with ghost layers") -----------------------
+def domain_partition(n_domains, index, **kw) -> dict:
+    """smcx_domain_partition: what slab `index` of `n_domains` holds (host arithmetic, no GPU needed)."""
+    lib = load_library()
+    defaults = dict(link_cell=4, kT_units=0, storage=0, kernel=0, device=0, trace_capacity=0)
+    defaults.update(kw)
+    p, _keep = _make_params(**defaults)
+    info = DomainInfo()
+    rc = lib.smcx_domain_partition(C.byref(p), int(n_domains), int(index), C.byref(info))
+    if rc != 0:
+        raise SmcxError(rc, "smcx_domain_partition")
+    return info.as_dict()
+
+
+def domain_plan_messages(n_domains, index, sweep, phase, first_sweep=0, **kw):
+    """smcx_domain_plan_messages: (send, recv), each (peer, tag, offset, bytes), of a slab in one phase
+    (-1 = window shift at the start of the sweep, 0..7 = after that colour pass).  Host arithmetic, no GPU needed."""
+    lib = load_library()
+    defaults = dict(link_cell=4, kT_units=0, storage=0, kernel=0, device=0, trace_capacity=0)
+    defaults.update(kw)
+    p, _keep = _make_params(**defaults)
+    send, recv = DomainMsg(), DomainMsg()
+    rc = lib.smcx_domain_plan_messages(C.byref(p), int(n_domains), int(index), int(sweep), int(first_sweep), int(phase),
+                                       C.byref(send), C.byref(recv))
+    if rc != 0:
+        raise SmcxError(rc, "smcx_domain_plan_messages")
+    return send.as_tuple(), recv.as_tuple()
+
+
+def sro_from_counts(half_counts, **kw):
+    """smcx_sro_from_counts: (alpha, ordered pair counts) of the whole lattice from the summed positive-half counts."""
+    lib = load_library()
+    defaults = dict(link_cell=4, kT_units=0, storage=0, kernel=0, device=0, trace_capacity=0)
+    defaults.update(kw)
+    p, _keep = _make_params(**defaults)
+    shape = (int(p.n_shells), int(p.n_species), int(p.n_species))
+    m = np.ascontiguousarray(half_counts, dtype=np.int64).reshape(shape)
+    alpha = np.zeros(shape, dtype=np.float64)
+    counts = np.zeros(shape, dtype=np.int64)
+    rc = lib.smcx_sro_from_counts(C.byref(p), m.ctypes.data_as(C.POINTER(C.c_int64)), alpha.ctypes.data_as(C.POINTER(C.c_double)),
+                                  counts.ctypes.data_as(C.POINTER(C.c_int64)))
+    if rc != 0:
+        raise SmcxError(rc, "smcx_sro_from_counts")
+    return alpha, counts
+
+
+class Domain:
+    """One smcx_domain_t: slab `index` of a lattice cut into `n_domains` slabs along z.  The workspace is a torch
+    uint8 tensor, so a caller can hand slices of the species storage (`storage_view`) to torch.distributed."""
+
+    def __init__(self, n_domains, index, lattice, dims, n_species, n_shells, epi, accept, seed, link_cell=4, kT_units=0,
+                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0, stream=None):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2509_20949_b200 needs a CUDA device; there is no CPU fallback")
+        self._lib = lib = load_library()
+        self._d = None
+        p, keep = _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage,
+                               kernel, device, trace_capacity)
+        need = C.c_size_t(0)
+        rc = lib.smcx_domain_workspace_bytes(C.byref(p), int(n_domains), int(index), C.byref(need))
+        if rc != 0:
+            raise SmcxError(rc, "smcx_domain_workspace_bytes")
+        self.device = torch.device("cuda", int(device))
+        with torch.cuda.device(self.device):
+            self._workspace = torch.empty(int(need.value), dtype=torch.uint8, device=self.device)
+            self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        p.stream = C.c_void_p(self._stream.cuda_stream)
+        p.d_workspace = C.c_void_p(self._workspace.data_ptr())
+        p.workspace_bytes = int(need.value)
+        d = C.c_void_p()
+        rc = lib.smcx_domain_create(C.byref(d), C.byref(p), int(n_domains), int(index))
+        if rc != 0:
+            raise SmcxError(rc, "smcx_domain_create")
+        self._d = d
+        del keep
+        info = DomainInfo()
+        self._check(lib.smcx_domain_info(d, C.byref(info)), "smcx_domain_info")
+        self.info = info.as_dict()
+        self.n_domains, self.index = int(n_domains), int(index)
+        self.n_species, self.n_shells = int(n_species), int(n_shells)
+        self.n_sites_whole = int(np.prod([int(x) for x in dims])) * (2 if int(lattice) == BCC else 4)
+        off = int(lib.smcx_domain_storage(d)) - self._workspace.data_ptr()
+        self._storage_view = self._workspace[off: off + self.info["z_layers"] * self.info["layer_bytes"]]
+
+    @classmethod
+    def _borrowed(cls, handle, owner, n_species, n_shells, n_sites_whole):
+        self = cls.__new__(cls)
+        self._lib = load_library()
+        self._d = C.c_void_p(handle)
+        self._owner, self._borrowed_handle = owner, True
+        self._workspace = self._storage_view = None
+        info = DomainInfo()
+        self._check(self._lib.smcx_domain_info(self._d, C.byref(info)), "smcx_domain_info")
+        self.info = info.as_dict()
+        self.n_domains, self.index = self.info["n_domains"], self.info["index"]
+        self.n_species, self.n_shells, self.n_sites_whole = int(n_species), int(n_shells), int(n_sites_whole)
+        return self
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise SmcxError(rc, what)
+
+    def close(self):
+        if getattr(self, "_borrowed_handle", False):
+            self._d = None
+            return
+        if getattr(self, "_d", None):
+            self._lib.smcx_domain_destroy(self._d)
+            self._d = None
+            self._workspace = self._storage_view = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def storage_view(self, msg):
+        """The bytes of message (peer, tag, offset, bytes) as a view of the workspace tensor."""
+        _, _, off, n = msg
+        return self._storage_view[off: off + n]
+
+    def set_species(self, whole):
+        s = np.ascontiguousarray(whole, dtype=np.uint8)
+        if s.size != self.n_sites_whole:
+            raise ValueError("the array must hold the whole lattice")
+        self._check(self._lib.smcx_domain_set_species(self._d, s.ctypes.data_as(C.POINTER(C.c_uint8))), "smcx_domain_set_species")
+
+    def species_into(self, whole):
+        """Write the layers this slab owns into `whole` (uint8 array of the whole lattice)."""
+        assert whole.dtype == np.uint8 and whole.size == self.n_sites_whole and whole.flags.c_contiguous
+        self._check(self._lib.smcx_domain_species(self._d, whole.ctypes.data_as(C.POINTER(C.c_uint8))), "smcx_domain_species")
+        return whole
+
+    def init_composition(self, counts):
+        c = np.ascontiguousarray(counts, dtype=np.int64)
+        self._check(self._lib.smcx_domain_init_composition(self._d, c.ctypes.data_as(C.POINTER(C.c_int64))), "smcx_domain_init_composition")
+
+    def set_temperature(self, kT_units, accept):
+        a = np.ascontiguousarray(accept, dtype=np.uint32)
+        self._check(self._lib.smcx_domain_set_temperature(self._d, int(kT_units), a.ctypes.data_as(C.POINTER(C.c_uint32)),
+                                                          int(a.size)), "smcx_domain_set_temperature")
+
+    def set_sweep_counter(self, t):
+        self._check(self._lib.smcx_domain_set_sweep_counter(self._d, int(t)), "smcx_domain_set_sweep_counter")
+
+    def begin_sweep(self):
+        send, recv = DomainMsg(), DomainMsg()
+        self._check(self._lib.smcx_domain_begin_sweep(self._d, C.byref(send), C.byref(recv)), "smcx_domain_begin_sweep")
+        return send.as_tuple(), recv.as_tuple()
+
+    def run_pass(self, colour, part=0):
+        self._check(self._lib.smcx_domain_pass(self._d, int(colour), int(part)), "smcx_domain_pass")
+
+    def pass_messages(self, colour):
+        send, recv = DomainMsg(), DomainMsg()
+        self._check(self._lib.smcx_domain_pass_messages(self._d, int(colour), C.byref(send), C.byref(recv)), "smcx_domain_pass_messages")
+        return send.as_tuple(), recv.as_tuple()
+
+    def end_sweep(self):
+        self._check(self._lib.smcx_domain_end_sweep(self._d), "smcx_domain_end_sweep")
+
+    def pair_counts(self) -> np.ndarray:
+        m = np.zeros((self.n_shells, self.n_species, self.n_species), dtype=np.int64)
+        self._check(self._lib.smcx_domain_pair_counts(self._d, m.ctypes.data_as(C.POINTER(C.c_int64))), "smcx_domain_pair_counts")
+        return m
+
+    def running_energy(self) -> int:
+        e = C.c_int64()
+        self._check(self._lib.smcx_domain_running_energy(self._d, C.byref(e)), "smcx_domain_running_energy")
+        return e.value
+
+    def energy_trace(self, first=0, count=None) -> np.ndarray:
+        if count is None:
+            count = self.stats()[0] - first
+        out = np.zeros(int(count), dtype=np.int64)
+        self._check(self._lib.smcx_domain_energy_trace(self._d, int(first), int(count), out.ctypes.data_as(C.POINTER(C.c_int64))),
+                    "smcx_domain_energy_trace")
+        return out
+
+    def stats(self):
+        a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
+        self._check(self._lib.smcx_domain_stats(self._d, C.byref(a), C.byref(b), C.byref(c)), "smcx_domain_stats")
+        return a.value, b.value, c.value
+
+    def synchronize(self):
+        self._check(self._lib.smcx_domain_synchronize(self._d), "smcx_domain_synchronize")
+
+    @property
+    def kernel_launches(self) -> int:
+        return int(self._lib.smcx_domain_kernel_launches(self._d))
+
+
+class DomainGroup:
+    """One smcx_domain_group_t: every slab of a lattice in this process (on one device or several), messages moved by
+    device-to-device / peer copies.  Same results as a Lattice of the whole."""
+
+    def __init__(self, n_domains, lattice, dims, n_species, n_shells, epi, accept, seed, link_cell=4, kT_units=0,
+                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, devices=None, overlap=True, trace_capacity=0):
+        import torch
+
+        if not torch.cuda.is_available():
+            raise RuntimeError("paper_2509_20949_b200 needs a CUDA device; there is no CPU fallback")
+        self._lib = lib = load_library()
+        self._g = None
+        p, keep = _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage,
+                               kernel, device, trace_capacity)
+        self.device = torch.device("cuda", int(device))
+        with torch.cuda.device(self.device):
+            self._stream = torch.cuda.current_stream(self.device)
+        p.stream = C.c_void_p(self._stream.cuda_stream)
+        dev = None
+        if devices is not None:
+            if len(devices) != n_domains:
+                raise ValueError("devices must have one entry per slab")
+            dev = (C.c_int32 * n_domains)(*[int(x) for x in devices])
+        g = C.c_void_p()
+        rc = lib.smcx_domain_group_create(C.byref(g), C.byref(p), int(n_domains), dev, 1 if overlap else 0)
+        if rc != 0:
+            raise SmcxError(rc, "smcx_domain_group_create")
+        self._g = g
+        del keep
+        self.n_domains = int(n_domains)
+        self.lattice, self.dims = int(lattice), tuple(int(d) for d in dims)
+        self.n_species, self.n_shells = int(n_species), int(n_shells)
+        self.n_sites = int(np.prod(self.dims)) * (2 if self.lattice == BCC else 4)
+        self.members = [Domain._borrowed(lib.smcx_domain_group_member(g, k), self, n_species, n_shells, self.n_sites)
+                        for k in range(self.n_domains)]
+
+    @classmethod
+    def from_config(cls, cfg, n_domains, **over):
+        kw = dict(lattice=cfg.lattice, dims=cfg.dims, n_species=cfg.n_species, n_shells=cfg.n_shells, epi=cfg.epi(),
+                  accept=cfg.accept_table(0), seed=cfg.seed, link_cell=cfg.link_cell, kT_units=cfg.kT_at(0))
+        kw.update(over)
+        return cls(n_domains, **kw)
+
+    def _check(self, rc, what):
+        if rc != 0:
+            raise SmcxError(rc, what)
+
+    def close(self):
+        if getattr(self, "_g", None):
+            for m in self.members:
+                m.close()
+            self._lib.smcx_domain_group_destroy(self._g)
+            self._g = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def sweep(self, n=1):
+        self._check(self._lib.smcx_domain_group_sweep(self._g, int(n)), "smcx_domain_group_sweep")
+
+    def set_temperature(self, kT_units, accept):
+        a = np.ascontiguousarray(accept, dtype=np.uint32)
+        self._check(self._lib.smcx_domain_group_set_temperature(self._g, int(kT_units), a.ctypes.data_as(C.POINTER(C.c_uint32)),
+                                                                int(a.size)), "smcx_domain_group_set_temperature")
+
+    def set_species(self, species):
+        s = np.ascontiguousarray(species, dtype=np.uint8)
+        if s.size != self.n_sites:
+            raise ValueError("species must have n_sites entries")
+        self._check(self._lib.smcx_domain_group_set_species(self._g, s.ctypes.data_as(C.POINTER(C.c_uint8))), "smcx_domain_group_set_species")
+
+    def init_composition(self, counts):
+        c = np.ascontiguousarray(counts, dtype=np.int64)
+        self._check(self._lib.smcx_domain_group_init_composition(self._g, c.ctypes.data_as(C.POINTER(C.c_int64))),
+                    "smcx_domain_group_init_composition")
+
+    def set_sweep_counter(self, t):
+        self._check(self._lib.smcx_domain_group_set_sweep_counter(self._g, int(t)), "smcx_domain_group_set_sweep_counter")
+
+    def species(self, out=None) -> np.ndarray:
+        if out is None:
+            out = np.empty(self.n_sites, dtype=np.uint8)
+        assert out.dtype == np.uint8 and out.size == self.n_sites and out.flags.c_contiguous
+        self._check(self._lib.smcx_domain_group_species(self._g, out.ctypes.data_as(C.POINTER(C.c_uint8))), "smcx_domain_group_species")
+        return out
+
+    def energy(self) -> int:
+        e = C.c_int64()
+        self._check(self._lib.smcx_domain_group_energy(self._g, C.byref(e)), "smcx_domain_group_energy")
+        return e.value
+
+    def running_energy(self) -> int:
+        e = C.c_int64()
+        self._check(self._lib.smcx_domain_group_running_energy(self._g, C.byref(e)), "smcx_domain_group_running_energy")
+        return e.value
+
+    def energy_trace(self, first=0, count=None) -> np.ndarray:
+        if count is None:
+            count = self.stats()[0] - first
+        out = np.zeros(int(count), dtype=np.int64)
+        self._check(self._lib.smcx_domain_group_energy_trace(self._g, int(first), int(count),
+                                                             out.ctypes.data_as(C.POINTER(C.c_int64))), "smcx_domain_group_energy_trace")
+        return out
+
+    def sro(self):
+        shape = (self.n_shells, self.n_species, self.n_species)
+        alpha = np.zeros(shape, dtype=np.float64)
+        counts = np.zeros(shape, dtype=np.int64)
+        self._check(self._lib.smcx_domain_group_sro(self._g, alpha.ctypes.data_as(C.POINTER(C.c_double)),
+                                                    counts.ctypes.data_as(C.POINTER(C.c_int64))), "smcx_domain_group_sro")
+        return alpha, counts
+
+    def stats(self):
+        a, b, c = C.c_int64(), C.c_int64(), C.c_int64()
+        self._check(self._lib.smcx_domain_group_stats(self._g, C.byref(a), C.byref(b), C.byref(c)), "smcx_domain_group_stats")
+        return a.value, b.value, c.value
+
+    def synchronize(self):
+        self._check(self._lib.smcx_domain_group_synchronize(self._g), "smcx_domain_group_synchronize")
+
+    @property
+    def kernel_launches(self) -> int:
+        return int(self._lib.smcx_domain_group_kernel_launches(self._g))
+
+    @property
+    def message_bytes(self) -> int:
+        return int(self._lib.smcx_domain_group_message_bytes(self._g))

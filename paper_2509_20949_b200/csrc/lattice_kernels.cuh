@@ -88,9 +88,11 @@ __device__ __forceinline__ unsigned long long feistel_permute(unsigned long long
 }
 
 // One thread per 16 consecutive sites (one packed word, or 16 bytes).
+// A slab window holds the sites site_offset .. site_offset + n_sites - 1 (mod n_global) of the whole lattice, whose
+// n_global sites the permutation acts on; a whole lattice has site_offset = 0, n_global = n_sites.
 template <class Store>
 __global__ void init_species_kernel(void* __restrict__ species, long long n_sites, int n_species, int h,
-                                    uint32_t k0, uint32_t k1) {
+                                    uint32_t k0, uint32_t k1, long long site_offset, long long n_global) {
   const long long n_groups = (n_sites + 15) >> 4;
   for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
        g += (long long)gridDim.x * blockDim.x) {
@@ -99,9 +101,12 @@ __global__ void init_species_kernel(void* __restrict__ species, long long n_site
     for (int k = 0; k < 16; ++k) {
       const long long i = g * 16 + k;
       vals[k] = 0;
-      if (i < n_sites)
-        vals[k] = (uint32_t)(feistel_permute((unsigned long long)i, h, (unsigned long long)n_sites, k0, k1) %
+      if (i < n_sites) {
+        long long ig = i + site_offset;
+        if (ig >= n_global) ig -= n_global;
+        vals[k] = (uint32_t)(feistel_permute((unsigned long long)ig, h, (unsigned long long)n_global, k0, k1) %
                              (unsigned long long)n_species);
+      }
     }
     Store::store16(species, g, n_sites, vals);
   }
@@ -113,7 +118,8 @@ struct CompositionCum { long long cum[kMaxSpecies]; };
 
 template <class Store>
 __global__ void init_composition_kernel(void* __restrict__ species, long long n_sites, int n_species, int h,
-                                        uint32_t k0, uint32_t k1, const CompositionCum C) {
+                                        uint32_t k0, uint32_t k1, const CompositionCum C, long long site_offset,
+                                        long long n_global) {
   const long long n_groups = (n_sites + 15) >> 4;
   for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < n_groups;
        g += (long long)gridDim.x * blockDim.x) {
@@ -123,7 +129,9 @@ __global__ void init_composition_kernel(void* __restrict__ species, long long n_
       const long long i = g * 16 + k;
       uint32_t s = 0;
       if (i < n_sites) {
-        const long long r = (long long)feistel_permute((unsigned long long)i, h, (unsigned long long)n_sites, k0, k1);
+        long long ig = i + site_offset;
+        if (ig >= n_global) ig -= n_global;
+        const long long r = (long long)feistel_permute((unsigned long long)ig, h, (unsigned long long)n_global, k0, k1);
         for (int p = 0; p < n_species - 1; ++p) s += r >= C.cum[p] ? 1u : 0u;
       }
       vals[k] = s;
@@ -221,9 +229,12 @@ pair_count_kernel(const Geom G, const void* __restrict__ species, unsigned long 
   const int n_hist = G.n_shells * n2;
   for (int k = threadIdx.x; k < n_hist; k += blockDim.x) s_hist[k] = 0u;
   __syncthreads();
-  const long long n_conv = (long long)G.Lx * G.Ly * G.Lz;
+  // source sites: layers [pc_z0, pc_z1) (a slab counts the bonds of the layers it owns; their partners lie inside
+  // its window, so the periodic wrap below never acts along z there)
+  const long long c_first = (long long)G.Lx * G.Ly * G.pc_z0;
+  const long long n_conv = (long long)G.Lx * G.Ly * G.pc_z1;
   const int Px = 2 * G.Lx, Py = 2 * G.Ly, Pz = 2 * G.Lz;
-  for (long long c = blockIdx.x * (long long)blockDim.x + threadIdx.x; c < n_conv;
+  for (long long c = c_first + blockIdx.x * (long long)blockDim.x + threadIdx.x; c < n_conv;
        c += (long long)gridDim.x * blockDim.x) {
     const int x = (int)(c % G.Lx);
     const long long r = c / G.Lx;
@@ -279,11 +290,12 @@ __device__ __forceinline__ uint32_t lop3_ind(uint32_t lo, uint32_t hi, uint32_t 
 __global__ void __launch_bounds__(256)
 pair_count_bcc2_kernel(const Geom G, const uint32_t* __restrict__ lat, unsigned long long* __restrict__ M) {
   const int rw = G.Lx >> 3;                                    // words per lattice row
-  const long long n_words = (long long)rw * G.Ly * G.Lz;
+  const long long w_first = (long long)rw * G.Ly * G.pc_z0;    // layers [pc_z0, pc_z1), see pair_count_kernel
+  const long long n_words = (long long)rw * G.Ly * G.pc_z1;
   uint32_t cnt0[16], cnt1[16];
 #pragma unroll
   for (int k = 0; k < 16; ++k) cnt0[k] = cnt1[k] = 0u;
-  for (long long wi = blockIdx.x * (long long)blockDim.x + threadIdx.x; wi < n_words;
+  for (long long wi = w_first + blockIdx.x * (long long)blockDim.x + threadIdx.x; wi < n_words;
        wi += (long long)gridDim.x * blockDim.x) {
     const int xw = (int)(wi % rw);
     const long long r = wi / rw;

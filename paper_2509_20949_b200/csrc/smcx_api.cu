@@ -96,6 +96,15 @@ struct Plan {
   int fcc_rep;      // sweep_fcc_thread: replicas of the look-up rows in shared memory
   FccTables fcc_tables;
   Layout lay;
+  // Slab window (params domain_count >= 2): this handle holds slab domain_index of the lattice cut along z
+  // (domain_api.inc).  n_sites then counts the sites of the window's storage, n_global those of the whole lattice.
+  bool window = false;
+  int dom_count = 1, dom_index = 0;
+  int row_first = 0, row_count = 0;   // link-cell rows owned
+  int z_base = 0;                     // layer of the whole lattice held in storage layer 0 (mod Lz_global)
+  int Lz_global = 0;
+  long long n_global = 0;
+  long long layer_sites = 0;          // sites per layer = Lx Ly B
 };
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
@@ -164,6 +173,46 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   const long long n_cells = (long long)G.ncx * G.ncy * G.ncz;
   if (n_cells > 0xffffffffll) return SMCX_E_BAD_DIMS;  // cell id is a 32-bit Philox counter word
   G.cells_per_colour = (unsigned)(n_cells / 8);
+  G.z_bias = G.Lz - G.H;
+  G.cz_global = 0;
+  G.iz_first = 0;
+  G.work_base = 0;
+  G.pc_z0 = 0;
+  G.pc_z1 = G.Lz;
+  plan->Lz_global = G.Lz;
+  plan->n_global = n_sites;
+  plan->layer_sites = (long long)G.Lx * G.Ly * G.B;
+  plan->window = false;
+  plan->dom_count = 1;
+  plan->dom_index = 0;
+  plan->row_first = 0;
+  plan->row_count = G.ncz;
+  plan->z_base = 0;
+  if (p->domain_count >= 2) {
+    // reading S11: slabs on pairs of link-cell rows; the window holds the rows' layers for every origin oz < w plus
+    // H ghost layers on either side, stored without wrap
+    const int D = p->domain_count, k = p->domain_index;
+    const int pairs = G.ncz / 2;
+    if (k < 0 || k >= D || D > pairs) return SMCX_E_BAD_DIMS;
+    int first = 0, count = 0;
+    for (int q = 0; q <= k; ++q) { first += count; count = 2 * (pairs / D + (q < pairs % D ? 1 : 0)); }
+    const int layers = count * w + w - 1 + 2 * G.H;
+    if (layers > G.Lz) return SMCX_E_BAD_DIMS;
+    plan->window = true;
+    plan->dom_count = D;
+    plan->dom_index = k;
+    plan->row_first = first;
+    plan->row_count = count;
+    plan->z_base = ((first * w - G.H) % G.Lz + G.Lz) % G.Lz;
+    G.Lz = layers;
+    G.ncz = count;
+    G.z_bias = 0;
+    G.cz_global = first;
+    G.cells_per_colour = (unsigned)((long long)G.ncx * G.ncy * count / 8);
+    G.pc_z0 = G.H;
+    G.pc_z1 = G.H + count * w;
+    n_sites = plan->layer_sites * layers;
+  }
   G.S = w * w * w * G.B;
   G.key0 = (uint32_t)(p->seed & 0xffffffffull);
   G.key1 = (uint32_t)(p->seed >> 32);
@@ -185,7 +234,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     }
   }
   plan->n_sites = n_sites;
-  plan->n_cells = n_cells;
+  plan->n_cells = plan->window ? (long long)G.ncx * G.ncy * G.ncz : n_cells;
 
   // kernel / storage choice
   bool fast_ok = thread_kernel_supported(G);
@@ -211,7 +260,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   if (kernel == SMCX_KERNEL_AUTO) {
     // FCC: the packed thread-per-cell kernel once every warp of every SM gets a batch of 32 cells; below that a pass
     // lasts as long as one cell's chain of trials, which is shorter with several lanes per cell
-    if (fcc_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && n_cells / 8 >= 148ll * kFccWarps * 32)))
+    if (fcc_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && plan->n_cells / 8 >= 148ll * kFccWarps * 32)))
       kernel = SMCX_KERNEL_FCC_THREAD;
     else if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_GROUP_PER_CELL;
     else if (!fast_ok) kernel = SMCX_KERNEL_GROUP_PER_CELL;
@@ -220,7 +269,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     // cell's chain of trials with either kernel, and concurrent launches of the persistent kernel
     // (replica ensembles) cost ~20 us each where those of the block kernel overlap freely (measured:
     // 32 replicas of BCC 64^3, 0.416 ms against 0.238 ms per sweep of all replicas).
-    else kernel = n_cells / 8 >= 148ll * kPersistMaxWarps * 32 ? SMCX_KERNEL_THREAD_PERSISTENT : SMCX_KERNEL_THREAD_PER_CELL;
+    else kernel = plan->n_cells / 8 >= 148ll * kPersistMaxWarps * 32 ? SMCX_KERNEL_THREAD_PERSISTENT : SMCX_KERNEL_THREAD_PER_CELL;
   }
   if (kernel == SMCX_KERNEL_THREAD_PER_CELL || kernel == SMCX_KERNEL_THREAD_PERSISTENT) {
     if (!fast_ok) return SMCX_E_UNSUPPORTED;
@@ -324,6 +373,9 @@ struct smcx {
   bool graphs_ok = true;
   int sm_count = 148;
   std::string err;
+  // slab window: origin oz of the sweep begun last (0 after an initial state or an upload, when every layer of the
+  // window is valid); the layers the slab owns are storage layers [H + win_oz, H + win_oz + row_count w)
+  int win_oz = 0;
 
   uint8_t* d_species() const { return reinterpret_cast<uint8_t*>(ws + plan.lay.species); }
   int32_t* d_epi() const { return reinterpret_cast<int32_t*>(ws + plan.lay.epi); }
@@ -381,10 +433,11 @@ int grid_for(const smcx* h, long long work_items, int block) {
 int launch_init(smcx* h) {
   const Plan& P = h->plan;
   int hh = 1;
-  while ((1ull << (2 * hh)) < (unsigned long long)P.n_sites) ++hh;
+  while ((1ull << (2 * hh)) < (unsigned long long)P.n_global) ++hh;
   const int grid = grid_for(h, (P.n_sites + 15) / 16, 256);
   SMCX_STORE_DISPATCH(P, init_species_kernel<Store><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh,
-                                                                                   P.G.key0, P.G.key1));
+                                                                                   P.G.key0, P.G.key1, (long long)P.z_base * P.layer_sites,
+                                                                                   P.n_global));
   h->launches++;
   SMCX_CUDA(h, cudaGetLastError());
   return SMCX_OK;
@@ -393,11 +446,15 @@ int launch_init(smcx* h) {
 // Runs the pair-count reduction and leaves M[s][x][y] (positive-half counts) in host_M.
 int run_pair_counts(smcx* h, std::vector<unsigned long long>& host_M) {
   const Plan& P = h->plan;
-  const Geom& G = P.G;
+  Geom G = P.G;
+  if (P.window) {   // the bonds of the layers the slab owns under the current origin
+    G.pc_z0 = G.H + h->win_oz;
+    G.pc_z1 = G.pc_z0 + P.row_count * G.w;
+  }
   const int n_hist = G.n_shells * G.n_species * G.n_species;
   zero_u64_kernel<<<1, 256, 0, h->stream>>>(h->d_counts(), n_hist);
   h->launches++;
-  const long long n_conv = (long long)G.Lx * G.Ly * G.Lz;
+  const long long n_conv = (long long)G.Lx * G.Ly * (G.pc_z1 - G.pc_z0);
   const int grid = grid_for(h, n_conv, 256);
   const size_t sm = (size_t)n_hist * sizeof(unsigned);
   if (P.storage == SMCX_STORAGE_2BIT && G.lattice == SMCX_BCC && G.n_shells == 2) {
@@ -478,9 +535,10 @@ int ensure_bounce(smcx* h) {
   return SMCX_OK;
 }
 
-int launch_colour_pass(smcx* h, int colour) {
+// One colour pass with the geometry G: the handle's own (smcx_sweep), or a copy of it restricted to some of the
+// link-cell rows of a slab (smcx_domain_pass).
+int launch_colour_pass(smcx* h, const Geom& G, int colour) {
   const Plan& P = h->plan;
-  const Geom& G = P.G;
   if (P.kernel == SMCX_KERNEL_THREAD_PERSISTENT) {
     const int warps = persist_warps_for(G.accept_len);
     if (warps > 0) {
@@ -531,7 +589,7 @@ int enqueue_sweep(smcx* h) {
   nvtxRangePushA("smcx sweep");
   for (int colour = 0; colour < 8; ++colour) {
     nvtxRangePushA(kPassName[colour]);
-    const int rc = launch_colour_pass(h, colour);
+    const int rc = launch_colour_pass(h, h->plan.G, colour);
     nvtxRangePop();
     if (rc != SMCX_OK) { nvtxRangePop(); return rc; }
   }
@@ -718,8 +776,25 @@ static int check_bad_state(smcx* h) {
   return bad ? SMCX_E_BAD_STATE : SMCX_OK;
 }
 
+// Runs of sites that are contiguous both in a host array of the whole lattice (site-id order) and in the handle's
+// storage: the whole lattice is one run; the storage layers [l0, l1) of a slab window are one or two (the window may
+// wrap around the periodic lattice).
+struct SiteRun { long long host_first, local_first, count; };
+static std::vector<SiteRun> site_runs(const smcx* h, int l0, int l1) {
+  const Plan& P = h->plan;
+  std::vector<SiteRun> runs;
+  if (!P.window) { runs.push_back({0, 0, P.n_sites}); return runs; }
+  const long long ls = P.layer_sites;
+  const int g0 = (P.z_base + l0) % P.Lz_global;
+  const int first = std::min(l1 - l0, P.Lz_global - g0);
+  runs.push_back({g0 * ls, l0 * ls, first * ls});
+  if (first < l1 - l0) runs.push_back({0, (l0 + first) * ls, (l1 - l0 - first) * ls});
+  return runs;
+}
+
 int smcx_set_species_device(smcx_t* h, const void* d_src) {
   if (!h || !d_src) return SMCX_E_NULL_ARG;
+  if (h->plan.window) return SMCX_E_UNSUPPORTED;
   DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   const uint8_t* src = reinterpret_cast<const uint8_t*>(d_src);
@@ -751,8 +826,11 @@ int smcx_set_species(smcx_t* h, const uint8_t* host_src) {
   const Plan& P = h->plan;
   int rc = clear_bad_state(h);
   if (rc != SMCX_OK) return rc;
+  // a slab window takes its layers (all of them, ghost layers included) out of the array of the whole lattice
+  const std::vector<SiteRun> runs = site_runs(h, 0, P.G.Lz);
   if (P.storage == SMCX_STORAGE_U8) {
-    SMCX_CUDA(h, cudaMemcpyAsync(h->d_species(), host_src, (size_t)P.n_sites, cudaMemcpyHostToDevice, h->stream));
+    for (const SiteRun& r : runs)
+      SMCX_CUDA(h, cudaMemcpyAsync(h->d_species() + r.local_first, host_src + r.host_first, (size_t)r.count, cudaMemcpyHostToDevice, h->stream));
     validate_u8_kernel<<<grid_for(h, P.n_sites, 256), 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, h->d_state());
     h->launches++;
   } else {
@@ -761,21 +839,23 @@ int smcx_set_species(smcx_t* h, const uint8_t* host_src) {
     SMCX_CUDA(h, cudaEventRecord(h->bounce_free[0], h->stream));   // the bounce buffers are free once earlier work is done
     SMCX_CUDA(h, cudaEventRecord(h->bounce_free[1], h->stream));
     int k = 0;
-    for (long long first = 0; first < P.n_sites; first += kChunkSites, k ^= 1) {
-      const long long cnt = std::min(kChunkSites, P.n_sites - first);
-      SMCX_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->bounce_free[k], 0));
-      SMCX_CUDA(h, cudaMemcpyAsync(h->bounce[k], host_src + first, (size_t)cnt, cudaMemcpyHostToDevice, h->copy_stream));
-      SMCX_CUDA(h, cudaEventRecord(h->bounce_full[k], h->copy_stream));
-      SMCX_CUDA(h, cudaStreamWaitEvent(h->stream, h->bounce_full[k], 0));
-      SMCX_STORE_DISPATCH(P, pack_kernel<Store><<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(
-                                 h->bounce[k], h->d_species(), first, cnt, P.G.n_species, h->d_state()));
-      h->launches++;
-      SMCX_CUDA(h, cudaGetLastError());
-      SMCX_CUDA(h, cudaEventRecord(h->bounce_free[k], h->stream));
-    }
+    for (const SiteRun& r : runs)
+      for (long long first = 0; first < r.count; first += kChunkSites, k ^= 1) {
+        const long long cnt = std::min(kChunkSites, r.count - first);
+        SMCX_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->bounce_free[k], 0));
+        SMCX_CUDA(h, cudaMemcpyAsync(h->bounce[k], host_src + r.host_first + first, (size_t)cnt, cudaMemcpyHostToDevice, h->copy_stream));
+        SMCX_CUDA(h, cudaEventRecord(h->bounce_full[k], h->copy_stream));
+        SMCX_CUDA(h, cudaStreamWaitEvent(h->stream, h->bounce_full[k], 0));
+        SMCX_STORE_DISPATCH(P, pack_kernel<Store><<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(
+                                   h->bounce[k], h->d_species(), r.local_first + first, cnt, P.G.n_species, h->d_state()));
+        h->launches++;
+        SMCX_CUDA(h, cudaGetLastError());
+        SMCX_CUDA(h, cudaEventRecord(h->bounce_free[k], h->stream));
+      }
   }
   rc = check_bad_state(h);
   if (rc != SMCX_OK) return rc;
+  h->win_oz = 0;   // slab window: every layer is valid again
   return reset_running_energy(h);
 }
 
@@ -787,6 +867,7 @@ int smcx_storage_bytes(smcx_t* h, size_t* bytes) {
 
 int smcx_species_packed(smcx_t* h, void* host_dst) {
   if (!h || !host_dst) return SMCX_E_NULL_ARG;
+  if (h->plan.window) return SMCX_E_UNSUPPORTED;
   DeviceGuard on_device(h->device);
   SMCX_CUDA(h, cudaMemcpyAsync(host_dst, h->d_species(), storage_bytes(h->plan.storage, h->plan.n_sites),
                                cudaMemcpyDeviceToHost, h->stream));
@@ -796,6 +877,7 @@ int smcx_species_packed(smcx_t* h, void* host_dst) {
 
 int smcx_set_species_packed(smcx_t* h, const void* host_src) {
   if (!h || !host_src) return SMCX_E_NULL_ARG;
+  if (h->plan.window) return SMCX_E_UNSUPPORTED;
   DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   int rc = clear_bad_state(h);
@@ -820,12 +902,14 @@ int smcx_init_composition(smcx_t* h, const int64_t* counts) {
     sum += counts[p];
     C.cum[p] = sum;
   }
-  if (sum != P.n_sites) return SMCX_E_BAD_STATE;
+  if (sum != P.n_global) return SMCX_E_BAD_STATE;
   int hh = 1;
-  while ((1ull << (2 * hh)) < (unsigned long long)P.n_sites) ++hh;
+  while ((1ull << (2 * hh)) < (unsigned long long)P.n_global) ++hh;
   const int grid = grid_for(h, (P.n_sites + 15) / 16, 256);
   SMCX_STORE_DISPATCH(P, init_composition_kernel<Store><<<grid, 256, 0, h->stream>>>(h->d_species(), P.n_sites, P.G.n_species, hh,
-                                                                                       P.G.key0, P.G.key1, C));
+                                                                                       P.G.key0, P.G.key1, C,
+                                                                                       (long long)P.z_base * P.layer_sites, P.n_global));
+  if (P.window) h->win_oz = 0;   // every layer of the window is valid again
   h->launches++;
   SMCX_CUDA(h, cudaGetLastError());
   return reset_running_energy(h);
@@ -853,6 +937,7 @@ int smcx_set_temperature(smcx_t* h, int32_t kT_units, const uint32_t* accept, in
 
 int smcx_sweep(smcx_t* h, int64_t n) {
   if (!h) return SMCX_E_NULL_ARG;
+  if (h->plan.window) return SMCX_E_UNSUPPORTED;   // a slab is stepped pass by pass through smcx_domain_*
   DeviceGuard on_device(h->device);
   if (n < 0 || h->sweeps_enqueued + n > 0xffffffffll) return SMCX_E_RANGE;  // t is a 32-bit counter word
   // Runs of sweeps at fixed parameters are replayed from a captured graph of one sweep (the kernels
@@ -941,6 +1026,7 @@ int smcx_energy_trace(smcx_t* h, int64_t first_sweep, int64_t count, int64_t* ds
 
 int smcx_species_device(smcx_t* h, void* d_dst) {
   if (!h || !d_dst) return SMCX_E_NULL_ARG;
+  if (h->plan.window) return SMCX_E_UNSUPPORTED;
   DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
   if (P.storage == SMCX_STORAGE_U8) {
@@ -955,13 +1041,18 @@ int smcx_species_device(smcx_t* h, void* d_dst) {
 }
 
 // Packed storage: chunk k is unpacked into bounce buffer k & 1 on the handle's stream and copied to the host on
-// the copy stream while chunk k + 1 is being unpacked; one synchronisation at the end.
+// the copy stream while chunk k + 1 is being unpacked; one synchronisation at the end.  A slab window writes the
+// layers it owns (under the origin of the last sweep) into their place in the array of the whole lattice and leaves
+// the rest of host_dst alone.
 int smcx_species(smcx_t* h, uint8_t* host_dst) {
   if (!h || !host_dst) return SMCX_E_NULL_ARG;
   DeviceGuard on_device(h->device);
   const Plan& P = h->plan;
+  const int l0 = P.window ? P.G.H + h->win_oz : 0;
+  const std::vector<SiteRun> runs = site_runs(h, l0, P.window ? l0 + P.row_count * P.G.w : P.G.Lz);
   if (P.storage == SMCX_STORAGE_U8) {
-    SMCX_CUDA(h, cudaMemcpyAsync(host_dst, h->d_species(), (size_t)P.n_sites, cudaMemcpyDeviceToHost, h->stream));
+    for (const SiteRun& r : runs)
+      SMCX_CUDA(h, cudaMemcpyAsync(host_dst + r.host_first, h->d_species() + r.local_first, (size_t)r.count, cudaMemcpyDeviceToHost, h->stream));
     SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
     return SMCX_OK;
   }
@@ -970,30 +1061,27 @@ int smcx_species(smcx_t* h, uint8_t* host_dst) {
   SMCX_CUDA(h, cudaEventRecord(h->bounce_free[0], h->stream));
   SMCX_CUDA(h, cudaEventRecord(h->bounce_free[1], h->stream));
   int k = 0;
-  for (long long first = 0; first < P.n_sites; first += kChunkSites, k ^= 1) {
-    const long long cnt = std::min(kChunkSites, P.n_sites - first);
-    SMCX_CUDA(h, cudaStreamWaitEvent(h->stream, h->bounce_free[k], 0));
-    SMCX_STORE_DISPATCH(P, unpack_kernel<Store><<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(
-                               h->d_species(), h->bounce[k], first, cnt));
-    h->launches++;
-    SMCX_CUDA(h, cudaGetLastError());
-    SMCX_CUDA(h, cudaEventRecord(h->bounce_full[k], h->stream));
-    SMCX_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->bounce_full[k], 0));
-    SMCX_CUDA(h, cudaMemcpyAsync(host_dst + first, h->bounce[k], (size_t)cnt, cudaMemcpyDeviceToHost, h->copy_stream));
-    SMCX_CUDA(h, cudaEventRecord(h->bounce_free[k], h->copy_stream));
-  }
+  for (const SiteRun& r : runs)
+    for (long long first = 0; first < r.count; first += kChunkSites, k ^= 1) {
+      const long long cnt = std::min(kChunkSites, r.count - first);
+      SMCX_CUDA(h, cudaStreamWaitEvent(h->stream, h->bounce_free[k], 0));
+      SMCX_STORE_DISPATCH(P, unpack_kernel<Store><<<grid_for(h, (cnt + 15) / 16, 256), 256, 0, h->stream>>>(
+                                 h->d_species(), h->bounce[k], r.local_first + first, cnt));
+      h->launches++;
+      SMCX_CUDA(h, cudaGetLastError());
+      SMCX_CUDA(h, cudaEventRecord(h->bounce_full[k], h->stream));
+      SMCX_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->bounce_full[k], 0));
+      SMCX_CUDA(h, cudaMemcpyAsync(host_dst + r.host_first + first, h->bounce[k], (size_t)cnt, cudaMemcpyDeviceToHost, h->copy_stream));
+      SMCX_CUDA(h, cudaEventRecord(h->bounce_free[k], h->copy_stream));
+    }
   SMCX_CUDA(h, cudaStreamSynchronize(h->copy_stream));
   SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
   return SMCX_OK;
 }
 
-int smcx_sro(smcx_t* h, double* alpha, int64_t* pair_counts) {
-  if (!h || !alpha) return SMCX_E_NULL_ARG;
-  DeviceGuard on_device(h->device);
-  std::vector<unsigned long long> M;
-  const int rc = run_pair_counts(h, M);
-  if (rc != SMCX_OK) return rc;
-  const Geom& G = h->plan.G;
+// Eq. 8 from the positive-half counts M of a whole lattice of N sites.
+static void sro_from_half_counts(const Geom& G, double N, const std::vector<unsigned long long>& M, double* alpha,
+                                 int64_t* pair_counts) {
   const int n = G.n_species;
   std::vector<int> Z(G.n_shells, 0);
   for (int m = 0; m < G.ZT; ++m) Z[G.shell_of[m]]++;
@@ -1009,7 +1097,6 @@ int smcx_sro(smcx_t* h, double* alpha, int64_t* pair_counts) {
     for (int b = 0; b < n; ++b) row += Ns[(size_t)a * n + b];
     n_of[a] = row / Z[0];
   }
-  const double N = (double)h->plan.n_sites;
   for (int s = 0; s < G.n_shells; ++s)
     for (int a = 0; a < n; ++a)
       for (int b = 0; b < n; ++b) {
@@ -1021,6 +1108,16 @@ int smcx_sro(smcx_t* h, double* alpha, int64_t* pair_counts) {
         alpha[idx] = 1.0 - P / c;
       }
   if (pair_counts) std::memcpy(pair_counts, Ns.data(), Ns.size() * sizeof(long long));
+}
+
+int smcx_sro(smcx_t* h, double* alpha, int64_t* pair_counts) {
+  if (!h || !alpha) return SMCX_E_NULL_ARG;
+  if (h->plan.window) return SMCX_E_UNSUPPORTED;   // partial counts: smcx_domain_pair_counts + smcx_sro_from_counts
+  DeviceGuard on_device(h->device);
+  std::vector<unsigned long long> M;
+  const int rc = run_pair_counts(h, M);
+  if (rc != SMCX_OK) return rc;
+  sro_from_half_counts(h->plan.G, (double)h->plan.n_sites, M, alpha, pair_counts);
   return SMCX_OK;
 }
 
@@ -1031,7 +1128,7 @@ int smcx_stats(smcx_t* h, int64_t* sweeps_done, int64_t* trials, int64_t* accept
   SMCX_CUDA(h, cudaMemcpyAsync(&st, h->d_state(), sizeof(st), cudaMemcpyDeviceToHost, h->stream));
   SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
   if (sweeps_done) *sweeps_done = (int64_t)st.sweep;
-  if (trials) *trials = (int64_t)st.sweep * h->plan.n_sites;
+  if (trials) *trials = (int64_t)st.sweep * (h->plan.window ? h->plan.layer_sites * h->plan.row_count * h->plan.G.w : h->plan.n_sites);
   if (accepted) *accepted = (int64_t)st.accepted;
   return SMCX_OK;
 }
@@ -1083,3 +1180,4 @@ int smcx_group_layout(const smcx_params_t* p, int32_t* lanes, int32_t* A, int32_
 }  // extern "C"
 
 #include "ensemble_api.inc"
+#include "domain_api.inc"

@@ -61,7 +61,7 @@ struct DevState {
   long long e_run;               // running energy E_0 + sum of accepted dE
   unsigned long long accepted;   // accepted swaps
   unsigned long long bad_state;  // set by validation kernels
-  unsigned work[8];              // per colour: batches of cells handed out so far in this sweep (sweep_fcc_thread); zeroed by sweep_epilogue
+  unsigned work[16];             // per colour (+ 8 for the second launch of a split pass, Geom::work_base): batches of cells handed out so far in this sweep (sweep_fcc_thread); zeroed by sweep_epilogue
 };
 
 // Lattice + link-cell geometry and the shell-offset tables.  Passed to kernels by value, i.e. it
@@ -76,6 +76,15 @@ struct Geom {
   int TW;              // tile edge = w + 2H
   int r0;              // per-axis reach of shell 0 (half-lattice units)
   int ncx, ncy, ncz;   // link cells per axis
+  // Slab windows (lattice parallelism, domain_api.inc): a handle that holds one slab of a lattice cut along z stores
+  // the layers of its window only (Lz = storage layers, never wrapped) and runs the link-cell rows it owns.
+  //   z_bias     tile origin: first tile layer = (oz + cz w + z_bias) mod Lz; Lz - H for a whole (periodic) lattice,
+  //              0 for a slab (storage layer 0 is H layers below its first row at origin 0);
+  //   cz_global  first link-cell row of the slab in the whole lattice (cell ids are global: they key the Philox stream);
+  //   iz_first   first row pair a launch works on (a pass may be split into the boundary row and the rest).
+  int z_bias, cz_global, iz_first;
+  int pc_z0, pc_z1;    // pair-count kernels: layers [pc_z0, pc_z1) of the source sites (the whole lattice, or the layers a slab owns)
+  int work_base;       // 0 or 8: which half of DevState::work a launch of sweep_fcc_thread draws its batches from
   unsigned cells_per_colour;
   int S;               // trials per cell = w^3 B
   int Z0;              // coordination number of shell 0

@@ -343,7 +343,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
   for (;;) {
     // a2: the next batch of 32 consecutive cells of the colour
     uint32_t batch = 0;
-    if (lane == 0) batch = atomicAdd(&st->work[colour], 1u);
+    if (lane == 0) batch = atomicAdd(&st->work[G.work_base + colour], 1u);
     batch = __shfl_sync(0xffffffffu, batch, 0);
     if (batch >= n_batches) break;
     const uint32_t m = batch * 32u + (uint32_t)lane;
@@ -352,7 +352,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
       colour_cell(G, m, colour, cx, cy, cz);
       const int x0 = (ox + cx * 4 - 2 + G.Lx) % G.Lx;
       const int t0y = (oy + cy * 4 - 2 + G.Ly) % G.Ly;
-      const int t0z = (oz + cz * 4 - 2 + G.Lz) % G.Lz;
+      const int t0z = tile_z0(G, oz, cz);
       const int wlo = x0 >> 3, sh = 4 * (x0 & 7);
       const int whi = wlo + 1 == rw ? 0 : wlo + 1;
       // a3: stage the tile: per row two 16-byte groups (four sublattice words each), funnel-shifted into four tile words
@@ -385,7 +385,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
         }
       }
       // a4-a6: the 256 trials of the cell, raster order: conventional cell c = (lz * 4 + ly) * 4 + lx, then b
-      const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
+      const uint32_t cell_id = global_cell_id(G, cx, cy, cz);
       const PhiloxCell pc = philox_cell_setup(cell_id, t, ctr3, G.rk0, G.rk1);
       int esum = 0;
 #pragma unroll 1

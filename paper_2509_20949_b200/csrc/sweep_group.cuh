@@ -355,7 +355,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
     colour_cell(G, m, colour, cx, cy, cz);
     t0x = (ox + cx * w - H + G.Lx) % G.Lx;
     t0y = (oy + cy * w - H + G.Ly) % G.Ly;
-    t0z = (oz + cz * w - H + G.Lz) % G.Lz;
+    t0z = tile_z0(G, oz, cz);
   }
   // a3: stage the tile, eight conventional cells per lane in flight (a group without a cell stages species
   // 0 everywhere: all its trials are no-ops)
@@ -390,7 +390,7 @@ sweep_group_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t*
   __syncthreads();  // tables + tiles visible
 
   {
-    const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
+    const uint32_t cell_id = global_cell_id(G, cx, cy, cz);
     const uint32_t ctr3 = TAG_TRIAL | ((uint32_t)colour << 8);
     const int nit = NIT > 0 ? NIT : (ZT + L - 1) / L;
     const int filter_E = G.filter_E;

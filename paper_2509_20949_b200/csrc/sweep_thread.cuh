@@ -511,7 +511,7 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
     colour_cell(G, m, colour, cx, cy, cz);
     const int x0 = (ox + cx * 4 - 2 + G.Lx) % G.Lx;
     const int t0y = (oy + cy * 4 - 2 + G.Ly) % G.Ly;
-    const int t0z = (oz + cz * 4 - 2 + G.Lz) % G.Lz;
+    const int t0z = tile_z0(G, oz, cz);
     const int rw = G.Lx >> 3;                                   // words per lattice row
     const int wlo = x0 >> 3, sh = 4 * (x0 & 7);
     const int whi = wlo + 1 == rw ? 0 : wlo + 1;
@@ -542,7 +542,7 @@ sweep_thread_per_cell(const Geom G, uint32_t* __restrict__ lattice, const int4* 
       }
     }
     // a4-a6: the 128 trials of this cell, raster order, one Philox call per two slots
-    const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
+    const uint32_t cell_id = global_cell_id(G, cx, cy, cz);
     const uint32_t ctr3 = TAG_TRIAL | ((uint32_t)colour << 8);
     TrialEnv env;
     env.coef = smem_ptr(s_coef0) + (threadIdx.x & 7) * 16;
@@ -712,7 +712,7 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
       colour_cell(G, m, colour, cx, cy, cz);
       const int x0 = (ox + cx * 4 - 2 + G.Lx) % G.Lx;
       const int t0y = (oy + cy * 4 - 2 + G.Ly) % G.Ly;
-      const int t0z = (oz + cz * 4 - 2 + G.Lz) % G.Lz;
+      const int t0z = tile_z0(G, oz, cz);
       const int wlo = x0 >> 3, sh = 4 * (x0 & 7);
       const int whi = wlo + 1 == rw ? 0 : wlo + 1;
       const uint32_t dwh = (uint32_t)(whi - wlo);
@@ -738,7 +738,7 @@ sweep_thread_persistent(const Geom G, uint32_t* __restrict__ lattice, const int4
           for (int ry = 0; ry < 8; ++ry) tile[(rz * 8 + ry) * NT] = __funnelshift_r(lo[ry], hi[ry], sh);
         }
       }
-      const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
+      const uint32_t cell_id = global_cell_id(G, cx, cy, cz);
       const PhiloxCell pc = philox_cell_setup(cell_id, t, ctr3, G.rk0, G.rk1);
 #define SMCX_PHILOX_PAIR(LX) philox_factored(pc, s_slot[q0 + LX], G.rk0, G.rk1)
 #pragma unroll 1

@@ -19,6 +19,13 @@ __device__ __forceinline__ void sweep_origin(const Geom& G, uint32_t t, int& ox,
   oz = (int)mulhi_u32(r.z, (uint32_t)G.w);
 }
 
+// Global id of link cell (cx, cy, cz) (cz counted inside the slab when the handle holds one): ctr[0] of S4.
+__device__ __forceinline__ uint32_t global_cell_id(const Geom& G, int cx, int cy, int cz) {
+  return (uint32_t)(((cz + G.cz_global) * G.ncy + cy) * G.ncx + cx);
+}
+// First layer (conventional cell) of the tile of a cell of row cz.
+__device__ __forceinline__ int tile_z0(const Geom& G, int oz, int cz) { return (oz + cz * G.w + G.z_bias) % G.Lz; }
+
 // m-th cell of a colour -> cell coordinates; cells of one colour are enumerated x fastest.
 __device__ __forceinline__ void colour_cell(const Geom& G, uint32_t m, int colour, int& cx, int& cy,
                                             int& cz) {
@@ -26,7 +33,7 @@ __device__ __forceinline__ void colour_cell(const Geom& G, uint32_t m, int colou
   const uint32_t ix = m % hx;
   const uint32_t r = m / hx;
   const uint32_t iy = r % hy;
-  const uint32_t iz = r / hy;
+  const uint32_t iz = r / hy + (uint32_t)G.iz_first;
   cx = (int)(2u * ix) + (colour & 1);
   cy = (int)(2u * iy) + ((colour >> 1) & 1);
   cz = (int)(2u * iz) + ((colour >> 2) & 1);
@@ -68,7 +75,7 @@ sweep_warp_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t* 
     // a3: stage the tile; its first conventional cell is (o + c w - H) mod L per axis.
     t0x = (ox + cx * w - H + G.Lx) % G.Lx;
     t0y = (oy + cy * w - H + G.Ly) % G.Ly;
-    t0z = (oz + cz * w - H + G.Lz) % G.Lz;
+    t0z = tile_z0(G, oz, cz);
     for (int idx = lane; idx < TW * TW * TW; idx += 32) {
       const int tx = idx % TW, ty = (idx / TW) % TW, tz = idx / (TW * TW);
       int gx = t0x + tx; if (gx >= G.Lx) gx -= G.Lx;
@@ -82,7 +89,7 @@ sweep_warp_per_cell(const Geom G, uint8_t* __restrict__ species, const int32_t* 
   __syncthreads();  // tables + tiles visible
 
   if (active) {
-    const uint32_t cell_id = (uint32_t)((cz * G.ncy + cy) * G.ncx + cx);
+    const uint32_t cell_id = global_cell_id(G, cx, cy, cz);
     const uint32_t ctr3 = TAG_TRIAL | ((uint32_t)colour << 8);
     const int ZT = G.ZT;
     uint32_t r_dir_even = 0, r_u_even = 0, r_dir_odd = 0, r_u_odd = 0;
@@ -169,7 +176,7 @@ __global__ void sweep_epilogue(DevState* st, long long* trace, int trace_capacit
   const unsigned long long t = st->sweep;
   trace[t % (unsigned long long)trace_capacity] = st->e_run;
   st->sweep = t + 1ull;
-  for (int c = 0; c < 8; ++c) st->work[c] = 0u;
+  for (int c = 0; c < 16; ++c) st->work[c] = 0u;
 }
 
 }  // namespace smcxk
