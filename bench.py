@@ -7,8 +7,9 @@ A "step" is one Monte Carlo sweep of the whole hot path (SURVEY.md 8(a), a1-a8: 
 passes with tile staging / proposal / dE / accept / write-back, energy trace), plus a9 (pair-count
 reduction -> energy + Warren-Cowley SRO) once every `sro_every` sweeps as the config prescribes and
 at least once inside the timed region.  N = 1 times BASELINE.json configs[3] (BCC 800^3, 1.024e9
-sites, the configuration the metric is quoted on).  N > 1 runs N independent replicas, one per GPU
-(the path is single-GPU by north_star: "replicas only", weak scaling, no data-path collective).
+sites, the configuration the metric is quoted on).  N > 1 cuts that one lattice into N slabs along z, one per GPU,
+with ghost layers exchanged after every colour pass (lattice parallelism; strong scaling); `--multi
+replicas` runs N independent lattices instead (weak scaling, no data-path collective).
 
 `--impl reference` times the CPU oracle (oracle/, test infrastructure) on the host cores for the
 same metric; under torchrun only rank 0 works.
@@ -354,6 +355,123 @@ def run_largest_single_gpu(sweeps: int = 20):
     return out
 
 
+def run_lattice_parallel_one_gpu(cfg, sweeps: int = 10, whole_sweep_ms=None):
+    """Lattice parallelism with every slab on this one GPU: the workload cut into
+    2 and 4 slabs with ghost layers, messages as device-to-device copies, with and without computation-communication
+    overlap.  Measures what the decomposition itself costs (split launches, messages, event ordering); the slabs
+    share one GPU, so this is not a scaling number."""
+    import paper_2509_20949_b200 as smcx
+
+    out = {"workload": workload_string(cfg), "note": "all slabs on one GPU: cost of the decomposition, not scaling",
+           "undivided_sweep_ms": whole_sweep_ms, "runs": []}
+    for n_slabs, overlap in ((2, True), (4, True), (4, False)):
+        g = smcx.DomainGroup.from_config(cfg, n_slabs, overlap=overlap)
+        ms = _time_sweeps(g, 3, sweeps)
+        b0 = g.message_bytes
+        g.sweep(1)
+        g.synchronize()
+        out["runs"].append({"slabs": n_slabs, "overlap": overlap, "sweep_ms": ms, "value": cfg.n_sites / (ms * 1e-3),
+                            "unit": "trial swaps/s", "message_bytes_per_sweep": int(g.message_bytes - b0),
+                            "vs_undivided": (whole_sweep_ms / ms) if whole_sweep_ms else None})
+        g.close()
+    return out
+
+
+def run_slabs(args, cfg, rank, world, local_rank):
+    """N > 1: the paper's lattice parallelism: the ONE lattice of the config cut into N slabs along z, one
+    per GPU / rank, ghost layers exchanged after every colour pass with torch.distributed send/recv (NCCL), the
+    boundary row of a pass first so that its message overlaps the other rows.  Strong scaling: the total
+    work is fixed.  Results are those of the undivided lattice bit for bit (tests/test_gpu_domains.py)."""
+    import torch
+    import torch.distributed as dist
+    from paper_2509_20949_b200 import distributed
+
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if not dist.is_initialized():
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        dist.barrier()
+        torch.cuda.synchronize()
+
+    kw = dict(lattice=cfg.lattice, dims=cfg.dims, n_species=cfg.n_species, n_shells=cfg.n_shells, epi=cfg.epi(),
+              accept=cfg.accept_table(0), seed=cfg.seed, link_cell=cfg.link_cell, kT_units=cfg.kT_at(0),
+              kernel=args.kernel, storage=args.storage, device=local_rank)
+    slab = distributed.SlabRank(rank, world, dist=dist, overlap=not args.no_overlap, **kw)
+    slab.sweep(args.warmup)
+    barrier()
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    time.sleep(0.25)
+    launches0 = slab.domain.kernel_launches
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    a.record()
+    slab.sweep(args.steps)
+    b.record()
+    barrier()
+    total_ms = a.elapsed_time(b)
+    clocks = sampler.stop()
+    launches = slab.domain.kernel_launches - launches0
+    owned = float(slab.domain.info["owned_sites"])
+    value, max_ms = aggregate_over_ranks(total_ms, owned * args.steps, dist, dev)
+    # end to end: every rank uploads its window of the host array, K x (table up, sweep, energy back), owned layers down
+    host = torch.empty(cfg.n_sites, dtype=torch.uint8).pin_memory().numpy()
+    host[:] = 0
+    slab.domain.species_into(host)
+    whole = torch.from_numpy(host).to(dev)
+    dist.all_reduce(whole)                       # owned layers are disjoint: the sum is the whole lattice
+    host[:] = whole.cpu().numpy()
+    del whole
+    e2e_steps = min(args.steps, 200)
+    table = cfg.accept_table(0)
+    barrier()
+    t0 = time.perf_counter()
+    slab.domain.set_species(host)
+    first = slab.domain.stats()[0]
+    for t in range(e2e_steps):
+        slab.domain.set_temperature(cfg.kT_at(0), table)
+        slab.sweep(1)
+        slab.domain.energy_trace(first + t, 1)
+    slab.domain.species_into(host)
+    counts = slab.pair_counts()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    e2e_value, _ = aggregate_over_ranks(e2e_s * 1e3, owned * e2e_steps, dist, dev)
+    window = slab.domain.info["z_layers"] * cfg.n_sites // cfg.dims[2]
+    if rank == 0:
+        peak, peak_kind = measured_peak()
+        launch_ms = max_ms / args.steps / 8.0
+        achieved = ALGO_BYTES_PER_TRIAL * (cfg.n_sites / 8.0 / world) / (launch_ms * 1e-3) / 1e9
+        out = {
+            "metric": metric_name(), "value": value, "unit": "trial swaps/s", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "int32", "data": "synthetic",
+            "config": {"workload": workload_string(cfg), "config_id": args.config,
+                       "step": "1 sweep of the one lattice = per GPU a window shift + 8 x (colour pass of its slab, ghost-layer message)",
+                       "parallelism": f"lattice parallelism: {world} slabs along z, one per GPU, ghost layers over NCCL send/recv, "
+                                      f"overlap {'on' if not args.no_overlap else 'off'}",
+                       "l2": "slab windows larger than the 126 MB L2 at the graded size; no flush"},
+            "pct_of_hbm_roofline": 100.0 * (value / world) * ALGO_BYTES_PER_TRIAL / (peak * 1e9),
+            "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                         "traffic": None, "traffic_note": "multi-GPU run: no ncu capture (profiles/ hold the single-GPU ones)",
+                         "peak_kind": peak_kind, "kernel": KERNEL_NAMES.get(args.kernel, "auto"),
+                         "what": "per GPU: algorithmic bytes of one colour pass of a slab / (step time / 8), message wait included",
+                         "algorithmic_bytes_per_trial": ALGO_BYTES_PER_TRIAL, "launch_ms": launch_ms},
+            "e2e": {"value": e2e_value, "unit": "trial swaps/s", "h2d_bytes_per_step": (window + e2e_steps * table.nbytes) / e2e_steps,
+                    "d2h_bytes_per_step": (owned + e2e_steps * 8 + counts.nbytes) / e2e_steps, "steps": e2e_steps,
+                    "what": "per rank: smcx_domain_set_species(host) + steps x (table up, sweep with messages, energy back) + "
+                            "smcx_domain_species(host) + pair counts, wall clock, max over ranks"},
+            "message_bytes_per_step_per_gpu": slab.message_bytes / max(1, args.warmup + args.steps + e2e_steps),
+            "gpu_launches": int(launches), "clocks": clocks,
+        }
+        print(json.dumps(out))
+    slab.close()
+    dist.barrier()
+    dist.destroy_process_group()
+
+
 def run_cuda(args, cfg, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -518,6 +636,8 @@ def run_cuda(args, cfg, rank, world, local_rank):
                 out["paper_shaped_fcc"] = run_paper_shaped_fcc(args.fcc_edge)
             if args.largest and args.config != 5:
                 out["largest_single_gpu"] = run_largest_single_gpu()
+            if args.slabs_leg and cfg.dims[2] // cfg.link_cell >= 16:
+                out["lattice_parallel_one_gpu"] = run_lattice_parallel_one_gpu(cfg, whole_sweep_ms=sweep_ms / args.steps)
         print(json.dumps(out))
     lat.close()
     if world > 1:
@@ -540,6 +660,12 @@ def main():
                          "conventional cells per edge (0: skip)")
     ap.add_argument("--no-largest", dest="largest", action="store_false",
                     help="skip the BCC 2000^3 (1.6e10 sites) leg that the default run adds as `largest_single_gpu`")
+    ap.add_argument("--no-slabs-leg", dest="slabs_leg", action="store_false",
+                    help="skip the `lattice_parallel_one_gpu` leg (the workload cut into 2 / 4 slabs on this one GPU)")
+    ap.add_argument("--multi", default="slabs", choices=["slabs", "replicas"],
+                    help="N > 1: `slabs` = the one lattice cut into N slabs, one per GPU (lattice parallelism, strong scaling); "
+                         "`replicas` = N independent lattices (weak scaling)")
+    ap.add_argument("--no-overlap", action="store_true", help="--multi slabs: send the ghost layers after the whole pass")
     ap.add_argument("--source-hash", action="store_true", help="print the source hash of every kernel (for profiles/dram_traffic.csv) and exit")
     ap.add_argument("--ensemble", type=int, default=128,
                     help="also time a replica-exchange ensemble of this many BCC 64^3 replicas (0: skip)")
@@ -555,6 +681,9 @@ def main():
     cfg = get_config(args.config)
     if args.impl == "reference":
         run_reference(args, cfg, rank)
+        return
+    if world > 1 and args.multi == "slabs":
+        run_slabs(args, cfg, rank, world, local_rank)
         return
     run_cuda(args, cfg, rank, world, local_rank)
 
