@@ -53,10 +53,11 @@ template <int NT> struct FccTile {
 };
 
 // Direction table, [b][dir]: what the partner j = i + O_0[dir] of a site of sublattice b needs.
-//   d01 = delta_0 | delta_1 << 16, d23 = delta_2 | delta_3 << 16: byte offsets (int16) from i's own row pointer to
-//         the base rows of j's four partner sublattices;
-//   rot = e3 | e2 << 8 (int8): a3_j = a3_i + e3, a2_j = 4 X + e2 (rotation amounts, see fcc_site).
-struct FccDirEntry { uint32_t d01, d23, rot, pad; };
+//   d[k]: byte offset from i's own row pointer to the base row of j's partner sublattice k (k = 0: j's own row);
+//   e3, e2: a3_j = a3_i + e3, a2_j = 4 X + e2 (rotation amounts, see fcc_site).
+// Full-width fields: two 16-byte loads per trial and no unpacking (the 16-bit packed form cost eight integer-pipe
+// instructions per trial, and that pipe is what binds the kernel: profiles/r2_fcc_kernel_ncu.md).
+struct FccDirEntry { int32_t d[4]; int32_t e3, e2, pad0, pad1; };
 struct FccTables { FccDirEntry dir[4][12]; };
 
 __host__ __device__ constexpr int fcc_beta(int b, int axis) {   // S0: basis positions, units of a/2
@@ -84,17 +85,12 @@ inline bool fcc_build_tables(const Geom& G, FccTables& T) {
       const int bj = bits == 0 ? 0 : bits == 6 ? 1 : bits == 5 ? 2 : bits == 3 ? 3 : -1;
       if (bj < 0) return false;
       const int dr = cell[1] + 8 * cell[2];
-      int delta[4];
-      for (int k = 0; k < 4; ++k) {
-        delta[k] = ((bj ^ k) - b) * FccTile<NT>::kSub + (dr + fcc_base_adj(bj, k)) * FccTile<NT>::kRow;
-        if (delta[k] < -32768 || delta[k] > 32767) return false;
-      }
-      const int e3 = 4 * cell[0], e2 = 4 * (cell[0] + fcc_beta(bj, 0) - 1);
       FccDirEntry& e = T.dir[b][d];
-      e.d01 = ((uint32_t)delta[0] & 0xFFFFu) | ((uint32_t)delta[1] << 16);
-      e.d23 = ((uint32_t)delta[2] & 0xFFFFu) | ((uint32_t)delta[3] << 16);
-      e.rot = ((uint32_t)e3 & 0xFFu) | (((uint32_t)e2 & 0xFFu) << 8);
-      e.pad = 0u;
+      for (int k = 0; k < 4; ++k)
+        e.d[k] = ((bj ^ k) - b) * FccTile<NT>::kSub + (dr + fcc_base_adj(bj, k)) * FccTile<NT>::kRow;
+      e.e3 = 4 * cell[0];
+      e.e2 = 4 * (cell[0] + fcc_beta(bj, 0) - 1);
+      e.pad0 = e.pad1 = 0;
     }
   return true;
 }
@@ -179,13 +175,15 @@ template <int NT>
 __host__ __device__ __forceinline__ void fcc_site_sum(const FccSite& S, uint32_t own_rot, const FccLut& L0, const FccLut& L1,
                                                       const FccLut& L2, uint32_t& lo, uint32_t& hi) {
   const uint32_t a3 = S.a3, a3m4 = a3 - 4u, a3m8 = a3 - 8u, a3p4 = a3 + 4u, a2 = S.a2, a2m8 = a2 - 8u;
+  // A look-up (PRMT) reads the low four nibbles of its selector word only, so an accumulator whose four nibbles all
+  // hold neighbours is ONE bit-select of two rotated rows (whatever lands in its upper half is ignored); nibbles
+  // that hold no neighbour must be zero (species code 0, cancelling between i and j), which costs a second operation.
   // k = 0: shell 1
   {
-    uint32_t A = own_rot & 0x0F0Fu;                                            // X - 1, X + 1 of the own row
-    A |= rotr32(fcc_ld<NT, -1>(S.p0), a3) & 0x00F0u;                          // (y - 1): nibble X -> 1
-    A |= rotr32(fcc_ld<NT, 1>(S.p0), a3m8) & 0xF000u;                         // (y + 1): nibble X -> 3
-    uint32_t B = rotr32(fcc_ld<NT, -8>(S.p0), a3p4) & 0x000Fu;                // (z - 1): nibble X -> 0
-    B |= rotr32(fcc_ld<NT, 8>(S.p0), a3) & 0x00F0u;                           // (z + 1): nibble X -> 1
+    uint32_t A = lop3<kLutSel>(rotr32(fcc_ld<NT, -1>(S.p0), a3), own_rot, 0x00F0u);        // (y - 1): nibble X -> 1; own row: X - 1, X + 1 at 0, 2
+    A = lop3<kLutSel>(rotr32(fcc_ld<NT, 1>(S.p0), a3m8), A, 0xF000u);                      // (y + 1): nibble X -> 3
+    const uint32_t B0 = rotr32(fcc_ld<NT, -8>(S.p0), a3p4) & 0x000Fu;                      // (z - 1): nibble X -> 0
+    const uint32_t B = lop3<kLutAndOr2>(rotr32(fcc_ld<NT, 8>(S.p0), a3), 0x00F0u, B0);     // (z + 1): nibble X -> 1; nibbles 2, 3 empty
     fcc_lookup(L1, A, lo, hi);
     fcc_lookup(L1, B, lo, hi);
   }
@@ -193,27 +191,27 @@ __host__ __device__ __forceinline__ void fcc_site_sum(const FccSite& S, uint32_t
   {
     const uint32_t w0 = rotr32(fcc_ld<NT, 0>(S.p1), a3), w1 = rotr32(fcc_ld<NT, 1>(S.p1), a3m4);
     const uint32_t w8 = rotr32(fcc_ld<NT, 8>(S.p1), a3), w9 = rotr32(fcc_ld<NT, 9>(S.p1), a3m4);
-    fcc_lookup(L2, ((w1 & 0xF0F0u) | (w0 & 0x0F0Fu)), lo, hi);
-    fcc_lookup(L2, ((w9 & 0xF0F0u) | (w8 & 0x0F0Fu)), lo, hi);
-    fcc_lookup(L0, ((w1 & 0x0F00u) | (w0 & 0x00F0u)), lo, hi);
-    fcc_lookup(L0, ((w9 & 0x0F00u) | (w8 & 0x00F0u)), lo, hi);
+    fcc_lookup(L2, lop3<kLutSel>(w1, w0, 0xF0F0u), lo, hi);
+    fcc_lookup(L2, lop3<kLutSel>(w9, w8, 0xF0F0u), lo, hi);
+    fcc_lookup(L0, lop3<kLutAndOr2>(w1, 0x0F00u, w0 & 0x00F0u), lo, hi);                   // two nibbles empty
+    fcc_lookup(L0, lop3<kLutAndOr2>(w9, 0x0F00u, w8 & 0x00F0u), lo, hi);
   }
   // k = 2: rows y - 1 .. y + 1 of two z layers, window of two nibbles: dy = 0 shell 0, else shell 2
   {
     const uint32_t m = rotr32(fcc_ld<NT, -1>(S.p2), a2), c = rotr32(fcc_ld<NT, 0>(S.p2), a2), p = rotr32(fcc_ld<NT, 1>(S.p2), a2m8);
     const uint32_t m8 = rotr32(fcc_ld<NT, 7>(S.p2), a2), c8 = rotr32(fcc_ld<NT, 8>(S.p2), a2m8), p8 = rotr32(fcc_ld<NT, 9>(S.p2), a2m8);
-    fcc_lookup(L0, ((c8 & 0xFF00u) | (c & 0x00FFu)), lo, hi);
-    fcc_lookup(L2, ((p & 0xFF00u) | (m & 0x00FFu)), lo, hi);
-    fcc_lookup(L2, ((p8 & 0xFF00u) | (m8 & 0x00FFu)), lo, hi);
+    fcc_lookup(L0, lop3<kLutSel>(c8, c, 0xFF00u), lo, hi);
+    fcc_lookup(L2, lop3<kLutSel>(p, m, 0xFF00u), lo, hi);
+    fcc_lookup(L2, lop3<kLutSel>(p8, m8, 0xFF00u), lo, hi);
   }
   // k = 3: rows z - 1 .. z + 1 of two y rows: dz = 0 shell 0, else shell 2
   {
     const uint32_t m = rotr32(fcc_ld<NT, -8>(S.p3), a2), m1 = rotr32(fcc_ld<NT, -7>(S.p3), a2m8);
     const uint32_t c = rotr32(fcc_ld<NT, 0>(S.p3), a2), c1 = rotr32(fcc_ld<NT, 1>(S.p3), a2m8);
     const uint32_t p = rotr32(fcc_ld<NT, 8>(S.p3), a2), p1 = rotr32(fcc_ld<NT, 9>(S.p3), a2m8);
-    fcc_lookup(L0, ((c1 & 0xFF00u) | (c & 0x00FFu)), lo, hi);
-    fcc_lookup(L2, ((m1 & 0xFF00u) | (m & 0x00FFu)), lo, hi);
-    fcc_lookup(L2, ((p1 & 0xFF00u) | (p & 0x00FFu)), lo, hi);
+    fcc_lookup(L0, lop3<kLutSel>(c1, c, 0xFF00u), lo, hi);
+    fcc_lookup(L2, lop3<kLutSel>(m1, m, 0xFF00u), lo, hi);
+    fcc_lookup(L2, lop3<kLutSel>(p1, p, 0xFF00u), lo, hi);
   }
 }
 
@@ -246,12 +244,12 @@ __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4,
   si.p3 = fcc_at<NT>(p_own, ((b ^ 3) - b) * T::kSub + fcc_base_adj(b, 3) * T::kRow);
   si.a3 = X4 - 4u;
   si.a2 = X4 + (uint32_t)(4 * (fcc_beta(b, 0) - 1));
-  sj.p0 = fcc_at<NT>(p_own, (int)(short)(E.d01 & 0xFFFFu));
-  sj.p1 = fcc_at<NT>(p_own, (int)E.d01 >> 16);
-  sj.p2 = fcc_at<NT>(p_own, (int)(short)(E.d23 & 0xFFFFu));
-  sj.p3 = fcc_at<NT>(p_own, (int)E.d23 >> 16);
-  sj.a3 = si.a3 + (uint32_t)(int)(signed char)(E.rot & 0xFFu);
-  sj.a2 = X4 + (uint32_t)(int)(signed char)((E.rot >> 8) & 0xFFu);
+  sj.p0 = fcc_at<NT>(p_own, E.d[0]);
+  sj.p1 = fcc_at<NT>(p_own, E.d[1]);
+  sj.p2 = fcc_at<NT>(p_own, E.d[2]);
+  sj.p3 = fcc_at<NT>(p_own, E.d[3]);
+  sj.a3 = si.a3 + (uint32_t)E.e3;
+  sj.a2 = X4 + (uint32_t)E.e2;
   const uint32_t own_i = rotr32(fcc_ld<NT, 0>(si.p0), si.a3), own_j = rotr32(fcc_ld<NT, 0>(sj.p0), sj.a3);
   const uint32_t a = (own_i >> 4) & 7u, sb = (own_j >> 4) & 7u;
   const uint32_t pair = a * 8u + sb;
@@ -318,7 +316,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
   for (int k = threadIdx.x; k < 64; k += blockDim.x) s_corr[k] = corr[k];
   if (kFilter)
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
-  for (int k = threadIdx.x; k < 48; k += blockDim.x) s_dir[k] = FT.dir[k / 12][k % 12];
+  for (int k = threadIdx.x; k < 48; k += blockDim.x) s_dir[k] = FT.dir[k / 12][k % 12];   // 32 bytes each
   const uint32_t t = (uint32_t)st->sweep;
   if (threadIdx.x < 128) s_slot[threadIdx.x] = philox_slot_entry(threadIdx.x, t, G.rk0, G.rk1);
   int ox, oy, oz;
@@ -397,8 +395,9 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
         const Philox4 r1 = philox_factored(pc, s_slot[2 * c + 1], G.rk0, G.rk1);
 #define SMCX_FCC_TRIAL(B, WDIR, U)                                                                          \
         {                                                                                                     \
-          const int4 e = lds_int4(dir_p, (int)((B * 12u + mulhi_u32(WDIR, 12u)) * 16u));                    \
-          const FccDirEntry E{(uint32_t)e.x, (uint32_t)e.y, (uint32_t)e.z, 0u};                              \
+          const smem_ptr_t ep = dir_p + (B * 12u + mulhi_u32(WDIR, 12u)) * 32u;                              \
+          const int4 e = lds_int4(ep, 0), f = lds_int4(ep, 16);                                               \
+          const FccDirEntry E{{e.x, e.y, e.z, e.w}, f.x, f.y, 0, 0};                                          \
           fcc_trial<B, NT, kFilter>(p_row + B * (kFccRows * NT), X4, E, U, env, esum, nacc);                  \
         }
         SMCX_FCC_TRIAL(0, r0.x, r0.y) SMCX_FCC_TRIAL(1, r0.z, r0.w) SMCX_FCC_TRIAL(2, r1.x, r1.y) SMCX_FCC_TRIAL(3, r1.z, r1.w)

@@ -162,6 +162,7 @@ constexpr int kLutSel = 0xE4;      // c ? a : b
 constexpr int kLutSelNotB = 0xB1;  // c ? a : ~b
 constexpr int kLutMaj = 0xE8;      // majority
 constexpr int kLutAndOr = 0xE0;    // a & (b | c)
+constexpr int kLutAndOr2 = 0xEA;   // (a & b) | c
 __host__ __device__ __forceinline__ int popc32(uint32_t v) {
 #ifdef __CUDA_ARCH__
   return __popc(v);

@@ -484,6 +484,7 @@ def test_sub_warp_kernel_table_formats(lanes, amplitude, kT):
     ((16, 8, 24), 2, 2, 300, 500),       # two shells: the third shell's rows are zero
     ((40, 24, 16), 5, 3, 15_000, 9_000), # differences that need the high byte of the look-up in full
     ((32, 32, 32), 3, 3, 400, 430),      # more than one batch of 32 cells per colour (64)
+    ((24, 24, 8), 5, 3, 400, 690),       # 9 cells per colour: a ragged batch
 ])
 def test_packed_fcc_kernel_against_the_oracle(dims, n_sp, n_sh, amp, kT):
     lat, w, seed = 1, 4, 515
