@@ -46,6 +46,8 @@ def _load():
         "oracle_create": (C.c_void_p, [C.c_int, i32p, C.c_int, C.c_int, i32p, C.c_int, u32p, C.c_int,
                                        C.c_uint64]),
         "oracle_destroy": (None, [C.c_void_p]),
+        "oracle_set_local_model": (None, [C.c_void_p, i32p]),
+        "oracle_site_energy": (C.c_int64, [C.c_void_p, C.c_int64]),
         "oracle_n_sites": (C.c_int64, [C.c_void_p]),
         "oracle_init_species": (None, [C.c_void_p]),
         "oracle_init_permutation": (C.c_uint64, [C.c_void_p, C.c_uint64]),
@@ -169,6 +171,19 @@ class Oracle:
                   epi=cfg.epi(), link_cell=cfg.link_cell, accept=cfg.accept_table(0), seed=cfg.seed)
         kw.update(over)
         return cls(init=init, threads=threads, **kw)
+
+    def set_local_model(self, quad):
+        """S12: nonlinear local-energy model; quad = W2[s][a][x][y] (x <= y used), the table given at
+        creation is its linear part W1[s][a][x].  None: back to pairwise EPI."""
+        if quad is None:
+            self._lib.oracle_set_local_model(self._h, None)
+            return
+        q = np.ascontiguousarray(quad, dtype=np.int32)
+        assert q.shape == (self.n_shells, self.n_species, self.n_species, self.n_species)
+        self._lib.oracle_set_local_model(self._h, _ptr(q, C.c_int32))
+
+    def site_energy(self, k: int) -> int:
+        return int(self._lib.oracle_site_energy(self._h, int(k)))
 
     def set_threads(self, n: int) -> int:
         """OpenMP threads over the cells of a colour (and over sites in the init / energy / pair-count

@@ -97,6 +97,11 @@ struct Oracle {
   int64_t trace_first = 0;              // resume (checkpointing): the sweep counter was set to this value
   int threads = 1;                      // OpenMP threads over the cells of a colour (1 = plain loop)
   mutable int64_t poison_reads = 0;     // S11: species values >= n_species met while evaluating energies
+  // S12: nonlinear local-energy model.  model 0: pairwise EPI (S1).  model 1: H = sum_i eps_i with
+  // eps_i a quadratic form of the neighbour species counts of site i; `epi` is then its linear part W1[s][a][x]
+  // (need not be symmetric) and `quad` its quadratic part W2[s][a][x][y] (entries with x <= y are used).
+  int model = 0;
+  std::vector<int32_t> quad;
 };
 
 constexpr uint8_t kPoison = 255;
@@ -209,7 +214,10 @@ bool in_positive_half(const Vec3& d) {
   return d.x > 0;
 }
 
+int64_t total_energy_local(const Oracle& o);
+
 int64_t total_energy(const Oracle& o) {
+  if (o.model == 1) return total_energy_local(o);
   int64_t H = 0;
   for (int s = 0; s < o.n_shells; ++s)
     for (const Vec3& d : o.shell[s]) {
@@ -219,6 +227,74 @@ int64_t total_energy(const Oracle& o) {
       for (int64_t i = 0; i < o.N; ++i) H += V(o, s, o.sigma[i], o.sigma[neighbour(o, i, d)]);
     }
   return H;
+}
+
+// ---------------------------------------------------------------------------------------
+// S12: a general nonlinear short-range model.  PAPER.md:118: "the qSRO model represents a general nonlinear
+// short-range model, where the local energies of all lattice sites within LIZ are calculated to determine the
+// energy change due to a MC move"; the model itself is the paper's Ref. 22 and its weights are not available.
+// Reading S12: the energy is a sum of local energies, H = sum_i eps(sigma_i, n_i), where
+// n_i[s][x] = number of neighbours of species x in shell s of site i (the local short-range order of the site) and
+//   eps(a, n) = sum_s ( sum_x W1[s][a][x] n[s][x]  +  sum_{x <= y} W2[s][a][x][y] n[s][x] n[s][y] ),
+// int32 weights, int64 energies.  The quadratic part couples pairs of neighbours of a site (three-body terms):
+// it cannot be written as a pair interaction.  With W2 = 0 and W1 = V symmetric the model is twice the EPI
+// Hamiltonian (every bond is seen from both ends).  A swap of i and j changes the own species of i and j and the
+// counts of every site that has i or j as a neighbour: dE is the sum, over that set U = {i, j} + N(i) + N(j), of
+// the local energies after the swap minus before -- evaluated here exactly that way, site by site from scratch.
+// ---------------------------------------------------------------------------------------
+int64_t site_energy(const Oracle& o, int64_t k) {
+  const int n = o.n_species;
+  const int a = o.sigma[k];
+  if (a >= n) { o.poison_reads++; return 0; }
+  int64_t e = 0;
+  std::vector<int64_t> cnt((size_t)n);
+  for (int s = 0; s < o.n_shells; ++s) {
+    std::fill(cnt.begin(), cnt.end(), (int64_t)0);
+    for (const Vec3& d : o.shell[s]) {
+      const int x = o.sigma[neighbour(o, k, d)];
+      if (x >= n) { o.poison_reads++; continue; }
+      cnt[(size_t)x]++;
+    }
+    for (int x = 0; x < n; ++x) {
+      e += (int64_t)o.epi[((size_t)s * n + a) * n + x] * cnt[(size_t)x];
+      for (int y = x; y < n; ++y)
+        e += (int64_t)o.quad[(((size_t)s * n + a) * n + x) * n + y] * cnt[(size_t)x] * cnt[(size_t)y];
+    }
+  }
+  return e;
+}
+
+int64_t total_energy_local(const Oracle& o) {
+  int64_t H = 0;
+#pragma omp parallel for reduction(+ : H) schedule(static) num_threads(o.threads) if (o.threads > 1)
+  for (int64_t k = 0; k < o.N; ++k) H += site_energy(o, k);
+  return H;
+}
+
+// the sites whose local energy a swap of i and j can change, each once
+void affected_sites(const Oracle& o, int64_t i, int64_t j, std::vector<int64_t>& U) {
+  U.clear();
+  U.push_back(i);
+  U.push_back(j);
+  for (int s = 0; s < o.n_shells; ++s)
+    for (const Vec3& d : o.shell[s]) {
+      // k has i as a neighbour at offset d  <=>  k = i - d; the shells are symmetric, so this is N(i) itself
+      U.push_back(neighbour(o, i, d));
+      U.push_back(neighbour(o, j, d));
+    }
+  std::sort(U.begin(), U.end());
+  U.erase(std::unique(U.begin(), U.end()), U.end());
+}
+
+int64_t swap_delta_local(Oracle& o, int64_t i, int64_t j) {
+  static thread_local std::vector<int64_t> U;
+  affected_sites(o, i, j, U);
+  int64_t before = 0, after = 0;
+  for (int64_t k : U) before += site_energy(o, k);
+  std::swap(o.sigma[i], o.sigma[j]);
+  for (int64_t k : U) after += site_energy(o, k);
+  std::swap(o.sigma[i], o.sigma[j]);
+  return after - before;
 }
 
 // S1: the sites bonded to i and to j (one entry per shell offset, shells in order), with
@@ -256,6 +332,7 @@ int64_t local_energy(const Oracle& o, int64_t i, int64_t j, const Bonds& bonds) 
 // S1: dE of swapping sigma_i and sigma_j = H(sigma') - H(sigma), the plain way:
 // local energy after the swap minus before.  The state is left unchanged.
 int64_t swap_delta(Oracle& o, int64_t i, int64_t j) {
+  if (o.model == 1) return swap_delta_local(o, i, j);
   static thread_local Bonds bonds;
   collect_bonds(o, i, j, bonds);
   const int64_t before = local_energy(o, i, j, bonds);
@@ -720,6 +797,23 @@ void* oracle_create(int lattice, const int* dims, int n_species, int n_shells, c
 
 void oracle_destroy(void* h) { delete (Oracle*)h; }
 
+// S12: switch the handle to the nonlinear local-energy model.  quad = W2[s][a][x][y], n_shells n^3 entries (x <= y
+// used); the table given at creation becomes the linear part W1[s][a][x].  quad == NULL: back to pairwise EPI.
+void oracle_set_local_model(void* h, const int32_t* quad) {
+  Oracle& o = *(Oracle*)h;
+  if (!quad) { o.model = 0; o.quad.clear(); }
+  else {
+    o.model = 1;
+    o.quad.assign(quad, quad + (size_t)o.n_shells * o.n_species * o.n_species * o.n_species);
+  }
+  o.E_valid = false;
+}
+
+int64_t oracle_site_energy(void* h, int64_t k) {
+  Oracle& o = *(Oracle*)h;
+  return o.model == 1 ? site_energy(o, k) : 0;
+}
+
 int64_t oracle_n_sites(void* h) { return ((Oracle*)h)->N; }
 
 void oracle_init_species(void* h) { init_species(*(Oracle*)h); }
@@ -786,7 +880,8 @@ int oracle_lc_valid(void* h) {
       if (s == 0) r0 = std::max(r0, m);
       R = std::max(R, m);
     }
-  return 2 * o.w >= 2 * r0 + R ? 1 : 0;
+  // S12: a trial of the local model reads the neighbours of the neighbours of i and j: reach r0 + 2 R
+  return 2 * o.w >= 2 * r0 + (o.model == 1 ? 2 * R : R) ? 1 : 0;
 }
 
 // n link-cell sweeps.  The caller is responsible for oracle_lc_valid(); an invalid w is

@@ -9,6 +9,7 @@ Recipes:
   * EPI: V_s(a,b)=V_s(b,a) = -A + mulhi32(philox(ctr=(a,b,s,TAG_EPI), key=seed)[0], 2A+1)
     for a <= b, i.e. uniform integers in [-A, A] in 0.1 meV units.  The paper prints no EPI
     values, so these stand in for the fitted Fe29Co29Ni28Al7Ti7 interactions.
+  * nonlinear local-energy model (reading S12): make_local_weights, uniform integer weights drawn the same way.
   * threshold table: T[d] = min(floor(exp(-d/kT_units) * 2^32), 2^32-1),
     len = floor(32 ln2 kT_units) + 2 (last entry is exactly 0).  Eq. 3, PAPER.md:60-63,
     in the integer form BASELINE.json's north_star fixes ("a 32-bit Philox draw compared
@@ -18,6 +19,7 @@ from .tables import (  # noqa: F401
     TAG_EPI,
     philox4x32_10,
     make_epi,
+    make_local_weights,
     make_accept_table,
     accept_table_len,
     anneal_kT_units,

@@ -48,6 +48,29 @@ def make_epi(n_shells: int, n_species: int, amplitude: int, seed: int) -> np.nda
     return v
 
 
+TAG_LOCAL = 7  # synthetic weights of the nonlinear local-energy model (reading S12)
+
+
+def make_local_weights(n_shells: int, n_species: int, amp_linear: int, amp_quad: int, seed: int):
+    """Synthetic integer weights of the nonlinear local-energy model (reading S12; the paper's qSRO weights, PAPER.md:118,
+    are not published): (W1, W2) with W1[s][a][x] uniform in [-amp_linear, amp_linear] (not symmetric) and
+    W2[s][a][x][y], x <= y, uniform in [-amp_quad, amp_quad] (0 for x > y), drawn like the EPI entries:
+    -A + mulhi32(philox(ctr=(index, a, s, TAG_LOCAL), key=seed)[0], 2A + 1), index = x for W1, n + x n + y for W2."""
+    key = (seed & _MASK, (seed >> 32) & _MASK)
+    n = n_species
+    w1 = np.zeros((n_shells, n, n), dtype=np.int32)
+    w2 = np.zeros((n_shells, n, n, n), dtype=np.int32)
+    for s in range(n_shells):
+        for a in range(n):
+            for x in range(n):
+                r = philox4x32_10((x, a, s, TAG_LOCAL), key)[0]
+                w1[s, a, x] = -amp_linear + ((r * (2 * amp_linear + 1)) >> 32)
+                for y in range(x, n):
+                    r = philox4x32_10((n + x * n + y, a, s, TAG_LOCAL), key)[0]
+                    w2[s, a, x, y] = -amp_quad + ((r * (2 * amp_quad + 1)) >> 32)
+    return w1, w2
+
+
 def accept_table_len(kT_units: int) -> int:
     return int(math.floor(32.0 * math.log(2.0) * kT_units)) + 2
 
