@@ -76,7 +76,20 @@ enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_4BIT = 4, SMCX
  * (same speed there, and concurrent lattices of a replica ensemble overlap freely).  Results never
  * depend on it. */
 enum { SMCX_KERNEL_AUTO = 0, SMCX_KERNEL_WARP_PER_CELL = 1, SMCX_KERNEL_THREAD_PER_CELL = 2,
-       SMCX_KERNEL_THREAD_PERSISTENT = 3, SMCX_KERNEL_GROUP_PER_CELL = 4, SMCX_KERNEL_FCC_THREAD = 5 };
+       SMCX_KERNEL_THREAD_PERSISTENT = 3, SMCX_KERNEL_GROUP_PER_CELL = 4, SMCX_KERNEL_FCC_THREAD = 5,
+       SMCX_KERNEL_LOCAL_WARP = 6 };
+
+/* Energy model.  EPI: the pairwise effective-pair-interaction Hamiltonian (reading S1).
+ * LOCAL: "a general nonlinear short-range model, where the local energies of all lattice sites within LIZ are
+ * calculated to determine the energy change due to a MC move" (the role of the paper's qSRO model, whose
+ * form and weights are its Ref. 22 and not available).  Reading S12: H = sum_i eps(sigma_i, n_i), n_i[s][x] = number of
+ * neighbours of species x in shell s of site i, eps(a, n) = sum_s ( sum_x W1[s][a][x] n[s][x] + sum_{x <= y}
+ * W2[s][a][x][y] n[s][x] n[s][y] ); int32 weights, int64 energies.  `epi` is then W1 (it need not be symmetric) and
+ * `local_quad` W2.  With W2 = 0 and W1 symmetric the model is twice the EPI Hamiltonian.  A trial reads the
+ * neighbours of the neighbours of i and j, so the link cell must satisfy 2w >= 2 r0 + 2 R; n_species <= 8; uint8
+ * storage; kernel SMCX_KERNEL_LOCAL_WARP (one warp per link cell).  smcx_energy returns H of this model;
+ * smcx_sro is unchanged.  Not available on slabs (smcx_domain_*). */
+enum { SMCX_MODEL_EPI = 0, SMCX_MODEL_LOCAL = 1 };
 
 enum {
   SMCX_OK = 0,
@@ -94,7 +107,7 @@ enum {
   SMCX_E_CUDA = -11,               /* CUDA error; text via smcx_last_error */
   SMCX_E_UNSUPPORTED = -12,        /* storage/kernel choice not valid for these parameters */
   SMCX_E_RANGE = -13,              /* trace range not retained, sweep counter overflow */
-  SMCX_E_EPI_RANGE = -14           /* EPI magnitudes so large that the int32 dE of a trial could overflow */
+  SMCX_E_EPI_RANGE = -14           /* EPI magnitudes / local-model weights so large that the int32 dE of a trial could overflow */
 };
 
 typedef struct {
@@ -122,6 +135,8 @@ typedef struct {
   int32_t group_warps;      /* GROUP_PER_CELL: warps per block, 1..8; 0 = as many as leave room for four blocks per SM */
   int32_t domain_count;     /* 0 or 1: the handle holds the whole lattice.  Set by smcx_domain_create (>= 2: the handle holds */
   int32_t domain_index;     /* slab domain_index of dims cut into domain_count slabs along z); leave both 0 otherwise */
+  int32_t model;            /* SMCX_MODEL_* */
+  const int32_t *local_quad;/* host, SMCX_MODEL_LOCAL: W2[n_shells][n_species][n_species][n_species] (x <= y used) */
 } smcx_params_t;
 
 /* Bytes of device workspace a handle with these parameters needs (species array in its storage

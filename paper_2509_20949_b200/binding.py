@@ -16,6 +16,8 @@ BCC, FCC = 0, 1
 STORAGE_AUTO, STORAGE_2BIT, STORAGE_4BIT, STORAGE_U8 = 0, 2, 4, 8
 KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT, KERNEL_GROUP_PER_CELL = 0, 1, 2, 3, 4
 KERNEL_FCC_THREAD = 5
+KERNEL_LOCAL_WARP = 6
+MODEL_EPI, MODEL_LOCAL = 0, 1
 
 
 class SmcxError(RuntimeError):
@@ -33,6 +35,7 @@ class _Params(C.Structure):
         ("stream", C.c_void_p), ("d_workspace", C.c_void_p), ("workspace_bytes", C.c_size_t),
         ("group_lanes", C.c_int32), ("group_warps", C.c_int32),
         ("domain_count", C.c_int32), ("domain_index", C.c_int32),
+        ("model", C.c_int32), ("local_quad", C.POINTER(C.c_int32)),
     ]
 
 
@@ -178,7 +181,7 @@ def _strerror(code: int) -> str:
 
 
 def _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage, kernel,
-                 device, trace_capacity, group_lanes=0, group_warps=0):
+                 device, trace_capacity, group_lanes=0, group_warps=0, local_quad=None):
     epi = np.ascontiguousarray(epi, dtype=np.int32)
     accept = np.ascontiguousarray(accept, dtype=np.uint32)
     p = _Params()
@@ -192,14 +195,22 @@ def _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cel
     p.seed = int(seed)
     p.storage, p.kernel, p.device, p.trace_capacity = int(storage), int(kernel), int(device), int(trace_capacity)
     p.group_lanes, p.group_warps = int(group_lanes), int(group_warps)
-    return p, (epi, accept)
+    quad = None
+    if local_quad is not None:      # SMCX_MODEL_LOCAL: epi is the linear part W1, local_quad the quadratic part W2
+        quad = np.ascontiguousarray(local_quad, dtype=np.int32)
+        if quad.shape != (int(n_shells), int(n_species), int(n_species), int(n_species)):
+            raise ValueError("local_quad must have shape [n_shells][n_species][n_species][n_species]")
+        p.model = MODEL_LOCAL
+        p.local_quad = quad.ctypes.data_as(C.POINTER(C.c_int32))
+    return p, (epi, accept, quad)
 
 
 class Lattice:
     """One smcx_t handle.  Methods mirror the C entry points of include/smcx.h."""
 
     def __init__(self, lattice, dims, n_species, n_shells, epi, accept, seed, link_cell=4, kT_units=0,
-                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0, group_lanes=0, group_warps=0):
+                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0, group_lanes=0, group_warps=0,
+                 local_quad=None):
         import torch  # device memory + stream only
 
         if not torch.cuda.is_available():
@@ -207,7 +218,7 @@ class Lattice:
         self._lib = lib = load_library()
         self._h = None
         p, keep = _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage,
-                               kernel, device, trace_capacity, group_lanes, group_warps)
+                               kernel, device, trace_capacity, group_lanes, group_warps, local_quad)
         need = C.c_size_t(0)
         rc = lib.smcx_workspace_bytes(C.byref(p), C.byref(need))
         if rc != 0:

@@ -4,6 +4,7 @@
 #include "../../include/smcx.h"
 
 #include <algorithm>
+#include <array>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -21,6 +22,7 @@
 #include "smcx_common.cuh"
 #include "sweep_fcc.cuh"
 #include "sweep_group.cuh"
+#include "sweep_local.cuh"
 #include "sweep_thread.cuh"
 #include "sweep_warp.cuh"
 
@@ -80,7 +82,7 @@ inline int floor_div2(int v) { return v >= 0 ? v / 2 : -((-v + 1) / 2); }
 inline bool is_thread_kernel(int k) { return k == SMCX_KERNEL_THREAD_PER_CELL || k == SMCX_KERNEL_THREAD_PERSISTENT; }
 
 struct Layout {
-  size_t species, epi, coef, gtable, fcc_lut, fcc_corr, accept, filter, trace, state, counts, total;
+  size_t species, epi, coef, gtable, fcc_lut, fcc_corr, quad, utab, ucount, accept, filter, trace, state, counts, total;
 };
 
 struct Plan {
@@ -96,6 +98,8 @@ struct Plan {
   int fcc_rep;      // sweep_fcc_thread: replicas of the look-up rows in shared memory
   FccTables fcc_tables;
   Layout lay;
+  int model = SMCX_MODEL_EPI;
+  int local_umax = 0;   // SMCX_MODEL_LOCAL: affected sites per (basis, direction), at most
   // Slab window (params domain_count >= 2): this handle holds slab domain_index of the lattice cut along z
   // (domain_api.inc).  n_sites then counts the sites of the window's storage, n_global those of the whole lattice.
   bool window = false;
@@ -124,7 +128,12 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   if (!p->epi) return SMCX_E_NULL_ARG;
   if (!p->accept || p->accept_len < 1 || p->accept_len > kAcceptCapacity) return SMCX_E_BAD_TABLE;
   const int n = p->n_species;
-  for (int s = 0; s < p->n_shells; ++s)
+  if (p->model != SMCX_MODEL_EPI && p->model != SMCX_MODEL_LOCAL) return SMCX_E_UNSUPPORTED;
+  const bool local = p->model == SMCX_MODEL_LOCAL;
+  plan->model = p->model;
+  if (local && !p->local_quad) return SMCX_E_NULL_ARG;
+  if (local && (n > kLocalMaxSpecies || p->domain_count >= 2)) return SMCX_E_UNSUPPORTED;
+  for (int s = 0; s < p->n_shells && !local; ++s)
     for (int a = 0; a < n; ++a)
       for (int b = 0; b < a; ++b)
         if (p->epi[(s * n + a) * n + b] != p->epi[(s * n + b) * n + a]) return SMCX_E_EPI_NOT_SYMMETRIC;
@@ -157,8 +166,10 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   G.Z0 = (int)shells[0].size();
   G.r0 = r0;
   // S2: same-colour cells must not interact during a pass: 2w >= 2 r0 + R (w in conventional cells).
-  if (2 * w < 2 * r0 + R) return SMCX_E_LINK_CELL_TOO_SMALL;
-  G.H = (r0 + R + 1) / 2;
+  // reading S12: a trial of the local model reads the neighbours of the neighbours of i and j (reach r0 + 2 R)
+  const int reach = local ? r0 + 2 * R : r0 + R;
+  if (2 * w < r0 + reach) return SMCX_E_LINK_CELL_TOO_SMALL;
+  G.H = (reach + 1) / 2;
   G.TW = w + 2 * G.H;
   group_default_layout(G);     // until group_tune_layout() has run
   long long n_sites = G.B;
@@ -257,6 +268,19 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     plan->fcc_rep = fcc_lut_rep(n);
   }
   int kernel = p->kernel, storage = p->storage;
+  if (local) {
+    if (kernel == SMCX_KERNEL_AUTO) kernel = SMCX_KERNEL_LOCAL_WARP;
+    if (kernel != SMCX_KERNEL_LOCAL_WARP) return SMCX_E_UNSUPPORTED;
+    fast_ok = fcc_ok = false;
+    // int32 arithmetic of the kernel: |eps| <= sum_s (Z_s max|W1| + Z_s^2 max|W2|), |dE| <= 2 |U| max|eps|
+    long long m1 = 0, m2 = 0, eps = 0;
+    for (int k = 0; k < p->n_shells * n * n; ++k) m1 = std::max(m1, std::llabs((long long)p->epi[k]));
+    for (int k = 0; k < p->n_shells * n * n * n; ++k) m2 = std::max(m2, std::llabs((long long)p->local_quad[k]));
+    for (int s = 0; s < p->n_shells; ++s) { const long long Z = (long long)shells[s].size(); eps += Z * m1 + Z * Z * m2; }
+    if (2 * (2 + 2ll * G.ZT) * eps >= (1ll << 31)) return SMCX_E_EPI_RANGE;
+  } else if (kernel == SMCX_KERNEL_LOCAL_WARP) {
+    return SMCX_E_UNSUPPORTED;
+  }
   if (kernel == SMCX_KERNEL_AUTO) {
     // FCC: the packed thread-per-cell kernel once every warp of every SM gets a batch of 32 cells; below that a pass
     // lasts as long as one cell's chain of trials, which is shorter with several lanes per cell
@@ -279,7 +303,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     if (!fcc_ok) return SMCX_E_UNSUPPORTED;
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_4BIT;
     if (storage != SMCX_STORAGE_4BIT) return SMCX_E_UNSUPPORTED;
-  } else if (kernel == SMCX_KERNEL_WARP_PER_CELL || kernel == SMCX_KERNEL_GROUP_PER_CELL) {
+  } else if (kernel == SMCX_KERNEL_WARP_PER_CELL || kernel == SMCX_KERNEL_GROUP_PER_CELL || kernel == SMCX_KERNEL_LOCAL_WARP) {
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_U8;
     if (storage != SMCX_STORAGE_U8) return SMCX_E_UNSUPPORTED;
   } else {
@@ -328,6 +352,11 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   L.gtable = off;  off += align_up((size_t)group_smem_layout(G, plan->group_lanes).d_bytes, 256);   // sub-warp kernel's difference table
   L.fcc_lut = off; off += align_up((size_t)64 * 3 * 8 * 16, 256);                                   // packed FCC kernel's look-up rows
   L.fcc_corr = off; off += align_up((size_t)64 * sizeof(int32_t), 256);
+  plan->local_umax = local ? 2 + 2 * G.ZT : 0;
+  L.quad = off;    off += align_up(local ? (size_t)p->n_shells * n * n * n * sizeof(int32_t) : 0, 256);
+  L.utab = off;    off += align_up((size_t)G.B * G.Z0 * plan->local_umax * sizeof(LocalUEntry), 256);
+  L.ucount = off;  off += align_up(local ? (size_t)G.B * G.Z0 * sizeof(int) : 0, 256);
+  if (local && local_smem_bytes(G, plan->local_umax) > 227 * 1024) return SMCX_E_LINK_CELL_TOO_SMALL;
   L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
   L.filter = off;  off += align_up((size_t)kFilterWords * sizeof(uint32_t), 256);
   L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
@@ -335,6 +364,55 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   L.counts = off;  off += align_up((size_t)kMaxShells * kMaxSpecies * kMaxSpecies * sizeof(unsigned long long), 256);
   L.total = off;
   return SMCX_OK;
+}
+
+// SMCX_MODEL_LOCAL: for every (basis b of i, direction), the sites whose local energy the swap changes -- i, j, their
+// neighbours, each once -- as tile-linear steps from i, with the shells in which such a site sees i and j.
+void build_local_utable(const Plan& P, int lattice, std::vector<LocalUEntry>& tab, std::vector<int>& count) {
+  const Geom& G = P.G;
+  const int umax = P.local_umax;
+  tab.assign((size_t)G.B * G.Z0 * umax, LocalUEntry{0, -1, -1, 0, 0, 0});
+  count.assign((size_t)G.B * G.Z0, 0);
+  auto shell_of_vec = [&](int x, int y, int z) {
+    for (int m = 0; m < G.ZT; ++m)
+      if (G.off[m][0] == x && G.off[m][1] == y && G.off[m][2] == z) return (int)G.shell_of[m];
+    return -1;
+  };
+  for (int b = 0; b < G.B; ++b) {
+    int bp[3];
+    basis_pos(lattice, b, bp);
+    for (int dir = 0; dir < G.Z0; ++dir) {
+      const int jx = G.off[dir][0], jy = G.off[dir][1], jz = G.off[dir][2];
+      std::vector<std::array<int, 3>> U;
+      auto add = [&](int x, int y, int z) {
+        for (const auto& v : U)
+          if (v[0] == x && v[1] == y && v[2] == z) return;
+        U.push_back({x, y, z});
+      };
+      add(0, 0, 0);
+      add(jx, jy, jz);
+      for (int m = 0; m < G.ZT; ++m) {
+        add(G.off[m][0], G.off[m][1], G.off[m][2]);
+        add(jx + G.off[m][0], jy + G.off[m][1], jz + G.off[m][2]);
+      }
+      LocalUEntry* out = tab.data() + (size_t)(b * G.Z0 + dir) * umax;
+      for (size_t k = 0; k < U.size(); ++k) {
+        const int vx = U[k][0], vy = U[k][1], vz = U[k][2];
+        const int qx = bp[0] + vx, qy = bp[1] + vy, qz = bp[2] + vz;
+        const int nb = basis_from_parity(lattice, qx, qy, qz);
+        const int d = ((floor_div2(qz) * G.TW + floor_div2(qy)) * G.TW + floor_div2(qx)) * G.B + (nb - b);
+        LocalUEntry e;
+        e.delta = (short)d;
+        e.shell_i = (signed char)shell_of_vec(-vx, -vy, -vz);            // i - u
+        e.shell_j = (signed char)shell_of_vec(jx - vx, jy - vy, jz - vz);  // j - u
+        e.kind = (vx == 0 && vy == 0 && vz == 0) ? 1 : ((vx == jx && vy == jy && vz == jz) ? 2 : 0);
+        e.basis = (unsigned char)nb;
+        e.pad = 0;
+        out[k] = e;
+      }
+      count[(size_t)b * G.Z0 + dir] = (int)U.size();
+    }
+  }
 }
 
 }  // namespace
@@ -383,6 +461,10 @@ struct smcx {
   int32_t* d_gtable() const { return reinterpret_cast<int32_t*>(ws + plan.lay.gtable); }
   uint32_t* d_fcc_lut() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.fcc_lut); }
   int32_t* d_fcc_corr() const { return reinterpret_cast<int32_t*>(ws + plan.lay.fcc_corr); }
+  int32_t* d_quad() const { return reinterpret_cast<int32_t*>(ws + plan.lay.quad); }
+  LocalUEntry* d_utab() const { return reinterpret_cast<LocalUEntry*>(ws + plan.lay.utab); }
+  int* d_ucount() const { return reinterpret_cast<int*>(ws + plan.lay.ucount); }
+  int lattice_type = 0;
   uint32_t* d_accept() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.accept); }
   uint32_t* d_filter() const { return reinterpret_cast<uint32_t*>(ws + plan.lay.filter); }
   long long* d_trace() const { return reinterpret_cast<long long*>(ws + plan.lay.trace); }
@@ -486,12 +568,36 @@ long long energy_from_counts(const smcx* h, const std::vector<unsigned long long
   return E;
 }
 
+// SMCX_MODEL_LOCAL: H = sum of the local energies, by local_energy_kernel.
+int run_local_energy(smcx* h, long long* E) {
+  const Plan& P = h->plan;
+  const Geom& G = P.G;
+  zero_u64_kernel<<<1, 32, 0, h->stream>>>(h->d_counts(), 1);
+  const size_t sm = ((size_t)G.n_shells * G.n_species * G.n_species * (1 + G.n_species)) * sizeof(int32_t);
+  const int grid = grid_for(h, P.n_sites, 256);
+  if (G.B == 2) local_energy_kernel<2><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_epi(), h->d_quad(), h->d_counts());
+  else local_energy_kernel<4><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_epi(), h->d_quad(), h->d_counts());
+  h->launches += 2;
+  SMCX_CUDA(h, cudaGetLastError());
+  unsigned long long v = 0;
+  SMCX_CUDA(h, cudaMemcpyAsync(&v, h->d_counts(), sizeof(v), cudaMemcpyDeviceToHost, h->stream));
+  SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
+  *E = (long long)v;
+  return SMCX_OK;
+}
+
 // Recompute H from the lattice and store it as the running energy.
 int reset_running_energy(smcx* h) {
-  std::vector<unsigned long long> M;
-  const int rc = run_pair_counts(h, M);
-  if (rc != SMCX_OK) return rc;
-  const long long E = energy_from_counts(h, M);
+  long long E = 0;
+  if (h->plan.model == SMCX_MODEL_LOCAL) {
+    const int rc = run_local_energy(h, &E);
+    if (rc != SMCX_OK) return rc;
+  } else {
+    std::vector<unsigned long long> M;
+    const int rc = run_pair_counts(h, M);
+    if (rc != SMCX_OK) return rc;
+    E = energy_from_counts(h, M);
+  }
   SMCX_CUDA(h, cudaMemcpyAsync(&h->d_state()->e_run, &E, sizeof(E), cudaMemcpyHostToDevice, h->stream));
   SMCX_CUDA(h, cudaStreamSynchronize(h->stream));
   return SMCX_OK;
@@ -561,6 +667,16 @@ int launch_colour_pass(smcx* h, const Geom& G, int colour) {
                                      P.fcc_rep, h->d_accept(), h->d_filter(), h->d_state(), colour, h->sm_count, h->stream);
     h->launches++;
     if (rc != 0) { h->err = "packed FCC thread-per-cell launch failed"; return SMCX_E_CUDA; }
+    return SMCX_OK;
+  }
+  if (P.kernel == SMCX_KERNEL_LOCAL_WARP) {
+    const LocalTables T{h->d_epi(), h->d_quad(), h->d_utab(), h->d_ucount(), P.local_umax};
+    const size_t sm = local_smem_bytes(G, P.local_umax);
+    const unsigned grid = (G.cells_per_colour + kLocalWarps - 1) / kLocalWarps;
+    if (G.B == 2) sweep_local_warp<2><<<grid, kLocalWarps * 32, sm, h->stream>>>(G, h->d_species(), T, h->d_accept(), h->d_state(), colour);
+    else sweep_local_warp<4><<<grid, kLocalWarps * 32, sm, h->stream>>>(G, h->d_species(), T, h->d_accept(), h->d_state(), colour);
+    h->launches++;
+    SMCX_CUDA(h, cudaGetLastError());
     return SMCX_OK;
   }
   if (P.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
@@ -699,6 +815,12 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
       const cudaError_t e = configure_group_per_cell(G, h->plan.group_lanes, h->plan.group_warps);
       if (e != cudaSuccess) { h->err = cudaGetErrorString(e); return fail(SMCX_E_CUDA); }
     }
+    if (h->plan.kernel == SMCX_KERNEL_LOCAL_WARP) {
+      const int lsm = (int)local_smem_bytes(G, h->plan.local_umax);
+      cudaError_t e = cudaFuncSetAttribute(sweep_local_warp<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, lsm);
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_local_warp<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lsm);
+      if (e != cudaSuccess) { h->err = cudaGetErrorString(e); return fail(SMCX_E_CUDA); }
+    }
     if (h->plan.kernel == SMCX_KERNEL_WARP_PER_CELL) {
       if (sm > 227 * 1024) return fail(SMCX_E_LINK_CELL_TOO_SMALL);
       cudaError_t e = G.B == 2
@@ -722,6 +844,14 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     if (h->plan.kernel == SMCX_KERNEL_GROUP_PER_CELL) {
       group_build_table(h->plan.G, h->plan.group_lanes, h->epi.data(), gtab);
       SMCX_CUDA(h, cudaMemcpyAsync(h->d_gtable(), gtab.data(), gtab.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+    }
+    std::vector<LocalUEntry> utab;
+    std::vector<int> ucount;
+    if (h->plan.model == SMCX_MODEL_LOCAL) {
+      build_local_utable(h->plan, p->lattice, utab, ucount);
+      SMCX_CUDA(h, cudaMemcpyAsync(h->d_quad(), p->local_quad, (size_t)p->n_shells * n * n * n * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
+      SMCX_CUDA(h, cudaMemcpyAsync(h->d_utab(), utab.data(), utab.size() * sizeof(LocalUEntry), cudaMemcpyHostToDevice, h->stream));
+      SMCX_CUDA(h, cudaMemcpyAsync(h->d_ucount(), ucount.data(), ucount.size() * sizeof(int), cudaMemcpyHostToDevice, h->stream));
     }
     std::vector<uint32_t> flut;
     std::vector<int32_t> fcorr;
@@ -989,6 +1119,12 @@ int smcx_synchronize(smcx_t* h) {
 int smcx_energy(smcx_t* h, int64_t* E) {
   if (!h || !E) return SMCX_E_NULL_ARG;
   DeviceGuard on_device(h->device);
+  if (h->plan.model == SMCX_MODEL_LOCAL) {
+    long long e = 0;
+    const int rc = run_local_energy(h, &e);
+    if (rc == SMCX_OK) *E = e;
+    return rc;
+  }
   std::vector<unsigned long long> M;
   const int rc = run_pair_counts(h, M);
   if (rc != SMCX_OK) return rc;

@@ -171,3 +171,21 @@ def test_sub_warp_tile_layout_is_a_valid_one(lat, dims, n_sp, n_shells, w):
     assert idx.min() >= 0 and idx.max() < L["tile_bytes"] and len(np.unique(idx)) == idx.size
     steps = (offs[:, 0] + L["A"] * offs[:, 1] + L["B"] * offs[:, 2])
     assert (steps % (1 << L["shift"]) == 0).all() and np.abs(steps >> L["shift"]).max() < 32768
+
+
+def test_local_model_parameter_validation():
+    """SMCX_MODEL_LOCAL (reading S12): its own link-cell bound (2w >= 2 r0 + 2R), at most 8 species, weights that keep the
+    int32 dE of a trial exact, no slabs."""
+    from smcx_inputs import make_local_weights
+    w1, w2 = make_local_weights(2, 4, 200, 25, 1)
+    ok = workspace_bytes(**_kw(epi=w1, local_quad=w2))
+    assert ok > 16 * 16 * 16 * 2
+    assert _code(epi=w1, local_quad=w2, link_cell=2) == E["LINK_CELL_TOO_SMALL"]      # fine for the pair model, not here
+    assert workspace_bytes(**_kw(link_cell=2)) > 0
+    w1b, w2b = make_local_weights(2, 9, 200, 25, 1)
+    assert _code(n_species=9, epi=w1b, local_quad=w2b) == E["UNSUPPORTED"]
+    assert _code(epi=w1, local_quad=w2 * 100000) == E["EPI_RANGE"]
+    assert _code(epi=w1, local_quad=w2, kernel=smcx.KERNEL_GROUP_PER_CELL) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_LOCAL_WARP) == E["UNSUPPORTED"]                     # that kernel serves the local model only
+    with pytest.raises(SmcxError):
+        smcx.domain_partition(2, 0, **_kw(dims=(16, 16, 32), epi=w1, local_quad=w2))
