@@ -339,6 +339,28 @@ def run_paper_shaped_fcc(edge: int = 400, sweeps: int = 10):
             "paper_h800_per_gpu": 3.5e9, "paper_note": "PAPER.md:130, EPI model on H800; other hardware and interactions: context"}
 
 
+def run_local_model(edge: int = 128, sweeps: int = 5):
+    """The nonlinear local-energy model (reading S12; the role of the paper's qSRO model):
+    FCC, five species 29/29/28/7/7, three shells, synthetic integer weights; every trial recomputes the local energies of
+    the 86 sites its swap affects.  Device-timed."""
+    import paper_2509_20949_b200 as smcx
+    from smcx_inputs import composition_counts, make_accept_table, make_local_weights
+
+    dims = (edge, edge, edge)
+    w1, w2 = make_local_weights(3, 5, 200, 25, 1007)
+    lat = smcx.Lattice(smcx.FCC, dims, 5, 3, w1, make_accept_table(2500), 1007, link_cell=4, kT_units=2500, local_quad=w2)
+    lat.init_composition(composition_counts(lat.n_sites, (29, 29, 28, 7, 7)))
+    ms = _time_sweeps(lat, 2, sweeps)
+    acc = lat.stats()
+    out = {"workload": f"FCC {edge}^3 conventional cells ({lat.n_sites} sites), 5 species 29/29/28/7/7, 3 shells, local-energy model "
+                       f"eps = W1.n + n.W2.n with synthetic int32 weights, kT=250 meV, link cell 4, seed 1007",
+           "kernel": "sweep_local_warp/u8", "value": lat.n_sites / (ms * 1e-3), "unit": "trial swaps/s", "sweep_ms": ms,
+           "accept_rate": acc[2] / max(1, acc[1]),
+           "paper_qsro_h800_per_gpu": 3.7e7, "paper_note": "PAPER.md:130, qSRO model on H800: another model and GPU, context only"}
+    lat.close()
+    return out
+
+
 def run_largest_single_gpu(sweeps: int = 20):
     """BASELINE.json configs[4]: BCC 2000^3, 1.6e10 sites (4 GB in 2-bit storage), device-timed."""
     import paper_2509_20949_b200 as smcx
@@ -636,6 +658,8 @@ def run_cuda(args, cfg, rank, world, local_rank):
                 out["paper_shaped_fcc"] = run_paper_shaped_fcc(args.fcc_edge)
             if args.largest and args.config != 5:
                 out["largest_single_gpu"] = run_largest_single_gpu()
+            if args.local_edge > 0:
+                out["local_energy_model"] = run_local_model(args.local_edge)
             if args.slabs_leg and cfg.dims[2] // cfg.link_cell >= 16:
                 out["lattice_parallel_one_gpu"] = run_lattice_parallel_one_gpu(cfg, whole_sweep_ms=sweep_ms / args.steps)
         print(json.dumps(out))
@@ -660,6 +684,8 @@ def main():
                          "conventional cells per edge (0: skip)")
     ap.add_argument("--no-largest", dest="largest", action="store_false",
                     help="skip the BCC 2000^3 (1.6e10 sites) leg that the default run adds as `largest_single_gpu`")
+    ap.add_argument("--local-edge", type=int, default=128,
+                    help="with --ensemble: also time the nonlinear local-energy model on an FCC lattice of this edge (0: skip)")
     ap.add_argument("--no-slabs-leg", dest="slabs_leg", action="store_false",
                     help="skip the `lattice_parallel_one_gpu` leg (the workload cut into 2 / 4 slabs on this one GPU)")
     ap.add_argument("--multi", default="slabs", choices=["slabs", "replicas"],

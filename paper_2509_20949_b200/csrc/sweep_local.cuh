@@ -41,22 +41,33 @@ struct LocalTables {
   int umax;
 };
 
-// eps(c, counts): cnt[s] holds the counts of shell s, species x in bits 8x .. 8x + 7
+// eps(c, counts): cnt[s] holds the counts of shell s, species x in bits 8x .. 8x + 7.  The loops run over all
+// kLocalMaxSpecies fields with compile-time bounds (fields of species >= n are zero, their weights are not read), so
+// that the weight loads of a shell are independent of one another and can all be in flight.
+// (Evaluating only the shells in which a site sees i or j -- the others cancel between before and after -- was
+// measured slower: the lanes of a warp then need different shells and the shell loops diverge; 1.0e8 -> 7.0e7 trials/s.)
 __device__ __forceinline__ int local_eps(const int32_t* __restrict__ s_w1, const int32_t* __restrict__ s_w2, int n, int n_shells,
                                          int c, const unsigned long long (&cnt)[kMaxShells]) {
   int e = 0;
 #pragma unroll
   for (int s = 0; s < kMaxShells; ++s) {
-    if (s >= n_shells) break;
-    const int32_t* l = s_w1 + (s * n + c) * n;
-    const int32_t* q = s_w2 + (s * n + c) * n * n;
-    const unsigned long long v = cnt[s];
-    for (int x = 0; x < n; ++x) {
-      const int nx = (int)((v >> (8 * x)) & 255ull);
-      if (nx == 0) continue;
-      int row = l[x];
-      for (int y = x; y < n; ++y) row += q[x * n + y] * (int)((v >> (8 * y)) & 255ull);
-      e += row * nx;
+    if (s < n_shells) {
+      const int32_t* l = s_w1 + (s * n + c) * n;
+      const int32_t* q = s_w2 + (s * n + c) * n * n;
+      const unsigned long long v = cnt[s];
+      int nx[kLocalMaxSpecies];
+#pragma unroll
+      for (int x = 0; x < kLocalMaxSpecies; ++x) nx[x] = (int)((v >> (8 * x)) & 255ull);
+#pragma unroll
+      for (int x = 0; x < kLocalMaxSpecies; ++x) {
+        if (x < n) {
+          int row = l[x];
+#pragma unroll
+          for (int y = x; y < kLocalMaxSpecies; ++y)
+            if (y < n) row += q[x * n + y] * nx[y];
+          e += row * nx[x];
+        }
+      }
     }
   }
   return e;
@@ -165,8 +176,11 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
 #pragma unroll
               for (int s = 0; s < kMaxShells; ++s) {
                 cnt[s] = 0ull;
-                if (s < n_shells)
-                  for (int mm = s_start[s]; mm < s_start[s + 1]; ++mm) cnt[s] += 1ull << (8 * (int)tile[su + dl[mm]]);
+                if (s < n_shells) {
+                  const int m1 = s_start[s + 1];
+#pragma unroll 6
+                  for (int mm = s_start[s]; mm < m1; ++mm) cnt[s] += 1ull << (8 * (int)tile[su + dl[mm]]);   // six loads in flight
+                }
               }
               const int c0 = tile[su];
               const int before = local_eps(s_w1, s_w2, n, n_shells, c0, cnt);
