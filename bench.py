@@ -386,13 +386,15 @@ def run_lattice_parallel_one_gpu(cfg, sweeps: int = 10, whole_sweep_ms=None):
 
     out = {"workload": workload_string(cfg), "note": "all slabs on one GPU: cost of the decomposition, not scaling",
            "undivided_sweep_ms": whole_sweep_ms, "runs": []}
-    for n_slabs, overlap in ((2, True), (4, True), (4, False)):
+    for n_slabs, overlap in ((2, 1), (4, 1), (4, 2), (4, 0)):
         g = smcx.DomainGroup.from_config(cfg, n_slabs, overlap=overlap)
         ms = _time_sweeps(g, 3, sweeps)
         b0 = g.message_bytes
         g.sweep(1)
         g.synchronize()
-        out["runs"].append({"slabs": n_slabs, "overlap": overlap, "sweep_ms": ms, "value": cfg.n_sites / (ms * 1e-3),
+        out["runs"].append({"slabs": n_slabs, "mode": {0: "pass, then copy", 1: "boundary row first, message fused into its kernel",
+                                                        2: "boundary row first, message copied on a second stream"}[overlap],
+                            "fused_messages_per_sweep": int(g.fused_messages // max(1, g.stats()[0])), "sweep_ms": ms, "value": cfg.n_sites / (ms * 1e-3),
                             "unit": "trial swaps/s", "message_bytes_per_sweep": int(g.message_bytes - b0),
                             "vs_undivided": (whole_sweep_ms / ms) if whole_sweep_ms else None})
         g.close()

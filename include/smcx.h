@@ -297,7 +297,8 @@ int64_t smcx_ensemble_kernel_launches(smcx_ensemble_t *e); /* ensemble kernels +
  * Two ways to run it.  smcx_domain_group_*: all slabs in one process, on one or several devices, messages as
  * device-to-device / peer copies ordered by events -- no host synchronisation inside a sweep.  smcx_domain_*: one slab
  * per handle (one process per GPU); the caller moves the messages (e.g. torch.distributed send/recv over NCCL on the
- * byte ranges the message calls name) between smcx_domain_pass calls. */
+ * byte ranges the message calls name) between smcx_domain_pass calls.  Within one process the pass messages of the packed
+ * kernels are fused into the sweep kernel (smcx_domain_pass_fused): the group then moves only the window shift by copy. */
 typedef struct smcx_domain smcx_domain_t;
 typedef struct smcx_domain_group smcx_domain_group_t;
 
@@ -347,6 +348,14 @@ int smcx_domain_set_sweep_counter(smcx_domain_t *d, int64_t t);
 int smcx_domain_begin_sweep(smcx_domain_t *d, smcx_domain_msg_t *send, smcx_domain_msg_t *recv);
 int smcx_domain_pass(smcx_domain_t *d, int32_t colour, int32_t part);
 int smcx_domain_pass_messages(smcx_domain_t *d, int32_t colour, smcx_domain_msg_t *send, smcx_domain_msg_t *recv);
+/* The boundary row of a pass (part 1) with its message FUSED into the kernel: while a cell writes its tile back it also
+ * stores the layers of the outgoing message straight into the neighbour's species storage -- only the bytes it modified,
+ * no copy kernel, no copy engine (peer stores over NVLink when the neighbour is on another GPU of this process).
+ * peer_storage = smcx_domain_storage() of the neighbour the pass sends to (a device pointer valid in this process, peer
+ * access enabled if it is on another device), peer_offset = the byte offset its smcx_domain_pass_messages gives for the
+ * incoming message.  The neighbour's next pass must wait for this launch (an event), nothing else.  SMCX_E_UNSUPPORTED
+ * if the slab's kernel has no fused write-back (the packed kernels THREAD_* and FCC_THREAD have): use part 1 + a copy. */
+int smcx_domain_pass_fused(smcx_domain_t *d, int32_t colour, void *peer_storage, int64_t peer_offset);
 int smcx_domain_end_sweep(smcx_domain_t *d);
 /* Partial results; their sums over the slabs are those of the whole lattice.  pair_counts: positive-half counts
  * M[s][x][y] of the bonds of the layers the slab owns; running energy / trace: the slab's share of H at the start plus
@@ -363,7 +372,9 @@ int smcx_sro_from_counts(const smcx_params_t *p, const int64_t *half_counts, dou
 
 /* All slabs in one process.  devices: n_domains device ordinals, or NULL = all on p->device (slabs of one GPU; what
  * the tests run).  Slabs on different devices need peer access (NVLink): SMCX_E_CUDA if a device cannot reach its
- * neighbours.  overlap != 0: boundary row first, message in flight while the other rows run (CCO).  p->stream orders
+ * neighbours.  overlap: 0 = a pass is one launch per slab, then the messages are copied; 1 = boundary row first, its message
+ * under way while the other rows run (CCO), fused into the boundary-row kernel where the slab's kernel can
+ * (smcx_domain_pass_fused), else a copy on a second stream; 2 = as 1 but always by copy.  p->stream orders
  * the group's calls: they fork from it and join it.  p->d_workspace is ignored (the library allocates). */
 int smcx_domain_group_create(smcx_domain_group_t **out, const smcx_params_t *p, int32_t n_domains, const int32_t *devices,
                              int32_t overlap);
@@ -382,7 +393,8 @@ int smcx_domain_group_sro(smcx_domain_group_t *g, double *alpha, int64_t *pair_c
 int smcx_domain_group_stats(smcx_domain_group_t *g, int64_t *sweeps_done, int64_t *trials, int64_t *accepted);
 int smcx_domain_group_synchronize(smcx_domain_group_t *g);
 int64_t smcx_domain_group_kernel_launches(smcx_domain_group_t *g);
-int64_t smcx_domain_group_message_bytes(smcx_domain_group_t *g);              /* bytes moved between slabs so far */
+int64_t smcx_domain_group_message_bytes(smcx_domain_group_t *g);              /* bytes moved between slabs by copies so far */
+int64_t smcx_domain_group_fused_messages(smcx_domain_group_t *g);             /* pass messages written by the sweep kernels themselves */
 
 const char *smcx_last_error(smcx_t *h); /* text of the last CUDA error seen by this handle */
 const char *smcx_strerror(int code);

@@ -162,6 +162,8 @@ def load_library(build_if_missing: bool = True):
         "smcx_domain_group_synchronize": (C.c_int, [vp]),
         "smcx_domain_group_kernel_launches": (C.c_int64, [vp]),
         "smcx_domain_group_message_bytes": (C.c_int64, [vp]),
+        "smcx_domain_group_fused_messages": (C.c_int64, [vp]),
+        "smcx_domain_pass_fused": (C.c_int, [vp, C.c_int32, vp, C.c_int64]),
         "smcx_last_error": (C.c_char_p, [vp]),
         "smcx_strerror": (C.c_char_p, [C.c_int]),
         "smcx_version": (C.c_char_p, []),
@@ -665,6 +667,15 @@ class Domain:
     def run_pass(self, colour, part=0):
         self._check(self._lib.smcx_domain_pass(self._d, int(colour), int(part)), "smcx_domain_pass")
 
+    def run_pass_fused(self, colour, peer_storage_ptr, peer_offset):
+        """smcx_domain_pass_fused: the boundary row of the pass, storing its message into the neighbour's storage."""
+        self._check(self._lib.smcx_domain_pass_fused(self._d, int(colour), C.c_void_p(int(peer_storage_ptr)), int(peer_offset)),
+                    "smcx_domain_pass_fused")
+
+    @property
+    def storage_ptr(self) -> int:
+        return int(self._lib.smcx_domain_storage(self._d))
+
     def pass_messages(self, colour):
         send, recv = DomainMsg(), DomainMsg()
         self._check(self._lib.smcx_domain_pass_messages(self._d, int(colour), C.byref(send), C.byref(recv)), "smcx_domain_pass_messages")
@@ -728,7 +739,7 @@ class DomainGroup:
                 raise ValueError("devices must have one entry per slab")
             dev = (C.c_int32 * n_domains)(*[int(x) for x in devices])
         g = C.c_void_p()
-        rc = lib.smcx_domain_group_create(C.byref(g), C.byref(p), int(n_domains), dev, 1 if overlap else 0)
+        rc = lib.smcx_domain_group_create(C.byref(g), C.byref(p), int(n_domains), dev, int(overlap))   # 0 / 1 (True) / 2
         if rc != 0:
             raise SmcxError(rc, "smcx_domain_group_create")
         self._g = g
@@ -834,3 +845,7 @@ class DomainGroup:
     @property
     def message_bytes(self) -> int:
         return int(self._lib.smcx_domain_group_message_bytes(self._g))
+
+    @property
+    def fused_messages(self) -> int:
+        return int(self._lib.smcx_domain_group_fused_messages(self._g))

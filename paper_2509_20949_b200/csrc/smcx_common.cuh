@@ -83,6 +83,12 @@ struct Geom {
   //   cz_global  first link-cell row of the slab in the whole lattice (cell ids are global: they key the Philox stream);
   //   iz_first   first row pair a launch works on (a pass may be split into the boundary row and the rest).
   int z_bias, cz_global, iz_first;
+  // Fused ghost-layer message (domain_api.inc): while it writes its tile back, the boundary row of a slab also stores the
+  // layers [peer_z0, peer_z1) of its window into the neighbour slab's storage (a device pointer in this process: the same
+  // GPU, or a peer GPU over NVLink), at the same word index of `peer_lat` = neighbour storage shifted by the difference
+  // of the two windows.  0 = no mirroring.
+  unsigned long long peer_lat;
+  int peer_z0, peer_z1;
   int pc_z0, pc_z1;    // pair-count kernels: layers [pc_z0, pc_z1) of the source sites (the whole lattice, or the layers a slab owns)
   int work_base;       // 0 or 8: which half of DevState::work a launch of sweep_fcc_thread draws its batches from
   unsigned cells_per_colour;

@@ -407,20 +407,27 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
       // a7: write back rows 1..6 x 1..6 of every sublattice: the bytes that lie wholly inside this tile
       {
         const uint32_t dwh = (uint32_t)(whi - wlo) * 4u;            // word step from the low to the high group of a row
+        uint32_t* const peer = reinterpret_cast<uint32_t*>(G.peer_lat);
         auto wb = [&](auto cc) {
           constexpr int C = decltype(cc)::value;
 #pragma unroll 1
           for (int rz = 1; rz < 7; ++rz) {
             int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
+            // fused ghost-layer message: layers the neighbour slab holds a copy of also go into its storage
+            const bool mirror = peer != nullptr && gz >= G.peer_z0 && gz < G.peer_z1;
 #pragma unroll
             for (int ry = 1; ry < 7; ++ry) {
               int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
               const uint32_t base = (((uint32_t)gz * zstride) + (uint32_t)gy * (uint32_t)rw + (uint32_t)wlo) * 4u;
 #pragma unroll
-              for (int s = 0; s < 4; ++s)
+              for (int s = 0; s < 4; ++s) {
+                const uint32_t v = tile[(s * kFccRows + rz * 8 + ry) * NT];
                 store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(lattice + base + s),
-                                                     reinterpret_cast<unsigned char*>(lattice + (uint32_t)(base + s + dwh)),
-                                                     tile[(s * kFccRows + rz * 8 + ry) * NT]);
+                                                     reinterpret_cast<unsigned char*>(lattice + (uint32_t)(base + s + dwh)), v);
+                if (mirror)
+                  store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(peer + base + s),
+                                                       reinterpret_cast<unsigned char*>(peer + (uint32_t)(base + s + dwh)), v);
+              }
             }
           }
         };

@@ -461,6 +461,7 @@ __device__ __forceinline__ void write_back_tile(const Geom& G, const uint32_t* t
     int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
     offy[ry - 1] = (uint32_t)gy * (uint32_t)rw + (uint32_t)wlo;
   }
+  uint32_t* const peer = reinterpret_cast<uint32_t*>(G.peer_lat);
 #pragma unroll 1
   for (int rz = 1; rz < 7; ++rz) {
     int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
@@ -471,6 +472,16 @@ __device__ __forceinline__ void write_back_tile(const Geom& G, const uint32_t* t
       store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(lattice + idx),
                                            reinterpret_cast<unsigned char*>(lattice + (uint32_t)(idx + dwh)),
                                            tile[(rz * 8 + ry) * NT]);
+    }
+    // fused ghost-layer message: the layers the neighbour slab holds a copy of go straight into its storage
+    if (peer != nullptr && gz >= G.peer_z0 && gz < G.peer_z1) {
+#pragma unroll
+      for (int ry = 1; ry < 7; ++ry) {
+        const uint32_t idx = zoff + offy[ry - 1];
+        store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(peer + idx),
+                                             reinterpret_cast<unsigned char*>(peer + (uint32_t)(idx + dwh)),
+                                             tile[(rz * 8 + ry) * NT]);
+      }
     }
   }
 }

@@ -1,11 +1,15 @@
 import os
 import sys
+import time
 
 import pytest
 
 ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
+
+
+SESSION_START = time.time()      # tests that take minutes of oracle time look at how much of the run's budget is left
 
 
 def pytest_configure(config):

@@ -38,7 +38,7 @@ BCC_KERNELS = [(smcx.KERNEL_THREAD_PERSISTENT, "persistent"), (smcx.KERNEL_THREA
 
 
 @pytest.mark.parametrize("kernel", [k for k, _ in BCC_KERNELS], ids=[n for _, n in BCC_KERNELS])
-@pytest.mark.parametrize("n_slabs,overlap", [(2, True), (4, True), (4, False)])
+@pytest.mark.parametrize("n_slabs,overlap", [(2, 1), (4, 1), (4, 2), (4, 0)])   # 1: fused / overlapped, 2: overlapped copies, 0: plain
 def test_bcc_slabs_against_the_undivided_oracle(kernel, n_slabs, overlap):
     kw = _kw(smcx.BCC, (16, 16, 32), 4, 2, seed=77)
     o = _oracle(kw)
@@ -51,6 +51,8 @@ def test_bcc_slabs_against_the_undivided_oracle(kernel, n_slabs, overlap):
         assert (g.species() == o.species()).all()
     _assert_same(g, o)
     assert g.message_bytes > 0 and g.kernel_launches > 0
+    packed = kernel in (smcx.KERNEL_THREAD_PERSISTENT, smcx.KERNEL_THREAD_PER_CELL)
+    assert (g.fused_messages > 0) == (packed and overlap == 1)    # the packed kernels write their pass messages themselves
     g.close()
 
 
@@ -60,11 +62,14 @@ def test_bcc_slabs_against_the_undivided_oracle(kernel, n_slabs, overlap):
 def test_fcc_five_species_slabs_against_the_undivided_oracle(kernel, storage, dims, n_slabs):
     kw = _kw(smcx.FCC, dims, 5, 3, seed=31, kT=690, amp=400)
     o = _oracle(kw)
-    g = smcx.DomainGroup(n_slabs, kernel=kernel, storage=storage, **kw)
-    g.sweep(6)
-    o.sweep(6)
-    _assert_same(g, o)
-    g.close()
+    for overlap in (1, 2):
+        g = smcx.DomainGroup(n_slabs, kernel=kernel, storage=storage, overlap=overlap, **kw)
+        g.sweep(6)
+        if overlap == 1:
+            o.sweep(6)
+        _assert_same(g, o)
+        assert (g.fused_messages > 0) == (kernel == smcx.KERNEL_FCC_THREAD and overlap == 1)
+        g.close()
 
 
 def test_uneven_slabs_anneal_upload_and_resume():
