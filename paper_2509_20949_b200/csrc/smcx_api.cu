@@ -264,7 +264,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   if (fcc_ok) {
     std::vector<uint32_t> lut;
     std::vector<int32_t> corr;
-    fcc_ok = fcc_build_lut(p->epi, n, p->n_shells, 1, lut, corr) && fcc_build_tables<32>(G, plan->fcc_tables);
+    fcc_ok = fcc_build_lut(p->epi, n, p->n_shells, 1, lut, corr) && fcc_build_tables<32, kFccWinRows>(G, plan->fcc_tables);
     plan->fcc_rep = fcc_lut_rep(n);
   }
   int kernel = p->kernel, storage = p->storage;

@@ -42,14 +42,16 @@
 
 namespace smcxk {
 
-constexpr int kFccWarps = 6;                 // 6 x 32 KB of tiles + tables in 227 KB
-constexpr int kFccRows = 64;                 // rows (y + 8 z) per sublattice of a tile
+constexpr int kFccWarps = 8;                 // 8 x 24 KB of tile windows + tables in 227 KB
+constexpr int kFccRows = 64;                 // rows (y + 8 z) per sublattice of a whole tile (8 layers)
+constexpr int kFccWinLayers = 6;             // z layers of the tile the kernel keeps in shared memory at a time
+constexpr int kFccWinRows = 8 * kFccWinLayers;
 constexpr int kFccMaxSpecies = 8;            // PRMT selectors are 3 bits
 constexpr int kFccBias = 32768;              // D + bias is looked up as two unsigned bytes
 
-template <int NT> struct FccTile {
+template <int NT, int ROWS = kFccRows> struct FccTile {
   static constexpr int kRow = 4 * NT;                 // bytes from one row to the next (NT lanes interleaved)
-  static constexpr int kSub = kFccRows * kRow;        // bytes from one sublattice to the next
+  static constexpr int kSub = ROWS * kRow;            // bytes from one sublattice to the next (ROWS rows each)
 };
 
 // Direction table, [b][dir]: what the partner j = i + O_0[dir] of a site of sublattice b needs.
@@ -70,7 +72,7 @@ __host__ __device__ constexpr int fcc_base_adj(int bs, int k) {
 }
 
 // Host: the table for row stride NT, from the shell-0 offsets of G (ascending (dz, dy, dx), S0).
-template <int NT>
+template <int NT, int ROWS = kFccRows>
 inline bool fcc_build_tables(const Geom& G, FccTables& T) {
   if (G.Z0 != 12) return false;
   for (int b = 0; b < 4; ++b)
@@ -87,7 +89,7 @@ inline bool fcc_build_tables(const Geom& G, FccTables& T) {
       const int dr = cell[1] + 8 * cell[2];
       FccDirEntry& e = T.dir[b][d];
       for (int k = 0; k < 4; ++k)
-        e.d[k] = ((bj ^ k) - b) * FccTile<NT>::kSub + (dr + fcc_base_adj(bj, k)) * FccTile<NT>::kRow;
+        e.d[k] = ((bj ^ k) - b) * FccTile<NT, ROWS>::kSub + (dr + fcc_base_adj(bj, k)) * FccTile<NT, ROWS>::kRow;
       e.e3 = 4 * cell[0];
       e.e2 = 4 * (cell[0] + fcc_beta(bj, 0) - 1);
       e.pad0 = e.pad1 = 0;
@@ -233,10 +235,10 @@ __host__ __device__ __forceinline__ FccLut fcc_load_lut(smem_ptr_t p) {
 
 // One trial (a4-a6).  p_own: row r of sublattice b in this lane's tile; X4 = 4 X, X the nibble of site i; E = the
 // direction-table entry of (b, drawn direction); u = acceptance draw.
-template <int b, int NT, bool kFilter>
+template <int b, int NT, bool kFilter, int ROWS = kFccRows>
 __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4, const FccDirEntry& E, uint32_t u,
                                                    const FccEnv& env, int& esum, unsigned& nacc) {
-  using T = FccTile<NT>;
+  using T = FccTile<NT, ROWS>;
   FccSite si, sj;
   si.p0 = p_own;
   si.p1 = fcc_at<NT>(p_own, ((b ^ 1) - b) * T::kSub + fcc_base_adj(b, 1) * T::kRow);
@@ -285,7 +287,7 @@ __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4,
 
 #ifdef __CUDACC__
 inline size_t fcc_smem_bytes(int rep) {
-  return (size_t)kFccWarps * FccTile<32>::kSub * 4 + (size_t)64 * 3 * rep * 16 + 64 * 4 + kFilterWords * 4 + sizeof(FccTables);
+  return (size_t)kFccWarps * FccTile<32, kFccWinRows>::kSub * 4 + (size_t)64 * 3 * rep * 16 + 64 * 4 + kFilterWords * 4 + sizeof(FccTables);
 }
 // replicas of the look-up rows: as many (8, 4, 2, 1) as fit next to the tiles
 inline int fcc_lut_rep(int n_species) {
@@ -303,8 +305,9 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
   constexpr int NT = 32;
   extern __shared__ __align__(16) uint32_t smem_w[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  uint32_t* tile = smem_w + warp * (4 * kFccRows * NT) + lane;                 // word (s * 64 + row) at tile[(s * 64 + row) * NT]
-  uint4* s_lut = reinterpret_cast<uint4*>(smem_w + kFccWarps * (4 * kFccRows * NT));
+  constexpr int WR = kFccWinRows;                                              // rows per sublattice of the resident window
+  uint32_t* tile = smem_w + warp * (4 * WR * NT) + lane;                       // word (s * WR + row) at tile[(s * WR + row) * NT]
+  uint4* s_lut = reinterpret_cast<uint4*>(smem_w + kFccWarps * (4 * WR * NT));
   int32_t* s_corr = reinterpret_cast<int32_t*>(s_lut + 64 * 3 * rep);
   uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_corr + 64);
   FccDirEntry* s_dir = reinterpret_cast<FccDirEntry*>(s_filt + kFilterWords);
@@ -353,16 +356,37 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
       const int t0z = tile_z0(G, oz, cz);
       const int wlo = x0 >> 3, sh = 4 * (x0 & 7);
       const int whi = wlo + 1 == rw ? 0 : wlo + 1;
-      // a3: stage the tile: per row two 16-byte groups (four sublattice words each), funnel-shifted into four tile words
-      {
-        uint32_t offy[8];
+      // The tile of a cell is 8 layers of conventional cells, but a trial in layer lz of the cell only touches the tile
+      // layers lz .. lz + 4.  The kernel keeps six layers resident (24 KB per warp instead of 32: eight warps per SM
+      // instead of six) and runs the cell in two halves: tile layers 0..5 for lz = 0, 1; then layer 1 is written back
+      // (layer 0 is never written), layers 2..5 move down two slots, layers 6, 7 are staged, and lz = 2, 3 run on
+      // tile layers 2..7.  Slot of tile layer rz in half h: rz - 2 h.
+      uint32_t offy[8];
 #pragma unroll
-        for (int ry = 0; ry < 8; ++ry) {
-          int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
-          offy[ry] = (uint32_t)gy * (uint32_t)rw;
-        }
+      for (int ry = 0; ry < 8; ++ry) {
+        int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
+        offy[ry] = (uint32_t)gy * (uint32_t)rw;
+      }
+      const uint32_t cell_id = global_cell_id(G, cx, cy, cz);
+      const PhiloxCell pc = philox_cell_setup(cell_id, t, ctr3, G.rk0, G.rk1);
+      const uint32_t dwh = (uint32_t)(whi - wlo) * 4u;            // word step from the low to the high group of a row
+      uint32_t* const peer = reinterpret_cast<uint32_t*>(G.peer_lat);
+      int esum = 0;
 #pragma unroll 1
-        for (int rz = 0; rz < 8; ++rz) {
+      for (int half = 0; half < 2; ++half) {
+        if (half == 1) {
+          // tile layers 2..5 move from slots 2..5 to slots 0..3
+#pragma unroll 1
+          for (int s = 0; s < 4; ++s) {
+            uint32_t* d = tile + s * WR * NT;
+#pragma unroll 8
+            for (int r = 0; r < 32; ++r) d[r * NT] = d[(r + 16) * NT];
+          }
+        }
+        // a3: stage tile layers [0, 6) / [6, 8): per row two 16-byte groups (four sublattice words each), funnel-shifted
+        // into four tile words
+#pragma unroll 1
+        for (int rz = half ? 6 : 0; rz < (half ? 8 : 6); ++rz) {
           int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
           const uint32_t zoff = (uint32_t)gz * zstride;
           uint4 lo[8], hi[8];
@@ -374,54 +398,46 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
           }
 #pragma unroll
           for (int ry = 0; ry < 8; ++ry) {
-            uint32_t* d = tile + (rz * 8 + ry) * NT;
-            d[0 * kFccRows * NT] = __funnelshift_r(lo[ry].x, hi[ry].x, sh);
-            d[1 * kFccRows * NT] = __funnelshift_r(lo[ry].y, hi[ry].y, sh);
-            d[2 * kFccRows * NT] = __funnelshift_r(lo[ry].z, hi[ry].z, sh);
-            d[3 * kFccRows * NT] = __funnelshift_r(lo[ry].w, hi[ry].w, sh);
+            uint32_t* d = tile + ((rz - 2 * half) * 8 + ry) * NT;
+            d[0 * WR * NT] = __funnelshift_r(lo[ry].x, hi[ry].x, sh);
+            d[1 * WR * NT] = __funnelshift_r(lo[ry].y, hi[ry].y, sh);
+            d[2 * WR * NT] = __funnelshift_r(lo[ry].z, hi[ry].z, sh);
+            d[3 * WR * NT] = __funnelshift_r(lo[ry].w, hi[ry].w, sh);
           }
         }
-      }
-      // a4-a6: the 256 trials of the cell, raster order: conventional cell c = (lz * 4 + ly) * 4 + lx, then b
-      const uint32_t cell_id = global_cell_id(G, cx, cy, cz);
-      const PhiloxCell pc = philox_cell_setup(cell_id, t, ctr3, G.rk0, G.rk1);
-      int esum = 0;
+        // a4-a6: 128 of the 256 trials of the cell, raster order: conventional cell c = (lz * 4 + ly) * 4 + lx, then b
 #pragma unroll 1
-      for (int c = 0; c < 64; ++c) {
-        const uint32_t X4 = 4u * (uint32_t)((c & 3) + 2);
-        const int row = ((c >> 2) & 3) + 2 + 8 * ((c >> 4) + 2);
-        uint32_t* p_row = tile + row * NT;
-        const Philox4 r0 = philox_factored(pc, s_slot[2 * c], G.rk0, G.rk1);
-        const Philox4 r1 = philox_factored(pc, s_slot[2 * c + 1], G.rk0, G.rk1);
+        for (int c = 32 * half; c < 32 * half + 32; ++c) {
+          const uint32_t X4 = 4u * (uint32_t)((c & 3) + 2);
+          const int row = ((c >> 2) & 3) + 2 + 8 * ((c >> 4) + 2 - 2 * half);
+          uint32_t* p_row = tile + row * NT;
+          const Philox4 r0 = philox_factored(pc, s_slot[2 * c], G.rk0, G.rk1);
+          const Philox4 r1 = philox_factored(pc, s_slot[2 * c + 1], G.rk0, G.rk1);
 #define SMCX_FCC_TRIAL(B, WDIR, U)                                                                          \
-        {                                                                                                     \
-          const smem_ptr_t ep = dir_p + (B * 12u + mulhi_u32(WDIR, 12u)) * 32u;                              \
-          const int4 e = lds_int4(ep, 0), f = lds_int4(ep, 16);                                               \
-          const FccDirEntry E{{e.x, e.y, e.z, e.w}, f.x, f.y, 0, 0};                                          \
-          fcc_trial<B, NT, kFilter>(p_row + B * (kFccRows * NT), X4, E, U, env, esum, nacc);                  \
-        }
-        SMCX_FCC_TRIAL(0, r0.x, r0.y) SMCX_FCC_TRIAL(1, r0.z, r0.w) SMCX_FCC_TRIAL(2, r1.x, r1.y) SMCX_FCC_TRIAL(3, r1.z, r1.w)
+          {                                                                                                   \
+            const smem_ptr_t ep = dir_p + (B * 12u + mulhi_u32(WDIR, 12u)) * 32u;                            \
+            const int4 e = lds_int4(ep, 0), f = lds_int4(ep, 16);                                             \
+            const FccDirEntry E{{e.x, e.y, e.z, e.w}, f.x, f.y, 0, 0};                                        \
+            fcc_trial<B, NT, kFilter, WR>(p_row + B * (WR * NT), X4, E, U, env, esum, nacc);                  \
+          }
+          SMCX_FCC_TRIAL(0, r0.x, r0.y) SMCX_FCC_TRIAL(1, r0.z, r0.w) SMCX_FCC_TRIAL(2, r1.x, r1.y) SMCX_FCC_TRIAL(3, r1.z, r1.w)
 #undef SMCX_FCC_TRIAL
-      }
-      esum_total += esum;     // |dE| < 2^23 (host check), 256 trials: exact in int32 per cell
-      // a7: write back rows 1..6 x 1..6 of every sublattice: the bytes that lie wholly inside this tile
-      {
-        const uint32_t dwh = (uint32_t)(whi - wlo) * 4u;            // word step from the low to the high group of a row
-        uint32_t* const peer = reinterpret_cast<uint32_t*>(G.peer_lat);
+        }
+        // a7: write back rows 1..6 of tile layer 1 (first half) / of tile layers 2..6 (second half), every sublattice:
+        // the bytes that lie wholly inside this tile
         auto wb = [&](auto cc) {
           constexpr int C = decltype(cc)::value;
 #pragma unroll 1
-          for (int rz = 1; rz < 7; ++rz) {
+          for (int rz = half ? 2 : 1; rz < (half ? 7 : 2); ++rz) {
             int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
             // fused ghost-layer message: layers the neighbour slab holds a copy of also go into its storage
             const bool mirror = peer != nullptr && gz >= G.peer_z0 && gz < G.peer_z1;
 #pragma unroll
             for (int ry = 1; ry < 7; ++ry) {
-              int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
-              const uint32_t base = (((uint32_t)gz * zstride) + (uint32_t)gy * (uint32_t)rw + (uint32_t)wlo) * 4u;
+              const uint32_t base = (((uint32_t)gz * zstride) + offy[ry] + (uint32_t)wlo) * 4u;
 #pragma unroll
               for (int s = 0; s < 4; ++s) {
-                const uint32_t v = tile[(s * kFccRows + rz * 8 + ry) * NT];
+                const uint32_t v = tile[(s * WR + (rz - 2 * half) * 8 + ry) * NT];
                 store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(lattice + base + s),
                                                      reinterpret_cast<unsigned char*>(lattice + (uint32_t)(base + s + dwh)), v);
                 if (mirror)
@@ -442,6 +458,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
           default: wb(std::integral_constant<int, 7>{}); break;
         }
       }
+      esum_total += esum;     // |dE| < 2^23 (host check), 256 trials: exact in int32 per cell
     }
   }
   // a8: one atomic pair per block
