@@ -44,9 +44,12 @@ struct LocalTables {
 // eps(c, counts): cnt[s] holds the counts of shell s, species x in bits 8x .. 8x + 7.  The loops run over all
 // kLocalMaxSpecies fields with compile-time bounds (fields of species >= n are zero, their weights are not read), so
 // that the weight loads of a shell are independent of one another and can all be in flight.
+// Not inlined, and the loop over the basis index in the kernel is not unrolled: with both inlined / unrolled the trial
+// loop was several times the instruction cache and ncu showed the warps waiting for instructions most of the time
+// (stall no_instruction 14.8 per issue).
 // (Evaluating only the shells in which a site sees i or j -- the others cancel between before and after -- was
 // measured slower: the lanes of a warp then need different shells and the shell loops diverge; 1.0e8 -> 7.0e7 trials/s.)
-__device__ __forceinline__ int local_eps(const int32_t* __restrict__ s_w1, const int32_t* __restrict__ s_w2, int n, int n_shells,
+__device__ __noinline__ int local_eps(const int32_t* __restrict__ s_w1, const int32_t* __restrict__ s_w2, int n, int n_shells,
                                          int c, const unsigned long long (&cnt)[kMaxShells]) {
   int e = 0;
 #pragma unroll
@@ -149,7 +152,7 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
       for (int ly = 0; ly < w; ++ly)
         for (int lx = 0; lx < w; ++lx) {
           const int conv = ((lz + H) * TW + (ly + H)) * TW + (lx + H);
-#pragma unroll
+#pragma unroll 1
           for (int b = 0; b < B; ++b, ++k) {
             if ((k & 63) == 0) {   // a4: 32 Philox calls cover the next 64 slots
               const Philox4 r = philox4x32_10(cell_id, (uint32_t)(k >> 1) + lane, t, ctr3, G.key0, G.key1);
