@@ -86,7 +86,7 @@ inline size_t local_smem_bytes(const Geom& G, int umax) {
 }
 
 template <int B>
-__global__ void __launch_bounds__(kLocalWarps * 32)
+__global__ void __launch_bounds__(kLocalWarps * 32, 3)
 sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables T, const uint32_t* __restrict__ accept,
                  DevState* __restrict__ st, int colour) {
   extern __shared__ __align__(16) unsigned char smem[];
