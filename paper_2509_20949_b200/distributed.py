@@ -54,18 +54,22 @@ class SlabRank:
     """One slab of a distributed lattice.  ``dist`` is ``torch.distributed`` (initialised by the caller, e.g. under
     torchrun with the NCCL backend) or None when ``world`` is a LocalWorld shared by the slabs of one process."""
 
-    def __init__(self, rank, world_size, dist=None, world=None, overlap=True, **lattice_kw):
+    def __init__(self, rank, world_size, dist=None, world=None, overlap=True, domain=None, **lattice_kw):
         import torch
 
         self.torch = torch
         self.rank, self.world_size = int(rank), int(world_size)
         self.dist, self.world = dist, world
         self.overlap = bool(overlap)
-        self.domain = _b.Domain(self.world_size, self.rank, **lattice_kw)
-        self.compute = self.domain._stream
-        with torch.cuda.device(self.domain.device):
-            self.side = torch.cuda.Stream(device=self.domain.device)
-        self._kw = {k: lattice_kw[k] for k in ("lattice", "dims", "n_species", "n_shells", "epi", "accept", "seed")}
+        # `domain`: an object with Domain's stepping calls and a `_storage_view` tensor (the host-side tests pass a
+        # stand-in whose storage is a CPU tensor, to run this driver over gloo); by default the slab on the GPU
+        self.domain = domain if domain is not None else _b.Domain(self.world_size, self.rank, **lattice_kw)
+        self.compute = getattr(self.domain, "_stream", None)
+        self.side = None
+        if self.compute is not None:
+            with torch.cuda.device(self.domain.device):
+                self.side = torch.cuda.Stream(device=self.domain.device)
+        self._kw = {k: lattice_kw[k] for k in ("lattice", "dims", "n_species", "n_shells", "epi", "accept", "seed") if k in lattice_kw}
         self._kw["link_cell"] = lattice_kw.get("link_cell", 4)
         self.message_bytes = 0
 
@@ -76,6 +80,8 @@ class SlabRank:
         if self.dist is None:
             self.world.post(self.rank, send, self.domain.storage_view(send))
             return (send, recv)
+        if self.side is None:                      # host stand-in: no streams to order
+            return exchange(self.dist, self.rank, self.domain._storage_view, send, recv)
         self.side.wait_stream(self.compute)
         with self.torch.cuda.stream(self.side):
             return exchange(self.dist, self.rank, self.domain._storage_view, send, recv)

@@ -130,3 +130,86 @@ def test_two_rank_gloo_exchange_moves_the_planned_layers():
         p.join(timeout=60)
         assert p.exitcode == 0
     assert res == [(0, True), (1, True)]
+
+
+class _HostSlab:
+    """Stand-in for binding.Domain with the same stepping calls, its species storage a CPU tensor: a "pass" stamps the
+    layers of its outgoing message with (sweep, phase, rank), so that the receiver can tell whether the driver moved the
+    right bytes at the right time.  The message plan is the library's own (smcx_domain_plan_messages, host arithmetic)."""
+
+    def __init__(self, world, rank, kw):
+        import torch
+        self.world, self.rank, self.kw = world, rank, kw
+        self.info = smcx.domain_partition(world, rank, **kw)
+        self.lb = self.info["layer_bytes"]
+        self._storage_view = torch.zeros(self.info["z_layers"] * self.lb, dtype=torch.uint8)
+        self.sweep, self.log = 0, []
+
+    def _stamp(self, phase):
+        send, _ = smcx.domain_plan_messages(self.world, self.rank, self.sweep, phase, **self.kw)
+        if send[3]:
+            self._storage_view[send[2]: send[2] + send[3]] = (7 * self.sweep + 3 * (phase + 1) + 11 * self.rank) % 251
+
+    def begin_sweep(self):
+        self._stamp(-1)
+        return smcx.domain_plan_messages(self.world, self.rank, self.sweep, -1, **self.kw)
+
+    def pass_messages(self, colour):
+        return smcx.domain_plan_messages(self.world, self.rank, self.sweep, colour, **self.kw)
+
+    def run_pass(self, colour, part=0):
+        self.log.append((self.sweep, colour, part))
+        if part in (0, 1):
+            self._stamp(colour)
+
+    def check(self, phase):
+        _, recv = smcx.domain_plan_messages(self.world, self.rank, self.sweep, phase, **self.kw)
+        if not recv[3]:
+            return True
+        want = (7 * self.sweep + 3 * (phase + 1) + 11 * recv[0]) % 251
+        return bool((self._storage_view[recv[2]: recv[2] + recv[3]] == want).all())
+
+    def end_sweep(self):
+        self.sweep += 1
+
+
+def _driver_worker(rank, world, port, overlap, q):
+    import torch.distributed as dist
+    sys.path.insert(0, ROOT)
+    from paper_2509_20949_b200 import distributed
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    kw = _kw(dims=(16, 16, 32))
+    slab = _HostSlab(world, rank, kw)
+    drv = distributed.SlabRank(rank, world, dist=dist, overlap=overlap, domain=slab)
+    ok = True
+    for _ in range(5):                       # SlabRank.sweep, with a check after every phase
+        drv.phase_end(drv.sweep_begin())
+        ok = ok and slab.check(-1)
+        for colour in range(8):
+            drv.phase_end(drv.pass_begin(colour))
+            ok = ok and slab.check(colour)
+        drv.sweep_end()
+    parts = sorted({p for _, _, p in slab.log})
+    q.put((rank, ok, parts, drv.message_bytes > 0))
+    dist.barrier()
+    dist.destroy_process_group()
+
+
+@pytest.mark.parametrize("overlap", [True, False])
+def test_two_rank_gloo_run_of_the_per_rank_driver(overlap):
+    """paper_2509_20949_b200.distributed.SlabRank -- the loop a torchrun job runs -- over gloo with a host stand-in for
+    the slab: every phase of five sweeps delivers the neighbour's stamped layers, with and without overlap."""
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = 33500 + os.getpid() % 2000 + (1 if overlap else 0)
+    procs = [ctx.Process(target=_driver_worker, args=(r, 2, port, overlap, q)) for r in range(2)]
+    for p in procs:
+        p.start()
+    res = sorted(q.get(timeout=180) for _ in range(2))
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    want_parts = [1, 2] if overlap else [0]
+    assert res == [(0, True, want_parts, True), (1, True, want_parts, True)]
