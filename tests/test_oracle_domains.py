@@ -90,3 +90,23 @@ def test_s11_poison_is_never_read_by_the_undivided_sweep():
     assert before.max() < 5
     o.sweep(2)
     assert np.bincount(o.species(), minlength=5).tolist() == np.bincount(before, minlength=5).tolist()
+
+
+def test_s11_with_the_local_energy_model_needs_three_ghost_layers():
+    """Reading S12 on slabs: a trial of the local model reads neighbours of neighbours (reach r0 + 2R = 5 half-units = 3
+    conventional cells), so the window needs H = 3 ghost layers and the pass message carries H + 1 = 4 layers; with those
+    the decomposed sweep equals the undivided one, with the pair model's two ghost layers poison is read."""
+    from smcx_inputs import make_local_weights
+
+    def lat():
+        w1, w2 = make_local_weights(2, 4, 200, 25, 13)
+        o = oracle.Oracle(oracle.BCC, (16, 16, 32), 4, 2, w1, 4, make_accept_table(900), 13)
+        o.set_local_model(w2)
+        return o
+
+    whole, cut, thin = lat(), lat(), lat()
+    whole.sweep(5)
+    assert cut.sweep_slabs(5, 2, ghost=3, order_seed=3) == 0
+    assert (cut.species() == whole.species()).all() and (cut.energy_trace() == whole.energy_trace()).all()
+    assert cut.energy() == whole.energy() == cut.running_energy()
+    assert thin.sweep_slabs(5, 2, ghost=2) > 0
