@@ -88,7 +88,7 @@ enum { SMCX_KERNEL_AUTO = 0, SMCX_KERNEL_WARP_PER_CELL = 1, SMCX_KERNEL_THREAD_P
  * `local_quad` W2.  With W2 = 0 and W1 symmetric the model is twice the EPI Hamiltonian.  A trial reads the
  * neighbours of the neighbours of i and j, so the link cell must satisfy 2w >= 2 r0 + 2 R; n_species <= 8; uint8
  * storage; kernel SMCX_KERNEL_LOCAL_WARP (one warp per link cell).  smcx_energy returns H of this model;
- * smcx_sro is unchanged.  Not available on slabs (smcx_domain_*). */
+ * smcx_sro is unchanged.  On slabs (smcx_domain_*) the window has H = 3 ghost layers and a pass message 4 layers. */
 enum { SMCX_MODEL_EPI = 0, SMCX_MODEL_LOCAL = 1 };
 
 enum {

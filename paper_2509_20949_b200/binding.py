@@ -562,7 +562,7 @@ class Domain:
     uint8 tensor, so a caller can hand slices of the species storage (`storage_view`) to torch.distributed."""
 
     def __init__(self, n_domains, index, lattice, dims, n_species, n_shells, epi, accept, seed, link_cell=4, kT_units=0,
-                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0, stream=None):
+                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0, stream=None, local_quad=None):
         import torch
 
         if not torch.cuda.is_available():
@@ -570,7 +570,7 @@ class Domain:
         self._lib = lib = load_library()
         self._d = None
         p, keep = _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage,
-                               kernel, device, trace_capacity)
+                               kernel, device, trace_capacity, local_quad=local_quad)
         need = C.c_size_t(0)
         rc = lib.smcx_domain_workspace_bytes(C.byref(p), int(n_domains), int(index), C.byref(need))
         if rc != 0:
@@ -720,7 +720,8 @@ class DomainGroup:
     device-to-device / peer copies.  Same results as a Lattice of the whole."""
 
     def __init__(self, n_domains, lattice, dims, n_species, n_shells, epi, accept, seed, link_cell=4, kT_units=0,
-                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, devices=None, overlap=True, trace_capacity=0):
+                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, devices=None, overlap=True, trace_capacity=0,
+                 local_quad=None):
         import torch
 
         if not torch.cuda.is_available():
@@ -728,7 +729,7 @@ class DomainGroup:
         self._lib = lib = load_library()
         self._g = None
         p, keep = _make_params(lattice, dims, n_species, n_shells, epi, accept, seed, link_cell, kT_units, storage,
-                               kernel, device, trace_capacity)
+                               kernel, device, trace_capacity, local_quad=local_quad)
         self.device = torch.device("cuda", int(device))
         with torch.cuda.device(self.device):
             self._stream = torch.cuda.current_stream(self.device)

@@ -132,7 +132,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   const bool local = p->model == SMCX_MODEL_LOCAL;
   plan->model = p->model;
   if (local && !p->local_quad) return SMCX_E_NULL_ARG;
-  if (local && (n > kLocalMaxSpecies || p->domain_count >= 2)) return SMCX_E_UNSUPPORTED;
+  if (local && n > kLocalMaxSpecies) return SMCX_E_UNSUPPORTED;
   for (int s = 0; s < p->n_shells && !local; ++s)
     for (int a = 0; a < n; ++a)
       for (int b = 0; b < a; ++b)
@@ -571,10 +571,14 @@ long long energy_from_counts(const smcx* h, const std::vector<unsigned long long
 // SMCX_MODEL_LOCAL: H = sum of the local energies, by local_energy_kernel.
 int run_local_energy(smcx* h, long long* E) {
   const Plan& P = h->plan;
-  const Geom& G = P.G;
+  Geom G = P.G;
+  if (P.window) {   // the local energies of the sites of the layers the slab owns under the current origin
+    G.pc_z0 = G.H + h->win_oz;
+    G.pc_z1 = G.pc_z0 + P.row_count * G.w;
+  }
   zero_u64_kernel<<<1, 32, 0, h->stream>>>(h->d_counts(), 1);
   const size_t sm = ((size_t)G.n_shells * G.n_species * G.n_species * (1 + G.n_species)) * sizeof(int32_t);
-  const int grid = grid_for(h, P.n_sites, 256);
+  const int grid = grid_for(h, P.layer_sites * (G.pc_z1 - G.pc_z0), 256);
   if (G.B == 2) local_energy_kernel<2><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_epi(), h->d_quad(), h->d_counts());
   else local_energy_kernel<4><<<grid, 256, sm, h->stream>>>(G, h->d_species(), h->d_epi(), h->d_quad(), h->d_counts());
   h->launches += 2;

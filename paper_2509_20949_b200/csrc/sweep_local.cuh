@@ -250,10 +250,13 @@ local_energy_kernel(const Geom G, const uint8_t* __restrict__ species, const int
   for (int k = threadIdx.x; k < n_shells * n * n; k += blockDim.x) s_w1[k] = w1[k];
   for (int k = threadIdx.x; k < n_shells * n * n * n; k += blockDim.x) s_w2[k] = w2[k];
   __syncthreads();
-  const long long n_sites = (long long)G.Lx * G.Ly * G.Lz * B;
+  // sites of the layers [pc_z0, pc_z1): the whole lattice, or the layers a slab owns (their neighbours lie inside
+  // its window, so the periodic wrap below never acts along z there)
+  const long long i_first = (long long)G.Lx * G.Ly * G.pc_z0 * B;
+  const long long n_sites = (long long)G.Lx * G.Ly * G.pc_z1 * B;
   const int Px = 2 * G.Lx, Py = 2 * G.Ly, Pz = 2 * G.Lz;
   long long sum = 0;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n_sites; i += (long long)gridDim.x * blockDim.x) {
+  for (long long i = i_first + blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n_sites; i += (long long)gridDim.x * blockDim.x) {
     const int b = (int)(i % B);
     const long long c = i / B;
     const int x = (int)(c % G.Lx);

@@ -151,3 +151,22 @@ def test_config4_shape_slabs_at_a_size_the_oracle_finishes():
     o.sweep(3)
     _assert_same(g, o)
     g.close()
+
+
+@pytest.mark.parametrize("lattice,dims,n_sp,n_sh,n_slabs", [(smcx.BCC, (16, 16, 32), 4, 2, 2), (smcx.FCC, (16, 16, 48), 5, 3, 3)])
+def test_local_energy_model_on_slabs(lattice, dims, n_sp, n_sh, n_slabs):
+    """Reading S12 on slabs: three ghost layers, four-layer pass messages; against the undivided oracle."""
+    from smcx_inputs import make_local_weights
+    w1, w2 = make_local_weights(n_sh, n_sp, 200, 25, 19)
+    table = make_accept_table(1500)
+    o = oracle.Oracle(lattice, dims, n_sp, n_sh, w1, 4, table, 19)
+    o.set_local_model(w2)
+    g = smcx.DomainGroup(n_slabs, lattice, dims, n_sp, n_sh, w1, table, 19, link_cell=4, local_quad=w2)
+    assert all(m.info["ghost"] == 3 for m in g.members)
+    assert g.energy() == o.energy() == g.running_energy()
+    for _ in range(5):
+        g.sweep(1)
+        o.sweep(1)
+        assert (g.species() == o.species()).all()
+    _assert_same(g, o)
+    g.close()

@@ -187,5 +187,5 @@ def test_local_model_parameter_validation():
     assert _code(epi=w1, local_quad=w2 * 100000) == E["EPI_RANGE"]
     assert _code(epi=w1, local_quad=w2, kernel=smcx.KERNEL_GROUP_PER_CELL) == E["UNSUPPORTED"]
     assert _code(kernel=smcx.KERNEL_LOCAL_WARP) == E["UNSUPPORTED"]                     # that kernel serves the local model only
-    with pytest.raises(SmcxError):
-        smcx.domain_partition(2, 0, **_kw(dims=(16, 16, 32), epi=w1, local_quad=w2))
+    info = smcx.domain_partition(2, 0, **_kw(dims=(16, 16, 32), epi=w1, local_quad=w2))
+    assert info["ghost"] == 3 and info["z_layers"] == info["row_count"] * 4 + 3 + 6      # neighbours of neighbours
