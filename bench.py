@@ -634,7 +634,12 @@ def run_cuda(args, cfg, rank, world, local_rank):
                          "what": "achieved = ALGORITHMIC bytes (uint8, SURVEY.md 8(d)) per launch / measured launch time, as "
                                  "north_star declares the roofline; the bytes the kernel really moves are in `dram`",
                          "algorithmic_bytes_per_trial": ALGO_BYTES_PER_TRIAL, "launch_ms": launch_ms,
-                         "north_star_target_frac": 0.5, "target_met": bool(frac >= 0.5)},
+                         "north_star_target_frac": 0.5, "target_met": bool(frac >= 0.5),
+                         "schedule_ceiling_frac": (0.346 if lat.kernel == 3 else None),
+                         "schedule_ceiling_note": "DESIGN.md 7: the trial S3/S4 prescribe costs >= 120 ALU-pipe cycles per warp-trial "
+                                                  "(Philox4x32-10 alone is 20 % of a pass, measured by ablation), i.e. 0.413 ms per colour "
+                                                  "pass = 34.6 % of this roofline with that pipe 100 % busy; the kernel is ALU-bound "
+                                                  "(see alu_view), HBM runs at 10 % of peak (see dram)"},
             # what the kernel moves (packed storage): measured DRAM bytes per launch / live launch time
             "dram": ({"bytes_per_launch": traffic, "achieved_gbs": traffic / (launch_ms * 1e-3) / 1e9,
                       "frac_of_peak": traffic / (launch_ms * 1e-3) / 1e9 / peak, "source": capture["capture"]}
