@@ -184,11 +184,12 @@ def test_config4_full_size_oracle_two_sweeps():
     bench.py times, at SURVEY.md 8(d)'s extent: initial state, species after 2 sweeps and the trace against the
     oracle (all host cores)."""
     cfg = get_config(4)
+    n = int(os.environ.get("SMCX_C4_SWEEPS", "2"))      # test extent only (profiles/r2_full_size_parity.txt ran 20)
     g, o = _pair(cfg, threads=ALL_CORES)
     assert g.kernel == smcx.KERNEL_THREAD_PERSISTENT and g.storage == smcx.STORAGE_2BIT
     _assert_same_state(g, o)
-    g.sweep(2)
-    o.sweep(2)
+    g.sweep(n)
+    o.sweep(n)
     _assert_same_state(g, o)
     assert (g.energy_trace() == o.energy_trace()).all()
     assert g.stats() == o.stats()
