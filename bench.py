@@ -392,7 +392,7 @@ def run_lattice_parallel_one_gpu(cfg, sweeps: int = 10, whole_sweep_ms=None):
         b0 = g.message_bytes
         g.sweep(1)
         g.synchronize()
-        out["runs"].append({"slabs": n_slabs, "mode": {0: "pass, then copy", 1: "boundary row first, message fused into its kernel",
+        out["runs"].append({"slabs": n_slabs, "mode": {0: "pass, then copy", 1: "boundary row (side stream, message fused into its kernel) and the other rows concurrently on disjoint SMs",
                                                         2: "boundary row first, message copied on a second stream"}[overlap],
                             "fused_messages_per_sweep": int(g.fused_messages // max(1, g.stats()[0])), "sweep_ms": ms, "value": cfg.n_sites / (ms * 1e-3),
                             "unit": "trial swaps/s", "message_bytes_per_sweep": int(g.message_bytes - b0),
