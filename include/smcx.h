@@ -348,6 +348,12 @@ int smcx_domain_set_sweep_counter(smcx_domain_t *d, int64_t t);
 int smcx_domain_begin_sweep(smcx_domain_t *d, smcx_domain_msg_t *send, smcx_domain_msg_t *recv);
 int smcx_domain_pass(smcx_domain_t *d, int32_t colour, int32_t part);
 int smcx_domain_pass_messages(smcx_domain_t *d, int32_t colour, smcx_domain_msg_t *send, smcx_domain_msg_t *recv);
+/* Parts 1 and 2 of a pass at the same time (computation-communication overlap): the boundary row on
+ * `side_stream` (a cudaStream_t of the slab's device; it is made to wait for the slab's stream first), the other rows on
+ * the slab's own stream, on disjoint sets of SMs where the kernel takes one block per SM.  The caller sends the pass
+ * message from side_stream (its layers are complete when the work enqueued there so far is) and lets the slab's stream
+ * wait for side_stream before the next pass. */
+int smcx_domain_pass_split(smcx_domain_t *d, int32_t colour, void *side_stream);
 /* The boundary row of a pass (part 1) with its message FUSED into the kernel: while a cell writes its tile back it also
  * stores the layers of the outgoing message straight into the neighbour's species storage -- only the bytes it modified,
  * no copy kernel, no copy engine (peer stores over NVLink when the neighbour is on another GPU of this process).

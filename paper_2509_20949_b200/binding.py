@@ -164,6 +164,7 @@ def load_library(build_if_missing: bool = True):
         "smcx_domain_group_message_bytes": (C.c_int64, [vp]),
         "smcx_domain_group_fused_messages": (C.c_int64, [vp]),
         "smcx_domain_pass_fused": (C.c_int, [vp, C.c_int32, vp, C.c_int64]),
+        "smcx_domain_pass_split": (C.c_int, [vp, C.c_int32, vp]),
         "smcx_last_error": (C.c_char_p, [vp]),
         "smcx_strerror": (C.c_char_p, [C.c_int]),
         "smcx_version": (C.c_char_p, []),
@@ -666,6 +667,10 @@ class Domain:
 
     def run_pass(self, colour, part=0):
         self._check(self._lib.smcx_domain_pass(self._d, int(colour), int(part)), "smcx_domain_pass")
+
+    def run_pass_split(self, colour, side_stream):
+        """smcx_domain_pass_split: boundary row on `side_stream` (a torch.cuda.Stream), the other rows on the slab's stream."""
+        self._check(self._lib.smcx_domain_pass_split(self._d, int(colour), C.c_void_p(side_stream.cuda_stream)), "smcx_domain_pass_split")
 
     def run_pass_fused(self, colour, peer_storage_ptr, peer_offset):
         """smcx_domain_pass_fused: the boundary row of the pass, storing its message into the neighbour's storage."""

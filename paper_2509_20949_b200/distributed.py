@@ -94,6 +94,9 @@ class SlabRank:
             return
         for work in pending:
             work.wait()            # NCCL: orders the current (compute) stream after the transfer
+        if getattr(self, "_side_busy", False):
+            self.compute.wait_stream(self.side)      # ... and after the boundary row itself
+            self._side_busy = False
 
     # -- one sweep, in the three steps a LocalWorld needs (post everything, then deliver) --------------------
     def sweep_begin(self):
@@ -101,7 +104,15 @@ class SlabRank:
 
     def pass_begin(self, colour):
         send, recv = self.domain.pass_messages(colour)
-        if self.overlap:
+        if self.overlap and self.side is not None and self.dist is not None:
+            # boundary row on the side stream, the other rows on the compute stream, at the same time; the message
+            # leaves from the side stream as soon as the boundary row is done
+            self.domain.run_pass_split(colour, self.side)
+            self.message_bytes += send[3]
+            with self.torch.cuda.stream(self.side):
+                pending = exchange(self.dist, self.rank, self.domain._storage_view, send, recv)
+            self._side_busy = True
+        elif self.overlap:
             self.domain.run_pass(colour, 1)          # the boundary row, whose layers the message carries
             pending = self._start(send, recv)
             self.domain.run_pass(colour, 2)          # the other rows run while the message is in flight

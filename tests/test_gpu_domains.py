@@ -170,3 +170,42 @@ def test_local_energy_model_on_slabs(lattice, dims, n_sp, n_sh, n_slabs):
         assert (g.species() == o.species()).all()
     _assert_same(g, o)
     g.close()
+
+
+@pytest.mark.parametrize("kernel", [smcx.KERNEL_THREAD_PERSISTENT, smcx.KERNEL_GROUP_PER_CELL], ids=["persistent", "group"])
+def test_pass_split_boundary_row_and_the_rest_at_the_same_time(kernel):
+    """smcx_domain_pass_split (what the per-rank NCCL driver calls): the boundary row on a side stream, the other rows on
+    the slab's stream, concurrently; messages moved by hand between three slabs."""
+    import torch
+    kw = _kw(smcx.BCC, (16, 16, 48), 4, 2, seed=33)
+    o = _oracle(kw)
+    slabs = [smcx.Domain(3, r, kernel=kernel, **kw) for r in range(3)]
+    side = [torch.cuda.Stream() for _ in slabs]
+
+    def move(plans):
+        torch.cuda.synchronize()
+        for r, (send, _) in enumerate(plans):
+            if send[3]:
+                dst = slabs[send[0]]
+                recv = plans[send[0]][1]
+                assert recv[0] == r and recv[3] == send[3]
+                dst.storage_view(recv).copy_(slabs[r].storage_view(send))
+        torch.cuda.synchronize()
+
+    for _ in range(5):
+        move([s.begin_sweep() for s in slabs])
+        for colour in range(8):
+            plans = [s.pass_messages(colour) for s in slabs]
+            for s, st in zip(slabs, side):
+                s.run_pass_split(colour, st)
+            move(plans)
+        for s in slabs:
+            s.end_sweep()
+    o.sweep(5)
+    whole = np.full(o.n_sites, 255, dtype=np.uint8)
+    for s in slabs:
+        s.species_into(whole)
+    assert (whole == o.species()).all()
+    assert sum(s.running_energy() for s in slabs) == o.running_energy()
+    for s in slabs:
+        s.close()
