@@ -30,8 +30,14 @@
 // PAPER.md:114) are spread over n OpenMP threads, each with its own tally of trials / accepted / sum dE
 // added up after the loop.  Same arithmetic, same order inside a cell; pinned bit for bit against the
 // one-thread run (tests/test_oracle_schedule.py).
-// Parity unpinned: the authors' own trajectories and Fig. 6 curves (their EPI values and
-// code are not available).
+// Also pinned: the decomposed sweep (S11, slabs with ghost layers) against the undivided one with poison
+// outside every slab's window and negative controls (tests/test_oracle_domains.py); the nonlinear local-energy model
+// (S12) against a numpy restatement, closed forms, brute-force dE, its linear limit (= twice the EPI
+// trajectory) and the exact Boltzmann histogram (tests/test_oracle_local_model.py); replica exchange (S9) against
+// rational arithmetic and exact histograms (tests/test_oracle_exchange.py).
+// Parity unpinned: the authors' own trajectories and Fig. 6 curves (their EPI values and code are not available,
+// PAPER.md:213-217); the paper's qSRO model itself (its Ref. 22: form and weights not available) -- S12 is a model of
+// the same kind with synthetic weights, pinned as stated, not the authors'.
 #include <algorithm>
 #include <array>
 #include <cmath>
