@@ -189,3 +189,18 @@ def test_local_model_parameter_validation():
     assert _code(kernel=smcx.KERNEL_LOCAL_WARP) == E["UNSUPPORTED"]                     # that kernel serves the local model only
     info = smcx.domain_partition(2, 0, **_kw(dims=(16, 16, 32), epi=w1, local_quad=w2))
     assert info["ghost"] == 3 and info["z_layers"] == info["row_count"] * 4 + 3 + 6      # neighbours of neighbours
+
+
+def test_header_is_c99_and_the_library_serves_a_plain_c_caller(tmp_path):
+    """include/smcx.h compiles as C99 with -pedantic; a C program dlopens libsmcx.so and exercises the host-only calls."""
+    import os
+    import subprocess
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    hdr = os.path.join(root, "include", "smcx.h")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-pedantic", "-Werror", "-fsyntax-only", "-x", "c", hdr])
+    smcx.load_library()
+    exe = str(tmp_path / "abi_from_c")
+    subprocess.check_call(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-o", exe,
+                           os.path.join(root, "tests", "host_checks", "abi_from_c.c"), "-ldl"])
+    out = subprocess.run([exe, smcx.library_path()], capture_output=True, text=True)
+    assert out.returncode == 0 and "abi_from_c ok" in out.stdout, out.stdout + out.stderr
