@@ -363,6 +363,29 @@ int smcx_domain_pass_split(smcx_domain_t *d, int32_t colour, void *side_stream);
  * if the slab's kernel has no fused write-back (the packed kernels THREAD_* and FCC_THREAD have): use part 1 + a copy. */
 int smcx_domain_pass_fused(smcx_domain_t *d, int32_t colour, void *peer_storage, int64_t peer_offset);
 int smcx_domain_end_sweep(smcx_domain_t *d);
+/* Connected slabs: one slab per PROCESS (one process per GPU), no host in the data path.  A slab is connected to the
+ * species storage and the two message flags of its neighbours -- device pointers valid in this process: exported with
+ * smcx_domain_ipc_export and mapped with CUDA IPC by smcx_domain_ipc_connect when the neighbour lives in another process
+ * (same GPU or a peer GPU over NVLink), or given directly to smcx_domain_connect when it lives in this one.  Then
+ * smcx_domain_sweep_connected(n) enqueues n whole sweeps: the window shift is pushed into the neighbour's storage by a
+ * device-to-device copy, the message of a colour pass is written there by the boundary-row kernel itself (as
+ * smcx_domain_pass_fused) while the other rows of the pass run concurrently, and every message is followed by a serial
+ * number stored into the neighbour's flag; the receiver's stream waits for that number (a stream memory operation, no
+ * kernel spins, no host thread is involved).  Slabs are connected once, all of them before any of them sweeps (a
+ * barrier of the caller's), and must be given the same sweep counts.  The slab's workspace must be the library's own
+ * allocation (smcx_params_t::d_workspace NULL) for smcx_domain_ipc_export. */
+typedef struct {
+  unsigned char handle[64];      /* cudaIpcMemHandle_t of the slab's workspace allocation */
+  int64_t storage_offset;        /* of the species storage inside it */
+  int64_t flags_offset;          /* of the two message flags (uint32: from the lower, from the upper neighbour) */
+  int32_t index, device;         /* slab index; CUDA device ordinal in the exporting process */
+} smcx_domain_ipc_t;
+int smcx_domain_ipc_export(smcx_domain_t *d, smcx_domain_ipc_t *out);
+int smcx_domain_ipc_connect(smcx_domain_t *d, const smcx_domain_ipc_t *lower, const smcx_domain_ipc_t *upper);
+void *smcx_domain_flags(smcx_domain_t *d);     /* device pointer of this slab's two message flags */
+int smcx_domain_connect(smcx_domain_t *d, void *lower_storage, void *lower_flags, void *upper_storage, void *upper_flags);
+int smcx_domain_sweep_connected(smcx_domain_t *d, int64_t n);   /* asynchronous */
+
 /* Partial results; their sums over the slabs are those of the whole lattice.  pair_counts: positive-half counts
  * M[s][x][y] of the bonds of the layers the slab owns; running energy / trace: the slab's share of H at the start plus
  * the dE its cells accepted.  Synchronise the slab's stream. */

@@ -51,6 +51,19 @@ class DomainInfo(C.Structure):
         return {k: int(getattr(self, k)) for k, _ in self._fields_}
 
 
+class DomainIpc(C.Structure):
+    """smcx_domain_ipc_t"""
+    _fields_ = [("handle", C.c_ubyte * 64), ("storage_offset", C.c_int64), ("flags_offset", C.c_int64),
+                ("index", C.c_int32), ("device", C.c_int32)]
+
+    def to_bytes(self) -> bytes:
+        return bytes(self)
+
+    @classmethod
+    def from_bytes(cls, b: bytes):
+        return cls.from_buffer_copy(b)
+
+
 class DomainMsg(C.Structure):
     """smcx_domain_msg_t"""
     _fields_ = [("peer", C.c_int32), ("tag", C.c_int32), ("offset", C.c_int64), ("bytes", C.c_int64)]
@@ -165,6 +178,11 @@ def load_library(build_if_missing: bool = True):
         "smcx_domain_group_fused_messages": (C.c_int64, [vp]),
         "smcx_domain_pass_fused": (C.c_int, [vp, C.c_int32, vp, C.c_int64]),
         "smcx_domain_pass_split": (C.c_int, [vp, C.c_int32, vp]),
+        "smcx_domain_ipc_export": (C.c_int, [vp, C.POINTER(DomainIpc)]),
+        "smcx_domain_ipc_connect": (C.c_int, [vp, C.POINTER(DomainIpc), C.POINTER(DomainIpc)]),
+        "smcx_domain_flags": (vp, [vp]),
+        "smcx_domain_connect": (C.c_int, [vp, vp, vp, vp, vp]),
+        "smcx_domain_sweep_connected": (C.c_int, [vp, C.c_int64]),
         "smcx_last_error": (C.c_char_p, [vp]),
         "smcx_strerror": (C.c_char_p, [C.c_int]),
         "smcx_version": (C.c_char_p, []),
@@ -563,7 +581,8 @@ class Domain:
     uint8 tensor, so a caller can hand slices of the species storage (`storage_view`) to torch.distributed."""
 
     def __init__(self, n_domains, index, lattice, dims, n_species, n_shells, epi, accept, seed, link_cell=4, kT_units=0,
-                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0, stream=None, local_quad=None):
+                 storage=STORAGE_AUTO, kernel=KERNEL_AUTO, device=0, trace_capacity=0, stream=None, local_quad=None,
+                 library_workspace=False):
         import torch
 
         if not torch.cuda.is_available():
@@ -578,11 +597,13 @@ class Domain:
             raise SmcxError(rc, "smcx_domain_workspace_bytes")
         self.device = torch.device("cuda", int(device))
         with torch.cuda.device(self.device):
-            self._workspace = torch.empty(int(need.value), dtype=torch.uint8, device=self.device)
+            # library_workspace: the library allocates (cudaMalloc), which smcx_domain_ipc_export needs; else a torch tensor
+            self._workspace = None if library_workspace else torch.empty(int(need.value), dtype=torch.uint8, device=self.device)
             self._stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         p.stream = C.c_void_p(self._stream.cuda_stream)
-        p.d_workspace = C.c_void_p(self._workspace.data_ptr())
-        p.workspace_bytes = int(need.value)
+        if self._workspace is not None:
+            p.d_workspace = C.c_void_p(self._workspace.data_ptr())
+            p.workspace_bytes = int(need.value)
         d = C.c_void_p()
         rc = lib.smcx_domain_create(C.byref(d), C.byref(p), int(n_domains), int(index))
         if rc != 0:
@@ -595,8 +616,10 @@ class Domain:
         self.n_domains, self.index = int(n_domains), int(index)
         self.n_species, self.n_shells = int(n_species), int(n_shells)
         self.n_sites_whole = int(np.prod([int(x) for x in dims])) * (2 if int(lattice) == BCC else 4)
-        off = int(lib.smcx_domain_storage(d)) - self._workspace.data_ptr()
-        self._storage_view = self._workspace[off: off + self.info["z_layers"] * self.info["layer_bytes"]]
+        self._storage_view = None
+        if self._workspace is not None:
+            off = int(lib.smcx_domain_storage(d)) - self._workspace.data_ptr()
+            self._storage_view = self._workspace[off: off + self.info["z_layers"] * self.info["layer_bytes"]]
 
     @classmethod
     def _borrowed(cls, handle, owner, n_species, n_shells, n_sites_whole):
@@ -667,6 +690,29 @@ class Domain:
 
     def run_pass(self, colour, part=0):
         self._check(self._lib.smcx_domain_pass(self._d, int(colour), int(part)), "smcx_domain_pass")
+
+    # -- connected slabs: one slab per process, no host in the data path ---------------------------------------------
+    def ipc_export(self) -> bytes:
+        """smcx_domain_ipc_export as bytes (to hand to the neighbours' processes)."""
+        out = DomainIpc()
+        self._check(self._lib.smcx_domain_ipc_export(self._d, C.byref(out)), "smcx_domain_ipc_export")
+        return out.to_bytes()
+
+    def ipc_connect(self, lower: bytes, upper: bytes):
+        lo, up = DomainIpc.from_bytes(lower), DomainIpc.from_bytes(upper)
+        self._check(self._lib.smcx_domain_ipc_connect(self._d, C.byref(lo), C.byref(up)), "smcx_domain_ipc_connect")
+
+    @property
+    def flags_ptr(self) -> int:
+        return int(self._lib.smcx_domain_flags(self._d))
+
+    def connect(self, lower, upper):
+        """smcx_domain_connect with neighbours that live in this process (Domain objects)."""
+        self._check(self._lib.smcx_domain_connect(self._d, C.c_void_p(lower.storage_ptr), C.c_void_p(lower.flags_ptr),
+                                                  C.c_void_p(upper.storage_ptr), C.c_void_p(upper.flags_ptr)), "smcx_domain_connect")
+
+    def sweep_connected(self, n=1):
+        self._check(self._lib.smcx_domain_sweep_connected(self._d, int(n)), "smcx_domain_sweep_connected")
 
     def run_pass_split(self, colour, side_stream):
         """smcx_domain_pass_split: boundary row on `side_stream` (a torch.cuda.Stream), the other rows on the slab's stream."""

@@ -61,6 +61,7 @@ struct DevState {
   long long e_run;               // running energy E_0 + sum of accepted dE
   unsigned long long accepted;   // accepted swaps
   unsigned long long bad_state;  // set by validation kernels
+  unsigned flag[2];              // connected slabs (domain_api.inc): serial of the last message that arrived from the lower [0] / upper [1] neighbour, written by that neighbour
   unsigned work[16];             // per colour (+ 8 for the second launch of a split pass, Geom::work_base): batches of cells handed out so far in this sweep (sweep_fcc_thread); zeroed by sweep_epilogue
 };
 

@@ -209,3 +209,30 @@ def test_pass_split_boundary_row_and_the_rest_at_the_same_time(kernel):
     assert sum(s.running_energy() for s in slabs) == o.running_energy()
     for s in slabs:
         s.close()
+
+
+@pytest.mark.parametrize("kernel,n_slabs", [(smcx.KERNEL_THREAD_PERSISTENT, 3), (smcx.KERNEL_GROUP_PER_CELL, 2)], ids=["persistent3", "group2"])
+def test_connected_slabs_in_one_process(kernel, n_slabs):
+    """smcx_domain_connect + smcx_domain_sweep_connected: every slab pushes its messages into its neighbours' storage and
+    signals them through a flag the neighbour's stream waits for; no host code between the passes.  The slabs live in
+    this process here (each on its own stream); tests/test_gpu_ipc_slabs.py runs them in separate processes."""
+    import torch
+    kw = _kw(smcx.BCC, (16, 16, 16 * n_slabs), 4, 2, seed=61)
+    o = _oracle(kw)
+    streams = [torch.cuda.Stream() for _ in range(n_slabs)]
+    slabs = [smcx.Domain(n_slabs, r, kernel=kernel, stream=streams[r], **kw) for r in range(n_slabs)]
+    for r, s in enumerate(slabs):
+        s.connect(slabs[(r - 1) % n_slabs], slabs[(r + 1) % n_slabs])
+    for n in (1, 4, 2):
+        for s in slabs:
+            s.sweep_connected(n)          # every call only enqueues: the slabs' streams sort the order out
+    torch.cuda.synchronize()
+    o.sweep(7)
+    whole = np.full(o.n_sites, 255, dtype=np.uint8)
+    for s in slabs:
+        s.species_into(whole)
+    assert (whole == o.species()).all()
+    assert sum(s.running_energy() for s in slabs) == o.running_energy()
+    assert (sum(s.energy_trace() for s in slabs) == o.energy_trace()).all()
+    for s in slabs:
+        s.close()
