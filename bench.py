@@ -410,10 +410,14 @@ def run_slabs(args, cfg, rank, world, local_rank):
     import torch.distributed as dist
     from paper_2509_20949_b200 import distributed
 
+    local_rank = local_rank % torch.cuda.device_count()      # several ranks may share a GPU (one-GPU test runs of this path)
     torch.cuda.set_device(local_rank)
     dev = torch.device("cuda", local_rank)
     if not dist.is_initialized():
-        dist.init_process_group("nccl", device_id=dev)
+        if args.dist_backend == "nccl":
+            dist.init_process_group("nccl", device_id=dev)
+        else:
+            dist.init_process_group(args.dist_backend)
 
     def barrier():
         dist.barrier()
@@ -422,7 +426,18 @@ def run_slabs(args, cfg, rank, world, local_rank):
     kw = dict(lattice=cfg.lattice, dims=cfg.dims, n_species=cfg.n_species, n_shells=cfg.n_shells, epi=cfg.epi(),
               accept=cfg.accept_table(0), seed=cfg.seed, link_cell=cfg.link_cell, kT_units=cfg.kT_at(0),
               kernel=args.kernel, storage=args.storage, device=local_rank)
-    slab = distributed.SlabRank(rank, world, dist=dist, overlap=not args.no_overlap, **kw)
+    transport = args.transport
+    slab = None
+    if transport == "ipc":
+        # ghost layers by peer stores from inside the sweep kernels, signalled through device flags (one node)
+        try:
+            slab = distributed.ConnectedSlabRank(rank, world, dist=dist, **kw)
+        except Exception as exc:                     # e.g. no peer access between two GPUs: every rank fails alike at connect
+            if rank == 0:
+                print(f"bench.py: connected slabs unavailable ({exc}); using NCCL messages", file=sys.stderr)
+            transport = "nccl"
+    if slab is None:
+        slab = distributed.SlabRank(rank, world, dist=dist, overlap=not args.no_overlap, **kw)
     slab.sweep(args.warmup)
     barrier()
     sampler = ClockSampler(local_rank)
@@ -474,8 +489,11 @@ def run_slabs(args, cfg, rank, world, local_rank):
             "vs_baseline": None, "dtype": "int32", "data": "synthetic",
             "config": {"workload": workload_string(cfg), "config_id": args.config,
                        "step": "1 sweep of the one lattice = per GPU a window shift + 8 x (colour pass of its slab, ghost-layer message)",
-                       "parallelism": f"lattice parallelism: {world} slabs along z, one per GPU, ghost layers over NCCL send/recv, "
-                                      f"overlap {'on' if not args.no_overlap else 'off'}",
+                       "parallelism": (f"lattice parallelism: {world} slabs along z, one per GPU, ghost layers written by the sweep "
+                                       "kernels into the neighbour GPU's memory (CUDA IPC peer stores), signalled by device flags"
+                                       if transport == "ipc" else
+                                       f"lattice parallelism: {world} slabs along z, one per GPU, ghost layers over NCCL send/recv, "
+                                       f"overlap {'on' if not args.no_overlap else 'off'}"),
                        "l2": "slab windows larger than the 126 MB L2 at the graded size; no flush"},
             "pct_of_hbm_roofline": 100.0 * (value / world) * ALGO_BYTES_PER_TRIAL / (peak * 1e9),
             "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
@@ -698,6 +716,11 @@ def main():
     ap.add_argument("--multi", default="slabs", choices=["slabs", "replicas"],
                     help="N > 1: `slabs` = the one lattice cut into N slabs, one per GPU (lattice parallelism, strong scaling); "
                          "`replicas` = N independent lattices (weak scaling)")
+    ap.add_argument("--dist-backend", default="nccl", choices=["nccl", "gloo"],
+                    help="--multi slabs: torch.distributed backend for handles, barriers and reductions (gloo: ranks that share a GPU)")
+    ap.add_argument("--transport", default="ipc", choices=["ipc", "nccl"],
+                    help="--multi slabs: how ghost layers travel: `ipc` = peer stores from the sweep kernels + device flags "
+                         "(connected slabs, one node), `nccl` = torch.distributed send/recv")
     ap.add_argument("--no-overlap", action="store_true", help="--multi slabs: send the ghost layers after the whole pass")
     ap.add_argument("--source-hash", action="store_true", help="print the source hash of every kernel (for profiles/dram_traffic.csv) and exit")
     ap.add_argument("--ensemble", type=int, default=128,

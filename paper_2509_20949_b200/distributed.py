@@ -165,6 +165,38 @@ class SlabRank:
         self.domain.close()
 
 
+class ConnectedSlabRank(SlabRank):
+    """One slab per process with NO host code in the data path (include/smcx.h, "Connected slabs"): the ranks exchange
+    CUDA IPC handles of their slabs once (`dist.all_gather_object`), map their neighbours' storage, and from then on
+    `sweep(n)` is one C call that enqueues n whole sweeps -- ghost layers are written by the sweep kernels straight into
+    the neighbour's memory (peer stores over NVLink between GPUs of a node) and signalled through device flags.
+    torch.distributed carries the handles and the partial reductions only.  All ranks must share a node."""
+
+    def __init__(self, rank, world_size, dist, **lattice_kw):
+        import torch
+
+        self.torch = torch
+        self.rank, self.world_size = int(rank), int(world_size)
+        self.dist, self.world, self.overlap = dist, None, True
+        self.domain = _b.Domain(self.world_size, self.rank, library_workspace=True, **lattice_kw)
+        self.compute, self.side = self.domain._stream, None
+        self._kw = {k: lattice_kw[k] for k in ("lattice", "dims", "n_species", "n_shells", "epi", "accept", "seed") if k in lattice_kw}
+        self._kw["link_cell"] = lattice_kw.get("link_cell", 4)
+        self.message_bytes = 0
+        handles = [None] * self.world_size
+        dist.all_gather_object(handles, self.domain.ipc_export())
+        self.domain.ipc_connect(handles[(self.rank - 1) % self.world_size], handles[(self.rank + 1) % self.world_size])
+        dist.barrier()                               # every slab connected (flags zeroed) before any slab sweeps
+
+    def sweep(self, n=1):
+        self.domain.sweep_connected(int(n))
+
+    def close(self):
+        self.domain.synchronize()
+        self.dist.barrier()                          # nobody unmaps a neighbour that is still being written to
+        self.domain.close()
+
+
 def run_local(slabs, n=1):
     """n sweeps of slabs that share a process and a LocalWorld: every phase is posted by all slabs, then delivered."""
     torch = slabs[0].torch

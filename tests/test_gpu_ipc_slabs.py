@@ -68,3 +68,21 @@ def test_slabs_in_separate_processes_over_cuda_ipc(world, kernel):
     o.sweep(6)
     assert (whole == o.species()).all()
     assert e_run == o.running_energy() and (trace == o.energy_trace()).all()
+
+
+def test_bench_slab_mode_under_torchrun_with_two_ranks_on_the_one_gpu():
+    """`bench.py --gpus 2` as the driver launches it (torchrun, one rank per slab), both ranks on this box's one GPU and
+    gloo instead of NCCL for the handles / reductions: the whole N > 1 path -- connected slabs over CUDA IPC, device-timed
+    sweeps, end-to-end leg, the JSON line -- runs and reports the one lattice's throughput (strong scaling)."""
+    import json
+    import subprocess
+    port = 36500 + os.getpid() % 2000
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", str(port), os.path.join(ROOT, "bench.py"), "--gpus", "2", "--config", "2", "--steps", "4",
+           "--warmup", "3", "--dist-backend", "gloo"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stdout[-2000:] + out.stderr[-2000:]
+    line = [l for l in out.stdout.splitlines() if l.startswith("{")][-1]
+    d = json.loads(line)
+    assert d["n_gpus"] == 2 and d["scaling"] == "strong" and d["value"] > 0 and d["e2e"]["value"] > 0
+    assert "CUDA IPC" in d["config"]["parallelism"] and d["gpu_launches"] > 0
