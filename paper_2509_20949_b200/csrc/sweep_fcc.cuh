@@ -235,7 +235,9 @@ __host__ __device__ __forceinline__ FccLut fcc_load_lut(smem_ptr_t p) {
 
 // One trial (a4-a6).  p_own: row r of sublattice b in this lane's tile; X4 = 4 X, X the nibble of site i; E = the
 // direction-table entry of (b, drawn direction); u = acceptance draw.
-template <int b, int NT, bool kFilter, int ROWS = kFccRows>
+// MODE (acceptance): 0 = T[dE] from global memory, 1 = two-level filter in shared memory (exact look-up in global memory
+// when u falls within E of the bound), 2 = the whole table T, followed by one zero entry, in shared memory at env.filt.
+template <int b, int NT, int MODE, int ROWS = kFccRows>
 __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4, const FccDirEntry& E, uint32_t u,
                                                    const FccEnv& env, int& esum, unsigned& nacc) {
   using T = FccTile<NT, ROWS>;
@@ -264,7 +266,11 @@ __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4,
   const int dE = (int)(lo_i - lo_j) + 256 * (int)(hi_i - hi_j) + corr;
   // Eq. 3 in integer form
   bool ok;
-  if (kFilter) {
+  if (MODE == 2) {
+    // dE <= 0 (huge as unsigned) and dE >= len clamp to the zero entry behind the table: decided by the sign test alone
+    const uint32_t i4 = 4u * min((uint32_t)dE, (uint32_t)env.accept_len);
+    ok = dE <= 0 || u < lds_u32(env.filt, i4);
+  } else if (MODE == 1) {
     const uint32_t dc = (uint32_t)min(max(dE, 0), kFilterDmax);
     const uint32_t ta = mulhi_u32(lds_u32(env.filt, 4u * (kFilterTr + (dc >> 6))), lds_u32(env.filt, 4u * (dc & 63u)));
     ok = u < ta;
@@ -286,39 +292,52 @@ __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4,
 }
 
 #ifdef __CUDACC__
-inline size_t fcc_smem_bytes(int rep) {
-  return (size_t)kFccWarps * FccTile<32, kFccWinRows>::kSub * 4 + (size_t)64 * 3 * rep * 16 + 64 * 4 + kFilterWords * 4 + sizeof(FccTables);
+constexpr int kFccMinWarps = 6;
+constexpr int kFccSmemMax = 232448 - 1536;                     // 227 KB less the static part / reserve
+// dynamic shared memory: tile windows of `warps` warps, look-up rows, corr, direction table, then the filter tables
+// (accept_words = kFilterWords) or the whole threshold table plus its zero entry (accept_words = len + 1)
+inline size_t fcc_smem_bytes(int rep, int warps = kFccWarps, size_t accept_words = kFilterWords) {
+  return (size_t)warps * FccTile<32, kFccWinRows>::kSub * 4 + (size_t)64 * 3 * rep * 16 + 64 * 4 + sizeof(FccTables) + accept_words * 4;
 }
 // replicas of the look-up rows: as many (8, 4, 2, 1) as fit next to the tiles
 inline int fcc_lut_rep(int n_species) {
   (void)n_species;
   for (int rep = 8; rep >= 1; rep >>= 1)
-    if (fcc_smem_bytes(rep) + 2048 <= 227 * 1024) return rep;
+    if (fcc_smem_bytes(rep) <= (size_t)kFccSmemMax) return rep;
   return 1;
 }
+// Warps per block with which the whole threshold table fits shared memory (8 .. 5; the kernel runs as fast with six
+// warps as with eight), or 0: then the two-level filter serves.
+inline int fcc_direct_warps(int rep, int accept_len) {
+  for (int w = kFccWarps; w >= kFccMinWarps; --w)
+    if (fcc_smem_bytes(rep, w, (size_t)accept_len + 1) <= (size_t)kFccSmemMax) return w;
+  return 0;
+}
 
-template <bool kFilter>
+template <int MODE>
 __global__ void __launch_bounds__(kFccWarps * 32, 1)
 sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattice, const uint4* __restrict__ lut,
                  const int32_t* __restrict__ corr, int rep, const uint32_t* __restrict__ accept,
                  const uint32_t* __restrict__ filt, DevState* __restrict__ st, int colour) {
   constexpr int NT = 32;
   extern __shared__ __align__(16) uint32_t smem_w[];
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
   constexpr int WR = kFccWinRows;                                              // rows per sublattice of the resident window
   uint32_t* tile = smem_w + warp * (4 * WR * NT) + lane;                       // word (s * WR + row) at tile[(s * WR + row) * NT]
-  uint4* s_lut = reinterpret_cast<uint4*>(smem_w + kFccWarps * (4 * WR * NT));
+  uint4* s_lut = reinterpret_cast<uint4*>(smem_w + n_warps * (4 * WR * NT));
   int32_t* s_corr = reinterpret_cast<int32_t*>(s_lut + 64 * 3 * rep);
-  uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_corr + 64);
-  FccDirEntry* s_dir = reinterpret_cast<FccDirEntry*>(s_filt + kFilterWords);
+  FccDirEntry* s_dir = reinterpret_cast<FccDirEntry*>(s_corr + 64);
+  uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_dir + 48);                  // filter tables, or the whole table T + a zero entry
   __shared__ uint2 s_slot[128];                                                // Philox products that depend on the slot pair only
   __shared__ long long s_e64[kFccWarps];
   __shared__ unsigned s_acc[kFccWarps];
 
   for (int k = threadIdx.x; k < 64 * 3 * rep; k += blockDim.x) s_lut[k] = lut[k];
   for (int k = threadIdx.x; k < 64; k += blockDim.x) s_corr[k] = corr[k];
-  if (kFilter)
+  if (MODE == 1)
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
+  if (MODE == 2)
+    for (int k = threadIdx.x; k <= G.accept_len; k += blockDim.x) s_filt[k] = k < G.accept_len ? accept[k] : 0u;
   for (int k = threadIdx.x; k < 48; k += blockDim.x) s_dir[k] = FT.dir[k / 12][k % 12];   // 32 bytes each
   const uint32_t t = (uint32_t)st->sweep;
   if (threadIdx.x < 128) s_slot[threadIdx.x] = philox_slot_entry(threadIdx.x, t, G.rk0, G.rk1);
@@ -418,7 +437,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
             const smem_ptr_t ep = dir_p + (B * 12u + mulhi_u32(WDIR, 12u)) * 32u;                            \
             const int4 e = lds_int4(ep, 0), f = lds_int4(ep, 16);                                             \
             const FccDirEntry E{{e.x, e.y, e.z, e.w}, f.x, f.y, 0, 0};                                        \
-            fcc_trial<B, NT, kFilter, WR>(p_row + B * (WR * NT), X4, E, U, env, esum, nacc);                  \
+            fcc_trial<B, NT, MODE, WR>(p_row + B * (WR * NT), X4, E, U, env, esum, nacc);                      \
           }
           SMCX_FCC_TRIAL(0, r0.x, r0.y) SMCX_FCC_TRIAL(1, r0.z, r0.w) SMCX_FCC_TRIAL(2, r1.x, r1.y) SMCX_FCC_TRIAL(3, r1.z, r1.w)
 #undef SMCX_FCC_TRIAL
@@ -470,7 +489,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
   __syncthreads();
   if (threadIdx.x == 0) {
     long long e = 0; unsigned a = 0;
-    for (int i = 0; i < kFccWarps; ++i) { e += s_e64[i]; a += s_acc[i]; }
+    for (int i = 0; i < n_warps; ++i) { e += s_e64[i]; a += s_acc[i]; }
     if (a) {
       atomicAdd(reinterpret_cast<unsigned long long*>(&st->e_run), (unsigned long long)e);
       atomicAdd(&st->accepted, (unsigned long long)a);
@@ -479,11 +498,13 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
 }
 
 inline int configure_fcc_thread(int rep) {
-  const int sm = (int)fcc_smem_bytes(rep);
-  if (cudaFuncSetAttribute(sweep_fcc_thread<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
-  if (cudaFuncSetAttribute(sweep_fcc_thread<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
-  cudaFuncSetAttribute(sweep_fcc_thread<true>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
-  cudaFuncSetAttribute(sweep_fcc_thread<false>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  (void)rep;
+  if (cudaFuncSetAttribute(sweep_fcc_thread<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kFccSmemMax) != cudaSuccess) return -1;
+  if (cudaFuncSetAttribute(sweep_fcc_thread<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kFccSmemMax) != cudaSuccess) return -1;
+  if (cudaFuncSetAttribute(sweep_fcc_thread<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kFccSmemMax) != cudaSuccess) return -1;
+  cudaFuncSetAttribute(sweep_fcc_thread<0>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(sweep_fcc_thread<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(sweep_fcc_thread<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   return 0;
 }
 
@@ -491,15 +512,19 @@ inline int launch_fcc_thread(const Geom& G, const FccTables& FT, uint32_t* latti
                              int rep, const uint32_t* accept, const uint32_t* d_filter, DevState* st, int colour, int sm_count,
                              cudaStream_t stream) {
   const unsigned n_batches = (G.cells_per_colour + 31u) / 32u;
-  const unsigned want = (n_batches + kFccWarps - 1) / kFccWarps;
+  // the whole threshold table in shared memory when it fits next to at least five warps of tiles, else the filter
+  const int direct = fcc_direct_warps(rep, G.accept_len);
+  const int warps = direct > 0 ? direct : kFccWarps;
+  const unsigned want = (n_batches + warps - 1) / warps;
   const unsigned grid = want < (unsigned)sm_count ? want : (unsigned)sm_count;
-  const size_t sm = fcc_smem_bytes(rep);
-  if (G.filter_E >= 0)
-    sweep_fcc_thread<true><<<grid, kFccWarps * 32, sm, stream>>>(G, FT, lattice, reinterpret_cast<const uint4*>(d_lut), d_corr, rep,
-                                                                 accept, d_filter, st, colour);
+  const uint4* lut4 = reinterpret_cast<const uint4*>(d_lut);
+  if (direct > 0)
+    sweep_fcc_thread<2><<<grid, warps * 32, fcc_smem_bytes(rep, warps, (size_t)G.accept_len + 1), stream>>>(
+        G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour);
+  else if (G.filter_E >= 0)
+    sweep_fcc_thread<1><<<grid, warps * 32, fcc_smem_bytes(rep), stream>>>(G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour);
   else
-    sweep_fcc_thread<false><<<grid, kFccWarps * 32, sm, stream>>>(G, FT, lattice, reinterpret_cast<const uint4*>(d_lut), d_corr, rep,
-                                                                  accept, d_filter, st, colour);
+    sweep_fcc_thread<0><<<grid, warps * 32, fcc_smem_bytes(rep), stream>>>(G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 #endif  // __CUDACC__
