@@ -236,3 +236,36 @@ def test_connected_slabs_in_one_process(kernel, n_slabs):
     assert (sum(s.energy_trace() for s in slabs) == o.energy_trace()).all()
     for s in slabs:
         s.close()
+
+
+def test_connected_slabs_fcc_packed_and_local_model():
+    """Connected slabs with the packed FCC kernel (messages fused into its write-back) and with the local-energy model
+    (three ghost layers, messages copied), three slabs each, stepped in turns."""
+    import torch
+    from smcx_inputs import make_local_weights
+    cases = []
+    kw = _kw(smcx.FCC, (16, 16, 48), 5, 3, seed=83, kT=690, amp=400)
+    cases.append((kw, dict(kernel=smcx.KERNEL_FCC_THREAD, storage=smcx.STORAGE_4BIT), None))
+    w1, w2 = make_local_weights(2, 4, 200, 25, 29)
+    kwl = dict(lattice=smcx.BCC, dims=(16, 16, 48), n_species=4, n_shells=2, epi=w1, accept=make_accept_table(1200), seed=29, link_cell=4)
+    cases.append((kwl, dict(local_quad=w2), w2))
+    for kw, extra, quad in cases:
+        o = _oracle(kw)
+        if quad is not None:
+            o.set_local_model(quad)
+        streams = [torch.cuda.Stream() for _ in range(3)]
+        slabs = [smcx.Domain(3, r, stream=streams[r], **extra, **kw) for r in range(3)]
+        for r, s in enumerate(slabs):
+            s.connect(slabs[(r - 1) % 3], slabs[(r + 1) % 3])
+        for _ in range(5):
+            for s in slabs:
+                s.sweep_connected(1)
+        torch.cuda.synchronize()
+        o.sweep(5)
+        whole = np.full(o.n_sites, 255, dtype=np.uint8)
+        for s in slabs:
+            s.species_into(whole)
+        assert (whole == o.species()).all()
+        assert sum(s.running_energy() for s in slabs) == o.running_energy()
+        for s in slabs:
+            s.close()
