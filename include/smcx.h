@@ -372,9 +372,10 @@ int smcx_domain_end_sweep(smcx_domain_t *d);
  * smcx_domain_pass_fused) while the other rows of the pass run concurrently, and every message is followed by a serial
  * number stored into the neighbour's flag; the receiver's stream waits for that number (a stream memory operation, no
  * kernel spins, no host thread is involved).  Slabs are connected once, all of them before any of them sweeps (a
- * barrier of the caller's), and must be given the same sweep counts.  Slabs that share a process must be stepped in
- * turns with small n (one thread enqueueing thousands of sweeps of one slab would fill the launch queue while its
- * neighbours, which it waits for, have not been enqueued yet).  The slab's workspace must be the library's own
+ * barrier of the caller's), and must be given the same sweep counts.  Slabs that share a process (tests) must be stepped
+ * in turns with small n, and there may be at most three of them: the device has 8 hardware work queues by default, and a
+ * stream that waits for a flag must not share a hardware work queue with the stream whose work sets it
+ * (smcx_domain_connect returns SMCX_E_UNSUPPORTED beyond that; one slab per process, the intended use, needs two queues).  The slab's workspace must be the library's own
  * allocation (smcx_params_t::d_workspace NULL) for smcx_domain_ipc_export. */
 typedef struct {
   unsigned char handle[64];      /* cudaIpcMemHandle_t of the slab's workspace allocation */

@@ -269,3 +269,22 @@ def test_connected_slabs_fcc_packed_and_local_model():
         assert sum(s.running_energy() for s in slabs) == o.running_energy()
         for s in slabs:
             s.close()
+
+
+def test_a_fourth_connected_slab_in_one_process_is_refused():
+    """Streams that wait for a flag must not share a hardware work queue with the stream that sets it; with the default
+    8 queues that allows three connected slabs (two streams each) per process -- the fourth is refused, not deadlocked."""
+    kw = _kw(smcx.BCC, (16, 16, 64), 4, 2, seed=3)
+    slabs = [smcx.Domain(4, r, **kw) for r in range(4)]
+    for r in range(3):
+        slabs[r].connect(slabs[(r - 1) % 4], slabs[(r + 1) % 4])
+    with pytest.raises(smcx.SmcxError) as ei:
+        slabs[3].connect(slabs[2], slabs[0])
+    assert ei.value.code == -12
+    for s in slabs:
+        s.close()
+    again = [smcx.Domain(2, r, **kw) for r in range(2)]          # closing gave the places back
+    for r in range(2):
+        again[r].connect(again[1 - r], again[1 - r])
+    for s in again:
+        s.close()
