@@ -99,7 +99,7 @@ struct Plan {
   FccTables fcc_tables;
   Layout lay;
   int model = SMCX_MODEL_EPI;
-  int local_umax = 0;   // SMCX_MODEL_LOCAL: affected sites per (basis, direction), at most
+  int local_umax = 0;   // SMCX_MODEL_LOCAL: affected sites per (basis, direction, shell), at most
   // Slab window (params domain_count >= 2): this handle holds slab domain_index of the lattice cut along z
   // (domain_api.inc).  n_sites then counts the sites of the window's storage, n_global those of the whole lattice.
   bool window = false;
@@ -352,10 +352,14 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   L.gtable = off;  off += align_up((size_t)group_smem_layout(G, plan->group_lanes).d_bytes, 256);   // sub-warp kernel's difference table
   L.fcc_lut = off; off += align_up((size_t)64 * 3 * 8 * 16, 256);                                   // packed FCC kernel's look-up rows
   L.fcc_corr = off; off += align_up((size_t)64 * sizeof(int32_t), 256);
-  plan->local_umax = local ? 2 + 2 * G.ZT : 0;
+  {   // SMCX_MODEL_LOCAL: affected (site, shell) pairs per (basis, direction, shell), at most: i, j and 2 Z_s neighbours
+    int zmax = 0;
+    for (int s2 = 0; s2 < p->n_shells; ++s2) zmax = std::max(zmax, (int)shells[s2].size());
+    plan->local_umax = local ? 2 + 2 * zmax : 0;
+  }
   L.quad = off;    off += align_up(local ? (size_t)p->n_shells * n * n * n * sizeof(int32_t) : 0, 256);
-  L.utab = off;    off += align_up((size_t)G.B * G.Z0 * plan->local_umax * sizeof(LocalUEntry), 256);
-  L.ucount = off;  off += align_up(local ? (size_t)G.B * G.Z0 * sizeof(int) : 0, 256);
+  L.utab = off;    off += align_up((size_t)G.B * G.Z0 * G.n_shells * plan->local_umax * sizeof(LocalUEntry), 256);
+  L.ucount = off;  off += align_up(local ? (size_t)G.B * G.Z0 * G.n_shells * sizeof(int) : 0, 256);
   if (local && local_smem_bytes(G, plan->local_umax) > 227 * 1024) return SMCX_E_LINK_CELL_TOO_SMALL;
   L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
   L.filter = off;  off += align_up((size_t)kFilterWords * sizeof(uint32_t), 256);
@@ -366,13 +370,13 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   return SMCX_OK;
 }
 
-// SMCX_MODEL_LOCAL: for every (basis b of i, direction), the sites whose local energy the swap changes -- i, j, their
-// neighbours, each once -- as tile-linear steps from i, with the shells in which such a site sees i and j.
+// SMCX_MODEL_LOCAL: for every (basis b of i, direction, shell s), the sites whose shell-s term of the local energy the
+// swap changes -- i, j, and the sites that see i or j in shell s, each once -- as tile-linear steps from i.
 void build_local_utable(const Plan& P, int lattice, std::vector<LocalUEntry>& tab, std::vector<int>& count) {
   const Geom& G = P.G;
   const int umax = P.local_umax;
-  tab.assign((size_t)G.B * G.Z0 * umax, LocalUEntry{0, -1, -1, 0, 0, 0});
-  count.assign((size_t)G.B * G.Z0, 0);
+  tab.assign((size_t)G.B * G.Z0 * G.n_shells * umax, LocalUEntry{0, 0});
+  count.assign((size_t)G.B * G.Z0 * G.n_shells, 0);
   auto shell_of_vec = [&](int x, int y, int z) {
     for (int m = 0; m < G.ZT; ++m)
       if (G.off[m][0] == x && G.off[m][1] == y && G.off[m][2] == z) return (int)G.shell_of[m];
@@ -395,22 +399,24 @@ void build_local_utable(const Plan& P, int lattice, std::vector<LocalUEntry>& ta
         add(G.off[m][0], G.off[m][1], G.off[m][2]);
         add(jx + G.off[m][0], jy + G.off[m][1], jz + G.off[m][2]);
       }
-      LocalUEntry* out = tab.data() + (size_t)(b * G.Z0 + dir) * umax;
-      for (size_t k = 0; k < U.size(); ++k) {
-        const int vx = U[k][0], vy = U[k][1], vz = U[k][2];
-        const int qx = bp[0] + vx, qy = bp[1] + vy, qz = bp[2] + vz;
-        const int nb = basis_from_parity(lattice, qx, qy, qz);
-        const int d = ((floor_div2(qz) * G.TW + floor_div2(qy)) * G.TW + floor_div2(qx)) * G.B + (nb - b);
-        LocalUEntry e;
-        e.delta = (short)d;
-        e.shell_i = (signed char)shell_of_vec(-vx, -vy, -vz);            // i - u
-        e.shell_j = (signed char)shell_of_vec(jx - vx, jy - vy, jz - vz);  // j - u
-        e.kind = (vx == 0 && vy == 0 && vz == 0) ? 1 : ((vx == jx && vy == jy && vz == jz) ? 2 : 0);
-        e.basis = (unsigned char)nb;
-        e.pad = 0;
-        out[k] = e;
+      for (int s = 0; s < G.n_shells; ++s) {
+        LocalUEntry* out = tab.data() + (size_t)((b * G.Z0 + dir) * G.n_shells + s) * umax;
+        int k = 0;
+        for (const auto& v : U) {
+          const int vx = v[0], vy = v[1], vz = v[2];
+          const unsigned kind = (vx == 0 && vy == 0 && vz == 0) ? 1u : ((vx == jx && vy == jy && vz == jz) ? 2u : 0u);
+          const bool sees_i = shell_of_vec(-vx, -vy, -vz) == s;              // i - u in shell s
+          const bool sees_j = shell_of_vec(jx - vx, jy - vy, jz - vz) == s;  // j - u in shell s
+          if (!kind && !sees_i && !sees_j) continue;                          // this term does not change
+          const int qx = bp[0] + vx, qy = bp[1] + vy, qz = bp[2] + vz;
+          const int nb = basis_from_parity(lattice, qx, qy, qz);
+          const int d = ((floor_div2(qz) * G.TW + floor_div2(qy)) * G.TW + floor_div2(qx)) * G.B + (nb - b);
+          out[k].delta = (short)d;
+          out[k].bits = (unsigned short)((sees_i ? 1u : 0u) | (sees_j ? 2u : 0u) | (kind << 2) | ((unsigned)nb << 4));
+          ++k;
+        }
+        count[(size_t)(b * G.Z0 + dir) * G.n_shells + s] = k;
       }
-      count[(size_t)b * G.Z0 + dir] = (int)U.size();
     }
   }
 }

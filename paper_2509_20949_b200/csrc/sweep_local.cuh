@@ -9,10 +9,14 @@
 // cells in shared memory (a trial reads the neighbours of the neighbours of i and j).  A swap of i and j changes the
 // local energy of the sites U = {i, j} + N(i) + N(j); which tile positions those are, relative to i, depends on the
 // basis index of i and on the drawn direction only, so the host lists them once (LocalUEntry) together with the
-// shells in which such a site sees i and j.  The lanes of the warp share the sites of U: a lane counts the species
-// around its site (counts of one shell packed as eight 8-bit fields of a 64-bit word), evaluates eps before the
-// swap, corrects the counts and the own species for the swap -- the algebraic shortcut the oracle does not take: it
-// swaps and recounts -- evaluates eps after, and one warp reduction gives dE.  Integer arithmetic throughout.
+// shells in which such a site sees i and j.  eps is a sum over shells, and the swap changes the term of shell s of a
+// site only if the site sees i or j in THAT shell (or is i or j itself): the host therefore lists the affected
+// (site, shell) pairs shell by shell (2 Z_s + 2 entries per shell instead of 2 ZT + 2 sites with all their shells).
+// The lanes of the warp share the entries of one shell at a time -- so all lanes count the same shell: no divergence --
+// : a lane counts the species of that shell around its site (eight 8-bit fields of a 64-bit word), evaluates the
+// shell's term before the swap, corrects the counts and the centre species for the swap -- the algebraic shortcut the
+// oracle does not take: it swaps and recounts whole sites -- evaluates it after, and one warp reduction gives dE.
+// Integer arithmetic throughout: the sum of the changed terms is exactly the oracle's difference of whole energies.
 #pragma once
 #include "smcx_common.cuh"
 #include "sweep_warp.cuh"
@@ -23,54 +27,44 @@ constexpr int kLocalWarps = 8;
 constexpr int kLocalMaxSpecies = 8;      // eight 8-bit counters per shell word
 constexpr int kLocalMaxU = 2 + 2 * kMaxNeighbours;
 
-// One affected site of a trial (b, dir): tile-linear step from i, the shells in which the site sees i and j
-// (-1: not a neighbour), kind 1 = the site is i, 2 = it is j, and its basis index.
+// One affected (site, shell) pair of a trial (b, dir): tile-linear step from i; bits: 0 = the site sees i in this shell,
+// 1 = it sees j in this shell, 2-3 = kind (1 = the site is i, 2 = it is j), 4-5 = its basis index.
 struct LocalUEntry {
   short delta;
-  signed char shell_i, shell_j;
-  unsigned char kind, basis;
-  short pad;
+  unsigned short bits;
 };
-static_assert(sizeof(LocalUEntry) == 8, "LocalUEntry is loaded as one 8-byte word");
+static_assert(sizeof(LocalUEntry) == 4, "LocalUEntry is loaded as one word");
 
 struct LocalTables {
   const int32_t* w1;          // [n_shells][n][n]
   const int32_t* w2;          // [n_shells][n][n][n], x <= y used
-  const LocalUEntry* utab;    // [B][Z0][umax]
-  const int* ucount;          // [B][Z0]
+  const LocalUEntry* utab;    // [B][Z0][n_shells][umax]
+  const int* ucount;          // [B][Z0][n_shells]
   int umax;
 };
 
-// eps(c, counts): cnt[s] holds the counts of shell s, species x in bits 8x .. 8x + 7.  The loops run over all
-// kLocalMaxSpecies fields with compile-time bounds (fields of species >= n are zero, their weights are not read), so
-// that the weight loads of a shell are independent of one another and can all be in flight.
-// Not inlined, and the loop over the basis index in the kernel is not unrolled: with both inlined / unrolled the trial
-// loop was several times the instruction cache and ncu showed the warps waiting for instructions most of the time
-// (stall no_instruction 14.8 per issue).
-// (Evaluating only the shells in which a site sees i or j -- the others cancel between before and after -- was
-// measured slower: the lanes of a warp then need different shells and the shell loops diverge; 1.0e8 -> 7.0e7 trials/s.)
-__device__ __noinline__ int local_eps(const int32_t* __restrict__ s_w1, const int32_t* __restrict__ s_w2, int n, int n_shells,
-                                         int c, const unsigned long long (&cnt)[kMaxShells]) {
+// The term of shell s of eps(c, .): v holds the counts of that shell, species x in bits 8x .. 8x + 7.  The loops run over
+// all kLocalMaxSpecies fields with compile-time bounds (fields of species >= n are zero, their weights are not read),
+// so that the weight loads are independent of one another and can all be in flight.  Not inlined, and the loop over the
+// basis index in the kernel is not unrolled: with both inlined / unrolled the trial loop was several times the
+// instruction cache and ncu showed the warps waiting for instructions most of the time (stall no_instruction 14.8 per
+// issue).
+__device__ __noinline__ int local_eps_shell(const int32_t* __restrict__ s_w1, const int32_t* __restrict__ s_w2, int n, int s, int c,
+                                            unsigned long long v) {
+  const int32_t* l = s_w1 + (s * n + c) * n;
+  const int32_t* q = s_w2 + (s * n + c) * n * n;
+  int nx[kLocalMaxSpecies];
+#pragma unroll
+  for (int x = 0; x < kLocalMaxSpecies; ++x) nx[x] = (int)((v >> (8 * x)) & 255ull);
   int e = 0;
 #pragma unroll
-  for (int s = 0; s < kMaxShells; ++s) {
-    if (s < n_shells) {
-      const int32_t* l = s_w1 + (s * n + c) * n;
-      const int32_t* q = s_w2 + (s * n + c) * n * n;
-      const unsigned long long v = cnt[s];
-      int nx[kLocalMaxSpecies];
+  for (int x = 0; x < kLocalMaxSpecies; ++x) {
+    if (x < n) {
+      int row = l[x];
 #pragma unroll
-      for (int x = 0; x < kLocalMaxSpecies; ++x) nx[x] = (int)((v >> (8 * x)) & 255ull);
-#pragma unroll
-      for (int x = 0; x < kLocalMaxSpecies; ++x) {
-        if (x < n) {
-          int row = l[x];
-#pragma unroll
-          for (int y = x; y < kLocalMaxSpecies; ++y)
-            if (y < n) row += q[x * n + y] * nx[y];
-          e += row * nx[x];
-        }
-      }
+      for (int y = x; y < kLocalMaxSpecies; ++y)
+        if (y < n) row += q[x * n + y] * nx[y];
+      e += row * nx[x];
     }
   }
   return e;
@@ -79,7 +73,7 @@ __device__ __noinline__ int local_eps(const int32_t* __restrict__ s_w1, const in
 inline size_t local_smem_bytes(const Geom& G, int umax) {
   const int n = G.n_species;
   size_t b = (size_t)G.n_shells * n * n * 4 + (size_t)G.n_shells * n * n * n * 4;
-  b += (size_t)G.B * G.Z0 * umax * sizeof(LocalUEntry) + (size_t)G.B * G.Z0 * 4;
+  b += (size_t)G.B * G.Z0 * G.n_shells * umax * sizeof(LocalUEntry) + (size_t)G.B * G.Z0 * G.n_shells * 4;
   b += (size_t)G.B * G.ZT * 2 + 16;
   b = (b + 15) & ~(size_t)15;
   return b + (size_t)kLocalWarps * (((size_t)G.TW * G.TW * G.TW * G.B + 15) & ~(size_t)15);
@@ -94,8 +88,8 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
   int32_t* s_w1 = reinterpret_cast<int32_t*>(smem);
   int32_t* s_w2 = s_w1 + n_shells * n * n;
   LocalUEntry* s_u = reinterpret_cast<LocalUEntry*>(s_w2 + n_shells * n * n * n);
-  int* s_ucount = reinterpret_cast<int*>(s_u + B * Z0 * T.umax);
-  short* s_delta = reinterpret_cast<short*>(s_ucount + B * Z0);
+  int* s_ucount = reinterpret_cast<int*>(s_u + B * Z0 * n_shells * T.umax);
+  short* s_delta = reinterpret_cast<short*>(s_ucount + B * Z0 * n_shells);
   const int tile_sites = G.TW * G.TW * G.TW * B;
   size_t tables = (size_t)(reinterpret_cast<unsigned char*>(s_delta + B * ZT) - smem) + 16;
   tables = (tables + 15) & ~(size_t)15;
@@ -107,8 +101,8 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
 
   for (int k = threadIdx.x; k < n_shells * n * n; k += blockDim.x) s_w1[k] = T.w1[k];
   for (int k = threadIdx.x; k < n_shells * n * n * n; k += blockDim.x) s_w2[k] = T.w2[k];
-  for (int k = threadIdx.x; k < B * Z0 * T.umax; k += blockDim.x) s_u[k] = T.utab[k];
-  for (int k = threadIdx.x; k < B * Z0; k += blockDim.x) s_ucount[k] = T.ucount[k];
+  for (int k = threadIdx.x; k < B * Z0 * n_shells * T.umax; k += blockDim.x) s_u[k] = T.utab[k];
+  for (int k = threadIdx.x; k < B * Z0 * n_shells; k += blockDim.x) s_ucount[k] = T.ucount[k];
   for (int k = threadIdx.x; k < B * ZT; k += blockDim.x) s_delta[k] = G.delta[k / ZT][k % ZT];
   if (threadIdx.x <= kMaxShells) {      // shells are listed one after the other: first neighbour of every shell
     int first = ZT;
@@ -166,34 +160,29 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
             const int sj = si + s_delta[b * ZT + dir];
             const int sa = tile[si], sb = tile[sj];
             if (sa == sb) continue;   // same species: counts as a trial only
-            // a5: local energies of the affected sites, before and after
+            // a5: the changed terms of the local energies, before and after, shell by shell
             const unsigned long long da = 1ull << (8 * sa), db = 1ull << (8 * sb);
-            const LocalUEntry* ue = s_u + (b * Z0 + dir) * T.umax;
-            const int nu = s_ucount[b * Z0 + dir];
             int part = 0;
-            for (int q = lane; q < nu; q += 32) {
-              const LocalUEntry e = ue[q];
-              const int su = si + e.delta;
-              const short* dl = s_delta + (int)e.basis * ZT;
-              unsigned long long cnt[kMaxShells];
-#pragma unroll
-              for (int s = 0; s < kMaxShells; ++s) {
-                cnt[s] = 0ull;
-                if (s < n_shells) {
-                  const int m1 = s_start[s + 1];
+            for (int s = 0; s < n_shells; ++s) {
+              const LocalUEntry* ue = s_u + ((b * Z0 + dir) * n_shells + s) * T.umax;
+              const int nu = s_ucount[(b * Z0 + dir) * n_shells + s];
+              const int m0 = s_start[s], m1 = s_start[s + 1];
+              for (int q = lane; q < nu; q += 32) {
+                const LocalUEntry e = ue[q];
+                const unsigned bits = e.bits;
+                const int su = si + e.delta;
+                const short* dl = s_delta + (int)((bits >> 4) & 3u) * ZT;
+                unsigned long long cnt = 0ull;
 #pragma unroll 6
-                  for (int mm = s_start[s]; mm < m1; ++mm) cnt[s] += 1ull << (8 * (int)tile[su + dl[mm]]);   // six loads in flight
-                }
+                for (int mm = m0; mm < m1; ++mm) cnt += 1ull << (8 * (int)tile[su + dl[mm]]);   // six loads in flight
+                const int c0 = tile[su];
+                const int before = local_eps_shell(s_w1, s_w2, n, s, c0, cnt);
+                if (bits & 1u) cnt += db - da;   // i turns from a into b
+                if (bits & 2u) cnt += da - db;   // j turns from b into a
+                const unsigned kind = (bits >> 2) & 3u;
+                const int c1 = kind == 1u ? sb : (kind == 2u ? sa : c0);
+                part += local_eps_shell(s_w1, s_w2, n, s, c1, cnt) - before;
               }
-              const int c0 = tile[su];
-              const int before = local_eps(s_w1, s_w2, n, n_shells, c0, cnt);
-#pragma unroll
-              for (int s = 0; s < kMaxShells; ++s) {
-                if ((int)e.shell_i == s) cnt[s] += db - da;   // i turns from a into b
-                if ((int)e.shell_j == s) cnt[s] += da - db;   // j turns from b into a
-              }
-              const int c1 = e.kind == 1 ? sb : (e.kind == 2 ? sa : c0);
-              part += local_eps(s_w1, s_w2, n, n_shells, c1, cnt) - before;
             }
             const int dE = __reduce_add_sync(0xffffffffu, part);
             // a6: Eq. 3 in integer form
@@ -286,7 +275,9 @@ local_energy_kernel(const Geom G, const uint8_t* __restrict__ species, const int
       for (int s = 0; s < kMaxShells; ++s)
         if (sh == s) cnt[s] += one;
     }
-    sum += local_eps(s_w1, s_w2, n, n_shells, (int)species[i], cnt);
+#pragma unroll
+    for (int s = 0; s < kMaxShells; ++s)
+      if (s < n_shells) sum += local_eps_shell(s_w1, s_w2, n, s, (int)species[i], cnt[s]);
   }
   for (int o = 16; o > 0; o >>= 1) sum += __shfl_down_sync(0xffffffffu, sum, o);
   if ((threadIdx.x & 31) == 0) s_sum[threadIdx.x >> 5] = sum;
