@@ -398,6 +398,37 @@ def run_lattice_parallel_one_gpu(cfg, sweeps: int = 10, whole_sweep_ms=None):
                             "unit": "trial swaps/s", "message_bytes_per_sweep": int(g.message_bytes - b0),
                             "vs_undivided": (whole_sweep_ms / ms) if whole_sweep_ms else None})
         g.close()
+    # connected slabs (the one-slab-per-process path of `--gpus N`) with both slabs in this process: messages written by
+    # the sweep kernels into the neighbour's storage, ordering by flags and stream memory waits, no events, no copies
+    import torch
+    kw = dict(lattice=cfg.lattice, dims=cfg.dims, n_species=cfg.n_species, n_shells=cfg.n_shells, epi=cfg.epi(),
+              accept=cfg.accept_table(0), seed=cfg.seed, link_cell=cfg.link_cell, kT_units=cfg.kT_at(0))
+    streams = [torch.cuda.Stream() for _ in range(2)]
+    slabs = [smcx.Domain(2, r, stream=streams[r], **kw) for r in range(2)]
+    for r in range(2):
+        slabs[r].connect(slabs[1 - r], slabs[1 - r])
+
+    def step(n):
+        for _ in range(n):
+            for sl in slabs:
+                sl.sweep_connected(1)
+    step(3)
+    torch.cuda.synchronize()
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for st in streams:
+        st.wait_event(a)
+    step(sweeps)
+    for st in streams:
+        torch.cuda.current_stream().wait_stream(st)
+    b.record()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b) / sweeps
+    out["runs"].append({"slabs": 2, "mode": "connected slabs (flags + stream memory waits, messages fused), both in this process",
+                        "fused_messages_per_sweep": 16, "sweep_ms": ms, "value": cfg.n_sites / (ms * 1e-3), "unit": "trial swaps/s",
+                        "message_bytes_per_sweep": None, "vs_undivided": (whole_sweep_ms / ms) if whole_sweep_ms else None})
+    for sl in slabs:
+        sl.close()
     return out
 
 
