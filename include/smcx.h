@@ -294,11 +294,18 @@ int64_t smcx_ensemble_kernel_launches(smcx_ensemble_t *e); /* ensemble kernels +
  *     and pass, H + 1 layers, contiguous in device storage (layers are the slowest index of every storage format);
  *   - overlap: a pass is launched as the boundary row first, then the message leaves on a copy stream while the
  *     other rows of the pass run.
- * Two ways to run it.  smcx_domain_group_*: all slabs in one process, on one or several devices, messages as
- * device-to-device / peer copies ordered by events -- no host synchronisation inside a sweep.  smcx_domain_*: one slab
- * per handle (one process per GPU); the caller moves the messages (e.g. torch.distributed send/recv over NCCL on the
- * byte ranges the message calls name) between smcx_domain_pass calls.  Within one process the pass messages of the packed
- * kernels are fused into the sweep kernel (smcx_domain_pass_fused): the group then moves only the window shift by copy. */
+ * Three ways to run it.  (1) Connected slabs, smcx_domain_ipc_* / smcx_domain_sweep_connected: one slab per process and
+ * GPU, the neighbours' storage mapped with CUDA IPC, messages written by the sweep kernels into the neighbour's memory
+ * and signalled through device flags -- no host code in the data path (see below).  (2) smcx_domain_group_*: all slabs
+ * in one process, on one or several devices, ordered by events; the pass messages of the packed kernels are fused into
+ * the boundary-row kernel (smcx_domain_pass_fused), which runs next to the other rows of the pass; only the window
+ * shift is a copy.  (3) smcx_domain_begin_sweep / _pass / _pass_split / _end_sweep: one slab per handle stepped by the
+ * caller, who moves the messages (e.g. torch.distributed send/recv over NCCL on the byte ranges the message calls
+ * name) -- for slabs on different nodes.
+ * Errors: the calls return SMCX_E_RANGE when used out of order (a pass outside begin/end_sweep, results asked for in
+ * the middle of a sweep), SMCX_E_BAD_DIMS for a cut the lattice does not allow, SMCX_E_UNSUPPORTED where stated, and
+ * otherwise what the underlying handle returns.  All pointers are the caller's; device pointers must be valid on the
+ * slab's device (peer access enabled when they belong to another GPU). */
 typedef struct smcx_domain smcx_domain_t;
 typedef struct smcx_domain_group smcx_domain_group_t;
 
