@@ -52,7 +52,7 @@ def measured_peak():
 
 
 KERNEL_NAMES = {1: "sweep_warp_per_cell", 2: "sweep_thread_per_cell", 3: "sweep_thread_persistent", 4: "sweep_group_per_cell",
-                5: "sweep_fcc_thread"}
+                5: "sweep_fcc_thread", 6: "sweep_local_warp", 7: "sweep_bcc4_thread"}
 STORAGE_NAMES = {2: "2bit", 4: "4bit", 8: "u8"}
 # Sources a kernel is compiled from: a number taken from an ncu capture (DRAM traffic, instruction counts per trial)
 # is only reported next to live timings while these files are what they were at the capture.
@@ -62,6 +62,8 @@ KERNEL_SOURCES = {
     3: ["sweep_thread.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
     4: ["sweep_group.cuh", "sweep_thread.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
     5: ["sweep_fcc.cuh", "sweep_thread.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
+    6: ["sweep_local.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
+    7: ["sweep_bcc4.cuh", "sweep_fcc.cuh", "sweep_thread.cuh", "sweep_warp.cuh", "smcx_common.cuh"],
 }
 CAPTURES = os.path.join(ROOT, "profiles", "dram_traffic.csv")
 
@@ -359,6 +361,28 @@ def run_local_model(edge: int = 128, sweeps: int = 5):
            "paper_qsro_h800_per_gpu": 3.7e7, "paper_note": "PAPER.md:130, qSRO model on H800: another model and GPU, context only"}
     lat.close()
     return out
+
+
+def run_bcc_five_species(edge: int = 800, sweeps: int = 10):
+    """The graded lattice shape with FIVE species (more than the 2-bit kernels take): BCC edge^3, two shells, kT = 60 meV;
+    the kernel AUTO picks (packed 4-bit BCC kernel, sweep_bcc4.cuh) and, beside it, the sub-warp kernel on uint8."""
+    import paper_2509_20949_b200 as smcx
+    from smcx_inputs import make_accept_table, make_epi
+
+    peak, _ = measured_peak()
+    out = {}
+    for key, kernel in (("auto", smcx.KERNEL_AUTO), ("sub_warp", smcx.KERNEL_GROUP_PER_CELL)):
+        lat = smcx.Lattice(smcx.BCC, (edge, edge, edge), 5, 2, make_epi(2, 5, 300, 1008), make_accept_table(600), 1008,
+                           link_cell=4, kT_units=600, kernel=kernel)
+        ms = _time_sweeps(lat, 3, sweeps)
+        out[key] = {"kernel": f"{KERNEL_NAMES[lat.kernel]}/{STORAGE_NAMES[lat.storage]}", "value": lat.n_sites / (ms * 1e-3), "sweep_ms": ms}
+        n_sites = lat.n_sites
+        lat.close()
+    v = out["auto"]["value"]
+    return {"workload": f"BCC {edge}^3 conventional cells ({n_sites} sites), 5 species equiatomic, 2-shell int32 EPI in [-300,300], "
+                        f"kT=60 meV, link cell 4, seed 1008", "kernel": out["auto"]["kernel"], "value": v, "unit": "trial swaps/s",
+            "sweep_ms": out["auto"]["sweep_ms"], "frac_of_hbm_roofline": v * ALGO_BYTES_PER_TRIAL / (peak * 1e9),
+            "sub_warp_kernel": out["sub_warp"]}
 
 
 def run_largest_single_gpu(sweeps: int = 20):
@@ -716,6 +740,8 @@ def run_cuda(args, cfg, rank, world, local_rank):
                 out["largest_single_gpu"] = run_largest_single_gpu()
             if args.local_edge > 0:
                 out["local_energy_model"] = run_local_model(args.local_edge)
+            if args.fcc_edge > 0:
+                out["bcc_five_species"] = run_bcc_five_species()
             if args.slabs_leg and cfg.dims[2] // cfg.link_cell >= 16:
                 out["lattice_parallel_one_gpu"] = run_lattice_parallel_one_gpu(cfg, whole_sweep_ms=sweep_ms / args.steps)
         print(json.dumps(out))

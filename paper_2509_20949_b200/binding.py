@@ -17,6 +17,7 @@ STORAGE_AUTO, STORAGE_2BIT, STORAGE_4BIT, STORAGE_U8 = 0, 2, 4, 8
 KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT, KERNEL_GROUP_PER_CELL = 0, 1, 2, 3, 4
 KERNEL_FCC_THREAD = 5
 KERNEL_LOCAL_WARP = 6
+KERNEL_BCC4_THREAD = 7
 MODEL_EPI, MODEL_LOCAL = 0, 1
 
 

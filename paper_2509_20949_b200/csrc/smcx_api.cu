@@ -20,6 +20,7 @@
 #include "ensemble_kernels.cuh"
 #include "lattice_kernels.cuh"
 #include "smcx_common.cuh"
+#include "sweep_bcc4.cuh"
 #include "sweep_fcc.cuh"
 #include "sweep_group.cuh"
 #include "sweep_local.cuh"
@@ -80,6 +81,8 @@ int basis_from_parity(int lattice, int px, int py, int pz) {
 inline int floor_div2(int v) { return v >= 0 ? v / 2 : -((-v + 1) / 2); }
 
 inline bool is_thread_kernel(int k) { return k == SMCX_KERNEL_THREAD_PER_CELL || k == SMCX_KERNEL_THREAD_PERSISTENT; }
+// kernels whose write-back can mirror the layers of a slab's pass message into the neighbour's storage
+inline bool has_fused_writeback(int k) { return is_thread_kernel(k) || k == SMCX_KERNEL_FCC_THREAD || k == SMCX_KERNEL_BCC4_THREAD; }
 
 struct Layout {
   size_t species, epi, coef, gtable, fcc_lut, fcc_corr, quad, utab, ucount, accept, filter, trace, state, counts, total;
@@ -97,6 +100,7 @@ struct Plan {
   bool coef_packed; // pack_thread_coefficients: the 16-bit coefficient rows are exact
   int fcc_rep;      // sweep_fcc_thread: replicas of the look-up rows in shared memory
   FccTables fcc_tables;
+  Bcc4Tables bcc4_tables;
   Layout lay;
   int model = SMCX_MODEL_EPI;
   int local_umax = 0;   // SMCX_MODEL_LOCAL: affected sites per (basis, direction, shell), at most
@@ -267,7 +271,15 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     fcc_ok = fcc_build_lut(p->epi, n, p->n_shells, 1, lut, corr) && fcc_build_tables<32, kFccWinRows>(G, plan->fcc_tables);
     plan->fcc_rep = fcc_lut_rep(n);
   }
+  // packed BCC kernel for up to 8 species (4-bit storage): geometry, and every EPI difference must fit the 16-bit look-up
+  bool bcc4_ok = bcc4_kernel_supported(G);
+  if (bcc4_ok) {
+    std::vector<uint32_t> lut;
+    std::vector<int32_t> corr;
+    bcc4_ok = fcc_build_lut(p->epi, n, p->n_shells, 1, lut, corr) && bcc4_build_tables<32>(G, plan->bcc4_tables);
+  }
   int kernel = p->kernel, storage = p->storage;
+  if (local) bcc4_ok = false;
   if (local) {
     if (kernel == SMCX_KERNEL_AUTO) kernel = SMCX_KERNEL_LOCAL_WARP;
     if (kernel != SMCX_KERNEL_LOCAL_WARP) return SMCX_E_UNSUPPORTED;
@@ -286,6 +298,8 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     // lasts as long as one cell's chain of trials, which is shorter with several lanes per cell
     if (fcc_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && plan->n_cells / 8 >= 148ll * kFccWarps * 32)))
       kernel = SMCX_KERNEL_FCC_THREAD;
+    else if (bcc4_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && !fast_ok && plan->n_cells / 8 >= 148ll * kBcc4Warps * 32)))
+      kernel = SMCX_KERNEL_BCC4_THREAD;
     else if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_GROUP_PER_CELL;
     else if (!fast_ok) kernel = SMCX_KERNEL_GROUP_PER_CELL;
     // The persistent kernel (one block of 20 warps and ~220 KB of shared memory per SM) pays off once
@@ -303,6 +317,11 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     if (!fcc_ok) return SMCX_E_UNSUPPORTED;
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_4BIT;
     if (storage != SMCX_STORAGE_4BIT) return SMCX_E_UNSUPPORTED;
+  } else if (kernel == SMCX_KERNEL_BCC4_THREAD) {
+    if (!bcc4_ok) return SMCX_E_UNSUPPORTED;
+    if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_4BIT;
+    if (storage != SMCX_STORAGE_4BIT) return SMCX_E_UNSUPPORTED;
+    plan->fcc_rep = bcc4_lut_rep();
   } else if (kernel == SMCX_KERNEL_WARP_PER_CELL || kernel == SMCX_KERNEL_GROUP_PER_CELL || kernel == SMCX_KERNEL_LOCAL_WARP) {
     if (storage == SMCX_STORAGE_AUTO) storage = SMCX_STORAGE_U8;
     if (storage != SMCX_STORAGE_U8) return SMCX_E_UNSUPPORTED;
@@ -426,7 +445,7 @@ void build_local_utable(const Plan& P, int lattice, std::vector<LocalUEntry>& ta
 // kernels that read the two-level acceptance filter tables
 inline bool uses_filter(const Plan& P) {
   return (is_thread_kernel(P.kernel) && P.coef_class == 2) || P.kernel == SMCX_KERNEL_GROUP_PER_CELL ||
-         P.kernel == SMCX_KERNEL_FCC_THREAD;
+         P.kernel == SMCX_KERNEL_FCC_THREAD || P.kernel == SMCX_KERNEL_BCC4_THREAD;
 }
 
 struct smcx {
@@ -679,6 +698,13 @@ int launch_colour_pass(smcx* h, const Geom& G, int colour) {
     if (rc != 0) { h->err = "packed FCC thread-per-cell launch failed"; return SMCX_E_CUDA; }
     return SMCX_OK;
   }
+  if (P.kernel == SMCX_KERNEL_BCC4_THREAD) {
+    const int rc = launch_bcc4_thread(G, P.bcc4_tables, reinterpret_cast<uint32_t*>(h->d_species()), h->d_fcc_lut(), h->d_fcc_corr(),
+                                      P.fcc_rep, h->d_accept(), h->d_filter(), h->d_state(), colour, h->sm_count, h->stream);
+    h->launches++;
+    if (rc != 0) { h->err = "packed BCC (4-bit) thread-per-cell launch failed"; return SMCX_E_CUDA; }
+    return SMCX_OK;
+  }
   if (P.kernel == SMCX_KERNEL_LOCAL_WARP) {
     const LocalTables T{h->d_epi(), h->d_quad(), h->d_utab(), h->d_ucount(), P.local_umax};
     const size_t sm = local_smem_bytes(G, P.local_umax);
@@ -804,6 +830,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
   }
   if (configure_thread_per_cell() != 0) return fail(SMCX_E_CUDA);
   if (h->plan.kernel == SMCX_KERNEL_FCC_THREAD && configure_fcc_thread(h->plan.fcc_rep) != 0) return fail(SMCX_E_CUDA);
+  if (h->plan.kernel == SMCX_KERNEL_BCC4_THREAD && configure_bcc4_thread(h->plan.fcc_rep) != 0) return fail(SMCX_E_CUDA);
   // every kernel of a sweep prefers the largest shared-memory carve-out: an SM whose carve-out must
   // change drains first, which serialises lattices that run concurrently (replica ensembles:
   // measured 45 us instead of 28 us per colour pass when the one-thread epilogue asked for the default)
@@ -865,7 +892,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     }
     std::vector<uint32_t> flut;
     std::vector<int32_t> fcorr;
-    if (h->plan.kernel == SMCX_KERNEL_FCC_THREAD) {
+    if (h->plan.kernel == SMCX_KERNEL_FCC_THREAD || h->plan.kernel == SMCX_KERNEL_BCC4_THREAD) {
       fcc_build_lut(h->epi.data(), h->plan.G.n_species, h->plan.G.n_shells, h->plan.fcc_rep, flut, fcorr);
       SMCX_CUDA(h, cudaMemcpyAsync(h->d_fcc_lut(), flut.data(), flut.size() * sizeof(uint32_t), cudaMemcpyHostToDevice, h->stream));
       SMCX_CUDA(h, cudaMemcpyAsync(h->d_fcc_corr(), fcorr.data(), fcorr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));

@@ -1,5 +1,5 @@
 // Packed thread-per-cell colour-pass kernel for FCC lattices (the paper's own lattice:
-// PAPER.md:118, 141, 165): FCC, the first 1..3 neighbour shells (12 + 6 + 24 neighbours), link cell w = 4,
+// PAPER.md:118, 141, 165): FCC, the first 2..3 neighbour shells (12 + 6 + 24 neighbours; the tile is 8^3 cells), link cell w = 4,
 // n_species <= 8, SMCX_STORAGE_4BIT.
 //
 // Layout facts the kernel rests on:

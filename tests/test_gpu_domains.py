@@ -288,3 +288,17 @@ def test_a_fourth_connected_slab_in_one_process_is_refused():
         again[r].connect(again[1 - r], again[1 - r])
     for s in again:
         s.close()
+
+
+def test_packed_bcc4_kernel_on_slabs_with_fused_messages():
+    """Five species on BCC (4-bit storage, SMCX_KERNEL_BCC4_THREAD) cut into 2 and 3 slabs; the kernel's write-back carries
+    the pass messages."""
+    kw = _kw(smcx.BCC, (16, 16, 48), 5, 2, seed=47)
+    o = _oracle(kw)
+    o.sweep(6)
+    for n_slabs in (2, 3):
+        g = smcx.DomainGroup(n_slabs, kernel=smcx.KERNEL_BCC4_THREAD, **kw)
+        g.sweep(6)
+        _assert_same(g, o)
+        assert g.fused_messages > 0
+        g.close()

@@ -591,3 +591,59 @@ def test_paper_shaped_fcc_full_size_invariants():
     o.sweep(3)
     _assert_same_state(s, o)
     assert (s.energy_trace() == o.energy_trace()).all() and s.stats() == o.stats()
+
+
+# ---- packed BCC kernel for up to 8 species (SMCX_KERNEL_BCC4_THREAD, SMCX_STORAGE_4BIT) ----------------------------
+@pytest.mark.parametrize("dims,n_sp,n_sh,amp,kT", [
+    ((16, 16, 16), 5, 2, 300, 600),       # five species: one more than the 2-bit kernels take
+    ((24, 16, 8), 8, 2, 400, 860),        # most species the look-up takes, one cell per colour along z
+    ((16, 8, 24), 6, 2, 300, 500),
+    ((40, 24, 16), 5, 2, 15_000, 9_000),  # differences that need the high byte of the look-up in full
+    ((32, 32, 32), 3, 2, 300, 430),       # more than one batch of 32 cells per colour; fewer species than 4 is fine too
+    ((24, 24, 8), 7, 2, 300, 700),        # 9 cells per colour: a ragged batch
+])
+def test_packed_bcc4_kernel_against_the_oracle(dims, n_sp, n_sh, amp, kT):
+    lat, w, seed = 0, 4, 616
+    epi = make_epi(n_sh, n_sp, amp, seed)
+    table = make_accept_table(kT)
+    g = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, seed, link_cell=w, kT_units=kT, kernel=smcx.KERNEL_BCC4_THREAD)
+    assert g.storage == smcx.STORAGE_4BIT and g.kernel == smcx.KERNEL_BCC4_THREAD
+    o = oracle.Oracle(lat, dims, n_sp, n_sh, epi, w, table, seed)
+    _assert_same_state(g, o)                       # S6 through Store4<2>
+    assert g.energy() == o.energy() == g.running_energy()
+    for _ in range(4):
+        g.sweep(1)
+        o.sweep(1)
+        _assert_same_state(g, o)
+    g.sweep(3)                                     # graph replay
+    o.sweep(3)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all()
+    assert g.stats() == o.stats() and g.stats()[2] > 0
+    assert g.energy() == o.energy() == g.running_energy()
+    _assert_sro(g, o)                              # pair counts on 4-bit BCC storage
+
+
+def test_packed_bcc4_agrees_with_the_other_bcc_kernels_and_round_trips_checkpoints():
+    """P14 on BCC: 4-bit storage (packed kernel), 2-bit storage (thread kernels) and uint8 (sub-warp kernel) walk the same
+    trajectory with 4 species; the packed checkpoint of the 4-bit handle resumes bit for bit."""
+    lat, dims, n_sp, n_sh, seed = 0, (32, 16, 24), 4, 2, 88
+    epi = make_epi(n_sh, n_sp, 300, seed)
+    table = make_accept_table(600)
+    hs = [smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, seed, link_cell=4, kT_units=600, kernel=k)
+          for k in (smcx.KERNEL_BCC4_THREAD, smcx.KERNEL_THREAD_PERSISTENT, smcx.KERNEL_GROUP_PER_CELL)]
+    assert [h.storage for h in hs] == [smcx.STORAGE_4BIT, smcx.STORAGE_2BIT, smcx.STORAGE_U8]
+    for h in hs:
+        h.sweep(5)
+    for h in hs[1:]:
+        assert (hs[0].species() == h.species()).all() and (hs[0].energy_trace() == h.energy_trace()).all()
+        assert hs[0].stats() == h.stats() and (hs[0].sro()[1] == h.sro()[1]).all()
+    a = hs[0]
+    assert a.storage_bytes() == a.n_sites // 2
+    packed, t = a.species_packed().copy(), a.stats()[0]
+    a.sweep(2)
+    b = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, seed, link_cell=4, kT_units=600, kernel=smcx.KERNEL_BCC4_THREAD)
+    b.set_species_packed(packed)
+    b.set_sweep_counter(t)
+    b.sweep(2)
+    assert (a.species() == b.species()).all()
