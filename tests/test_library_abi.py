@@ -64,8 +64,11 @@ def test_parameter_validation_codes():
     assert _code(accept=np.zeros(0, np.uint32)) == E["BAD_TABLE"]
     assert _code(storage=smcx.STORAGE_2BIT, kernel=smcx.KERNEL_WARP_PER_CELL) == E["UNSUPPORTED"]
     assert _code(lattice=1, n_shells=3, epi=make_epi(3, 4, 300, 1), kernel=smcx.KERNEL_THREAD_PER_CELL) == E["UNSUPPORTED"]
-    # 4-bit storage belongs to the packed FCC kernel
-    assert _code(storage=smcx.STORAGE_4BIT) == E["UNSUPPORTED"]                                  # BCC
+    # 4-bit storage belongs to the packed FCC / BCC kernels (the BCC one: two shells, link cell 4, <= 8 species)
+    assert workspace_bytes(**_kw(storage=smcx.STORAGE_4BIT)) > 16 * 16 * 16                       # BCC, 2 shells: sweep_bcc4_thread
+    assert _code(storage=smcx.STORAGE_4BIT, n_shells=1, epi=make_epi(1, 4, 300, 1)) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_BCC4_THREAD, n_species=9, epi=make_epi(2, 9, 300, 1)) == E["UNSUPPORTED"]
+    assert _code(kernel=smcx.KERNEL_BCC4_THREAD, storage=smcx.STORAGE_U8) == E["UNSUPPORTED"]
     fcc = dict(lattice=1, n_shells=3, n_species=5, epi=make_epi(3, 5, 400, 1))
     assert _code(storage=smcx.STORAGE_4BIT, kernel=smcx.KERNEL_GROUP_PER_CELL, **fcc) == E["UNSUPPORTED"]
     assert _code(kernel=smcx.KERNEL_FCC_THREAD, storage=smcx.STORAGE_U8, **fcc) == E["UNSUPPORTED"]
