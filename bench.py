@@ -311,7 +311,12 @@ def _time_sweeps(lat, warm: int, sweeps: int) -> float:
     return a.elapsed_time(b) / sweeps
 
 
-def run_paper_shaped_fcc(edge: int = 400, sweeps: int = 10):
+# Edge of the `paper_shaped_fcc` leg: FCC 640^3 = 1.05e9 sites, the size of the paper's per-GPU lattices (PAPER.md:141
+# "1e9 sites per GPU", PAPER.md:165 1.07e9 sites).  tests/test_gpu_parity.py checks the same lattice.
+PAPER_FCC_EDGE = 640
+
+
+def run_paper_shaped_fcc(edge: int = PAPER_FCC_EDGE, sweeps: int = 10):
     """A lattice of the paper's own shape: FCC, five species in the proportions
     29/29/28/7/7 (reading S10), three shells, kT = 86 meV, synthetic EPI; the kernel AUTO picks (packed FCC kernel on
     4-bit storage) and, beside it, the sub-warp kernel on uint8 storage; device-timed."""
@@ -761,7 +766,7 @@ def main():
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 warp-per-cell, 2 thread-per-cell, 3 thread-per-cell persistent, 4 sub-warp group per cell, 5 packed FCC thread-per-cell")
     ap.add_argument("--storage", type=int, default=0, help="0 auto, 2 packed 2-bit, 4 packed 4-bit, 8 uint8")
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--fcc-edge", type=int, default=400,
+    ap.add_argument("--fcc-edge", type=int, default=PAPER_FCC_EDGE,
                     help="with --ensemble: also time the sub-warp kernel on an FCC lattice of the paper's shape, this many "
                          "conventional cells per edge (0: skip)")
     ap.add_argument("--no-largest", dest="largest", action="store_false",

@@ -562,12 +562,14 @@ def test_packed_checkpoint_roundtrip(storage, lat, dims, n_sp, kernel):
 
 
 def test_paper_shaped_fcc_full_size_invariants():
-    """The lattice bench.py times as `paper_shaped_fcc` (FCC 400^3, 29/29/28/7/7, three shells) in the launch
+    """The lattice bench.py times as `paper_shaped_fcc` (FCC 640^3 = 1.05e9 sites, 29/29/28/7/7, three shells) in the launch
     configuration it is timed in (AUTO -> packed FCC kernel): conservation, energy bookkeeping, H = 1/2 sum V N; and the
     same build against the oracle on a 96 x 80 x 64 box (ragged batches: 12 * 10 * 8 / 8 = 120 cells per colour)."""
     from smcx_inputs import composition_counts
     epi, table = make_epi(3, 5, 400, 1006), make_accept_table(860)
-    g = smcx.Lattice(smcx.FCC, (400, 400, 400), 5, 3, epi, table, 1006, link_cell=4, kT_units=860)
+    import bench
+    edge = bench.PAPER_FCC_EDGE
+    g = smcx.Lattice(smcx.FCC, (edge, edge, edge), 5, 3, epi, table, 1006, link_cell=4, kT_units=860)
     assert g.kernel == smcx.KERNEL_FCC_THREAD and g.storage == smcx.STORAGE_4BIT
     counts = composition_counts(g.n_sites, (29, 29, 28, 7, 7))
     g.init_composition(counts)
