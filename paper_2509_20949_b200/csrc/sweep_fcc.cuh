@@ -42,16 +42,28 @@
 
 namespace smcxk {
 
-constexpr int kFccWarps = 8;                 // 8 x 24 KB of tile windows + tables in 227 KB
+constexpr int kFccWarps = 12;                // 12 x 16 KB of tile windows + tables in 227 KB
 constexpr int kFccRows = 64;                 // rows (y + 8 z) per sublattice of a whole tile (8 layers)
-constexpr int kFccWinLayers = 6;             // z layers of the tile the kernel keeps in shared memory at a time
+constexpr int kFccWinLayers = 4;             // z layers per sublattice the kernel keeps in shared memory at a time
 constexpr int kFccWinRows = 8 * kFccWinLayers;
 constexpr int kFccMaxSpecies = 8;            // PRMT selectors are 3 bits
 constexpr int kFccBias = 32768;              // D + bias is looked up as two unsigned bytes
 
+__host__ __device__ constexpr int fcc_beta(int b, int axis) {   // S0: basis positions, units of a/2
+  return axis == 0 ? ((b >> 1) & 1) : axis == 1 ? (b & 1) : (((b >> 1) ^ b) & 1);
+}
+
+// ROWS = 64: the whole tile, row y + 8 z of sublattice s at word s * 64 + row.
+// ROWS < 64 (the kernel's window of kFccWinLayers layers): the trials of layer lz of the cell (tile layer lz + 2) reach
+// three half-units up and down, i.e. tile layers lz + 1 .. lz + 4 of the sublattices with beta_z = 0 and lz .. lz + 3 of
+// those with beta_z = 1 -- four layers each.  Sublattice s keeps tile layer rz in slot rz - lz - (1 - beta_z(s)); seen
+// from the row pointers of the gather this is a constant offset per sublattice (sub()), so the trial code is the same.
 template <int NT, int ROWS = kFccRows> struct FccTile {
   static constexpr int kRow = 4 * NT;                 // bytes from one row to the next (NT lanes interleaved)
   static constexpr int kSub = ROWS * kRow;            // bytes from one sublattice to the next (ROWS rows each)
+  __host__ __device__ static constexpr int sub(int s) {   // byte offset of row 0 of (virtual) slot 0 of sublattice s
+    return s * kSub - (ROWS < kFccRows ? (1 - fcc_beta(s, 2)) * 8 * kRow : 0);
+  }
 };
 
 // Direction table, [b][dir]: what the partner j = i + O_0[dir] of a site of sublattice b needs.
@@ -62,9 +74,6 @@ template <int NT, int ROWS = kFccRows> struct FccTile {
 struct FccDirEntry { int32_t d[4]; int32_t e3, e2, pad0, pad1; };
 struct FccTables { FccDirEntry dir[4][12]; };
 
-__host__ __device__ constexpr int fcc_beta(int b, int axis) {   // S0: basis positions, units of a/2
-  return axis == 0 ? ((b >> 1) & 1) : axis == 1 ? (b & 1) : (((b >> 1) ^ b) & 1);
-}
 // offset (rows) of the base row of partner sublattice bs ^ k relative to the site's own row
 __host__ __device__ constexpr int fcc_base_adj(int bs, int k) {
   const int oy = fcc_beta(bs, 1) - 1, oz = fcc_beta(bs, 2) - 1;
@@ -89,7 +98,7 @@ inline bool fcc_build_tables(const Geom& G, FccTables& T) {
       const int dr = cell[1] + 8 * cell[2];
       FccDirEntry& e = T.dir[b][d];
       for (int k = 0; k < 4; ++k)
-        e.d[k] = ((bj ^ k) - b) * FccTile<NT, ROWS>::kSub + (dr + fcc_base_adj(bj, k)) * FccTile<NT, ROWS>::kRow;
+        e.d[k] = FccTile<NT, ROWS>::sub(bj ^ k) - FccTile<NT, ROWS>::sub(b) + (dr + fcc_base_adj(bj, k)) * FccTile<NT, ROWS>::kRow;
       e.e3 = 4 * cell[0];
       e.e2 = 4 * (cell[0] + fcc_beta(bj, 0) - 1);
       e.pad0 = e.pad1 = 0;
@@ -243,9 +252,9 @@ __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4,
   using T = FccTile<NT, ROWS>;
   FccSite si, sj;
   si.p0 = p_own;
-  si.p1 = fcc_at<NT>(p_own, ((b ^ 1) - b) * T::kSub + fcc_base_adj(b, 1) * T::kRow);
-  si.p2 = fcc_at<NT>(p_own, ((b ^ 2) - b) * T::kSub + fcc_base_adj(b, 2) * T::kRow);
-  si.p3 = fcc_at<NT>(p_own, ((b ^ 3) - b) * T::kSub + fcc_base_adj(b, 3) * T::kRow);
+  si.p1 = fcc_at<NT>(p_own, T::sub(b ^ 1) - T::sub(b) + fcc_base_adj(b, 1) * T::kRow);
+  si.p2 = fcc_at<NT>(p_own, T::sub(b ^ 2) - T::sub(b) + fcc_base_adj(b, 2) * T::kRow);
+  si.p3 = fcc_at<NT>(p_own, T::sub(b ^ 3) - T::sub(b) + fcc_base_adj(b, 3) * T::kRow);
   si.a3 = X4 - 4u;
   si.a2 = X4 + (uint32_t)(4 * (fcc_beta(b, 0) - 1));
   sj.p0 = fcc_at<NT>(p_own, E.d[0]);
@@ -292,7 +301,12 @@ __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4,
 }
 
 #ifdef __CUDACC__
-constexpr int kFccMinWarps = 6;
+__device__ __forceinline__ int2 lds_int2(smem_ptr_t addr) {
+  int2 v;
+  asm("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
+  return v;
+}
+constexpr int kFccMinWarps = 10;
 constexpr int kFccSmemMax = 232448 - 1536;                     // 227 KB less the static part / reserve
 // dynamic shared memory: tile windows of `warps` warps, look-up rows, corr, direction table, then the filter tables
 // (accept_words = kFilterWords) or the whole threshold table plus its zero entry (accept_words = len + 1)
@@ -326,8 +340,11 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
   uint32_t* tile = smem_w + warp * (4 * WR * NT) + lane;                       // word (s * WR + row) at tile[(s * WR + row) * NT]
   uint4* s_lut = reinterpret_cast<uint4*>(smem_w + n_warps * (4 * WR * NT));
   int32_t* s_corr = reinterpret_cast<int32_t*>(s_lut + 64 * 3 * rep);
-  FccDirEntry* s_dir = reinterpret_cast<FccDirEntry*>(s_corr + 64);
-  uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_dir + 48);                  // filter tables, or the whole table T + a zero entry
+  // direction table as three arrays of 8-byte entries (row offsets d0, d1; d2, d3; rotation amounts): the twelve entries
+  // of a sublattice lie in 24 different banks, so the lanes of a warp, each with its own direction, never collide (with
+  // 32-byte entries side by side a 16-byte load took 2.3 wavefronts per quarter warp)
+  int2* s_dir = reinterpret_cast<int2*>(s_corr + 64);
+  uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_dir + 3 * 48);              // filter tables, or the whole table T + a zero entry
   __shared__ uint2 s_slot[128];                                                // Philox products that depend on the slot pair only
   __shared__ long long s_e64[kFccWarps];
   __shared__ unsigned s_acc[kFccWarps];
@@ -338,7 +355,12 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
   if (MODE == 2)
     for (int k = threadIdx.x; k <= G.accept_len; k += blockDim.x) s_filt[k] = k < G.accept_len ? accept[k] : 0u;
-  for (int k = threadIdx.x; k < 48; k += blockDim.x) s_dir[k] = FT.dir[k / 12][k % 12];   // 32 bytes each
+  for (int k = threadIdx.x; k < 48; k += blockDim.x) {
+    const FccDirEntry& e = FT.dir[k / 12][k % 12];
+    s_dir[k] = make_int2(e.d[0], e.d[1]);
+    s_dir[48 + k] = make_int2(e.d[2], e.d[3]);
+    s_dir[96 + k] = make_int2(e.e3, e.e2);
+  }
   const uint32_t t = (uint32_t)st->sweep;
   if (threadIdx.x < 128) s_slot[threadIdx.x] = philox_slot_entry(threadIdx.x, t, G.rk0, G.rk1);
   int ox, oy, oz;
@@ -375,11 +397,11 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
       const int t0z = tile_z0(G, oz, cz);
       const int wlo = x0 >> 3, sh = 4 * (x0 & 7);
       const int whi = wlo + 1 == rw ? 0 : wlo + 1;
-      // The tile of a cell is 8 layers of conventional cells, but a trial in layer lz of the cell only touches the tile
-      // layers lz .. lz + 4.  The kernel keeps six layers resident (24 KB per warp instead of 32: eight warps per SM
-      // instead of six) and runs the cell in two halves: tile layers 0..5 for lz = 0, 1; then layer 1 is written back
-      // (layer 0 is never written), layers 2..5 move down two slots, layers 6, 7 are staged, and lz = 2, 3 run on
-      // tile layers 2..7.  Slot of tile layer rz in half h: rz - 2 h.
+      // The tile of a cell is 8 layers of conventional cells, but the trials of layer lz of the cell only touch four
+      // layers of every sublattice (FccTile): the kernel keeps those resident (16 KB per warp: twelve warps per SM) and
+      // runs the cell in four steps.  Between two steps the lowest layer of every window is written back (it is final:
+      // later trials only reach higher layers), the other three move down a slot and one new layer is staged.
+      // Class 1 = sublattices 0, 3 (beta_z = 0, window tile layers lz + 1 .. lz + 4), class 0 = sublattices 1, 2 (lz .. lz + 3).
       uint32_t offy[8];
 #pragma unroll
       for (int ry = 0; ry < 8; ++ry) {
@@ -391,63 +413,43 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
       const uint32_t dwh = (uint32_t)(whi - wlo) * 4u;            // word step from the low to the high group of a row
       uint32_t* const peer = reinterpret_cast<uint32_t*>(G.peer_lat);
       int esum = 0;
-#pragma unroll 1
-      for (int half = 0; half < 2; ++half) {
-        if (half == 1) {
-          // tile layers 2..5 move from slots 2..5 to slots 0..3
-#pragma unroll 1
-          for (int s = 0; s < 4; ++s) {
-            uint32_t* d = tile + s * WR * NT;
-#pragma unroll 8
-            for (int r = 0; r < 32; ++r) d[r * NT] = d[(r + 16) * NT];
-          }
+      // a3: stage tile layer rz of the two sublattices of a class into a slot: per row two 16-byte groups (four
+      // sublattice words each, two of them used), funnel-shifted into the tile words
+      auto stage = [&](auto cls_c, int slot, int rz) {
+        constexpr int CLS = decltype(cls_c)::value;
+        int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
+        const uint32_t zoff = (uint32_t)gz * zstride;
+        uint4 lo[8], hi[8];
+#pragma unroll
+        for (int ry = 0; ry < 8; ++ry) {
+          const uint4* row = reinterpret_cast<const uint4*>(lattice) + (zoff + offy[ry]);
+          lo[ry] = row[wlo];
+          hi[ry] = row[whi];
         }
-        // a3: stage tile layers [0, 6) / [6, 8): per row two 16-byte groups (four sublattice words each), funnel-shifted
-        // into four tile words
-#pragma unroll 1
-        for (int rz = half ? 6 : 0; rz < (half ? 8 : 6); ++rz) {
-          int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
-          const uint32_t zoff = (uint32_t)gz * zstride;
-          uint4 lo[8], hi[8];
 #pragma unroll
-          for (int ry = 0; ry < 8; ++ry) {
-            const uint4* row = reinterpret_cast<const uint4*>(lattice) + (zoff + offy[ry]);
-            lo[ry] = row[wlo];
-            hi[ry] = row[whi];
-          }
-#pragma unroll
-          for (int ry = 0; ry < 8; ++ry) {
-            uint32_t* d = tile + ((rz - 2 * half) * 8 + ry) * NT;
+        for (int ry = 0; ry < 8; ++ry) {
+          uint32_t* d = tile + (slot * 8 + ry) * NT;
+          if (CLS) {
             d[0 * WR * NT] = __funnelshift_r(lo[ry].x, hi[ry].x, sh);
+            d[3 * WR * NT] = __funnelshift_r(lo[ry].w, hi[ry].w, sh);
+          } else {
             d[1 * WR * NT] = __funnelshift_r(lo[ry].y, hi[ry].y, sh);
             d[2 * WR * NT] = __funnelshift_r(lo[ry].z, hi[ry].z, sh);
-            d[3 * WR * NT] = __funnelshift_r(lo[ry].w, hi[ry].w, sh);
           }
         }
-        // a4-a6: 128 of the 256 trials of the cell, raster order: conventional cell c = (lz * 4 + ly) * 4 + lx, then b
+      };
+      // a7: write back rows 1..6 of the layers that leave the windows after step lz - 1 (lz = 4: of everything still
+      // resident), tile layers 1..6 only: the bytes that lie wholly inside this tile
+      auto wb = [&](auto cc, int lz) {
+        constexpr int C = decltype(cc)::value;
 #pragma unroll 1
-        for (int c = 32 * half; c < 32 * half + 32; ++c) {
-          const uint32_t X4 = 4u * (uint32_t)((c & 3) + 2);
-          const int row = ((c >> 2) & 3) + 2 + 8 * ((c >> 4) + 2 - 2 * half);
-          uint32_t* p_row = tile + row * NT;
-          const Philox4 r0 = philox_factored(pc, s_slot[2 * c], G.rk0, G.rk1);
-          const Philox4 r1 = philox_factored(pc, s_slot[2 * c + 1], G.rk0, G.rk1);
-#define SMCX_FCC_TRIAL(B, WDIR, U)                                                                          \
-          {                                                                                                   \
-            const smem_ptr_t ep = dir_p + (B * 12u + mulhi_u32(WDIR, 12u)) * 32u;                            \
-            const int4 e = lds_int4(ep, 0), f = lds_int4(ep, 16);                                             \
-            const FccDirEntry E{{e.x, e.y, e.z, e.w}, f.x, f.y, 0, 0};                                        \
-            fcc_trial<B, NT, MODE, WR>(p_row + B * (WR * NT), X4, E, U, env, esum, nacc);                      \
-          }
-          SMCX_FCC_TRIAL(0, r0.x, r0.y) SMCX_FCC_TRIAL(1, r0.z, r0.w) SMCX_FCC_TRIAL(2, r1.x, r1.y) SMCX_FCC_TRIAL(3, r1.z, r1.w)
-#undef SMCX_FCC_TRIAL
-        }
-        // a7: write back rows 1..6 of tile layer 1 (first half) / of tile layers 2..6 (second half), every sublattice:
-        // the bytes that lie wholly inside this tile
-        auto wb = [&](auto cc) {
-          constexpr int C = decltype(cc)::value;
+        for (int cls = 0; cls < 2; ++cls) {
+          const int first = lz - 1 + cls, n_slots = lz == 4 ? 4 : 1;
+          const int sa = cls ? 0 : 1, sb = cls ? 3 : 2;
 #pragma unroll 1
-          for (int rz = half ? 2 : 1; rz < (half ? 7 : 2); ++rz) {
+          for (int slot = 0; slot < n_slots; ++slot) {
+            const int rz = first + slot;
+            if (rz < 1 || rz > 6) continue;
             int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
             // fused ghost-layer message: layers the neighbour slab holds a copy of also go into its storage
             const bool mirror = peer != nullptr && gz >= G.peer_z0 && gz < G.peer_z1;
@@ -455,28 +457,69 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
             for (int ry = 1; ry < 7; ++ry) {
               const uint32_t base = (((uint32_t)gz * zstride) + offy[ry] + (uint32_t)wlo) * 4u;
 #pragma unroll
-              for (int s = 0; s < 4; ++s) {
-                const uint32_t v = tile[(s * WR + (rz - 2 * half) * 8 + ry) * NT];
-                store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(lattice + base + s),
-                                                     reinterpret_cast<unsigned char*>(lattice + (uint32_t)(base + s + dwh)), v);
+              for (int q = 0; q < 2; ++q) {
+                const int sq = q ? sb : sa;
+                const uint32_t v = tile[(sq * WR + slot * 8 + ry) * NT];
+                store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(lattice + base + sq),
+                                                     reinterpret_cast<unsigned char*>(lattice + (uint32_t)(base + sq + dwh)), v);
                 if (mirror)
-                  store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(peer + base + s),
-                                                       reinterpret_cast<unsigned char*>(peer + (uint32_t)(base + s + dwh)), v);
+                  store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(peer + base + sq),
+                                                       reinterpret_cast<unsigned char*>(peer + (uint32_t)(base + sq + dwh)), v);
               }
             }
           }
-        };
+        }
+      };
+      auto write_back = [&](int lz) {
         switch (x0 & 7) {
-          case 0: wb(std::integral_constant<int, 0>{}); break;
-          case 1: wb(std::integral_constant<int, 1>{}); break;
-          case 2: wb(std::integral_constant<int, 2>{}); break;
-          case 3: wb(std::integral_constant<int, 3>{}); break;
-          case 4: wb(std::integral_constant<int, 4>{}); break;
-          case 5: wb(std::integral_constant<int, 5>{}); break;
-          case 6: wb(std::integral_constant<int, 6>{}); break;
-          default: wb(std::integral_constant<int, 7>{}); break;
+          case 0: wb(std::integral_constant<int, 0>{}, lz); break;
+          case 1: wb(std::integral_constant<int, 1>{}, lz); break;
+          case 2: wb(std::integral_constant<int, 2>{}, lz); break;
+          case 3: wb(std::integral_constant<int, 3>{}, lz); break;
+          case 4: wb(std::integral_constant<int, 4>{}, lz); break;
+          case 5: wb(std::integral_constant<int, 5>{}, lz); break;
+          case 6: wb(std::integral_constant<int, 6>{}, lz); break;
+          default: wb(std::integral_constant<int, 7>{}, lz); break;
+        }
+      };
+#pragma unroll 1
+      for (int lz = 0; lz < 4; ++lz) {
+        if (lz > 0) {
+          write_back(lz);
+          // slots 1..3 of every sublattice move down one slot
+#pragma unroll 1
+          for (int s = 0; s < 4; ++s) {
+            uint32_t* d = tile + s * WR * NT;
+#pragma unroll 8
+            for (int r = 0; r < 24; ++r) d[r * NT] = d[(r + 8) * NT];
+          }
+        }
+#pragma unroll 1
+        for (int slot = lz ? 3 : 0; slot < 4; ++slot) {
+          stage(std::integral_constant<int, 0>{}, slot, lz + slot);
+          stage(std::integral_constant<int, 1>{}, slot, lz + 1 + slot);
+        }
+        // a4-a6: the 64 trials of layer lz of the cell, raster order: conventional cell c = (lz * 4 + ly) * 4 + lx, then b;
+        // site i sits in (virtual) slot 2 of its sublattice's window
+        using TW = FccTile<NT, WR>;
+#pragma unroll 1
+        for (int c = 16 * lz; c < 16 * lz + 16; ++c) {
+          const uint32_t X4 = 4u * (uint32_t)((c & 3) + 2);
+          uint32_t* p_row = tile + (((c >> 2) & 3) + 2 + 16) * NT;
+          const Philox4 r0 = philox_factored(pc, s_slot[2 * c], G.rk0, G.rk1);
+          const Philox4 r1 = philox_factored(pc, s_slot[2 * c + 1], G.rk0, G.rk1);
+#define SMCX_FCC_TRIAL(B, WDIR, U)                                                                          \
+          {                                                                                                   \
+            const smem_ptr_t ep = dir_p + (B * 12u + mulhi_u32(WDIR, 12u)) * 8u;                             \
+            const int2 e = lds_int2(ep), g = lds_int2(ep + 48u * 8u), f = lds_int2(ep + 96u * 8u);            \
+            const FccDirEntry E{{e.x, e.y, g.x, g.y}, f.x, f.y, 0, 0};                                        \
+            fcc_trial<B, NT, MODE, WR>(const_cast<uint32_t*>(fcc_at<NT>(p_row, TW::sub(B))), X4, E, U, env, esum, nacc); \
+          }
+          SMCX_FCC_TRIAL(0, r0.x, r0.y) SMCX_FCC_TRIAL(1, r0.z, r0.w) SMCX_FCC_TRIAL(2, r1.x, r1.y) SMCX_FCC_TRIAL(3, r1.z, r1.w)
+#undef SMCX_FCC_TRIAL
         }
       }
+      write_back(4);
       esum_total += esum;     // |dE| < 2^23 (host check), 256 trials: exact in int32 per cell
     }
   }
@@ -512,7 +555,7 @@ inline int launch_fcc_thread(const Geom& G, const FccTables& FT, uint32_t* latti
                              int rep, const uint32_t* accept, const uint32_t* d_filter, DevState* st, int colour, int sm_count,
                              cudaStream_t stream) {
   const unsigned n_batches = (G.cells_per_colour + 31u) / 32u;
-  // the whole threshold table in shared memory when it fits next to at least five warps of tiles, else the filter
+  // the whole threshold table in shared memory when it fits next to at least kFccMinWarps warps of tiles, else the filter
   const int direct = fcc_direct_warps(rep, G.accept_len);
   const int warps = direct > 0 ? direct : kFccWarps;
   const unsigned want = (n_batches + warps - 1) / warps;
