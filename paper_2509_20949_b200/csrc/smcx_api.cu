@@ -99,6 +99,7 @@ struct Plan {
   int coef_class;   // build_thread_coefficients: 2 = the filter variant of the thread kernel applies
   bool coef_packed; // pack_thread_coefficients: the 16-bit coefficient rows are exact
   int fcc_rep;      // sweep_fcc_thread: replicas of the look-up rows in shared memory
+  int accept_tail_from = 0;   // T[k] >= T[d] for every d > k holds for all k >= this (0 for a table that never increases)
   FccTables fcc_tables;
   Bcc4Tables bcc4_tables;
   Layout lay;
@@ -380,7 +381,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   L.utab = off;    off += align_up((size_t)G.B * G.Z0 * G.n_shells * plan->local_umax * sizeof(LocalUEntry), 256);
   L.ucount = off;  off += align_up(local ? (size_t)G.B * G.Z0 * G.n_shells * sizeof(int) : 0, 256);
   if (local && local_smem_bytes(G, plan->local_umax) > 227 * 1024) return SMCX_E_LINK_CELL_TOO_SMALL;
-  L.accept = off;  off += align_up((size_t)kAcceptCapacity * sizeof(uint32_t), 256);
+  L.accept = off;  off += align_up(((size_t)kAcceptCapacity + 1) * sizeof(uint32_t), 256);   // T and the zero entry behind it
   L.filter = off;  off += align_up((size_t)kFilterWords * sizeof(uint32_t), 256);
   L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
   L.state = off;   off += align_up(sizeof(DevState), 256);
@@ -638,12 +639,21 @@ int upload_table(smcx* h, const uint32_t* accept, int len) {
   h->staging_next = (slot + 1) % kStagingSlots;
   SMCX_CUDA(h, cudaEventSynchronize(h->staging_ev[slot]));
   std::memcpy(h->staging[slot], accept, (size_t)len * sizeof(uint32_t));
-  SMCX_CUDA(h, cudaMemcpyAsync(h->d_accept(), h->staging[slot], (size_t)len * sizeof(uint32_t),
+  h->staging[slot][len] = 0u;    // dE >= len is a rejection (S5): kernels that clamp dE to len read this entry
+  {
+    // the table is input data and need not be monotone: from which entry on does T[k] bound everything behind it
+    // (what sweep_fcc_thread<2> relies on when it holds only the head of T in shared memory)
+    int m = len;
+    uint32_t run_max = 0u;
+    while (m > 0 && accept[m - 1] >= run_max) { run_max = accept[m - 1]; --m; }
+    h->plan.accept_tail_from = m;
+  }
+  SMCX_CUDA(h, cudaMemcpyAsync(h->d_accept(), h->staging[slot], ((size_t)len + 1) * sizeof(uint32_t),
                                cudaMemcpyHostToDevice, h->stream));
   h->plan.G.filter_E = -1;
   h->plan.G.filter_nq = 0;
   if (uses_filter(h->plan)) {
-    uint32_t* filt = h->staging[slot] + kAcceptCapacity;
+    uint32_t* filt = h->staging[slot] + kAcceptCapacity + 1;
     int nq = 0;
     const int E = build_accept_filter(accept, len, filt, &nq);
     if (E >= 0) {
@@ -693,7 +703,7 @@ int launch_colour_pass(smcx* h, const Geom& G, int colour) {
   }
   if (P.kernel == SMCX_KERNEL_FCC_THREAD) {
     const int rc = launch_fcc_thread(G, P.fcc_tables, reinterpret_cast<uint32_t*>(h->d_species()), h->d_fcc_lut(), h->d_fcc_corr(),
-                                     P.fcc_rep, h->d_accept(), h->d_filter(), h->d_state(), colour, h->sm_count, h->stream);
+                                     P.fcc_rep, h->d_accept(), h->d_filter(), h->d_state(), colour, h->sm_count, P.accept_tail_from, h->stream);
     h->launches++;
     if (rc != 0) { h->err = "packed FCC thread-per-cell launch failed"; return SMCX_E_CUDA; }
     return SMCX_OK;
@@ -823,7 +833,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     h->ws = reinterpret_cast<char*>(ws);
     h->owns_ws = true;
   }
-  h->staging_cap = ((size_t)kAcceptCapacity + kFilterWords) * sizeof(uint32_t);
+  h->staging_cap = ((size_t)kAcceptCapacity + 1 + kFilterWords) * sizeof(uint32_t);
   for (int s = 0; s < kStagingSlots; ++s) {
     if (cudaMallocHost(reinterpret_cast<void**>(&h->staging[s]), h->staging_cap) != cudaSuccess) return fail(SMCX_E_NO_MEMORY);
     if (cudaEventCreateWithFlags(&h->staging_ev[s], cudaEventDisableTiming) != cudaSuccess) return fail(SMCX_E_CUDA);

@@ -235,6 +235,7 @@ struct FccEnv {
   uint32_t lut_shell_bytes;  // bytes from one shell to the next = rep * 16
   const uint32_t* accept;
   int accept_len, filter_E;
+  int direct_len;            // MODE 2: entries of T held in shared memory at filt (followed by one bound entry)
 };
 
 __host__ __device__ __forceinline__ FccLut fcc_load_lut(smem_ptr_t p) {
@@ -245,7 +246,9 @@ __host__ __device__ __forceinline__ FccLut fcc_load_lut(smem_ptr_t p) {
 // One trial (a4-a6).  p_own: row r of sublattice b in this lane's tile; X4 = 4 X, X the nibble of site i; E = the
 // direction-table entry of (b, drawn direction); u = acceptance draw.
 // MODE (acceptance): 0 = T[dE] from global memory, 1 = two-level filter in shared memory (exact look-up in global memory
-// when u falls within E of the bound), 2 = the whole table T, followed by one zero entry, in shared memory at env.filt.
+// when u falls within E of the bound), 2 = the first direct_len entries of T in shared memory at env.filt, followed by
+// the bound T[direct_len] (0 when that is the whole table): T does not increase, so for dE >= direct_len a draw
+// u >= T[direct_len] is a rejection and only a smaller one (rare: T[direct_len] is small) needs T[dE] from global memory.
 template <int b, int NT, int MODE, int ROWS = kFccRows>
 __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4, const FccDirEntry& E, uint32_t u,
                                                    const FccEnv& env, int& esum, unsigned& nacc) {
@@ -276,9 +279,18 @@ __host__ __device__ __forceinline__ void fcc_trial(uint32_t* p_own, uint32_t X4,
   // Eq. 3 in integer form
   bool ok;
   if (MODE == 2) {
-    // dE <= 0 (huge as unsigned) and dE >= len clamp to the zero entry behind the table: decided by the sign test alone
-    const uint32_t i4 = 4u * min((uint32_t)dE, (uint32_t)env.accept_len);
-    ok = dE <= 0 || u < lds_u32(env.filt, i4);
+    // dE <= 0 (huge as unsigned) and dE >= direct_len clamp to the bound entry behind the table
+    uint32_t thr = lds_u32(env.filt, 4u * min((uint32_t)dE, (uint32_t)env.direct_len));
+    // beyond the resident part: T[dE] itself, by a predicated load (no branch: the trial stays one basic block); the
+    // library keeps a zero entry behind T in device memory, which serves dE >= len
+    const bool far = dE >= env.direct_len && u < thr;
+    const uint32_t* tp = env.accept + min(dE, env.accept_len);
+#ifdef __CUDA_ARCH__
+    asm("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p ld.global.nc.u32 %0, [%1]; }" : "+r"(thr) : "l"(tp), "r"((uint32_t)far));
+#else
+    if (far) thr = *tp;
+#endif
+    ok = dE <= 0 || u < thr;
   } else if (MODE == 1) {
     const uint32_t dc = (uint32_t)min(max(dE, 0), kFilterDmax);
     const uint32_t ta = mulhi_u32(lds_u32(env.filt, 4u * (kFilterTr + (dc >> 6))), lds_u32(env.filt, 4u * (dc & 63u)));
@@ -306,7 +318,6 @@ __device__ __forceinline__ int2 lds_int2(smem_ptr_t addr) {
   asm("ld.shared.v2.s32 {%0, %1}, [%2];" : "=r"(v.x), "=r"(v.y) : "r"(addr));
   return v;
 }
-constexpr int kFccMinWarps = 10;
 constexpr int kFccSmemMax = 232448 - 1536;                     // 227 KB less the static part / reserve
 // dynamic shared memory: tile windows of `warps` warps, look-up rows, corr, direction table, then the filter tables
 // (accept_words = kFilterWords) or the whole threshold table plus its zero entry (accept_words = len + 1)
@@ -320,19 +331,27 @@ inline int fcc_lut_rep(int n_species) {
     if (fcc_smem_bytes(rep) <= (size_t)kFccSmemMax) return rep;
   return 1;
 }
-// Warps per block with which the whole threshold table fits shared memory (8 .. 5; the kernel runs as fast with six
-// warps as with eight), or 0: then the two-level filter serves.
-inline int fcc_direct_warps(int rep, int accept_len) {
-  for (int w = kFccWarps; w >= kFccMinWarps; --w)
-    if (fcc_smem_bytes(rep, w, (size_t)accept_len + 1) <= (size_t)kFccSmemMax) return w;
-  return 0;
+// Acceptance from the table itself (MODE 2) when at least kFccDirectMin of its entries fit shared memory next to
+// kFccDirectWarps warps of tiles (beyond them T is small and the exact look-up in global memory rare); measured on
+// FCC 640^3: the table next to 10 / 9 / 8 / 7 warps 7.87 / 7.65 / 7.42 / 7.04e10 against 7.50e10 with the two-level
+// filter and twelve warps.  Returns the number of entries to hold (<= accept_len), or 0: then the filter serves.
+constexpr int kFccDirectWarps = 11;
+constexpr int kFccDirectMin = 4096;
+inline int fcc_direct_entries(int rep, int accept_len, int* warps) {
+  if (fcc_smem_bytes(rep, kFccWarps, (size_t)accept_len + 1) <= (size_t)kFccSmemMax) { *warps = kFccWarps; return accept_len; }
+  *warps = kFccDirectWarps;
+  const size_t fixed = fcc_smem_bytes(rep, kFccDirectWarps, 1);
+  if (fixed > (size_t)kFccSmemMax) return 0;
+  const size_t room = ((size_t)kFccSmemMax - fixed) / 4;
+  if (room >= (size_t)accept_len) return accept_len;
+  return room >= (size_t)kFccDirectMin ? (int)room : 0;
 }
 
 template <int MODE>
 __global__ void __launch_bounds__(kFccWarps * 32, 1)
 sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattice, const uint4* __restrict__ lut,
                  const int32_t* __restrict__ corr, int rep, const uint32_t* __restrict__ accept,
-                 const uint32_t* __restrict__ filt, DevState* __restrict__ st, int colour) {
+                 const uint32_t* __restrict__ filt, DevState* __restrict__ st, int colour, int direct_len) {
   constexpr int NT = 32;
   extern __shared__ __align__(16) uint32_t smem_w[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31, n_warps = blockDim.x >> 5;
@@ -354,7 +373,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
   if (MODE == 1)
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
   if (MODE == 2)
-    for (int k = threadIdx.x; k <= G.accept_len; k += blockDim.x) s_filt[k] = k < G.accept_len ? accept[k] : 0u;
+    for (int k = threadIdx.x; k <= direct_len; k += blockDim.x) s_filt[k] = k < G.accept_len ? accept[k] : 0u;
   for (int k = threadIdx.x; k < 48; k += blockDim.x) {
     const FccDirEntry& e = FT.dir[k / 12][k % 12];
     s_dir[k] = make_int2(e.d[0], e.d[1]);
@@ -375,6 +394,7 @@ sweep_fcc_thread(const Geom G, const FccTables FT, uint32_t* __restrict__ lattic
   env.accept = accept;
   env.accept_len = G.accept_len;
   env.filter_E = G.filter_E;
+  env.direct_len = direct_len;
   const smem_ptr_t dir_p = smem_ptr(s_dir);
   const int rw = G.Lx >> 3;                                     // groups of 8 cells per lattice row
   const uint32_t zstride = (uint32_t)G.Ly * (uint32_t)rw;
@@ -553,21 +573,23 @@ inline int configure_fcc_thread(int rep) {
 
 inline int launch_fcc_thread(const Geom& G, const FccTables& FT, uint32_t* lattice, const uint32_t* d_lut, const int32_t* d_corr,
                              int rep, const uint32_t* accept, const uint32_t* d_filter, DevState* st, int colour, int sm_count,
-                             cudaStream_t stream) {
+                             int tail_from, cudaStream_t stream) {
   const unsigned n_batches = (G.cells_per_colour + 31u) / 32u;
-  // the whole threshold table in shared memory when it fits next to at least kFccMinWarps warps of tiles, else the filter
-  const int direct = fcc_direct_warps(rep, G.accept_len);
-  const int warps = direct > 0 ? direct : kFccWarps;
+  int warps = kFccWarps;
+  int direct = fcc_direct_entries(rep, G.accept_len, &warps);
+  // the head of T only: sound if T[direct] bounds every later entry (tail_from: checked by the host at upload)
+  if (direct < G.accept_len && direct < tail_from) direct = 0;
+  if (direct == 0) warps = kFccWarps;
   const unsigned want = (n_batches + warps - 1) / warps;
   const unsigned grid = want < (unsigned)sm_count ? want : (unsigned)sm_count;
   const uint4* lut4 = reinterpret_cast<const uint4*>(d_lut);
   if (direct > 0)
-    sweep_fcc_thread<2><<<grid, warps * 32, fcc_smem_bytes(rep, warps, (size_t)G.accept_len + 1), stream>>>(
-        G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour);
+    sweep_fcc_thread<2><<<grid, warps * 32, fcc_smem_bytes(rep, warps, (size_t)direct + 1), stream>>>(
+        G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour, direct);
   else if (G.filter_E >= 0)
-    sweep_fcc_thread<1><<<grid, warps * 32, fcc_smem_bytes(rep), stream>>>(G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour);
+    sweep_fcc_thread<1><<<grid, warps * 32, fcc_smem_bytes(rep), stream>>>(G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour, 0);
   else
-    sweep_fcc_thread<0><<<grid, warps * 32, fcc_smem_bytes(rep), stream>>>(G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour);
+    sweep_fcc_thread<0><<<grid, warps * 32, fcc_smem_bytes(rep), stream>>>(G, FT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour, 0);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 #endif  // __CUDACC__

@@ -55,7 +55,7 @@ static long long local_energy(const uint32_t* tile, int n_shells, const int p[3]
   return e;
 }
 
-template <bool F>
+template <int F>
 static void run_trial(int b, uint32_t* p_own, uint32_t X4, const FccDirEntry& E, uint32_t u, const FccEnv& env, int& es, unsigned& na) {
   switch (b) {
     case 0: fcc_trial<0, 1, F>(p_own, X4, E, u, env, es, na); break;
@@ -98,7 +98,13 @@ int main() {
     FccEnv env;
     env.lut = smem_ptr(lut_p) + (rep % lrep) * 16; env.corr = smem_ptr(corr.data()); env.filt = smem_ptr(filt);
     env.lut_pair_bytes = 3u * lrep * 16u; env.lut_shell_bytes = lrep * 16u;
-    env.accept = T.data(); env.accept_len = len; env.filter_E = Ef;
+    env.accept = T.data(); env.accept_len = len; env.filter_E = Ef; env.direct_len = 0;
+    // MODE 2: the first K entries of T and the bound T[K] in "shared memory" (K = len: the whole table and a zero)
+    const int K = rep % 3 == 0 ? len : 1 + (int)(rng() % (uint32_t)len);
+    std::vector<uint32_t> direct((size_t)K + 1);
+    for (int d = 0; d <= K; ++d) direct[d] = d < len ? T[d] : 0u;
+    FccEnv env2 = env;
+    env2.filt = smem_ptr(direct.data()); env2.direct_len = K;
     uint32_t tile[256];
     for (auto& w : tile) { w = 0; for (int f = 0; f < 8; ++f) w |= (uint32_t)(rng() % nsp) << (4 * f); }
     for (int it = 0; it < 3000; ++it) {
@@ -122,12 +128,13 @@ int main() {
         okref = dEref <= 0 || (dEref < len && u < T[dEref]);
         if (!okref) memcpy(ref, tile, sizeof(tile));
       } else if (it % 3 == 0) u = rng() % 4;
-      for (int variant = 0; variant < 2; ++variant) {
+      for (int variant = 0; variant < 3; ++variant) {
         uint32_t got[256]; memcpy(got, tile, sizeof(tile));
         int es = 0; unsigned na = 0;
         uint32_t* p_own = got + b * 64 + y + 8 * z;
-        if (variant == 0) run_trial<true>(b, p_own, 4u * X, FT.dir[b][dir], u, env, es, na);
-        else run_trial<false>(b, p_own, 4u * X, FT.dir[b][dir], u, env, es, na);
+        if (variant == 0) run_trial<1>(b, p_own, 4u * X, FT.dir[b][dir], u, env, es, na);
+        else if (variant == 1) run_trial<0>(b, p_own, 4u * X, FT.dir[b][dir], u, env, es, na);
+        else run_trial<2>(b, p_own, 4u * X, FT.dir[b][dir], u, env2, es, na);
         const bool same = memcmp(got, ref, sizeof(ref)) == 0;
         if (!same || na != (okref ? 1u : 0u) || es != (okref ? (int)dEref : 0)) {
           if (bad < 10) printf("MISMATCH variant %d b %d X %d y %d z %d dir %d a %d b %d dEref %lld okref %d got es %d na %u same %d u %u nsp %d shells %d\n",

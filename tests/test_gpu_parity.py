@@ -497,6 +497,42 @@ def test_packed_fcc_kernel_against_the_oracle(dims, n_sp, n_sh, amp, kT):
     _assert_sro(g, o)                              # pair counts on 4-bit storage
 
 
+@pytest.mark.parametrize("kind", ["staircase", "short", "non_monotone", "bump_in_the_tail", "tiny_kT"])
+def test_packed_fcc_kernel_arbitrary_threshold_tables(kind):
+    """The packed FCC kernel keeps the head of T in shared memory and takes T[dE] from global memory behind it, which
+    is sound only if T[K] bounds the tail (the host checks that at upload): tables that are not of the exp(-d/kT) form
+    must give the oracle's decisions all the same -- a staircase (never increases: head in shared memory), one that fits
+    shared memory whole, a random one (no bound: the kernel must fall back to the plain look-up), one that increases
+    once far out in the tail, and one so short that every positive dE is beyond it."""
+    lat, dims, n_sp, n_sh, w, seed = 1, (16, 16, 24), 5, 3, 4, 808
+    epi = make_epi(n_sh, n_sp, 400, seed)
+    rng = np.random.default_rng(12)
+    if kind == "staircase":
+        table = np.repeat(np.sort(rng.integers(0, 2 ** 32, 50, dtype=np.uint64))[::-1], 200).astype(np.uint32)   # 10,000 entries
+    elif kind == "short":
+        table = make_accept_table(860)[:3000].copy()        # ends at exp(-3.5): dE >= 3000 is always rejected
+    elif kind == "non_monotone":
+        table = rng.integers(0, 2 ** 32, 9000, dtype=np.uint64).astype(np.uint32)
+    elif kind == "bump_in_the_tail":
+        table = make_accept_table(860).copy()
+        table[7000:7040] = 2 ** 31                          # beyond the resident head, far above T[K]
+    else:
+        table = make_accept_table(1)                        # 24 entries
+    g = smcx.Lattice(lat, dims, n_sp, n_sh, epi, table, seed, link_cell=w, kT_units=860, kernel=smcx.KERNEL_FCC_THREAD)
+    o = oracle.Oracle(lat, dims, n_sp, n_sh, epi, w, table, seed)
+    g.sweep(3)
+    o.sweep(3)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all() and g.stats() == o.stats()
+    table2 = make_accept_table(1720)                        # and on to a regular long table on the same handles
+    g.set_temperature(1720, table2)
+    o.set_temperature(table2)
+    g.sweep(2)
+    o.sweep(2)
+    _assert_same_state(g, o)
+    assert (g.energy_trace() == o.energy_trace()).all() and g.stats() == o.stats() and g.stats()[2] > 0
+
+
 def test_p14_four_bit_and_uint8_storage_agree():
     """P14: SMCX_STORAGE_4BIT (packed FCC kernel) and SMCX_STORAGE_U8 (sub-warp and warp kernels) give identical
     smcx_species, traces and pair counts, on the paper's composition with stage-wise cooling."""
