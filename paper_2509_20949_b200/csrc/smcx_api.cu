@@ -277,7 +277,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   if (bcc4_ok) {
     std::vector<uint32_t> lut;
     std::vector<int32_t> corr;
-    bcc4_ok = fcc_build_lut(p->epi, n, p->n_shells, 1, lut, corr) && bcc4_build_tables<32>(G, plan->bcc4_tables);
+    bcc4_ok = fcc_build_lut(p->epi, n, p->n_shells, 1, lut, corr) && bcc4_build_tables<32, kBcc4WinRows>(G, plan->bcc4_tables);
   }
   int kernel = p->kernel, storage = p->storage;
   if (local) bcc4_ok = false;
@@ -710,7 +710,7 @@ int launch_colour_pass(smcx* h, const Geom& G, int colour) {
   }
   if (P.kernel == SMCX_KERNEL_BCC4_THREAD) {
     const int rc = launch_bcc4_thread(G, P.bcc4_tables, reinterpret_cast<uint32_t*>(h->d_species()), h->d_fcc_lut(), h->d_fcc_corr(),
-                                      P.fcc_rep, h->d_accept(), h->d_filter(), h->d_state(), colour, h->sm_count, h->stream);
+                                      P.fcc_rep, h->d_accept(), h->d_filter(), h->d_state(), colour, h->sm_count, P.accept_tail_from, h->stream);
     h->launches++;
     if (rc != 0) { h->err = "packed BCC (4-bit) thread-per-cell launch failed"; return SMCX_E_CUDA; }
     return SMCX_OK;

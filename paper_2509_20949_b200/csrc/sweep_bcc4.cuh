@@ -26,12 +26,18 @@
 
 namespace smcxk {
 
-constexpr int kBcc4Warps = 12;                // 12 x 16 KB of tiles + tables in 227 KB
-constexpr int kBcc4Rows = 64;                 // rows (y + 8 z) per sublattice of a tile
+constexpr int kBcc4Warps = 20;                // 20 x 8 KB of tile windows + tables + the head of T in 227 KB
+constexpr int kBcc4Rows = 64;                 // rows (y + 8 z) per sublattice of a whole tile (8 layers)
+constexpr int kBcc4WinRows = 32;              // the kernel keeps four layers per sublattice resident
 
-template <int NT> struct Bcc4Tile {
+// ROWS = 64: the whole tile.  ROWS < 64 (the kernel's window): the trials of layer lz of the cell (tile layer lz + 2)
+// reach three half-units up and down, i.e. tile layers lz + 1 .. lz + 4 of the corner sublattice and lz .. lz + 3 of
+// the centre sublattice; sublattice s keeps tile layer rz in slot rz - lz - (1 - s), which the row pointers of the
+// gather see as a constant offset per sublattice (sub()), exactly as in sweep_fcc.cuh.
+template <int NT, int ROWS = kBcc4Rows> struct Bcc4Tile {
   static constexpr int kRow = 4 * NT;                 // bytes from one row to the next (NT lanes interleaved)
-  static constexpr int kSub = kBcc4Rows * kRow;       // bytes from one sublattice to the other
+  static constexpr int kSub = ROWS * kRow;            // bytes from one sublattice to the other
+  __host__ __device__ static constexpr int sub(int s) { return s * kSub - (ROWS < kBcc4Rows ? (1 - s) * 8 * kRow : 0); }
 };
 
 // Direction table, [b][dir] (dir = dx | dy << 1 | dz << 2, S0's order of the eight nearest neighbours): byte offsets from
@@ -40,8 +46,9 @@ template <int NT> struct Bcc4Tile {
 struct Bcc4DirEntry { int32_t d0, d1, e3, e2; };
 struct Bcc4Tables { Bcc4DirEntry dir[2][8]; };
 
-template <int NT>
+template <int NT, int ROWS = kBcc4Rows>
 inline bool bcc4_build_tables(const Geom& G, Bcc4Tables& T) {
+  using TL = Bcc4Tile<NT, ROWS>;
   if (G.Z0 != 8) return false;
   for (int b = 0; b < 2; ++b)
     for (int d = 0; d < 8; ++d) {
@@ -55,8 +62,8 @@ inline bool bcc4_build_tables(const Geom& G, Bcc4Tables& T) {
       const int bj = 1 - b, oj = bj - 1;
       const int dr = cell[1] + 8 * cell[2];
       Bcc4DirEntry& e = T.dir[b][d];
-      e.d0 = (bj - b) * Bcc4Tile<NT>::kSub + dr * Bcc4Tile<NT>::kRow;
-      e.d1 = (dr + oj + 8 * oj) * Bcc4Tile<NT>::kRow;  // back on i's sublattice: (b - b) * kSub = 0
+      e.d0 = TL::sub(bj) - TL::sub(b) + dr * TL::kRow;
+      e.d1 = (dr + oj + 8 * oj) * TL::kRow;            // back on i's sublattice
       e.e3 = 4 * cell[0];
       e.e2 = 4 * (cell[0] + oj);
     }
@@ -97,15 +104,16 @@ __host__ __device__ __forceinline__ void bcc4_site_sum(const Bcc4Site& S, uint32
 }
 
 // One trial (a4-a6).  p_own: row r of sublattice b in this lane's tile; X4 = 4 X, X the nibble of site i; E = the
-// direction-table entry of (b, drawn direction); u = acceptance draw.  MODE as in fcc_trial (0 global, 1 filter).
-template <int b, int NT, int MODE>
+// direction-table entry of (b, drawn direction); u = acceptance draw.  MODE as in fcc_trial (0 global, 1 filter, 2 head
+// of the table in shared memory).
+template <int b, int NT, int MODE, int ROWS = kBcc4Rows>
 __host__ __device__ __forceinline__ void bcc4_trial(uint32_t* p_own, uint32_t X4, const Bcc4DirEntry& E, uint32_t u,
                                                     const FccEnv& env, int& esum, unsigned& nacc) {
-  using T = Bcc4Tile<NT>;
+  using T = Bcc4Tile<NT, ROWS>;
   constexpr int o = b - 1;
   Bcc4Site si, sj;
   si.p0 = p_own;
-  si.p1 = fcc_at<NT>(p_own, ((1 - b) - b) * T::kSub + (o + 8 * o) * T::kRow);
+  si.p1 = fcc_at<NT>(p_own, T::sub(1 - b) - T::sub(b) + (o + 8 * o) * T::kRow);
   si.a3 = X4 - 4u;
   si.a2 = X4 + (uint32_t)(4 * o);
   sj.p0 = fcc_at<NT>(p_own, E.d0);
@@ -123,7 +131,19 @@ __host__ __device__ __forceinline__ void bcc4_trial(uint32_t* p_own, uint32_t X4
   bcc4_site_sum<NT>(sj, own_j, L0, L1, lo_j, hi_j);
   const int dE = (int)(lo_i - lo_j) + 256 * (int)(hi_i - hi_j) + corr;
   bool ok;
-  if (MODE == 1) {
+  if (MODE == 2) {
+    // as sweep_fcc_thread<2>: the head of T in shared memory followed by the bound T[direct_len]; behind it T[dE] itself
+    // by a predicated load (the library keeps a zero entry behind T in device memory, which serves dE >= len)
+    uint32_t thr = lds_u32(env.filt, 4u * min((uint32_t)dE, (uint32_t)env.direct_len));
+    const bool far = dE >= env.direct_len && u < thr;
+    const uint32_t* tp = env.accept + min(dE, env.accept_len);
+#ifdef __CUDA_ARCH__
+    asm("{ .reg .pred p; setp.ne.u32 p, %2, 0; @p ld.global.nc.u32 %0, [%1]; }" : "+r"(thr) : "l"(tp), "r"((uint32_t)far));
+#else
+    if (far) thr = *tp;
+#endif
+    ok = dE <= 0 || u < thr;
+  } else if (MODE == 1) {
     const uint32_t dc = (uint32_t)min(max(dE, 0), kFilterDmax);
     const uint32_t ta = mulhi_u32(lds_u32(env.filt, 4u * (kFilterTr + (dc >> 6))), lds_u32(env.filt, 4u * (dc & 63u)));
     ok = u < ta;
@@ -146,29 +166,41 @@ __host__ __device__ __forceinline__ void bcc4_trial(uint32_t* p_own, uint32_t X4
 
 
 #ifdef __CUDACC__
-inline size_t bcc4_smem_bytes(int rep) {
-  return (size_t)kBcc4Warps * Bcc4Tile<32>::kSub * 2 + (size_t)64 * 3 * rep * 16 + 64 * 4 + sizeof(Bcc4Tables) + kFilterWords * 4;
+constexpr int kBcc4SmemMax = 232448 - 1024;                    // 227 KB less the static part
+// dynamic shared memory: tile windows, look-up rows, corr, direction table, then the filter tables (accept_words =
+// kFilterWords) or the head of the threshold table plus its bound entry
+inline size_t bcc4_smem_bytes(int rep, size_t accept_words = kFilterWords) {
+  return (size_t)kBcc4Warps * Bcc4Tile<32, kBcc4WinRows>::kSub * 2 + (size_t)64 * 3 * rep * 16 + 64 * 4 + sizeof(Bcc4Tables) + accept_words * 4;
 }
 inline int bcc4_lut_rep() {
   for (int rep = 8; rep >= 1; rep >>= 1)
-    if (bcc4_smem_bytes(rep) + 2560 <= 227 * 1024) return rep;
+    if (bcc4_smem_bytes(rep) <= (size_t)kBcc4SmemMax) return rep;
   return 1;
+}
+// entries of T to hold in shared memory (sweep_bcc4_thread<2>), or 0: too few fit
+constexpr int kBcc4DirectMin = 4096;
+inline int bcc4_direct_entries(int rep, int accept_len) {
+  const size_t fixed = bcc4_smem_bytes(rep, 1);
+  if (fixed > (size_t)kBcc4SmemMax) return 0;
+  const size_t room = ((size_t)kBcc4SmemMax - fixed) / 4;
+  if (room >= (size_t)accept_len) return accept_len;
+  return room >= (size_t)kBcc4DirectMin ? (int)room : 0;
 }
 
 template <int MODE>
 __global__ void __launch_bounds__(kBcc4Warps * 32, 1)
 sweep_bcc4_thread(const Geom G, const Bcc4Tables BT, uint32_t* __restrict__ lattice, const uint4* __restrict__ lut,
                   const int32_t* __restrict__ corr, int rep, const uint32_t* __restrict__ accept,
-                  const uint32_t* __restrict__ filt, DevState* __restrict__ st, int colour) {
+                  const uint32_t* __restrict__ filt, DevState* __restrict__ st, int colour, int direct_len) {
   constexpr int NT = 32;
-  constexpr int R = kBcc4Rows;
+  constexpr int WR = kBcc4WinRows;
   extern __shared__ __align__(16) uint32_t smem_w[];
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  uint32_t* tile = smem_w + warp * (2 * R * NT) + lane;                        // word (s * 64 + row) at tile[(s * 64 + row) * NT]
-  uint4* s_lut = reinterpret_cast<uint4*>(smem_w + kBcc4Warps * (2 * R * NT));
+  uint32_t* tile = smem_w + warp * (2 * WR * NT) + lane;                       // word (s * WR + row) at tile[(s * WR + row) * NT]
+  uint4* s_lut = reinterpret_cast<uint4*>(smem_w + kBcc4Warps * (2 * WR * NT));
   int32_t* s_corr = reinterpret_cast<int32_t*>(s_lut + 64 * 3 * rep);
   Bcc4DirEntry* s_dir = reinterpret_cast<Bcc4DirEntry*>(s_corr + 64);
-  uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_dir + 16);
+  uint32_t* s_filt = reinterpret_cast<uint32_t*>(s_dir + 16);                  // filter tables, or the head of T + its bound
   __shared__ uint2 s_slot[64];                                                 // Philox products that depend on the slot pair only
   __shared__ long long s_e64[kBcc4Warps];
   __shared__ unsigned s_acc[kBcc4Warps];
@@ -177,6 +209,8 @@ sweep_bcc4_thread(const Geom G, const Bcc4Tables BT, uint32_t* __restrict__ latt
   for (int k = threadIdx.x; k < 64; k += blockDim.x) s_corr[k] = corr[k];
   if (MODE == 1)
     for (int k = threadIdx.x; k < kFilterWords; k += blockDim.x) s_filt[k] = filt[k];
+  if (MODE == 2)
+    for (int k = threadIdx.x; k <= direct_len; k += blockDim.x) s_filt[k] = k < G.accept_len ? accept[k] : 0u;
   for (int k = threadIdx.x; k < 16; k += blockDim.x) s_dir[k] = BT.dir[k >> 3][k & 7];
   const uint32_t t = (uint32_t)st->sweep;
   if (threadIdx.x < 64) s_slot[threadIdx.x] = philox_slot_entry(threadIdx.x, t, G.rk0, G.rk1);
@@ -192,6 +226,7 @@ sweep_bcc4_thread(const Geom G, const Bcc4Tables BT, uint32_t* __restrict__ latt
   env.accept = accept;
   env.accept_len = G.accept_len;
   env.filter_E = G.filter_E;
+  env.direct_len = direct_len;
   const smem_ptr_t dir_p = smem_ptr(s_dir);
   const int rw = G.Lx >> 3;                                     // groups of 8 cells per lattice row
   const uint32_t zstride = (uint32_t)G.Ly * (uint32_t)rw;
@@ -220,82 +255,104 @@ sweep_bcc4_thread(const Geom G, const Bcc4Tables BT, uint32_t* __restrict__ latt
         int gy = t0y + ry; if (gy >= G.Ly) gy -= G.Ly;
         offy[ry] = (uint32_t)gy * (uint32_t)rw;
       }
-      // a3: stage the tile: per row two 8-byte groups (the two sublattice words each), funnel-shifted into two tile words
-#pragma unroll 1
-      for (int rz = 0; rz < 8; ++rz) {
-        int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
-        const uint32_t zoff = (uint32_t)gz * zstride;
-        uint2 lo[8], hi[8];
-#pragma unroll
-        for (int ry = 0; ry < 8; ++ry) {
-          const uint2* row = reinterpret_cast<const uint2*>(lattice) + (zoff + offy[ry]);
-          lo[ry] = row[wlo];
-          hi[ry] = row[whi];
-        }
-#pragma unroll
-        for (int ry = 0; ry < 8; ++ry) {
-          uint32_t* d = tile + (rz * 8 + ry) * NT;
-          d[0] = __funnelshift_r(lo[ry].x, hi[ry].x, sh);
-          d[R * NT] = __funnelshift_r(lo[ry].y, hi[ry].y, sh);
-        }
-      }
-      // a4-a6: the 128 trials of the cell, raster order: conventional cell c = (lz * 4 + ly) * 4 + lx, then b; one Philox
-      // call per conventional cell (slots 2 c and 2 c + 1)
       const uint32_t cell_id = global_cell_id(G, cx, cy, cz);
       const PhiloxCell pc = philox_cell_setup(cell_id, t, ctr3, G.rk0, G.rk1);
+      const uint32_t dwh = (uint32_t)(whi - wlo) * 2u;            // word step from the low to the high group of a row
+      uint32_t* const peer = reinterpret_cast<uint32_t*>(G.peer_lat);
       int esum = 0;
-#pragma unroll 1
-      for (int c = 0; c < 64; ++c) {
-        const uint32_t X4 = 4u * (uint32_t)((c & 3) + 2);
-        const int row = ((c >> 2) & 3) + 2 + 8 * ((c >> 4) + 2);
-        uint32_t* p_row = tile + row * NT;
-        const Philox4 r = philox_factored(pc, s_slot[c], G.rk0, G.rk1);
-#define SMCX_BCC4_TRIAL(B, WDIR, U)                                                                        \
-        {                                                                                                    \
-          const int4 e = lds_int4(dir_p, (int)((B * 8u + ((WDIR) >> 29)) * 16u));                          \
-          const Bcc4DirEntry E{e.x, e.y, e.z, e.w};                                                         \
-          bcc4_trial<B, NT, MODE>(p_row + B * (R * NT), X4, E, U, env, esum, nacc);                         \
+      // The cell runs in four steps of 32 trials (layer lz of the cell); between two steps the lowest layer of either
+      // window is written back (final: later trials only reach higher layers), the other three move down a slot and one
+      // new layer is staged.  Sublattice 0 holds tile layers lz + 1 .. lz + 4, sublattice 1 lz .. lz + 3.
+      // a3: stage tile layer rz of sublattice S into a slot: per row two 8-byte groups (the two sublattice words, one of
+      // them used), funnel-shifted into the tile word
+      auto stage = [&](auto sub_c, int slot, int rz) {
+        constexpr int S = decltype(sub_c)::value;
+        int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
+        const uint32_t zoff = (uint32_t)gz * zstride;
+        uint32_t lo[8], hi[8];
+#pragma unroll
+        for (int ry = 0; ry < 8; ++ry) {
+          const uint32_t* row = lattice + 2u * (zoff + offy[ry]) + S;
+          lo[ry] = row[2 * wlo];
+          hi[ry] = row[2 * whi];
         }
-        SMCX_BCC4_TRIAL(0, r.x, r.y) SMCX_BCC4_TRIAL(1, r.z, r.w)
-#undef SMCX_BCC4_TRIAL
-      }
-      esum_total += esum;     // |dE| < 2^23 (host check), 128 trials: exact in int32 per cell
-      // a7: write back rows 1..6 x 1..6 of both sublattices: the bytes that lie wholly inside this tile
-      {
-        const uint32_t dwh = (uint32_t)(whi - wlo) * 2u;            // word step from the low to the high group of a row
-        uint32_t* const peer = reinterpret_cast<uint32_t*>(G.peer_lat);
-        auto wb = [&](auto cc) {
-          constexpr int C = decltype(cc)::value;
+#pragma unroll
+        for (int ry = 0; ry < 8; ++ry) tile[(S * WR + slot * 8 + ry) * NT] = __funnelshift_r(lo[ry], hi[ry], sh);
+      };
+      // a7: write back rows 1..6 of the layers that leave the windows after step lz - 1 (lz = 4: of everything still
+      // resident), tile layers 1..6 only: the bytes that lie wholly inside this tile
+      auto wb = [&](auto cc, int lz) {
+        constexpr int C = decltype(cc)::value;
 #pragma unroll 1
-          for (int rz = 1; rz < 7; ++rz) {
+        for (int sq = 0; sq < 2; ++sq) {
+          const int first = lz - sq, n_slots = lz == 4 ? 4 : 1;   // window of sublattice sq in step lz - 1: from lz - 1 + (1 - sq)
+#pragma unroll 1
+          for (int slot = 0; slot < n_slots; ++slot) {
+            const int rz = first + slot;
+            if (rz < 1 || rz > 6) continue;
             int gz = t0z + rz; if (gz >= G.Lz) gz -= G.Lz;
             const bool mirror = peer != nullptr && gz >= G.peer_z0 && gz < G.peer_z1;   // fused ghost-layer message
 #pragma unroll
             for (int ry = 1; ry < 7; ++ry) {
-              const uint32_t base = (((uint32_t)gz * zstride) + offy[ry] + (uint32_t)wlo) * 2u;
-#pragma unroll
-              for (int s = 0; s < 2; ++s) {
-                const uint32_t v = tile[(s * R + rz * 8 + ry) * NT];
-                store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(lattice + base + s),
-                                                     reinterpret_cast<unsigned char*>(lattice + (uint32_t)(base + s + dwh)), v);
-                if (mirror)
-                  store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(peer + base + s),
-                                                       reinterpret_cast<unsigned char*>(peer + (uint32_t)(base + s + dwh)), v);
-              }
+              const uint32_t base = (((uint32_t)gz * zstride) + offy[ry] + (uint32_t)wlo) * 2u + (uint32_t)sq;
+              const uint32_t v = tile[(sq * WR + slot * 8 + ry) * NT];
+              store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(lattice + base),
+                                                   reinterpret_cast<unsigned char*>(lattice + (uint32_t)(base + dwh)), v);
+              if (mirror)
+                store_tile_bytes<C, (4 * C + 7) / 8>(reinterpret_cast<unsigned char*>(peer + base),
+                                                     reinterpret_cast<unsigned char*>(peer + (uint32_t)(base + dwh)), v);
             }
           }
-        };
+        }
+      };
+      auto write_back = [&](int lz) {
         switch (x0 & 7) {
-          case 0: wb(std::integral_constant<int, 0>{}); break;
-          case 1: wb(std::integral_constant<int, 1>{}); break;
-          case 2: wb(std::integral_constant<int, 2>{}); break;
-          case 3: wb(std::integral_constant<int, 3>{}); break;
-          case 4: wb(std::integral_constant<int, 4>{}); break;
-          case 5: wb(std::integral_constant<int, 5>{}); break;
-          case 6: wb(std::integral_constant<int, 6>{}); break;
-          default: wb(std::integral_constant<int, 7>{}); break;
+          case 0: wb(std::integral_constant<int, 0>{}, lz); break;
+          case 1: wb(std::integral_constant<int, 1>{}, lz); break;
+          case 2: wb(std::integral_constant<int, 2>{}, lz); break;
+          case 3: wb(std::integral_constant<int, 3>{}, lz); break;
+          case 4: wb(std::integral_constant<int, 4>{}, lz); break;
+          case 5: wb(std::integral_constant<int, 5>{}, lz); break;
+          case 6: wb(std::integral_constant<int, 6>{}, lz); break;
+          default: wb(std::integral_constant<int, 7>{}, lz); break;
+        }
+      };
+      using TW = Bcc4Tile<NT, WR>;
+#pragma unroll 1
+      for (int lz = 0; lz < 4; ++lz) {
+        if (lz > 0) {
+          write_back(lz);
+#pragma unroll 1
+          for (int s = 0; s < 2; ++s) {                           // slots 1..3 move down one slot
+            uint32_t* d = tile + s * WR * NT;
+#pragma unroll 8
+            for (int r = 0; r < 24; ++r) d[r * NT] = d[(r + 8) * NT];
+          }
+        }
+#pragma unroll 1
+        for (int slot = lz ? 3 : 0; slot < 4; ++slot) {
+          stage(std::integral_constant<int, 0>{}, slot, lz + 1 + slot);
+          stage(std::integral_constant<int, 1>{}, slot, lz + slot);
+        }
+        // a4-a6: the 32 trials of layer lz of the cell, raster order: conventional cell c = (lz * 4 + ly) * 4 + lx, then
+        // b; one Philox call per conventional cell (slots 2 c and 2 c + 1); site i sits in (virtual) slot 2 of its window
+#pragma unroll 1
+        for (int c = 16 * lz; c < 16 * lz + 16; ++c) {
+          const uint32_t X4 = 4u * (uint32_t)((c & 3) + 2);
+          uint32_t* p_row = tile + (((c >> 2) & 3) + 2 + 16) * NT;
+          const Philox4 r = philox_factored(pc, s_slot[c], G.rk0, G.rk1);
+#define SMCX_BCC4_TRIAL(B, WDIR, U)                                                                        \
+          {                                                                                                  \
+            const int4 e = lds_int4(dir_p, (int)((B * 8u + ((WDIR) >> 29)) * 16u));                        \
+            const Bcc4DirEntry E{e.x, e.y, e.z, e.w};                                                       \
+            bcc4_trial<B, NT, MODE, WR>(const_cast<uint32_t*>(fcc_at<NT>(p_row, TW::sub(B))), X4, E, U, env, esum, nacc); \
+          }
+          SMCX_BCC4_TRIAL(0, r.x, r.y) SMCX_BCC4_TRIAL(1, r.z, r.w)
+#undef SMCX_BCC4_TRIAL
         }
       }
+      write_back(4);
+      esum_total += esum;     // |dE| < 2^23 (host check), 128 trials: exact in int32 per cell
     }
   }
   // a8: one atomic pair per block
@@ -316,26 +373,33 @@ sweep_bcc4_thread(const Geom G, const Bcc4Tables BT, uint32_t* __restrict__ latt
 }
 
 inline int configure_bcc4_thread(int rep) {
-  const int sm = (int)bcc4_smem_bytes(rep);
-  if (cudaFuncSetAttribute(sweep_bcc4_thread<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
-  if (cudaFuncSetAttribute(sweep_bcc4_thread<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm) != cudaSuccess) return -1;
+  (void)rep;
+  if (cudaFuncSetAttribute(sweep_bcc4_thread<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, kBcc4SmemMax) != cudaSuccess) return -1;
+  if (cudaFuncSetAttribute(sweep_bcc4_thread<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, kBcc4SmemMax) != cudaSuccess) return -1;
+  if (cudaFuncSetAttribute(sweep_bcc4_thread<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, kBcc4SmemMax) != cudaSuccess) return -1;
   cudaFuncSetAttribute(sweep_bcc4_thread<0>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   cudaFuncSetAttribute(sweep_bcc4_thread<1>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+  cudaFuncSetAttribute(sweep_bcc4_thread<2>, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   return 0;
 }
 
 inline int launch_bcc4_thread(const Geom& G, const Bcc4Tables& BT, uint32_t* lattice, const uint32_t* d_lut, const int32_t* d_corr,
                               int rep, const uint32_t* accept, const uint32_t* d_filter, DevState* st, int colour, int sm_count,
-                              cudaStream_t stream) {
+                              int tail_from, cudaStream_t stream) {
   const unsigned n_batches = (G.cells_per_colour + 31u) / 32u;
   const unsigned want = (n_batches + kBcc4Warps - 1) / kBcc4Warps;
   const unsigned grid = want < (unsigned)sm_count ? want : (unsigned)sm_count;
-  const size_t sm = bcc4_smem_bytes(rep);
   const uint4* lut4 = reinterpret_cast<const uint4*>(d_lut);
-  if (G.filter_E >= 0)
-    sweep_bcc4_thread<1><<<grid, kBcc4Warps * 32, sm, stream>>>(G, BT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour);
+  // the head of T in shared memory: sound if T[direct] bounds every later entry (tail_from: checked by the host at upload)
+  int direct = bcc4_direct_entries(rep, G.accept_len);
+  if (direct < G.accept_len && direct < tail_from) direct = 0;
+  if (direct > 0)
+    sweep_bcc4_thread<2><<<grid, kBcc4Warps * 32, bcc4_smem_bytes(rep, (size_t)direct + 1), stream>>>(
+        G, BT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour, direct);
+  else if (G.filter_E >= 0)
+    sweep_bcc4_thread<1><<<grid, kBcc4Warps * 32, bcc4_smem_bytes(rep), stream>>>(G, BT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour, 0);
   else
-    sweep_bcc4_thread<0><<<grid, kBcc4Warps * 32, sm, stream>>>(G, BT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour);
+    sweep_bcc4_thread<0><<<grid, kBcc4Warps * 32, bcc4_smem_bytes(rep), stream>>>(G, BT, lattice, lut4, d_corr, rep, accept, d_filter, st, colour, 0);
   return cudaGetLastError() == cudaSuccess ? 0 : -1;
 }
 #endif  // __CUDACC__
