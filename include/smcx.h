@@ -111,7 +111,8 @@ enum {
   SMCX_E_CUDA = -11,               /* CUDA error; text via smcx_last_error */
   SMCX_E_UNSUPPORTED = -12,        /* storage/kernel choice not valid for these parameters */
   SMCX_E_RANGE = -13,              /* trace range not retained, sweep counter overflow */
-  SMCX_E_EPI_RANGE = -14           /* EPI magnitudes / local-model weights so large that the int32 dE of a trial could overflow */
+  SMCX_E_EPI_RANGE = -14,          /* EPI magnitudes / local-model weights so large that the int32 dE of a trial could overflow */
+  SMCX_E_STATIC_SCRATCH = -15      /* smcx_pair_counts_static: n_shells * n_species^2 > SMCX_STATIC_PAIR_COUNTS_MAX */
 };
 
 typedef struct {
@@ -438,6 +439,28 @@ int smcx_domain_group_synchronize(smcx_domain_group_t *g);
 int64_t smcx_domain_group_kernel_launches(smcx_domain_group_t *g);
 int64_t smcx_domain_group_message_bytes(smcx_domain_group_t *g);              /* bytes moved between slabs by copies so far */
 int64_t smcx_domain_group_fused_messages(smcx_domain_group_t *g);             /* pass messages written by the sweep kernels themselves */
+
+/* ---- Pair counts without any device allocation (a9; Eq. 8; reading S7) ---------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, serving loops, harnesses that forbid it):
+ * the ordered pair counts N_s(p',p) of a lattice the CALLER holds in device memory, with the accumulator of the
+ * reduction in a file-scope device array of the library instead of a handle's workspace.  Calls no cudaMalloc,
+ * cudaFree or allocating library routine, needs no smcx_t handle, and does not synchronise.
+ *   lattice, dims, n_species, n_shells: as in smcx_params_t (dims[a] >= 2; no divisibility requirement).
+ *   d_species:      device, N = B * dims[0] * dims[1] * dims[2] bytes, one uint8 species per site in the site order of
+ *                   smcx_species (values >= n_species are not checked: undefined counts).  Read only.
+ *   d_pair_counts:  device, [n_shells][n_species][n_species] int64, written by the call: the same values smcx_sro
+ *                   returns in pair_counts for that lattice (bit-exact: integer counts).
+ *   stream:         cudaStream_t the three kernels (clear, count, finish) are enqueued on; NULL = default stream.
+ * Limit: n_shells * n_species^2 <= SMCX_STATIC_PAIR_COUNTS_MAX (1024 entries = 8 KB of device memory that every GPU
+ * which loads the library holds until the process exits); beyond it SMCX_E_STATIC_SCRATCH (e.g. 5 shells x 16 species).
+ * The array is shared by every call on a device and keeps the last call's contents; each call clears it first.  Calls
+ * that overlap on one GPU (different streams, threads or processes' worth of streams in one process) RACE on it: issue
+ * them on one stream or order them with events.  The device current at the call is the one used; the first call on a
+ * device resolves the array's device address (cudaGetSymbolAddress).  Errors: SMCX_E_NULL_ARG, SMCX_E_BAD_LATTICE,
+ * SMCX_E_BAD_SPECIES, SMCX_E_BAD_SHELLS, SMCX_E_BAD_DIMS, SMCX_E_STATIC_SCRATCH, SMCX_E_CUDA (launch failure). */
+#define SMCX_STATIC_PAIR_COUNTS_MAX 1024
+int smcx_pair_counts_static(int32_t lattice, const int32_t *dims, int32_t n_species, int32_t n_shells,
+                            const uint8_t *d_species, int64_t *d_pair_counts, void *stream);
 
 const char *smcx_last_error(smcx_t *h); /* text of the last CUDA error seen by this handle */
 const char *smcx_strerror(int code);

@@ -11,5 +11,5 @@ from .binding import (  # noqa: F401
     KERNEL_AUTO, KERNEL_WARP_PER_CELL, KERNEL_THREAD_PER_CELL, KERNEL_THREAD_PERSISTENT, KERNEL_GROUP_PER_CELL,
     KERNEL_FCC_THREAD, KERNEL_LOCAL_WARP, KERNEL_BCC4_THREAD, MODEL_EPI, MODEL_LOCAL,
     SmcxError, Lattice, Ensemble, Domain, DomainGroup, load_library, library_path, exported_symbols,
-    domain_partition, domain_plan_messages, sro_from_counts,
+    domain_partition, domain_plan_messages, sro_from_counts, pair_counts_static, STATIC_PAIR_COUNTS_MAX,
 )

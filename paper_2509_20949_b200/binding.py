@@ -124,6 +124,7 @@ def load_library(build_if_missing: bool = True):
         "smcx_shell_offsets": (C.c_int, [vp, C.c_int32, i32p, C.c_int32, i32p]),
         "smcx_get_config": (C.c_int, [vp, i32p, i32p, i64p, i64p]),
         "smcx_kernel_launches": (C.c_int64, [vp]),
+        "smcx_pair_counts_static": (C.c_int, [C.c_int32, i32p, C.c_int32, C.c_int32, vp, vp, vp]),
         "smcx_group_layout": (C.c_int, [C.POINTER(_Params), i32p, i32p, i32p, i32p, i32p, i32p, C.POINTER(C.c_uint8)]),
         "smcx_ensemble_create": (C.c_int, [C.POINTER(vp), C.POINTER(_Params), C.c_int32, i32p,
                                            C.POINTER(C.POINTER(C.c_uint32)), i32p, C.POINTER(C.c_uint64), C.c_uint64]),
@@ -558,6 +559,23 @@ def domain_plan_messages(n_domains, index, sweep, phase, first_sweep=0, **kw):
     if rc != 0:
         raise SmcxError(rc, "smcx_domain_plan_messages")
     return send.as_tuple(), recv.as_tuple()
+
+
+STATIC_PAIR_COUNTS_MAX = 1024
+
+
+def pair_counts_static(lattice, dims, n_species, n_shells, d_species, d_pair_counts, stream=None):
+    """smcx_pair_counts_static: ordered pair counts of the uint8 device tensor `d_species` into the int64 device tensor
+    `d_pair_counts` ([n_shells][n_species][n_species]) with the library's static device scratch: no device allocation,
+    no handle, no synchronisation.  Both tensors are the caller's."""
+    lib = load_library()
+    d = (C.c_int32 * 3)(*[int(x) for x in dims])
+    sp = int(stream.cuda_stream) if stream is not None else 0
+    rc = lib.smcx_pair_counts_static(int(lattice), d, int(n_species), int(n_shells), C.c_void_p(d_species.data_ptr()),
+                                     C.c_void_p(d_pair_counts.data_ptr()), C.c_void_p(sp))
+    if rc != 0:
+        raise SmcxError(rc, "smcx_pair_counts_static")
+    return d_pair_counts
 
 
 def sro_from_counts(half_counts, **kw):

@@ -784,6 +784,7 @@ const char* smcx_strerror(int code) {
     case SMCX_E_UNSUPPORTED: return "storage/kernel choice not valid for these parameters";
     case SMCX_E_RANGE: return "range not available";
     case SMCX_E_EPI_RANGE: return "EPI magnitudes too large: the int32 energy change of a trial could overflow";
+    case SMCX_E_STATIC_SCRATCH: return "n_shells * n_species^2 exceeds SMCX_STATIC_PAIR_COUNTS_MAX (1024), the size of the library's static device scratch";
     default: return "unknown error";
   }
 }
@@ -1364,3 +1365,4 @@ int smcx_group_layout(const smcx_params_t* p, int32_t* lanes, int32_t* A, int32_
 
 #include "ensemble_api.inc"
 #include "domain_api.inc"
+#include "static_scratch_api.inc"
