@@ -70,9 +70,27 @@ __device__ __noinline__ int local_eps_shell(const int32_t* __restrict__ s_w1, co
   return e;
 }
 
+// eps_s(c, n + e_to - e_from) - eps_s(c, n) for a site that keeps its own species c and sees ONE of the swapped sites in
+// shell s (that neighbour turns from species `from` into `to`): with g_t(y) = 2 q_tt for y = t, q_{min(t,y) max(t,y)}
+// otherwise (s_g, built by the block from W2),
+//   l_to - l_from + q_toto + q_fromfrom - q_fromto + sum_y (g_to(y) - g_from(y)) n_y
+// -- n multiply-adds instead of two evaluations of the quadratic form.  Exact integer algebra: the same value (mod 2^32)
+// as the difference of the two evaluations.
+__device__ __forceinline__ int local_delta_shell(const int32_t* __restrict__ s_w1, const int32_t* __restrict__ s_g, int n, int s,
+                                                 int c, int from, int to, unsigned long long v) {
+  const int32_t* l = s_w1 + (s * n + c) * n;
+  const int32_t* gt = s_g + ((s * n + c) * n + to) * n;
+  const int32_t* gf = s_g + ((s * n + c) * n + from) * n;
+  int e = l[to] - l[from] + ((gt[to] + gf[from]) >> 1) - gf[to];
+#pragma unroll
+  for (int y = 0; y < kLocalMaxSpecies; ++y)
+    if (y < n) e += (gt[y] - gf[y]) * (int)((v >> (8 * y)) & 255ull);
+  return e;
+}
+
 inline size_t local_smem_bytes(const Geom& G, int umax) {
   const int n = G.n_species;
-  size_t b = (size_t)G.n_shells * n * n * 4 + (size_t)G.n_shells * n * n * n * 4;
+  size_t b = (size_t)G.n_shells * n * n * 4 + 2 * (size_t)G.n_shells * n * n * n * 4;     // W1, W2, g
   b += (size_t)G.B * G.Z0 * G.n_shells * umax * sizeof(LocalUEntry) + (size_t)G.B * G.Z0 * G.n_shells * 4;
   b += (size_t)G.B * G.ZT * 2 + 16;
   b = (b + 15) & ~(size_t)15;
@@ -87,7 +105,8 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
   const int n = G.n_species, n_shells = G.n_shells, ZT = G.ZT, Z0 = G.Z0;
   int32_t* s_w1 = reinterpret_cast<int32_t*>(smem);
   int32_t* s_w2 = s_w1 + n_shells * n * n;
-  LocalUEntry* s_u = reinterpret_cast<LocalUEntry*>(s_w2 + n_shells * n * n * n);
+  int32_t* s_g = s_w2 + n_shells * n * n * n;
+  LocalUEntry* s_u = reinterpret_cast<LocalUEntry*>(s_g + n_shells * n * n * n);
   int* s_ucount = reinterpret_cast<int*>(s_u + B * Z0 * n_shells * T.umax);
   short* s_delta = reinterpret_cast<short*>(s_ucount + B * Z0 * n_shells);
   const int tile_sites = G.TW * G.TW * G.TW * B;
@@ -100,7 +119,11 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
   __shared__ int s_start[kMaxShells + 1];
 
   for (int k = threadIdx.x; k < n_shells * n * n; k += blockDim.x) s_w1[k] = T.w1[k];
-  for (int k = threadIdx.x; k < n_shells * n * n * n; k += blockDim.x) s_w2[k] = T.w2[k];
+  for (int k = threadIdx.x; k < n_shells * n * n * n; k += blockDim.x) {
+    s_w2[k] = T.w2[k];
+    const int y = k % n, tt = (k / n) % n, sc = k / (n * n);          // g_t(y) of (shell, centre) sc
+    s_g[k] = y == tt ? 2 * T.w2[(sc * n + tt) * n + tt] : T.w2[(sc * n + min(tt, y)) * n + max(tt, y)];
+  }
   for (int k = threadIdx.x; k < B * Z0 * n_shells * T.umax; k += blockDim.x) s_u[k] = T.utab[k];
   for (int k = threadIdx.x; k < B * Z0 * n_shells; k += blockDim.x) s_ucount[k] = T.ucount[k];
   for (int k = threadIdx.x; k < B * ZT; k += blockDim.x) s_delta[k] = G.delta[k / ZT][k % ZT];
@@ -163,26 +186,37 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
             // a5: the changed terms of the local energies, before and after, shell by shell
             const unsigned long long da = 1ull << (8 * sa), db = 1ull << (8 * sb);
             int part = 0;
+            // sites other than i and j: they keep their species, and the shell-s term of such a site changes only if
+            // it sees exactly one of i, j in shell s (one neighbour changes species; seeing both, its counts stay)
             for (int s = 0; s < n_shells; ++s) {
               const LocalUEntry* ue = s_u + ((b * Z0 + dir) * n_shells + s) * T.umax;
               const int nu = s_ucount[(b * Z0 + dir) * n_shells + s];
               const int m0 = s_start[s], m1 = s_start[s + 1];
               for (int q = lane; q < nu; q += 32) {
                 const LocalUEntry e = ue[q];
-                const unsigned bits = e.bits;
+                const unsigned bits = e.bits, see = bits & 3u;
+                if ((bits & 12u) != 0u || see == 0u || see == 3u) continue;
                 const int su = si + e.delta;
                 const short* dl = s_delta + (int)((bits >> 4) & 3u) * ZT;
                 unsigned long long cnt = 0ull;
 #pragma unroll 6
                 for (int mm = m0; mm < m1; ++mm) cnt += 1ull << (8 * (int)tile[su + dl[mm]]);   // six loads in flight
-                const int c0 = tile[su];
-                const int before = local_eps_shell(s_w1, s_w2, n, s, c0, cnt);
-                if (bits & 1u) cnt += db - da;   // i turns from a into b
-                if (bits & 2u) cnt += da - db;   // j turns from b into a
-                const unsigned kind = (bits >> 2) & 3u;
-                const int c1 = kind == 1u ? sb : (kind == 2u ? sa : c0);
-                part += local_eps_shell(s_w1, s_w2, n, s, c1, cnt) - before;
+                // sees i: that neighbour turns from a into b; sees j: from b into a
+                part += local_delta_shell(s_w1, s_g, n, s, tile[su], see == 1u ? sa : sb, see == 1u ? sb : sa, cnt);
               }
+            }
+            // i and j themselves change species (and see each other in shell 0, where j is a nearest neighbour of i):
+            // both evaluations of every shell term, one (site, shell) per lane
+            if (lane < 2 * n_shells) {
+              const int s = lane >> 1, who = lane & 1;
+              const int su = who ? sj : si;
+              const short* dl = s_delta + (su & (B - 1)) * ZT;           // tile index = cell * B + basis
+              unsigned long long cnt = 0ull;
+#pragma unroll 6
+              for (int mm = s_start[s]; mm < s_start[s + 1]; ++mm) cnt += 1ull << (8 * (int)tile[su + dl[mm]]);
+              const int before = local_eps_shell(s_w1, s_w2, n, s, who ? sb : sa, cnt);
+              if (s == 0) cnt += who ? db - da : da - db;                // j sees i turn from a into b; i sees j turn from b into a
+              part += local_eps_shell(s_w1, s_w2, n, s, who ? sa : sb, cnt) - before;
             }
             const int dE = __reduce_add_sync(0xffffffffu, part);
             // a6: Eq. 3 in integer form
