@@ -719,8 +719,17 @@ int launch_colour_pass(smcx* h, const Geom& G, int colour) {
     const LocalTables T{h->d_epi(), h->d_quad(), h->d_utab(), h->d_ucount(), P.local_umax};
     const size_t sm = local_smem_bytes(G, P.local_umax);
     const unsigned grid = (G.cells_per_colour + kLocalWarps - 1) / kLocalWarps;
-    if (G.B == 2) sweep_local_warp<2><<<grid, kLocalWarps * 32, sm, h->stream>>>(G, h->d_species(), T, h->d_accept(), h->d_state(), colour);
-    else sweep_local_warp<4><<<grid, kLocalWarps * 32, sm, h->stream>>>(G, h->d_species(), T, h->d_accept(), h->d_state(), colour);
+    int zmax = 0;
+    for (int s2 = 0, m2 = 0; s2 < G.n_shells; ++s2) {
+      int z = 0;
+      while (m2 < G.ZT && (int)G.shell_of[m2] == s2) { ++m2; ++z; }
+      zmax = std::max(zmax, z);
+    }
+    const bool narrow = G.n_species <= kLocalNarrowSpecies && zmax <= kLocalNarrowMaxZ;   // 5-bit count fields in a 32-bit word
+    if (G.B == 2 && narrow) sweep_local_warp<2, true><<<grid, kLocalWarps * 32, sm, h->stream>>>(G, h->d_species(), T, h->d_accept(), h->d_state(), colour);
+    else if (G.B == 2) sweep_local_warp<2, false><<<grid, kLocalWarps * 32, sm, h->stream>>>(G, h->d_species(), T, h->d_accept(), h->d_state(), colour);
+    else if (narrow) sweep_local_warp<4, true><<<grid, kLocalWarps * 32, sm, h->stream>>>(G, h->d_species(), T, h->d_accept(), h->d_state(), colour);
+    else sweep_local_warp<4, false><<<grid, kLocalWarps * 32, sm, h->stream>>>(G, h->d_species(), T, h->d_accept(), h->d_state(), colour);
     h->launches++;
     SMCX_CUDA(h, cudaGetLastError());
     return SMCX_OK;
@@ -865,8 +874,10 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     }
     if (h->plan.kernel == SMCX_KERNEL_LOCAL_WARP) {
       const int lsm = (int)local_smem_bytes(G, h->plan.local_umax);
-      cudaError_t e = cudaFuncSetAttribute(sweep_local_warp<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, lsm);
-      if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_local_warp<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, lsm);
+      cudaError_t e = cudaFuncSetAttribute(sweep_local_warp<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lsm);
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_local_warp<4, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, lsm);
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_local_warp<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lsm);
+      if (e == cudaSuccess) e = cudaFuncSetAttribute(sweep_local_warp<4, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, lsm);
       if (e != cudaSuccess) { h->err = cudaGetErrorString(e); return fail(SMCX_E_CUDA); }
     }
     if (h->plan.kernel == SMCX_KERNEL_WARP_PER_CELL) {

@@ -76,17 +76,23 @@ __device__ __noinline__ int local_eps_shell(const int32_t* __restrict__ s_w1, co
 //   l_to - l_from + q_toto + q_fromfrom - q_fromto + sum_y (g_to(y) - g_from(y)) n_y
 // -- n multiply-adds instead of two evaluations of the quadratic form.  Exact integer algebra: the same value (mod 2^32)
 // as the difference of the two evaluations.
+template <class CountWord, int FIELD>
 __device__ __forceinline__ int local_delta_shell(const int32_t* __restrict__ s_w1, const int32_t* __restrict__ s_g, int n, int s,
-                                                 int c, int from, int to, unsigned long long v) {
+                                                 int c, int from, int to, CountWord v) {
   const int32_t* l = s_w1 + (s * n + c) * n;
   const int32_t* gt = s_g + ((s * n + c) * n + to) * n;
   const int32_t* gf = s_g + ((s * n + c) * n + from) * n;
   int e = l[to] - l[from] + ((gt[to] + gf[from]) >> 1) - gf[to];
+  constexpr int kFields = (int)(8 * sizeof(CountWord)) / FIELD;
 #pragma unroll
-  for (int y = 0; y < kLocalMaxSpecies; ++y)
-    if (y < n) e += (gt[y] - gf[y]) * (int)((v >> (8 * y)) & 255ull);
+  for (int y = 0; y < kFields; ++y)
+    if (y < n) e += (gt[y] - gf[y]) * (int)((v >> (FIELD * y)) & (CountWord)((1 << FIELD) - 1));
   return e;
 }
+// The counts of the sites that keep their species: eight 8-bit fields of a 64-bit word, or -- n_species <= 6 -- six 5-bit
+// fields of a 32-bit word (a shell has at most 24 neighbours), which halves the arithmetic of the counting loop.
+constexpr int kLocalNarrowSpecies = 6;
+constexpr int kLocalNarrowMaxZ = 31;
 
 inline size_t local_smem_bytes(const Geom& G, int umax) {
   const int n = G.n_species;
@@ -97,7 +103,7 @@ inline size_t local_smem_bytes(const Geom& G, int umax) {
   return b + (size_t)kLocalWarps * (((size_t)G.TW * G.TW * G.TW * G.B + 15) & ~(size_t)15);
 }
 
-template <int B>
+template <int B, bool NARROW>
 __global__ void __launch_bounds__(kLocalWarps * 32, 3)
 sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables T, const uint32_t* __restrict__ accept,
                  DevState* __restrict__ st, int colour) {
@@ -198,11 +204,19 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
                 if ((bits & 12u) != 0u || see == 0u || see == 3u) continue;
                 const int su = si + e.delta;
                 const short* dl = s_delta + (int)((bits >> 4) & 3u) * ZT;
-                unsigned long long cnt = 0ull;
-#pragma unroll 6
-                for (int mm = m0; mm < m1; ++mm) cnt += 1ull << (8 * (int)tile[su + dl[mm]]);   // six loads in flight
                 // sees i: that neighbour turns from a into b; sees j: from b into a
-                part += local_delta_shell(s_w1, s_g, n, s, tile[su], see == 1u ? sa : sb, see == 1u ? sb : sa, cnt);
+                const int from = see == 1u ? sa : sb, to = see == 1u ? sb : sa;
+                if (NARROW) {
+                  uint32_t cnt = 0u;
+#pragma unroll 6
+                  for (int mm = m0; mm < m1; ++mm) cnt += 1u << (5 * (int)tile[su + dl[mm]]);    // six loads in flight
+                  part += local_delta_shell<uint32_t, 5>(s_w1, s_g, n, s, tile[su], from, to, cnt);
+                } else {
+                  unsigned long long cnt = 0ull;
+#pragma unroll 6
+                  for (int mm = m0; mm < m1; ++mm) cnt += 1ull << (8 * (int)tile[su + dl[mm]]);
+                  part += local_delta_shell<unsigned long long, 8>(s_w1, s_g, n, s, tile[su], from, to, cnt);
+                }
               }
             }
             // i and j themselves change species (and see each other in shell 0, where j is a nearest neighbour of i):

@@ -24,6 +24,8 @@ def _pair(lattice, dims, n_sp, n_sh, seed, kT, amp1=200, amp2=25):
     (smcx.BCC, (24, 16, 32), 2, 1, 500),       # one shell, two species, a ragged grid of cells
     (smcx.FCC, (16, 16, 16), 5, 3, 2500),      # the paper's lattice type: 42 neighbours, 86 affected sites per trial
     (smcx.FCC, (16, 24, 16), 8, 2, 1500),      # most species the packed counters take
+    (smcx.BCC, (16, 16, 16), 6, 2, 900),       # most species of the 5-bit count fields (32-bit count word)
+    (smcx.FCC, (16, 16, 16), 7, 1, 1200),      # one more: 8-bit fields again
 ])
 def test_local_model_against_the_oracle(lattice, dims, n_sp, n_sh, kT):
     g, o = _pair(lattice, dims, n_sp, n_sh, seed=41, kT=kT)
