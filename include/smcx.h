@@ -70,11 +70,11 @@ enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_4BIT = 4, SMCX
  * |V_s(b,x) - V_s(a,x)| < 32768: one thread per link cell on a packed tile (one 32-bit word per sublattice row of 8
  * cells), neighbours gathered by rotations and bit-selects, the EPI differences applied four neighbours at a time by
  * byte-permute look-ups (PRMT) and byte dot products (sweep_fcc.cuh).  What AUTO picks for such lattices when
- * a colour has at least 148 * 6 * 32 link cells (below that the sub-warp kernel's shorter chain per trial wins).
+ * a colour has at least 12,000 link cells (measured crossover; below that the sub-warp kernel's shorter chain per trial wins).
  * BCC4_THREAD: BCC, the first two shells, link_cell = 4, n_species <= 8, 4BIT storage, every |V_s(b,x) - V_s(a,x)| < 32768:
  * the BCC counterpart of FCC_THREAD (one thread per link cell on a 512-byte packed tile, nine row loads per site, the same
  * PRMT look-ups; sweep_bcc4.cuh).  What AUTO picks for BCC lattices with 5..8 species when a colour has at least
- * 148 * 12 * 32 link cells.
+ * 12,000 link cells.
  * AUTO picks, when the parameters allow a thread kernel, THREAD_PERSISTENT for lattices that give every
  * warp of every SM a batch of cells (>= 148*20*32 link cells per colour) and THREAD_PER_CELL below that
  * (same speed there, and concurrent lattices of a replica ensemble overlap freely).  Results never

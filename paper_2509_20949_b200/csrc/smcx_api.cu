@@ -31,6 +31,7 @@ using namespace smcxk;
 
 namespace {
 
+constexpr long long kPackedMinCellsPerColour = 12000;   // AUTO: packed 4-bit kernels from this many link cells per colour
 constexpr int kAcceptCapacity = 1 << 20;  // entries reserved on the device for the threshold table
 constexpr int kStagingSlots = 4;
 constexpr long long kChunkSites = 1ll << 26;  // bounce-buffer size for packed <-> uint8 transfers
@@ -295,11 +296,14 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     return SMCX_E_UNSUPPORTED;
   }
   if (kernel == SMCX_KERNEL_AUTO) {
-    // FCC: the packed thread-per-cell kernel once every warp of every SM gets a batch of 32 cells; below that a pass
-    // lasts as long as one cell's chain of trials, which is shorter with several lanes per cell
-    if (fcc_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && plan->n_cells / 8 >= 148ll * kFccWarps * 32)))
+    // The packed thread-per-cell kernels (a warp = 32 cells, a pass at least one cell's chain of trials long) against the
+    // sub-warp kernel (several lanes per cell), measured on lattices of growing size (profiles/README.md): the packed
+    // kernels win from about 12,000 link cells per colour on (2.5 batches of 32 cells per SM) -- FCC 192^3: 1.9e10 against
+    // 1.6e10, FCC 256^3: 4.6e10 against 1.8e10; BCC with five species 256^3: 4.8e10 against 2.4e10 -- and lose below
+    // (8,000 cells per colour: 1.06e10 against 1.3e10).
+    if (fcc_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && plan->n_cells / 8 >= kPackedMinCellsPerColour)))
       kernel = SMCX_KERNEL_FCC_THREAD;
-    else if (bcc4_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && !fast_ok && plan->n_cells / 8 >= 148ll * kBcc4Warps * 32)))
+    else if (bcc4_ok && (storage == SMCX_STORAGE_4BIT || (storage == SMCX_STORAGE_AUTO && !fast_ok && plan->n_cells / 8 >= kPackedMinCellsPerColour)))
       kernel = SMCX_KERNEL_BCC4_THREAD;
     else if (storage == SMCX_STORAGE_U8) kernel = SMCX_KERNEL_GROUP_PER_CELL;
     else if (!fast_ok) kernel = SMCX_KERNEL_GROUP_PER_CELL;
