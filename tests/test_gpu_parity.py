@@ -533,6 +533,22 @@ def test_packed_fcc_kernel_arbitrary_threshold_tables(kind):
     assert (g.energy_trace() == o.energy_trace()).all() and g.stats() == o.stats() and g.stats()[2] > 0
 
 
+def test_auto_picks_the_packed_kernels_from_12000_cells_per_colour():
+    """AUTO's measured crossover (profiles/README.md): packed 4-bit kernels from 12,000 link cells per colour on, the
+    sub-warp kernel below; 4-species BCC always a 2-bit thread kernel.  Results never depend on the choice (P14)."""
+    def pick(lattice, edge, n_sp, n_sh):
+        g = smcx.Lattice(lattice, (edge,) * 3, n_sp, n_sh, make_epi(n_sh, n_sp, 300, 3), make_accept_table(600), 3,
+                         link_cell=4, kT_units=600)
+        k, st = g.kernel, g.storage
+        g.close()
+        return k, st
+    assert pick(smcx.FCC, 160, 5, 3) == (smcx.KERNEL_GROUP_PER_CELL, smcx.STORAGE_U8)        # 8,000 cells per colour
+    assert pick(smcx.FCC, 192, 5, 3) == (smcx.KERNEL_FCC_THREAD, smcx.STORAGE_4BIT)          # 13,824
+    assert pick(smcx.BCC, 160, 5, 2) == (smcx.KERNEL_GROUP_PER_CELL, smcx.STORAGE_U8)
+    assert pick(smcx.BCC, 192, 5, 2) == (smcx.KERNEL_BCC4_THREAD, smcx.STORAGE_4BIT)
+    assert pick(smcx.BCC, 192, 4, 2) == (smcx.KERNEL_THREAD_PER_CELL, smcx.STORAGE_2BIT)
+
+
 def test_p14_four_bit_and_uint8_storage_agree():
     """P14: SMCX_STORAGE_4BIT (packed FCC kernel) and SMCX_STORAGE_U8 (sub-warp and warp kernels) give identical
     smcx_species, traces and pair counts, on the paper's composition with stage-wise cooling."""
