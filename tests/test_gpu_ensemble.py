@@ -117,6 +117,35 @@ def test_fcc_five_species_ensemble_with_the_sub_warp_kernel():
     g.close()
 
 
+@pytest.mark.parametrize("lat,dims,n_sp,n_sh,kernel", [
+    (1, (16, 16, 8), 5, 3, smcx.KERNEL_FCC_THREAD),
+    (0, (16, 8, 16), 6, 2, smcx.KERNEL_BCC4_THREAD),
+], ids=["fcc_thread", "bcc4_thread"])
+def test_ensembles_on_the_packed_kernels(lat, dims, n_sp, n_sh, kernel):
+    """Replica exchange with the packed 4-bit kernels: their acceptance reads the head of the threshold table from
+    shared memory and relies on a property of the table the host checks at upload; in an ensemble the tables move
+    between replicas on the device (replica_apply_tables_kernel), with different lengths padded to the longest."""
+    from smcx_inputs import make_epi
+    w = 4
+    epi = make_epi(n_sh, n_sp, 400, 1003)
+    kTs = [300, 690, 1500]
+    tables = [make_accept_table(k) for k in kTs]
+    seeds = [41, 42, 43]
+    g = smcx.Ensemble(lat, dims, n_sp, n_sh, epi, kTs, tables, seeds, 77, link_cell=w, kernel=kernel)
+    assert g.replicas[0].kernel == kernel and g.replicas[0].storage == smcx.STORAGE_4BIT
+    reps = [oracle.Oracle(lat, dims, n_sp, n_sh, epi, w, tables[r], seeds[r]) for r in range(3)]
+    for o in reps:
+        o.tag = reps.index(o)
+    g.run(6, 2)
+    for rnd in range(6):
+        for o in reps:
+            o.sweep(2)
+        oracle.replica_exchange(reps, kTs, tables, rnd & 1, 77, rnd)
+    st = _assert_slots_equal(g, reps, [o.tag for o in reps])
+    assert int(st["attempted"].sum()) > 0
+    g.close()
+
+
 def test_two_replicas_parity_one_is_a_no_op():
     cfg = scaled_config(1, (16, 16, 16))
     kTs = [600, 640]
