@@ -220,17 +220,17 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
               }
             }
             // i and j themselves change species (and see each other in shell 0, where j is a nearest neighbour of i):
-            // both evaluations of every shell term, one (site, shell) per lane
-            if (lane < 2 * n_shells) {
-              const int s = lane >> 1, who = lane & 1;
+            // the shell terms before and after, one (site, shell, before / after) per lane
+            if (lane < 4 * n_shells) {
+              const int s = lane >> 2, who = (lane >> 1) & 1, after = lane & 1;
               const int su = who ? sj : si;
               const short* dl = s_delta + (su & (B - 1)) * ZT;           // tile index = cell * B + basis
               unsigned long long cnt = 0ull;
 #pragma unroll 6
               for (int mm = s_start[s]; mm < s_start[s + 1]; ++mm) cnt += 1ull << (8 * (int)tile[su + dl[mm]]);
-              const int before = local_eps_shell(s_w1, s_w2, n, s, who ? sb : sa, cnt);
-              if (s == 0) cnt += who ? db - da : da - db;                // j sees i turn from a into b; i sees j turn from b into a
-              part += local_eps_shell(s_w1, s_w2, n, s, who ? sa : sb, cnt) - before;
+              if (after && s == 0) cnt += who ? db - da : da - db;       // j sees i turn from a into b; i sees j turn from b into a
+              const int v = local_eps_shell(s_w1, s_w2, n, s, (who != 0) == (after != 0) ? sa : sb, cnt);
+              part += after ? v : -v;
             }
             const int dE = __reduce_add_sync(0xffffffffu, part);
             // a6: Eq. 3 in integer form
