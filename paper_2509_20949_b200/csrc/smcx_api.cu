@@ -379,11 +379,20 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   {   // SMCX_MODEL_LOCAL: affected (site, shell) pairs per (basis, direction, shell), at most: i, j and 2 Z_s neighbours
     int zmax = 0;
     for (int s2 = 0; s2 < p->n_shells; ++s2) zmax = std::max(zmax, (int)shells[s2].size());
-    plan->local_umax = local ? 2 + 2 * zmax : 0;
+    // units of the flat list (build_local_utable): per shell at most 2 Z_s sites, each in ceil(Z_s / 12) chunks
+    int units = 0;
+    for (int s2 = 0; s2 < p->n_shells; ++s2) {
+      const int z = (int)shells[s2].size();
+      units += 2 * z * ((z + kLocalChunk - 1) / kLocalChunk);
+      const int last = z % kLocalChunk == 0 ? kLocalChunk : z % kLocalChunk;     // length of the last (or only) chunk
+      if (local && local_chunk_code(last) < 0) return SMCX_E_UNSUPPORTED;
+    }
+    (void)zmax;
+    plan->local_umax = local ? units : 0;
   }
   L.quad = off;    off += align_up(local ? (size_t)p->n_shells * n * n * n * sizeof(int32_t) : 0, 256);
-  L.utab = off;    off += align_up((size_t)G.B * G.Z0 * G.n_shells * plan->local_umax * sizeof(LocalUEntry), 256);
-  L.ucount = off;  off += align_up(local ? (size_t)G.B * G.Z0 * G.n_shells * sizeof(int) : 0, 256);
+  L.utab = off;    off += align_up((size_t)G.B * G.Z0 * plan->local_umax * sizeof(LocalUEntry), 256);
+  L.ucount = off;  off += align_up(local ? (size_t)G.B * G.Z0 * sizeof(int) : 0, 256);
   if (local && local_smem_bytes(G, plan->local_umax) > 227 * 1024) return SMCX_E_LINK_CELL_TOO_SMALL;
   L.accept = off;  off += align_up(((size_t)kAcceptCapacity + 1) * sizeof(uint32_t), 256);   // T and the zero entry behind it
   L.filter = off;  off += align_up((size_t)kFilterWords * sizeof(uint32_t), 256);
@@ -399,13 +408,15 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
 void build_local_utable(const Plan& P, int lattice, std::vector<LocalUEntry>& tab, std::vector<int>& count) {
   const Geom& G = P.G;
   const int umax = P.local_umax;
-  tab.assign((size_t)G.B * G.Z0 * G.n_shells * umax, LocalUEntry{0, 0});
-  count.assign((size_t)G.B * G.Z0 * G.n_shells, 0);
+  tab.assign((size_t)G.B * G.Z0 * umax, LocalUEntry{0, 0});
+  count.assign((size_t)G.B * G.Z0, 0);
   auto shell_of_vec = [&](int x, int y, int z) {
     for (int m = 0; m < G.ZT; ++m)
       if (G.off[m][0] == x && G.off[m][1] == y && G.off[m][2] == z) return (int)G.shell_of[m];
     return -1;
   };
+  std::vector<int> start(G.n_shells + 1, G.ZT);
+  for (int m = G.ZT - 1; m >= 0; --m) start[G.shell_of[m]] = m;
   for (int b = 0; b < G.B; ++b) {
     int bp[3];
     basis_pos(lattice, b, bp);
@@ -417,30 +428,38 @@ void build_local_utable(const Plan& P, int lattice, std::vector<LocalUEntry>& ta
           if (v[0] == x && v[1] == y && v[2] == z) return;
         U.push_back({x, y, z});
       };
-      add(0, 0, 0);
-      add(jx, jy, jz);
       for (int m = 0; m < G.ZT; ++m) {
         add(G.off[m][0], G.off[m][1], G.off[m][2]);
         add(jx + G.off[m][0], jy + G.off[m][1], jz + G.off[m][2]);
       }
+      // units, longest chunks first so that the lanes of a round count about equally many neighbours
+      std::vector<LocalUEntry> units[kLocalChunk + 1];
       for (int s = 0; s < G.n_shells; ++s) {
-        LocalUEntry* out = tab.data() + (size_t)((b * G.Z0 + dir) * G.n_shells + s) * umax;
-        int k = 0;
+        const int zs = start[s + 1] - start[s];
         for (const auto& v : U) {
           const int vx = v[0], vy = v[1], vz = v[2];
-          const unsigned kind = (vx == 0 && vy == 0 && vz == 0) ? 1u : ((vx == jx && vy == jy && vz == jz) ? 2u : 0u);
+          if ((vx == 0 && vy == 0 && vz == 0) || (vx == jx && vy == jy && vz == jz)) continue;   // i, j: the kernel's own round
           const bool sees_i = shell_of_vec(-vx, -vy, -vz) == s;              // i - u in shell s
           const bool sees_j = shell_of_vec(jx - vx, jy - vy, jz - vz) == s;  // j - u in shell s
-          if (!kind && !sees_i && !sees_j) continue;                          // this term does not change
+          if (sees_i == sees_j) continue;                                     // sees neither, or both: its counts stay
           const int qx = bp[0] + vx, qy = bp[1] + vy, qz = bp[2] + vz;
           const int nb = basis_from_parity(lattice, qx, qy, qz);
           const int d = ((floor_div2(qz) * G.TW + floor_div2(qy)) * G.TW + floor_div2(qx)) * G.B + (nb - b);
-          out[k].delta = (short)d;
-          out[k].bits = (unsigned short)((sees_i ? 1u : 0u) | (sees_j ? 2u : 0u) | (kind << 2) | ((unsigned)nb << 4));
-          ++k;
+          for (int c0 = 0; c0 < zs; c0 += kLocalChunk) {
+            const int len = std::min(kLocalChunk, zs - c0);
+            LocalUEntry e;
+            e.delta = (short)d;
+            e.bits = (unsigned short)((sees_j ? 1u : 0u) | (c0 == 0 ? 2u : 0u) | ((unsigned)nb << 2) | ((unsigned)s << 4) |
+                                      ((unsigned)(start[s] + c0) << 7) | ((unsigned)local_chunk_code(len) << 14));
+            units[len].push_back(e);
+          }
         }
-        count[(size_t)(b * G.Z0 + dir) * G.n_shells + s] = k;
       }
+      LocalUEntry* out = tab.data() + (size_t)(b * G.Z0 + dir) * umax;
+      int k = 0;
+      for (int len = kLocalChunk; len >= 1; --len)
+        for (const LocalUEntry& e : units[len]) out[k++] = e;
+      count[(size_t)b * G.Z0 + dir] = k;
     }
   }
 }

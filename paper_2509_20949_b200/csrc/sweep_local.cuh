@@ -27,8 +27,13 @@ constexpr int kLocalWarps = 8;
 constexpr int kLocalMaxSpecies = 8;      // eight 8-bit counters per shell word
 constexpr int kLocalMaxU = 2 + 2 * kMaxNeighbours;
 
-// One affected (site, shell) pair of a trial (b, dir): tile-linear step from i; bits: 0 = the site sees i in this shell,
-// 1 = it sees j in this shell, 2-3 = kind (1 = the site is i, 2 = it is j), 4-5 = its basis index.
+// One unit of work of a trial (b, dir): a site u other than i and j that sees exactly one of them in shell s, and a chunk
+// of at most kLocalChunk of u's shell-s neighbours to count (the change of u's shell term is linear in its counts, see
+// local_delta_shell, so the chunks of a site simply add up; the first chunk adds the constant).  delta: tile-linear step
+// from i to u; bits: 0 = u sees j (else i), 1 = first chunk of the site, 2-3 = basis index of u, 4-6 = shell,
+// 7-13 = first neighbour (index into the shell list) of the chunk, 14-15 = chunk length code.
+constexpr int kLocalChunk = 12;
+__host__ __device__ inline int local_chunk_code(int len) { return len == 12 ? 3 : len == 8 ? 2 : len == 6 ? 1 : len == 4 ? 0 : -1; }
 struct LocalUEntry {
   short delta;
   unsigned short bits;
@@ -38,8 +43,8 @@ static_assert(sizeof(LocalUEntry) == 4, "LocalUEntry is loaded as one word");
 struct LocalTables {
   const int32_t* w1;          // [n_shells][n][n]
   const int32_t* w2;          // [n_shells][n][n][n], x <= y used
-  const LocalUEntry* utab;    // [B][Z0][n_shells][umax]
-  const int* ucount;          // [B][Z0][n_shells]
+  const LocalUEntry* utab;    // [B][Z0][umax]: the units of (basis of i, direction), longest chunks first
+  const int* ucount;          // [B][Z0]
   int umax;
 };
 
@@ -78,11 +83,11 @@ __device__ __noinline__ int local_eps_shell(const int32_t* __restrict__ s_w1, co
 // as the difference of the two evaluations.
 template <class CountWord, int FIELD>
 __device__ __forceinline__ int local_delta_shell(const int32_t* __restrict__ s_w1, const int32_t* __restrict__ s_g, int n, int s,
-                                                 int c, int from, int to, CountWord v) {
+                                                 int c, int from, int to, bool with_const, CountWord v) {
   const int32_t* l = s_w1 + (s * n + c) * n;
   const int32_t* gt = s_g + ((s * n + c) * n + to) * n;
   const int32_t* gf = s_g + ((s * n + c) * n + from) * n;
-  int e = l[to] - l[from] + ((gt[to] + gf[from]) >> 1) - gf[to];
+  int e = with_const ? l[to] - l[from] + ((gt[to] + gf[from]) >> 1) - gf[to] : 0;
   constexpr int kFields = (int)(8 * sizeof(CountWord)) / FIELD;
 #pragma unroll
   for (int y = 0; y < kFields; ++y)
@@ -97,7 +102,7 @@ constexpr int kLocalNarrowMaxZ = 31;
 inline size_t local_smem_bytes(const Geom& G, int umax) {
   const int n = G.n_species;
   size_t b = (size_t)G.n_shells * n * n * 4 + 2 * (size_t)G.n_shells * n * n * n * 4;     // W1, W2, g
-  b += (size_t)G.B * G.Z0 * G.n_shells * umax * sizeof(LocalUEntry) + (size_t)G.B * G.Z0 * G.n_shells * 4;
+  b += (size_t)G.B * G.Z0 * umax * sizeof(LocalUEntry) + (size_t)G.B * G.Z0 * 4;
   b += (size_t)G.B * G.ZT * 2 + 16;
   b = (b + 15) & ~(size_t)15;
   return b + (size_t)kLocalWarps * (((size_t)G.TW * G.TW * G.TW * G.B + 15) & ~(size_t)15);
@@ -113,8 +118,8 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
   int32_t* s_w2 = s_w1 + n_shells * n * n;
   int32_t* s_g = s_w2 + n_shells * n * n * n;
   LocalUEntry* s_u = reinterpret_cast<LocalUEntry*>(s_g + n_shells * n * n * n);
-  int* s_ucount = reinterpret_cast<int*>(s_u + B * Z0 * n_shells * T.umax);
-  short* s_delta = reinterpret_cast<short*>(s_ucount + B * Z0 * n_shells);
+  int* s_ucount = reinterpret_cast<int*>(s_u + B * Z0 * T.umax);
+  short* s_delta = reinterpret_cast<short*>(s_ucount + B * Z0);
   const int tile_sites = G.TW * G.TW * G.TW * B;
   size_t tables = (size_t)(reinterpret_cast<unsigned char*>(s_delta + B * ZT) - smem) + 16;
   tables = (tables + 15) & ~(size_t)15;
@@ -130,8 +135,8 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
     const int y = k % n, tt = (k / n) % n, sc = k / (n * n);          // g_t(y) of (shell, centre) sc
     s_g[k] = y == tt ? 2 * T.w2[(sc * n + tt) * n + tt] : T.w2[(sc * n + min(tt, y)) * n + max(tt, y)];
   }
-  for (int k = threadIdx.x; k < B * Z0 * n_shells * T.umax; k += blockDim.x) s_u[k] = T.utab[k];
-  for (int k = threadIdx.x; k < B * Z0 * n_shells; k += blockDim.x) s_ucount[k] = T.ucount[k];
+  for (int k = threadIdx.x; k < B * Z0 * T.umax; k += blockDim.x) s_u[k] = T.utab[k];
+  for (int k = threadIdx.x; k < B * Z0; k += blockDim.x) s_ucount[k] = T.ucount[k];
   for (int k = threadIdx.x; k < B * ZT; k += blockDim.x) s_delta[k] = G.delta[k / ZT][k % ZT];
   if (threadIdx.x <= kMaxShells) {      // shells are listed one after the other: first neighbour of every shell
     int first = ZT;
@@ -192,30 +197,44 @@ sweep_local_warp(const Geom G, uint8_t* __restrict__ species, const LocalTables 
             // a5: the changed terms of the local energies, before and after, shell by shell
             const unsigned long long da = 1ull << (8 * sa), db = 1ull << (8 * sb);
             int part = 0;
-            // sites other than i and j: they keep their species, and the shell-s term of such a site changes only if
-            // it sees exactly one of i, j in shell s (one neighbour changes species; seeing both, its counts stay)
-            for (int s = 0; s < n_shells; ++s) {
-              const LocalUEntry* ue = s_u + ((b * Z0 + dir) * n_shells + s) * T.umax;
-              const int nu = s_ucount[(b * Z0 + dir) * n_shells + s];
-              const int m0 = s_start[s], m1 = s_start[s + 1];
+            // sites other than i and j keep their species, and the shell-s term of such a site changes only if it sees
+            // exactly one of i, j in shell s (one neighbour changes species; seeing both, its counts stay): the host lists
+            // those sites, their neighbours cut into chunks of at most kLocalChunk (LocalUEntry), one unit per lane
+            {
+              const LocalUEntry* ue = s_u + (b * Z0 + dir) * T.umax;
+              const int nu = s_ucount[b * Z0 + dir];
               for (int q = lane; q < nu; q += 32) {
                 const LocalUEntry e = ue[q];
-                const unsigned bits = e.bits, see = bits & 3u;
-                if ((bits & 12u) != 0u || see == 0u || see == 3u) continue;
+                const unsigned bits = e.bits;
                 const int su = si + e.delta;
-                const short* dl = s_delta + (int)((bits >> 4) & 3u) * ZT;
+                const short* dl = s_delta + (int)((bits >> 2) & 3u) * ZT + (int)((bits >> 7) & 127u);
+                const unsigned code = bits >> 14;                        // chunk length 4, 6, 8, 12
+                const int s = (int)((bits >> 4) & 7u);
                 // sees i: that neighbour turns from a into b; sees j: from b into a
-                const int from = see == 1u ? sa : sb, to = see == 1u ? sb : sa;
+                const int from = (bits & 1u) ? sb : sa, to = (bits & 1u) ? sa : sb;
                 if (NARROW) {
                   uint32_t cnt = 0u;
-#pragma unroll 6
-                  for (int mm = m0; mm < m1; ++mm) cnt += 1u << (5 * (int)tile[su + dl[mm]]);    // six loads in flight
-                  part += local_delta_shell<uint32_t, 5>(s_w1, s_g, n, s, tile[su], from, to, cnt);
+#pragma unroll
+                  for (int mm = 0; mm < 4; ++mm) cnt += 1u << (5 * (int)tile[su + dl[mm]]);
+                  if (code >= 1u) {
+#pragma unroll
+                    for (int mm = 4; mm < 6; ++mm) cnt += 1u << (5 * (int)tile[su + dl[mm]]);
+                  }
+                  if (code >= 2u) {
+#pragma unroll
+                    for (int mm = 6; mm < 8; ++mm) cnt += 1u << (5 * (int)tile[su + dl[mm]]);
+                  }
+                  if (code >= 3u) {
+#pragma unroll
+                    for (int mm = 8; mm < 12; ++mm) cnt += 1u << (5 * (int)tile[su + dl[mm]]);
+                  }
+                  part += local_delta_shell<uint32_t, 5>(s_w1, s_g, n, s, tile[su], from, to, (bits & 2u) != 0u, cnt);
                 } else {
                   unsigned long long cnt = 0ull;
+                  const int len = code == 3u ? 12 : 4 + 2 * (int)code;
 #pragma unroll 6
-                  for (int mm = m0; mm < m1; ++mm) cnt += 1ull << (8 * (int)tile[su + dl[mm]]);
-                  part += local_delta_shell<unsigned long long, 8>(s_w1, s_g, n, s, tile[su], from, to, cnt);
+                  for (int mm = 0; mm < len; ++mm) cnt += 1ull << (8 * (int)tile[su + dl[mm]]);
+                  part += local_delta_shell<unsigned long long, 8>(s_w1, s_g, n, s, tile[su], from, to, (bits & 2u) != 0u, cnt);
                 }
               }
             }
