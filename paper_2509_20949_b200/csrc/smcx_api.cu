@@ -126,6 +126,8 @@ size_t storage_bytes(int storage, long long n_sites) {
 }
 
 
+void build_local_utable(const Plan& P, int lattice, std::vector<LocalUEntry>& tab, std::vector<int>& count);
+
 int make_plan(const smcx_params_t* p, Plan* plan) {
   if (!p || !plan) return SMCX_E_NULL_ARG;
   if (p->lattice != SMCX_BCC && p->lattice != SMCX_FCC) return SMCX_E_BAD_LATTICE;
@@ -389,6 +391,15 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
     }
     (void)zmax;
     plan->local_umax = local ? units : 0;
+    if (local) {
+      // the exact length of the longest list (sites that see both i and j drop out): shared memory per block
+      std::vector<LocalUEntry> tab;
+      std::vector<int> count;
+      build_local_utable(*plan, p->lattice, tab, count);
+      int longest = 1;
+      for (int c : count) longest = std::max(longest, c);
+      plan->local_umax = longest;
+    }
   }
   L.quad = off;    off += align_up(local ? (size_t)p->n_shells * n * n * n * sizeof(int32_t) : 0, 256);
   L.utab = off;    off += align_up((size_t)G.B * G.Z0 * plan->local_umax * sizeof(LocalUEntry), 256);
