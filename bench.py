@@ -346,7 +346,12 @@ def run_paper_shaped_fcc(edge: int = PAPER_FCC_EDGE, sweeps: int = 10):
             "paper_h800_per_gpu": 3.5e9, "paper_note": "PAPER.md:130, EPI model on H800; other hardware and interactions: context"}
 
 
-def run_local_model(edge: int = 128, sweeps: int = 5):
+# Edge of the `local_energy_model` leg: FCC 256^3 = 6.7e7 sites, 32,768 link cells (warps) per colour pass, i.e. many waves
+# of the 24 warps an SM holds; at 128^3 a pass is 1.15 waves (5.8-7.2e8 trials/s against 9.9e8).
+LOCAL_EDGE = 256
+
+
+def run_local_model(edge: int = LOCAL_EDGE, sweeps: int = 10):
     """The nonlinear local-energy model (reading S12; the role of the paper's qSRO model):
     FCC, five species 29/29/28/7/7, three shells, synthetic integer weights; every trial recomputes the local energies of
     the 86 sites its swap affects.  Device-timed."""
@@ -357,7 +362,7 @@ def run_local_model(edge: int = 128, sweeps: int = 5):
     w1, w2 = make_local_weights(3, 5, 200, 25, 1007)
     lat = smcx.Lattice(smcx.FCC, dims, 5, 3, w1, make_accept_table(2500), 1007, link_cell=4, kT_units=2500, local_quad=w2)
     lat.init_composition(composition_counts(lat.n_sites, (29, 29, 28, 7, 7)))
-    ms = _time_sweeps(lat, 2, sweeps)
+    ms = _time_sweeps(lat, 3, sweeps)
     acc = lat.stats()
     out = {"workload": f"FCC {edge}^3 conventional cells ({lat.n_sites} sites), 5 species 29/29/28/7/7, 3 shells, local-energy model "
                        f"eps = W1.n + n.W2.n with synthetic int32 weights, kT=250 meV, link cell 4, seed 1007",
@@ -771,7 +776,7 @@ def main():
                          "conventional cells per edge (0: skip)")
     ap.add_argument("--no-largest", dest="largest", action="store_false",
                     help="skip the BCC 2000^3 (1.6e10 sites) leg that the default run adds as `largest_single_gpu`")
-    ap.add_argument("--local-edge", type=int, default=128,
+    ap.add_argument("--local-edge", type=int, default=LOCAL_EDGE,
                     help="with --ensemble: also time the nonlinear local-energy model on an FCC lattice of this edge (0: skip)")
     ap.add_argument("--no-slabs-leg", dest="slabs_leg", action="store_false",
                     help="skip the `lattice_parallel_one_gpu` leg (the workload cut into 2 / 4 slabs on this one GPU)")
