@@ -101,6 +101,7 @@ struct Plan {
   bool coef_packed; // pack_thread_coefficients: the 16-bit coefficient rows are exact
   int fcc_rep;      // sweep_fcc_thread: replicas of the look-up rows in shared memory
   int accept_tail_from = 0;   // T[k] >= T[d] for every d > k holds for all k >= this (0 for a table that never increases)
+  int accept_tail_floor = 0;  // replica of an ensemble: the same for the weakest of the ensemble's tables (they move on the device)
   FccTables fcc_tables;
   Bcc4Tables bcc4_tables;
   Layout lay;
@@ -680,7 +681,7 @@ int upload_table(smcx* h, const uint32_t* accept, int len) {
     int m = len;
     uint32_t run_max = 0u;
     while (m > 0 && accept[m - 1] >= run_max) { run_max = accept[m - 1]; --m; }
-    h->plan.accept_tail_from = m;
+    h->plan.accept_tail_from = std::max(m, h->plan.accept_tail_floor);
   }
   SMCX_CUDA(h, cudaMemcpyAsync(h->d_accept(), h->staging[slot], ((size_t)len + 1) * sizeof(uint32_t),
                                cudaMemcpyHostToDevice, h->stream));
