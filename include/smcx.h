@@ -75,6 +75,10 @@ enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_4BIT = 4, SMCX
  * the BCC counterpart of FCC_THREAD (one thread per link cell on a 512-byte packed tile, nine row loads per site, the same
  * PRMT look-ups; sweep_bcc4.cuh).  What AUTO picks for BCC lattices with 5..8 species when a colour has at least
  * 12,000 link cells.
+ * smcx_sweep runs the eight colour passes of THREAD_PERSISTENT as ONE launch, the passes pipelined through completion
+ * counters in device memory (sweep_thread_sweep.cuh), for an undivided lattice of up to 2.4e6 link cells per colour --
+ * for one handle per process at a time (the first such handle alive; the others launch per colour): two of these launches
+ * at once could starve each other of SMs.  Same results either way.
  * AUTO picks, when the parameters allow a thread kernel, THREAD_PERSISTENT for lattices that give every
  * warp of every SM a batch of cells (>= 148*20*32 link cells per colour) and THREAD_PER_CELL below that
  * (same speed there, and concurrent lattices of a replica ensemble overlap freely).  Results never

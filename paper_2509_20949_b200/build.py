@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libsmcx.so")
 SOURCES = ["smcx_api.cu"]
-HEADERS = ["smcx_common.cuh", "sweep_warp.cuh", "sweep_thread.cuh", "sweep_group.cuh", "sweep_fcc.cuh", "sweep_bcc4.cuh", "sweep_local.cuh", "domain_api.inc", "static_scratch_api.inc", "lattice_kernels.cuh", "ensemble_kernels.cuh", "ensemble_api.inc",
+HEADERS = ["smcx_common.cuh", "sweep_warp.cuh", "sweep_thread.cuh", "sweep_thread_sweep.cuh", "sweep_group.cuh", "sweep_fcc.cuh", "sweep_bcc4.cuh", "sweep_local.cuh", "domain_api.inc", "static_scratch_api.inc", "lattice_kernels.cuh", "ensemble_kernels.cuh", "ensemble_api.inc",
            os.path.join("..", "..", "include", "smcx.h")]
 
 NVCC_FLAGS = [

@@ -4,6 +4,7 @@
 #include "../../include/smcx.h"
 
 #include <algorithm>
+#include <atomic>
 #include <array>
 #include <cmath>
 #include <cstdio>
@@ -25,9 +26,14 @@
 #include "sweep_group.cuh"
 #include "sweep_local.cuh"
 #include "sweep_thread.cuh"
+#include "sweep_thread_sweep.cuh"
 #include "sweep_warp.cuh"
 
 using namespace smcxk;
+
+struct smcx;
+static std::atomic<smcx*> g_whole_sweep_owner{nullptr};   // see smcx_create
+constexpr long long kWholeSweepMaxCells = 2400000;         // link cells per colour: about 25 rounds of batches
 
 namespace {
 
@@ -86,7 +92,7 @@ inline bool is_thread_kernel(int k) { return k == SMCX_KERNEL_THREAD_PER_CELL ||
 inline bool has_fused_writeback(int k) { return is_thread_kernel(k) || k == SMCX_KERNEL_FCC_THREAD || k == SMCX_KERNEL_BCC4_THREAD; }
 
 struct Layout {
-  size_t species, epi, coef, gtable, fcc_lut, fcc_corr, quad, utab, ucount, accept, filter, trace, state, counts, total;
+  size_t species, epi, coef, gtable, fcc_lut, fcc_corr, quad, utab, ucount, accept, filter, trace, state, counts, progress, total;
 };
 
 struct Plan {
@@ -411,6 +417,7 @@ int make_plan(const smcx_params_t* p, Plan* plan) {
   L.trace = off;   off += align_up((size_t)G.trace_capacity * sizeof(long long), 256);
   L.state = off;   off += align_up(sizeof(DevState), 256);
   L.counts = off;  off += align_up((size_t)kMaxShells * kMaxSpecies * kMaxSpecies * sizeof(unsigned long long), 256);
+  L.progress = off; off += align_up(whole_sweep_progress_words(G) * sizeof(unsigned), 256);   // sweep_thread_whole_sweep
   L.total = off;
   return SMCX_OK;
 }
@@ -490,6 +497,8 @@ struct smcx {
   cudaStream_t stream = nullptr;
   char* ws = nullptr;
   bool owns_ws = false;
+  long long graph_launches = 9;   // kernels per replay of sweep_graph
+  bool whole_sweep = false;   // smcx_sweep runs the eight colour passes as one launch (sweep_thread_sweep.cuh)
   std::vector<int32_t> epi;
   int kT_units = 0;
   uint32_t* staging[kStagingSlots] = {nullptr, nullptr, nullptr, nullptr};
@@ -531,6 +540,7 @@ struct smcx {
   long long* d_trace() const { return reinterpret_cast<long long*>(ws + plan.lay.trace); }
   DevState* d_state() const { return reinterpret_cast<DevState*>(ws + plan.lay.state); }
   unsigned long long* d_counts() const { return reinterpret_cast<unsigned long long*>(ws + plan.lay.counts); }
+  unsigned* d_progress() const { return reinterpret_cast<unsigned*>(ws + plan.lay.progress); }
 };
 
 namespace {
@@ -793,6 +803,18 @@ int enqueue_sweep(smcx* h) {
   static const char* const kPassName[8] = {"smcx colour 0", "smcx colour 1", "smcx colour 2", "smcx colour 3",
                                            "smcx colour 4", "smcx colour 5", "smcx colour 6", "smcx colour 7"};
   nvtxRangePushA("smcx sweep");
+  if (h->whole_sweep && persist_warps_for(h->plan.G.accept_len) > 0) {
+    // the eight passes pipelined in one launch (+ the launch that advances its sweep count)
+    const Plan& P = h->plan;
+    const int rc = launch_whole_sweep(P.G, reinterpret_cast<uint32_t*>(h->d_species()), h->d_coef(), P.coef_packed, h->d_accept(),
+                                      h->d_state(), h->d_progress(), persist_warps_for(P.G.accept_len), h->sm_count, h->stream);
+    h->launches += 2;
+    if (rc != 0) { h->err = "whole-sweep launch failed"; nvtxRangePop(); return SMCX_E_CUDA; }
+    sweep_epilogue<<<1, 1, 0, h->stream>>>(h->d_state(), h->d_trace(), h->plan.G.trace_capacity);
+    h->launches++;
+    nvtxRangePop();
+    return SMCX_OK;
+  }
   for (int colour = 0; colour < 8; ++colour) {
     nvtxRangePushA(kPassName[colour]);
     const int rc = launch_colour_pass(h, h->plan.G, colour);
@@ -884,6 +906,8 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     if (cudaEventCreateWithFlags(&h->staging_ev[s], cudaEventDisableTiming) != cudaSuccess) return fail(SMCX_E_CUDA);
   }
   if (configure_thread_per_cell() != 0) return fail(SMCX_E_CUDA);
+  if (h->plan.kernel == SMCX_KERNEL_THREAD_PERSISTENT && configure_whole_sweep() != 0) return fail(SMCX_E_CUDA);
+  cudaFuncSetAttribute(whole_sweep_epoch, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
   if (h->plan.kernel == SMCX_KERNEL_FCC_THREAD && configure_fcc_thread(h->plan.fcc_rep) != 0) return fail(SMCX_E_CUDA);
   if (h->plan.kernel == SMCX_KERNEL_BCC4_THREAD && configure_bcc4_thread(h->plan.fcc_rep) != 0) return fail(SMCX_E_CUDA);
   // every kernel of a sweep prefers the largest shared-memory carve-out: an SM whose carve-out must
@@ -955,6 +979,7 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
       SMCX_CUDA(h, cudaMemcpyAsync(h->d_fcc_corr(), fcorr.data(), fcorr.size() * sizeof(int32_t), cudaMemcpyHostToDevice, h->stream));
     }
     SMCX_CUDA(h, cudaMemsetAsync(h->d_trace(), 0, (size_t)h->plan.G.trace_capacity * sizeof(long long), h->stream));
+    SMCX_CUDA(h, cudaMemsetAsync(h->d_progress(), 0, whole_sweep_progress_words(h->plan.G) * sizeof(unsigned), h->stream));
     SMCX_CUDA(h, cudaStreamSynchronize(h->stream));  // &zero and epi must stay valid until copied
     int r = upload_table(h, p->accept, p->accept_len);
     if (r != SMCX_OK) return r;
@@ -963,12 +988,25 @@ int smcx_create(smcx_t** out, const smcx_params_t* p) {
     return reset_running_energy(h);
   }();
   if (rc != SMCX_OK) return fail(rc);
+  // The whole-sweep launch (its warps wait for other blocks of the same launch) goes to one handle per process at a
+  // time: an undivided lattice on the persistent kernel with at most kWholeSweepMaxCells link cells per colour (beyond
+  // that a pass is many rounds of batches, the colour boundaries cost little and the bookkeeping more: measured).  Two
+  // such launches at once could each hold SMs while waiting for blocks of their own that find none free.
+  if (h->plan.kernel == SMCX_KERNEL_THREAD_PERSISTENT && !h->plan.window && h->plan.G.iz_first == 0 &&
+      h->plan.n_cells / 8 <= kWholeSweepMaxCells) {
+    smcx* none = nullptr;
+    h->whole_sweep = g_whole_sweep_owner.compare_exchange_strong(none, h);
+  }
   *out = h;
   return SMCX_OK;
 }
 
 void smcx_destroy(smcx_t* h) {
   if (!h) return;
+  {
+    smcx* me = h;
+    g_whole_sweep_owner.compare_exchange_strong(me, nullptr);
+  }
   DeviceGuard on_device(h->device);
   if (h->stream || h->ws) cudaStreamSynchronize(h->stream);
   for (int s = 0; s < kStagingSlots; ++s) {
@@ -1177,6 +1215,7 @@ int smcx_sweep(smcx_t* h, int64_t n) {
         h->stream = h->capture_stream;
         ok = enqueue_sweep(h) == SMCX_OK;
         h->stream = user;
+        h->graph_launches = h->launches - launches_before;     // kernels one replay of the graph launches
         h->launches = launches_before;
         ok = (cudaStreamEndCapture(h->capture_stream, &graph) == cudaSuccess) && ok && graph;
       }
@@ -1188,7 +1227,7 @@ int smcx_sweep(smcx_t* h, int64_t n) {
     if (h->sweep_graph) {
       for (int64_t s = 0; s < n; ++s) {
         SMCX_CUDA(h, cudaGraphLaunch(h->sweep_graph, h->stream));
-        h->launches += 9;
+        h->launches += h->graph_launches;
         h->sweeps_enqueued++;
       }
       return SMCX_OK;
