@@ -78,7 +78,10 @@ enum { SMCX_STORAGE_AUTO = 0, SMCX_STORAGE_2BIT = 2, SMCX_STORAGE_4BIT = 4, SMCX
  * smcx_sweep runs the eight colour passes of THREAD_PERSISTENT as ONE launch, the passes pipelined through completion
  * counters in device memory (sweep_thread_sweep.cuh), for an undivided lattice of up to 2.4e6 link cells per colour --
  * for one handle per process at a time (the first such handle alive; the others launch per colour): two of these launches
- * at once could starve each other of SMs.  Same results either way.
+ * at once could starve each other of SMs.  Same results either way.  The launch has one block per SM and its warps
+ * wait for one another's results, so every block must become resident: run it on a whole GPU (not inside an MPS
+ * partition that exposes fewer SMs than the device reports); other kernels that merely occupy SMs for a while only
+ * delay it.
  * AUTO picks, when the parameters allow a thread kernel, THREAD_PERSISTENT for lattices that give every
  * warp of every SM a batch of cells (>= 148*20*32 link cells per colour) and THREAD_PER_CELL below that
  * (same speed there, and concurrent lattices of a replica ensemble overlap freely).  Results never
